@@ -1,0 +1,188 @@
+/*
+ * wilson_cg.h — C ABI of the B200-native Wilson-Dirac / CG library (libwilson_cg.so).
+ *
+ * The library is the hot path of arXiv:2111.14958 ("Implementation of the conjugate gradient
+ * algorithm for heterogeneous systems"): the 4D Wilson-Dirac operator D / D-dagger as a
+ * matrix-free stencil and the paper's conjugate gradient on D D-dagger, all of it hand-written
+ * CUDA for sm_100a.  Citations are lines of the paper text and, where the paper is
+ * silent, the readings listed in DESIGN.md ("Readings", G1..G18, C-1, C-2).
+ *
+ * Conventions common to every call
+ * --------------------------------
+ *  * Return value: 0 = WD_OK; < 0 = error (see WD_ERR_*); cg_solve* may also return
+ *    +1 = WD_NOT_CONVERGED (max_iter reached; the current psi = D-dagger y has been written).
+ *    No C++ exception crosses this boundary.  wd_last_error(ctx) gives a ctx-owned,
+ *    NUL-terminated description of the last failure (valid until the next call on that ctx).
+ *  * A "device pointer" is a CUDA device address in the current device's primary context
+ *    (e.g. torch.Tensor.data_ptr()); a "host pointer" is ordinary host memory (pinned memory
+ *    makes the copies faster but is not required).  Every buffer passed in is owned by the
+ *    caller and is never freed, resized or (for inputs) written by the library.
+ *  * The ctx owns its CG workspace (r, p, q, y, device scalars, reduction partials, staging
+ *    buffers of the *_host calls), allocated lazily with cudaMalloc and freed by wd_destroy.
+ *  * All device work is enqueued on the ctx stream given to wd_create.  wd_pack_*, wd_unpack_*,
+ *    wd_apply are asynchronous on that stream; cg_solve, wd_norm2 and the *_host calls return
+ *    after their result is available on the host.
+ *  * A ctx is not thread-safe; use one ctx per host thread / stream.
+ *
+ * Canonical (caller-visible) layouts — x fastest, interleaved (re, im), element type float
+ * (precision 32) or double (precision 64):
+ *    site   s = x + Lx*(y + Ly*(z + Lz*t)),  dims = {Lx, Ly, Lz, Lt},  V = Lx*Ly*Lz*Lt
+ *    spinor psi[s][alpha 0..3][a 0..2][2]            24 reals per site   (Eq. 1, PAPER.md:27-32:
+ *                                                    alpha = spin index, a = colour index)
+ *    gauge  U[s][mu 0..3][a 0..2][b 0..2][2]         72 reals per site;  mu = 0:x 1:y 2:z 3:t;
+ *                                                    U_mu(x) sits on the link x -> x+mu, row a, col b.
+ *
+ * Native (internal, site-planar SoA) layouts — produced by wd_pack_*, consumed by wd_apply /
+ * cg_solve; opaque to the caller except for their size (wd_*_native_bytes):
+ *    precision 32: spinor = 6 planes of float4  (plane j holds complex components 2j, 2j+1 of
+ *                  the 12 = alpha*3+a), plane stride V;   gauge = 4*9 planes of float2
+ *                  (plane mu*9 + a*3+b), plane stride V.
+ *    precision 64: spinor = 12 planes of double2, gauge = 36 planes of double2.
+ *    Every per-thread access is one 128-bit (spinor) or 64/128-bit (gauge) load and a warp
+ *    reads consecutive sites of one plane: 512 contiguous bytes per spinor plane.
+ *
+ * The operator (reading C-1; the paper only cites Wilson, and states
+ * gamma5 D gamma5 = D-dagger):
+ *    (D psi)(x) = psi(x) - kappa sum_mu [ s+ (1 - gamma_mu) U_mu(x)          psi(x+mu)
+ *                                       + s- (1 + gamma_mu) U_mu(x-mu)^dagger psi(x-mu) ]
+ *    D-dagger: gamma_mu -> -gamma_mu.   x +- mu is taken modulo L_mu (periodic); in t the hop that
+ *    wraps the boundary carries the factor bc_t (-1 antiperiodic, +1 periodic), applied in-kernel.
+ *    gamma matrices: chiral basis of reading C-2 (gamma5 = diag(1,1,-1,-1)).
+ */
+#ifndef WILSON_CG_H
+#define WILSON_CG_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WD_OK 0
+#define WD_NOT_CONVERGED 1
+#define WD_ERR_ARG (-1)     /* NULL pointer, aliasing out == in, non-finite kappa, r_min <= 0, max_iter < 0 */
+#define WD_ERR_DIMS (-2)    /* an extent < 4 (forward and backward neighbours must be distinct sites) or volume too large */
+#define WD_ERR_CUDA (-3)    /* a CUDA runtime call or kernel launch failed; wd_last_error() has the CUDA string */
+#define WD_ERR_ALLOC (-4)   /* cudaMalloc / host allocation failed */
+#define WD_ERR_PRECISION (-5) /* precision not 32 or 64 */
+
+typedef struct wd_ctx wd_ctx; /* opaque */
+
+/* Result record of cg_solve / cg_solve_host (host memory, written before the call returns). */
+typedef struct wd_cg_info {
+    int iterations;        /* k = number of completed CG loop bodies */
+    int converged;         /* 1 iff sqrt(rr) < r_min*sqrt(<eta,eta>) at exit (reading G4) */
+    double rel_residual;   /* sqrt(rr/<eta,eta>), rr the recursed residual norm^2 */
+    double eta_norm2;      /* <eta,eta> */
+    double gpu_ms;         /* device time of init + loop + final D-dagger (CUDA events on the ctx stream) */
+    double total_ms;       /* *_host calls: device time including H2D copies, pack, solve, unpack, D2H; else = gpu_ms */
+    int kernel_launches;   /* number of this library's kernels launched by the call */
+    int reserved;
+} wd_cg_info;
+
+/*
+ * wd_create — make a context for one lattice geometry and precision.
+ *   out          receives the ctx (host pointer to a pointer).
+ *   dims         {Lx, Ly, Lz, Lt}, each >= 4 (any integer, e.g. 14); V*36 must fit in 31 bits.
+ *   precision    32 (float) or 64 (double): the arithmetic type of fields and stencil.  Dot products
+ *                are always accumulated, and alpha/beta formed, in fp64 (reading G17).
+ *   bc_t         -1 antiperiodic in t (all BASELINE configs), +1 periodic.  x, y, z are periodic.
+ *   cuda_stream  a cudaStream_t (as void*) owned by the caller, or NULL for the legacy default stream.
+ * Errors: WD_ERR_ARG, WD_ERR_DIMS, WD_ERR_PRECISION, WD_ERR_CUDA (no usable device), WD_ERR_ALLOC.
+ */
+int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_t, void *cuda_stream);
+
+/* wd_destroy — free the ctx and everything it owns (synchronises the ctx stream first). NULL is OK. */
+int wd_destroy(wd_ctx *ctx);
+
+/* Last error text of this ctx ("" if none).  ctx == NULL returns the text of the last failed wd_create. */
+const char *wd_last_error(wd_ctx *ctx);
+
+/* Sizes in bytes of the native buffers the caller must allocate (device memory). */
+size_t wd_gauge_native_bytes(wd_ctx *ctx);   /* 72 * V * sizeof(real) */
+size_t wd_spinor_native_bytes(wd_ctx *ctx);  /* 24 * V * sizeof(real) */
+
+/*
+ * wd_pack_gauge / wd_pack_spinor / wd_unpack_spinor — pure permutations between the canonical
+ * and the native layout.  Device pointers; in and out must not overlap.
+ * The antiperiodic sign is NOT folded into the links.  Asynchronous on the ctx stream.
+ */
+int wd_pack_gauge(wd_ctx *ctx, const void *U_canonical_dev, void *U_native_dev);
+int wd_pack_spinor(wd_ctx *ctx, const void *psi_canonical_dev, void *psi_native_dev);
+int wd_unpack_spinor(wd_ctx *ctx, const void *psi_native_dev, void *psi_canonical_dev);
+
+/*
+ * wd_apply — out = D psi (dagger = 0) or D-dagger psi (dagger != 0); the paper's "sparse-matrix
+ * vector multiplication" done matrix-free: for each of the 8 neighbours, spin
+ * projection to a half-spinor, one SU(3) (or SU(3)-dagger) multiply, boundary sign, reconstruction
+ * (reading C-1/C-2; row a7 of SURVEY.md 8(a)).
+ *   U_native, psi_native, out_native: device pointers, native layout; out must not alias psi.
+ *   kappa: hopping parameter (finite).  Asynchronous on the ctx stream.
+ */
+int wd_apply(wd_ctx *ctx, const void *U_native, const void *psi_native, void *out_native,
+             double kappa, int dagger);
+
+/*
+ * cg_solve — solve D psi = eta (Eq. 1) by the paper's CG on D D-dagger followed
+ * by one multiplication with D-dagger (readings G1-G5):
+ *     y <- 0; r <- eta; p <- r; rr <- <r,r>
+ *     while sqrt(rr) >= r_min*sqrt(<eta,eta>) and k < max_iter:
+ *         q <- D-dagger p ; alpha <- rr / <q,q>        (one kernel: stencil + fused |q|^2)
+ *         r <- r - alpha D q ; rr' <- <r,r>            (one kernel: stencil + fused update + |r|^2)
+ *         y <- y + alpha p ; beta <- rr'/rr ; p <- r + beta p ; rr <- rr' ; k <- k+1   (one kernel)
+ *     psi <- D-dagger y
+ * alpha, beta, rr, k and the loop condition live in device memory; the host only polls.
+ *   U_native, eta_native: device inputs (native layout); psi_native_out: device output, must not alias eta.
+ *   r_min: relative tolerance (> 0); max_iter >= 0.  eta == 0 gives psi = 0, 0 iterations, WD_OK.
+ *   info: host pointer, may be NULL.
+ * Returns WD_OK, WD_NOT_CONVERGED or an error.  Synchronous (returns after info is filled).
+ */
+int cg_solve(wd_ctx *ctx, const void *U_native, const void *eta_native, void *psi_native_out,
+             double kappa, double r_min, int max_iter, wd_cg_info *info);
+
+/*
+ * Host-buffer forms: the same operations with HOST pointers in the CANONICAL layout.  Each call
+ * copies its inputs to the device, packs, runs the device path above, unpacks and copies the result
+ * back, on the ctx stream, and returns when the host output is complete.  U_host may be NULL in
+ * cg_solve_host / wd_apply_host to reuse the gauge field of the previous *_host call on this ctx.
+ */
+int wd_apply_host(wd_ctx *ctx, const void *U_host, const void *psi_host, void *out_host,
+                  double kappa, int dagger);
+int cg_solve_host(wd_ctx *ctx, const void *U_host, const void *eta_host, void *psi_host_out,
+                  double kappa, double r_min, int max_iter, wd_cg_info *info);
+
+/*
+ * wd_cg_history — rr = <r,r> after 0, 1, ..., k iterations of the last cg_solve / cg_solve_host on this
+ * ctx (the device-side record of the recursed residual; used to compare convergence with the oracle).
+ *   out: host pointer to n doubles.  Returns the number of values written (<= k+1), or < 0 on error.
+ */
+int wd_cg_history(wd_ctx *ctx, double *out, int n);
+
+/*
+ * wd_norm2 — <a,a> = sum over all 12V complex components of |a|^2 (the paper's dot-product kernel,
+ * PAPER.md:60), fp64 accumulation, deterministic single-pass grid reduction.
+ *   a_native: device pointer; result: host pointer.  Synchronous.
+ */
+int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
+
+/*
+ * Tuning knobs (the paper's workgroup-size tuning):
+ *   wd_num_tiles()            number of compiled CTA tile shapes.
+ *   wd_tile_shape(i, shape)   writes {BX,BY,BZ,BT} of tile i (threads per CTA = product); returns 0 or WD_ERR_ARG.
+ *   wd_set_tile(ctx, i)       select tile i for the stencil kernels of this ctx; i = -1 restores the automatic choice.
+ *   wd_get_tile(ctx)          index in use.
+ *   wd_set_poll_interval(ctx, n)  CG iterations enqueued between two host polls of the device stop flag (n >= 1; 0 = automatic).
+ */
+int wd_num_tiles(void);
+int wd_tile_shape(int index, int shape[4]);
+int wd_set_tile(wd_ctx *ctx, int index);
+int wd_get_tile(wd_ctx *ctx);
+int wd_set_poll_interval(wd_ctx *ctx, int n);
+
+/* Library version string, e.g. "wilson_cg 0.1 sm_100a". */
+const char *wd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WILSON_CG_H */

@@ -1,0 +1,575 @@
+// wilson_cg.cu — the C ABI of include/wilson_cg.h: context, launch logic, the device-resident CG loop.
+// Every arithmetic step runs in the kernels of wilson_kernels.cuh; this file only sizes grids,
+// enqueues launches on the caller's stream and polls the device stop flag.
+#include "../../include/wilson_cg.h"
+#include "wilson_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+
+using namespace wd;
+
+// ---------------------------------------------------------------- tile table (the workgroup-size knob)
+// X(index, BX, BY, BZ, BT).  Tiles with more than 256 threads are compiled for fp32 only
+// (fp64 needs > 128 registers per thread).
+#define WD_TILES_SMALL(X) \
+    X(0, 8, 4, 4, 2)      \
+    X(1, 16, 4, 2, 2)     \
+    X(2, 32, 2, 2, 2)     \
+    X(3, 4, 4, 4, 4)      \
+    X(4, 16, 4, 4, 1)     \
+    X(5, 8, 4, 2, 2)      \
+    X(6, 16, 2, 2, 2)     \
+    X(7, 4, 4, 4, 2)
+#define WD_TILES_LARGE(X) \
+    X(8, 8, 4, 4, 4)      \
+    X(9, 16, 4, 4, 2)     \
+    X(10, 32, 4, 2, 2)    \
+    X(11, 16, 8, 2, 2)
+#define WD_NUM_TILES 12
+#define WD_NUM_TILES_SMALL 8
+
+static const int kTileShape[WD_NUM_TILES][4] = {
+#define X(i, a, b, c, d) {a, b, c, d},
+    WD_TILES_SMALL(X) WD_TILES_LARGE(X)
+#undef X
+};
+
+struct wd_ctx {
+    int dims[4];
+    int V;
+    int precision;
+    int bc_t;
+    cudaStream_t stream;
+    int tile;       // tile index in use
+    int tile_user;  // -1 = automatic
+    int poll;       // 0 = automatic
+    int sm_count;
+    // CG workspace (native layout), device
+    void *r, *p, *q, *y;
+    CgScalars *sc;
+    double *partials;
+    size_t partials_cap;
+    unsigned int *counter;
+    double *hist;
+    int hist_cap;
+    double *result_dev;
+    // pinned host mirrors
+    CgScalars *sc_host;
+    double *result_host;
+    // staging of the *_host calls
+    void *U_can, *U_nat, *s_can, *s_nat_in, *s_nat_out;
+    int have_gauge;
+    cudaEvent_t ev[4];
+    int last_iters;
+    int launches;
+    char err[512];
+};
+
+static char g_create_err[512] = "";
+
+static int fail(wd_ctx *ctx, int code, const char *fmt, ...)
+{
+    char *dst = ctx ? ctx->err : g_create_err;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(ctx, expr)                                                                              \
+    do {                                                                                                 \
+        cudaError_t e_ = (expr);                                                                         \
+        if (e_ != cudaSuccess)                                                                           \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? WD_ERR_ALLOC : WD_ERR_CUDA, "%s: %s", #expr, \
+                        cudaGetErrorString(e_));                                                         \
+    } while (0)
+
+static inline size_t real_bytes(const wd_ctx *c) { return c->precision == 32 ? 4 : 8; }
+static inline size_t spinor_bytes(const wd_ctx *c) { return (size_t)24 * c->V * real_bytes(c); }
+static inline size_t gauge_bytes(const wd_ctx *c) { return (size_t)72 * c->V * real_bytes(c); }
+static inline size_t spinor_vecs(const wd_ctx *c) { return (size_t)(c->precision == 32 ? 6 : 12) * c->V; }
+
+static Geom make_geom(const wd_ctx *c, int tile)
+{
+    Geom g;
+    for (int d = 0; d < 4; ++d) {
+        g.L[d] = c->dims[d];
+        g.nt[d] = (c->dims[d] + kTileShape[tile][d] - 1) / kTileShape[tile][d];
+    }
+    g.V = c->V;
+    g.bc_t = c->bc_t;
+    return g;
+}
+static long tile_blocks(const wd_ctx *c, int tile)
+{
+    long n = 1;
+    for (int d = 0; d < 4; ++d) n *= (c->dims[d] + kTileShape[tile][d] - 1) / kTileShape[tile][d];
+    return n;
+}
+static int tile_threads(int tile)
+{
+    return kTileShape[tile][0] * kTileShape[tile][1] * kTileShape[tile][2] * kTileShape[tile][3];
+}
+static bool tile_ok(const wd_ctx *c, int tile)
+{
+    if (tile < 0 || tile >= WD_NUM_TILES) return false;
+    if (c->precision == 64 && tile >= WD_NUM_TILES_SMALL) return false;
+    return true;
+}
+// Automatic choice: least padded threads; ties go to the preferred order below.
+static int auto_tile(const wd_ctx *c)
+{
+    static const int pref32[] = {8, 9, 10, 11, 0, 1, 2, 3, 4, 5, 6, 7};
+    static const int pref64[] = {0, 1, 2, 3, 4, 5, 6, 7};
+    const int *pref = c->precision == 32 ? pref32 : pref64;
+    const int n = c->precision == 32 ? 12 : 8;
+    int best = pref[0];
+    double best_waste = 1e300;
+    for (int i = 0; i < n; ++i) {
+        const int t = pref[i];
+        const double waste = (double)tile_blocks(c, t) * tile_threads(t) / (double)c->V;
+        if (waste < best_waste - 1e-12) { best_waste = waste; best = t; }
+    }
+    return best;
+}
+
+// ---------------------------------------------------------------- launches
+template <typename real, int DAG, int MODE>
+static cudaError_t launch_dslash_t(wd_ctx *c, int tile, const void *U, const void *in, void *out, double kappa,
+                                   void *r, int it)
+{
+    using svec = typename Field<real>::svec;
+    using gvec = typename Field<real>::gvec;
+    const Geom g = make_geom(c, tile);
+    const unsigned int grid = (unsigned int)tile_blocks(c, tile);
+#define X(i, a, b, cc, d)                                                                                     \
+    case i:                                                                                                   \
+        dslash_kernel<real, DAG, MODE, a, b, cc, d><<<grid, a * b * cc * d, 0, c->stream>>>(                  \
+            g, (const gvec *)U, (const svec *)in, (svec *)out, (real)kappa, (svec *)r, c->sc, c->partials,    \
+            c->counter, c->hist, it);                                                                         \
+        break;
+    if constexpr (sizeof(real) == 4) {
+        switch (tile) {
+            WD_TILES_SMALL(X)
+            WD_TILES_LARGE(X)
+            default: return cudaErrorInvalidValue;
+        }
+    } else {
+        switch (tile) {
+            WD_TILES_SMALL(X)
+            default: return cudaErrorInvalidValue;
+        }
+    }
+#undef X
+    c->launches++;
+    return cudaGetLastError();
+}
+
+template <int DAG, int MODE>
+static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void *out, double kappa, void *r, int it)
+{
+    if (c->precision == 32) return launch_dslash_t<float, DAG, MODE>(c, c->tile, U, in, out, kappa, r, it);
+    return launch_dslash_t<double, DAG, MODE>(c, c->tile, U, in, out, kappa, r, it);
+}
+
+static unsigned int vec_grid(const wd_ctx *c, size_t n)
+{
+    const size_t need = (n + VEC_NT - 1) / VEC_NT;
+    const size_t cap = (size_t)c->sm_count * 16;  // 16 CTAs of 256 threads per SM, grid-stride beyond
+    return (unsigned int)(need < cap ? (need ? need : 1) : cap);
+}
+
+static int ensure_workspace(wd_ctx *c, int max_iter)
+{
+    const size_t sb = spinor_bytes(c);
+    if (!c->r) {
+        CUDA_TRY(c, cudaMalloc(&c->r, sb));
+        CUDA_TRY(c, cudaMalloc(&c->p, sb));
+        CUDA_TRY(c, cudaMalloc(&c->q, sb));
+        CUDA_TRY(c, cudaMalloc(&c->y, sb));
+    }
+    if (max_iter + 1 > c->hist_cap) {
+        if (c->hist) cudaFree(c->hist);
+        c->hist = nullptr;
+        c->hist_cap = 0;
+        CUDA_TRY(c, cudaMalloc(&c->hist, sizeof(double) * (size_t)(max_iter + 1)));
+        c->hist_cap = max_iter + 1;
+    }
+    return WD_OK;
+}
+
+static int ensure_partials(wd_ctx *c)
+{
+    // enough for the largest grid any kernel of this ctx can use (smallest tile = 128 threads, no padding bound: use
+    // the per-tile maximum) and the vector kernels
+    size_t need = (size_t)c->sm_count * 16;
+    for (int t = 0; t < WD_NUM_TILES; ++t) {
+        const size_t nb = (size_t)tile_blocks(c, t);
+        if (nb > need) need = nb;
+    }
+    if (need > c->partials_cap) {
+        if (c->partials) cudaFree(c->partials);
+        c->partials = nullptr;
+        c->partials_cap = 0;
+        CUDA_TRY(c, cudaMalloc(&c->partials, need * sizeof(double)));
+        c->partials_cap = need;
+    }
+    return WD_OK;
+}
+
+// ---------------------------------------------------------------- context
+extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_t, void *cuda_stream)
+{
+    if (!out || !dims) return fail(nullptr, WD_ERR_ARG, "wd_create: NULL argument");
+    *out = nullptr;
+    if (precision != 32 && precision != 64) return fail(nullptr, WD_ERR_PRECISION, "wd_create: precision must be 32 or 64");
+    if (bc_t != -1 && bc_t != 1) return fail(nullptr, WD_ERR_ARG, "wd_create: bc_t must be -1 or +1");
+    double vol = 1.0;
+    for (int d = 0; d < 4; ++d) {
+        if (dims[d] < 4) return fail(nullptr, WD_ERR_DIMS, "wd_create: extent %d of direction %d is < 4", dims[d], d);
+        vol *= dims[d];
+    }
+    if (vol * 36.0 >= 2147483647.0) return fail(nullptr, WD_ERR_DIMS, "wd_create: volume too large for 32-bit plane indexing");
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(nullptr, WD_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    int sms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return fail(nullptr, WD_ERR_CUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+    wd_ctx *c = (wd_ctx *)calloc(1, sizeof(wd_ctx));
+    if (!c) return fail(nullptr, WD_ERR_ALLOC, "wd_create: out of host memory");
+    for (int d = 0; d < 4; ++d) c->dims[d] = dims[d];
+    c->V = (int)vol;
+    c->precision = precision;
+    c->bc_t = bc_t;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->sm_count = sms;
+    c->tile_user = -1;
+    c->tile = auto_tile(c);
+    bool ok = true;
+    ok = ok && cudaMalloc(&c->sc, sizeof(CgScalars)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->counter, sizeof(unsigned int)) == cudaSuccess;
+    ok = ok && cudaMalloc(&c->result_dev, sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMallocHost(&c->sc_host, sizeof(CgScalars)) == cudaSuccess;
+    ok = ok && cudaMallocHost(&c->result_host, sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMemsetAsync(c->counter, 0, sizeof(unsigned int), c->stream) == cudaSuccess;
+    ok = ok && cudaMemsetAsync(c->sc, 0, sizeof(CgScalars), c->stream) == cudaSuccess;
+    for (int i = 0; i < 4 && ok; ++i) ok = cudaEventCreate(&c->ev[i]) == cudaSuccess;
+    if (ok) ok = ensure_partials(c) == WD_OK;
+    if (!ok) {
+        fail(nullptr, WD_ERR_ALLOC, "wd_create: allocating the ctx state failed: %s", cudaGetErrorString(cudaGetLastError()));
+        wd_destroy(c);
+        return WD_ERR_ALLOC;
+    }
+    *out = c;
+    return WD_OK;
+}
+
+extern "C" int wd_destroy(wd_ctx *c)
+{
+    if (!c) return WD_OK;
+    cudaStreamSynchronize(c->stream);
+    void *dev[] = {c->r, c->p, c->q, c->y, c->sc, c->partials, c->counter, c->hist, c->result_dev,
+                   c->U_can, c->U_nat, c->s_can, c->s_nat_in, c->s_nat_out};
+    for (void *ptr : dev)
+        if (ptr) cudaFree(ptr);
+    if (c->sc_host) cudaFreeHost(c->sc_host);
+    if (c->result_host) cudaFreeHost(c->result_host);
+    for (int i = 0; i < 4; ++i)
+        if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    free(c);
+    return WD_OK;
+}
+
+extern "C" const char *wd_last_error(wd_ctx *c) { return c ? c->err : g_create_err; }
+extern "C" size_t wd_gauge_native_bytes(wd_ctx *c) { return c ? gauge_bytes(c) : 0; }
+extern "C" size_t wd_spinor_native_bytes(wd_ctx *c) { return c ? spinor_bytes(c) : 0; }
+extern "C" const char *wd_version(void) { return "wilson_cg 0.1 sm_100a"; }
+
+extern "C" int wd_num_tiles(void) { return WD_NUM_TILES; }
+extern "C" int wd_tile_shape(int index, int shape[4])
+{
+    if (index < 0 || index >= WD_NUM_TILES || !shape) return WD_ERR_ARG;
+    for (int d = 0; d < 4; ++d) shape[d] = kTileShape[index][d];
+    return WD_OK;
+}
+extern "C" int wd_set_tile(wd_ctx *c, int index)
+{
+    if (!c) return WD_ERR_ARG;
+    if (index == -1) {
+        c->tile_user = -1;
+        c->tile = auto_tile(c);
+        return WD_OK;
+    }
+    if (!tile_ok(c, index)) return fail(c, WD_ERR_ARG, "wd_set_tile: tile %d not available for precision %d", index, c->precision);
+    c->tile_user = index;
+    c->tile = index;
+    return WD_OK;
+}
+extern "C" int wd_get_tile(wd_ctx *c) { return c ? c->tile : WD_ERR_ARG; }
+extern "C" int wd_set_poll_interval(wd_ctx *c, int n)
+{
+    if (!c || n < 0) return WD_ERR_ARG;
+    c->poll = n;
+    return WD_OK;
+}
+
+// ---------------------------------------------------------------- a0: pack / unpack
+extern "C" int wd_pack_gauge(wd_ctx *c, const void *can, void *nat)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!can || !nat || can == nat) return fail(c, WD_ERR_ARG, "wd_pack_gauge: NULL or aliased argument");
+    const unsigned int grid = (c->V + VEC_NT - 1) / VEC_NT;
+    if (c->precision == 32)
+        pack_gauge_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float2 *)can, (float2 *)nat, c->V);
+    else
+        pack_gauge_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V);
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+    return WD_OK;
+}
+extern "C" int wd_pack_spinor(wd_ctx *c, const void *can, void *nat)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!can || !nat || can == nat) return fail(c, WD_ERR_ARG, "wd_pack_spinor: NULL or aliased argument");
+    const unsigned int grid = (c->V + VEC_NT - 1) / VEC_NT;
+    if (c->precision == 32)
+        pack_spinor_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float4 *)can, (float4 *)nat, c->V);
+    else
+        pack_spinor_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V);
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+    return WD_OK;
+}
+extern "C" int wd_unpack_spinor(wd_ctx *c, const void *nat, void *can)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!can || !nat || can == nat) return fail(c, WD_ERR_ARG, "wd_unpack_spinor: NULL or aliased argument");
+    const unsigned int grid = (c->V + VEC_NT - 1) / VEC_NT;
+    if (c->precision == 32)
+        unpack_spinor_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float4 *)nat, (float4 *)can, c->V);
+    else
+        unpack_spinor_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)nat, (double2 *)can, c->V);
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+    return WD_OK;
+}
+
+// ---------------------------------------------------------------- a7: wd_apply
+extern "C" int wd_apply(wd_ctx *c, const void *U, const void *psi, void *out, double kappa, int dagger)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!U || !psi || !out || psi == out) return fail(c, WD_ERR_ARG, "wd_apply: NULL argument or out aliases psi");
+    if (!std::isfinite(kappa)) return fail(c, WD_ERR_ARG, "wd_apply: kappa is not finite");
+    cudaError_t e = dagger ? launch_dslash<1, MODE_PLAIN>(c, U, psi, out, kappa, nullptr, 0)
+                           : launch_dslash<0, MODE_PLAIN>(c, U, psi, out, kappa, nullptr, 0);
+    CUDA_TRY(c, e);
+    return WD_OK;
+}
+
+extern "C" int wd_norm2(wd_ctx *c, const void *a, double *result)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!a || !result) return fail(c, WD_ERR_ARG, "wd_norm2: NULL argument");
+    const size_t n = spinor_vecs(c);
+    const unsigned int grid = vec_grid(c, n);
+    if (c->precision == 32)
+        norm2_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float4 *)a, n, c->partials, c->counter, c->result_dev);
+    else
+        norm2_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)a, n, c->partials, c->counter, c->result_dev);
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+    CUDA_TRY(c, cudaMemcpyAsync(c->result_host, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    *result = *c->result_host;
+    return WD_OK;
+}
+
+// ---------------------------------------------------------------- a1-a6: cg_solve
+static int auto_poll(const wd_ctx *c)
+{
+    // enqueue about 0.4 ms of modelled work (1536 B/site/iteration fp32 at ~6 TB/s) between two polls
+    const double t_iter = (c->precision == 32 ? 1536.0 : 3072.0) * c->V / 6.0e12;
+    int n = (int)std::ceil(4.0e-4 / (t_iter > 1e-9 ? t_iter : 1e-9));
+    if (n < 4) n = 4;
+    if (n > 32) n = 32;
+    return n;
+}
+
+static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, double kappa, double r_min, int max_iter,
+                     wd_cg_info *info, bool record_events)
+{
+    int rc = ensure_workspace(c, max_iter);
+    if (rc != WD_OK) return rc;
+    const size_t n = spinor_vecs(c);
+    const unsigned int vgrid = vec_grid(c, n);
+    if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
+    if (c->precision == 32)
+        cg_init_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((const float4 *)eta, (float4 *)c->y, (float4 *)c->r,
+                                                               (float4 *)c->p, n, c->sc, c->partials, c->counter,
+                                                               c->hist, r_min, max_iter);
+    else
+        cg_init_kernel<double><<<vgrid, VEC_NT, 0, c->stream>>>((const double2 *)eta, (double2 *)c->y, (double2 *)c->r,
+                                                                (double2 *)c->p, n, c->sc, c->partials, c->counter,
+                                                                c->hist, r_min, max_iter);
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+
+    const int poll = c->poll > 0 ? c->poll : auto_poll(c);
+    int launched = 0;
+    while (launched < max_iter) {
+        const int chunk = (max_iter - launched) < poll ? (max_iter - launched) : poll;
+        for (int i = 0; i < chunk; ++i) {
+            const int it = launched + i;
+            // a2: q = D-dagger p, qq, alpha
+            CUDA_TRY(c, (launch_dslash<1, MODE_QQ>(c, U, c->p, c->q, kappa, nullptr, it)));
+            // a3: r -= alpha D q, rr', beta, loop condition
+            CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it)));
+            // a4: y += alpha p ; p = r + beta p
+            if (c->precision == 32)
+                cg_update_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((float4 *)c->y, (float4 *)c->p,
+                                                                          (const float4 *)c->r, n, c->sc, it);
+            else
+                cg_update_kernel<double><<<vgrid, VEC_NT, 0, c->stream>>>((double2 *)c->y, (double2 *)c->p,
+                                                                           (const double2 *)c->r, n, c->sc, it);
+            c->launches++;
+            CUDA_TRY(c, cudaGetLastError());
+        }
+        launched += chunk;
+        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (c->sc_host->k_stop <= launched) break;  // the device loop condition failed (or eta = 0)
+    }
+    // a6: psi = D-dagger y ("then we multiply the solution by D-dagger")
+    CUDA_TRY(c, (launch_dslash<1, MODE_PLAIN>(c, U, c->y, psi, kappa, nullptr, 0)));
+    if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    const CgScalars &s = *c->sc_host;
+    c->last_iters = s.k;
+    if (info) {
+        info->iterations = s.k;
+        info->converged = s.converged;
+        info->rel_residual = s.eta2 > 0.0 ? std::sqrt(s.rr / s.eta2) : 0.0;
+        info->eta_norm2 = s.eta2;
+        float ms = 0.f;
+        if (record_events) CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]));
+        info->gpu_ms = ms;
+        info->total_ms = ms;
+        info->kernel_launches = c->launches;
+        info->reserved = 0;
+    }
+    return s.converged ? WD_OK : WD_NOT_CONVERGED;
+}
+
+static int check_cg_args(wd_ctx *c, const void *a, const void *b, const void *out, double kappa, double r_min,
+                         int max_iter, const char *who)
+{
+    if (!a && !c->have_gauge) return fail(c, WD_ERR_ARG, "%s: NULL gauge field", who);
+    if (!b || !out || b == out) return fail(c, WD_ERR_ARG, "%s: NULL argument or output aliases eta", who);
+    if (!std::isfinite(kappa)) return fail(c, WD_ERR_ARG, "%s: kappa is not finite", who);
+    if (!(r_min > 0.0) || !std::isfinite(r_min)) return fail(c, WD_ERR_ARG, "%s: r_min must be > 0", who);
+    if (max_iter < 0) return fail(c, WD_ERR_ARG, "%s: max_iter < 0", who);
+    return WD_OK;
+}
+
+extern "C" int cg_solve(wd_ctx *c, const void *U, const void *eta, void *psi, double kappa, double r_min, int max_iter,
+                        wd_cg_info *info)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!U) return fail(c, WD_ERR_ARG, "cg_solve: NULL gauge field");
+    int rc = check_cg_args(c, U, eta, psi, kappa, r_min, max_iter, "cg_solve");
+    if (rc != WD_OK) return rc;
+    c->launches = 0;
+    return cg_device(c, U, eta, psi, kappa, r_min, max_iter, info, true);
+}
+
+/* rr after 0..k iterations of the last cg_solve on this ctx (device history copied to the host). */
+extern "C" int wd_cg_history(wd_ctx *c, double *out, int n)
+{
+    if (!c || !out || n < 0) return WD_ERR_ARG;
+    if (n > c->last_iters + 1) n = c->last_iters + 1;
+    if (n > c->hist_cap) n = c->hist_cap;
+    if (n > 0) {
+        CUDA_TRY(c, cudaMemcpyAsync(out, c->hist, sizeof(double) * n, cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    }
+    return n;
+}
+
+// ---------------------------------------------------------------- host-buffer forms
+static int ensure_staging(wd_ctx *c)
+{
+    if (!c->U_can) CUDA_TRY(c, cudaMalloc(&c->U_can, gauge_bytes(c)));
+    if (!c->U_nat) CUDA_TRY(c, cudaMalloc(&c->U_nat, gauge_bytes(c)));
+    if (!c->s_can) CUDA_TRY(c, cudaMalloc(&c->s_can, spinor_bytes(c)));
+    if (!c->s_nat_in) CUDA_TRY(c, cudaMalloc(&c->s_nat_in, spinor_bytes(c)));
+    if (!c->s_nat_out) CUDA_TRY(c, cudaMalloc(&c->s_nat_out, spinor_bytes(c)));
+    return WD_OK;
+}
+
+static int stage_inputs(wd_ctx *c, const void *U_host, const void *s_host)
+{
+    int rc = ensure_staging(c);
+    if (rc != WD_OK) return rc;
+    if (U_host) {
+        CUDA_TRY(c, cudaMemcpyAsync(c->U_can, U_host, gauge_bytes(c), cudaMemcpyHostToDevice, c->stream));
+        rc = wd_pack_gauge(c, c->U_can, c->U_nat);
+        if (rc != WD_OK) return rc;
+        c->have_gauge = 1;
+    }
+    CUDA_TRY(c, cudaMemcpyAsync(c->s_can, s_host, spinor_bytes(c), cudaMemcpyHostToDevice, c->stream));
+    return wd_pack_spinor(c, c->s_can, c->s_nat_in);
+}
+
+static int return_output(wd_ctx *c, void *out_host)
+{
+    int rc = wd_unpack_spinor(c, c->s_nat_out, c->s_can);
+    if (rc != WD_OK) return rc;
+    CUDA_TRY(c, cudaMemcpyAsync(out_host, c->s_can, spinor_bytes(c), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaEventRecord(c->ev[3], c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return WD_OK;
+}
+
+extern "C" int wd_apply_host(wd_ctx *c, const void *U_host, const void *psi_host, void *out_host, double kappa, int dagger)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!U_host && !c->have_gauge) return fail(c, WD_ERR_ARG, "wd_apply_host: NULL gauge field and none cached");
+    if (!psi_host || !out_host || psi_host == out_host) return fail(c, WD_ERR_ARG, "wd_apply_host: NULL or aliased argument");
+    if (!std::isfinite(kappa)) return fail(c, WD_ERR_ARG, "wd_apply_host: kappa is not finite");
+    c->launches = 0;
+    int rc = stage_inputs(c, U_host, psi_host);
+    if (rc != WD_OK) return rc;
+    rc = wd_apply(c, c->U_nat, c->s_nat_in, c->s_nat_out, kappa, dagger);
+    if (rc != WD_OK) return rc;
+    return return_output(c, out_host);
+}
+
+extern "C" int cg_solve_host(wd_ctx *c, const void *U_host, const void *eta_host, void *psi_host, double kappa,
+                             double r_min, int max_iter, wd_cg_info *info)
+{
+    if (!c) return WD_ERR_ARG;
+    int rc = check_cg_args(c, U_host, eta_host, psi_host, kappa, r_min, max_iter, "cg_solve_host");
+    if (rc != WD_OK) return rc;
+    c->launches = 0;
+    CUDA_TRY(c, cudaEventRecord(c->ev[2], c->stream));
+    rc = stage_inputs(c, U_host, eta_host);
+    if (rc != WD_OK) return rc;
+    const int status = cg_device(c, c->U_nat, c->s_nat_in, c->s_nat_out, kappa, r_min, max_iter, info, true);
+    if (status < 0) return status;
+    rc = return_output(c, psi_host);
+    if (rc != WD_OK) return rc;
+    if (info) {
+        float ms = 0.f;
+        CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev[2], c->ev[3]));
+        info->total_ms = ms;
+        info->kernel_launches = c->launches;
+    }
+    return status;
+}

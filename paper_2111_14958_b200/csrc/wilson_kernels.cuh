@@ -1,0 +1,504 @@
+// wilson_kernels.cuh — device code of the Wilson-Dirac stencil and the fused CG kernels (sm_100a).
+//
+// What is computed (citations: PAPER.md = the paper text; C-1/C-2/Gnn = readings in DESIGN.md):
+//   * D / D-dagger of reading C-1 as a matrix-free 9-point stencil: per site and direction, spin
+//     projection to a half-spinor BEFORE the SU(3) multiply, U (forward) or U^dagger (backward, by
+//     index transposition + conjugation of the neighbour's link), boundary sign on the t-wrap hop,
+//     reconstruction into the 4-spinor accumulator.  This replaces the paper's COO SpMV
+//     (PAPER.md:50-56), which it calls "not optimal".
+//   * the CG recurrence of PAPER.md:46-48 (readings G1-G5) with its dot products and vector updates
+//     fused into the stencil passes: MODE_QQ produces |D-dagger p|^2 and alpha, MODE_RUPD applies
+//     r <- r - alpha D q and produces |r|^2, beta and the loop condition, all in device memory.
+//
+// Data layout (include/wilson_cg.h "Native layouts"): site-planar SoA.  A spinor is NSP planes of
+// 128-bit vectors (float4 = two complex components, double2 = one), a link 9 planes of one complex
+// each; plane stride = V; the site index inside a plane is lexicographic, x fastest.  One thread owns
+// one site; a CTA owns a BX x BY x BZ x BT tile so that the 8 neighbours of most sites are fetched by
+// the same CTA (L1 reuse) and all loads of a warp are contiguous runs of BX sites.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace wd {
+
+struct Geom {
+    int L[4];    // Lx, Ly, Lz, Lt
+    int V;       // volume = plane stride
+    int nt[4];   // tiles per direction (ceil)
+    int bc_t;    // -1 antiperiodic, +1 periodic
+};
+
+// Device-resident CG state.  All fp64 (reading G17).
+struct CgScalars {
+    double rr;        // <r,r> (recursed)
+    double qq;        // <q,q>, q = D-dagger p
+    double alpha;     // rr / qq
+    double beta;      // rr' / rr
+    double eta2;      // <eta,eta>
+    double r_min;     // relative tolerance
+    int k;            // completed loop bodies
+    int k_stop;       // kernels of iteration `it` run iff it < k_stop (initially max_iter)
+    int max_iter;
+    int converged;
+};
+
+template <typename real> struct Field;
+template <> struct Field<float> {
+    using svec = float4;
+    using gvec = float2;
+    static constexpr int NSP = 6;  // spinor planes
+};
+template <> struct Field<double> {
+    using svec = double2;
+    using gvec = double2;
+    static constexpr int NSP = 12;
+};
+
+// ---------------------------------------------------------------- loads / stores
+__device__ __forceinline__ void load_spinor(const float4 *__restrict__ base, size_t V, int s, float v[24])
+{
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        const float4 t = __ldg(base + j * V + s);
+        v[4 * j + 0] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
+    }
+}
+__device__ __forceinline__ void load_spinor(const double2 *__restrict__ base, size_t V, int s, double v[24])
+{
+#pragma unroll
+    for (int j = 0; j < 12; ++j) {
+        const double2 t = __ldg(base + j * V + s);
+        v[2 * j + 0] = t.x; v[2 * j + 1] = t.y;
+    }
+}
+// Read-write fields (r in MODE_RUPD): coherent load, not the read-only path.
+__device__ __forceinline__ void load_spinor_rw(const float4 *base, size_t V, int s, float v[24])
+{
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+        const float4 t = base[j * V + s];
+        v[4 * j + 0] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
+    }
+}
+__device__ __forceinline__ void load_spinor_rw(const double2 *base, size_t V, int s, double v[24])
+{
+#pragma unroll
+    for (int j = 0; j < 12; ++j) {
+        const double2 t = base[j * V + s];
+        v[2 * j + 0] = t.x; v[2 * j + 1] = t.y;
+    }
+}
+__device__ __forceinline__ void store_spinor(float4 *base, size_t V, int s, const float v[24])
+{
+#pragma unroll
+    for (int j = 0; j < 6; ++j) base[j * V + s] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+}
+__device__ __forceinline__ void store_spinor(double2 *base, size_t V, int s, const double v[24])
+{
+#pragma unroll
+    for (int j = 0; j < 12; ++j) base[j * V + s] = make_double2(v[2 * j], v[2 * j + 1]);
+}
+template <typename gvec, typename real>
+__device__ __forceinline__ void load_link(const gvec *__restrict__ U, size_t V, int mu, int s, real u[18])
+{
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        const gvec t = __ldg(U + (size_t)(mu * 9 + k) * V + s);
+        u[2 * k] = t.x; u[2 * k + 1] = t.y;
+    }
+}
+
+// ---------------------------------------------------------------- spin projection (reading C-2)
+// v[(alpha*3+c)*2+ri] -> h[(sp*3+c)*2+ri], the upper two rows of (1 + S gamma_MU) v, S = +-1.
+template <int MU, int S, typename real>
+__device__ __forceinline__ void project(const real v[24], real h[12])
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const real p0r = v[(0 + c) * 2], p0i = v[(0 + c) * 2 + 1];
+        const real p1r = v[(3 + c) * 2], p1i = v[(3 + c) * 2 + 1];
+        const real p2r = v[(6 + c) * 2], p2i = v[(6 + c) * 2 + 1];
+        const real p3r = v[(9 + c) * 2], p3i = v[(9 + c) * 2 + 1];
+        real h0r, h0i, h1r, h1i;
+        if (MU == 0) {        // h0 = p0 + S i p3 ; h1 = p1 + S i p2
+            h0r = p0r - S * p3i; h0i = p0i + S * p3r;
+            h1r = p1r - S * p2i; h1i = p1i + S * p2r;
+        } else if (MU == 1) { // h0 = p0 - S p3 ; h1 = p1 + S p2
+            h0r = p0r - S * p3r; h0i = p0i - S * p3i;
+            h1r = p1r + S * p2r; h1i = p1i + S * p2i;
+        } else if (MU == 2) { // h0 = p0 + S i p2 ; h1 = p1 - S i p3
+            h0r = p0r - S * p2i; h0i = p0i + S * p2r;
+            h1r = p1r + S * p3i; h1i = p1i - S * p3r;
+        } else {              // h0 = p0 + S p2 ; h1 = p1 + S p3
+            h0r = p0r + S * p2r; h0i = p0i + S * p2i;
+            h1r = p1r + S * p3r; h1i = p1i + S * p3i;
+        }
+        h[(0 + c) * 2] = h0r; h[(0 + c) * 2 + 1] = h0i;
+        h[(3 + c) * 2] = h1r; h[(3 + c) * 2 + 1] = h1i;
+    }
+}
+
+// g = U h (ADJ = false) or U^dagger h (ADJ = true) on both spin components of the half-spinor.
+template <bool ADJ, typename real>
+__device__ __forceinline__ void mul_su3(const real u[18], const real h[12], real g[12])
+{
+#pragma unroll
+    for (int sp = 0; sp < 2; ++sp)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            real gr = 0, gi = 0;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const real ur = ADJ ? u[(c * 3 + a) * 2] : u[(a * 3 + c) * 2];
+                const real ui = ADJ ? -u[(c * 3 + a) * 2 + 1] : u[(a * 3 + c) * 2 + 1];
+                const real hr = h[(sp * 3 + c) * 2], hi = h[(sp * 3 + c) * 2 + 1];
+                gr = fma(ur, hr, gr); gr = fma(-ui, hi, gr);
+                gi = fma(ur, hi, gi); gi = fma(ui, hr, gi);
+            }
+            g[(sp * 3 + a) * 2] = gr; g[(sp * 3 + a) * 2 + 1] = gi;
+        }
+}
+
+// acc += sg * reconstruct_{MU,S}(g): rows 0,1 get g, rows 2,3 the table of reading C-2.
+template <int MU, int S, typename real>
+__device__ __forceinline__ void reconstruct(const real g[12], real sg, real acc[24])
+{
+    const real c = sg * S;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const real g0r = g[(0 + a) * 2], g0i = g[(0 + a) * 2 + 1];
+        const real g1r = g[(3 + a) * 2], g1i = g[(3 + a) * 2 + 1];
+        acc[(0 + a) * 2] = fma(sg, g0r, acc[(0 + a) * 2]);
+        acc[(0 + a) * 2 + 1] = fma(sg, g0i, acc[(0 + a) * 2 + 1]);
+        acc[(3 + a) * 2] = fma(sg, g1r, acc[(3 + a) * 2]);
+        acc[(3 + a) * 2 + 1] = fma(sg, g1i, acc[(3 + a) * 2 + 1]);
+        if (MU == 0) {        // row2 += -S i g1 ; row3 += -S i g0
+            acc[(6 + a) * 2] = fma(c, g1i, acc[(6 + a) * 2]);
+            acc[(6 + a) * 2 + 1] = fma(-c, g1r, acc[(6 + a) * 2 + 1]);
+            acc[(9 + a) * 2] = fma(c, g0i, acc[(9 + a) * 2]);
+            acc[(9 + a) * 2 + 1] = fma(-c, g0r, acc[(9 + a) * 2 + 1]);
+        } else if (MU == 1) { // row2 += S g1 ; row3 += -S g0
+            acc[(6 + a) * 2] = fma(c, g1r, acc[(6 + a) * 2]);
+            acc[(6 + a) * 2 + 1] = fma(c, g1i, acc[(6 + a) * 2 + 1]);
+            acc[(9 + a) * 2] = fma(-c, g0r, acc[(9 + a) * 2]);
+            acc[(9 + a) * 2 + 1] = fma(-c, g0i, acc[(9 + a) * 2 + 1]);
+        } else if (MU == 2) { // row2 += -S i g0 ; row3 += S i g1
+            acc[(6 + a) * 2] = fma(c, g0i, acc[(6 + a) * 2]);
+            acc[(6 + a) * 2 + 1] = fma(-c, g0r, acc[(6 + a) * 2 + 1]);
+            acc[(9 + a) * 2] = fma(-c, g1i, acc[(9 + a) * 2]);
+            acc[(9 + a) * 2 + 1] = fma(c, g1r, acc[(9 + a) * 2 + 1]);
+        } else {              // row2 += S g0 ; row3 += S g1
+            acc[(6 + a) * 2] = fma(c, g0r, acc[(6 + a) * 2]);
+            acc[(6 + a) * 2 + 1] = fma(c, g0i, acc[(6 + a) * 2 + 1]);
+            acc[(9 + a) * 2] = fma(c, g1r, acc[(9 + a) * 2]);
+            acc[(9 + a) * 2 + 1] = fma(c, g1i, acc[(9 + a) * 2 + 1]);
+        }
+    }
+}
+
+// One hop: acc += sg (1 + S gamma_MU) (x) [U or U^dagger](link_site) in(spinor_site).
+template <int MU, int S, bool ADJ, typename real, typename svec, typename gvec>
+__device__ __forceinline__ void hop(const gvec *__restrict__ U, const svec *__restrict__ in, size_t V,
+                                    int link_site, int spinor_site, real sg, real acc[24])
+{
+    real v[24], h[12], u[18], g[12];
+    load_spinor(in, V, spinor_site, v);
+    load_link<gvec, real>(U, V, MU, link_site, u);
+    project<MU, S, real>(v, h);
+    mul_su3<ADJ, real>(u, h, g);
+    reconstruct<MU, S, real>(g, sg, acc);
+}
+
+// acc = sum over the 8 hops at site s = (x,y,z,t).  DAG = 0: D (forward projector 1 - gamma), 1: D-dagger.
+template <int DAG, typename real, typename svec, typename gvec>
+__device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const svec *__restrict__ in,
+                                            int x, int y, int z, int t, int s, real acc[24])
+{
+    constexpr int SF = DAG ? +1 : -1;
+    const size_t V = (size_t)g.V;
+    const int L0 = g.L[0], L1 = g.L[1], L2 = g.L[2], L3 = g.L[3];
+    const int s1 = L0, s2 = L0 * L1, s3 = L0 * L1 * L2;
+#pragma unroll
+    for (int i = 0; i < 24; ++i) acc[i] = 0;
+    {
+        const int sf = s + (x == L0 - 1 ? 1 - L0 : 1);
+        const int sb = s + (x == 0 ? L0 - 1 : -1);
+        hop<0, SF, false, real>(U, in, V, s, sf, (real)1, acc);
+        hop<0, -SF, true, real>(U, in, V, sb, sb, (real)1, acc);
+    }
+    {
+        const int sf = s + (y == L1 - 1 ? (1 - L1) * s1 : s1);
+        const int sb = s + (y == 0 ? (L1 - 1) * s1 : -s1);
+        hop<1, SF, false, real>(U, in, V, s, sf, (real)1, acc);
+        hop<1, -SF, true, real>(U, in, V, sb, sb, (real)1, acc);
+    }
+    {
+        const int sf = s + (z == L2 - 1 ? (1 - L2) * s2 : s2);
+        const int sb = s + (z == 0 ? (L2 - 1) * s2 : -s2);
+        hop<2, SF, false, real>(U, in, V, s, sf, (real)1, acc);
+        hop<2, -SF, true, real>(U, in, V, sb, sb, (real)1, acc);
+    }
+    {
+        // boundary sign sigma+- of reading C-1: only the hop that wraps the t boundary carries bc_t
+        const bool wf = (t == L3 - 1), wb = (t == 0);
+        const int sf = s + (wf ? (1 - L3) * s3 : s3);
+        const int sb = s + (wb ? (L3 - 1) * s3 : -s3);
+        const real sgf = wf ? (real)g.bc_t : (real)1;
+        const real sgb = wb ? (real)g.bc_t : (real)1;
+        hop<3, SF, false, real>(U, in, V, s, sf, sgf, acc);
+        hop<3, -SF, true, real>(U, in, V, sb, sb, sgb, acc);
+    }
+}
+
+// ---------------------------------------------------------------- deterministic reductions
+// Fixed-shape tree: warp shuffle -> one slot per warp -> warp 0.  Result valid on thread 0.
+template <int NT>
+__device__ __forceinline__ double block_sum(double v, double *sm /* >= 32 doubles */)
+{
+    constexpr int NW = (NT + 31) / 32;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (lane == 0) sm[w] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (w == 0) {
+        t = lane < NW ? sm[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+    }
+    __syncthreads();
+    return t;
+}
+
+// Single-pass grid reduction: every CTA stores its partial; the CTA that draws the last ticket sums
+// the partials in index order (same order every run -> run-to-run identical alpha, beta).
+// Returns true on thread 0 of that last CTA only, with the grid total in *total.
+template <int NT>
+__device__ __forceinline__ bool grid_sum(double v, double *partials, unsigned int *counter, double *total)
+{
+    __shared__ double sm[32];
+    __shared__ int is_last;
+    const double b = block_sum<NT>(v, sm);
+    if (threadIdx.x == 0) {
+        partials[blockIdx.x] = b;
+        __threadfence();
+        const unsigned int ticket = atomicAdd(counter, 1u);
+        is_last = (ticket == gridDim.x - 1);
+        __threadfence();
+    }
+    __syncthreads();
+    if (!is_last) return false;
+    double a = 0.0;
+    for (unsigned int i = threadIdx.x; i < gridDim.x; i += NT) a += __ldcg(partials + i);
+    const double tot = block_sum<NT>(a, sm);
+    if (threadIdx.x == 0) {
+        *counter = 0u;  // ready for the next launch on this stream
+        *total = tot;
+        return true;
+    }
+    return false;
+}
+
+// Scalar epilogues, run by one thread of the last CTA.
+__device__ __forceinline__ void finish_qq(CgScalars *sc, double qq)
+{
+    sc->qq = qq;
+    sc->alpha = sc->rr / qq;                       // alpha <- |r|^2 / |D-dagger p|^2 (G1)
+}
+__device__ __forceinline__ void finish_rr(CgScalars *sc, double rr_new, int it, double *hist)
+{
+    sc->beta = rr_new / sc->rr;                    // beta <- |r'|^2 / |r|^2 (G1)
+    sc->rr = rr_new;
+    sc->k = it + 1;
+    if (hist) hist[it + 1] = rr_new;
+    // while |r| >= r_min read as relative 2-norm (G4): stop as soon as it fails
+    if (!(sqrt(rr_new) >= sc->r_min * sqrt(sc->eta2))) {
+        sc->k_stop = it + 1;
+        sc->converged = 1;
+    }
+}
+
+// ---------------------------------------------------------------- the stencil kernel
+enum { MODE_PLAIN = 0, MODE_QQ = 1, MODE_RUPD = 2 };
+
+// MODE_PLAIN : out = D in / D-dagger in                                  (wd_apply, a6, a7)
+// MODE_QQ    : out = q = D-dagger p, qq = |q|^2, alpha = rr/qq           (a2)
+// MODE_RUPD  : s = D q (not stored), r <- r - alpha s, rr' = |r|^2, beta, loop condition   (a3)
+template <typename real, int DAG, int MODE, int BX, int BY, int BZ, int BT>
+__global__ void __launch_bounds__(BX *BY *BZ *BT)
+dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
+              const typename Field<real>::svec *__restrict__ in, typename Field<real>::svec *out, real kappa,
+              typename Field<real>::svec *r, CgScalars *sc, double *partials, unsigned int *counter,
+              double *hist, int it)
+{
+    using svec = typename Field<real>::svec;
+    using gvec = typename Field<real>::gvec;
+    constexpr int NT = BX * BY * BZ * BT;
+    if (MODE != MODE_PLAIN) {
+        if (it >= sc->k_stop) return;  // uniform over the grid: over-launched iterations are no-ops
+    }
+    int b = blockIdx.x;
+    const int tx = b % g.nt[0]; b /= g.nt[0];
+    const int ty = b % g.nt[1]; b /= g.nt[1];
+    const int tz = b % g.nt[2]; b /= g.nt[2];
+    const int tt = b;
+    const int tid = threadIdx.x;
+    const int x = tx * BX + tid % BX;
+    const int y = ty * BY + (tid / BX) % BY;
+    const int z = tz * BZ + (tid / (BX * BY)) % BZ;
+    const int t = tt * BT + tid / (BX * BY * BZ);
+    const bool active = (x < g.L[0]) && (y < g.L[1]) && (z < g.L[2]) && (t < g.L[3]);
+    const size_t V = (size_t)g.V;
+    double local = 0.0;
+    if (active) {
+        const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
+        real acc[24], c[24];
+        hopping_sum<DAG, real, svec, gvec>(g, U, in, x, y, z, t, s, acc);
+        load_spinor(in, V, s, c);
+#pragma unroll
+        for (int i = 0; i < 24; ++i) c[i] = fma(-kappa, acc[i], c[i]);  // (D in)(x) = in(x) - kappa * hops
+        if (MODE == MODE_RUPD) {
+            const real alpha = (real)sc->alpha;
+            real rv[24];
+            load_spinor_rw(r, V, s, rv);
+            real n2 = 0;
+#pragma unroll
+            for (int i = 0; i < 24; ++i) {
+                rv[i] = fma(-alpha, c[i], rv[i]);                      // r <- r - alpha D D-dagger p
+                n2 = fma(rv[i], rv[i], n2);
+            }
+            store_spinor(r, V, s, rv);
+            local = (double)n2;
+        } else {
+            store_spinor(out, V, s, c);
+            if (MODE == MODE_QQ) {
+                real n2 = 0;
+#pragma unroll
+                for (int i = 0; i < 24; ++i) n2 = fma(c[i], c[i], n2);
+                local = (double)n2;
+            }
+        }
+    }
+    if (MODE != MODE_PLAIN) {
+        double total;
+        if (grid_sum<NT>(local, partials, counter, &total)) {
+            if (MODE == MODE_QQ) finish_qq(sc, total);
+            else finish_rr(sc, total, it, hist);
+        }
+    }
+}
+
+// ---------------------------------------------------------------- streaming vector kernels
+constexpr int VEC_NT = 256;
+
+template <typename vec> __device__ __forceinline__ double vnorm2(const vec &a);
+template <> __device__ __forceinline__ double vnorm2<float4>(const float4 &a)
+{
+    return (double)(a.x * a.x + a.y * a.y + a.z * a.z + a.w * a.w);
+}
+template <> __device__ __forceinline__ double vnorm2<double2>(const double2 &a) { return a.x * a.x + a.y * a.y; }
+
+__device__ __forceinline__ float4 vzero(float4) { return make_float4(0.f, 0.f, 0.f, 0.f); }
+__device__ __forceinline__ double2 vzero(double2) { return make_double2(0.0, 0.0); }
+__device__ __forceinline__ float4 vaxpy(float a, const float4 &x, const float4 &y)
+{
+    return make_float4(fmaf(a, x.x, y.x), fmaf(a, x.y, y.y), fmaf(a, x.z, y.z), fmaf(a, x.w, y.w));
+}
+__device__ __forceinline__ double2 vaxpy(double a, const double2 &x, const double2 &y)
+{
+    return make_double2(fma(a, x.x, y.x), fma(a, x.y, y.y));
+}
+
+// a1: y <- 0, r <- eta, p <- eta, rr = eta2 = <eta,eta>, k = 0 ("psi <- psi0; r <- eta - D psi; p <- r", psi0 = 0)
+template <typename real>
+__global__ void __launch_bounds__(VEC_NT)
+cg_init_kernel(const typename Field<real>::svec *__restrict__ eta, typename Field<real>::svec *y,
+               typename Field<real>::svec *r, typename Field<real>::svec *p, size_t n, CgScalars *sc,
+               double *partials, unsigned int *counter, double *hist, double r_min, int max_iter)
+{
+    using svec = typename Field<real>::svec;
+    double local = 0.0;
+    for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT) {
+        const svec e = __ldg(eta + i);
+        y[i] = vzero(e);
+        r[i] = e;
+        p[i] = e;
+        local += vnorm2<svec>(e);
+    }
+    double total;
+    if (grid_sum<VEC_NT>(local, partials, counter, &total)) {
+        sc->rr = total; sc->eta2 = total; sc->qq = 0.0; sc->alpha = 0.0; sc->beta = 0.0;
+        sc->r_min = r_min; sc->k = 0; sc->max_iter = max_iter;
+        const bool go = total > 0.0 && (sqrt(total) >= r_min * sqrt(total));
+        sc->k_stop = go ? max_iter : 0;
+        sc->converged = go ? 0 : 1;
+        if (hist) hist[0] = total;
+    }
+}
+
+// a4: y <- y + alpha p ; p <- r + beta p   ("psi <- psi + alpha p", "p <- r + beta p"; G3: y, not psi)
+template <typename real>
+__global__ void __launch_bounds__(VEC_NT)
+cg_update_kernel(typename Field<real>::svec *y, typename Field<real>::svec *p,
+                 const typename Field<real>::svec *__restrict__ r, size_t n, const CgScalars *sc, int it)
+{
+    using svec = typename Field<real>::svec;
+    if (it >= sc->k_stop) return;
+    const real alpha = (real)sc->alpha, beta = (real)sc->beta;
+    for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT) {
+        const svec pv = p[i];
+        const svec rv = __ldg(r + i);
+        y[i] = vaxpy(alpha, pv, y[i]);
+        p[i] = vaxpy(beta, pv, rv);
+    }
+}
+
+// the paper's dot-product kernel on its own: <a,a>
+template <typename real>
+__global__ void __launch_bounds__(VEC_NT)
+norm2_kernel(const typename Field<real>::svec *__restrict__ a, size_t n, double *partials, unsigned int *counter,
+             double *result)
+{
+    using svec = typename Field<real>::svec;
+    double local = 0.0;
+    for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT)
+        local += vnorm2<svec>(__ldg(a + i));
+    double total;
+    if (grid_sum<VEC_NT>(local, partials, counter, &total)) *result = total;
+}
+
+// ---------------------------------------------------------------- a0: canonical <-> native permutations
+// canonical gauge U[s][mu][a][b] (complex) -> native plane (mu*9 + a*3+b), one thread per site.
+template <typename real>
+__global__ void __launch_bounds__(VEC_NT)
+pack_gauge_kernel(const typename Field<real>::gvec *__restrict__ can, typename Field<real>::gvec *nat, int V)
+{
+    const int s = blockIdx.x * VEC_NT + threadIdx.x;
+    if (s >= V) return;
+#pragma unroll 4
+    for (int k = 0; k < 36; ++k) nat[(size_t)k * V + s] = __ldg(can + (size_t)s * 36 + k);
+}
+// canonical spinor psi[s][alpha][a] (24 reals = NSP vectors, contiguous) <-> native planes.
+template <typename real>
+__global__ void __launch_bounds__(VEC_NT)
+pack_spinor_kernel(const typename Field<real>::svec *__restrict__ can, typename Field<real>::svec *nat, int V)
+{
+    constexpr int NSP = Field<real>::NSP;
+    const int s = blockIdx.x * VEC_NT + threadIdx.x;
+    if (s >= V) return;
+#pragma unroll
+    for (int j = 0; j < NSP; ++j) nat[(size_t)j * V + s] = __ldg(can + (size_t)s * NSP + j);
+}
+template <typename real>
+__global__ void __launch_bounds__(VEC_NT)
+unpack_spinor_kernel(const typename Field<real>::svec *__restrict__ nat, typename Field<real>::svec *can, int V)
+{
+    constexpr int NSP = Field<real>::NSP;
+    const int s = blockIdx.x * VEC_NT + threadIdx.x;
+    if (s >= V) return;
+#pragma unroll
+    for (int j = 0; j < NSP; ++j) can[(size_t)s * NSP + j] = __ldg(nat + (size_t)j * V + s);
+}
+
+}  // namespace wd

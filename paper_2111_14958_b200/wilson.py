@@ -1,0 +1,272 @@
+"""Thin ctypes binding of the C-ABI library (include/wilson_cg.h) — argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the ABI; there is no CPU fallback: if the
+shared object is missing this module raises at first use (build it with
+`python -m paper_2111_14958_b200.build`).  PyTorch is used for device memory and streams only.
+
+Names follow the header: wd_create -> WilsonContext, wd_apply -> .wd_apply, cg_solve -> .cg_solve, ...
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import re
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libwilson_cg.so")
+HEADER_PATH = os.path.join(os.path.dirname(HERE), "include", "wilson_cg.h")
+
+WD_OK = 0
+WD_NOT_CONVERGED = 1
+
+_lib = None
+
+
+class WdCgInfo(ctypes.Structure):
+    _fields_ = [
+        ("iterations", ctypes.c_int),
+        ("converged", ctypes.c_int),
+        ("rel_residual", ctypes.c_double),
+        ("eta_norm2", ctypes.c_double),
+        ("gpu_ms", ctypes.c_double),
+        ("total_ms", ctypes.c_double),
+        ("kernel_launches", ctypes.c_int),
+        ("reserved", ctypes.c_int),
+    ]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
+
+
+class WilsonError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"wilson_cg error {code}: {msg}")
+        self.code = code
+
+
+def declared_symbols(header_path: str = HEADER_PATH):
+    """Function names declared in include/wilson_cg.h (used by the symbol-export test)."""
+    text = open(header_path).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b((?:wd|cg)_[a-z0-9_]+)\s*\(", text)))
+
+
+def load_library(path: str = LIB_PATH):
+    """dlopen the library and declare the prototypes.  Raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(path):
+        raise FileNotFoundError(
+            f"{path} not found: build it with `python -m paper_2111_14958_b200.build` (no CPU fallback exists)")
+    lib = ctypes.CDLL(path)
+    vp, ip, dp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)
+    cd, ci = ctypes.c_double, ctypes.c_int
+    lib.wd_create.argtypes = [ctypes.POINTER(vp), ip, ci, ci, vp]
+    lib.wd_destroy.argtypes = [vp]
+    lib.wd_last_error.argtypes = [vp]
+    lib.wd_last_error.restype = ctypes.c_char_p
+    lib.wd_gauge_native_bytes.argtypes = [vp]
+    lib.wd_gauge_native_bytes.restype = ctypes.c_size_t
+    lib.wd_spinor_native_bytes.argtypes = [vp]
+    lib.wd_spinor_native_bytes.restype = ctypes.c_size_t
+    lib.wd_pack_gauge.argtypes = [vp, vp, vp]
+    lib.wd_pack_spinor.argtypes = [vp, vp, vp]
+    lib.wd_unpack_spinor.argtypes = [vp, vp, vp]
+    lib.wd_apply.argtypes = [vp, vp, vp, vp, cd, ci]
+    lib.cg_solve.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
+    lib.wd_apply_host.argtypes = [vp, vp, vp, vp, cd, ci]
+    lib.cg_solve_host.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
+    lib.wd_cg_history.argtypes = [vp, dp, ci]
+    lib.wd_norm2.argtypes = [vp, vp, dp]
+    lib.wd_num_tiles.argtypes = []
+    lib.wd_tile_shape.argtypes = [ci, ip]
+    lib.wd_set_tile.argtypes = [vp, ci]
+    lib.wd_get_tile.argtypes = [vp]
+    lib.wd_set_poll_interval.argtypes = [vp, ci]
+    lib.wd_version.argtypes = []
+    lib.wd_version.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def tile_shapes():
+    lib = load_library()
+    out = []
+    for i in range(lib.wd_num_tiles()):
+        shp = (ctypes.c_int * 4)()
+        lib.wd_tile_shape(i, shp)
+        out.append(tuple(shp))
+    return out
+
+
+def _torch():
+    import torch
+
+    return torch
+
+
+class WilsonContext:
+    """wd_create / wd_destroy plus one method per ABI call.  Tensors are torch CUDA tensors
+    (canonical layout: complex64/complex128 of shape (V,4,3,3) and (V,4,3); native buffers are opaque
+    1-D real tensors from `empty_gauge()` / `empty_spinor()`)."""
+
+    def __init__(self, dims, precision=32, bc_t=-1, stream=None):
+        torch = _torch()
+        if not torch.cuda.is_available():
+            raise RuntimeError("wilson_cg needs a CUDA device (no CPU fallback)")
+        self.lib = load_library()
+        self.dims = tuple(int(d) for d in dims)
+        self.volume = int(np.prod(self.dims))
+        self.precision = int(precision)
+        self.bc_t = int(bc_t)
+        self.real_dtype = torch.float32 if precision == 32 else torch.float64
+        self.complex_dtype = torch.complex64 if precision == 32 else torch.complex128
+        self.np_complex = np.complex64 if precision == 32 else np.complex128
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self._ctx = ctypes.c_void_p()
+        d = (ctypes.c_int * 4)(*self.dims)
+        rc = self.lib.wd_create(ctypes.byref(self._ctx), d, self.precision, self.bc_t,
+                                ctypes.c_void_p(self.stream.cuda_stream))
+        if rc != WD_OK:
+            raise WilsonError(rc, self.lib.wd_last_error(None).decode())
+
+    # -- plumbing
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self.lib.wd_destroy(self._ctx)
+            self._ctx = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def _check(self, rc, allow_not_converged=False):
+        if rc == WD_OK or (allow_not_converged and rc == WD_NOT_CONVERGED):
+            return rc
+        raise WilsonError(rc, self.lib.wd_last_error(self._ctx).decode())
+
+    @staticmethod
+    def _p(t):
+        return ctypes.c_void_p(t.data_ptr())
+
+    def empty_gauge(self):
+        torch = _torch()
+        n = self.lib.wd_gauge_native_bytes(self._ctx) // (4 if self.precision == 32 else 8)
+        return torch.empty(n, dtype=self.real_dtype, device="cuda")
+
+    def empty_spinor(self):
+        torch = _torch()
+        n = self.lib.wd_spinor_native_bytes(self._ctx) // (4 if self.precision == 32 else 8)
+        return torch.empty(n, dtype=self.real_dtype, device="cuda")
+
+    def _canon(self, t, shape):
+        torch = _torch()
+        if t.dtype != self.complex_dtype or tuple(t.shape) != shape or not t.is_cuda or not t.is_contiguous():
+            raise ValueError(f"expected contiguous CUDA {self.complex_dtype} tensor of shape {shape}")
+        return t
+
+    # -- a0
+    def wd_pack_gauge(self, U_canonical, out=None):
+        U_canonical = self._canon(U_canonical, (self.volume, 4, 3, 3))
+        out = self.empty_gauge() if out is None else out
+        self._check(self.lib.wd_pack_gauge(self._ctx, self._p(U_canonical), self._p(out)))
+        return out
+
+    def wd_pack_spinor(self, psi_canonical, out=None):
+        psi_canonical = self._canon(psi_canonical, (self.volume, 4, 3))
+        out = self.empty_spinor() if out is None else out
+        self._check(self.lib.wd_pack_spinor(self._ctx, self._p(psi_canonical), self._p(out)))
+        return out
+
+    def wd_unpack_spinor(self, psi_native, out=None):
+        torch = _torch()
+        if out is None:
+            out = torch.empty((self.volume, 4, 3), dtype=self.complex_dtype, device="cuda")
+        self._check(self.lib.wd_unpack_spinor(self._ctx, self._p(psi_native), self._p(out)))
+        return out
+
+    # -- a7
+    def wd_apply(self, U_native, psi_native, kappa, dagger=False, out=None):
+        out = self.empty_spinor() if out is None else out
+        self._check(self.lib.wd_apply(self._ctx, self._p(U_native), self._p(psi_native), self._p(out),
+                                      float(kappa), int(bool(dagger))))
+        return out
+
+    # -- a1..a6
+    def cg_solve(self, U_native, eta_native, kappa, r_min, max_iter, out=None):
+        out = self.empty_spinor() if out is None else out
+        info = WdCgInfo()
+        rc = self.lib.cg_solve(self._ctx, self._p(U_native), self._p(eta_native), self._p(out), float(kappa),
+                               float(r_min), int(max_iter), ctypes.byref(info))
+        self._check(rc, allow_not_converged=True)
+        d = info.as_dict()
+        d["status"] = rc
+        return out, d
+
+    def wd_cg_history(self, n=None):
+        n = int(n) if n is not None else 1 << 20
+        buf = np.zeros(n, dtype=np.float64)
+        got = self.lib.wd_cg_history(self._ctx, buf.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), n)
+        if got < 0:
+            self._check(got)
+        return buf[:got].copy()
+
+    def wd_norm2(self, a_native):
+        res = ctypes.c_double()
+        self._check(self.lib.wd_norm2(self._ctx, self._p(a_native), ctypes.byref(res)))
+        return res.value
+
+    # -- host-buffer forms (numpy arrays or pinned torch CPU tensors, canonical layout)
+    def _host_ptr(self, a, shape, writable=False):
+        torch = _torch()
+        if isinstance(a, torch.Tensor):
+            if a.is_cuda or a.dtype != self.complex_dtype or tuple(a.shape) != shape or not a.is_contiguous():
+                raise ValueError(f"expected contiguous CPU {self.complex_dtype} tensor of shape {shape}")
+            return ctypes.c_void_p(a.data_ptr())
+        if a.dtype != self.np_complex or a.shape != shape or not a.flags.c_contiguous:
+            raise ValueError(f"expected C-contiguous {self.np_complex} array of shape {shape}")
+        if writable and not a.flags.writeable:
+            raise ValueError("output array is read-only")
+        return ctypes.c_void_p(a.ctypes.data)
+
+    def wd_apply_host(self, U_host, psi_host, kappa, dagger=False, out=None):
+        V = self.volume
+        out = np.empty((V, 4, 3), dtype=self.np_complex) if out is None else out
+        up = self._host_ptr(U_host, (V, 4, 3, 3)) if U_host is not None else None
+        self._check(self.lib.wd_apply_host(self._ctx, up, self._host_ptr(psi_host, (V, 4, 3)),
+                                           self._host_ptr(out, (V, 4, 3), True), float(kappa), int(bool(dagger))))
+        return out
+
+    def cg_solve_host(self, U_host, eta_host, kappa, r_min, max_iter, out=None):
+        V = self.volume
+        out = np.empty((V, 4, 3), dtype=self.np_complex) if out is None else out
+        up = self._host_ptr(U_host, (V, 4, 3, 3)) if U_host is not None else None
+        info = WdCgInfo()
+        rc = self.lib.cg_solve_host(self._ctx, up, self._host_ptr(eta_host, (V, 4, 3)),
+                                    self._host_ptr(out, (V, 4, 3), True), float(kappa), float(r_min),
+                                    int(max_iter), ctypes.byref(info))
+        self._check(rc, allow_not_converged=True)
+        d = info.as_dict()
+        d["status"] = rc
+        return out, d
+
+    # -- tuning knobs
+    def wd_set_tile(self, index):
+        self._check(self.lib.wd_set_tile(self._ctx, int(index)))
+
+    def wd_get_tile(self):
+        return int(self.lib.wd_get_tile(self._ctx))
+
+    def wd_set_poll_interval(self, n):
+        self._check(self.lib.wd_set_poll_interval(self._ctx, int(n)))

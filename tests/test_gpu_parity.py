@@ -1,0 +1,358 @@
+"""-m gpu parity tests: the CUDA path, called through the C ABI (ctypes binding), against the fp64
+CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star; readings G15, G16, G18 in DESIGN.md):
+  * wd_apply: max over sites of |out_gpu(x) - out_ref(x)|_2 / |out_ref(x)|_2  <= 1e-5 (fp32), 1e-12 (fp64);
+  * cg_solve: iteration count within +-2 % of the oracle's, final TRUE residual |eta - D psi|/|eta|
+    (evaluated by the oracle's fp64 D) within a factor 2 of the oracle's;
+  * pack / unpack are permutations: bit-exact.
+For fp32 runs the oracle consumes the fp32-rounded inputs promoted to fp64, so both sides see the
+identical operator and source.
+"""
+import ctypes
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_2111_14958_b200 import inputs
+import gpu_util as gu
+import lattice_math as lm
+
+pytestmark = pytest.mark.gpu
+
+TOL_APPLY = {32: 1e-5, 64: 1e-12}
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+CFG_TEST = 700
+
+
+@pytest.fixture(scope="module")
+def wilson():
+    import torch
+
+    assert torch.cuda.is_available(), "the -m gpu tests need a CUDA device"
+    from paper_2111_14958_b200 import build as wbuild
+    from paper_2111_14958_b200 import wilson as w
+
+    wbuild.build()
+    w.load_library()
+    return w
+
+
+def iters_close(a, b):
+    return abs(a - b) <= max(0.02 * b, 0.0) + 1e-9 or abs(a - b) <= math.floor(0.02 * b + 0.5)
+
+
+# ---------------------------------------------------------------- a0: layouts
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 10, 8), (14, 14, 14, 14)])
+def test_pack_unpack_are_exact_permutations(wilson, precision, dims):
+    V = int(np.prod(dims))
+    cdt = gu.np_complex(precision)
+    rdt = np.float32 if precision == 32 else np.float64
+    psi = inputs.source_field(CFG_TEST, dims, dtype=cdt, field=inputs.FIELD_AUX)
+    U = inputs.gauge_field(CFG_TEST, dims, "haar", dtype=cdt)
+    with wilson.WilsonContext(dims, precision) as ctx:
+        pn = ctx.wd_pack_spinor(gu.to_device(psi))
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        back = gu.to_host(ctx.wd_unpack_spinor(pn))
+        pn_h, Un_h = gu.to_host(pn), gu.to_host(Un)
+    assert back.tobytes() == psi.tobytes()
+    # native spinor: NSP planes of 128-bit vectors, plane stride V (include/wilson_cg.h)
+    nsp, w = (6, 4) if precision == 32 else (12, 2)
+    want = psi.view(rdt).reshape(V, nsp, w).transpose(1, 0, 2)
+    assert pn_h.reshape(nsp, V, w).tobytes() == np.ascontiguousarray(want).tobytes()
+    # native gauge: plane mu*9 + a*3+b of one complex, plane stride V
+    want_u = U.view(rdt).reshape(V, 36, 2).transpose(1, 0, 2)
+    assert Un_h.reshape(36, V, 2).tobytes() == np.ascontiguousarray(want_u).tobytes()
+
+
+# ---------------------------------------------------------------- a7: wd_apply
+def _apply_case(wilson, oracle, dims, links, kappa, precision, bc_t, cfg_seed, tile=None):
+    cdt = gu.np_complex(precision)
+    U = inputs.gauge_field(cfg_seed, dims, links, dtype=cdt)
+    psi = inputs.source_field(cfg_seed, dims, dtype=cdt, field=inputs.FIELD_AUX)
+    worst = 0.0
+    with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+        if tile is not None:
+            ctx.wd_set_tile(tile)
+        for dagger in (False, True):
+            got = gu.apply_on_gpu(ctx, U, psi, kappa, dagger)
+            want = oracle.wd_apply(dims, U.astype(np.complex128), psi.astype(np.complex128), kappa, dagger, bc_t)
+            site, glob = lm.per_site_rel_err(got, want)
+            assert site <= TOL_APPLY[precision], (dims, precision, dagger, bc_t, tile, site, glob)
+            worst = max(worst, site)
+    return worst
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("cfg_index", [0, 1, 2])
+def test_wd_apply_baseline_configs(wilson, oracle, cfg_index, precision):
+    cfg = inputs.CONFIGS[cfg_index]
+    _apply_case(wilson, oracle, cfg.dims, cfg.links, cfg.kappa, precision, cfg.bc_t, cfg.index)
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("bc_t", [-1, 1])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 10, 8), (5, 7, 4, 6), (18, 4, 6, 4), (4, 4, 4, 34)])
+def test_wd_apply_ragged_and_anisotropic(wilson, oracle, dims, bc_t, precision):
+    """extents that are not multiples of any tile edge, all four extents different, both boundary conditions"""
+    _apply_case(wilson, oracle, dims, "haar", 0.12, precision, bc_t, CFG_TEST + 1)
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_every_tile_shape(wilson, oracle, precision):
+    n = len(wilson.tile_shapes())
+    ran = 0
+    for tile in range(n):
+        for dims in [(14, 14, 14, 14), (16, 8, 8, 4)]:
+            try:
+                _apply_case(wilson, oracle, dims, "haar", 0.12, precision, -1, CFG_TEST + 2, tile=tile)
+                ran += 1
+            except wilson.WilsonError as e:
+                assert precision == 64 and e.code == -1  # large tiles are fp32-only
+    assert ran >= 8
+
+
+def test_wd_apply_free_field_plane_wave(wilson):
+    """closed form, no oracle: D on a plane wave in the free field (pin P3) at a volume spanning many tiles"""
+    dims, kappa = (16, 12, 8, 20), 0.124
+    U = inputs.gauge_field(0, dims, "unit")
+    n = np.array([3, 5, 1, 7])
+    p = lm.momenta(dims, n, -1)
+    u = inputs.complex_gaussian(inputs.slice_rng(CFG_TEST, inputs.FIELD_AUX, 0), (4, 3))
+    psi = lm.plane_wave(dims, p, u)
+    want = np.einsum("ij,xja->xia", lm.free_dirac_symbol(p, kappa), psi)
+    want_dag = np.einsum("ij,xja->xia", lm.free_dirac_symbol(p, kappa).conj().T, psi)
+    with wilson.WilsonContext(dims, 64) as ctx:
+        assert lm.per_site_rel_err(gu.apply_on_gpu(ctx, U, psi, kappa, False), want)[0] < 1e-12
+        assert lm.per_site_rel_err(gu.apply_on_gpu(ctx, U, psi, kappa, True), want_dag)[0] < 1e-12
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_wd_apply_32_4_sampled_sites(wilson, oracle, precision):
+    """BASELINE config 3 at full size, bench launch configuration; the oracle evaluates sampled sites one by one"""
+    cfg = inputs.CONFIGS[3]
+    U, psi = gu.config_fields(3, precision)
+    V = cfg.volume
+    rng = np.random.Generator(np.random.PCG64(5))
+    lx, ly, lz, lt = cfg.dims
+    edge = [0, lx - 1, lx, V - 1, V - lx, lx * ly * lz * (lt - 1), lx * ly * lz - 1, lx * ly - 1]
+    sites = np.unique(np.concatenate([edge, rng.choice(V, 4000, replace=False)])).astype(np.int64)
+    U64, psi64 = U.astype(np.complex128), psi.astype(np.complex128)
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        for dagger in (False, True):
+            got = gu.apply_on_gpu(ctx, U, psi, cfg.kappa, dagger)[sites]
+            want = oracle.wd_apply_sites(cfg.dims, U64, psi64, cfg.kappa, sites, dagger, cfg.bc_t)
+            assert lm.per_site_rel_err(got, want)[0] <= TOL_APPLY[precision]
+
+
+# ---------------------------------------------------------------- reductions
+@pytest.mark.parametrize("precision", [32, 64])
+def test_norm2_matches_oracle_and_is_deterministic(wilson, oracle, precision):
+    dims = (14, 14, 14, 14)
+    a = inputs.source_field(CFG_TEST + 3, dims, dtype=gu.np_complex(precision))
+    with wilson.WilsonContext(dims, precision) as ctx:
+        an = ctx.wd_pack_spinor(gu.to_device(a))
+        got = [ctx.wd_norm2(an) for _ in range(3)]
+    want = oracle.norm2(a.astype(np.complex128))
+    assert got[0] == got[1] == got[2]
+    assert abs(got[0] - want) <= (1e-6 if precision == 32 else 1e-13) * want
+    assert abs(want / (2 * 12 * np.prod(dims)) - 1) < 0.01  # pin P9: re, im each N(0,1)
+
+
+# ---------------------------------------------------------------- a1-a6: cg_solve
+def _cg_case(wilson, oracle, cfg, precision, r_min, poll=None):
+    U, eta = gu.config_fields(cfg.index, precision)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        if poll:
+            ctx.wd_set_poll_interval(poll)
+        psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, r_min, cfg.max_iter)
+        hist = ctx.wd_cg_history()
+    psi_o, info_o = oracle.cg_solve(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t, history=True)
+    res_gpu = oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
+    res_orc = oracle.true_residual(cfg.dims, U64, eta64, psi_o, cfg.kappa, cfg.bc_t)
+    assert info["status"] == 0 and info["converged"] == 1 and info_o["converged"]
+    assert iters_close(info["iterations"], info_o["iterations"]), (info["iterations"], info_o["iterations"])
+    assert res_gpu <= 2.0 * res_orc, (res_gpu, res_orc)
+    assert res_gpu < 2.0 * r_min
+    # the device-side record of the recursed residual follows the oracle's history
+    n = min(len(hist), len(info_o["rr_history"]))
+    assert len(hist) == info["iterations"] + 1
+    rel = np.abs(hist[:n] - info_o["rr_history"][:n]) / info_o["rr_history"][:n]
+    assert rel[0] < (1e-6 if precision == 32 else 1e-13)
+    assert np.max(rel[: max(2, n // 2)]) < (2e-2 if precision == 32 else 1e-6)
+    # solutions agree to what the tolerance allows: |dpsi| <= |D^-1| (|r_gpu| + |r_orc|)
+    diff = np.linalg.norm(psi - psi_o) / np.linalg.norm(psi_o)
+    assert diff < 4.0 * r_min / (1.0 - 8.0 * cfg.kappa) * (1 + 8 * cfg.kappa)
+    return info, info_o, res_gpu, res_orc
+
+
+@pytest.mark.parametrize("cfg_index", [0, 1, 2])
+def test_cg_solve_fp32_baseline_configs(wilson, oracle, cfg_index):
+    cfg = inputs.CONFIGS[cfg_index]
+    _cg_case(wilson, oracle, cfg, 32, cfg.r_min)
+
+
+@pytest.mark.parametrize("cfg_index", [0, 1, 2])
+def test_cg_solve_fp64_tight(wilson, oracle, cfg_index):
+    cfg = inputs.CONFIGS[cfg_index]
+    _cg_case(wilson, oracle, cfg, 64, 1e-10)
+
+
+def test_cg_result_independent_of_poll_interval_and_repeatable(wilson):
+    cfg = inputs.CONFIGS[1]
+    U, eta = gu.config_fields(1, 32)
+    outs = []
+    for poll in (1, 7, 32, 7):
+        with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+            ctx.wd_set_poll_interval(poll)
+            psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
+            outs.append((psi.tobytes(), info["iterations"], info["rel_residual"]))
+    assert all(o == outs[0] for o in outs)
+
+
+def test_cg_edge_cases(wilson, oracle):
+    cfg = inputs.CONFIGS[0]
+    U, eta = gu.config_fields(0, 64)
+    with wilson.WilsonContext(cfg.dims, 64, cfg.bc_t) as ctx:
+        # eta = 0: psi = 0, no iterations, OK
+        psi, info = gu.solve_on_gpu(ctx, U, np.zeros_like(eta), cfg.kappa, 1e-8, 100)
+        assert info["status"] == 0 and info["iterations"] == 0 and not psi.any()
+        # max_iter = 0: nothing iterated, psi = D-dagger 0 = 0, not converged
+        psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, 1e-8, 0)
+        assert info["status"] == 1 and info["iterations"] == 0 and not psi.any()
+        # max_iter reached: exactly the oracle's iterate after 5 loop bodies
+        psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, 1e-12, 5)
+        psi_o, info_o = oracle.cg_solve(cfg.dims, U, eta, cfg.kappa, 1e-12, 5, cfg.bc_t)
+        assert info["status"] == 1 and info["converged"] == 0 and info["iterations"] == 5 == info_o["iterations"]
+        assert np.linalg.norm(psi - psi_o) / np.linalg.norm(psi_o) < 1e-12
+        assert abs(info["rel_residual"] - info_o["rel_residual"]) < 1e-12 * info_o["rel_residual"] + 1e-15
+        # kappa = 0: D = 1, one iteration, psi = eta (pin P7)
+        psi, info = gu.solve_on_gpu(ctx, U, eta, 0.0, 1e-12, 10)
+        assert info["iterations"] == 1 and np.max(np.abs(psi - eta)) < 1e-14
+        # r_min >= 1: the loop condition fails at once
+        psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, 1.5, 10)
+        assert info["status"] == 0 and info["iterations"] == 0
+
+
+def test_cg_free_field_finite_termination(wilson):
+    """pin P8: K plane waves with distinct |D(p)|^2 terminate after exactly K iterations, exact solution known"""
+    dims, kappa = (8, 8, 8, 8), 0.12
+    U = inputs.gauge_field(0, dims, "unit")
+    rng = inputs.slice_rng(CFG_TEST + 4, inputs.FIELD_AUX, 0)
+    eta = np.zeros((int(np.prod(dims)), 4, 3), dtype=np.complex128)
+    want = np.zeros_like(eta)
+    modes = [(0, 0, 0, 0), (1, 2, 0, 3), (3, 1, 2, 1)]
+    for n in modes:
+        p = lm.momenta(dims, np.array(n), -1)
+        u = inputs.complex_gaussian(rng, (4, 3))
+        eta += lm.plane_wave(dims, p, u)
+        want += lm.plane_wave(dims, p, lm.free_dirac_inverse(p, kappa) @ u)
+    with wilson.WilsonContext(dims, 64) as ctx:
+        psi, info = gu.solve_on_gpu(ctx, U, eta, kappa, 1e-11, 50)
+    assert info["iterations"] == len(modes)
+    assert np.linalg.norm(psi - want) / np.linalg.norm(want) < 1e-10
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_cg_point_source_closed_form_32_4(wilson, precision):
+    """T3 / pin P8 at BASELINE volume 32^4, no oracle CG needed: pure-gauge links U = g(x) g(x+mu)^dagger
+    (every link non-trivial) and a point source; the exact solution is g(x) times the free propagator (FFT)."""
+    dims, kappa = (32, 32, 32, 32), 0.12
+    V = int(np.prod(dims))
+    g = inputs.gauge_transform_field(CFG_TEST + 5, dims)
+    U = lm.pure_gauge_links(dims, g)
+    x0 = (3, 31, 0, 17)
+    s0 = int(lm.site_index(dims, np.array(x0)))
+    u = inputs.complex_gaussian(inputs.slice_rng(CFG_TEST + 5, inputs.FIELD_AUX, 0), (4, 3))
+    eta = np.zeros((V, 4, 3), dtype=np.complex128)
+    eta[s0] = u
+    # D[U] psi = eta  <=>  D_free (g^-1 psi) = g^-1 eta
+    free = lm.free_point_propagator(dims, kappa, x0, np.einsum("ba,ib->ia", np.conj(g[s0]), u), -1)
+    want = np.einsum("xab,xib->xia", g, free)
+    cdt = gu.np_complex(precision)
+    tol = 1e-6 if precision == 32 else 1e-11
+    with wilson.WilsonContext(dims, precision) as ctx:
+        psi, info = gu.solve_on_gpu(ctx, U.astype(cdt), eta.astype(cdt), kappa, tol, 2000)
+    assert info["status"] == 0
+    err = np.linalg.norm(psi - want) / np.linalg.norm(want)
+    assert err < (2e-5 if precision == 32 else 1e-9), err
+
+
+def _golden(name):
+    path = os.path.join(GOLDEN, name)
+    if not os.path.exists(path):
+        pytest.skip(f"{name} not generated yet (tests/golden/make_golden.py)")
+    with open(path) as f:
+        return json.load(f)
+
+
+@pytest.mark.parametrize("cfg_index,precision", [(3, 32), (3, 64), (4, 32)])
+def test_cg_large_configs_against_stored_oracle(wilson, oracle, cfg_index, precision):
+    """BASELINE configs 3 and 4 at full size.  The oracle's CG takes minutes to an hour there, so its result
+    is stored by tests/golden/make_golden.py (oracle only); the true residual of the GPU solution is still
+    evaluated live by the oracle's fp64 D on the full lattice."""
+    gold = _golden(f"cg_config{cfg_index}_fp{precision}.json")
+    cfg = inputs.CONFIGS[cfg_index]
+    U, eta = gu.config_fields(cfg_index, precision)
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, gold["r_min"], cfg.max_iter)
+        hist = ctx.wd_cg_history()
+    assert info["status"] == 0
+    assert iters_close(info["iterations"], gold["iterations"]), (info["iterations"], gold["iterations"])
+    assert abs(info["eta_norm2"] - gold["eta_norm2"]) < (1e-6 if precision == 32 else 1e-12) * gold["eta_norm2"]
+    res = oracle.true_residual(cfg.dims, U.astype(np.complex128), eta.astype(np.complex128),
+                               psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
+    assert res <= 2.0 * gold["true_residual"], (res, gold["true_residual"])
+    sites = np.array(gold["sample_sites"])
+    want = (np.array(gold["psi_samples_re"]) + 1j * np.array(gold["psi_samples_im"])).reshape(-1, 4, 3)
+    diff = np.linalg.norm(psi[sites] - want) / np.linalg.norm(want)
+    assert diff < 4.0 * gold["r_min"] / (1.0 - 8.0 * cfg.kappa) * (1 + 8 * cfg.kappa), diff
+    n = min(len(hist), len(gold["rr_history"])) // 2
+    gh = np.array(gold["rr_history"][:n])
+    assert np.max(np.abs(hist[:n] - gh) / gh) < (5e-2 if precision == 32 else 1e-5)
+
+
+# ---------------------------------------------------------------- host-buffer forms and errors
+@pytest.mark.parametrize("precision", [32, 64])
+def test_host_forms_equal_device_forms(wilson, precision):
+    cfg = inputs.CONFIGS[1]
+    U, eta = gu.config_fields(1, precision)
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        psi_d, info_d = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
+        psi_h, info_h = ctx.cg_solve_host(U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
+        assert psi_h.tobytes() == psi_d.tobytes() and info_h["iterations"] == info_d["iterations"]
+        assert info_h["total_ms"] >= info_h["gpu_ms"] > 0 and info_h["kernel_launches"] >= 3 * info_h["iterations"]
+        out_d = gu.apply_on_gpu(ctx, U, eta, cfg.kappa, True)
+        out_h = ctx.wd_apply_host(None, eta, cfg.kappa, True)  # reuses the cached gauge field
+        assert out_h.tobytes() == out_d.tobytes()
+
+
+def test_error_codes(wilson):
+    cfg = inputs.CONFIGS[0]
+    U, eta = gu.config_fields(0, 32)
+    with wilson.WilsonContext(cfg.dims, 32) as ctx:
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        en = ctx.wd_pack_spinor(gu.to_device(eta))
+        with pytest.raises(wilson.WilsonError) as e:
+            ctx.wd_apply(Un, en, cfg.kappa, False, out=en)  # out aliases psi
+        assert e.value.code == -1
+        with pytest.raises(wilson.WilsonError):
+            ctx.wd_apply(Un, en, float("nan"), False)
+        with pytest.raises(wilson.WilsonError):
+            ctx.cg_solve(Un, en, cfg.kappa, 0.0, 10)
+        with pytest.raises(wilson.WilsonError):
+            ctx.cg_solve(Un, en, cfg.kappa, 1e-6, -1)
+        with pytest.raises(wilson.WilsonError):
+            ctx.wd_set_tile(99)
+        assert ctx.lib.wd_apply(ctx._ctx, None, None, None, 0.1, 0) == -1
+        assert b"wd_apply" in ctx.lib.wd_last_error(ctx._ctx)
+        # the ctx is still usable after errors
+        assert ctx.wd_norm2(en) > 0
+    with pytest.raises(wilson.WilsonError) as e:
+        wilson.WilsonContext((4, 4, 3, 4))
+    assert e.value.code == -2
