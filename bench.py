@@ -1,0 +1,313 @@
+#!/usr/bin/env python
+"""bench.py — the measurement contract of this repo.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--precision 32|64] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over one synthetic lattice: cg_solve (a1 init, the fused CG
+loop a2-a5 until |r|/|eta| < r_min, a6 final D-dagger) on BASELINE.json's config I (default 4: 48^3x96,
+the paper's quoted production volume, and the largest single-GPU config).  The metric is
+BASELINE.json's: Wilson D D-dagger CG GFLOP/s with the fixed flop convention (2976 flop/site/iteration +
+1368 flop/site for the final D-dagger), plus the achieved fraction of the HBM roofline of the dominant
+kernel.  Inputs are seeded and synthetic (paper_2111_14958_b200/inputs.py); they stand in for the paper's
+unspecified gauge fields.
+
+`value`   : device-resident inputs (native layout already in HBM), CUDA events around K steps.
+`e2e`     : the same solve through the C-ABI host-buffer call cg_solve_host (pinned HOST canonical
+            buffers; H2D copies of U and eta, pack, solve, unpack and the D2H copy of psi inside the timed region).
+`roofline`: the dominant kernel (a3: D pass + fused r update + |r|^2, 576 B/site fp32) timed live with CUDA
+            events around each of its launches inside the timed steps (wd_set_profile).
+`cpu_baseline`: the fp64 CPU oracle, as it stands, on a bounded sample (max_iter = 2) of the same workload.
+
+N > 1 (torchrun): the path does not shard (north_star: one GPU, no collectives) -> N independent replicas
+("replicas only"); value = total flops of all ranks / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2111_14958_b200 import inputs  # noqa: E402
+
+FLOP_ITER = 2976        # per site per CG iteration (reading G14)
+FLOP_APPLY = 1368       # per site per D / D-dagger application
+BYTES_A3 = {32: 576, 64: 1152}     # a3: read q, U, r; write r
+BYTES_ITER = {32: 1536, 64: 3072}  # a2 + a3 + a4
+METRIC = "Wilson DD-dagger CG GFLOP/s (fp32, 1 B200; roofline = achieved HBM GB/s fraction)"
+
+
+def cg_flops(volume, iterations):
+    return float(volume) * (FLOP_ITER * iterations + FLOP_APPLY)
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def stored_traffic(cfg_index, precision):
+    """dram bytes per launch of the a3 kernel from the committed ncu --set full capture, or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(f"config{cfg_index}_fp{precision}_a3")
+    except Exception:
+        return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML every 100 ms while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.samples, self.reasons, self.max_mhz = index, False, [], set(), None
+
+    def run(self):
+        try:
+            import pynvml as nv
+
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {
+                getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+                getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+                getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+                getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+                getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake",
+            }
+            while not self.stop_flag:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                try:
+                    mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                    for bit, name in names.items():
+                        if mask & bit:
+                            self.reasons.add(name)
+                except Exception:
+                    pass
+                time.sleep(0.1)
+        except Exception as e:  # NVML missing: report that rather than fail the bench
+            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+
+    def result(self):
+        self.stop_flag = True
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_sample(cfg, precision, U, eta, sample_iters):
+    """The oracle, as it stands, on a bounded sample: `sample_iters` CG iterations + the final D-dagger."""
+    from oracle import wilson_oracle
+
+    U64 = U.astype(np.complex128)
+    eta64 = eta.astype(np.complex128)
+    t0 = time.perf_counter()
+    _, info = wilson_oracle.cg_solve(cfg.dims, U64, eta64, cfg.kappa, 1e-30, sample_iters, cfg.bc_t)
+    dt = time.perf_counter() - t0
+    gflops = cg_flops(cfg.volume, info["iterations"]) / dt / 1e9
+    return gflops, dt, wilson_oracle.num_threads(), info["iterations"]
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle on the host cores, each step a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    sample_iters = args.sample_iters
+    U, eta = inputs.config_inputs(cfg, dtype=np.complex64 if args.precision == 32 else np.complex128)
+    times, cores, its = [], 1, sample_iters
+    for i in range(args.warmup + args.steps):
+        gf, dt, cores, its = oracle_sample(cfg, args.precision, U, eta, sample_iters)
+        if i >= args.warmup:
+            times.append(dt)
+    t = float(np.mean(times))
+    value = cg_flops(cfg.volume, its) / t / 1e9
+    sample = f"{its} CG iterations + final D-dagger of config {cfg.index} ({cfg.name}), fp64 oracle, full lattice"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config{cfg.index}: {cfg.name} Wilson CG, kappa={cfg.kappa}, links={cfg.links}",
+                   "precision": args.precision},
+        "cpu_baseline": {"value": value, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json configs index (default 4: 48^3x96)")
+    ap.add_argument("--precision", type=int, default=32, choices=[32, 64])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--tile", type=int, default=-1, help="CTA tile index (-1 = library's automatic choice)")
+    ap.add_argument("--sample-iters", type=int, default=2, help="CG iterations of the oracle's bounded sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    cfg = inputs.CONFIGS[args.config]
+    r_min = cfg.r_min if args.precision == 32 else 1e-10
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+
+    import torch
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_2111_14958_b200 import build as wbuild
+    from paper_2111_14958_b200 import wilson
+
+    if rank == 0:
+        wbuild.build()
+    if dist:
+        dist.barrier()
+    wilson.load_library()
+
+    cdt = np.complex64 if args.precision == 32 else np.complex128
+    U, eta = inputs.config_inputs(cfg, dtype=cdt)   # seeded, identical on every rank (replicas)
+    V = cfg.volume
+    ctx = wilson.WilsonContext(cfg.dims, args.precision, cfg.bc_t)
+    if args.tile >= 0:
+        ctx.wd_set_tile(args.tile)
+    U_dev = torch.from_numpy(U).cuda()
+    Un = ctx.wd_pack_gauge(U_dev)
+    del U_dev
+    eta_dev = torch.from_numpy(eta).cuda()
+    en = ctx.wd_pack_spinor(eta_dev)
+    del eta_dev
+    psi_n = ctx.empty_spinor()
+    torch.cuda.synchronize()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---------------- device-resident arm
+    for _ in range(args.warmup):
+        ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=psi_n)
+    ctx.wd_set_profile(True)
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches, iters = 0, 0
+    e0.record()
+    for _ in range(args.steps):
+        _, info = ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=psi_n)
+        launches += info["kernel_launches"]
+        iters = info["iterations"]
+    e1.record()
+    barrier()
+    clocks = sampler.result()
+    ms_total = e0.elapsed_time(e1)
+    prof = ctx.wd_get_profile()
+    ctx.wd_set_profile(False)
+    if dist:
+        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * cg_flops(V, iters) / (ms_step * 1e-3) / 1e9
+
+    # ---------------- roofline of the dominant kernel (a3), timed live inside the steps above
+    peak, peak_src = measured_peak()
+    a3_ms = prof["a3_ms"] / max(prof["iterations"], 1)
+    a3_bytes = BYTES_A3[args.precision] * V
+    achieved = a3_bytes / (a3_ms * 1e-3) / 1e9 if a3_ms > 0 else None
+    iter_ms = (prof["a2_ms"] + prof["a3_ms"] + prof["a4_ms"]) / max(prof["iterations"], 1)
+    roofline = {
+        "bound": "hbm", "kernel": "dslash_kernel<MODE_RUPD> (a3: D pass + r update + |r|^2)",
+        "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak if achieved else None,
+        "peak_source": peak_src, "traffic": stored_traffic(cfg.index, args.precision),
+        "algorithmic_bytes_per_launch": a3_bytes, "avg_launch_ms": a3_ms,
+        "per_kernel_ms": {"a2": prof["a2_ms"] / max(prof["iterations"], 1), "a3": a3_ms,
+                          "a4": prof["a4_ms"] / max(prof["iterations"], 1)},
+        "cg_iteration": {"achieved": BYTES_ITER[args.precision] * V / (iter_ms * 1e-3) / 1e9 if iter_ms > 0 else None,
+                         "frac": BYTES_ITER[args.precision] * V / (iter_ms * 1e-3) / 1e9 / peak if iter_ms > 0 else None,
+                         "frac_of_8TBs": BYTES_ITER[args.precision] * V / (iter_ms * 1e-3) / 1e9 / 8000.0 if iter_ms > 0 else None,
+                         "bytes_per_site": BYTES_ITER[args.precision], "ms": iter_ms},
+    }
+
+    # ---------------- end to end through the host-buffer C-ABI call
+    e2e = None
+    if not args.no_e2e:
+        U_pin = torch.from_numpy(U).pin_memory()
+        eta_pin = torch.from_numpy(eta).pin_memory()
+        psi_pin = torch.empty((V, 4, 3), dtype=torch.complex64 if args.precision == 32 else torch.complex128).pin_memory()
+        ctx.cg_solve_host(U_pin, eta_pin, cfg.kappa, r_min, cfg.max_iter, out=psi_pin)  # warm-up (allocates staging)
+        barrier()
+        t0 = time.perf_counter()
+        n_e2e = max(1, min(args.steps, 3))
+        for _ in range(n_e2e):
+            _, info_h = ctx.cg_solve_host(U_pin, eta_pin, cfg.kappa, r_min, cfg.max_iter, out=psi_pin)
+        barrier()
+        dt = (time.perf_counter() - t0) / n_e2e
+        if dist:
+            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * cg_flops(V, info_h["iterations"]) / dt / 1e9, "unit": "GFLOP/s",
+               "h2d_bytes_per_step": int(U.nbytes + eta.nbytes), "d2h_bytes_per_step": int(eta.nbytes),
+               "ms_per_step": dt * 1e3, "steps": n_e2e}
+        del U_pin, eta_pin, psi_pin
+
+    # ---------------- the oracle on the host cores (rank 0, N = 1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        gf, dt, cores, its = oracle_sample(cfg, args.precision, U, eta, args.sample_iters)
+        cpu = {"value": gf, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "seconds": dt,
+               "sample": f"{its} CG iterations + final D-dagger of config {cfg.index} ({cfg.name}), fp64 oracle, full lattice"}
+
+    ws_bytes = (72 + 24 * 6) * V * (4 if args.precision == 32 else 8)
+    line = {
+        "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32" if args.precision == 32 else "f64", "data": "synthetic",
+        "config": {"workload": f"config{cfg.index}: {cfg.name} Wilson CG on D D-dagger, kappa={cfg.kappa}, "
+                               f"links={cfg.links}, r_min={r_min:g}, antiperiodic t",
+                   "volume": V, "cg_iterations": iters, "tile": list(wilson.tile_shapes()[ctx.wd_get_tile()]),
+                   "l2_policy": f"inputs larger than L2 (working set {ws_bytes / 1e6:.0f} MB vs 126 MB L2)"
+                   if ws_bytes > 2 * 126e6 else "working set fits L2 (latency-bound regime, no roofline claim)",
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+    }
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if dist:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -167,17 +167,33 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
 
 /*
  * Tuning knobs (the paper's workgroup-size tuning):
- *   wd_num_tiles()            number of compiled CTA tile shapes.
+ *   wd_num_tiles()            number of compiled stencil launch configurations ("tiles").
  *   wd_tile_shape(i, shape)   writes {BX,BY,BZ,BT} of tile i (threads per CTA = product); returns 0 or WD_ERR_ARG.
+ *   wd_tile_info(i, info)     writes {min resident CTAs per SM asked of the compiler, 1 if the hop loop is
+ *                             software-pipelined, 1 if also compiled for precision 64}.
  *   wd_set_tile(ctx, i)       select tile i for the stencil kernels of this ctx; i = -1 restores the automatic choice.
  *   wd_get_tile(ctx)          index in use.
+ *   wd_set_zchunk(ctx, layers)    z extent (in sites) of one chunk of the CTA rasterisation x,y,z-in-chunk,t,z-chunk that
+ *                             keeps the +-t neighbours of a tile in L2; 0 = automatic (fits a 40 MB reuse distance).
  *   wd_set_poll_interval(ctx, n)  CG iterations enqueued between two host polls of the device stop flag (n >= 1; 0 = automatic).
  */
 int wd_num_tiles(void);
 int wd_tile_shape(int index, int shape[4]);
+int wd_tile_info(int index, int info[3]);
 int wd_set_tile(wd_ctx *ctx, int index);
 int wd_get_tile(wd_ctx *ctx);
+int wd_set_zchunk(wd_ctx *ctx, int layers);
 int wd_set_poll_interval(wd_ctx *ctx, int n);
+
+/*
+ * Per-kernel timing of the CG loop (measurement aid).  With profiling on, cg_solve records
+ * CUDA events on the ctx stream around the three kernels of every iteration (a2: D-dagger pass + |q|^2,
+ * a3: D pass + r update + |r|^2, a4: axpy-xpay) and accumulates their device times.
+ *   wd_set_profile(ctx, on)            switch on/off and clear the accumulators.
+ *   wd_get_profile(ctx, ms, iters)     ms[0..2] = accumulated milliseconds of a2, a3, a4 over *iters iterations.
+ */
+int wd_set_profile(wd_ctx *ctx, int on);
+int wd_get_profile(wd_ctx *ctx, double ms[3], long *iterations);
 
 /* Library version string, e.g. "wilson_cg 0.1 sm_100a". */
 const char *wd_version(void);

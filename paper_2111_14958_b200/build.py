@@ -1,49 +1,60 @@
 """Build step of the C-ABI library: nvcc, sm_100a only, in-tree (paper_2111_14958_b200/libwilson_cg.so).
 
-`python -m paper_2111_14958_b200.build [--force]` or `__graft_entry__.build()`.  nvcc cross-compiles
-without a GPU.  The .so is git-ignored and travels to the GPU box with the gpurun snapshot.
+`python -m paper_2111_14958_b200.build [--force] [-v]` or `__graft_entry__.build()`.  nvcc cross-compiles
+without a GPU.  The translation units compile in parallel; objects and the .so are git-ignored and travel
+to the GPU box with the gpurun snapshot.
 """
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
+OBJDIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libwilson_cg.so")
-SOURCES = [os.path.join(CSRC, "wilson_cg.cu")]
-DEPENDS = SOURCES + [os.path.join(CSRC, "wilson_kernels.cuh"), os.path.join(ROOT, "include", "wilson_cg.h")]
+UNITS = ["wilson_cg.cu", "wilson_dslash_f32.cu", "wilson_dslash_f64.cu"]
+HEADERS = [os.path.join(CSRC, "wilson_kernels.cuh"), os.path.join(CSRC, "wilson_launch.cuh"),
+           os.path.join(ROOT, "include", "wilson_cg.h")]
 
-NVCC_FLAGS = [
-    "-std=c++17", "-O3", "-lineinfo",
-    "-gencode", "arch=compute_100a,code=sm_100a",
-    "--shared", "-Xcompiler", "-fPIC",
-    "--threads", "0",
-]
+ARCH_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a"]
+NVCC_FLAGS = ["-std=c++17", "-O3", "-lineinfo"] + ARCH_FLAGS + ["-Xcompiler", "-fPIC"]
 
 
 def nvcc_path() -> str:
-    for cand in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
-        if cand and (os.path.isabs(cand) and os.path.exists(cand) or not os.path.isabs(cand)):
-            return cand
-    return "nvcc"
+    cand = os.environ.get("NVCC") or "/usr/local/cuda/bin/nvcc"
+    return cand if os.path.exists(cand) else "nvcc"
 
 
-def is_stale() -> bool:
-    if not os.path.exists(LIB):
+def _stale(target, deps) -> bool:
+    if not os.path.exists(target):
         return True
-    t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(p) > t for p in DEPENDS)
+    t = os.path.getmtime(target)
+    return any(os.path.getmtime(p) > t for p in deps)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile libwilson_cg.so if missing or older than its sources.  Returns its path."""
-    if force or is_stale():
+    os.makedirs(OBJDIR, exist_ok=True)
+    objs, jobs = [], []
+    for unit in UNITS:
+        src = os.path.join(CSRC, unit)
+        obj = os.path.join(OBJDIR, unit.replace(".cu", ".o"))
+        objs.append(obj)
+        if force or _stale(obj, [src] + HEADERS):
+            cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+            jobs.append(cmd)
+    if jobs:
+        with ThreadPoolExecutor(len(jobs)) as pool:
+            for rc, cmd in zip(pool.map(lambda c: subprocess.run(c, cwd=CSRC).returncode, jobs), jobs):
+                if rc != 0:
+                    raise RuntimeError("nvcc failed: " + " ".join(cmd))
+    if jobs or force or _stale(LIB, objs):
         tmp = LIB + f".{os.getpid()}.tmp"
-        cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
-        subprocess.check_call(cmd, cwd=CSRC)
+        subprocess.check_call([nvcc_path()] + ARCH_FLAGS + ["--shared", "-o", tmp] + objs)
         os.replace(tmp, LIB)
     return LIB
 

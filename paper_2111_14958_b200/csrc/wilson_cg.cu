@@ -2,7 +2,7 @@
 // Every arithmetic step runs in the kernels of wilson_kernels.cuh; this file only sizes grids,
 // enqueues launches on the caller's stream and polls the device stop flag.
 #include "../../include/wilson_cg.h"
-#include "wilson_kernels.cuh"
+#include "wilson_launch.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -11,32 +11,6 @@
 #include <cstring>
 
 using namespace wd;
-
-// ---------------------------------------------------------------- tile table (the workgroup-size knob)
-// X(index, BX, BY, BZ, BT).  Tiles with more than 256 threads are compiled for fp32 only
-// (fp64 needs > 128 registers per thread).
-#define WD_TILES_SMALL(X) \
-    X(0, 8, 4, 4, 2)      \
-    X(1, 16, 4, 2, 2)     \
-    X(2, 32, 2, 2, 2)     \
-    X(3, 4, 4, 4, 4)      \
-    X(4, 16, 4, 4, 1)     \
-    X(5, 8, 4, 2, 2)      \
-    X(6, 16, 2, 2, 2)     \
-    X(7, 4, 4, 4, 2)
-#define WD_TILES_LARGE(X) \
-    X(8, 8, 4, 4, 4)      \
-    X(9, 16, 4, 4, 2)     \
-    X(10, 32, 4, 2, 2)    \
-    X(11, 16, 8, 2, 2)
-#define WD_NUM_TILES 12
-#define WD_NUM_TILES_SMALL 8
-
-static const int kTileShape[WD_NUM_TILES][4] = {
-#define X(i, a, b, c, d) {a, b, c, d},
-    WD_TILES_SMALL(X) WD_TILES_LARGE(X)
-#undef X
-};
 
 struct wd_ctx {
     int dims[4];
@@ -47,6 +21,8 @@ struct wd_ctx {
     int tile;       // tile index in use
     int tile_user;  // -1 = automatic
     int poll;       // 0 = automatic
+    int zchunk_user;      // z layers per rasterisation chunk, 0 = automatic
+    double l2_budget_mb;  // reuse-distance budget of the automatic choice
     int sm_count;
     // CG workspace (native layout), device
     void *r, *p, *q, *y;
@@ -64,6 +40,12 @@ struct wd_ctx {
     void *U_can, *U_nat, *s_can, *s_nat_in, *s_nat_out;
     int have_gauge;
     cudaEvent_t ev[4];
+    // per-kernel-class timing (wd_set_profile): 4 events per iteration of one poll chunk
+    int profile;
+    cudaEvent_t *pev;
+    int pev_cap;            // iterations the pool covers
+    double prof_ms[3];      // accumulated device time of a2, a3, a4
+    long prof_n;            // iterations accumulated
     int last_iters;
     int launches;
     char err[512];
@@ -90,48 +72,62 @@ static int fail(wd_ctx *ctx, int code, const char *fmt, ...)
     } while (0)
 
 static inline size_t real_bytes(const wd_ctx *c) { return c->precision == 32 ? 4 : 8; }
-static inline size_t spinor_bytes(const wd_ctx *c) { return (size_t)24 * c->V * real_bytes(c); }
-static inline size_t gauge_bytes(const wd_ctx *c) { return (size_t)72 * c->V * real_bytes(c); }
-static inline size_t spinor_vecs(const wd_ctx *c) { return (size_t)(c->precision == 32 ? 6 : 12) * c->V; }
+static inline size_t vpad(const wd_ctx *c) { return ((size_t)c->V + SB - 1) / SB * SB; }  // volume padded to whole site blocks
+static inline int padded(const wd_ctx *c) { return vpad(c) != (size_t)c->V; }
+static inline size_t spinor_bytes(const wd_ctx *c) { return (size_t)24 * vpad(c) * real_bytes(c); }       // native
+static inline size_t gauge_bytes(const wd_ctx *c) { return (size_t)72 * vpad(c) * real_bytes(c); }        // native
+static inline size_t spinor_can_bytes(const wd_ctx *c) { return (size_t)24 * c->V * real_bytes(c); }     // canonical
+static inline size_t gauge_can_bytes(const wd_ctx *c) { return (size_t)72 * c->V * real_bytes(c); }      // canonical
+static inline size_t spinor_vecs(const wd_ctx *c) { return (size_t)(c->precision == 32 ? 6 : 12) * vpad(c); }
 
 static Geom make_geom(const wd_ctx *c, int tile)
 {
     Geom g;
     for (int d = 0; d < 4; ++d) {
         g.L[d] = c->dims[d];
-        g.nt[d] = (c->dims[d] + kTileShape[tile][d] - 1) / kTileShape[tile][d];
+        g.nt[d] = (c->dims[d] + kTiles[tile].b[d] - 1) / kTiles[tile].b[d];
     }
     g.V = c->V;
     g.bc_t = c->bc_t;
+    // z chunk of the CTA rasterisation: the largest divisor of the z tile count whose t-reuse distance
+    // Lx*Ly*(zc*BZ)*BT sites * ~600 B (spinor in/out, gauge, halos) stays within the L2 budget.
+    const double layer = 600.0 * c->dims[0] * c->dims[1] * kTiles[tile].b[3];   // bytes per z layer of one t-tile row
+    const double budget = c->l2_budget_mb * 1.0e6;
+    int zc = 1;
+    if (c->zchunk_user > 0) {
+        zc = (c->zchunk_user + kTiles[tile].b[2] - 1) / kTiles[tile].b[2];
+        if (zc > g.nt[2]) zc = g.nt[2];
+    } else {
+        for (int d = 1; d <= g.nt[2]; ++d)
+            if (g.nt[2] % d == 0 && layer * d * kTiles[tile].b[2] <= budget) zc = d;
+    }
+    g.zc = zc;
     return g;
 }
 static long tile_blocks(const wd_ctx *c, int tile)
 {
     long n = 1;
-    for (int d = 0; d < 4; ++d) n *= (c->dims[d] + kTileShape[tile][d] - 1) / kTileShape[tile][d];
+    for (int d = 0; d < 4; ++d) n *= (c->dims[d] + kTiles[tile].b[d] - 1) / kTiles[tile].b[d];
     return n;
 }
 static int tile_threads(int tile)
 {
-    return kTileShape[tile][0] * kTileShape[tile][1] * kTileShape[tile][2] * kTileShape[tile][3];
+    return kTiles[tile].b[0] * kTiles[tile].b[1] * kTiles[tile].b[2] * kTiles[tile].b[3];
 }
 static bool tile_ok(const wd_ctx *c, int tile)
 {
     if (tile < 0 || tile >= WD_NUM_TILES) return false;
-    if (c->precision == 64 && tile >= WD_NUM_TILES_SMALL) return false;
+    if (c->precision == 64 && !kTiles[tile].f64) return false;
     return true;
 }
-// Automatic choice: least padded threads; ties go to the preferred order below.
+// Automatic choice: the first row of the table (rows are in order of measured preference) among those compiled
+// for this precision that waste the fewest threads on tiles overhanging the lattice.
 static int auto_tile(const wd_ctx *c)
 {
-    static const int pref32[] = {8, 9, 10, 11, 0, 1, 2, 3, 4, 5, 6, 7};
-    static const int pref64[] = {0, 1, 2, 3, 4, 5, 6, 7};
-    const int *pref = c->precision == 32 ? pref32 : pref64;
-    const int n = c->precision == 32 ? 12 : 8;
-    int best = pref[0];
+    int best = -1;
     double best_waste = 1e300;
-    for (int i = 0; i < n; ++i) {
-        const int t = pref[i];
+    for (int t = 0; t < WD_NUM_TILES; ++t) {
+        if (!tile_ok(c, t)) continue;
         const double waste = (double)tile_blocks(c, t) * tile_threads(t) / (double)c->V;
         if (waste < best_waste - 1e-12) { best_waste = waste; best = t; }
     }
@@ -139,42 +135,17 @@ static int auto_tile(const wd_ctx *c)
 }
 
 // ---------------------------------------------------------------- launches
-template <typename real, int DAG, int MODE>
-static cudaError_t launch_dslash_t(wd_ctx *c, int tile, const void *U, const void *in, void *out, double kappa,
-                                   void *r, int it)
-{
-    using svec = typename Field<real>::svec;
-    using gvec = typename Field<real>::gvec;
-    const Geom g = make_geom(c, tile);
-    const unsigned int grid = (unsigned int)tile_blocks(c, tile);
-#define X(i, a, b, cc, d)                                                                                     \
-    case i:                                                                                                   \
-        dslash_kernel<real, DAG, MODE, a, b, cc, d><<<grid, a * b * cc * d, 0, c->stream>>>(                  \
-            g, (const gvec *)U, (const svec *)in, (svec *)out, (real)kappa, (svec *)r, c->sc, c->partials,    \
-            c->counter, c->hist, it);                                                                         \
-        break;
-    if constexpr (sizeof(real) == 4) {
-        switch (tile) {
-            WD_TILES_SMALL(X)
-            WD_TILES_LARGE(X)
-            default: return cudaErrorInvalidValue;
-        }
-    } else {
-        switch (tile) {
-            WD_TILES_SMALL(X)
-            default: return cudaErrorInvalidValue;
-        }
-    }
-#undef X
-    c->launches++;
-    return cudaGetLastError();
-}
-
 template <int DAG, int MODE>
 static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void *out, double kappa, void *r, int it)
 {
-    if (c->precision == 32) return launch_dslash_t<float, DAG, MODE>(c, c->tile, U, in, out, kappa, r, it);
-    return launch_dslash_t<double, DAG, MODE>(c, c->tile, U, in, out, kappa, r, it);
+    DslashArgs a;
+    a.g = make_geom(c, c->tile);
+    a.grid = (unsigned int)tile_blocks(c, c->tile);
+    a.stream = c->stream;
+    a.U = U; a.in = in; a.out = out; a.kappa = kappa; a.r = r;
+    a.sc = c->sc; a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = it;
+    c->launches++;
+    return c->precision == 32 ? launch_dslash_f32(c->tile, DAG, MODE, a) : launch_dslash_f64(c->tile, DAG, MODE, a);
 }
 
 static unsigned int vec_grid(const wd_ctx *c, size_t n)
@@ -251,6 +222,7 @@ extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_
     c->sm_count = sms;
     c->tile_user = -1;
     c->tile = auto_tile(c);
+    c->l2_budget_mb = 40.0;
     bool ok = true;
     ok = ok && cudaMalloc(&c->sc, sizeof(CgScalars)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->counter, sizeof(unsigned int)) == cudaSuccess;
@@ -282,6 +254,8 @@ extern "C" int wd_destroy(wd_ctx *c)
     if (c->result_host) cudaFreeHost(c->result_host);
     for (int i = 0; i < 4; ++i)
         if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    for (int i = 0; i < 4 * c->pev_cap; ++i) cudaEventDestroy(c->pev[i]);
+    free(c->pev);
     free(c);
     return WD_OK;
 }
@@ -295,7 +269,13 @@ extern "C" int wd_num_tiles(void) { return WD_NUM_TILES; }
 extern "C" int wd_tile_shape(int index, int shape[4])
 {
     if (index < 0 || index >= WD_NUM_TILES || !shape) return WD_ERR_ARG;
-    for (int d = 0; d < 4; ++d) shape[d] = kTileShape[index][d];
+    for (int d = 0; d < 4; ++d) shape[d] = kTiles[index].b[d];
+    return WD_OK;
+}
+extern "C" int wd_tile_info(int index, int info[3])
+{
+    if (index < 0 || index >= WD_NUM_TILES || !info) return WD_ERR_ARG;
+    info[0] = kTiles[index].minb; info[1] = kTiles[index].pipe; info[2] = kTiles[index].f64;
     return WD_OK;
 }
 extern "C" int wd_set_tile(wd_ctx *c, int index)
@@ -312,10 +292,32 @@ extern "C" int wd_set_tile(wd_ctx *c, int index)
     return WD_OK;
 }
 extern "C" int wd_get_tile(wd_ctx *c) { return c ? c->tile : WD_ERR_ARG; }
+extern "C" int wd_set_zchunk(wd_ctx *c, int layers)
+{
+    if (!c || layers < 0) return WD_ERR_ARG;
+    c->zchunk_user = layers;
+    return WD_OK;
+}
 extern "C" int wd_set_poll_interval(wd_ctx *c, int n)
 {
     if (!c || n < 0) return WD_ERR_ARG;
     c->poll = n;
+    return WD_OK;
+}
+
+extern "C" int wd_set_profile(wd_ctx *c, int on)
+{
+    if (!c) return WD_ERR_ARG;
+    c->profile = on ? 1 : 0;
+    c->prof_ms[0] = c->prof_ms[1] = c->prof_ms[2] = 0.0;
+    c->prof_n = 0;
+    return WD_OK;
+}
+extern "C" int wd_get_profile(wd_ctx *c, double ms[3], long *iterations)
+{
+    if (!c || !ms || !iterations) return WD_ERR_ARG;
+    for (int j = 0; j < 3; ++j) ms[j] = c->prof_ms[j];
+    *iterations = c->prof_n;
     return WD_OK;
 }
 
@@ -324,11 +326,12 @@ extern "C" int wd_pack_gauge(wd_ctx *c, const void *can, void *nat)
 {
     if (!c) return WD_ERR_ARG;
     if (!can || !nat || can == nat) return fail(c, WD_ERR_ARG, "wd_pack_gauge: NULL or aliased argument");
-    const unsigned int grid = (c->V + VEC_NT - 1) / VEC_NT;
+    const int Vp = (int)vpad(c);
+    const unsigned int grid = (Vp + VEC_NT - 1) / VEC_NT;
     if (c->precision == 32)
-        pack_gauge_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float2 *)can, (float2 *)nat, c->V);
+        pack_gauge_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float2 *)can, (float2 *)nat, c->V, Vp);
     else
-        pack_gauge_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V);
+        pack_gauge_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V, Vp);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
     return WD_OK;
@@ -337,11 +340,12 @@ extern "C" int wd_pack_spinor(wd_ctx *c, const void *can, void *nat)
 {
     if (!c) return WD_ERR_ARG;
     if (!can || !nat || can == nat) return fail(c, WD_ERR_ARG, "wd_pack_spinor: NULL or aliased argument");
-    const unsigned int grid = (c->V + VEC_NT - 1) / VEC_NT;
+    const int Vp = (int)vpad(c);
+    const unsigned int grid = (Vp + VEC_NT - 1) / VEC_NT;
     if (c->precision == 32)
-        pack_spinor_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float4 *)can, (float4 *)nat, c->V);
+        pack_spinor_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float4 *)can, (float4 *)nat, c->V, Vp);
     else
-        pack_spinor_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V);
+        pack_spinor_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V, Vp);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
     return WD_OK;
@@ -379,9 +383,9 @@ extern "C" int wd_norm2(wd_ctx *c, const void *a, double *result)
     const size_t n = spinor_vecs(c);
     const unsigned int grid = vec_grid(c, n);
     if (c->precision == 32)
-        norm2_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float4 *)a, n, c->partials, c->counter, c->result_dev);
+        norm2_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float4 *)a, n, c->V, padded(c), c->partials, c->counter, c->result_dev);
     else
-        norm2_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)a, n, c->partials, c->counter, c->result_dev);
+        norm2_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)a, n, c->V, padded(c), c->partials, c->counter, c->result_dev);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
     CUDA_TRY(c, cudaMemcpyAsync(c->result_host, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -411,25 +415,35 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
     if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
     if (c->precision == 32)
         cg_init_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((const float4 *)eta, (float4 *)c->y, (float4 *)c->r,
-                                                               (float4 *)c->p, n, c->sc, c->partials, c->counter,
-                                                               c->hist, r_min, max_iter);
+                                                               (float4 *)c->p, n, c->V, padded(c), c->sc, c->partials,
+                                                               c->counter, c->hist, r_min, max_iter);
     else
         cg_init_kernel<double><<<vgrid, VEC_NT, 0, c->stream>>>((const double2 *)eta, (double2 *)c->y, (double2 *)c->r,
-                                                                (double2 *)c->p, n, c->sc, c->partials, c->counter,
-                                                                c->hist, r_min, max_iter);
+                                                                (double2 *)c->p, n, c->V, padded(c), c->sc, c->partials,
+                                                                c->counter, c->hist, r_min, max_iter);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
 
     const int poll = c->poll > 0 ? c->poll : auto_poll(c);
+    if (c->profile && c->pev_cap < poll) {
+        cudaEvent_t *pe = (cudaEvent_t *)realloc(c->pev, sizeof(cudaEvent_t) * 4 * (size_t)poll);
+        if (!pe) return fail(c, WD_ERR_ALLOC, "cg_solve: out of host memory");
+        c->pev = pe;
+        for (; c->pev_cap < poll; ++c->pev_cap)
+            for (int j = 0; j < 4; ++j) CUDA_TRY(c, cudaEventCreate(&c->pev[4 * c->pev_cap + j]));
+    }
     int launched = 0;
     while (launched < max_iter) {
         const int chunk = (max_iter - launched) < poll ? (max_iter - launched) : poll;
         for (int i = 0; i < chunk; ++i) {
             const int it = launched + i;
+            if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 0], c->stream));
             // a2: q = D-dagger p, qq, alpha
             CUDA_TRY(c, (launch_dslash<1, MODE_QQ>(c, U, c->p, c->q, kappa, nullptr, it)));
+            if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 1], c->stream));
             // a3: r -= alpha D q, rr', beta, loop condition
             CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it)));
+            if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 2], c->stream));
             // a4: y += alpha p ; p = r + beta p
             if (c->precision == 32)
                 cg_update_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((float4 *)c->y, (float4 *)c->p,
@@ -439,10 +453,22 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
                                                                            (const double2 *)c->r, n, c->sc, it);
             c->launches++;
             CUDA_TRY(c, cudaGetLastError());
+            if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 3], c->stream));
         }
-        launched += chunk;
         CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
         CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (c->profile) {
+            // only iterations that really ran (it < k_stop) count; over-launched ones are no-ops
+            for (int i = 0; i < chunk && launched + i < c->sc_host->k_stop; ++i) {
+                for (int j = 0; j < 3; ++j) {
+                    float ms = 0.f;
+                    CUDA_TRY(c, cudaEventElapsedTime(&ms, c->pev[4 * i + j], c->pev[4 * i + j + 1]));
+                    c->prof_ms[j] += ms;
+                }
+                c->prof_n++;
+            }
+        }
+        launched += chunk;
         if (c->sc_host->k_stop <= launched) break;  // the device loop condition failed (or eta = 0)
     }
     // a6: psi = D-dagger y ("then we multiply the solution by D-dagger")
@@ -505,9 +531,9 @@ extern "C" int wd_cg_history(wd_ctx *c, double *out, int n)
 // ---------------------------------------------------------------- host-buffer forms
 static int ensure_staging(wd_ctx *c)
 {
-    if (!c->U_can) CUDA_TRY(c, cudaMalloc(&c->U_can, gauge_bytes(c)));
+    if (!c->U_can) CUDA_TRY(c, cudaMalloc(&c->U_can, gauge_can_bytes(c)));
     if (!c->U_nat) CUDA_TRY(c, cudaMalloc(&c->U_nat, gauge_bytes(c)));
-    if (!c->s_can) CUDA_TRY(c, cudaMalloc(&c->s_can, spinor_bytes(c)));
+    if (!c->s_can) CUDA_TRY(c, cudaMalloc(&c->s_can, spinor_can_bytes(c)));
     if (!c->s_nat_in) CUDA_TRY(c, cudaMalloc(&c->s_nat_in, spinor_bytes(c)));
     if (!c->s_nat_out) CUDA_TRY(c, cudaMalloc(&c->s_nat_out, spinor_bytes(c)));
     return WD_OK;
@@ -518,12 +544,12 @@ static int stage_inputs(wd_ctx *c, const void *U_host, const void *s_host)
     int rc = ensure_staging(c);
     if (rc != WD_OK) return rc;
     if (U_host) {
-        CUDA_TRY(c, cudaMemcpyAsync(c->U_can, U_host, gauge_bytes(c), cudaMemcpyHostToDevice, c->stream));
+        CUDA_TRY(c, cudaMemcpyAsync(c->U_can, U_host, gauge_can_bytes(c), cudaMemcpyHostToDevice, c->stream));
         rc = wd_pack_gauge(c, c->U_can, c->U_nat);
         if (rc != WD_OK) return rc;
         c->have_gauge = 1;
     }
-    CUDA_TRY(c, cudaMemcpyAsync(c->s_can, s_host, spinor_bytes(c), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->s_can, s_host, spinor_can_bytes(c), cudaMemcpyHostToDevice, c->stream));
     return wd_pack_spinor(c, c->s_can, c->s_nat_in);
 }
 
@@ -531,7 +557,7 @@ static int return_output(wd_ctx *c, void *out_host)
 {
     int rc = wd_unpack_spinor(c, c->s_nat_out, c->s_can);
     if (rc != WD_OK) return rc;
-    CUDA_TRY(c, cudaMemcpyAsync(out_host, c->s_can, spinor_bytes(c), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(out_host, c->s_can, spinor_can_bytes(c), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaEventRecord(c->ev[3], c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return WD_OK;

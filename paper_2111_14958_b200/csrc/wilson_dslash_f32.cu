@@ -1,0 +1,8 @@
+// fp32 instantiations of the stencil kernel (one translation unit per precision so that they compile in parallel).
+#include "wilson_launch.cuh"
+namespace wd {
+cudaError_t launch_dslash_f32(int tile, int dagger, int mode, const DslashArgs &a)
+{
+    return launch_dslash_any<float>(tile, dagger, mode, a);
+}
+}  // namespace wd

@@ -10,11 +10,11 @@
 //     fused into the stencil passes: MODE_QQ produces |D-dagger p|^2 and alpha, MODE_RUPD applies
 //     r <- r - alpha D q and produces |r|^2, beta and the loop condition, all in device memory.
 //
-// Data layout (include/wilson_cg.h "Native layouts"): site-planar SoA.  A spinor is NSP planes of
-// 128-bit vectors (float4 = two complex components, double2 = one), a link 9 planes of one complex
-// each; plane stride = V; the site index inside a plane is lexicographic, x fastest.  One thread owns
-// one site; a CTA owns a BX x BY x BZ x BT tile so that the 8 neighbours of most sites are fetched by
-// the same CTA (L1 reuse) and all loads of a warp are contiguous runs of BX sites.
+// Data layout (include/wilson_cg.h "Native layouts"): site-blocked SoA.  Blocks of 32 lexicographic sites;
+// inside a block a spinor is NSP planes of 128-bit vectors (float4 = two complex components, double2 = one)
+// and the 4 links are 36 planes of one complex each.  One thread owns one site; a CTA owns a
+// BX x BY x BZ x BT tile so that the 8 neighbours of most sites are fetched by the same CTA (L1 reuse) and
+// all loads of a warp are contiguous runs of BX sites.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -26,7 +26,27 @@ struct Geom {
     int V;       // volume = plane stride
     int nt[4];   // tiles per direction (ceil)
     int bc_t;    // -1 antiperiodic, +1 periodic
+    int zc;      // z tiles per chunk of the CTA rasterisation (see tile_of_block)
 };
+
+// CTA rasterisation.  Tiles are visited x, y, z-within-chunk fastest, then t, then z-chunk: the sites a CTA
+// shares with its +-t neighbours (2 spinor layers and one layer of U_t per tile) are then touched again
+// after Lx*Ly*(zc*BZ)*BT sites instead of after a whole t-slice, which keeps them in L2 on lattices whose
+// t-slice (spinor + gauge) is larger than L2 (48^3x96: 42 MB per slice).  Only the chunk faces in z are
+// read twice from DRAM.  zc = nt[2] is the plain lexicographic order.
+__device__ __forceinline__ void tile_of_block(const Geom &g, int b, int &tx, int &ty, int &tz, int &tt)
+{
+    const int per_z = g.nt[0] * g.nt[1];
+    const int per_chunk = per_z * g.zc * g.nt[3];      // blocks of a full chunk
+    const int c = b / per_chunk;
+    int rem = b - c * per_chunk;
+    const int z0 = c * g.zc;
+    const int zc = min(g.zc, g.nt[2] - z0);            // the last chunk may be shorter
+    tx = rem % g.nt[0]; rem /= g.nt[0];
+    ty = rem % g.nt[1]; rem /= g.nt[1];
+    tz = z0 + rem % zc;
+    tt = rem / zc;
+}
 
 // Device-resident CG state.  All fp64 (reading G17).
 struct CgScalars {
@@ -54,56 +74,82 @@ template <> struct Field<double> {
     static constexpr int NSP = 12;
 };
 
-// ---------------------------------------------------------------- loads / stores
-__device__ __forceinline__ void load_spinor(const float4 *__restrict__ base, size_t V, int s, float v[24])
+// ---------------------------------------------------------------- site-blocked SoA addressing
+// Sites are grouped in blocks of SB = 32 consecutive lexicographic sites (x fastest).  Inside a block the
+// data is planar: spinor block = NSP planes x 32 sites x 128-bit vector (3 KB fp32), gauge block =
+// 36 planes (mu*9 + a*3+b) x 32 sites x one complex (9 KB fp32).  A warp reading one plane of one block
+// reads 512 (256) contiguous bytes, and every plane of a site is at a COMPILE-TIME offset from the
+// site's base address, so the 15 loads of a hop share one address register and use immediate offsets
+// (the site-planar layout with stride V cost ~30 % of all issued instructions in address arithmetic).
+// The volume is padded up to a multiple of 32 sites; pad lanes are never read as sites and are skipped
+// by the vector kernels.
+constexpr int SB = 32;
+constexpr int SB_SHIFT = 5;
+
+template <typename svec, int NSP>
+__device__ __forceinline__ size_t spinor_index(int s)
 {
+    return (size_t)(s >> SB_SHIFT) * (NSP * SB) + (s & (SB - 1));
+}
+__device__ __forceinline__ size_t gauge_index(int s) { return (size_t)(s >> SB_SHIFT) * (36 * SB) + (s & (SB - 1)); }
+
+// ---------------------------------------------------------------- loads / stores
+__device__ __forceinline__ void load_spinor(const float4 *__restrict__ base, int s, float v[24])
+{
+    const float4 *p = base + spinor_index<float4, 6>(s);
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
-        const float4 t = __ldg(base + j * V + s);
+        const float4 t = __ldg(p + j * SB);
         v[4 * j + 0] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
     }
 }
-__device__ __forceinline__ void load_spinor(const double2 *__restrict__ base, size_t V, int s, double v[24])
+__device__ __forceinline__ void load_spinor(const double2 *__restrict__ base, int s, double v[24])
 {
+    const double2 *p = base + spinor_index<double2, 12>(s);
 #pragma unroll
     for (int j = 0; j < 12; ++j) {
-        const double2 t = __ldg(base + j * V + s);
+        const double2 t = __ldg(p + j * SB);
         v[2 * j + 0] = t.x; v[2 * j + 1] = t.y;
     }
 }
 // Read-write fields (r in MODE_RUPD): coherent load, not the read-only path.
-__device__ __forceinline__ void load_spinor_rw(const float4 *base, size_t V, int s, float v[24])
+__device__ __forceinline__ void load_spinor_rw(const float4 *base, int s, float v[24])
 {
+    const float4 *p = base + spinor_index<float4, 6>(s);
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
-        const float4 t = base[j * V + s];
+        const float4 t = p[j * SB];
         v[4 * j + 0] = t.x; v[4 * j + 1] = t.y; v[4 * j + 2] = t.z; v[4 * j + 3] = t.w;
     }
 }
-__device__ __forceinline__ void load_spinor_rw(const double2 *base, size_t V, int s, double v[24])
+__device__ __forceinline__ void load_spinor_rw(const double2 *base, int s, double v[24])
 {
+    const double2 *p = base + spinor_index<double2, 12>(s);
 #pragma unroll
     for (int j = 0; j < 12; ++j) {
-        const double2 t = base[j * V + s];
+        const double2 t = p[j * SB];
         v[2 * j + 0] = t.x; v[2 * j + 1] = t.y;
     }
 }
-__device__ __forceinline__ void store_spinor(float4 *base, size_t V, int s, const float v[24])
+__device__ __forceinline__ void store_spinor(float4 *base, int s, const float v[24])
 {
+    float4 *p = base + spinor_index<float4, 6>(s);
 #pragma unroll
-    for (int j = 0; j < 6; ++j) base[j * V + s] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+    for (int j = 0; j < 6; ++j) p[j * SB] = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
 }
-__device__ __forceinline__ void store_spinor(double2 *base, size_t V, int s, const double v[24])
+__device__ __forceinline__ void store_spinor(double2 *base, int s, const double v[24])
 {
+    double2 *p = base + spinor_index<double2, 12>(s);
 #pragma unroll
-    for (int j = 0; j < 12; ++j) base[j * V + s] = make_double2(v[2 * j], v[2 * j + 1]);
+    for (int j = 0; j < 12; ++j) p[j * SB] = make_double2(v[2 * j], v[2 * j + 1]);
 }
-template <typename gvec, typename real>
-__device__ __forceinline__ void load_link(const gvec *__restrict__ U, size_t V, int mu, int s, real u[18])
+template <int MU, typename gvec, typename real>
+__device__ __forceinline__ void load_link(const gvec *__restrict__ U, int s, real u[18])
 {
+    const gvec *p = U + gauge_index(s) + MU * 9 * SB;
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
-        const gvec t = __ldg(U + (size_t)(mu * 9 + k) * V + s);
+        const gvec t = __ldg(p + k * SB);
         u[2 * k] = t.x; u[2 * k + 1] = t.y;
     }
 }
@@ -196,57 +242,83 @@ __device__ __forceinline__ void reconstruct(const real g[12], real sg, real acc[
     }
 }
 
-// One hop: acc += sg (1 + S gamma_MU) (x) [U or U^dagger](link_site) in(spinor_site).
-template <int MU, int S, bool ADJ, typename real, typename svec, typename gvec>
-__device__ __forceinline__ void hop(const gvec *__restrict__ U, const svec *__restrict__ in, size_t V,
-                                    int link_site, int spinor_site, real sg, real acc[24])
+// One hop, split into its loads and its arithmetic so that the loads of the next hop can be in flight
+// while this one is computed:  acc += sg (1 + S gamma_MU) (x) [U or U^dagger](link_site) in(spinor_site).
+template <int MU, typename real, typename svec, typename gvec>
+__device__ __forceinline__ void hop_load(const gvec *__restrict__ U, const svec *__restrict__ in,
+                                         int link_site, int spinor_site, real v[24], real u[18])
 {
-    real v[24], h[12], u[18], g[12];
-    load_spinor(in, V, spinor_site, v);
-    load_link<gvec, real>(U, V, MU, link_site, u);
+    load_spinor(in, spinor_site, v);
+    load_link<MU, gvec, real>(U, link_site, u);
+}
+template <int MU, int S, bool ADJ, typename real>
+__device__ __forceinline__ void hop_compute(const real v[24], const real u[18], real sg, real acc[24])
+{
+    real h[12], g[12];
     project<MU, S, real>(v, h);
     mul_su3<ADJ, real>(u, h, g);
     reconstruct<MU, S, real>(g, sg, acc);
 }
 
-// acc = sum over the 8 hops at site s = (x,y,z,t).  DAG = 0: D (forward projector 1 - gamma), 1: D-dagger.
-template <int DAG, typename real, typename svec, typename gvec>
-__device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const svec *__restrict__ in,
-                                            int x, int y, int z, int t, int s, real acc[24])
+// Neighbour sites and boundary signs of site s = (x,y,z,t).
+struct Hops {
+    int f[4], b[4];
+};
+__device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, int t, int s)
 {
-    constexpr int SF = DAG ? +1 : -1;
-    const size_t V = (size_t)g.V;
     const int L0 = g.L[0], L1 = g.L[1], L2 = g.L[2], L3 = g.L[3];
     const int s1 = L0, s2 = L0 * L1, s3 = L0 * L1 * L2;
+    Hops h;
+    h.f[0] = s + (x == L0 - 1 ? 1 - L0 : 1);
+    h.b[0] = s + (x == 0 ? L0 - 1 : -1);
+    h.f[1] = s + (y == L1 - 1 ? (1 - L1) * s1 : s1);
+    h.b[1] = s + (y == 0 ? (L1 - 1) * s1 : -s1);
+    h.f[2] = s + (z == L2 - 1 ? (1 - L2) * s2 : s2);
+    h.b[2] = s + (z == 0 ? (L2 - 1) * s2 : -s2);
+    h.f[3] = s + (t == L3 - 1 ? (1 - L3) * s3 : s3);
+    h.b[3] = s + (t == 0 ? (L3 - 1) * s3 : -s3);
+    return h;
+}
+
+// acc = sum over the 8 hops at site s; then c = centre spinor in(s) (loaded last so that its latency
+// overlaps the last hop).  DAG = 0: D (forward projector 1 - gamma), 1: D-dagger.
+// PIPE = 0: hop after hop (load, compute).  PIPE = 1: software pipeline, two register buffers: the loads of
+// hop k+1 are issued before hop k is computed, so every thread keeps one hop (168 B fp32) in flight while
+// it computes (memory-level parallelism without more threads).
+template <int DAG, int PIPE, typename real, typename svec, typename gvec>
+__device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const svec *__restrict__ in,
+                                            int x, int y, int z, int t, int s, real acc[24], real c[24])
+{
+    constexpr int SF = DAG ? +1 : -1;
+    const Hops n = neighbours(g, x, y, z, t, s);
+    // boundary sign sigma+- of reading C-1: only the hop that wraps the t boundary carries bc_t
+    const real sgf = (t == g.L[3] - 1) ? (real)g.bc_t : (real)1;
+    const real sgb = (t == 0) ? (real)g.bc_t : (real)1;
+    const real one = (real)1;
 #pragma unroll
     for (int i = 0; i < 24; ++i) acc[i] = 0;
-    {
-        const int sf = s + (x == L0 - 1 ? 1 - L0 : 1);
-        const int sb = s + (x == 0 ? L0 - 1 : -1);
-        hop<0, SF, false, real>(U, in, V, s, sf, (real)1, acc);
-        hop<0, -SF, true, real>(U, in, V, sb, sb, (real)1, acc);
-    }
-    {
-        const int sf = s + (y == L1 - 1 ? (1 - L1) * s1 : s1);
-        const int sb = s + (y == 0 ? (L1 - 1) * s1 : -s1);
-        hop<1, SF, false, real>(U, in, V, s, sf, (real)1, acc);
-        hop<1, -SF, true, real>(U, in, V, sb, sb, (real)1, acc);
-    }
-    {
-        const int sf = s + (z == L2 - 1 ? (1 - L2) * s2 : s2);
-        const int sb = s + (z == 0 ? (L2 - 1) * s2 : -s2);
-        hop<2, SF, false, real>(U, in, V, s, sf, (real)1, acc);
-        hop<2, -SF, true, real>(U, in, V, sb, sb, (real)1, acc);
-    }
-    {
-        // boundary sign sigma+- of reading C-1: only the hop that wraps the t boundary carries bc_t
-        const bool wf = (t == L3 - 1), wb = (t == 0);
-        const int sf = s + (wf ? (1 - L3) * s3 : s3);
-        const int sb = s + (wb ? (L3 - 1) * s3 : -s3);
-        const real sgf = wf ? (real)g.bc_t : (real)1;
-        const real sgb = wb ? (real)g.bc_t : (real)1;
-        hop<3, SF, false, real>(U, in, V, s, sf, sgf, acc);
-        hop<3, -SF, true, real>(U, in, V, sb, sb, sgb, acc);
+    if (PIPE == 0) {
+        real v[24], u[18];
+        hop_load<0, real>(U, in, s, n.f[0], v, u);       hop_compute<0, SF, false, real>(v, u, one, acc);
+        hop_load<0, real>(U, in, n.b[0], n.b[0], v, u);  hop_compute<0, -SF, true, real>(v, u, one, acc);
+        hop_load<1, real>(U, in, s, n.f[1], v, u);       hop_compute<1, SF, false, real>(v, u, one, acc);
+        hop_load<1, real>(U, in, n.b[1], n.b[1], v, u);  hop_compute<1, -SF, true, real>(v, u, one, acc);
+        hop_load<2, real>(U, in, s, n.f[2], v, u);       hop_compute<2, SF, false, real>(v, u, one, acc);
+        hop_load<2, real>(U, in, n.b[2], n.b[2], v, u);  hop_compute<2, -SF, true, real>(v, u, one, acc);
+        hop_load<3, real>(U, in, s, n.f[3], v, u);       hop_compute<3, SF, false, real>(v, u, sgf, acc);
+        hop_load<3, real>(U, in, n.b[3], n.b[3], v, u);  hop_compute<3, -SF, true, real>(v, u, sgb, acc);
+        load_spinor(in, s, c);
+    } else {
+        real va[24], ua[18], vb[24], ub[18];
+        hop_load<0, real>(U, in, s, n.f[0], va, ua);
+        hop_load<0, real>(U, in, n.b[0], n.b[0], vb, ub);  hop_compute<0, SF, false, real>(va, ua, one, acc);
+        hop_load<1, real>(U, in, s, n.f[1], va, ua);       hop_compute<0, -SF, true, real>(vb, ub, one, acc);
+        hop_load<1, real>(U, in, n.b[1], n.b[1], vb, ub);  hop_compute<1, SF, false, real>(va, ua, one, acc);
+        hop_load<2, real>(U, in, s, n.f[2], va, ua);       hop_compute<1, -SF, true, real>(vb, ub, one, acc);
+        hop_load<2, real>(U, in, n.b[2], n.b[2], vb, ub);  hop_compute<2, SF, false, real>(va, ua, one, acc);
+        hop_load<3, real>(U, in, s, n.f[3], va, ua);       hop_compute<2, -SF, true, real>(vb, ub, one, acc);
+        hop_load<3, real>(U, in, n.b[3], n.b[3], vb, ub);  hop_compute<3, SF, false, real>(va, ua, sgf, acc);
+        load_spinor(in, s, c);                             hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
     }
 }
 
@@ -325,8 +397,8 @@ enum { MODE_PLAIN = 0, MODE_QQ = 1, MODE_RUPD = 2 };
 // MODE_PLAIN : out = D in / D-dagger in                                  (wd_apply, a6, a7)
 // MODE_QQ    : out = q = D-dagger p, qq = |q|^2, alpha = rr/qq           (a2)
 // MODE_RUPD  : s = D q (not stored), r <- r - alpha s, rr' = |r|^2, beta, loop condition   (a3)
-template <typename real, int DAG, int MODE, int BX, int BY, int BZ, int BT>
-__global__ void __launch_bounds__(BX *BY *BZ *BT)
+template <typename real, int DAG, int MODE, int BX, int BY, int BZ, int BT, int MINB, int PIPE>
+__global__ void __launch_bounds__(BX *BY *BZ *BT, MINB)
 dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
               const typename Field<real>::svec *__restrict__ in, typename Field<real>::svec *out, real kappa,
               typename Field<real>::svec *r, CgScalars *sc, double *partials, unsigned int *counter,
@@ -338,40 +410,35 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     if (MODE != MODE_PLAIN) {
         if (it >= sc->k_stop) return;  // uniform over the grid: over-launched iterations are no-ops
     }
-    int b = blockIdx.x;
-    const int tx = b % g.nt[0]; b /= g.nt[0];
-    const int ty = b % g.nt[1]; b /= g.nt[1];
-    const int tz = b % g.nt[2]; b /= g.nt[2];
-    const int tt = b;
+    int tx, ty, tz, tt;
+    tile_of_block(g, blockIdx.x, tx, ty, tz, tt);
     const int tid = threadIdx.x;
     const int x = tx * BX + tid % BX;
     const int y = ty * BY + (tid / BX) % BY;
     const int z = tz * BZ + (tid / (BX * BY)) % BZ;
     const int t = tt * BT + tid / (BX * BY * BZ);
     const bool active = (x < g.L[0]) && (y < g.L[1]) && (z < g.L[2]) && (t < g.L[3]);
-    const size_t V = (size_t)g.V;
     double local = 0.0;
     if (active) {
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24];
-        hopping_sum<DAG, real, svec, gvec>(g, U, in, x, y, z, t, s, acc);
-        load_spinor(in, V, s, c);
+        hopping_sum<DAG, PIPE, real, svec, gvec>(g, U, in, x, y, z, t, s, acc, c);
 #pragma unroll
         for (int i = 0; i < 24; ++i) c[i] = fma(-kappa, acc[i], c[i]);  // (D in)(x) = in(x) - kappa * hops
         if (MODE == MODE_RUPD) {
             const real alpha = (real)sc->alpha;
             real rv[24];
-            load_spinor_rw(r, V, s, rv);
+            load_spinor_rw(r, s, rv);
             real n2 = 0;
 #pragma unroll
             for (int i = 0; i < 24; ++i) {
                 rv[i] = fma(-alpha, c[i], rv[i]);                      // r <- r - alpha D D-dagger p
                 n2 = fma(rv[i], rv[i], n2);
             }
-            store_spinor(r, V, s, rv);
+            store_spinor(r, s, rv);
             local = (double)n2;
         } else {
-            store_spinor(out, V, s, c);
+            store_spinor(out, s, c);
             if (MODE == MODE_QQ) {
                 real n2 = 0;
 #pragma unroll
@@ -410,17 +477,28 @@ __device__ __forceinline__ double2 vaxpy(double a, const double2 &x, const doubl
     return make_double2(fma(a, x.x, y.x), fma(a, x.y, y.y));
 }
 
+// Element i of a native spinor buffer (i counts 128-bit vectors) belongs to site (i / (NSP*SB))*SB + i % SB.
+// `V` is the number of real sites; when the volume is not a multiple of SB the pad lanes of the last block
+// are skipped (padded == 0 -> no test at all).
+template <int NSP>
+__device__ __forceinline__ bool real_site(size_t i, int V, int padded)
+{
+    if (!padded) return true;
+    const size_t blk = i / (NSP * SB);
+    return (int)(blk * SB + (i & (SB - 1))) < V;
+}
+
 // a1: y <- 0, r <- eta, p <- eta, rr = eta2 = <eta,eta>, k = 0 ("psi <- psi0; r <- eta - D psi; p <- r", psi0 = 0)
 template <typename real>
 __global__ void __launch_bounds__(VEC_NT)
 cg_init_kernel(const typename Field<real>::svec *__restrict__ eta, typename Field<real>::svec *y,
-               typename Field<real>::svec *r, typename Field<real>::svec *p, size_t n, CgScalars *sc,
-               double *partials, unsigned int *counter, double *hist, double r_min, int max_iter)
+               typename Field<real>::svec *r, typename Field<real>::svec *p, size_t n, int V, int padded,
+               CgScalars *sc, double *partials, unsigned int *counter, double *hist, double r_min, int max_iter)
 {
     using svec = typename Field<real>::svec;
     double local = 0.0;
     for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT) {
-        const svec e = __ldg(eta + i);
+        const svec e = real_site<Field<real>::NSP>(i, V, padded) ? __ldg(eta + i) : svec();
         y[i] = vzero(e);
         r[i] = e;
         p[i] = e;
@@ -457,48 +535,58 @@ cg_update_kernel(typename Field<real>::svec *y, typename Field<real>::svec *p,
 // the paper's dot-product kernel on its own: <a,a>
 template <typename real>
 __global__ void __launch_bounds__(VEC_NT)
-norm2_kernel(const typename Field<real>::svec *__restrict__ a, size_t n, double *partials, unsigned int *counter,
-             double *result)
+norm2_kernel(const typename Field<real>::svec *__restrict__ a, size_t n, int V, int padded, double *partials,
+             unsigned int *counter, double *result)
 {
     using svec = typename Field<real>::svec;
     double local = 0.0;
     for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT)
-        local += vnorm2<svec>(__ldg(a + i));
+        if (real_site<Field<real>::NSP>(i, V, padded)) local += vnorm2<svec>(__ldg(a + i));
     double total;
     if (grid_sum<VEC_NT>(local, partials, counter, &total)) *result = total;
 }
 
 // ---------------------------------------------------------------- a0: canonical <-> native permutations
-// canonical gauge U[s][mu][a][b] (complex) -> native plane (mu*9 + a*3+b), one thread per site.
+// One thread per (padded) site.  canonical gauge U[s][mu][a][b] (36 complex, contiguous) -> plane mu*9+a*3+b of
+// the site's block; canonical spinor psi[s][alpha][a] (NSP vectors, contiguous) -> plane j.  Pad lanes get zeros.
 template <typename real>
 __global__ void __launch_bounds__(VEC_NT)
-pack_gauge_kernel(const typename Field<real>::gvec *__restrict__ can, typename Field<real>::gvec *nat, int V)
+pack_gauge_kernel(const typename Field<real>::gvec *__restrict__ can, typename Field<real>::gvec *nat, int V, int Vpad)
 {
+    using gvec = typename Field<real>::gvec;
     const int s = blockIdx.x * VEC_NT + threadIdx.x;
-    if (s >= V) return;
+    if (s >= Vpad) return;
+    gvec *p = nat + gauge_index(s);
+    if (s < V) {
 #pragma unroll 4
-    for (int k = 0; k < 36; ++k) nat[(size_t)k * V + s] = __ldg(can + (size_t)s * 36 + k);
+        for (int k = 0; k < 36; ++k) p[k * SB] = __ldg(can + (size_t)s * 36 + k);
+    } else {
+        for (int k = 0; k < 36; ++k) p[k * SB] = gvec();
+    }
 }
-// canonical spinor psi[s][alpha][a] (24 reals = NSP vectors, contiguous) <-> native planes.
 template <typename real>
 __global__ void __launch_bounds__(VEC_NT)
-pack_spinor_kernel(const typename Field<real>::svec *__restrict__ can, typename Field<real>::svec *nat, int V)
+pack_spinor_kernel(const typename Field<real>::svec *__restrict__ can, typename Field<real>::svec *nat, int V, int Vpad)
 {
+    using svec = typename Field<real>::svec;
     constexpr int NSP = Field<real>::NSP;
     const int s = blockIdx.x * VEC_NT + threadIdx.x;
-    if (s >= V) return;
+    if (s >= Vpad) return;
+    svec *p = nat + spinor_index<svec, NSP>(s);
 #pragma unroll
-    for (int j = 0; j < NSP; ++j) nat[(size_t)j * V + s] = __ldg(can + (size_t)s * NSP + j);
+    for (int j = 0; j < NSP; ++j) p[j * SB] = s < V ? __ldg(can + (size_t)s * NSP + j) : svec();
 }
 template <typename real>
 __global__ void __launch_bounds__(VEC_NT)
 unpack_spinor_kernel(const typename Field<real>::svec *__restrict__ nat, typename Field<real>::svec *can, int V)
 {
+    using svec = typename Field<real>::svec;
     constexpr int NSP = Field<real>::NSP;
     const int s = blockIdx.x * VEC_NT + threadIdx.x;
     if (s >= V) return;
+    const svec *p = nat + spinor_index<svec, NSP>(s);
 #pragma unroll
-    for (int j = 0; j < NSP; ++j) can[(size_t)s * NSP + j] = __ldg(nat + (size_t)j * V + s);
+    for (int j = 0; j < NSP; ++j) can[(size_t)s * NSP + j] = __ldg(p + j * SB);
 }
 
 }  // namespace wd

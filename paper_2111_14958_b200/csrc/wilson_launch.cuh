@@ -1,0 +1,95 @@
+// wilson_launch.cuh — the table of compiled stencil launch configurations and the per-precision launchers.
+// A "tile" (the name of the C ABI, wd_set_tile) is one row: CTA tile BX x BY x BZ x BT (threads per CTA =
+// product), MINB = minimum resident CTAs per SM asked of ptxas (bounds registers per thread), PIPE = 1 for
+// the software-pipelined hop loop.  This is the CUDA analogue of the paper's workgroup-size knob
+// (PAPER.md:58,76).  F64 = 1 if the row is also compiled for double precision.
+#pragma once
+#include "wilson_kernels.cuh"
+
+// Rows are in order of preference (measured on B200, profiles/): the automatic choice takes the first row
+// with the fewest padded threads for the lattice and precision at hand.
+//   X(index, BX, BY, BZ, BT, MINB, PIPE, F64)
+#define WD_TILE_TABLE(X) \
+    X(0, 32, 2, 2, 1, 4, 1, 0) \
+    X(1, 16, 2, 2, 2, 4, 1, 0) \
+    X(2, 32, 2, 2, 2, 2, 1, 0) \
+    X(3, 32, 2, 1, 1, 8, 1, 0) \
+    X(4, 16, 2, 4, 2, 2, 1, 0) \
+    X(5, 16, 4, 2, 2, 2, 1, 0) \
+    X(6, 8, 4, 2, 2, 4, 1, 0) \
+    X(7, 16, 2, 2, 1, 8, 1, 0) \
+    X(8, 32, 2, 2, 1, 2, 1, 1) \
+    X(9, 16, 2, 2, 1, 4, 1, 1) \
+    X(10, 16, 2, 2, 2, 2, 1, 1) \
+    X(11, 8, 4, 2, 1, 4, 1, 1) \
+    X(12, 8, 2, 2, 2, 4, 1, 1) \
+    X(13, 4, 4, 2, 2, 4, 1, 1) \
+    X(14, 4, 4, 4, 2, 2, 1, 1) \
+    X(15, 16, 2, 2, 2, 0, 0, 1) \
+    X(16, 8, 4, 4, 2, 0, 0, 1)
+#define WD_NUM_TILES 17
+
+namespace wd {
+
+struct TileInfo {
+    int b[4];
+    int minb, pipe, f64;
+};
+static const TileInfo kTiles[WD_NUM_TILES] = {
+#define X(i, a, b, c, d, m, p, f) {{a, b, c, d}, m, p, f},
+    WD_TILE_TABLE(X)
+#undef X
+};
+
+struct DslashArgs {
+    Geom g;
+    unsigned int grid;
+    cudaStream_t stream;
+    const void *U;
+    const void *in;
+    void *out;
+    double kappa;
+    void *r;
+    CgScalars *sc;
+    double *partials;
+    unsigned int *counter;
+    double *hist;
+    int it;
+};
+
+// dagger in {0,1}; mode in {MODE_PLAIN, MODE_QQ (dagger = 1 only), MODE_RUPD (dagger = 0 only)}
+cudaError_t launch_dslash_f32(int tile, int dagger, int mode, const DslashArgs &a);
+cudaError_t launch_dslash_f64(int tile, int dagger, int mode, const DslashArgs &a);
+
+template <typename real, int DAG, int MODE>
+static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
+{
+    using svec = typename Field<real>::svec;
+    using gvec = typename Field<real>::gvec;
+    switch (tile) {
+#define X(i, bx, by, bz, bt, m, p, f)                                                                          \
+    case i:                                                                                                    \
+        if constexpr (sizeof(real) == 4 || f) {                                                                \
+            dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p><<<a.grid, bx * by * bz * bt, 0, a.stream>>>(  \
+                a.g, (const gvec *)a.U, (const svec *)a.in, (svec *)a.out, (real)a.kappa, (svec *)a.r, a.sc,   \
+                a.partials, a.counter, a.hist, a.it);                                                          \
+            return cudaGetLastError();                                                                         \
+        }                                                                                                      \
+        return cudaErrorInvalidValue;
+        WD_TILE_TABLE(X)
+#undef X
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+template <typename real>
+static cudaError_t launch_dslash_any(int tile, int dagger, int mode, const DslashArgs &a)
+{
+    if (mode == MODE_PLAIN)
+        return dagger ? launch_dslash_tile<real, 1, MODE_PLAIN>(tile, a) : launch_dslash_tile<real, 0, MODE_PLAIN>(tile, a);
+    if (mode == MODE_QQ && dagger) return launch_dslash_tile<real, 1, MODE_QQ>(tile, a);
+    if (mode == MODE_RUPD && !dagger) return launch_dslash_tile<real, 0, MODE_RUPD>(tile, a);
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace wd

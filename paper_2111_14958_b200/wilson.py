@@ -83,9 +83,13 @@ def load_library(path: str = LIB_PATH):
     lib.wd_norm2.argtypes = [vp, vp, dp]
     lib.wd_num_tiles.argtypes = []
     lib.wd_tile_shape.argtypes = [ci, ip]
+    lib.wd_tile_info.argtypes = [ci, ip]
     lib.wd_set_tile.argtypes = [vp, ci]
     lib.wd_get_tile.argtypes = [vp]
+    lib.wd_set_zchunk.argtypes = [vp, ci]
     lib.wd_set_poll_interval.argtypes = [vp, ci]
+    lib.wd_set_profile.argtypes = [vp, ci]
+    lib.wd_get_profile.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_long)]
     lib.wd_version.argtypes = []
     lib.wd_version.restype = ctypes.c_char_p
     _lib = lib
@@ -99,6 +103,17 @@ def tile_shapes():
         shp = (ctypes.c_int * 4)()
         lib.wd_tile_shape(i, shp)
         out.append(tuple(shp))
+    return out
+
+
+def tile_infos():
+    """[(BX,BY,BZ,BT, min_blocks_per_sm, pipelined, has_fp64), ...] for every compiled launch configuration."""
+    lib = load_library()
+    out = []
+    for i, shp in enumerate(tile_shapes()):
+        info = (ctypes.c_int * 3)()
+        lib.wd_tile_info(i, info)
+        out.append(tuple(shp) + tuple(info))
     return out
 
 
@@ -267,6 +282,19 @@ class WilsonContext:
 
     def wd_get_tile(self):
         return int(self.lib.wd_get_tile(self._ctx))
+
+    def wd_set_profile(self, on):
+        self._check(self.lib.wd_set_profile(self._ctx, int(bool(on))))
+
+    def wd_get_profile(self):
+        """{'a2_ms', 'a3_ms', 'a4_ms', 'iterations'}: accumulated device time per kernel class of the CG loop."""
+        ms = (ctypes.c_double * 3)()
+        n = ctypes.c_long()
+        self._check(self.lib.wd_get_profile(self._ctx, ms, ctypes.byref(n)))
+        return {"a2_ms": ms[0], "a3_ms": ms[1], "a4_ms": ms[2], "iterations": n.value}
+
+    def wd_set_zchunk(self, layers):
+        self._check(self.lib.wd_set_zchunk(self._ctx, int(layers)))
 
     def wd_set_poll_interval(self, n):
         self._check(self.lib.wd_set_poll_interval(self._ctx, int(n)))

@@ -47,7 +47,7 @@ def iters_close(a, b):
 
 # ---------------------------------------------------------------- a0: layouts
 @pytest.mark.parametrize("precision", [32, 64])
-@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 10, 8), (14, 14, 14, 14)])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 10, 8), (5, 7, 4, 6), (14, 14, 14, 14)])
 def test_pack_unpack_are_exact_permutations(wilson, precision, dims):
     V = int(np.prod(dims))
     cdt = gu.np_complex(precision)
@@ -60,13 +60,19 @@ def test_pack_unpack_are_exact_permutations(wilson, precision, dims):
         back = gu.to_host(ctx.wd_unpack_spinor(pn))
         pn_h, Un_h = gu.to_host(pn), gu.to_host(Un)
     assert back.tobytes() == psi.tobytes()
-    # native spinor: NSP planes of 128-bit vectors, plane stride V (include/wilson_cg.h)
+    # native layout (include/wilson_cg.h): blocks of 32 lexicographic sites; inside a block the spinor is NSP
+    # planes of 128-bit vectors, the gauge field 36 planes (mu*9 + a*3+b) of one complex; pad lanes are zero
+    nblk = (V + 31) // 32
+    Vp = nblk * 32
     nsp, w = (6, 4) if precision == 32 else (12, 2)
-    want = psi.view(rdt).reshape(V, nsp, w).transpose(1, 0, 2)
-    assert pn_h.reshape(nsp, V, w).tobytes() == np.ascontiguousarray(want).tobytes()
-    # native gauge: plane mu*9 + a*3+b of one complex, plane stride V
-    want_u = U.view(rdt).reshape(V, 36, 2).transpose(1, 0, 2)
-    assert Un_h.reshape(36, V, 2).tobytes() == np.ascontiguousarray(want_u).tobytes()
+    want = np.zeros((Vp, nsp, w), dtype=rdt)
+    want[:V] = psi.view(rdt).reshape(V, nsp, w)
+    want = want.reshape(nblk, 32, nsp, w).transpose(0, 2, 1, 3)
+    assert pn_h.size == Vp * 24 and pn_h.tobytes() == np.ascontiguousarray(want).tobytes()
+    want_u = np.zeros((Vp, 36, 2), dtype=rdt)
+    want_u[:V] = U.view(rdt).reshape(V, 36, 2)
+    want_u = want_u.reshape(nblk, 32, 36, 2).transpose(0, 2, 1, 3)
+    assert Un_h.size == Vp * 72 and Un_h.tobytes() == np.ascontiguousarray(want_u).tobytes()
 
 
 # ---------------------------------------------------------------- a7: wd_apply
