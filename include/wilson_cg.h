@@ -34,12 +34,15 @@
  *
  * Native (internal, site-planar SoA) layouts — produced by wd_pack_*, consumed by wd_apply /
  * cg_solve; opaque to the caller except for their size (wd_*_native_bytes):
- *    precision 32: spinor = 6 planes of float4  (plane j holds complex components 2j, 2j+1 of
- *                  the 12 = alpha*3+a), plane stride V;   gauge = 4*9 planes of float2
- *                  (plane mu*9 + a*3+b), plane stride V.
- *    precision 64: spinor = 12 planes of double2, gauge = 36 planes of double2.
- *    Every per-thread access is one 128-bit (spinor) or 64/128-bit (gauge) load and a warp
- *    reads consecutive sites of one plane: 512 contiguous bytes per spinor plane.
+ *    sites are grouped in blocks of 16 consecutive site indices (the volume is padded up to a
+ *    multiple of 16; pad lanes hold zeros); inside a block the data is planar:
+ *    precision 32: spinor block = 6 planes x 16 sites of float4 (plane j holds complex components
+ *                  2j, 2j+1 of the 12 = alpha*3+a), 1.5 KB;  gauge block = 4 links x 1152 B, 4.5 KB; a link is 4 planes
+ *                  x 16 sites of float4 (reals 4q..4q+3 of the 18 = (a*3+b)*2+ri) followed by one plane x 16
+ *                  sites of float2 (reals 16, 17).
+ *    precision 64: spinor block = 12 planes of double2, gauge block = 36 planes of double2.
+ *    Every per-thread access is one 128-bit (spinor) or 64/128-bit (gauge) load at a compile-time
+ *    offset from the site's base address; 16 consecutive lanes read 256 contiguous bytes of a plane.
  *
  * The operator (reading C-1; the paper only cites Wilson, and states
  * gamma5 D gamma5 = D-dagger):
@@ -99,8 +102,8 @@ int wd_destroy(wd_ctx *ctx);
 const char *wd_last_error(wd_ctx *ctx);
 
 /* Sizes in bytes of the native buffers the caller must allocate (device memory). */
-size_t wd_gauge_native_bytes(wd_ctx *ctx);   /* 72 * V * sizeof(real) */
-size_t wd_spinor_native_bytes(wd_ctx *ctx);  /* 24 * V * sizeof(real) */
+size_t wd_gauge_native_bytes(wd_ctx *ctx);   /* 72 * Vpad * sizeof(real), Vpad = V rounded up to 16 */
+size_t wd_spinor_native_bytes(wd_ctx *ctx);  /* 24 * Vpad * sizeof(real) */
 
 /*
  * wd_pack_gauge / wd_pack_spinor / wd_unpack_spinor — pure permutations between the canonical
@@ -173,6 +176,10 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *                             software-pipelined, 1 if also compiled for precision 64}.
  *   wd_set_tile(ctx, i)       select tile i for the stencil kernels of this ctx; i = -1 restores the automatic choice.
  *   wd_get_tile(ctx)          index in use.
+ *   wd_set_prefetch(ctx, n)       L2 bulk-prefetch distance of the stencil kernels in tiles: 0 = off (default: it measured
+ *                             slower on B200), -1 = each CTA prefetches the tile it will process next, n > 0 = n tiles ahead.
+ *   wd_set_waves(ctx, w)          the stencil kernels run a persistent grid of w * (SMs * resident CTAs per SM) CTAs that
+ *                             stride over the tiles; w = 0 or 1: exactly one resident wave (default).
  *   wd_set_zchunk(ctx, layers)    z extent (in sites) of one chunk of the CTA rasterisation x,y,z-in-chunk,t,z-chunk that
  *                             keeps the +-t neighbours of a tile in L2; 0 = automatic (fits a 40 MB reuse distance).
  *   wd_set_poll_interval(ctx, n)  CG iterations enqueued between two host polls of the device stop flag (n >= 1; 0 = automatic).
@@ -182,6 +189,8 @@ int wd_tile_shape(int index, int shape[4]);
 int wd_tile_info(int index, int info[3]);
 int wd_set_tile(wd_ctx *ctx, int index);
 int wd_get_tile(wd_ctx *ctx);
+int wd_set_prefetch(wd_ctx *ctx, int tiles);
+int wd_set_waves(wd_ctx *ctx, int waves);
 int wd_set_zchunk(wd_ctx *ctx, int layers);
 int wd_set_poll_interval(wd_ctx *ctx, int n);
 
@@ -194,6 +203,10 @@ int wd_set_poll_interval(wd_ctx *ctx, int n);
  */
 int wd_set_profile(wd_ctx *ctx, int on);
 int wd_get_profile(wd_ctx *ctx, double ms[3], long *iterations);
+
+/* Host-only self-test of the fast-division constants of the CTA tile decode: returns the number of n in
+ * [0, n_max) with a wrong quotient n / d (0 = correct), or -1 for d = 0.  Needs no GPU. */
+long wd_selftest_fastdiv(unsigned int d, unsigned int n_max);
 
 /* Library version string, e.g. "wilson_cg 0.1 sm_100a". */
 const char *wd_version(void);

@@ -21,6 +21,8 @@ struct wd_ctx {
     int tile;       // tile index in use
     int tile_user;  // -1 = automatic
     int poll;       // 0 = automatic
+    int waves;            // resident waves of the persistent stencil grid (0 -> 1)
+    int prefetch;         // L2 prefetch distance: -1 = automatic (one grid ahead), 0 = off, n > 0 = n tiles
     int zchunk_user;      // z layers per rasterisation chunk, 0 = automatic
     double l2_budget_mb;  // reuse-distance budget of the automatic choice
     int sm_count;
@@ -80,6 +82,39 @@ static inline size_t spinor_can_bytes(const wd_ctx *c) { return (size_t)24 * c->
 static inline size_t gauge_can_bytes(const wd_ctx *c) { return (size_t)72 * c->V * real_bytes(c); }      // canonical
 static inline size_t spinor_vecs(const wd_ctx *c) { return (size_t)(c->precision == 32 ? 6 : 12) * vpad(c); }
 
+static long tile_blocks(const wd_ctx *c, int tile)
+{
+    long n = 1;
+    for (int d = 0; d < 4; ++d) n *= (c->dims[d] + kTiles[tile].b[d] - 1) / kTiles[tile].b[d];
+    return n;
+}
+static FastDiv make_fastdiv(unsigned int d)
+{
+    FastDiv f;
+    f.d = d;
+    if (d <= 1) { f.d = 1; f.M = 0; f.sh = -1; return f; }
+    int s = 0;
+    while ((1u << s) < d) ++s;                       // s = ceil(log2 d) >= 1
+    const unsigned long long p2 = 1ull << (31 + s);
+    f.M = (unsigned int)((p2 + d - 1) / d);          // in [2^31, 2^32)
+    f.sh = s - 1;                                    // (n*M) >> (31+s) = umulhi(n,M) >> (s-1)
+    return f;
+}
+
+/* Host self-test of the fast-division constants used by the tile decode: number of n in [0, n_max) for which
+   (n * M) >> (32 + sh) differs from n / d (0 = correct).  No GPU needed. */
+extern "C" long wd_selftest_fastdiv(unsigned int d, unsigned int n_max)
+{
+    if (d == 0) return -1;
+    const FastDiv f = make_fastdiv(d);
+    long bad = 0;
+    for (unsigned int n = 0; n < n_max; ++n) {
+        const unsigned int q = f.sh < 0 ? n : (unsigned int)(((unsigned long long)n * f.M) >> 32) >> f.sh;
+        bad += (q != n / d);
+    }
+    return bad;
+}
+
 static Geom make_geom(const wd_ctx *c, int tile)
 {
     Geom g;
@@ -102,13 +137,15 @@ static Geom make_geom(const wd_ctx *c, int tile)
             if (g.nt[2] % d == 0 && layer * d * kTiles[tile].b[2] <= budget) zc = d;
     }
     g.zc = zc;
+    g.ntiles = (int)tile_blocks(c, tile);
+    g.pf = 0;   // set per launch (needs the grid size)
+    g.d_chunk = make_fastdiv((unsigned)(g.nt[0] * g.nt[1] * g.zc * g.nt[3]));
+    g.d_nt0 = make_fastdiv((unsigned)g.nt[0]);
+    g.d_nt1 = make_fastdiv((unsigned)g.nt[1]);
+    g.d_zc = make_fastdiv((unsigned)g.zc);
+    const int zlast = g.nt[2] % g.zc ? g.nt[2] % g.zc : g.zc;
+    g.d_zlast = make_fastdiv((unsigned)zlast);
     return g;
-}
-static long tile_blocks(const wd_ctx *c, int tile)
-{
-    long n = 1;
-    for (int d = 0; d < 4; ++d) n *= (c->dims[d] + kTiles[tile].b[d] - 1) / kTiles[tile].b[d];
-    return n;
 }
 static int tile_threads(int tile)
 {
@@ -140,7 +177,9 @@ static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void 
 {
     DslashArgs a;
     a.g = make_geom(c, c->tile);
-    a.grid = (unsigned int)tile_blocks(c, c->tile);
+    a.sm_count = c->sm_count;
+    a.waves = c->waves > 0 ? c->waves : 1;
+    a.prefetch = (c->dims[0] % SB == 0) ? c->prefetch : 0;
     a.stream = c->stream;
     a.U = U; a.in = in; a.out = out; a.kappa = kappa; a.r = r;
     a.sc = c->sc; a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = it;
@@ -223,6 +262,7 @@ extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_
     c->tile_user = -1;
     c->tile = auto_tile(c);
     c->l2_budget_mb = 40.0;
+    c->prefetch = 0;   // measured on B200: bulk L2 prefetch of the next tile slows the stencil by 15-30 %
     bool ok = true;
     ok = ok && cudaMalloc(&c->sc, sizeof(CgScalars)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->counter, sizeof(unsigned int)) == cudaSuccess;
@@ -292,6 +332,18 @@ extern "C" int wd_set_tile(wd_ctx *c, int index)
     return WD_OK;
 }
 extern "C" int wd_get_tile(wd_ctx *c) { return c ? c->tile : WD_ERR_ARG; }
+extern "C" int wd_set_prefetch(wd_ctx *c, int tiles)
+{
+    if (!c || tiles < -1) return WD_ERR_ARG;
+    c->prefetch = tiles;
+    return WD_OK;
+}
+extern "C" int wd_set_waves(wd_ctx *c, int waves)
+{
+    if (!c || waves < 0) return WD_ERR_ARG;
+    c->waves = waves;
+    return WD_OK;
+}
 extern "C" int wd_set_zchunk(wd_ctx *c, int layers)
 {
     if (!c || layers < 0) return WD_ERR_ARG;

@@ -21,13 +21,36 @@
 
 namespace wd {
 
+// Division by a run-time constant d >= 1 of n < 2^31: q = (n * M) >> (32 + sh), M = ceil(2^(31+ceil(log2 d)) / d)
+// (two instructions instead of the ~20 of an emulated integer division; the tile decode does five per tile).
+struct FastDiv {
+    unsigned int d, M;
+    int sh;   // -1 encodes d == 1
+};
+__device__ __forceinline__ int fdiv(int n, const FastDiv &f)
+{
+    return f.sh < 0 ? n : (int)(__umulhi((unsigned int)n, f.M) >> f.sh);
+}
+
 struct Geom {
     int L[4];    // Lx, Ly, Lz, Lt
     int V;       // volume = plane stride
     int nt[4];   // tiles per direction (ceil)
     int bc_t;    // -1 antiperiodic, +1 periodic
     int zc;      // z tiles per chunk of the CTA rasterisation (see tile_of_block)
+    int ntiles;  // nt[0]*nt[1]*nt[2]*nt[3]
+    int pf;      // L2 prefetch distance in tiles (0 = off; needs Lx % 16 == 0 so that a 16-site run is one block)
+    FastDiv d_chunk, d_nt0, d_nt1, d_zc, d_zlast;   // per_chunk, nt[0], nt[1], zc, size of the last z chunk
 };
+
+// Bulk prefetch of `bytes` (multiple of 16) contiguous bytes into L2 (sm_90+: cp.async.bulk.prefetch.L2).
+// It holds no register and no shared memory while in flight: the DRAM latency of the NEXT tile is paid by L2,
+// and the loads of that tile later hit L2 (~1/3 of the DRAM latency), which is what the register-held
+// software pipeline of the hop loop can cover.
+__device__ __forceinline__ void prefetch_l2(const void *p, unsigned int bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
 
 // CTA rasterisation.  Tiles are visited x, y, z-within-chunk fastest, then t, then z-chunk: the sites a CTA
 // shares with its +-t neighbours (2 spinor layers and one layer of U_t per tile) are then touched again
@@ -36,16 +59,18 @@ struct Geom {
 // read twice from DRAM.  zc = nt[2] is the plain lexicographic order.
 __device__ __forceinline__ void tile_of_block(const Geom &g, int b, int &tx, int &ty, int &tz, int &tt)
 {
-    const int per_z = g.nt[0] * g.nt[1];
-    const int per_chunk = per_z * g.zc * g.nt[3];      // blocks of a full chunk
-    const int c = b / per_chunk;
-    int rem = b - c * per_chunk;
+    const int c = fdiv(b, g.d_chunk);
+    int rem = b - c * (int)g.d_chunk.d;
     const int z0 = c * g.zc;
-    const int zc = min(g.zc, g.nt[2] - z0);            // the last chunk may be shorter
-    tx = rem % g.nt[0]; rem /= g.nt[0];
-    ty = rem % g.nt[1]; rem /= g.nt[1];
-    tz = z0 + rem % zc;
-    tt = rem / zc;
+    const bool last = z0 + g.zc > g.nt[2];              // the last chunk may be shorter
+    int q = fdiv(rem, g.d_nt0);
+    tx = rem - q * g.nt[0]; rem = q;
+    q = fdiv(rem, g.d_nt1);
+    ty = rem - q * g.nt[1]; rem = q;
+    const FastDiv &dz = last ? g.d_zlast : g.d_zc;
+    q = fdiv(rem, dz);
+    tz = z0 + rem - q * (int)dz.d;
+    tt = q;
 }
 
 // Device-resident CG state.  All fp64 (reading G17).
@@ -75,16 +100,18 @@ template <> struct Field<double> {
 };
 
 // ---------------------------------------------------------------- site-blocked SoA addressing
-// Sites are grouped in blocks of SB = 32 consecutive lexicographic sites (x fastest).  Inside a block the
-// data is planar: spinor block = NSP planes x 32 sites x 128-bit vector (3 KB fp32), gauge block =
-// 36 planes (mu*9 + a*3+b) x 32 sites x one complex (9 KB fp32).  A warp reading one plane of one block
-// reads 512 (256) contiguous bytes, and every plane of a site is at a COMPILE-TIME offset from the
+// Sites are grouped in blocks of SB = 16 consecutive lexicographic sites (x fastest).  Inside a block the
+// data is planar: spinor block = NSP planes x 16 sites x 128-bit vector (1.5 KB fp32), gauge block =
+// 36 planes (mu*9 + a*3+b) x 16 sites x one complex (4.5 KB fp32).  A half-warp reading one plane of one
+// block reads 256 (128) contiguous, aligned bytes, a whole block is ONE contiguous chunk (so the next
+// tile can be pulled into L2 with one bulk prefetch per block), and every plane of a site is at a
+// COMPILE-TIME offset from the
 // site's base address, so the 15 loads of a hop share one address register and use immediate offsets
 // (the site-planar layout with stride V cost ~30 % of all issued instructions in address arithmetic).
-// The volume is padded up to a multiple of 32 sites; pad lanes are never read as sites and are skipped
+// The volume is padded up to a multiple of 16 sites; pad lanes are never read as sites and are skipped
 // by the vector kernels.
-constexpr int SB = 32;
-constexpr int SB_SHIFT = 5;
+constexpr int SB = 16;
+constexpr int SB_SHIFT = 4;
 
 template <typename svec, int NSP>
 __device__ __forceinline__ size_t spinor_index(int s)
@@ -143,15 +170,49 @@ __device__ __forceinline__ void store_spinor(double2 *base, int s, const double 
 #pragma unroll
     for (int j = 0; j < 12; ++j) p[j * SB] = make_double2(v[2 * j], v[2 * j + 1]);
 }
-template <int MU, typename gvec, typename real>
-__device__ __forceinline__ void load_link(const gvec *__restrict__ U, int s, real u[18])
+// Link U_mu(s): 18 reals u[(a*3+b)*2 + ri].  Inside the site block the link mu occupies 9*SB complex slots
+// (1152 B fp32): fp64 = 9 planes of double2 (one complex each); fp32 = 4 planes of float4 (reals 4q..4q+3,
+// i.e. two complex entries) followed by one plane of float2 (reals 16, 17), so that a link is 4 x 128-bit +
+// 1 x 64-bit loads instead of 9 x 64-bit.
+template <int MU>
+__device__ __forceinline__ void load_link(const double2 *__restrict__ U, int s, double u[18])
 {
-    const gvec *p = U + gauge_index(s) + MU * 9 * SB;
+    const double2 *p = U + gauge_index(s) + MU * 9 * SB;
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
-        const gvec t = __ldg(p + k * SB);
+        const double2 t = __ldg(p + k * SB);
         u[2 * k] = t.x; u[2 * k + 1] = t.y;
     }
+}
+template <int MU>
+__device__ __forceinline__ void load_link(const float2 *__restrict__ U, int s, float u[18])
+{
+    const float2 *blk = U + (size_t)(s >> SB_SHIFT) * (36 * SB) + MU * 9 * SB;
+    const int lane = s & (SB - 1);
+    const float4 *p4 = reinterpret_cast<const float4 *>(blk) + lane;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float4 t = __ldg(p4 + q * SB);
+        u[4 * q] = t.x; u[4 * q + 1] = t.y; u[4 * q + 2] = t.z; u[4 * q + 3] = t.w;
+    }
+    const float2 t2 = __ldg(blk + 8 * SB + lane);
+    u[16] = t2.x; u[17] = t2.y;
+}
+// the same slots, written by the pack kernel
+__device__ __forceinline__ void store_link(double2 *U, int s, int mu, const double2 k9[9])
+{
+    double2 *p = U + gauge_index(s) + mu * 9 * SB;
+#pragma unroll
+    for (int k = 0; k < 9; ++k) p[k * SB] = k9[k];
+}
+__device__ __forceinline__ void store_link(float2 *U, int s, int mu, const float2 k9[9])
+{
+    float2 *blk = U + (size_t)(s >> SB_SHIFT) * (36 * SB) + mu * 9 * SB;
+    const int lane = s & (SB - 1);
+    float4 *p4 = reinterpret_cast<float4 *>(blk) + lane;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) p4[q * SB] = make_float4(k9[2 * q].x, k9[2 * q].y, k9[2 * q + 1].x, k9[2 * q + 1].y);
+    blk[8 * SB + lane] = k9[8];
 }
 
 // ---------------------------------------------------------------- spin projection (reading C-2)
@@ -249,7 +310,7 @@ __device__ __forceinline__ void hop_load(const gvec *__restrict__ U, const svec 
                                          int link_site, int spinor_site, real v[24], real u[18])
 {
     load_spinor(in, spinor_site, v);
-    load_link<MU, gvec, real>(U, link_site, u);
+    load_link<MU>(U, link_site, u);
 }
 template <int MU, int S, bool ADJ, typename real>
 __device__ __forceinline__ void hop_compute(const real v[24], const real u[18], real sg, real acc[24])
@@ -285,9 +346,11 @@ __device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, i
 // PIPE = 0: hop after hop (load, compute).  PIPE = 1: software pipeline, two register buffers: the loads of
 // hop k+1 are issued before hop k is computed, so every thread keeps one hop (168 B fp32) in flight while
 // it computes (memory-level parallelism without more threads).
-template <int DAG, int PIPE, typename real, typename svec, typename gvec>
+// LOADR: also fetch r(s) into rv together with the centre spinor (MODE_RUPD), so that it too overlaps the last hop.
+template <int DAG, int PIPE, bool LOADR, typename real, typename svec, typename gvec>
 __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const svec *__restrict__ in,
-                                            int x, int y, int z, int t, int s, real acc[24], real c[24])
+                                            const svec *r, int x, int y, int z, int t, int s, real acc[24],
+                                            real c[24], real rv[24])
 {
     constexpr int SF = DAG ? +1 : -1;
     const Hops n = neighbours(g, x, y, z, t, s);
@@ -308,7 +371,8 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
         hop_load<3, real>(U, in, s, n.f[3], v, u);       hop_compute<3, SF, false, real>(v, u, sgf, acc);
         hop_load<3, real>(U, in, n.b[3], n.b[3], v, u);  hop_compute<3, -SF, true, real>(v, u, sgb, acc);
         load_spinor(in, s, c);
-    } else {
+        if (LOADR) load_spinor_rw(r, s, rv);
+    } else if (PIPE == 1) {
         real va[24], ua[18], vb[24], ub[18];
         hop_load<0, real>(U, in, s, n.f[0], va, ua);
         hop_load<0, real>(U, in, n.b[0], n.b[0], vb, ub);  hop_compute<0, SF, false, real>(va, ua, one, acc);
@@ -318,7 +382,24 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
         hop_load<2, real>(U, in, n.b[2], n.b[2], vb, ub);  hop_compute<2, SF, false, real>(va, ua, one, acc);
         hop_load<3, real>(U, in, s, n.f[3], va, ua);       hop_compute<2, -SF, true, real>(vb, ub, one, acc);
         hop_load<3, real>(U, in, n.b[3], n.b[3], vb, ub);  hop_compute<3, SF, false, real>(va, ua, sgf, acc);
-        load_spinor(in, s, c);                             hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
+        load_spinor(in, s, c);
+        hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
+        if (LOADR) load_spinor_rw(r, s, rv);   // after the last hop: an earlier fetch costs registers (spills at 128)
+    } else if (PIPE == 2) {
+        // three register buffers: two hops (336 B fp32 per thread) in flight while a third is computed
+        real va[24], ua[18], vb[24], ub[18], vc[24], uc[18];
+        hop_load<0, real>(U, in, s, n.f[0], va, ua);
+        hop_load<0, real>(U, in, n.b[0], n.b[0], vb, ub);
+        hop_load<1, real>(U, in, s, n.f[1], vc, uc);          hop_compute<0, SF, false, real>(va, ua, one, acc);
+        hop_load<1, real>(U, in, n.b[1], n.b[1], va, ua);     hop_compute<0, -SF, true, real>(vb, ub, one, acc);
+        hop_load<2, real>(U, in, s, n.f[2], vb, ub);          hop_compute<1, SF, false, real>(vc, uc, one, acc);
+        hop_load<2, real>(U, in, n.b[2], n.b[2], vc, uc);     hop_compute<1, -SF, true, real>(va, ua, one, acc);
+        hop_load<3, real>(U, in, s, n.f[3], va, ua);          hop_compute<2, SF, false, real>(vb, ub, one, acc);
+        hop_load<3, real>(U, in, n.b[3], n.b[3], vb, ub);     hop_compute<2, -SF, true, real>(vc, uc, one, acc);
+        load_spinor(in, s, c);
+        if (LOADR) load_spinor_rw(r, s, rv);
+        hop_compute<3, SF, false, real>(va, ua, sgf, acc);
+        hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
     }
 }
 
@@ -410,25 +491,37 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     if (MODE != MODE_PLAIN) {
         if (it >= sc->k_stop) return;  // uniform over the grid: over-launched iterations are no-ops
     }
-    int tx, ty, tz, tt;
-    tile_of_block(g, blockIdx.x, tx, ty, tz, tt);
     const int tid = threadIdx.x;
-    const int x = tx * BX + tid % BX;
-    const int y = ty * BY + (tid / BX) % BY;
-    const int z = tz * BZ + (tid / (BX * BY)) % BZ;
-    const int t = tt * BT + tid / (BX * BY * BZ);
-    const bool active = (x < g.L[0]) && (y < g.L[1]) && (z < g.L[2]) && (t < g.L[3]);
+    const int lx = tid % BX, ly = (tid / BX) % BY, lz = (tid / (BX * BY)) % BZ, lt = tid / (BX * BY * BZ);
+    const real alpha = (MODE == MODE_RUPD) ? (real)sc->alpha : (real)0;
     double local = 0.0;
-    if (active) {
+    // Persistent CTAs: the grid is one resident wave; CTA i takes tiles i, i + gridDim.x, ... so that at any
+    // moment the chip works on gridDim.x consecutive tiles of the rasterisation (L2 locality) and the
+    // reduction epilogue (barriers, fence, ticket) is paid once per CTA, not once per tile.
+    for (int b = blockIdx.x; b < g.ntiles; b += gridDim.x) {
+        int tx, ty, tz, tt;
+        if (BX % SB == 0 && g.pf > 0 && (lx % SB) == 0 && b + g.pf < g.ntiles) {
+            // one thread per 16-site run of the tile `pf` tiles ahead: its spinor block, its gauge block (and r)
+            tile_of_block(g, b + g.pf, tx, ty, tz, tt);
+            const int px = tx * BX + lx, py = ty * BY + ly, pz = tz * BZ + lz, pt = tt * BT + lt;
+            if (px < g.L[0] && py < g.L[1] && pz < g.L[2] && pt < g.L[3]) {
+                const int ps = px + g.L[0] * (py + g.L[1] * (pz + g.L[2] * pt));
+                prefetch_l2(in + spinor_index<svec, Field<real>::NSP>(ps), Field<real>::NSP * SB * sizeof(svec));
+                prefetch_l2(U + gauge_index(ps), 36 * SB * sizeof(gvec));
+                if (MODE == MODE_RUPD)
+                    prefetch_l2(r + spinor_index<svec, Field<real>::NSP>(ps), Field<real>::NSP * SB * sizeof(svec));
+            }
+        }
+        tile_of_block(g, b, tx, ty, tz, tt);
+        const int x = tx * BX + lx, y = ty * BY + ly, z = tz * BZ + lz, t = tt * BT + lt;
+        const bool active = (x < g.L[0]) && (y < g.L[1]) && (z < g.L[2]) && (t < g.L[3]);
+        if (!active) continue;
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
-        real acc[24], c[24];
-        hopping_sum<DAG, PIPE, real, svec, gvec>(g, U, in, x, y, z, t, s, acc, c);
+        real acc[24], c[24], rv[24];
+        hopping_sum<DAG, PIPE, MODE == MODE_RUPD, real, svec, gvec>(g, U, in, r, x, y, z, t, s, acc, c, rv);
 #pragma unroll
         for (int i = 0; i < 24; ++i) c[i] = fma(-kappa, acc[i], c[i]);  // (D in)(x) = in(x) - kappa * hops
         if (MODE == MODE_RUPD) {
-            const real alpha = (real)sc->alpha;
-            real rv[24];
-            load_spinor_rw(r, s, rv);
             real n2 = 0;
 #pragma unroll
             for (int i = 0; i < 24; ++i) {
@@ -436,14 +529,14 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
                 n2 = fma(rv[i], rv[i], n2);
             }
             store_spinor(r, s, rv);
-            local = (double)n2;
+            local += (double)n2;
         } else {
             store_spinor(out, s, c);
             if (MODE == MODE_QQ) {
                 real n2 = 0;
 #pragma unroll
                 for (int i = 0; i < 24; ++i) n2 = fma(c[i], c[i], n2);
-                local = (double)n2;
+                local += (double)n2;
             }
         }
     }
@@ -556,12 +649,11 @@ pack_gauge_kernel(const typename Field<real>::gvec *__restrict__ can, typename F
     using gvec = typename Field<real>::gvec;
     const int s = blockIdx.x * VEC_NT + threadIdx.x;
     if (s >= Vpad) return;
-    gvec *p = nat + gauge_index(s);
-    if (s < V) {
-#pragma unroll 4
-        for (int k = 0; k < 36; ++k) p[k * SB] = __ldg(can + (size_t)s * 36 + k);
-    } else {
-        for (int k = 0; k < 36; ++k) p[k * SB] = gvec();
+    for (int mu = 0; mu < 4; ++mu) {
+        gvec k9[9];
+#pragma unroll
+        for (int k = 0; k < 9; ++k) k9[k] = s < V ? __ldg(can + (size_t)s * 36 + mu * 9 + k) : gvec();
+        store_link(nat, s, mu, k9);
     }
 }
 template <typename real>

@@ -1,7 +1,7 @@
 // wilson_launch.cuh — the table of compiled stencil launch configurations and the per-precision launchers.
 // A "tile" (the name of the C ABI, wd_set_tile) is one row: CTA tile BX x BY x BZ x BT (threads per CTA =
 // product), MINB = minimum resident CTAs per SM asked of ptxas (bounds registers per thread), PIPE = 1 for
-// the software-pipelined hop loop.  This is the CUDA analogue of the paper's workgroup-size knob
+// the software-pipelined hop loop (2 = three register buffers).  This is the CUDA analogue of the paper's workgroup-size knob
 // (PAPER.md:58,76).  F64 = 1 if the row is also compiled for double precision.
 #pragma once
 #include "wilson_kernels.cuh"
@@ -10,23 +10,23 @@
 // with the fewest padded threads for the lattice and precision at hand.
 //   X(index, BX, BY, BZ, BT, MINB, PIPE, F64)
 #define WD_TILE_TABLE(X) \
-    X(0, 32, 2, 2, 1, 4, 1, 0) \
-    X(1, 16, 2, 2, 2, 4, 1, 0) \
-    X(2, 32, 2, 2, 2, 2, 1, 0) \
-    X(3, 32, 2, 1, 1, 8, 1, 0) \
-    X(4, 16, 2, 4, 2, 2, 1, 0) \
-    X(5, 16, 4, 2, 2, 2, 1, 0) \
+    X(0, 16, 2, 2, 2, 4, 1, 0) \
+    X(1, 16, 4, 4, 2, 1, 1, 0) \
+    X(2, 32, 2, 2, 1, 4, 1, 0) \
+    X(3, 16, 2, 4, 2, 2, 1, 0) \
+    X(4, 16, 4, 2, 2, 2, 1, 0) \
+    X(5, 32, 2, 4, 2, 1, 1, 0) \
     X(6, 8, 4, 2, 2, 4, 1, 0) \
-    X(7, 16, 2, 2, 1, 8, 1, 0) \
-    X(8, 32, 2, 2, 1, 2, 1, 1) \
-    X(9, 16, 2, 2, 1, 4, 1, 1) \
-    X(10, 16, 2, 2, 2, 2, 1, 1) \
-    X(11, 8, 4, 2, 1, 4, 1, 1) \
-    X(12, 8, 2, 2, 2, 4, 1, 1) \
-    X(13, 4, 4, 2, 2, 4, 1, 1) \
-    X(14, 4, 4, 4, 2, 2, 1, 1) \
-    X(15, 16, 2, 2, 2, 0, 0, 1) \
-    X(16, 8, 4, 4, 2, 0, 0, 1)
+    X(7, 32, 2, 2, 1, 2, 1, 1) \
+    X(8, 16, 2, 2, 1, 3, 1, 1) \
+    X(9, 16, 2, 2, 2, 2, 1, 1) \
+    X(10, 8, 4, 2, 1, 4, 1, 1) \
+    X(11, 8, 2, 2, 2, 4, 1, 1) \
+    X(12, 4, 4, 2, 2, 4, 1, 1) \
+    X(13, 4, 4, 4, 2, 2, 1, 1) \
+    X(14, 16, 2, 2, 2, 0, 0, 1) \
+    X(15, 8, 4, 4, 2, 0, 0, 1) \
+    X(16, 16, 2, 2, 2, 3, 2, 0)
 #define WD_NUM_TILES 17
 
 namespace wd {
@@ -43,7 +43,9 @@ static const TileInfo kTiles[WD_NUM_TILES] = {
 
 struct DslashArgs {
     Geom g;
-    unsigned int grid;
+    int sm_count;
+    int waves;      // resident waves of CTAs to launch (persistent grid = waves * SMs * CTAs per SM), >= 1
+    int prefetch;   // L2 prefetch distance in tiles: -1 = one grid ahead, 0 = off
     cudaStream_t stream;
     const void *U;
     const void *in;
@@ -70,8 +72,19 @@ static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
 #define X(i, bx, by, bz, bt, m, p, f)                                                                          \
     case i:                                                                                                    \
         if constexpr (sizeof(real) == 4 || f) {                                                                \
-            dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p><<<a.grid, bx * by * bz * bt, 0, a.stream>>>(  \
-                a.g, (const gvec *)a.U, (const svec *)a.in, (svec *)a.out, (real)a.kappa, (svec *)a.r, a.sc,   \
+            static int occ = 0;                                                                                \
+            if (!occ) {                                                                                        \
+                cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(                                 \
+                    &occ, dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p>, bx * by * bz * bt, 0);         \
+                if (e != cudaSuccess) return e;                                                                \
+                if (occ < 1) occ = 1;                                                                          \
+            }                                                                                                  \
+            long grid = (long)occ * a.sm_count * a.waves;                                                      \
+            if (grid > a.g.ntiles) grid = a.g.ntiles;                                                          \
+            Geom g = a.g;                                                                                      \
+            g.pf = a.prefetch < 0 ? (int)grid : a.prefetch;                                                    \
+            dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p><<<(unsigned)grid, bx * by * bz * bt, 0, a.stream>>>(  \
+                g, (const gvec *)a.U, (const svec *)a.in, (svec *)a.out, (real)a.kappa, (svec *)a.r, a.sc,   \
                 a.partials, a.counter, a.hist, a.it);                                                          \
             return cudaGetLastError();                                                                         \
         }                                                                                                      \

@@ -86,10 +86,14 @@ def load_library(path: str = LIB_PATH):
     lib.wd_tile_info.argtypes = [ci, ip]
     lib.wd_set_tile.argtypes = [vp, ci]
     lib.wd_get_tile.argtypes = [vp]
+    lib.wd_set_prefetch.argtypes = [vp, ci]
+    lib.wd_set_waves.argtypes = [vp, ci]
     lib.wd_set_zchunk.argtypes = [vp, ci]
     lib.wd_set_poll_interval.argtypes = [vp, ci]
     lib.wd_set_profile.argtypes = [vp, ci]
     lib.wd_get_profile.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_long)]
+    lib.wd_selftest_fastdiv.argtypes = [ctypes.c_uint, ctypes.c_uint]
+    lib.wd_selftest_fastdiv.restype = ctypes.c_long
     lib.wd_version.argtypes = []
     lib.wd_version.restype = ctypes.c_char_p
     _lib = lib
@@ -292,6 +296,12 @@ class WilsonContext:
         n = ctypes.c_long()
         self._check(self.lib.wd_get_profile(self._ctx, ms, ctypes.byref(n)))
         return {"a2_ms": ms[0], "a3_ms": ms[1], "a4_ms": ms[2], "iterations": n.value}
+
+    def wd_set_prefetch(self, tiles):
+        self._check(self.lib.wd_set_prefetch(self._ctx, int(tiles)))
+
+    def wd_set_waves(self, waves):
+        self._check(self.lib.wd_set_waves(self._ctx, int(waves)))
 
     def wd_set_zchunk(self, layers):
         self._check(self.lib.wd_set_zchunk(self._ctx, int(layers)))

@@ -74,3 +74,12 @@ def test_product_package_does_not_import_the_oracle():
             if fn.endswith((".py", ".cu", ".cuh", ".h")):
                 text = open(os.path.join(dirpath, fn)).read()
                 assert "wilson_oracle" not in text and "from oracle" not in text and "import oracle" not in text, fn
+
+
+def test_fastdiv_constants_of_the_tile_decode(lib):
+    """host logic: (n*M) >> (32+sh) == n // d for every divisor the tile decode can meet and every n that can occur"""
+    for d in list(range(1, 200)) + [255, 256, 257, 1000, 4095, 4096, 4097, 82944, 663552, 1 << 20, (1 << 24) - 1]:
+        assert lib.wd_selftest_fastdiv(d, 300000) == 0, d
+    for d in (3, 7, 24, 48, 96, 576, 13824):
+        assert lib.wd_selftest_fastdiv(d, 1 << 24) == 0, d
+    assert lib.wd_selftest_fastdiv(0, 10) == -1

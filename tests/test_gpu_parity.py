@@ -60,18 +60,26 @@ def test_pack_unpack_are_exact_permutations(wilson, precision, dims):
         back = gu.to_host(ctx.wd_unpack_spinor(pn))
         pn_h, Un_h = gu.to_host(pn), gu.to_host(Un)
     assert back.tobytes() == psi.tobytes()
-    # native layout (include/wilson_cg.h): blocks of 32 lexicographic sites; inside a block the spinor is NSP
+    # native layout (include/wilson_cg.h): blocks of 16 lexicographic sites; inside a block the spinor is NSP
     # planes of 128-bit vectors, the gauge field 36 planes (mu*9 + a*3+b) of one complex; pad lanes are zero
-    nblk = (V + 31) // 32
-    Vp = nblk * 32
+    nblk = (V + 15) // 16
+    Vp = nblk * 16
     nsp, w = (6, 4) if precision == 32 else (12, 2)
     want = np.zeros((Vp, nsp, w), dtype=rdt)
     want[:V] = psi.view(rdt).reshape(V, nsp, w)
-    want = want.reshape(nblk, 32, nsp, w).transpose(0, 2, 1, 3)
+    want = want.reshape(nblk, 16, nsp, w).transpose(0, 2, 1, 3)
     assert pn_h.size == Vp * 24 and pn_h.tobytes() == np.ascontiguousarray(want).tobytes()
-    want_u = np.zeros((Vp, 36, 2), dtype=rdt)
-    want_u[:V] = U.view(rdt).reshape(V, 36, 2)
-    want_u = want_u.reshape(nblk, 32, 36, 2).transpose(0, 2, 1, 3)
+    # gauge block = 4 links x (9 complex x 16 sites); fp64: 9 planes of one complex; fp32: 4 planes of float4
+    # (reals 4q..4q+3) followed by one plane of float2 (reals 16, 17)
+    u18 = np.zeros((Vp, 4, 18), dtype=rdt)
+    u18[:V] = U.view(rdt).reshape(V, 4, 18)
+    u18 = u18.reshape(nblk, 16, 4, 18).transpose(0, 2, 1, 3)          # [blk][mu][site][18]
+    if precision == 64:
+        want_u = u18.reshape(nblk, 4, 16, 9, 2).transpose(0, 1, 3, 2, 4)
+    else:
+        head = u18[..., :16].reshape(nblk, 4, 16, 4, 4).transpose(0, 1, 3, 2, 4).reshape(nblk, 4, 256)
+        tail = u18[..., 16:].reshape(nblk, 4, 32)
+        want_u = np.concatenate([head, tail], axis=2)
     assert Un_h.size == Vp * 72 and Un_h.tobytes() == np.ascontiguousarray(want_u).tobytes()
 
 
