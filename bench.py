@@ -49,6 +49,28 @@ def cg_flops(volume, iterations):
     return float(volume) * (FLOP_ITER * iterations + FLOP_APPLY)
 
 
+def workload_name(cfg, r_min):
+    return (f"config{cfg.index}: {cfg.name} Wilson CG on D D-dagger, kappa={cfg.kappa}, links={cfg.links}, "
+            f"r_min={r_min:g}, antiperiodic t")
+
+
+def max_over_ranks(x, dist=None, device="cpu"):
+    """Time-like quantity -> max over all ranks (the slowest rank bounds the job).  dist = torch.distributed or None."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(x)
+    import torch
+
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world, volume, iterations, seconds):
+    """Replicas only: every rank solves the same lattice, so the job's flops are world x one solve; the time is
+    the max over ranks."""
+    return world * cg_flops(volume, iterations) / seconds / 1e9
+
+
 def measured_peak():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -140,13 +162,54 @@ def run_reference(args, cfg):
         "impl": "reference", "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"config{cfg.index}: {cfg.name} Wilson CG, kappa={cfg.kappa}, links={cfg.links}",
-                   "precision": args.precision},
+        "config": {"workload": workload_name(cfg, cfg.r_min if args.precision == 32 else 1e-10), "volume": cfg.volume,
+                   "sample_cg_iterations": its, "parallelism": "host cores (oracle)"},
         "cpu_baseline": {"value": value, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_sweep(args, cfg, ctx, wilson, Un, en, psi_n, r_min):
+    """Per launch configuration: device time of a2 / a3 / a4 per CG iteration (CUDA events inside the solve) and
+    of a standalone wd_apply, as achieved algorithmic GB/s."""
+    import torch
+
+    V = cfg.volume
+    b2, b3, b4 = (480, 576, 480) if args.precision == 32 else (960, 1152, 960)
+    for tile, inf in enumerate(wilson.tile_infos()):
+        try:
+            ctx.wd_set_tile(tile)
+        except wilson.WilsonError:
+            continue  # not compiled for this precision
+        ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=psi_n)
+        ctx.wd_set_profile(True)
+        for _ in range(max(1, args.steps)):
+            _, info = ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=psi_n)
+        p = ctx.wd_get_profile()
+        ctx.wd_set_profile(False)
+        n = max(p["iterations"], 1)
+        a2, a3, a4 = p["a2_ms"] / n, p["a3_ms"] / n, p["a4_ms"] / n
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 100
+        e0.record()
+        for _ in range(reps):
+            ctx.wd_apply(Un, en, cfg.kappa, False, out=psi_n)
+        e1.record()
+        torch.cuda.synchronize()
+        ap_ms = e0.elapsed_time(e1) / reps
+        gbs = lambda b, ms: b * V / (ms * 1e-3) / 1e9 if ms > 0 else None
+        print(json.dumps({
+            "sweep": f"config{cfg.index}", "precision": args.precision, "tile_index": tile, "tile": list(inf[:4]),
+            "threads": inf[0] * inf[1] * inf[2] * inf[3], "min_blocks_per_sm": inf[4], "pipeline": inf[5],
+            "iterations": info["iterations"], "a2_us": a2 * 1e3, "a3_us": a3 * 1e3, "a4_us": a4 * 1e3,
+            "a2_gbs": gbs(b2, a2), "a3_gbs": gbs(b3, a3), "a4_gbs": gbs(b4, a4),
+            "cg_iteration_gbs": gbs(b2 + b3 + b4, a2 + a3 + a4), "solve_ms": info["gpu_ms"],
+            "wd_apply_x100_us": ap_ms * 1e3, "wd_apply_gbs": gbs(b2, ap_ms),
+            "wd_apply_gflops": FLOP_APPLY * V / (ap_ms * 1e-3) / 1e9}), flush=True)
+    ctx.close()
     return 0
 
 
@@ -160,6 +223,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--tile", type=int, default=-1, help="CTA tile index (-1 = library's automatic choice)")
     ap.add_argument("--sample-iters", type=int, default=2, help="CG iterations of the oracle's bounded sample")
+    ap.add_argument("--sweep", action="store_true",
+                    help="time every compiled launch configuration (the paper's workgroup-size tuning, PAPER.md:76) "
+                         "on this config and print one JSON line per configuration instead of the bench line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -212,6 +278,9 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
+    if args.sweep:
+        return run_sweep(args, cfg, ctx, wilson, Un, en, psi_n, r_min)
+
     # ---------------- device-resident arm
     for _ in range(args.warmup):
         ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=psi_n)
@@ -232,12 +301,9 @@ def main():
     ms_total = e0.elapsed_time(e1)
     prof = ctx.wd_get_profile()
     ctx.wd_set_profile(False)
-    if dist:
-        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dist, "cuda")
     ms_step = ms_total / args.steps
-    value = world * cg_flops(V, iters) / (ms_step * 1e-3) / 1e9
+    value = whole_job_value(world, V, iters, ms_step * 1e-3)
 
     # ---------------- roofline of the dominant kernel (a3), timed live inside the steps above
     peak, peak_src = measured_peak()
@@ -272,11 +338,8 @@ def main():
             _, info_h = ctx.cg_solve_host(U_pin, eta_pin, cfg.kappa, r_min, cfg.max_iter, out=psi_pin)
         barrier()
         dt = (time.perf_counter() - t0) / n_e2e
-        if dist:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": world * cg_flops(V, info_h["iterations"]) / dt / 1e9, "unit": "GFLOP/s",
+        dt = max_over_ranks(dt, dist, "cuda")
+        e2e = {"value": whole_job_value(world, V, info_h["iterations"], dt), "unit": "GFLOP/s",
                "h2d_bytes_per_step": int(U.nbytes + eta.nbytes), "d2h_bytes_per_step": int(eta.nbytes),
                "ms_per_step": dt * 1e3, "steps": n_e2e}
         del U_pin, eta_pin, psi_pin
@@ -293,9 +356,7 @@ def main():
         "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32" if args.precision == 32 else "f64", "data": "synthetic",
-        "config": {"workload": f"config{cfg.index}: {cfg.name} Wilson CG on D D-dagger, kappa={cfg.kappa}, "
-                               f"links={cfg.links}, r_min={r_min:g}, antiperiodic t",
-                   "volume": V, "cg_iterations": iters, "tile": list(wilson.tile_shapes()[ctx.wd_get_tile()]),
+        "config": {"workload": workload_name(cfg, r_min), "volume": V, "cg_iterations": iters, "tile": list(wilson.tile_shapes()[ctx.wd_get_tile()]),
                    "l2_policy": f"inputs larger than L2 (working set {ws_bytes / 1e6:.0f} MB vs 126 MB L2)"
                    if ws_bytes > 2 * 126e6 else "working set fits L2 (latency-bound regime, no roofline claim)",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
