@@ -80,7 +80,7 @@ typedef struct wd_cg_info {
     double gpu_ms;         /* device time of init + loop + final D-dagger (CUDA events on the ctx stream) */
     double total_ms;       /* *_host calls: device time including H2D copies, pack, solve, unpack, D2H; else = gpu_ms */
     int kernel_launches;   /* number of this library's kernels launched by the call */
-    int reserved;
+    int cg_mode;           /* 1 = three kernels per iteration, 2 = whole solve in one cooperative launch */
 } wd_cg_info;
 
 /*
@@ -176,6 +176,9 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *                             software-pipelined, 1 if also compiled for precision 64}.
  *   wd_set_tile(ctx, i)       select tile i for the stencil kernels of this ctx; i = -1 restores the automatic choice.
  *   wd_get_tile(ctx)          index in use.
+ *   wd_set_cg_mode(ctx, m)        0 = automatic (one cooperative launch for the whole solve when V <= 65536 sites in fp32 /
+ *                             32768 in fp64 — the paper's own 4^4..14^4 range — else three kernels per iteration), 1 = always three kernels,
+ *                             2 = always one launch (grid barriers between the phases; same recurrence and precision).
  *   wd_set_prefetch(ctx, n)       L2 bulk-prefetch distance of the stencil kernels in tiles: 0 = off (default: it measured
  *                             slower on B200), -1 = each CTA prefetches the tile it will process next, n > 0 = n tiles ahead.
  *   wd_set_waves(ctx, w)          the stencil kernels run a persistent grid of w * (SMs * resident CTAs per SM) CTAs that
@@ -189,6 +192,7 @@ int wd_tile_shape(int index, int shape[4]);
 int wd_tile_info(int index, int info[3]);
 int wd_set_tile(wd_ctx *ctx, int index);
 int wd_get_tile(wd_ctx *ctx);
+int wd_set_cg_mode(wd_ctx *ctx, int mode);
 int wd_set_prefetch(wd_ctx *ctx, int tiles);
 int wd_set_waves(wd_ctx *ctx, int waves);
 int wd_set_zchunk(wd_ctx *ctx, int layers);

@@ -12,6 +12,11 @@
 
 using namespace wd;
 
+// Largest volume solved by the one-launch CG kernel in automatic mode (sites).  Measured on B200 (profiles/).
+#ifndef WD_ONELAUNCH_MAX_SITES
+#define WD_ONELAUNCH_MAX_SITES 65536
+#endif
+
 struct wd_ctx {
     int dims[4];
     int V;
@@ -22,6 +27,9 @@ struct wd_ctx {
     int tile_user;  // -1 = automatic
     int poll;       // 0 = automatic
     int waves;            // resident waves of the persistent stencil grid (0 -> 1)
+    int cg_mode;          // 0 = automatic, 1 = three kernels per iteration, 2 = one cooperative launch
+    int coop_ok;          // device supports cooperative launches
+    int last_cg_mode;     // what the last cg_solve used
     int prefetch;         // L2 prefetch distance: -1 = automatic (one grid ahead), 0 = off, n > 0 = n tiles
     int zchunk_user;      // z layers per rasterisation chunk, 0 = automatic
     double l2_budget_mb;  // reuse-distance budget of the automatic choice
@@ -115,29 +123,31 @@ extern "C" long wd_selftest_fastdiv(unsigned int d, unsigned int n_max)
     return bad;
 }
 
-static Geom make_geom(const wd_ctx *c, int tile)
+static Geom make_geom_dims(const wd_ctx *c, const int tb[4], int zchunk_user);
+static Geom make_geom(const wd_ctx *c, int tile) { return make_geom_dims(c, kTiles[tile].b, c->zchunk_user); }
+static Geom make_geom_dims(const wd_ctx *c, const int tb[4], int zchunk_user)
 {
     Geom g;
     for (int d = 0; d < 4; ++d) {
         g.L[d] = c->dims[d];
-        g.nt[d] = (c->dims[d] + kTiles[tile].b[d] - 1) / kTiles[tile].b[d];
+        g.nt[d] = (c->dims[d] + tb[d] - 1) / tb[d];
     }
     g.V = c->V;
     g.bc_t = c->bc_t;
     // z chunk of the CTA rasterisation: the largest divisor of the z tile count whose t-reuse distance
     // Lx*Ly*(zc*BZ)*BT sites * ~600 B (spinor in/out, gauge, halos) stays within the L2 budget.
-    const double layer = 600.0 * c->dims[0] * c->dims[1] * kTiles[tile].b[3];   // bytes per z layer of one t-tile row
+    const double layer = 600.0 * c->dims[0] * c->dims[1] * tb[3];   // bytes per z layer of one t-tile row
     const double budget = c->l2_budget_mb * 1.0e6;
     int zc = 1;
-    if (c->zchunk_user > 0) {
-        zc = (c->zchunk_user + kTiles[tile].b[2] - 1) / kTiles[tile].b[2];
+    if (zchunk_user > 0) {
+        zc = (zchunk_user + tb[2] - 1) / tb[2];
         if (zc > g.nt[2]) zc = g.nt[2];
     } else {
         for (int d = 1; d <= g.nt[2]; ++d)
-            if (g.nt[2] % d == 0 && layer * d * kTiles[tile].b[2] <= budget) zc = d;
+            if (g.nt[2] % d == 0 && layer * d * tb[2] <= budget) zc = d;
     }
     g.zc = zc;
-    g.ntiles = (int)tile_blocks(c, tile);
+    g.ntiles = g.nt[0] * g.nt[1] * g.nt[2] * g.nt[3];
     g.pf = 0;   // set per launch (needs the grid size)
     g.d_chunk = make_fastdiv((unsigned)(g.nt[0] * g.nt[1] * g.zc * g.nt[3]));
     g.d_nt0 = make_fastdiv((unsigned)g.nt[0]);
@@ -217,7 +227,7 @@ static int ensure_partials(wd_ctx *c)
 {
     // enough for the largest grid any kernel of this ctx can use (smallest tile = 128 threads, no padding bound: use
     // the per-tile maximum) and the vector kernels
-    size_t need = (size_t)c->sm_count * 16;
+    size_t need = (size_t)c->sm_count * 32 * 3;   // one-launch CG: 3 buffers x (at most 32 resident CTAs per SM)
     for (int t = 0; t < WD_NUM_TILES; ++t) {
         const size_t nb = (size_t)tile_blocks(c, t);
         if (nb > need) need = nb;
@@ -259,6 +269,7 @@ extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_
     c->bc_t = bc_t;
     c->stream = (cudaStream_t)cuda_stream;
     c->sm_count = sms;
+    cudaDeviceGetAttribute(&c->coop_ok, cudaDevAttrCooperativeLaunch, dev);
     c->tile_user = -1;
     c->tile = auto_tile(c);
     c->l2_budget_mb = 40.0;
@@ -332,6 +343,13 @@ extern "C" int wd_set_tile(wd_ctx *c, int index)
     return WD_OK;
 }
 extern "C" int wd_get_tile(wd_ctx *c) { return c ? c->tile : WD_ERR_ARG; }
+extern "C" int wd_set_cg_mode(wd_ctx *c, int mode)
+{
+    if (!c || mode < 0 || mode > 2) return WD_ERR_ARG;
+    if (mode == 2 && !c->coop_ok) return fail(c, WD_ERR_CUDA, "wd_set_cg_mode: the device does not support cooperative launches");
+    c->cg_mode = mode;
+    return WD_OK;
+}
 extern "C" int wd_set_prefetch(wd_ctx *c, int tiles)
 {
     if (!c || tiles < -1) return WD_ERR_ARG;
@@ -457,11 +475,78 @@ static int auto_poll(const wd_ctx *c)
     return n;
 }
 
+// Small-volume path: the whole solve in one cooperative launch.
+static int small_tile_for(const wd_ctx *c)
+{
+    int best = 0;
+    double best_waste = 1e300;
+    for (int t = 0; t < WD_NUM_SMALL_TILES; ++t) {
+        double blocks = 1.0, threads = 1.0;
+        for (int d = 0; d < 4; ++d) {
+            blocks *= (c->dims[d] + kSmallTiles[t][d] - 1) / kSmallTiles[t][d];
+            threads *= kSmallTiles[t][d];
+        }
+        const double waste = blocks * threads / (double)c->V;
+        if (waste < best_waste - 1e-12) { best_waste = waste; best = t; }
+    }
+    return best;
+}
+
+static bool use_onelaunch(const wd_ctx *c)
+{
+    if (!c->coop_ok) return false;
+    if (c->cg_mode == 1) return false;
+    if (c->cg_mode == 2) return true;
+    // automatic: volumes whose CG iteration is shorter than three launches (measured crossover on B200: between
+    // 16^4 and 24^4 in fp32, between 14^4 and 16^4 in fp64)
+    return (long)c->V * (c->precision == 64 ? 2 : 1) <= WD_ONELAUNCH_MAX_SITES;
+}
+
+static int cg_onelaunch(wd_ctx *c, const void *U, const void *eta, void *psi, double kappa, double r_min, int max_iter)
+{
+    const int st = small_tile_for(c);
+    CgOneLaunchArgs a;
+    a.g = make_geom_dims(c, kSmallTiles[st], 0);
+    a.sm_count = c->sm_count;
+    a.stream = c->stream;
+    a.U = U; a.eta = eta; a.y = c->y; a.r = c->r; a.p = c->p; a.q = c->q; a.psi = psi;
+    a.kappa = kappa; a.sc = c->sc; a.partials = c->partials; a.partials_cap = c->partials_cap; a.hist = c->hist;
+    a.r_min = r_min; a.max_iter = max_iter;
+    c->launches++;
+    CUDA_TRY(c, c->precision == 32 ? launch_cg_onelaunch_f32(st, a) : launch_cg_onelaunch_f64(st, a));
+    return WD_OK;
+}
+
 static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, double kappa, double r_min, int max_iter,
                      wd_cg_info *info, bool record_events)
 {
     int rc = ensure_workspace(c, max_iter);
     if (rc != WD_OK) return rc;
+    if (use_onelaunch(c)) {
+        c->last_cg_mode = 2;
+        if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
+        rc = cg_onelaunch(c, U, eta, psi, kappa, r_min, max_iter);
+        if (rc != WD_OK) return rc;
+        if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
+        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        const CgScalars &s1 = *c->sc_host;
+        c->last_iters = s1.k;
+        if (info) {
+            info->iterations = s1.k;
+            info->converged = s1.converged;
+            info->rel_residual = s1.eta2 > 0.0 ? std::sqrt(s1.rr / s1.eta2) : 0.0;
+            info->eta_norm2 = s1.eta2;
+            float ms = 0.f;
+            if (record_events) CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]));
+            info->gpu_ms = ms;
+            info->total_ms = ms;
+            info->kernel_launches = c->launches;
+            info->cg_mode = 2;
+        }
+        return s1.converged ? WD_OK : WD_NOT_CONVERGED;
+    }
+    c->last_cg_mode = 1;
     const size_t n = spinor_vecs(c);
     const unsigned int vgrid = vec_grid(c, n);
     if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
@@ -540,7 +625,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
         info->gpu_ms = ms;
         info->total_ms = ms;
         info->kernel_launches = c->launches;
-        info->reserved = 0;
+        info->cg_mode = 1;
     }
     return s.converged ? WD_OK : WD_NOT_CONVERGED;
 }

@@ -5,4 +5,8 @@ cudaError_t launch_dslash_f32(int tile, int dagger, int mode, const DslashArgs &
 {
     return launch_dslash_any<float>(tile, dagger, mode, a);
 }
+cudaError_t launch_cg_onelaunch_f32(int small_tile, const CgOneLaunchArgs &a)
+{
+    return launch_cg_onelaunch_any<float>(small_tile, a);
+}
 }  // namespace wd

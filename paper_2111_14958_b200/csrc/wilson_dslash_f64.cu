@@ -5,4 +5,8 @@ cudaError_t launch_dslash_f64(int tile, int dagger, int mode, const DslashArgs &
 {
     return launch_dslash_any<double>(tile, dagger, mode, a);
 }
+cudaError_t launch_cg_onelaunch_f64(int small_tile, const CgOneLaunchArgs &a)
+{
+    return launch_cg_onelaunch_any<double>(small_tile, a);
+}
 }  // namespace wd

@@ -16,6 +16,7 @@
 // BX x BY x BZ x BT tile so that the 8 neighbours of most sites are fetched by the same CTA (L1 reuse) and
 // all loads of a warp are contiguous runs of BX sites.
 #pragma once
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -305,11 +306,19 @@ __device__ __forceinline__ void reconstruct(const real g[12], real sg, real acc[
 
 // One hop, split into its loads and its arithmetic so that the loads of the next hop can be in flight
 // while this one is computed:  acc += sg (1 + S gamma_MU) (x) [U or U^dagger](link_site) in(spinor_site).
-template <int MU, typename real, typename svec, typename gvec>
-__device__ __forceinline__ void hop_load(const gvec *__restrict__ U, const svec *__restrict__ in,
+// RO = true: `in` is not written while the kernel runs -> read-only (non-coherent) path; false: coherent loads
+// (the one-launch CG kernel reads fields other CTAs wrote before the last grid barrier).
+template <bool RO, typename svec, typename real>
+__device__ __forceinline__ void load_spinor_sel(const svec *in, int s, real v[24])
+{
+    if (RO) load_spinor(in, s, v);
+    else load_spinor_rw(in, s, v);
+}
+template <int MU, bool RO, typename real, typename svec, typename gvec>
+__device__ __forceinline__ void hop_load(const gvec *__restrict__ U, const svec *in,
                                          int link_site, int spinor_site, real v[24], real u[18])
 {
-    load_spinor(in, spinor_site, v);
+    load_spinor_sel<RO>(in, spinor_site, v);
     load_link<MU>(U, link_site, u);
 }
 template <int MU, int S, bool ADJ, typename real>
@@ -347,8 +356,8 @@ __device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, i
 // hop k+1 are issued before hop k is computed, so every thread keeps one hop (168 B fp32) in flight while
 // it computes (memory-level parallelism without more threads).
 // LOADR: also fetch r(s) into rv together with the centre spinor (MODE_RUPD), so that it too overlaps the last hop.
-template <int DAG, int PIPE, bool LOADR, typename real, typename svec, typename gvec>
-__device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const svec *__restrict__ in,
+template <int DAG, int PIPE, bool LOADR, bool RO, typename real, typename svec, typename gvec>
+__device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const svec *in,
                                             const svec *r, int x, int y, int z, int t, int s, real acc[24],
                                             real c[24], real rv[24])
 {
@@ -362,41 +371,41 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
     for (int i = 0; i < 24; ++i) acc[i] = 0;
     if (PIPE == 0) {
         real v[24], u[18];
-        hop_load<0, real>(U, in, s, n.f[0], v, u);       hop_compute<0, SF, false, real>(v, u, one, acc);
-        hop_load<0, real>(U, in, n.b[0], n.b[0], v, u);  hop_compute<0, -SF, true, real>(v, u, one, acc);
-        hop_load<1, real>(U, in, s, n.f[1], v, u);       hop_compute<1, SF, false, real>(v, u, one, acc);
-        hop_load<1, real>(U, in, n.b[1], n.b[1], v, u);  hop_compute<1, -SF, true, real>(v, u, one, acc);
-        hop_load<2, real>(U, in, s, n.f[2], v, u);       hop_compute<2, SF, false, real>(v, u, one, acc);
-        hop_load<2, real>(U, in, n.b[2], n.b[2], v, u);  hop_compute<2, -SF, true, real>(v, u, one, acc);
-        hop_load<3, real>(U, in, s, n.f[3], v, u);       hop_compute<3, SF, false, real>(v, u, sgf, acc);
-        hop_load<3, real>(U, in, n.b[3], n.b[3], v, u);  hop_compute<3, -SF, true, real>(v, u, sgb, acc);
-        load_spinor(in, s, c);
+        hop_load<0, RO, real>(U, in, s, n.f[0], v, u);       hop_compute<0, SF, false, real>(v, u, one, acc);
+        hop_load<0, RO, real>(U, in, n.b[0], n.b[0], v, u);  hop_compute<0, -SF, true, real>(v, u, one, acc);
+        hop_load<1, RO, real>(U, in, s, n.f[1], v, u);       hop_compute<1, SF, false, real>(v, u, one, acc);
+        hop_load<1, RO, real>(U, in, n.b[1], n.b[1], v, u);  hop_compute<1, -SF, true, real>(v, u, one, acc);
+        hop_load<2, RO, real>(U, in, s, n.f[2], v, u);       hop_compute<2, SF, false, real>(v, u, one, acc);
+        hop_load<2, RO, real>(U, in, n.b[2], n.b[2], v, u);  hop_compute<2, -SF, true, real>(v, u, one, acc);
+        hop_load<3, RO, real>(U, in, s, n.f[3], v, u);       hop_compute<3, SF, false, real>(v, u, sgf, acc);
+        hop_load<3, RO, real>(U, in, n.b[3], n.b[3], v, u);  hop_compute<3, -SF, true, real>(v, u, sgb, acc);
+        load_spinor_sel<RO>(in, s, c);
         if (LOADR) load_spinor_rw(r, s, rv);
     } else if (PIPE == 1) {
         real va[24], ua[18], vb[24], ub[18];
-        hop_load<0, real>(U, in, s, n.f[0], va, ua);
-        hop_load<0, real>(U, in, n.b[0], n.b[0], vb, ub);  hop_compute<0, SF, false, real>(va, ua, one, acc);
-        hop_load<1, real>(U, in, s, n.f[1], va, ua);       hop_compute<0, -SF, true, real>(vb, ub, one, acc);
-        hop_load<1, real>(U, in, n.b[1], n.b[1], vb, ub);  hop_compute<1, SF, false, real>(va, ua, one, acc);
-        hop_load<2, real>(U, in, s, n.f[2], va, ua);       hop_compute<1, -SF, true, real>(vb, ub, one, acc);
-        hop_load<2, real>(U, in, n.b[2], n.b[2], vb, ub);  hop_compute<2, SF, false, real>(va, ua, one, acc);
-        hop_load<3, real>(U, in, s, n.f[3], va, ua);       hop_compute<2, -SF, true, real>(vb, ub, one, acc);
-        hop_load<3, real>(U, in, n.b[3], n.b[3], vb, ub);  hop_compute<3, SF, false, real>(va, ua, sgf, acc);
-        load_spinor(in, s, c);
+        hop_load<0, RO, real>(U, in, s, n.f[0], va, ua);
+        hop_load<0, RO, real>(U, in, n.b[0], n.b[0], vb, ub);  hop_compute<0, SF, false, real>(va, ua, one, acc);
+        hop_load<1, RO, real>(U, in, s, n.f[1], va, ua);       hop_compute<0, -SF, true, real>(vb, ub, one, acc);
+        hop_load<1, RO, real>(U, in, n.b[1], n.b[1], vb, ub);  hop_compute<1, SF, false, real>(va, ua, one, acc);
+        hop_load<2, RO, real>(U, in, s, n.f[2], va, ua);       hop_compute<1, -SF, true, real>(vb, ub, one, acc);
+        hop_load<2, RO, real>(U, in, n.b[2], n.b[2], vb, ub);  hop_compute<2, SF, false, real>(va, ua, one, acc);
+        hop_load<3, RO, real>(U, in, s, n.f[3], va, ua);       hop_compute<2, -SF, true, real>(vb, ub, one, acc);
+        hop_load<3, RO, real>(U, in, n.b[3], n.b[3], vb, ub);  hop_compute<3, SF, false, real>(va, ua, sgf, acc);
+        load_spinor_sel<RO>(in, s, c);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
         if (LOADR) load_spinor_rw(r, s, rv);   // after the last hop: an earlier fetch costs registers (spills at 128)
     } else if (PIPE == 2) {
         // three register buffers: two hops (336 B fp32 per thread) in flight while a third is computed
         real va[24], ua[18], vb[24], ub[18], vc[24], uc[18];
-        hop_load<0, real>(U, in, s, n.f[0], va, ua);
-        hop_load<0, real>(U, in, n.b[0], n.b[0], vb, ub);
-        hop_load<1, real>(U, in, s, n.f[1], vc, uc);          hop_compute<0, SF, false, real>(va, ua, one, acc);
-        hop_load<1, real>(U, in, n.b[1], n.b[1], va, ua);     hop_compute<0, -SF, true, real>(vb, ub, one, acc);
-        hop_load<2, real>(U, in, s, n.f[2], vb, ub);          hop_compute<1, SF, false, real>(vc, uc, one, acc);
-        hop_load<2, real>(U, in, n.b[2], n.b[2], vc, uc);     hop_compute<1, -SF, true, real>(va, ua, one, acc);
-        hop_load<3, real>(U, in, s, n.f[3], va, ua);          hop_compute<2, SF, false, real>(vb, ub, one, acc);
-        hop_load<3, real>(U, in, n.b[3], n.b[3], vb, ub);     hop_compute<2, -SF, true, real>(vc, uc, one, acc);
-        load_spinor(in, s, c);
+        hop_load<0, RO, real>(U, in, s, n.f[0], va, ua);
+        hop_load<0, RO, real>(U, in, n.b[0], n.b[0], vb, ub);
+        hop_load<1, RO, real>(U, in, s, n.f[1], vc, uc);          hop_compute<0, SF, false, real>(va, ua, one, acc);
+        hop_load<1, RO, real>(U, in, n.b[1], n.b[1], va, ua);     hop_compute<0, -SF, true, real>(vb, ub, one, acc);
+        hop_load<2, RO, real>(U, in, s, n.f[2], vb, ub);          hop_compute<1, SF, false, real>(vc, uc, one, acc);
+        hop_load<2, RO, real>(U, in, n.b[2], n.b[2], vc, uc);     hop_compute<1, -SF, true, real>(va, ua, one, acc);
+        hop_load<3, RO, real>(U, in, s, n.f[3], va, ua);          hop_compute<2, SF, false, real>(vb, ub, one, acc);
+        hop_load<3, RO, real>(U, in, n.b[3], n.b[3], vb, ub);     hop_compute<2, -SF, true, real>(vc, uc, one, acc);
+        load_spinor_sel<RO>(in, s, c);
         if (LOADR) load_spinor_rw(r, s, rv);
         hop_compute<3, SF, false, real>(va, ua, sgf, acc);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
@@ -518,7 +527,7 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
         if (!active) continue;
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24], rv[24];
-        hopping_sum<DAG, PIPE, MODE == MODE_RUPD, real, svec, gvec>(g, U, in, r, x, y, z, t, s, acc, c, rv);
+        hopping_sum<DAG, PIPE, MODE == MODE_RUPD, true, real, svec, gvec>(g, U, in, r, x, y, z, t, s, acc, c, rv);
 #pragma unroll
         for (int i = 0; i < 24; ++i) c[i] = fma(-kappa, acc[i], c[i]);  // (D in)(x) = in(x) - kappa * hops
         if (MODE == MODE_RUPD) {
@@ -546,6 +555,151 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
             if (MODE == MODE_QQ) finish_qq(sc, total);
             else finish_rr(sc, total, it, hist);
         }
+    }
+}
+
+// ---------------------------------------------------------------- the whole CG in ONE launch (small volumes)
+// SURVEY.md 8(f1).  On the paper's own volumes (4^4 ... 14^4) one CG iteration moves 0.4-59 MB, all of
+// it L2-resident: 0.05-9 us of memory time, far below three kernel launches.  This kernel runs init, the loop
+// and the final D-dagger in a single cooperative launch; the three phases of an iteration are separated by
+// grid barriers instead of kernel boundaries.  Every CTA sums the per-CTA partials in the same fixed order, so
+// alpha, beta and the loop test are identical everywhere (no broadcast, deterministic).  The recurrence and the
+// precision rules are exactly those of the three-kernel path.
+template <int NT>
+__device__ __forceinline__ double all_cta_sum(const double *partials, int n, double *sm)
+{
+    double a = 0.0;
+    for (int i = threadIdx.x; i < n; i += NT) a += __ldcg(partials + i);
+    const double t = block_sum<NT>(a, sm);
+    if (threadIdx.x == 0) sm[32] = t;
+    __syncthreads();
+    const double out = sm[32];
+    __syncthreads();
+    return out;
+}
+
+template <typename real, int BX, int BY, int BZ, int BT, int MINB, int PIPE>
+__global__ void __launch_bounds__(BX *BY *BZ *BT, MINB)
+cg_onelaunch_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
+                    const typename Field<real>::svec *__restrict__ eta, typename Field<real>::svec *y,
+                    typename Field<real>::svec *r, typename Field<real>::svec *p, typename Field<real>::svec *q,
+                    typename Field<real>::svec *psi, real kappa, CgScalars *sc, double *partials, double *hist,
+                    double r_min, int max_iter)
+{
+    namespace cg = cooperative_groups;
+    using svec = typename Field<real>::svec;
+    using gvec = typename Field<real>::gvec;
+    constexpr int NT = BX * BY * BZ * BT;
+    cg::grid_group grid = cg::this_grid();
+    __shared__ double sm[33];
+    const int G = gridDim.x;
+    double *part0 = partials, *part1 = partials + G, *part2 = partials + 2 * G;
+    const int tid = threadIdx.x;
+    const int lx = tid % BX, ly = (tid / BX) % BY, lz = (tid / (BX * BY)) % BZ, lt = tid / (BX * BY * BZ);
+
+#define WD_FOR_EACH_SITE(...)                                                                     \
+    for (int b_ = blockIdx.x; b_ < g.ntiles; b_ += G) {                                             \
+        int tx_, ty_, tz_, tt_;                                                                     \
+        tile_of_block(g, b_, tx_, ty_, tz_, tt_);                                                   \
+        const int x = tx_ * BX + lx, y_ = ty_ * BY + ly, z = tz_ * BZ + lz, t = tt_ * BT + lt;      \
+        if (x < g.L[0] && y_ < g.L[1] && z < g.L[2] && t < g.L[3]) {                                \
+            const int s = x + g.L[0] * (y_ + g.L[1] * (z + g.L[2] * t));                            \
+            __VA_ARGS__                                                                             \
+        }                                                                                           \
+    }
+
+    // a1: y <- 0, r <- eta, p <- eta, rr = <eta,eta>
+    double local = 0.0;
+    WD_FOR_EACH_SITE({
+        real e[24], zero[24];
+        load_spinor(eta, s, e);
+        real n2 = 0;
+#pragma unroll
+        for (int i = 0; i < 24; ++i) { zero[i] = 0; n2 = fma(e[i], e[i], n2); }
+        store_spinor(y, s, zero); store_spinor(r, s, e); store_spinor(p, s, e);
+        local += (double)n2;
+    })
+    {
+        const double bsum = block_sum<NT>(local, sm);
+        if (tid == 0) part0[blockIdx.x] = bsum;
+    }
+    grid.sync();
+    const double eta2 = all_cta_sum<NT>(part0, G, sm);
+    double rr = eta2, alpha = 0.0, beta = 0.0;
+    int k = 0;
+    bool go = eta2 > 0.0 && (sqrt(rr) >= r_min * sqrt(eta2));
+    if (blockIdx.x == 0 && tid == 0 && hist) hist[0] = eta2;
+
+    while (go && k < max_iter) {
+        // a2: q = D-dagger p, qq
+        local = 0.0;
+        WD_FOR_EACH_SITE({
+            real acc[24], c[24], dummy[24];
+            hopping_sum<1, PIPE, false, false, real, svec, gvec>(g, U, p, nullptr, x, y_, z, t, s, acc, c, dummy);
+            real n2 = 0;
+#pragma unroll
+            for (int i = 0; i < 24; ++i) { c[i] = fma(-kappa, acc[i], c[i]); n2 = fma(c[i], c[i], n2); }
+            store_spinor(q, s, c);
+            local += (double)n2;
+        })
+        {
+            const double bsum = block_sum<NT>(local, sm);
+            if (tid == 0) part1[blockIdx.x] = bsum;
+        }
+        grid.sync();
+        const double qq = all_cta_sum<NT>(part1, G, sm);
+        alpha = rr / qq;                                     // alpha <- |r|^2 / |D-dagger p|^2 (G1)
+        const real al = (real)alpha;
+        // a3: r <- r - alpha D q, rr'
+        local = 0.0;
+        WD_FOR_EACH_SITE({
+            real acc[24], c[24], rv[24];
+            hopping_sum<0, PIPE, true, false, real, svec, gvec>(g, U, q, r, x, y_, z, t, s, acc, c, rv);
+            real n2 = 0;
+#pragma unroll
+            for (int i = 0; i < 24; ++i) {
+                c[i] = fma(-kappa, acc[i], c[i]);
+                rv[i] = fma(-al, c[i], rv[i]);
+                n2 = fma(rv[i], rv[i], n2);
+            }
+            store_spinor(r, s, rv);
+            local += (double)n2;
+        })
+        {
+            const double bsum = block_sum<NT>(local, sm);
+            if (tid == 0) part2[blockIdx.x] = bsum;
+        }
+        grid.sync();
+        const double rr_new = all_cta_sum<NT>(part2, G, sm);
+        beta = rr_new / rr;                                  // beta <- |r'|^2 / |r|^2
+        const real be = (real)beta;
+        // a4: y <- y + alpha p ; p <- r + beta p (own sites only)
+        WD_FOR_EACH_SITE({
+            real yv[24], pv[24], rv[24];
+            load_spinor_rw(y, s, yv); load_spinor_rw(p, s, pv); load_spinor_rw(r, s, rv);
+#pragma unroll
+            for (int i = 0; i < 24; ++i) { yv[i] = fma(al, pv[i], yv[i]); pv[i] = fma(be, pv[i], rv[i]); }
+            store_spinor(y, s, yv); store_spinor(p, s, pv);
+        })
+        rr = rr_new;
+        ++k;
+        if (blockIdx.x == 0 && tid == 0 && hist) hist[k] = rr;
+        go = sqrt(rr) >= r_min * sqrt(eta2);                 // while |r| >= r_min (G4)
+        grid.sync();                                         // p complete before its neighbours are read
+    }
+    // a6: psi = D-dagger y
+    WD_FOR_EACH_SITE({
+        real acc[24], c[24], dummy[24];
+        hopping_sum<1, PIPE, false, false, real, svec, gvec>(g, U, y, nullptr, x, y_, z, t, s, acc, c, dummy);
+#pragma unroll
+        for (int i = 0; i < 24; ++i) c[i] = fma(-kappa, acc[i], c[i]);
+        store_spinor(psi, s, c);
+    })
+#undef WD_FOR_EACH_SITE
+    if (blockIdx.x == 0 && tid == 0) {
+        sc->rr = rr; sc->eta2 = eta2; sc->alpha = alpha; sc->beta = beta; sc->qq = 0.0; sc->r_min = r_min;
+        sc->k = k; sc->k_stop = k; sc->max_iter = max_iter;
+        sc->converged = go ? 0 : 1;
     }
 }
 

@@ -29,6 +29,18 @@
     X(16, 16, 2, 2, 2, 3, 2, 0)
 #define WD_NUM_TILES 17
 
+// Launch configurations of the one-launch CG kernel (small volumes): 64- and 128-thread tiles,
+// no register bound (ptxas then hoists the loads of all 8 hops: one memory round trip per site instead of 8,
+// which is what matters when the lattice lives in L2 and there are few warps per SM).
+//   Y(index, BX, BY, BZ, BT, MINB, PIPE)
+#define WD_SMALL_TABLE(Y)  \
+    Y(0, 4, 4, 2, 2, 1, 0) \
+    Y(1, 8, 4, 2, 1, 1, 0) \
+    Y(2, 16, 2, 2, 1, 1, 0) \
+    Y(3, 16, 2, 2, 2, 1, 0) \
+    Y(4, 8, 4, 2, 2, 1, 0)
+#define WD_NUM_SMALL_TILES 5
+
 namespace wd {
 
 struct TileInfo {
@@ -40,6 +52,30 @@ static const TileInfo kTiles[WD_NUM_TILES] = {
     WD_TILE_TABLE(X)
 #undef X
 };
+
+static const int kSmallTiles[WD_NUM_SMALL_TILES][4] = {
+#define Y(i, a, b, c, d, m, p) {a, b, c, d},
+    WD_SMALL_TABLE(Y)
+#undef Y
+};
+
+struct CgOneLaunchArgs {
+    Geom g;            // nt / ntiles / fast-division constants for the chosen small tile
+    int sm_count;
+    cudaStream_t stream;
+    const void *U;
+    const void *eta;
+    void *y, *r, *p, *q, *psi;
+    double kappa;
+    CgScalars *sc;
+    double *partials;  // 3 * grid doubles
+    size_t partials_cap;
+    double *hist;
+    double r_min;
+    int max_iter;
+};
+cudaError_t launch_cg_onelaunch_f32(int small_tile, const CgOneLaunchArgs &a);
+cudaError_t launch_cg_onelaunch_f64(int small_tile, const CgOneLaunchArgs &a);
 
 struct DslashArgs {
     Geom g;
@@ -91,6 +127,43 @@ static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
         return cudaErrorInvalidValue;
         WD_TILE_TABLE(X)
 #undef X
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+template <typename real>
+static cudaError_t launch_cg_onelaunch_any(int small_tile, const CgOneLaunchArgs &a)
+{
+    using svec = typename Field<real>::svec;
+    using gvec = typename Field<real>::gvec;
+    switch (small_tile) {
+#define Y(i, bx, by, bz, bt, mb_, pi_)                                                                           \
+    case i: {                                                                                                  \
+        auto kern = cg_onelaunch_kernel<real, bx, by, bz, bt, mb_, pi_>;                                      \
+        static int occ = 0;                                                                                    \
+        if (!occ) {                                                                                            \
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, bx * by * bz * bt, 0);   \
+            if (e != cudaSuccess) return e;                                                                    \
+            if (occ < 1) return cudaErrorLaunchOutOfResources;                                                 \
+        }                                                                                                      \
+        long grid = (long)occ * a.sm_count;            /* all CTAs must be co-resident (grid barrier) */       \
+        if (grid > a.g.ntiles) grid = a.g.ntiles;                                                              \
+        if ((size_t)(3 * grid) > a.partials_cap) return cudaErrorInvalidValue;                                 \
+        Geom g = a.g;                                                                                          \
+        const gvec *U = (const gvec *)a.U;                                                                     \
+        const svec *eta = (const svec *)a.eta;                                                                 \
+        svec *y = (svec *)a.y, *r = (svec *)a.r, *pp = (svec *)a.p, *q = (svec *)a.q, *psi = (svec *)a.psi;    \
+        real kappa = (real)a.kappa;                                                                            \
+        CgScalars *sc = a.sc;                                                                                  \
+        double *partials = a.partials, *hist = a.hist;                                                         \
+        double r_min = a.r_min;                                                                                \
+        int max_iter = a.max_iter;                                                                             \
+        void *args[] = {&g, &U, &eta, &y, &r, &pp, &q, &psi, &kappa, &sc, &partials, &hist, &r_min, &max_iter}; \
+        return cudaLaunchCooperativeKernel((const void *)kern, dim3((unsigned)grid), dim3(bx * by * bz * bt),  \
+                                           args, 0, a.stream);                                                 \
+    }
+        WD_SMALL_TABLE(Y)
+#undef Y
         default: return cudaErrorInvalidValue;
     }
 }

@@ -33,11 +33,11 @@ class WdCgInfo(ctypes.Structure):
         ("gpu_ms", ctypes.c_double),
         ("total_ms", ctypes.c_double),
         ("kernel_launches", ctypes.c_int),
-        ("reserved", ctypes.c_int),
+        ("cg_mode", ctypes.c_int),
     ]
 
     def as_dict(self):
-        return {k: getattr(self, k) for k, _ in self._fields_ if k != "reserved"}
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "_"}
 
 
 class WilsonError(RuntimeError):
@@ -86,6 +86,7 @@ def load_library(path: str = LIB_PATH):
     lib.wd_tile_info.argtypes = [ci, ip]
     lib.wd_set_tile.argtypes = [vp, ci]
     lib.wd_get_tile.argtypes = [vp]
+    lib.wd_set_cg_mode.argtypes = [vp, ci]
     lib.wd_set_prefetch.argtypes = [vp, ci]
     lib.wd_set_waves.argtypes = [vp, ci]
     lib.wd_set_zchunk.argtypes = [vp, ci]
@@ -296,6 +297,10 @@ class WilsonContext:
         n = ctypes.c_long()
         self._check(self.lib.wd_get_profile(self._ctx, ms, ctypes.byref(n)))
         return {"a2_ms": ms[0], "a3_ms": ms[1], "a4_ms": ms[2], "iterations": n.value}
+
+    def wd_set_cg_mode(self, mode):
+        """0 automatic, 1 three kernels per iteration, 2 whole solve in one cooperative launch"""
+        self._check(self.lib.wd_set_cg_mode(self._ctx, int(mode)))
 
     def wd_set_prefetch(self, tiles):
         self._check(self.lib.wd_set_prefetch(self._ctx, int(tiles)))

@@ -178,14 +178,19 @@ def test_norm2_matches_oracle_and_is_deterministic(wilson, oracle, precision):
 
 
 # ---------------------------------------------------------------- a1-a6: cg_solve
-def _cg_case(wilson, oracle, cfg, precision, r_min, poll=None):
+def _cg_case(wilson, oracle, cfg, precision, r_min, poll=None, mode=0):
+    """mode: 0 automatic, 1 three kernels per iteration, 2 whole solve in one cooperative launch"""
     U, eta = gu.config_fields(cfg.index, precision)
     U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
     with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
         if poll:
             ctx.wd_set_poll_interval(poll)
+        ctx.wd_set_cg_mode(mode)
         psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, r_min, cfg.max_iter)
         hist = ctx.wd_cg_history()
+    if mode:
+        assert info["cg_mode"] == mode
+        assert info["kernel_launches"] == 1 if mode == 2 else info["kernel_launches"] >= 3 * info["iterations"] + 2
     psi_o, info_o = oracle.cg_solve(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t, history=True)
     res_gpu = oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
     res_orc = oracle.true_residual(cfg.dims, U64, eta64, psi_o, cfg.kappa, cfg.bc_t)
@@ -205,16 +210,47 @@ def _cg_case(wilson, oracle, cfg, precision, r_min, poll=None):
     return info, info_o, res_gpu, res_orc
 
 
+@pytest.mark.parametrize("mode", [1, 2])
 @pytest.mark.parametrize("cfg_index", [0, 1, 2])
-def test_cg_solve_fp32_baseline_configs(wilson, oracle, cfg_index):
+def test_cg_solve_fp32_baseline_configs(wilson, oracle, cfg_index, mode):
+    """both CG drivers: three kernels per iteration (mode 1) and the one-launch cooperative kernel (mode 2)"""
     cfg = inputs.CONFIGS[cfg_index]
-    _cg_case(wilson, oracle, cfg, 32, cfg.r_min)
+    _cg_case(wilson, oracle, cfg, 32, cfg.r_min, mode=mode)
 
 
+@pytest.mark.parametrize("mode", [1, 2])
 @pytest.mark.parametrize("cfg_index", [0, 1, 2])
-def test_cg_solve_fp64_tight(wilson, oracle, cfg_index):
+def test_cg_solve_fp64_tight(wilson, oracle, cfg_index, mode):
     cfg = inputs.CONFIGS[cfg_index]
-    _cg_case(wilson, oracle, cfg, 64, 1e-10)
+    _cg_case(wilson, oracle, cfg, 64, 1e-10, mode=mode)
+
+
+def test_cg_automatic_mode_by_volume(wilson):
+    """4^4 .. 14^4 (the paper's range) take the one-launch kernel, 32^4 the three-kernel loop"""
+    for ci, want in ((0, 2), (2, 2)):
+        cfg = inputs.CONFIGS[ci]
+        U, eta = gu.config_fields(ci, 32)
+        with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+            _, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
+        assert info["cg_mode"] == want and info["kernel_launches"] == 1
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_cg_onelaunch_ragged_lattice(wilson, oracle, precision):
+    """one-launch kernel on extents that no tile divides, periodic t as well"""
+    for dims, bc_t in (((6, 4, 10, 8), -1), ((5, 7, 4, 6), 1)):
+        cdt = gu.np_complex(precision)
+        U = inputs.gauge_field(CFG_TEST + 6, dims, "near_identity", dtype=cdt)
+        eta = inputs.source_field(CFG_TEST + 6, dims, dtype=cdt)
+        tol = 1e-6 if precision == 32 else 1e-11
+        with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+            ctx.wd_set_cg_mode(2)
+            psi, info = gu.solve_on_gpu(ctx, U, eta, 0.12, tol, 500)
+        U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+        psi_o, info_o = oracle.cg_solve(dims, U64, eta64, 0.12, tol, 500, bc_t)
+        assert info["status"] == 0 and iters_close(info["iterations"], info_o["iterations"])
+        res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), 0.12, bc_t)
+        assert res <= 2.0 * oracle.true_residual(dims, U64, eta64, psi_o, 0.12, bc_t)
 
 
 def test_cg_result_independent_of_poll_interval_and_repeatable(wilson):
@@ -223,16 +259,27 @@ def test_cg_result_independent_of_poll_interval_and_repeatable(wilson):
     outs = []
     for poll in (1, 7, 32, 7):
         with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+            ctx.wd_set_cg_mode(1)
             ctx.wd_set_poll_interval(poll)
+            psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
+            outs.append((psi.tobytes(), info["iterations"], info["rel_residual"]))
+    assert all(o == outs[0] for o in outs)
+    # the one-launch kernel is repeatable too (fixed-order sums of the per-CTA partials in every CTA)
+    outs = []
+    for _ in range(3):
+        with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+            ctx.wd_set_cg_mode(2)
             psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
             outs.append((psi.tobytes(), info["iterations"], info["rel_residual"]))
     assert all(o == outs[0] for o in outs)
 
 
-def test_cg_edge_cases(wilson, oracle):
+@pytest.mark.parametrize("mode", [1, 2])
+def test_cg_edge_cases(wilson, oracle, mode):
     cfg = inputs.CONFIGS[0]
     U, eta = gu.config_fields(0, 64)
     with wilson.WilsonContext(cfg.dims, 64, cfg.bc_t) as ctx:
+        ctx.wd_set_cg_mode(mode)
         # eta = 0: psi = 0, no iterations, OK
         psi, info = gu.solve_on_gpu(ctx, U, np.zeros_like(eta), cfg.kappa, 1e-8, 100)
         assert info["status"] == 0 and info["iterations"] == 0 and not psi.any()
@@ -340,7 +387,7 @@ def test_host_forms_equal_device_forms(wilson, precision):
         psi_d, info_d = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
         psi_h, info_h = ctx.cg_solve_host(U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
         assert psi_h.tobytes() == psi_d.tobytes() and info_h["iterations"] == info_d["iterations"]
-        assert info_h["total_ms"] >= info_h["gpu_ms"] > 0 and info_h["kernel_launches"] >= 3 * info_h["iterations"]
+        assert info_h["total_ms"] >= info_h["gpu_ms"] > 0 and info_h["kernel_launches"] >= 4
         out_d = gu.apply_on_gpu(ctx, U, eta, cfg.kappa, True)
         out_h = ctx.wd_apply_host(None, eta, cfg.kappa, True)  # reuses the cached gauge field
         assert out_h.tobytes() == out_d.tobytes()
