@@ -172,6 +172,70 @@ def run_reference(args, cfg):
     return 0
 
 
+def time_wd_apply(ctx, Un, en, out, kappa, dagger, reps=100):
+    """device time per application over `reps` back-to-back applications (CUDA events on the ctx stream)"""
+    import torch
+
+    for _ in range(5):
+        ctx.wd_apply(Un, en, kappa, dagger, out=out)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(reps):
+        ctx.wd_apply(Un, en, kappa, dagger, out=out)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def run_report(args):
+    """every config, wd_apply D and D-dagger (100 applications each, BASELINE.json configs[2])
+    and the whole CG solve."""
+    import torch
+
+    from paper_2111_14958_b200 import build as wbuild
+    from paper_2111_14958_b200 import wilson
+
+    wbuild.build()
+    wilson.load_library()
+    for ci, prec in ((0, 32), (1, 32), (2, 32), (3, 32), (3, 64), (4, 32)):
+        cfg = inputs.CONFIGS[ci]
+        r_min = cfg.r_min if prec == 32 else 1e-10
+        U, eta = inputs.config_inputs(cfg, dtype=np.complex64 if prec == 32 else np.complex128)
+        V = cfg.volume
+        with wilson.WilsonContext(cfg.dims, prec, cfg.bc_t) as ctx:
+            Un = ctx.wd_pack_gauge(torch.from_numpy(U).cuda())
+            en = ctx.wd_pack_spinor(torch.from_numpy(eta).cuda())
+            out = ctx.empty_spinor()
+            d_ms = time_wd_apply(ctx, Un, en, out, cfg.kappa, False)
+            dd_ms = time_wd_apply(ctx, Un, en, out, cfg.kappa, True)
+            for _ in range(2):
+                ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=out)
+            ctx.wd_set_profile(True)
+            ms = []
+            for _ in range(3):
+                _, info = ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=out)
+                ms.append(info["gpu_ms"])
+            prof = ctx.wd_get_profile()
+            t = float(np.median(ms))
+            it = info["iterations"]
+            bpi = BYTES_ITER[prec]
+            iter_ms = (prof["a2_ms"] + prof["a3_ms"] + prof["a4_ms"]) / prof["iterations"] if prof["iterations"] else None
+            print(json.dumps({
+                "report": f"config{ci}", "name": cfg.name, "precision": prec, "volume": V,
+                "wd_apply_D_us": d_ms * 1e3, "wd_apply_Ddag_us": dd_ms * 1e3, "applications": 100,
+                "wd_apply_D_gflops": FLOP_APPLY * V / (d_ms * 1e-3) / 1e9,
+                "wd_apply_Ddag_gflops": FLOP_APPLY * V / (dd_ms * 1e-3) / 1e9,
+                "wd_apply_D_gbs": (480 if prec == 32 else 960) * V / (d_ms * 1e-3) / 1e9,
+                "cg_iterations": it, "cg_rel_residual": info["rel_residual"], "cg_mode": info["cg_mode"],
+                "cg_solve_ms": t, "cg_gflops": cg_flops(V, it) / (t * 1e-3) / 1e9,
+                "cg_us_per_iteration": t / max(it, 1) * 1e3,
+                "cg_iteration_gbs_live": bpi * V / (iter_ms * 1e-3) / 1e9 if iter_ms else None,
+                "cg_iteration_gbs_whole_solve": bpi * V * it / (t * 1e-3) / 1e9,
+                "tile": list(wilson.tile_shapes()[ctx.wd_get_tile()])}), flush=True)
+    return 0
+
+
 def run_sweep(args, cfg, ctx, wilson, Un, en, psi_n, r_min):
     """Per launch configuration: device time of a2 / a3 / a4 per CG iteration (CUDA events inside the solve) and
     of a standalone wd_apply, as achieved algorithmic GB/s."""
@@ -226,6 +290,9 @@ def main():
     ap.add_argument("--sweep", action="store_true",
                     help="time every compiled launch configuration (the paper's workgroup-size tuning, PAPER.md:76) "
                          "on this config and print one JSON line per configuration instead of the bench line")
+    ap.add_argument("--report", action="store_true",
+                    help="one JSON line per BASELINE config (0..4, plus config 3 in fp64): wd_apply D / D-dagger over 100 "
+                         "applications and the CG solve; the table of BASELINE.md section 3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -242,6 +309,8 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
+    if args.report:
+        return run_report(args) if rank == 0 else 0
     dist = None
     if world > 1:
         import torch.distributed as dist
