@@ -240,6 +240,195 @@ int oracle_cg_solve(const int L[4], int bc_t, const double *U, const double *eta
     return converged ? 0 : 1;
 }
 
+/* <a,b> = sum conj(a_i) b_i, plain summation. */
+static cplx cdot(const cplx *a, const cplx *b, long n)
+{
+    double re = 0.0, im = 0.0;
+#pragma omp parallel for schedule(static) reduction(+ : re, im)
+    for (long i = 0; i < n; ++i) {
+        const cplx t = conj(a[i]) * b[i];
+        re += creal(t);
+        im += cimag(t);
+    }
+    return re + im * I;
+}
+
+/*
+ * BiCGSTAB on D directly.  The paper only NAMES the method ("the
+ * biconjugate gradient stabilized method (BiCGSTAB)", general reference [8]) and prints no listing;
+ * reading B1 of DESIGN.md: the standard unpreconditioned listing with shadow residual rhat = r0,
+ * psi0 = 0, complex inner products <a,b> = sum conj(a) b, and the same relative stopping test as
+ * the CG (reading G4), evaluated at the top of the loop:
+ *   psi <- 0; r <- eta; rhat <- r; p <- r; rho <- <rhat,r>
+ *   while sqrt(<r,r>) >= r_min sqrt(<eta,eta>) and k < max_iter:
+ *       v <- D p;           alpha <- rho / <rhat,v>
+ *       s <- r - alpha v
+ *       t <- D s;           omega <- <t,s> / <t,t>
+ *       psi <- psi + alpha p + omega s
+ *       r <- s - omega t;   rho' <- <rhat,r>
+ *       beta <- (rho'/rho)(alpha/omega);  p <- r + beta (p - omega v);  rho <- rho';  k <- k+1
+ * A breakdown (rho, <rhat,v>, <t,t> or omega exactly 0 or not finite) leaves the loop: returns 2.
+ * Pins (tests/test_oracle_pins.py): dense LU solve on 2^4 (B-P1), first iterate from the dense matrix
+ * (B-P2), termination in <= 2 iterations on a free-field plane wave whose 4x4 symbol has two distinct
+ * eigenvalues and in 1 iteration at kappa = 0 (B-P3), closed-form plane-wave-sum inverse (B-P4).
+ * Returns 0 converged, 1 max_iter reached, 2 breakdown, <0 bad argument / out of memory.
+ */
+int oracle_bicgstab_solve(const int L[4], int bc_t, const double *U, const double *eta, double *psi_out,
+                          double kappa, double r_min, int max_iter, oracle_cg_info *info, double *rr_history)
+{
+    if (!L || !U || !eta || !psi_out || max_iter < 0 || !(r_min > 0.0)) return -1;
+    for (int d = 0; d < 4; ++d)
+        if (L[d] < 2) return -2;
+    const long n = volume_of(L) * 12;
+    const cplx *b = (const cplx *)eta;
+    cplx *x = (cplx *)psi_out;
+    cplx *r = malloc((size_t)n * sizeof(cplx));
+    cplx *p = malloc((size_t)n * sizeof(cplx));
+    cplx *v = malloc((size_t)n * sizeof(cplx));
+    cplx *s = malloc((size_t)n * sizeof(cplx));
+    cplx *t = malloc((size_t)n * sizeof(cplx));
+    if (!r || !p || !v || !s || !t) {
+        free(r); free(p); free(v); free(s); free(t);
+        return -4;
+    }
+#ifdef _OPENMP
+    double t0 = omp_get_wtime();
+#endif
+    memset(x, 0, (size_t)n * sizeof(cplx));
+    memcpy(r, b, (size_t)n * sizeof(cplx));
+    memcpy(p, b, (size_t)n * sizeof(cplx));
+    const cplx *rhat = b; /* rhat = r0 = eta */
+    double rr = norm2(r, n);
+    const double eta2 = rr;
+    cplx rho = rr; /* <rhat,r0> = <eta,eta> */
+    int k = 0, breakdown = 0;
+    if (rr_history) rr_history[0] = rr;
+
+    if (eta2 > 0.0) {
+        while (sqrt(rr) >= r_min * sqrt(eta2) && k < max_iter) {
+            oracle_wd_apply(L, bc_t, U, (const double *)p, (double *)v, kappa, 0); /* v = D p */
+            const cplx rv = cdot(rhat, v, n);
+            if (rv == 0.0 || rho == 0.0) { breakdown = 1; break; }
+            const cplx alpha = rho / rv;
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; ++i) s[i] = r[i] - alpha * v[i];
+            oracle_wd_apply(L, bc_t, U, (const double *)s, (double *)t, kappa, 0); /* t = D s */
+            const double tt = norm2(t, n);
+            if (tt == 0.0) { /* s = 0: psi + alpha p is exact */
+#pragma omp parallel for schedule(static)
+                for (long i = 0; i < n; ++i) x[i] += alpha * p[i];
+                memset(r, 0, (size_t)n * sizeof(cplx));
+                rr = 0.0;
+                ++k;
+                if (rr_history) rr_history[k] = rr;
+                break;
+            }
+            const cplx omega = cdot(t, s, n) / tt;
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; ++i) x[i] += alpha * p[i] + omega * s[i];
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; ++i) r[i] = s[i] - omega * t[i];
+            const cplx rho_new = cdot(rhat, r, n);
+            rr = norm2(r, n);
+            ++k;
+            if (rr_history) rr_history[k] = rr;
+            if (omega == 0.0 || !isfinite(creal(omega)) || !isfinite(cimag(omega))) { breakdown = 1; break; }
+            const cplx beta = (rho_new / rho) * (alpha / omega);
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; ++i) p[i] = r[i] + beta * (p[i] - omega * v[i]);
+            rho = rho_new;
+        }
+    }
+    const int converged = (eta2 == 0.0) || (sqrt(rr) < r_min * sqrt(eta2));
+    if (info) {
+        info->iterations = k;
+        info->converged = converged;
+        info->rel_residual = eta2 > 0.0 ? sqrt(rr / eta2) : 0.0;
+        info->eta_norm2 = eta2;
+#ifdef _OPENMP
+        info->seconds = omp_get_wtime() - t0;
+#else
+        info->seconds = 0.0;
+#endif
+    }
+    free(r); free(p); free(v); free(s); free(t);
+    return converged ? 0 : (breakdown ? 2 : 1);
+}
+
+/*
+ * The paper's own data structure: D (dagger = 0) or D-dagger (dagger = 1) in
+ * coordinate format, assembled entry by entry from reading C-1.  Vector index i = (s*4 + alpha)*3 + a.
+ * Every row holds 1 + 8*2*3 = 49 entries (N_NZ = 588 V); entry k = row*49 + j with
+ *   j = 0                         the diagonal, Val = 1
+ *   j = 1 + (mu*2 + dir)*6 + n*3 + b,  dir 0 = forward hop, 1 = backward hop; n = 0,1 counts the two spin columns
+ *       beta (ascending) in which row alpha of (1 -+ gamma_mu) is non-zero; b = colour column:
+ *       forward : Val = -kappa sigma+ (1 - g gamma_mu)[alpha][beta] U_mu(x)[a][b],             Col = (x+mu, beta, b)
+ *       backward: Val = -kappa sigma- (1 + g gamma_mu)[alpha][beta] conj(U_mu(x-mu)[b][a]),    Col = (x-mu, beta, b)
+ *   (g = +1 for D, -1 for D-dagger).  val: 2*nnz doubles (re, im), row/col: nnz ints.
+ */
+long oracle_coo_nnz(const int L[4]) { return volume_of(L) * 588; }
+
+int oracle_coo_assemble(const int L[4], int bc_t, const double *U_, double kappa, int dagger, double *val_,
+                        int *row, int *col)
+{
+    if (!L || !U_ || !val_ || !row || !col) return -1;
+    const cplx *U = (const cplx *)U_;
+    cplx *val = (cplx *)val_;
+    const long V = volume_of(L);
+    if (V * 12 > 2147483647L) return -2;
+    const double g = dagger ? -1.0 : 1.0;
+    for (long s = 0; s < V; ++s) {
+        int x[4];
+        long rem = s;
+        for (int d = 0; d < 4; ++d) { x[d] = (int)(rem % L[d]); rem /= L[d]; }
+        for (int al = 0; al < 4; ++al)
+            for (int a = 0; a < 3; ++a) {
+                const long r = (s * 4 + al) * 3 + a;
+                long k = r * 49;
+                val[k] = 1.0; row[k] = (int)r; col[k] = (int)r; ++k;
+                for (int mu = 0; mu < 4; ++mu)
+                    for (int dir = 0; dir < 2; ++dir) {
+                        int y[4];
+                        memcpy(y, x, sizeof y);
+                        y[mu] = dir == 0 ? (x[mu] + 1) % L[mu] : (x[mu] - 1 + L[mu]) % L[mu];
+                        const long sn = site_of(L, y);
+                        const int wraps = dir == 0 ? (x[3] == L[3] - 1) : (x[3] == 0);
+                        const double sig = (mu == 3 && bc_t == -1 && wraps) ? -1.0 : 1.0;
+                        const double sgn = dir == 0 ? -g : g; /* (1 - g gamma) forward, (1 + g gamma) backward */
+                        int n = 0;
+                        for (int be = 0; be < 4; ++be) {
+                            const cplx pr = (al == be ? 1.0 : 0.0) + sgn * GAMMA[mu][al][be];
+                            if (pr == 0.0) continue;
+                            for (int b = 0; b < 3; ++b) {
+                                const cplx u = dir == 0 ? U[(s * 4 + mu) * 9 + a * 3 + b]
+                                                        : conj(U[(sn * 4 + mu) * 9 + b * 3 + a]);
+                                val[k] = -kappa * sig * pr * u;
+                                row[k] = (int)r;
+                                col[k] = (int)((sn * 4 + be) * 3 + b);
+                                ++k;
+                            }
+                            ++n;
+                        }
+                        if (n != 2) return -5; /* every row of (1 -+ gamma_mu) has exactly two non-zeros */
+                    }
+                if (k != (r + 1) * 49) return -5;
+            }
+    }
+    return 0;
+}
+
+/* Alg. COO of PAPER.md:52-54, verbatim: for k = 1..N_NZ: out[Row[k]] = out[Row[k]] + Val[k]*in[Col[k]]. */
+int oracle_coo_spmv(long nnz, const double *val_, const int *row, const int *col, const double *in_, double *out_,
+                    long n_out)
+{
+    if (!val_ || !row || !col || !in_ || !out_) return -1;
+    const cplx *val = (const cplx *)val_, *in = (const cplx *)in_;
+    cplx *out = (cplx *)out_;
+    for (long i = 0; i < n_out; ++i) out[i] = 0.0;
+    for (long k = 0; k < nnz; ++k) out[row[k]] = out[row[k]] + val[k] * in[col[k]];
+    return 0;
+}
+
 int oracle_num_threads(void)
 {
 #ifdef _OPENMP

@@ -59,6 +59,15 @@ def _load():
         lib.oracle_cg_solve.argtypes = [i4, ctypes.c_int, dp, dp, dp, ctypes.c_double, ctypes.c_double,
                                         ctypes.c_int, ctypes.POINTER(OracleCgInfo), dp]
         lib.oracle_cg_solve.restype = ctypes.c_int
+        lib.oracle_bicgstab_solve.argtypes = lib.oracle_cg_solve.argtypes
+        lib.oracle_bicgstab_solve.restype = ctypes.c_int
+        ip = ctypes.POINTER(ctypes.c_int)
+        lib.oracle_coo_nnz.argtypes = [i4]
+        lib.oracle_coo_nnz.restype = ctypes.c_long
+        lib.oracle_coo_assemble.argtypes = [i4, ctypes.c_int, dp, ctypes.c_double, ctypes.c_int, dp, ip, ip]
+        lib.oracle_coo_assemble.restype = ctypes.c_int
+        lib.oracle_coo_spmv.argtypes = [ctypes.c_long, dp, ip, ip, dp, dp, ctypes.c_long]
+        lib.oracle_coo_spmv.restype = ctypes.c_int
         lib.oracle_norm2.argtypes = [dp, ctypes.c_long]
         lib.oracle_norm2.restype = ctypes.c_double
         lib.oracle_num_threads.restype = ctypes.c_int
@@ -138,6 +147,67 @@ def cg_solve(dims, U, eta, kappa, r_min, max_iter, bc_t=-1, history=False):
     if history:
         out["rr_history"] = hist[: info.iterations + 1].copy()
     return psi, out
+
+
+def bicgstab_solve(dims, U, eta, kappa, r_min, max_iter, bc_t=-1, history=False):
+    """BiCGSTAB on D directly (the paper names the method at PAPER.md:32; listing = reading B1).
+
+    Returns (psi, info) like cg_solve; status 2 = breakdown."""
+    d, vol = _dims(dims)
+    U = _c128(U, (vol, 4, 3, 3))
+    eta = _c128(eta, (vol, 4, 3))
+    psi = np.empty_like(eta)
+    info = OracleCgInfo()
+    hist = np.zeros(max_iter + 1, dtype=np.float64) if history else None
+    rc = _load().oracle_bicgstab_solve(
+        d, int(bc_t), _ptr(U), _ptr(eta), _ptr(psi), float(kappa), float(r_min), int(max_iter),
+        ctypes.byref(info), _ptr(hist) if history else None)
+    if rc < 0:
+        raise RuntimeError(f"oracle_bicgstab_solve failed: {rc}")
+    out = {
+        "iterations": info.iterations,
+        "converged": bool(info.converged),
+        "rel_residual": info.rel_residual,
+        "eta_norm2": info.eta_norm2,
+        "seconds": info.seconds,
+        "status": rc,
+    }
+    if history:
+        out["rr_history"] = hist[: info.iterations + 1].copy()
+    return psi, out
+
+
+def coo_assemble(dims, U, kappa, dagger=False, bc_t=-1):
+    """D (or D-dagger) in the paper's coordinate format: (val complex128[nnz], row int32[nnz],
+    col int32[nnz]), nnz = 588 V, entry order as documented in wilson_oracle.c."""
+    d, vol = _dims(dims)
+    U = _c128(U, (vol, 4, 3, 3))
+    nnz = int(_load().oracle_coo_nnz(d))
+    val = np.empty(nnz, dtype=np.complex128)
+    row = np.empty(nnz, dtype=np.int32)
+    col = np.empty(nnz, dtype=np.int32)
+    ip = ctypes.POINTER(ctypes.c_int)
+    rc = _load().oracle_coo_assemble(d, int(bc_t), _ptr(U), float(kappa), int(bool(dagger)), _ptr(val),
+                                     row.ctypes.data_as(ip), col.ctypes.data_as(ip))
+    if rc != 0:
+        raise RuntimeError(f"oracle_coo_assemble failed: {rc}")
+    return val, row, col
+
+
+def coo_spmv(val, row, col, vec):
+    """The paper's SpMV loop out[Row[k]] += Val[k] * in[Col[k]], serial, fp64."""
+    val = np.ascontiguousarray(val, dtype=np.complex128)
+    row = np.ascontiguousarray(row, dtype=np.int32)
+    col = np.ascontiguousarray(col, dtype=np.int32)
+    shape = np.shape(vec)
+    vin = np.ascontiguousarray(vec, dtype=np.complex128).reshape(-1)
+    out = np.empty_like(vin)
+    ip = ctypes.POINTER(ctypes.c_int)
+    rc = _load().oracle_coo_spmv(val.size, _ptr(val), row.ctypes.data_as(ip), col.ctypes.data_as(ip), _ptr(vin),
+                                 _ptr(out), out.size)
+    if rc != 0:
+        raise RuntimeError(f"oracle_coo_spmv failed: {rc}")
+    return out.reshape(shape)
 
 
 def norm2(a) -> float:

@@ -126,6 +126,30 @@ def free_point_propagator(dims, kappa, x0, u, bc_t=-1):
     return psi.reshape(lx * ly * lz * lt, 4, 3)
 
 
+def free_solve(dims, kappa, eta, bc_t=-1):
+    """Exact psi with D psi = eta in the free field (U = 1) for ANY source: Fourier transform, multiply every mode
+    by the closed-form D(p)^-1 (pin P8), transform back.  The half-integer t momenta of the antiperiodic case are
+    handled by untwisting the source with exp(-i pi t/Lt) and twisting the solution back."""
+    lx, ly, lz, lt = dims
+    f = np.asarray(eta, dtype=np.complex128).reshape(lt, lz, ly, lx, 4, 3)
+    tw = np.exp(1j * np.pi * np.arange(lt) / lt)[:, None, None, None, None, None] if bc_t == -1 else 1.0
+    ft = np.fft.fftn(f / tw, axes=(0, 1, 2, 3))
+    nt = np.arange(lt)[:, None, None, None]
+    pt = (2 * nt + 1) * np.pi / lt if bc_t == -1 else 2 * np.pi * nt / lt
+    pz = 2 * np.pi * np.arange(lz)[None, :, None, None] / lz
+    py = 2 * np.pi * np.arange(ly)[None, None, :, None] / ly
+    px = 2 * np.pi * np.arange(lx)[None, None, None, :] / lx
+    a = 1.0 - 2.0 * kappa * (np.cos(px) + np.cos(py) + np.cos(pz) + np.cos(pt))
+    sn = [np.sin(px) + 0 * a, np.sin(py) + 0 * a, np.sin(pz) + 0 * a, np.sin(pt) + 0 * a]
+    den = a * a + 4.0 * kappa * kappa * (sn[0] ** 2 + sn[1] ** 2 + sn[2] ** 2 + sn[3] ** 2)
+    out = a[..., None, None] * ft
+    for mu in range(4):
+        out = out - 2j * kappa * sn[mu][..., None, None] * np.einsum("ij,...ja->...ia", GAMMA[mu], ft)
+    out = out / den[..., None, None]
+    psi = np.fft.ifftn(out, axes=(0, 1, 2, 3)) * tw
+    return psi.reshape(lx * ly * lz * lt, 4, 3)
+
+
 def gauge_rotate_links(dims, U, g):
     """U'_mu(x) = g(x) U_mu(x) g(x+mu)^dagger."""
     out = np.empty_like(U)

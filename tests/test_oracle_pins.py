@@ -370,3 +370,151 @@ def test_p11_coo_spmv(oracle):
     np.add.at(out, row, val * psi.reshape(-1)[col])
     got = oracle.wd_apply(dims, U, psi, kappa, False, -1)
     assert np.max(np.abs(got.reshape(-1) - out)) < 1e-13
+
+
+# ---------------------------------------------------------------- BiCGSTAB (reading B1)
+@pytest.mark.parametrize("bc_t", [-1, +1])
+def test_bp1_bicgstab_matches_dense_solve(oracle, bc_t):
+    dims = (2, 2, 2, 2)
+    kappa = 0.12
+    U = inputs.gauge_field(CFG_TEST + 20, dims, "haar")
+    eta = inputs.source_field(CFG_TEST + 20, dims)
+    M = lm.dense_wilson(dims, U, kappa, bc_t)
+    exact = np.linalg.solve(M, eta.reshape(-1)).reshape(eta.shape)
+    psi, info = oracle.bicgstab_solve(dims, U, eta, kappa, 1e-12, 500, bc_t, history=True)
+    assert info["converged"] and info["status"] == 0
+    assert np.linalg.norm(psi - exact) < 1e-10 * np.linalg.norm(exact)
+    assert info["rr_history"][0] == pytest.approx(np.vdot(eta, eta).real, rel=1e-14)
+    # residual identity: the recursed r equals eta - D psi
+    assert abs(oracle.true_residual(dims, U, eta, psi, kappa, bc_t) - info["rel_residual"]) < 1e-12
+
+
+def test_bp2_bicgstab_first_iterates_from_dense_matrix(oracle):
+    """The listing of reading B1 retyped with the dense matrix (complex alpha, omega, beta; <a,b> = sum conj(a) b):
+    pins the inner-product conjugation, the order of the updates and the beta formula."""
+    dims = (2, 2, 2, 2)
+    kappa = 0.11
+    U = inputs.gauge_field(CFG_TEST + 21, dims, "haar")
+    eta = inputs.source_field(CFG_TEST + 21, dims)
+    M = lm.dense_wilson(dims, U, kappa, -1)
+    b = eta.reshape(-1)
+    x = np.zeros_like(b)
+    r = b.copy()
+    rhat = b.copy()
+    p = r.copy()
+    rho = np.vdot(rhat, r)
+    for k in range(1, 4):
+        v = M @ p
+        alpha = rho / np.vdot(rhat, v)
+        s = r - alpha * v
+        t = M @ s
+        omega = np.vdot(t, s) / np.vdot(t, t)
+        x = x + alpha * p + omega * s
+        r = s - omega * t
+        rho_new = np.vdot(rhat, r)
+        beta = (rho_new / rho) * (alpha / omega)
+        p = r + beta * (p - omega * v)
+        rho = rho_new
+        psi, info = oracle.bicgstab_solve(dims, U, eta, kappa, 1e-30, k, -1, history=True)
+        assert info["iterations"] == k and info["status"] == 1
+        assert np.linalg.norm(psi.reshape(-1) - x) < 1e-12 * np.linalg.norm(x)
+        assert info["rr_history"][k] == pytest.approx(np.vdot(r, r).real, rel=1e-9)
+    # alpha and omega are genuinely complex here (a real-arithmetic shortcut would fail above)
+    assert abs(alpha.imag) > 1e-6 * abs(alpha) or abs(omega.imag) > 1e-6 * abs(omega)
+
+
+def test_bp3_bicgstab_finite_termination(oracle):
+    """Free field, one plane wave: D acts as the 4x4 symbol a + 2 i kappa gamma.sin p, a normal matrix with two
+    distinct eigenvalues a +- 2 i kappa |sin p| -> BiCGSTAB is exact after 2 iterations; kappa = 0 -> after 1."""
+    dims = (4, 6, 4, 8)
+    kappa = 0.12
+    U = unit_gauge(dims)
+    rng = np.random.default_rng(5)
+    p = lm.momenta(dims, np.array((1, 2, 0, 3), float), -1)
+    u = rng.standard_normal((4, 3)) + 1j * rng.standard_normal((4, 3))
+    ev = np.linalg.eigvals(lm.free_dirac_symbol(p, kappa))
+    assert len(np.unique(np.round(ev, 10))) == 2
+    eta = lm.plane_wave(dims, p, u)
+    psi, info = oracle.bicgstab_solve(dims, U, eta, kappa, 1e-11, 50, -1)
+    assert info["iterations"] == 2 and info["converged"]
+    exact = lm.plane_wave(dims, p, lm.free_dirac_inverse(p, kappa) @ u)
+    assert np.linalg.norm(psi - exact) < 1e-10 * np.linalg.norm(exact)
+    Uh = inputs.gauge_field(CFG_TEST + 22, dims, "haar")
+    src = inputs.source_field(CFG_TEST + 22, dims)
+    psi, info = oracle.bicgstab_solve(dims, Uh, src, 0.0, 1e-12, 10)
+    assert info["iterations"] == 1 and np.max(np.abs(psi - src)) < 1e-14
+
+
+def test_bp4_bicgstab_point_source_and_edge_cases(oracle):
+    dims = (4, 6, 4, 8)
+    kappa = 0.12
+    V = int(np.prod(dims))
+    rng = np.random.default_rng(3)
+    # one point source in the free field: alpha = 1 (unit diagonal), s = kappa H delta, and
+    # rho' = <delta, r1> = omega kappa^2 (H^2 delta)(x0) = 0 because (1 - gamma_mu)(1 + gamma_mu) = 0:
+    # a genuine BiCGSTAB breakdown after exactly one iteration, reported as status 2.
+    x0 = (1, 4, 2, 5)
+    u = rng.standard_normal((4, 3)) + 1j * rng.standard_normal((4, 3))
+    eta = np.zeros((V, 4, 3), dtype=np.complex128)
+    eta[int(lm.site_index(dims, np.array(x0)))] = u
+    psi, info = oracle.bicgstab_solve(dims, unit_gauge(dims), eta, kappa, 1e-12, 2000, -1)
+    assert info["status"] == 2 and info["iterations"] == 1 and not info["converged"]
+    # a Gaussian source (no such symmetry): exact solution mode by mode with the closed-form D(p)^-1 (pin P8);
+    # the Fourier route itself is checked against the point-source propagator first
+    chk = lm.free_solve(dims, kappa, eta, -1)
+    assert np.linalg.norm(chk - lm.free_point_propagator(dims, kappa, x0, u, -1)) < 1e-12 * np.linalg.norm(chk)
+    eta = inputs.source_field(CFG_TEST + 23, dims)
+    exact = lm.free_solve(dims, kappa, eta, -1)
+    psi, info = oracle.bicgstab_solve(dims, unit_gauge(dims), eta, kappa, 1e-12, 2000, -1)
+    assert info["converged"] and info["iterations"] > 5
+    assert np.linalg.norm(psi - exact) < 1e-9 * np.linalg.norm(exact)
+    # the same solution as the CG route on a Haar field
+    cfg = inputs.CONFIGS[0]
+    Uc, ec = inputs.config_inputs(cfg)
+    pb, ib = oracle.bicgstab_solve(cfg.dims, Uc, ec, cfg.kappa, 1e-11, 1000)
+    pc, ic = oracle.cg_solve(cfg.dims, Uc, ec, cfg.kappa, 1e-11, 1000)
+    assert ib["converged"] and ic["converged"] and ib["iterations"] < ic["iterations"]
+    assert np.linalg.norm(pb - pc) < 1e-9 * np.linalg.norm(pc)
+    # eta = 0 and max_iter = 0
+    z, iz = oracle.bicgstab_solve(cfg.dims, Uc, np.zeros_like(ec), cfg.kappa, 1e-6, 10)
+    assert iz["iterations"] == 0 and iz["converged"] and np.all(z == 0)
+    z, iz = oracle.bicgstab_solve(cfg.dims, Uc, ec, cfg.kappa, 1e-6, 0)
+    assert iz["iterations"] == 0 and iz["status"] == 1 and np.all(z == 0)
+
+
+# ---------------------------------------------------------------- COO assembly (SURVEY.md 8(f2); PAPER.md:50-56)
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (3, 4, 3, 4)])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_cp1_coo_assembly_is_the_dense_matrix(oracle, dims, dagger):
+    """The assembled (Val, Row, Col) scattered into a dense array equals the Kronecker-block matrix (its
+    conjugate transpose for dagger); 49 entries per row, N_NZ = 588 V (duplicates on 2^4 are summed)."""
+    V = int(np.prod(dims))
+    kappa = 0.12
+    U = inputs.gauge_field(CFG_TEST + 30, dims, "haar")
+    val, row, col = oracle.coo_assemble(dims, U, kappa, dagger, -1)
+    assert val.size == 588 * V and np.all(np.bincount(row, minlength=12 * V) == 49)
+    assert np.all(row[::49] == np.arange(12 * V)) and np.all(col[::49] == np.arange(12 * V)) and np.all(val[::49] == 1)
+    M = lm.dense_wilson(dims, U, kappa, -1)
+    if dagger:
+        M = M.conj().T
+    A = np.zeros_like(M)
+    np.add.at(A, (row, col), val)
+    assert np.max(np.abs(A - M)) < 1e-14
+    if min(dims) > 2:   # all (row, col) pairs distinct
+        assert len(set(zip(row.tolist(), col.tolist()))) == val.size
+
+
+def test_cp2_coo_spmv_equals_stencil(oracle):
+    dims = (4, 6, 4, 8)
+    kappa = 0.124
+    U = inputs.gauge_field(CFG_TEST + 31, dims, "near_identity")
+    psi = rand_spinor(CFG_TEST + 31, dims)
+    for dagger in (False, True):
+        val, row, col = oracle.coo_assemble(dims, U, kappa, dagger, -1)
+        got = oracle.coo_spmv(val, row, col, psi)
+        want = oracle.wd_apply(dims, U, psi, kappa, dagger, -1)
+        assert np.max(np.abs(got - want)) < 1e-13
+    # numpy's scatter-add on the same arrays (an independent execution of the paper's loop)
+    ref = np.zeros(psi.size, dtype=np.complex128)
+    np.add.at(ref, row, val * psi.reshape(-1)[col])
+    assert np.max(np.abs(ref - got.reshape(-1))) < 1e-13
