@@ -63,6 +63,7 @@ extern "C" {
 
 #define WD_OK 0
 #define WD_NOT_CONVERGED 1
+#define WD_BREAKDOWN 2       /* bicgstab_solve only: a denominator of the recurrence vanished; psi holds the last iterate */
 #define WD_ERR_ARG (-1)     /* NULL pointer, aliasing out == in, non-finite kappa, r_min <= 0, max_iter < 0 */
 #define WD_ERR_DIMS (-2)    /* an extent < 4 (forward and backward neighbours must be distinct sites) or volume too large */
 #define WD_ERR_CUDA (-3)    /* a CUDA runtime call or kernel launch failed; wd_last_error() has the CUDA string */
@@ -80,7 +81,7 @@ typedef struct wd_cg_info {
     double gpu_ms;         /* device time of init + loop + final D-dagger (CUDA events on the ctx stream) */
     double total_ms;       /* *_host calls: device time including H2D copies, pack, solve, unpack, D2H; else = gpu_ms */
     int kernel_launches;   /* number of this library's kernels launched by the call */
-    int cg_mode;           /* 1 = three kernels per iteration, 2 = whole solve in one cooperative launch */
+    int cg_mode;           /* 1 = three kernels per iteration, 2 = whole solve in one cooperative launch, 3 = BiCGSTAB */
 } wd_cg_info;
 
 /*
@@ -142,6 +143,25 @@ int wd_apply(wd_ctx *ctx, const void *U_native, const void *psi_native, void *ou
  */
 int cg_solve(wd_ctx *ctx, const void *U_native, const void *eta_native, void *psi_native_out,
              double kappa, double r_min, int max_iter, wd_cg_info *info);
+
+/*
+ * bicgstab_solve — solve D psi = eta with BiCGSTAB applied to D directly.  The paper names the
+ * method among the Krylov solvers of lattice QCD but prints no listing; reading B1 is the
+ * standard unpreconditioned recurrence with shadow residual rhat = r0 = eta, psi0 = 0, <a,b> = sum conj(a) b:
+ *     psi <- 0; r <- eta; p <- r; rho <- <rhat,r>
+ *     while sqrt(<r,r>) >= r_min*sqrt(<eta,eta>) and k < max_iter:
+ *         v <- D p ; alpha <- rho / <rhat,v>                                   (stencil + fused complex dot)
+ *         s <- r - alpha v                                                     (vector kernel)
+ *         t <- D s ; omega <- <t,s> / <t,t>                                    (stencil + fused dots)
+ *         psi <- psi + alpha p + omega s ; r <- s - omega t ; rho' <- <rhat,r> ; rr <- <r,r>   (one kernel)
+ *         beta <- (rho'/rho)(alpha/omega) ; p <- r + beta (p - omega v) ; rho <- rho' ; k <- k+1
+ * Complex alpha, omega, beta, rho live in device memory in fp64; loop control as in cg_solve.
+ * Arguments and ownership as cg_solve (device pointers, native layout; psi must not alias eta).
+ * Returns WD_OK, WD_NOT_CONVERGED, WD_BREAKDOWN (rho, <rhat,v> or omega vanished) or an error.  Synchronous.
+ * info->cg_mode = 3.  wd_cg_history works as after cg_solve.
+ */
+int bicgstab_solve(wd_ctx *ctx, const void *U_native, const void *eta_native, void *psi_native_out,
+                   double kappa, double r_min, int max_iter, wd_cg_info *info);
 
 /*
  * Host-buffer forms: the same operations with HOST pointers in the CANONICAL layout.  Each call
@@ -207,6 +227,9 @@ int wd_set_poll_interval(wd_ctx *ctx, int n);
  */
 int wd_set_profile(wd_ctx *ctx, int on);
 int wd_get_profile(wd_ctx *ctx, double ms[3], long *iterations);
+/* The same for bicgstab_solve: ms[0..4] = accumulated milliseconds of its five kernels (D p + <rhat,v>; s update;
+ * D s + dots; psi/r update + dots; p update) over *iters sampled iterations (the first of every poll chunk). */
+int wd_get_profile_bicgstab(wd_ctx *ctx, double ms[5], long *iterations);
 
 /* Host-only self-test of the fast-division constants of the CTA tile decode: returns the number of n in
  * [0, n_max) with a wrong quotient n / d (0 = correct), or -1 for d = 0.  Needs no GPU. */

@@ -36,6 +36,7 @@ struct wd_ctx {
     int sm_count;
     // CG workspace (native layout), device
     void *r, *p, *q, *y;
+    void *w5;             // fifth work vector (BiCGSTAB: t)
     CgScalars *sc;
     double *partials;
     size_t partials_cap;
@@ -56,6 +57,9 @@ struct wd_ctx {
     int pev_cap;            // iterations the pool covers
     double prof_ms[3];      // accumulated device time of a2, a3, a4
     long prof_n;            // iterations accumulated
+    cudaEvent_t bev[6];     // BiCGSTAB: events around the five kernels of the first iteration of every poll chunk
+    double bprof_ms[5];
+    long bprof_n;
     int last_iters;
     int launches;
     char err[512];
@@ -212,6 +216,9 @@ static int ensure_workspace(wd_ctx *c, int max_iter)
         CUDA_TRY(c, cudaMalloc(&c->p, sb));
         CUDA_TRY(c, cudaMalloc(&c->q, sb));
         CUDA_TRY(c, cudaMalloc(&c->y, sb));
+        // pad lanes (V not a multiple of 16) are never written by the stencil: zero them once so that the
+        // vector kernels can stream whole buffers
+        for (void *b : {c->r, c->p, c->q, c->y}) CUDA_TRY(c, cudaMemsetAsync(b, 0, sb, c->stream));
     }
     if (max_iter + 1 > c->hist_cap) {
         if (c->hist) cudaFree(c->hist);
@@ -232,6 +239,7 @@ static int ensure_partials(wd_ctx *c)
         const size_t nb = (size_t)tile_blocks(c, t);
         if (nb > need) need = nb;
     }
+    need *= 3;                                    // up to three values per CTA (grid_sum_n)
     if (need > c->partials_cap) {
         if (c->partials) cudaFree(c->partials);
         c->partials = nullptr;
@@ -297,7 +305,7 @@ extern "C" int wd_destroy(wd_ctx *c)
 {
     if (!c) return WD_OK;
     cudaStreamSynchronize(c->stream);
-    void *dev[] = {c->r, c->p, c->q, c->y, c->sc, c->partials, c->counter, c->hist, c->result_dev,
+    void *dev[] = {c->r, c->p, c->q, c->y, c->w5, c->sc, c->partials, c->counter, c->hist, c->result_dev,
                    c->U_can, c->U_nat, c->s_can, c->s_nat_in, c->s_nat_out};
     for (void *ptr : dev)
         if (ptr) cudaFree(ptr);
@@ -306,6 +314,8 @@ extern "C" int wd_destroy(wd_ctx *c)
     for (int i = 0; i < 4; ++i)
         if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     for (int i = 0; i < 4 * c->pev_cap; ++i) cudaEventDestroy(c->pev[i]);
+    for (int i = 0; i < 6; ++i)
+        if (c->bev[i]) cudaEventDestroy(c->bev[i]);
     free(c->pev);
     free(c);
     return WD_OK;
@@ -381,6 +391,8 @@ extern "C" int wd_set_profile(wd_ctx *c, int on)
     c->profile = on ? 1 : 0;
     c->prof_ms[0] = c->prof_ms[1] = c->prof_ms[2] = 0.0;
     c->prof_n = 0;
+    for (int j = 0; j < 5; ++j) c->bprof_ms[j] = 0.0;
+    c->bprof_n = 0;
     return WD_OK;
 }
 extern "C" int wd_get_profile(wd_ctx *c, double ms[3], long *iterations)
@@ -650,6 +662,124 @@ extern "C" int cg_solve(wd_ctx *c, const void *U, const void *eta, void *psi, do
     if (rc != WD_OK) return rc;
     c->launches = 0;
     return cg_device(c, U, eta, psi, kappa, r_min, max_iter, info, true);
+}
+
+// ---------------------------------------------------------------- f4: BiCGSTAB on D (reading B1)
+template <int MODE>
+static cudaError_t launch_dslash_bi(wd_ctx *c, const void *U, const void *in, void *out, double kappa, void *rhat, int it)
+{
+    DslashArgs a;
+    a.g = make_geom(c, c->tile);
+    a.sm_count = c->sm_count;
+    a.waves = c->waves > 0 ? c->waves : 1;
+    a.prefetch = 0;
+    a.stream = c->stream;
+    a.U = U; a.in = in; a.out = out; a.kappa = kappa; a.r = rhat;
+    a.sc = c->sc; a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = it;
+    c->launches++;
+    return c->precision == 32 ? launch_dslash_bi_f32(c->tile, MODE, a) : launch_dslash_bi_f64(c->tile, MODE, a);
+}
+
+template <typename real>
+static int bicgstab_loop(wd_ctx *c, const void *U, const void *eta_, void *psi_, double kappa, double r_min, int max_iter)
+{
+    using svec = typename Field<real>::svec;
+    const svec *eta = (const svec *)eta_;
+    svec *psi = (svec *)psi_, *r = (svec *)c->r, *p = (svec *)c->p, *v = (svec *)c->q, *s = (svec *)c->y, *t = (svec *)c->w5;
+    const size_t n = spinor_vecs(c);
+    const unsigned int vgrid = vec_grid(c, n);
+    bi_init_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(eta, psi, r, p, n, c->V, padded(c), c->sc, c->partials, c->counter,
+                                                         c->hist, r_min, max_iter);
+    c->launches++;
+    CUDA_TRY(c, cudaGetLastError());
+    const int poll = c->poll > 0 ? c->poll : auto_poll(c);
+    int launched = 0;
+    while (launched < max_iter) {
+        const int chunk = (max_iter - launched) < poll ? (max_iter - launched) : poll;
+        for (int i = 0; i < chunk; ++i) {
+            const int it = launched + i;
+            if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[0], c->stream));
+            // v = D p, <rhat,v>, alpha
+            CUDA_TRY(c, (launch_dslash_bi<MODE_RV>(c, U, p, v, kappa, (void *)eta, it)));
+            if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[1], c->stream));
+            // s = r - alpha v
+            bi_s_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(s, r, v, n, c->sc, it);
+            if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[2], c->stream));
+            // t = D s, <t,s>, <t,t>, omega
+            CUDA_TRY(c, (launch_dslash_bi<MODE_TS>(c, U, s, t, kappa, nullptr, it)));
+            if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[3], c->stream));
+            // psi += alpha p + omega s ; r = s - omega t ; rho', rr, beta, loop test
+            bi_xr_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(psi, r, p, s, t, eta, n, c->sc, c->partials, c->counter,
+                                                               c->hist, it);
+            if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[4], c->stream));
+            // p = r + beta (p - omega v)
+            bi_p_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(p, r, v, n, c->sc, it);
+            if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[5], c->stream));
+            c->launches += 3;
+            CUDA_TRY(c, cudaGetLastError());
+        }
+        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (c->profile && launched < c->sc_host->k_stop) {   // the first iteration of the chunk really ran
+            for (int j = 0; j < 5; ++j) {
+                float ms = 0.f;
+                CUDA_TRY(c, cudaEventElapsedTime(&ms, c->bev[j], c->bev[j + 1]));
+                c->bprof_ms[j] += ms;
+            }
+            c->bprof_n++;
+        }
+        launched += chunk;
+        if (c->sc_host->k_stop <= launched) break;
+    }
+    return WD_OK;
+}
+
+extern "C" int bicgstab_solve(wd_ctx *c, const void *U, const void *eta, void *psi, double kappa, double r_min,
+                              int max_iter, wd_cg_info *info)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!U) return fail(c, WD_ERR_ARG, "bicgstab_solve: NULL gauge field");
+    int rc = check_cg_args(c, U, eta, psi, kappa, r_min, max_iter, "bicgstab_solve");
+    if (rc != WD_OK) return rc;
+    rc = ensure_workspace(c, max_iter);
+    if (rc != WD_OK) return rc;
+    if (!c->w5) {
+        CUDA_TRY(c, cudaMalloc(&c->w5, spinor_bytes(c)));
+        CUDA_TRY(c, cudaMemsetAsync(c->w5, 0, spinor_bytes(c), c->stream));
+    }
+    if (c->profile && !c->bev[0])
+        for (int j = 0; j < 6; ++j) CUDA_TRY(c, cudaEventCreate(&c->bev[j]));
+    c->launches = 0;
+    CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
+    rc = c->precision == 32 ? bicgstab_loop<float>(c, U, eta, psi, kappa, r_min, max_iter)
+                            : bicgstab_loop<double>(c, U, eta, psi, kappa, r_min, max_iter);
+    if (rc != WD_OK) return rc;
+    CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    const CgScalars &s = *c->sc_host;
+    c->last_iters = s.k;
+    if (info) {
+        info->iterations = s.k;
+        info->converged = s.converged;
+        info->rel_residual = s.eta2 > 0.0 ? std::sqrt(s.rr / s.eta2) : 0.0;
+        info->eta_norm2 = s.eta2;
+        float ms = 0.f;
+        CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]));
+        info->gpu_ms = ms;
+        info->total_ms = ms;
+        info->kernel_launches = c->launches;
+        info->cg_mode = 3;
+    }
+    return s.converged ? WD_OK : (s.breakdown ? WD_BREAKDOWN : WD_NOT_CONVERGED);
+}
+
+extern "C" int wd_get_profile_bicgstab(wd_ctx *c, double ms[5], long *iterations)
+{
+    if (!c || !ms || !iterations) return WD_ERR_ARG;
+    for (int j = 0; j < 5; ++j) ms[j] = c->bprof_ms[j];
+    *iterations = c->bprof_n;
+    return WD_OK;
 }
 
 /* rr after 0..k iterations of the last cg_solve on this ctx (device history copied to the host). */

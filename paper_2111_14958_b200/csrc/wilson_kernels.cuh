@@ -86,6 +86,12 @@ struct CgScalars {
     int k_stop;       // kernels of iteration `it` run iff it < k_stop (initially max_iter)
     int max_iter;
     int converged;
+    // BiCGSTAB only (reading B1): complex scalars as (re, im)
+    double rho[2];    // <rhat, r>
+    double calpha[2]; // rho / <rhat, v>
+    double omega[2];  // <t,s> / <t,t>
+    double cbeta[2];  // (rho'/rho)(alpha/omega)
+    int breakdown;    // a denominator was 0 or not finite: the loop stopped without converging
 };
 
 template <typename real> struct Field;
@@ -462,6 +468,42 @@ __device__ __forceinline__ bool grid_sum(double v, double *partials, unsigned in
     return false;
 }
 
+// The same single-pass reduction for N values at once (BiCGSTAB needs a complex and a real dot product per pass).
+// partials holds N * gridDim.x doubles, value j of CTA b at j * gridDim.x + b.
+template <int NT, int N>
+__device__ __forceinline__ bool grid_sum_n(const double v[N], double *partials, unsigned int *counter, double total[N])
+{
+    __shared__ double sm[32];
+    __shared__ int is_last;
+    double b[N];
+#pragma unroll
+    for (int j = 0; j < N; ++j) b[j] = block_sum<NT>(v[j], sm);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int j = 0; j < N; ++j) partials[(size_t)j * gridDim.x + blockIdx.x] = b[j];
+        __threadfence();
+        const unsigned int ticket = atomicAdd(counter, 1u);
+        is_last = (ticket == gridDim.x - 1);
+        __threadfence();
+    }
+    __syncthreads();
+    if (!is_last) return false;
+    double tot[N];
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+        double a = 0.0;
+        for (unsigned int i = threadIdx.x; i < gridDim.x; i += NT) a += __ldcg(partials + (size_t)j * gridDim.x + i);
+        tot[j] = block_sum<NT>(a, sm);
+    }
+    if (threadIdx.x == 0) {
+        *counter = 0u;
+#pragma unroll
+        for (int j = 0; j < N; ++j) total[j] = tot[j];
+        return true;
+    }
+    return false;
+}
+
 // Scalar epilogues, run by one thread of the last CTA.
 __device__ __forceinline__ void finish_qq(CgScalars *sc, double qq)
 {
@@ -481,12 +523,63 @@ __device__ __forceinline__ void finish_rr(CgScalars *sc, double rr_new, int it, 
     }
 }
 
+// BiCGSTAB scalar epilogues (reading B1).  Complex division in fp64; a zero or non-finite denominator stops the
+// loop (k_stop) and raises `breakdown`.
+__device__ __forceinline__ bool cdiv(const double a[2], const double b[2], double q[2])
+{
+    const double d = b[0] * b[0] + b[1] * b[1];
+    q[0] = (a[0] * b[0] + a[1] * b[1]) / d;
+    q[1] = (a[1] * b[0] - a[0] * b[1]) / d;
+    return d > 0.0 && isfinite(q[0]) && isfinite(q[1]);
+}
+__device__ __forceinline__ void bi_stop(CgScalars *sc, int it)
+{
+    sc->k_stop = it;   // kernels of iteration `it` launched after this one are no-ops
+    sc->breakdown = 1;
+}
+// after v = D p: alpha <- rho / <rhat, v>
+__device__ __forceinline__ void finish_rv(CgScalars *sc, const double rv[2], int it)
+{
+    if (!cdiv(sc->rho, rv, sc->calpha) || (sc->rho[0] == 0.0 && sc->rho[1] == 0.0)) bi_stop(sc, it);
+}
+// after t = D s: omega <- <t,s> / <t,t>   (tt = 0 means s = 0: omega = 0 and the x/r update finishes the solve)
+__device__ __forceinline__ void finish_ts(CgScalars *sc, const double ts[2], double tt)
+{
+    sc->omega[0] = tt > 0.0 ? ts[0] / tt : 0.0;
+    sc->omega[1] = tt > 0.0 ? ts[1] / tt : 0.0;
+}
+// after r <- s - omega t: rho' = <rhat, r>, rr = <r,r>; beta <- (rho'/rho)(alpha/omega); k <- k+1; loop test
+__device__ __forceinline__ void finish_bi(CgScalars *sc, const double rho_new[2], double rr_new, int it, double *hist)
+{
+    sc->rr = rr_new;
+    sc->k = it + 1;
+    if (hist) hist[it + 1] = rr_new;
+    if (!(sqrt(rr_new) >= sc->r_min * sqrt(sc->eta2))) {
+        sc->k_stop = it + 1;
+        sc->converged = 1;
+        return;
+    }
+    double a[2], b[2];
+    const bool ok = cdiv(rho_new, sc->rho, a) && cdiv(sc->calpha, sc->omega, b);
+    if (!ok) {
+        sc->k_stop = it + 1;
+        sc->breakdown = 1;
+        return;
+    }
+    sc->cbeta[0] = a[0] * b[0] - a[1] * b[1];
+    sc->cbeta[1] = a[0] * b[1] + a[1] * b[0];
+    sc->rho[0] = rho_new[0];
+    sc->rho[1] = rho_new[1];
+}
+
 // ---------------------------------------------------------------- the stencil kernel
-enum { MODE_PLAIN = 0, MODE_QQ = 1, MODE_RUPD = 2 };
+enum { MODE_PLAIN = 0, MODE_QQ = 1, MODE_RUPD = 2, MODE_RV = 3, MODE_TS = 4 };
 
 // MODE_PLAIN : out = D in / D-dagger in                                  (wd_apply, a6, a7)
 // MODE_QQ    : out = q = D-dagger p, qq = |q|^2, alpha = rr/qq           (a2)
 // MODE_RUPD  : s = D q (not stored), r <- r - alpha s, rr' = |r|^2, beta, loop condition   (a3)
+// MODE_RV    : out = v = D p, <rhat, v> (rhat passed as `r`, read only), alpha = rho/<rhat,v>   (BiCGSTAB)
+// MODE_TS    : out = t = D s, <t,s> and <t,t>, omega = <t,s>/<t,t>                              (BiCGSTAB)
 template <typename real, int DAG, int MODE, int BX, int BY, int BZ, int BT, int MINB, int PIPE>
 __global__ void __launch_bounds__(BX *BY *BZ *BT, MINB)
 dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
@@ -503,7 +596,7 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     const int tid = threadIdx.x;
     const int lx = tid % BX, ly = (tid / BX) % BY, lz = (tid / (BX * BY)) % BZ, lt = tid / (BX * BY * BZ);
     const real alpha = (MODE == MODE_RUPD) ? (real)sc->alpha : (real)0;
-    double local = 0.0;
+    double local = 0.0, local1 = 0.0, local2 = 0.0;
     // Persistent CTAs: the grid is one resident wave; CTA i takes tiles i, i + gridDim.x, ... so that at any
     // moment the chip works on gridDim.x consecutive tiles of the rasterisation (L2 locality) and the
     // reduction epilogue (barriers, fence, ticket) is paid once per CTA, not once per tile.
@@ -527,10 +620,35 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
         if (!active) continue;
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24], rv[24];
-        hopping_sum<DAG, PIPE, MODE == MODE_RUPD, true, real, svec, gvec>(g, U, in, r, x, y, z, t, s, acc, c, rv);
+        hopping_sum<DAG, PIPE, MODE == MODE_RUPD || MODE == MODE_RV, true, real, svec, gvec>(g, U, in, r, x, y, z, t, s,
+                                                                                            acc, c, rv);
+        if constexpr (MODE == MODE_TS) {
+            // c holds s(x); t(x) = s(x) - kappa * hops replaces it component by component
+            real tsr = 0, tsi = 0, tt = 0;
+#pragma unroll
+            for (int j = 0; j < 12; ++j) {
+                const real sr = c[2 * j], si = c[2 * j + 1];
+                const real tr = fma(-kappa, acc[2 * j], sr), ti = fma(-kappa, acc[2 * j + 1], si);
+                tsr = fma(tr, sr, tsr); tsr = fma(ti, si, tsr);      // conj(t) s
+                tsi = fma(tr, si, tsi); tsi = fma(-ti, sr, tsi);
+                tt = fma(tr, tr, tt); tt = fma(ti, ti, tt);
+                c[2 * j] = tr; c[2 * j + 1] = ti;
+            }
+            store_spinor(out, s, c);
+            local += (double)tsr; local1 += (double)tsi; local2 += (double)tt;
+        } else {
 #pragma unroll
         for (int i = 0; i < 24; ++i) c[i] = fma(-kappa, acc[i], c[i]);  // (D in)(x) = in(x) - kappa * hops
-        if (MODE == MODE_RUPD) {
+        if (MODE == MODE_RV) {
+            real dr = 0, di = 0;
+#pragma unroll
+            for (int j = 0; j < 12; ++j) {                              // conj(rhat) v
+                dr = fma(rv[2 * j], c[2 * j], dr); dr = fma(rv[2 * j + 1], c[2 * j + 1], dr);
+                di = fma(rv[2 * j], c[2 * j + 1], di); di = fma(-rv[2 * j + 1], c[2 * j], di);
+            }
+            store_spinor(out, s, c);
+            local += (double)dr; local1 += (double)di;
+        } else if (MODE == MODE_RUPD) {
             real n2 = 0;
 #pragma unroll
             for (int i = 0; i < 24; ++i) {
@@ -548,13 +666,22 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
                 local += (double)n2;
             }
         }
+        }  // MODE != MODE_TS
     }
-    if (MODE != MODE_PLAIN) {
+    if (MODE == MODE_QQ || MODE == MODE_RUPD) {
         double total;
         if (grid_sum<NT>(local, partials, counter, &total)) {
             if (MODE == MODE_QQ) finish_qq(sc, total);
             else finish_rr(sc, total, it, hist);
         }
+    } else if (MODE == MODE_RV) {
+        const double v2[2] = {local, local1};
+        double tot[2];
+        if (grid_sum_n<NT, 2>(v2, partials, counter, tot)) finish_rv(sc, tot, it);
+    } else if (MODE == MODE_TS) {
+        const double v3[3] = {local, local1, local2};
+        double tot[3];
+        if (grid_sum_n<NT, 3>(v3, partials, counter, tot)) finish_ts(sc, tot, tot[2]);
     }
 }
 
@@ -777,6 +904,108 @@ cg_update_kernel(typename Field<real>::svec *y, typename Field<real>::svec *p,
         y[i] = vaxpy(alpha, pv, y[i]);
         p[i] = vaxpy(beta, pv, rv);
     }
+}
+
+// ---------------------------------------------------------------- BiCGSTAB vector kernels (reading B1)
+// complex a (ar + i ai) times x plus y on one 128-bit vector (fp32: two complex numbers, fp64: one)
+__device__ __forceinline__ float4 vcaxpy(float ar, float ai, const float4 &x, const float4 &y)
+{
+    return make_float4(fmaf(-ai, x.y, fmaf(ar, x.x, y.x)), fmaf(ai, x.x, fmaf(ar, x.y, y.y)),
+                       fmaf(-ai, x.w, fmaf(ar, x.z, y.z)), fmaf(ai, x.z, fmaf(ar, x.w, y.w)));
+}
+__device__ __forceinline__ double2 vcaxpy(double ar, double ai, const double2 &x, const double2 &y)
+{
+    return make_double2(fma(-ai, x.y, fma(ar, x.x, y.x)), fma(ai, x.x, fma(ar, x.y, y.y)));
+}
+// conj(a) b summed over the complex numbers of one vector: (re, im)
+__device__ __forceinline__ void vcdot(const float4 &a, const float4 &b, double &re, double &im)
+{
+    re += (double)(a.x * b.x + a.y * b.y + a.z * b.z + a.w * b.w);
+    im += (double)(a.x * b.y - a.y * b.x + a.z * b.w - a.w * b.z);
+}
+__device__ __forceinline__ void vcdot(const double2 &a, const double2 &b, double &re, double &im)
+{
+    re += a.x * b.x + a.y * b.y;
+    im += a.x * b.y - a.y * b.x;
+}
+
+// psi <- 0; r <- eta; p <- eta; rho = rr = eta2 = <eta,eta>; k = 0   (rhat = eta itself, never copied)
+template <typename real>
+__global__ void __launch_bounds__(VEC_NT)
+bi_init_kernel(const typename Field<real>::svec *__restrict__ eta, typename Field<real>::svec *psi,
+               typename Field<real>::svec *r, typename Field<real>::svec *p, size_t n, int V, int padded,
+               CgScalars *sc, double *partials, unsigned int *counter, double *hist, double r_min, int max_iter)
+{
+    using svec = typename Field<real>::svec;
+    double local = 0.0;
+    for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT) {
+        const svec e = real_site<Field<real>::NSP>(i, V, padded) ? __ldg(eta + i) : svec();
+        psi[i] = vzero(e);
+        r[i] = e;
+        p[i] = e;
+        local += vnorm2<svec>(e);
+    }
+    double total;
+    if (grid_sum<VEC_NT>(local, partials, counter, &total)) {
+        sc->rr = total; sc->eta2 = total; sc->qq = 0.0; sc->alpha = 0.0; sc->beta = 0.0;
+        sc->rho[0] = total; sc->rho[1] = 0.0;
+        sc->calpha[0] = sc->calpha[1] = sc->omega[0] = sc->omega[1] = sc->cbeta[0] = sc->cbeta[1] = 0.0;
+        sc->r_min = r_min; sc->k = 0; sc->max_iter = max_iter; sc->breakdown = 0;
+        const bool go = total > 0.0 && (sqrt(total) >= r_min * sqrt(total));
+        sc->k_stop = go ? max_iter : 0;
+        sc->converged = go ? 0 : 1;
+        if (hist) hist[0] = total;
+    }
+}
+
+// s <- r - alpha v
+template <typename real>
+__global__ void __launch_bounds__(VEC_NT)
+bi_s_kernel(typename Field<real>::svec *s, const typename Field<real>::svec *__restrict__ r,
+            const typename Field<real>::svec *__restrict__ v, size_t n, const CgScalars *sc, int it)
+{
+    if (it >= sc->k_stop) return;
+    const real ar = (real)(-sc->calpha[0]), ai = (real)(-sc->calpha[1]);
+    for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT)
+        s[i] = vcaxpy(ar, ai, __ldg(v + i), __ldg(r + i));
+}
+
+// psi <- psi + alpha p + omega s ; r <- s - omega t ; rho' = <rhat,r> ; rr = <r,r> ; beta ; k ; loop test
+template <typename real>
+__global__ void __launch_bounds__(VEC_NT)
+bi_xr_kernel(typename Field<real>::svec *psi, typename Field<real>::svec *r,
+             const typename Field<real>::svec *__restrict__ p, const typename Field<real>::svec *__restrict__ s,
+             const typename Field<real>::svec *__restrict__ t, const typename Field<real>::svec *__restrict__ rhat,
+             size_t n, CgScalars *sc, double *partials, unsigned int *counter, double *hist, int it)
+{
+    using svec = typename Field<real>::svec;
+    if (it >= sc->k_stop) return;
+    const real ar = (real)sc->calpha[0], ai = (real)sc->calpha[1];
+    const real wr = (real)sc->omega[0], wi = (real)sc->omega[1];
+    double v3[3] = {0.0, 0.0, 0.0};
+    for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT) {
+        const svec sv = __ldg(s + i);
+        psi[i] = vcaxpy(wr, wi, sv, vcaxpy(ar, ai, __ldg(p + i), psi[i]));
+        const svec rn = vcaxpy(-wr, -wi, __ldg(t + i), sv);
+        r[i] = rn;
+        vcdot(__ldg(rhat + i), rn, v3[0], v3[1]);
+        v3[2] += vnorm2<svec>(rn);
+    }
+    double tot[3];
+    if (grid_sum_n<VEC_NT, 3>(v3, partials, counter, tot)) finish_bi(sc, tot, tot[2], it, hist);
+}
+
+// p <- r + beta (p - omega v)
+template <typename real>
+__global__ void __launch_bounds__(VEC_NT)
+bi_p_kernel(typename Field<real>::svec *p, const typename Field<real>::svec *__restrict__ r,
+            const typename Field<real>::svec *__restrict__ v, size_t n, const CgScalars *sc, int it)
+{
+    if (it >= sc->k_stop) return;
+    const real br = (real)sc->cbeta[0], bi = (real)sc->cbeta[1];
+    const real wr = (real)(-sc->omega[0]), wi = (real)(-sc->omega[1]);
+    for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT)
+        p[i] = vcaxpy(br, bi, vcaxpy(wr, wi, __ldg(v + i), p[i]), __ldg(r + i));
 }
 
 // the paper's dot-product kernel on its own: <a,a>

@@ -98,6 +98,9 @@ struct DslashArgs {
 // dagger in {0,1}; mode in {MODE_PLAIN, MODE_QQ (dagger = 1 only), MODE_RUPD (dagger = 0 only)}
 cudaError_t launch_dslash_f32(int tile, int dagger, int mode, const DslashArgs &a);
 cudaError_t launch_dslash_f64(int tile, int dagger, int mode, const DslashArgs &a);
+// BiCGSTAB passes (D only): mode in {MODE_RV, MODE_TS}
+cudaError_t launch_dslash_bi_f32(int tile, int mode, const DslashArgs &a);
+cudaError_t launch_dslash_bi_f64(int tile, int mode, const DslashArgs &a);
 
 template <typename real, int DAG, int MODE>
 static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)

@@ -20,6 +20,7 @@ HEADER_PATH = os.path.join(os.path.dirname(HERE), "include", "wilson_cg.h")
 
 WD_OK = 0
 WD_NOT_CONVERGED = 1
+WD_BREAKDOWN = 2
 
 _lib = None
 
@@ -77,6 +78,8 @@ def load_library(path: str = LIB_PATH):
     lib.wd_unpack_spinor.argtypes = [vp, vp, vp]
     lib.wd_apply.argtypes = [vp, vp, vp, vp, cd, ci]
     lib.cg_solve.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
+    lib.bicgstab_solve.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
+    lib.wd_get_profile_bicgstab.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_long)]
     lib.wd_apply_host.argtypes = [vp, vp, vp, vp, cd, ci]
     lib.cg_solve_host.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
     lib.wd_cg_history.argtypes = [vp, dp, ci]
@@ -172,7 +175,7 @@ class WilsonContext:
         self.close()
 
     def _check(self, rc, allow_not_converged=False):
-        if rc == WD_OK or (allow_not_converged and rc == WD_NOT_CONVERGED):
+        if rc == WD_OK or (allow_not_converged and rc in (WD_NOT_CONVERGED, WD_BREAKDOWN)):
             return rc
         raise WilsonError(rc, self.lib.wd_last_error(self._ctx).decode())
 
@@ -233,6 +236,23 @@ class WilsonContext:
         d = info.as_dict()
         d["status"] = rc
         return out, d
+
+    # -- f4
+    def bicgstab_solve(self, U_native, eta_native, kappa, r_min, max_iter, out=None):
+        out = self.empty_spinor() if out is None else out
+        info = WdCgInfo()
+        rc = self.lib.bicgstab_solve(self._ctx, self._p(U_native), self._p(eta_native), self._p(out), float(kappa),
+                                     float(r_min), int(max_iter), ctypes.byref(info))
+        self._check(rc, allow_not_converged=True)
+        d = info.as_dict()
+        d["status"] = rc
+        return out, d
+
+    def wd_get_profile_bicgstab(self):
+        ms = (ctypes.c_double * 5)()
+        n = ctypes.c_long()
+        self._check(self.lib.wd_get_profile_bicgstab(self._ctx, ms, ctypes.byref(n)))
+        return {"ms": list(ms), "iterations": n.value}
 
     def wd_cg_history(self, n=None):
         n = int(n) if n is not None else 1 << 20
