@@ -164,6 +164,34 @@ int bicgstab_solve(wd_ctx *ctx, const void *U_native, const void *eta_native, vo
                    double kappa, double r_min, int max_iter, wd_cg_info *info);
 
 /*
+ * The paper's own route: "we store the sparse matrix D in the so-called coordinate format, i.e. D is
+ * stored using three arrays: one array contains the value of the non-zero elements and the other two arrays the
+ * corresponding row and column indices", and the SpMV loop
+ *     for k = 1..N_NZ: out[Row[k]] = out[Row[k]] + Val[k]*in[Col[k]].
+ * Vectors are in the CANONICAL layout: component index i = (s*4 + alpha)*3 + a, complex interleaved, 12 V entries.
+ *
+ * wd_coo_nnz       N_NZ = 588 V (49 entries in each of the 12 V rows: the diagonal and 8 hops x 2 spin x 3 colour).
+ * wd_coo_assemble  writes D (dagger = 0) or D-dagger (dagger != 0) for the gauge field U_native (device, native layout):
+ *                  val_dev: N_NZ complex numbers of the ctx precision, row_dev / col_dev: N_NZ 32-bit ints (device,
+ *                  caller-owned).  Entry k = row*49 + j; j = 0 is the diagonal (Val = 1); j = 1 + (mu*2 + dir)*6 + n*3 + b
+ *                  with dir 0 = forward hop, 1 = backward hop, n = 0, 1 the two spin columns beta (ascending) in which
+ *                  row alpha of (1 -+ gamma_mu) is non-zero, b the colour column:
+ *                    forward : Val = -kappa s+ (1 - gamma_mu)[alpha][beta] U_mu(x)[a][b],            Col = (x+mu, beta, b)
+ *                    backward: Val = -kappa s- (1 + gamma_mu)[alpha][beta] conj(U_mu(x-mu)[b][a]),   Col = (x-mu, beta, b)
+ *                  (gamma_mu -> -gamma_mu for D-dagger; s+- = bc_t on the hop that wraps in t).  Needs 12 V < 2^31.
+ * wd_coo_spmv      out = 0, then the loop above for ANY coordinate-format matrix with 12 V rows (entries in any order,
+ *                  duplicates are summed): parallel over k, equal rows of adjacent entries are combined inside a warp
+ *                  before one atomic add per run (the sum order of a row is therefore not fixed: results agree to
+ *                  rounding, not bitwise).  in_dev, out_dev: canonical vectors on the device, must not alias.
+ * All three are asynchronous on the ctx stream.  Errors: WD_ERR_ARG, WD_ERR_DIMS, WD_ERR_CUDA.
+ */
+size_t wd_coo_nnz(wd_ctx *ctx);
+int wd_coo_assemble(wd_ctx *ctx, const void *U_native, double kappa, int dagger, void *val_dev, int *row_dev,
+                    int *col_dev);
+int wd_coo_spmv(wd_ctx *ctx, size_t nnz, const void *val_dev, const int *row_dev, const int *col_dev,
+                const void *in_dev, void *out_dev);
+
+/*
  * Host-buffer forms: the same operations with HOST pointers in the CANONICAL layout.  Each call
  * copies its inputs to the device, packs, runs the device path above, unpacks and copies the result
  * back, on the ctx stream, and returns when the host output is complete.  U_host may be NULL in

@@ -51,7 +51,7 @@ def declared_symbols(header_path: str = HEADER_PATH):
     """Function names declared in include/wilson_cg.h (used by the symbol-export test)."""
     text = open(header_path).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b((?:wd|cg)_[a-z0-9_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b((?:wd|cg|bicgstab)_[a-z0-9_]+)\s*\(", text)))
 
 
 def load_library(path: str = LIB_PATH):
@@ -80,6 +80,10 @@ def load_library(path: str = LIB_PATH):
     lib.cg_solve.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
     lib.bicgstab_solve.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
     lib.wd_get_profile_bicgstab.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_long)]
+    lib.wd_coo_nnz.argtypes = [vp]
+    lib.wd_coo_nnz.restype = ctypes.c_size_t
+    lib.wd_coo_assemble.argtypes = [vp, vp, cd, ci, vp, vp, vp]
+    lib.wd_coo_spmv.argtypes = [vp, ctypes.c_size_t, vp, vp, vp, vp, vp]
     lib.wd_apply_host.argtypes = [vp, vp, vp, vp, cd, ci]
     lib.cg_solve_host.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
     lib.wd_cg_history.argtypes = [vp, dp, ci]
@@ -253,6 +257,33 @@ class WilsonContext:
         n = ctypes.c_long()
         self._check(self.lib.wd_get_profile_bicgstab(self._ctx, ms, ctypes.byref(n)))
         return {"ms": list(ms), "iterations": n.value}
+
+    # -- f2: the paper's coordinate-format route
+    def wd_coo_nnz(self):
+        return int(self.lib.wd_coo_nnz(self._ctx))
+
+    def wd_coo_assemble(self, U_native, kappa, dagger=False):
+        """(val complex[nnz], row int32[nnz], col int32[nnz]) CUDA tensors"""
+        torch = _torch()
+        nnz = self.wd_coo_nnz()
+        val = torch.empty(nnz, dtype=self.complex_dtype, device="cuda")
+        row = torch.empty(nnz, dtype=torch.int32, device="cuda")
+        col = torch.empty(nnz, dtype=torch.int32, device="cuda")
+        self._check(self.lib.wd_coo_assemble(self._ctx, self._p(U_native), float(kappa), int(bool(dagger)),
+                                             self._p(val), self._p(row), self._p(col)))
+        return val, row, col
+
+    def wd_coo_spmv(self, val, row, col, vec_canonical, out=None):
+        torch = _torch()
+        vec_canonical = self._canon(vec_canonical, (self.volume, 4, 3))
+        if val.dtype != self.complex_dtype or row.dtype != torch.int32 or col.dtype != torch.int32:
+            raise ValueError("val must have the ctx complex dtype, row/col int32")
+        if not (val.is_cuda and row.is_cuda and col.is_cuda) or not (row.numel() == col.numel() == val.numel()):
+            raise ValueError("val, row, col must be CUDA tensors of equal length")
+        out = torch.empty_like(vec_canonical) if out is None else out
+        self._check(self.lib.wd_coo_spmv(self._ctx, val.numel(), self._p(val), self._p(row), self._p(col),
+                                         self._p(vec_canonical), self._p(out)))
+        return out
 
     def wd_cg_history(self, n=None):
         n = int(n) if n is not None else 1 << 20

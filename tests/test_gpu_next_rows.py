@@ -137,3 +137,73 @@ def test_bicgstab_32_4_closed_form(wilson, precision):
     assert info["status"] == 0
     err = np.linalg.norm(psi - want) / np.linalg.norm(want)
     assert err < (2e-5 if precision == 32 else 1e-9), err
+
+
+# ---------------------------------------------------------------- f2: the paper's COO route
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("dagger", [False, True])
+@pytest.mark.parametrize("dims,links", [((4, 4, 4, 4), "haar"), ((5, 7, 4, 6), "near_identity")])
+def test_coo_assembly_matches_oracle(wilson, oracle, dims, links, dagger, precision):
+    """Row, Col bit-exact against the oracle's assembly from the definition; Val to one rounding of the run precision"""
+    kappa = 0.124
+    cdt = gu.np_complex(precision)
+    U = inputs.gauge_field(CFG_TEST + 10, dims, links, dtype=cdt)
+    with wilson.WilsonContext(dims, precision) as ctx:
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        val, row, col = (gu.to_host(t) for t in ctx.wd_coo_assemble(Un, kappa, dagger))
+        assert ctx.wd_coo_nnz() == 588 * int(np.prod(dims)) == val.size
+    val_o, row_o, col_o = oracle.coo_assemble(dims, U.astype(np.complex128), kappa, dagger, -1)
+    assert row.dtype == np.int32 and np.array_equal(row, row_o) and np.array_equal(col, col_o)
+    assert np.max(np.abs(val - val_o)) <= (3e-7 if precision == 32 else 1e-15) * np.max(np.abs(val_o))
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("cfg_index", [0, 1, 2])
+def test_coo_spmv_baseline_configs(wilson, oracle, cfg_index, precision):
+    """the paper's loop on the GPU == the oracle's serial loop == the matrix-free stencil (14^4: N_NZ = 22 588 608,
+    the largest volume of the paper's range)"""
+    cfg = inputs.CONFIGS[cfg_index]
+    U, eta = gu.config_fields(cfg.index, precision)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    tol = 1e-5 if precision == 32 else 1e-12
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        eta_d = gu.to_device(eta)
+        for dagger in (False, True):
+            val, row, col = ctx.wd_coo_assemble(Un, cfg.kappa, dagger)
+            got = gu.to_host(ctx.wd_coo_spmv(val, row, col, eta_d))
+            want = oracle.wd_apply(cfg.dims, U64, eta64, cfg.kappa, dagger, cfg.bc_t)
+            assert lm.per_site_rel_err(got, want)[0] <= tol
+            stencil = gu.to_host(ctx.wd_unpack_spinor(ctx.wd_apply(Un, ctx.wd_pack_spinor(eta_d), cfg.kappa, dagger)))
+            assert lm.per_site_rel_err(got, stencil)[0] <= 2 * tol
+        if cfg_index < 2:   # the oracle's own serial COO loop on its own assembly (seconds at 8^4)
+            vo, ro, co = oracle.coo_assemble(cfg.dims, U64, cfg.kappa, True, cfg.bc_t)
+            assert lm.per_site_rel_err(got, oracle.coo_spmv(vo, ro, co, eta64))[0] <= tol
+
+
+def test_coo_spmv_any_entry_order_and_duplicates(wilson, oracle):
+    """the loop is defined for any coordinate-format matrix: shuffled entries, repeated (row, col) pairs, empty rows"""
+    import torch
+
+    dims = (4, 4, 4, 4)
+    n = 12 * 256
+    rng = np.random.default_rng(7)
+    nnz = 50_001   # ragged: not a multiple of the warp size
+    row = rng.integers(0, n // 2, nnz).astype(np.int32)          # upper half of the rows stays empty
+    row[:64] = 5                                                  # a run longer than a warp
+    row[100:140:2] = 9                                            # equal rows that are NOT adjacent
+    col = rng.integers(0, n, nnz).astype(np.int32)
+    val = (rng.standard_normal(nnz) + 1j * rng.standard_normal(nnz))
+    x = (rng.standard_normal(n) + 1j * rng.standard_normal(n))
+    want = np.zeros(n, dtype=np.complex128)
+    np.add.at(want, row, val * x[col])
+    assert np.max(np.abs(want - oracle.coo_spmv(val, row, col, x))) < 1e-12
+    with wilson.WilsonContext(dims, 64) as ctx:
+        got = gu.to_host(ctx.wd_coo_spmv(gu.to_device(val), gu.to_device(row), gu.to_device(col),
+                                         gu.to_device(x.reshape(256, 4, 3)))).reshape(-1)
+        assert np.max(np.abs(got - want)) < 1e-12 * np.max(np.abs(want))
+        assert not got[n // 2:].any()
+        empty = ctx.wd_coo_spmv(torch.empty(0, dtype=torch.complex128, device="cuda"),
+                                torch.empty(0, dtype=torch.int32, device="cuda"),
+                                torch.empty(0, dtype=torch.int32, device="cuda"), gu.to_device(x.reshape(256, 4, 3)))
+        assert not gu.to_host(empty).any()
