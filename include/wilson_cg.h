@@ -103,8 +103,24 @@ int wd_destroy(wd_ctx *ctx);
 const char *wd_last_error(wd_ctx *ctx);
 
 /* Sizes in bytes of the native buffers the caller must allocate (device memory). */
-size_t wd_gauge_native_bytes(wd_ctx *ctx);   /* 72 * Vpad * sizeof(real), Vpad = V rounded up to 16 */
+size_t wd_gauge_native_bytes(wd_ctx *ctx);   /* 72 (48 with 12-real links) * Vpad * sizeof(real), Vpad = V rounded up to 16 */
 size_t wd_spinor_native_bytes(wd_ctx *ctx);  /* 24 * Vpad * sizeof(real) */
+
+/*
+ * wd_set_gauge_recon — number of reals stored per link in the NATIVE gauge layout (byte reduction):
+ *   18 (default): all nine complex entries;
+ *   12: rows 0 and 1 only (fp32: 3 planes of float4 per link and 16-site block, fp64: 6 planes of double2); the stencil
+ *       kernels rebuild row 2 = conj(row0 x row1) in registers, exact for special-unitary links.  The gauge traffic of a
+ *       stencil pass drops from 288 to 192 B/site in fp32 (wd_apply 480 -> 384, CG iteration 1536 -> 1344).
+ *       The caller's links must be SU(3) to the accuracy wanted: the rebuilt row differs from the stored one by the
+ *       unitarity defect of rows 0, 1.
+ * Call it BEFORE wd_gauge_native_bytes / wd_pack_gauge: native gauge buffers of the two formats are not interchangeable,
+ * and a gauge field staged by an earlier *_host call is dropped.  With 12, cg_solve always uses the three-kernel loop,
+ * and bicgstab_solve / wd_coo_assemble return WD_ERR_ARG (compiled for 18-real links only).
+ * wd_get_gauge_recon returns 18 or 12.
+ */
+int wd_set_gauge_recon(wd_ctx *ctx, int reals_per_link);
+int wd_get_gauge_recon(wd_ctx *ctx);
 
 /*
  * wd_pack_gauge / wd_pack_spinor / wd_unpack_spinor — pure permutations between the canonical

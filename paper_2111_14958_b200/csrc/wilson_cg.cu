@@ -117,11 +117,13 @@ static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void 
     a.g = make_geom(c, c->tile);
     a.sm_count = c->sm_count;
     a.waves = c->waves > 0 ? c->waves : 1;
-    a.prefetch = (c->dims[0] % SB == 0) ? c->prefetch : 0;
+    a.prefetch = (c->dims[0] % SB == 0 && c->recon == 18) ? c->prefetch : 0;
     a.stream = c->stream;
     a.U = U; a.in = in; a.out = out; a.kappa = kappa; a.r = r;
     a.sc = c->sc; a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = it;
     c->launches++;
+    if (c->recon == 12)
+        return c->precision == 32 ? launch_dslash12_f32(c->tile, DAG, MODE, a) : launch_dslash12_f64(c->tile, DAG, MODE, a);
     return c->precision == 32 ? launch_dslash_f32(c->tile, DAG, MODE, a) : launch_dslash_f64(c->tile, DAG, MODE, a);
 }
 
@@ -199,6 +201,7 @@ extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_
     c->V = (int)vol;
     c->precision = precision;
     c->bc_t = bc_t;
+    c->recon = 18;
     c->stream = (cudaStream_t)cuda_stream;
     c->sm_count = sms;
     cudaDeviceGetAttribute(&c->coop_ok, cudaDevAttrCooperativeLaunch, dev);
@@ -281,9 +284,23 @@ extern "C" int wd_set_cg_mode(wd_ctx *c, int mode)
 {
     if (!c || mode < 0 || mode > 2) return WD_ERR_ARG;
     if (mode == 2 && !c->coop_ok) return fail(c, WD_ERR_CUDA, "wd_set_cg_mode: the device does not support cooperative launches");
+    if (mode == 2 && c->recon != 18) return fail(c, WD_ERR_ARG, "wd_set_cg_mode: the one-launch kernel needs 18-real links");
     c->cg_mode = mode;
     return WD_OK;
 }
+extern "C" int wd_set_gauge_recon(wd_ctx *c, int reals)
+{
+    if (!c) return WD_ERR_ARG;
+    if (reals != 18 && reals != 12) return fail(c, WD_ERR_ARG, "wd_set_gauge_recon: %d reals per link (18 or 12)", reals);
+    if (reals != c->recon) {
+        // the staged gauge field of the *_host calls is in the old format
+        if (c->U_nat) { cudaStreamSynchronize(c->stream); cudaFree(c->U_nat); c->U_nat = nullptr; }
+        c->have_gauge = 0;
+    }
+    c->recon = reals;
+    return WD_OK;
+}
+extern "C" int wd_get_gauge_recon(wd_ctx *c) { return c ? c->recon : WD_ERR_ARG; }
 extern "C" int wd_set_prefetch(wd_ctx *c, int tiles)
 {
     if (!c || tiles < -1) return WD_ERR_ARG;
@@ -334,10 +351,14 @@ extern "C" int wd_pack_gauge(wd_ctx *c, const void *can, void *nat)
     if (!can || !nat || can == nat) return fail(c, WD_ERR_ARG, "wd_pack_gauge: NULL or aliased argument");
     const int Vp = (int)vpad(c);
     const unsigned int grid = (Vp + VEC_NT - 1) / VEC_NT;
-    if (c->precision == 32)
-        pack_gauge_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float2 *)can, (float2 *)nat, c->V, Vp);
+    if (c->precision == 32 && c->recon == 18)
+        pack_gauge_kernel<float, 18><<<grid, VEC_NT, 0, c->stream>>>((const float2 *)can, (float2 *)nat, c->V, Vp);
+    else if (c->precision == 32)
+        pack_gauge_kernel<float, 12><<<grid, VEC_NT, 0, c->stream>>>((const float2 *)can, (float2 *)nat, c->V, Vp);
+    else if (c->recon == 18)
+        pack_gauge_kernel<double, 18><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V, Vp);
     else
-        pack_gauge_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V, Vp);
+        pack_gauge_kernel<double, 12><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V, Vp);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
     return WD_OK;
@@ -430,7 +451,7 @@ static int small_tile_for(const wd_ctx *c)
 
 static bool use_onelaunch(const wd_ctx *c)
 {
-    if (!c->coop_ok) return false;
+    if (!c->coop_ok || c->recon != 18) return false;   // the one-launch kernel is compiled for 18-real links only
     if (c->cg_mode == 1) return false;
     if (c->cg_mode == 2) return true;
     // automatic: volumes whose CG iteration is shorter than three launches (measured crossover on B200: between
@@ -665,6 +686,7 @@ extern "C" int bicgstab_solve(wd_ctx *c, const void *U, const void *eta, void *p
     if (!U) return fail(c, WD_ERR_ARG, "bicgstab_solve: NULL gauge field");
     int rc = check_cg_args(c, U, eta, psi, kappa, r_min, max_iter, "bicgstab_solve");
     if (rc != WD_OK) return rc;
+    if (c->recon != 18) return fail(c, WD_ERR_ARG, "bicgstab_solve: compiled for 18-real links only (wd_set_gauge_recon)");
     rc = ensure_workspace(c, max_iter);
     if (rc != WD_OK) return rc;
     if (!c->w5) {

@@ -132,6 +132,7 @@ extern "C" int wd_coo_assemble(wd_ctx *c, const void *U_native, double kappa, in
     if (!c) return WD_ERR_ARG;
     if (!U_native || !val || !row || !col) return fail(c, WD_ERR_ARG, "wd_coo_assemble: NULL argument");
     if (!std::isfinite(kappa)) return fail(c, WD_ERR_ARG, "wd_coo_assemble: kappa is not finite");
+    if (c->recon != 18) return fail(c, WD_ERR_ARG, "wd_coo_assemble: needs 18-real links (wd_set_gauge_recon)");
     if ((double)c->V * 12.0 >= 2147483647.0) return fail(c, WD_ERR_DIMS, "wd_coo_assemble: 12 V does not fit a 32-bit index");
     Geom g;
     for (int d = 0; d < 4; ++d) g.L[d] = c->dims[d];

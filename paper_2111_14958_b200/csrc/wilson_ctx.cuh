@@ -12,6 +12,7 @@ struct wd_ctx {
     int V;
     int precision;
     int bc_t;
+    int recon;            // reals stored per link: 18 (default) or 12 (rows 0, 1; row 2 rebuilt in the kernels)
     cudaStream_t stream;
     int tile;       // tile index in use
     int tile_user;  // -1 = automatic
@@ -79,7 +80,7 @@ static inline size_t real_bytes(const wd_ctx *c) { return c->precision == 32 ? 4
 static inline size_t vpad(const wd_ctx *c) { return ((size_t)c->V + wd::SB - 1) / wd::SB * wd::SB; }  // volume padded to whole site blocks
 static inline int padded(const wd_ctx *c) { return vpad(c) != (size_t)c->V; }
 static inline size_t spinor_bytes(const wd_ctx *c) { return (size_t)24 * vpad(c) * real_bytes(c); }       // native
-static inline size_t gauge_bytes(const wd_ctx *c) { return (size_t)72 * vpad(c) * real_bytes(c); }        // native
+static inline size_t gauge_bytes(const wd_ctx *c) { return (size_t)(c->recon == 12 ? 48 : 72) * vpad(c) * real_bytes(c); }        // native
 static inline size_t spinor_can_bytes(const wd_ctx *c) { return (size_t)24 * c->V * real_bytes(c); }     // canonical
 static inline size_t gauge_can_bytes(const wd_ctx *c) { return (size_t)72 * c->V * real_bytes(c); }      // canonical
 static inline size_t spinor_vecs(const wd_ctx *c) { return (size_t)(c->precision == 32 ? 6 : 12) * vpad(c); }

@@ -205,6 +205,59 @@ __device__ __forceinline__ void load_link(const float2 *__restrict__ U, int s, f
     const float2 t2 = __ldg(blk + 8 * SB + lane);
     u[16] = t2.x; u[17] = t2.y;
 }
+// 12-real storage: only rows 0 and 1 of the SU(3) matrix are kept (fp32: 3 planes of float4 per
+// link, 768 B per link and 16-site block; fp64: 6 planes of double2); the third row is rebuilt in registers as
+// conj(row0 x row1), which is exact for a special-unitary matrix (and accurate to the unitarity defect of the
+// stored rows otherwise).  Gauge traffic drops from 288 to 192 B/site in fp32.
+template <typename real>
+__device__ __forceinline__ void rebuild_row2(real u[18])
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+        const real ar = u[c1 * 2], ai = u[c1 * 2 + 1], br = u[(3 + c2) * 2], bi = u[(3 + c2) * 2 + 1];
+        const real cr = u[c2 * 2], ci = u[c2 * 2 + 1], dr = u[(3 + c1) * 2], di = u[(3 + c1) * 2 + 1];
+        // conj(a b - c d)
+        u[(6 + c) * 2] = fma(ar, br, -ai * bi) - fma(cr, dr, -ci * di);
+        u[(6 + c) * 2 + 1] = -(fma(ar, bi, ai * br) - fma(cr, di, ci * dr));
+    }
+}
+template <int MU>
+__device__ __forceinline__ void load_link12(const double2 *__restrict__ U, int s, double u[18])
+{
+    const double2 *p = U + (size_t)(s >> SB_SHIFT) * (24 * SB) + MU * 6 * SB + (s & (SB - 1));
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const double2 t = __ldg(p + k * SB);
+        u[2 * k] = t.x; u[2 * k + 1] = t.y;
+    }
+    rebuild_row2(u);
+}
+template <int MU>
+__device__ __forceinline__ void load_link12(const float2 *__restrict__ U, int s, float u[18])
+{
+    const float2 *blk = U + (size_t)(s >> SB_SHIFT) * (24 * SB) + MU * 6 * SB;
+    const float4 *p4 = reinterpret_cast<const float4 *>(blk) + (s & (SB - 1));
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        const float4 t = __ldg(p4 + q * SB);
+        u[4 * q] = t.x; u[4 * q + 1] = t.y; u[4 * q + 2] = t.z; u[4 * q + 3] = t.w;
+    }
+    rebuild_row2(u);
+}
+__device__ __forceinline__ void store_link12(double2 *U, int s, int mu, const double2 k9[9])
+{
+    double2 *p = U + (size_t)(s >> SB_SHIFT) * (24 * SB) + mu * 6 * SB + (s & (SB - 1));
+#pragma unroll
+    for (int k = 0; k < 6; ++k) p[k * SB] = k9[k];
+}
+__device__ __forceinline__ void store_link12(float2 *U, int s, int mu, const float2 k9[9])
+{
+    float2 *blk = U + (size_t)(s >> SB_SHIFT) * (24 * SB) + mu * 6 * SB;
+    float4 *p4 = reinterpret_cast<float4 *>(blk) + (s & (SB - 1));
+#pragma unroll
+    for (int q = 0; q < 3; ++q) p4[q * SB] = make_float4(k9[2 * q].x, k9[2 * q].y, k9[2 * q + 1].x, k9[2 * q + 1].y);
+}
 // the same slots, written by the pack kernel
 __device__ __forceinline__ void store_link(double2 *U, int s, int mu, const double2 k9[9])
 {
@@ -320,12 +373,15 @@ __device__ __forceinline__ void load_spinor_sel(const svec *in, int s, real v[24
     if (RO) load_spinor(in, s, v);
     else load_spinor_rw(in, s, v);
 }
-template <int MU, bool RO, typename real, typename svec, typename gvec>
+// RECON = 18: all nine complex entries are stored; 12: rows 0, 1 stored, row 2 rebuilt.  With RECON = 12 the rebuild
+// happens at load time, i.e. inside the software pipeline one hop ahead of its use.
+template <int MU, bool RO, int RECON, typename real, typename svec, typename gvec>
 __device__ __forceinline__ void hop_load(const gvec *__restrict__ U, const svec *in,
                                          int link_site, int spinor_site, real v[24], real u[18])
 {
     load_spinor_sel<RO>(in, spinor_site, v);
-    load_link<MU>(U, link_site, u);
+    if (RECON == 12) load_link12<MU>(U, link_site, u);
+    else load_link<MU>(U, link_site, u);
 }
 template <int MU, int S, bool ADJ, typename real>
 __device__ __forceinline__ void hop_compute(const real v[24], const real u[18], real sg, real acc[24])
@@ -362,7 +418,7 @@ __device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, i
 // hop k+1 are issued before hop k is computed, so every thread keeps one hop (168 B fp32) in flight while
 // it computes (memory-level parallelism without more threads).
 // LOADR: also fetch r(s) into rv together with the centre spinor (MODE_RUPD), so that it too overlaps the last hop.
-template <int DAG, int PIPE, bool LOADR, bool RO, typename real, typename svec, typename gvec>
+template <int DAG, int PIPE, bool LOADR, bool RO, typename real, typename svec, typename gvec, int RECON = 18>
 __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const svec *in,
                                             const svec *r, int x, int y, int z, int t, int s, real acc[24],
                                             real c[24], real rv[24])
@@ -377,40 +433,40 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
     for (int i = 0; i < 24; ++i) acc[i] = 0;
     if (PIPE == 0) {
         real v[24], u[18];
-        hop_load<0, RO, real>(U, in, s, n.f[0], v, u);       hop_compute<0, SF, false, real>(v, u, one, acc);
-        hop_load<0, RO, real>(U, in, n.b[0], n.b[0], v, u);  hop_compute<0, -SF, true, real>(v, u, one, acc);
-        hop_load<1, RO, real>(U, in, s, n.f[1], v, u);       hop_compute<1, SF, false, real>(v, u, one, acc);
-        hop_load<1, RO, real>(U, in, n.b[1], n.b[1], v, u);  hop_compute<1, -SF, true, real>(v, u, one, acc);
-        hop_load<2, RO, real>(U, in, s, n.f[2], v, u);       hop_compute<2, SF, false, real>(v, u, one, acc);
-        hop_load<2, RO, real>(U, in, n.b[2], n.b[2], v, u);  hop_compute<2, -SF, true, real>(v, u, one, acc);
-        hop_load<3, RO, real>(U, in, s, n.f[3], v, u);       hop_compute<3, SF, false, real>(v, u, sgf, acc);
-        hop_load<3, RO, real>(U, in, n.b[3], n.b[3], v, u);  hop_compute<3, -SF, true, real>(v, u, sgb, acc);
+        hop_load<0, RO, RECON, real>(U, in, s, n.f[0], v, u);       hop_compute<0, SF, false, real>(v, u, one, acc);
+        hop_load<0, RO, RECON, real>(U, in, n.b[0], n.b[0], v, u);  hop_compute<0, -SF, true, real>(v, u, one, acc);
+        hop_load<1, RO, RECON, real>(U, in, s, n.f[1], v, u);       hop_compute<1, SF, false, real>(v, u, one, acc);
+        hop_load<1, RO, RECON, real>(U, in, n.b[1], n.b[1], v, u);  hop_compute<1, -SF, true, real>(v, u, one, acc);
+        hop_load<2, RO, RECON, real>(U, in, s, n.f[2], v, u);       hop_compute<2, SF, false, real>(v, u, one, acc);
+        hop_load<2, RO, RECON, real>(U, in, n.b[2], n.b[2], v, u);  hop_compute<2, -SF, true, real>(v, u, one, acc);
+        hop_load<3, RO, RECON, real>(U, in, s, n.f[3], v, u);       hop_compute<3, SF, false, real>(v, u, sgf, acc);
+        hop_load<3, RO, RECON, real>(U, in, n.b[3], n.b[3], v, u);  hop_compute<3, -SF, true, real>(v, u, sgb, acc);
         load_spinor_sel<RO>(in, s, c);
         if (LOADR) load_spinor_rw(r, s, rv);
     } else if (PIPE == 1) {
         real va[24], ua[18], vb[24], ub[18];
-        hop_load<0, RO, real>(U, in, s, n.f[0], va, ua);
-        hop_load<0, RO, real>(U, in, n.b[0], n.b[0], vb, ub);  hop_compute<0, SF, false, real>(va, ua, one, acc);
-        hop_load<1, RO, real>(U, in, s, n.f[1], va, ua);       hop_compute<0, -SF, true, real>(vb, ub, one, acc);
-        hop_load<1, RO, real>(U, in, n.b[1], n.b[1], vb, ub);  hop_compute<1, SF, false, real>(va, ua, one, acc);
-        hop_load<2, RO, real>(U, in, s, n.f[2], va, ua);       hop_compute<1, -SF, true, real>(vb, ub, one, acc);
-        hop_load<2, RO, real>(U, in, n.b[2], n.b[2], vb, ub);  hop_compute<2, SF, false, real>(va, ua, one, acc);
-        hop_load<3, RO, real>(U, in, s, n.f[3], va, ua);       hop_compute<2, -SF, true, real>(vb, ub, one, acc);
-        hop_load<3, RO, real>(U, in, n.b[3], n.b[3], vb, ub);  hop_compute<3, SF, false, real>(va, ua, sgf, acc);
+        hop_load<0, RO, RECON, real>(U, in, s, n.f[0], va, ua);
+        hop_load<0, RO, RECON, real>(U, in, n.b[0], n.b[0], vb, ub);  hop_compute<0, SF, false, real>(va, ua, one, acc);
+        hop_load<1, RO, RECON, real>(U, in, s, n.f[1], va, ua);       hop_compute<0, -SF, true, real>(vb, ub, one, acc);
+        hop_load<1, RO, RECON, real>(U, in, n.b[1], n.b[1], vb, ub);  hop_compute<1, SF, false, real>(va, ua, one, acc);
+        hop_load<2, RO, RECON, real>(U, in, s, n.f[2], va, ua);       hop_compute<1, -SF, true, real>(vb, ub, one, acc);
+        hop_load<2, RO, RECON, real>(U, in, n.b[2], n.b[2], vb, ub);  hop_compute<2, SF, false, real>(va, ua, one, acc);
+        hop_load<3, RO, RECON, real>(U, in, s, n.f[3], va, ua);       hop_compute<2, -SF, true, real>(vb, ub, one, acc);
+        hop_load<3, RO, RECON, real>(U, in, n.b[3], n.b[3], vb, ub);  hop_compute<3, SF, false, real>(va, ua, sgf, acc);
         load_spinor_sel<RO>(in, s, c);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
         if (LOADR) load_spinor_rw(r, s, rv);   // after the last hop: an earlier fetch costs registers (spills at 128)
     } else if (PIPE == 2) {
         // three register buffers: two hops (336 B fp32 per thread) in flight while a third is computed
         real va[24], ua[18], vb[24], ub[18], vc[24], uc[18];
-        hop_load<0, RO, real>(U, in, s, n.f[0], va, ua);
-        hop_load<0, RO, real>(U, in, n.b[0], n.b[0], vb, ub);
-        hop_load<1, RO, real>(U, in, s, n.f[1], vc, uc);          hop_compute<0, SF, false, real>(va, ua, one, acc);
-        hop_load<1, RO, real>(U, in, n.b[1], n.b[1], va, ua);     hop_compute<0, -SF, true, real>(vb, ub, one, acc);
-        hop_load<2, RO, real>(U, in, s, n.f[2], vb, ub);          hop_compute<1, SF, false, real>(vc, uc, one, acc);
-        hop_load<2, RO, real>(U, in, n.b[2], n.b[2], vc, uc);     hop_compute<1, -SF, true, real>(va, ua, one, acc);
-        hop_load<3, RO, real>(U, in, s, n.f[3], va, ua);          hop_compute<2, SF, false, real>(vb, ub, one, acc);
-        hop_load<3, RO, real>(U, in, n.b[3], n.b[3], vb, ub);     hop_compute<2, -SF, true, real>(vc, uc, one, acc);
+        hop_load<0, RO, RECON, real>(U, in, s, n.f[0], va, ua);
+        hop_load<0, RO, RECON, real>(U, in, n.b[0], n.b[0], vb, ub);
+        hop_load<1, RO, RECON, real>(U, in, s, n.f[1], vc, uc);          hop_compute<0, SF, false, real>(va, ua, one, acc);
+        hop_load<1, RO, RECON, real>(U, in, n.b[1], n.b[1], va, ua);     hop_compute<0, -SF, true, real>(vb, ub, one, acc);
+        hop_load<2, RO, RECON, real>(U, in, s, n.f[2], vb, ub);          hop_compute<1, SF, false, real>(vc, uc, one, acc);
+        hop_load<2, RO, RECON, real>(U, in, n.b[2], n.b[2], vc, uc);     hop_compute<1, -SF, true, real>(va, ua, one, acc);
+        hop_load<3, RO, RECON, real>(U, in, s, n.f[3], va, ua);          hop_compute<2, SF, false, real>(vb, ub, one, acc);
+        hop_load<3, RO, RECON, real>(U, in, n.b[3], n.b[3], vb, ub);     hop_compute<2, -SF, true, real>(vc, uc, one, acc);
         load_spinor_sel<RO>(in, s, c);
         if (LOADR) load_spinor_rw(r, s, rv);
         hop_compute<3, SF, false, real>(va, ua, sgf, acc);
@@ -580,7 +636,7 @@ enum { MODE_PLAIN = 0, MODE_QQ = 1, MODE_RUPD = 2, MODE_RV = 3, MODE_TS = 4 };
 // MODE_RUPD  : s = D q (not stored), r <- r - alpha s, rr' = |r|^2, beta, loop condition   (a3)
 // MODE_RV    : out = v = D p, <rhat, v> (rhat passed as `r`, read only), alpha = rho/<rhat,v>   (BiCGSTAB)
 // MODE_TS    : out = t = D s, <t,s> and <t,t>, omega = <t,s>/<t,t>                              (BiCGSTAB)
-template <typename real, int DAG, int MODE, int BX, int BY, int BZ, int BT, int MINB, int PIPE>
+template <typename real, int DAG, int MODE, int BX, int BY, int BZ, int BT, int MINB, int PIPE, int RECON = 18>
 __global__ void __launch_bounds__(BX *BY *BZ *BT, MINB)
 dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
               const typename Field<real>::svec *__restrict__ in, typename Field<real>::svec *out, real kappa,
@@ -620,8 +676,8 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
         if (!active) continue;
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24], rv[24];
-        hopping_sum<DAG, PIPE, MODE == MODE_RUPD || MODE == MODE_RV, true, real, svec, gvec>(g, U, in, r, x, y, z, t, s,
-                                                                                            acc, c, rv);
+        hopping_sum<DAG, PIPE, MODE == MODE_RUPD || MODE == MODE_RV, true, real, svec, gvec, RECON>(g, U, in, r, x, y, z, t,
+                                                                                                   s, acc, c, rv);
         if constexpr (MODE == MODE_TS) {
             // c holds s(x); t(x) = s(x) - kappa * hops replaces it component by component
             real tsr = 0, tsi = 0, tt = 0;
@@ -1025,7 +1081,7 @@ norm2_kernel(const typename Field<real>::svec *__restrict__ a, size_t n, int V, 
 // ---------------------------------------------------------------- a0: canonical <-> native permutations
 // One thread per (padded) site.  canonical gauge U[s][mu][a][b] (36 complex, contiguous) -> plane mu*9+a*3+b of
 // the site's block; canonical spinor psi[s][alpha][a] (NSP vectors, contiguous) -> plane j.  Pad lanes get zeros.
-template <typename real>
+template <typename real, int RECON = 18>
 __global__ void __launch_bounds__(VEC_NT)
 pack_gauge_kernel(const typename Field<real>::gvec *__restrict__ can, typename Field<real>::gvec *nat, int V, int Vpad)
 {
@@ -1036,7 +1092,8 @@ pack_gauge_kernel(const typename Field<real>::gvec *__restrict__ can, typename F
         gvec k9[9];
 #pragma unroll
         for (int k = 0; k < 9; ++k) k9[k] = s < V ? __ldg(can + (size_t)s * 36 + mu * 9 + k) : gvec();
-        store_link(nat, s, mu, k9);
+        if (RECON == 12) store_link12(nat, s, mu, k9);
+        else store_link(nat, s, mu, k9);
     }
 }
 template <typename real>

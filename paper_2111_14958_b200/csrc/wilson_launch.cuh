@@ -98,11 +98,14 @@ struct DslashArgs {
 // dagger in {0,1}; mode in {MODE_PLAIN, MODE_QQ (dagger = 1 only), MODE_RUPD (dagger = 0 only)}
 cudaError_t launch_dslash_f32(int tile, int dagger, int mode, const DslashArgs &a);
 cudaError_t launch_dslash_f64(int tile, int dagger, int mode, const DslashArgs &a);
+// the same with 12-real link storage (wd_set_gauge_recon(ctx, 12))
+cudaError_t launch_dslash12_f32(int tile, int dagger, int mode, const DslashArgs &a);
+cudaError_t launch_dslash12_f64(int tile, int dagger, int mode, const DslashArgs &a);
 // BiCGSTAB passes (D only): mode in {MODE_RV, MODE_TS}
 cudaError_t launch_dslash_bi_f32(int tile, int mode, const DslashArgs &a);
 cudaError_t launch_dslash_bi_f64(int tile, int mode, const DslashArgs &a);
 
-template <typename real, int DAG, int MODE>
+template <typename real, int DAG, int MODE, int RECON = 18>
 static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
 {
     using svec = typename Field<real>::svec;
@@ -114,7 +117,7 @@ static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
             static int occ = 0;                                                                                \
             if (!occ) {                                                                                        \
                 cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(                                 \
-                    &occ, dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p>, bx * by * bz * bt, 0);         \
+                    &occ, dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON>, bx * by * bz * bt, 0);         \
                 if (e != cudaSuccess) return e;                                                                \
                 if (occ < 1) occ = 1;                                                                          \
             }                                                                                                  \
@@ -122,7 +125,7 @@ static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
             if (grid > a.g.ntiles) grid = a.g.ntiles;                                                          \
             Geom g = a.g;                                                                                      \
             g.pf = a.prefetch < 0 ? (int)grid : a.prefetch;                                                    \
-            dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p><<<(unsigned)grid, bx * by * bz * bt, 0, a.stream>>>(  \
+            dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON><<<(unsigned)grid, bx * by * bz * bt, 0, a.stream>>>(  \
                 g, (const gvec *)a.U, (const svec *)a.in, (svec *)a.out, (real)a.kappa, (svec *)a.r, a.sc,   \
                 a.partials, a.counter, a.hist, a.it);                                                          \
             return cudaGetLastError();                                                                         \
@@ -171,13 +174,14 @@ static cudaError_t launch_cg_onelaunch_any(int small_tile, const CgOneLaunchArgs
     }
 }
 
-template <typename real>
+template <typename real, int RECON = 18>
 static cudaError_t launch_dslash_any(int tile, int dagger, int mode, const DslashArgs &a)
 {
     if (mode == MODE_PLAIN)
-        return dagger ? launch_dslash_tile<real, 1, MODE_PLAIN>(tile, a) : launch_dslash_tile<real, 0, MODE_PLAIN>(tile, a);
-    if (mode == MODE_QQ && dagger) return launch_dslash_tile<real, 1, MODE_QQ>(tile, a);
-    if (mode == MODE_RUPD && !dagger) return launch_dslash_tile<real, 0, MODE_RUPD>(tile, a);
+        return dagger ? launch_dslash_tile<real, 1, MODE_PLAIN, RECON>(tile, a)
+                      : launch_dslash_tile<real, 0, MODE_PLAIN, RECON>(tile, a);
+    if (mode == MODE_QQ && dagger) return launch_dslash_tile<real, 1, MODE_QQ, RECON>(tile, a);
+    if (mode == MODE_RUPD && !dagger) return launch_dslash_tile<real, 0, MODE_RUPD, RECON>(tile, a);
     return cudaErrorInvalidValue;
 }
 

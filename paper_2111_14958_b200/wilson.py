@@ -95,6 +95,8 @@ def load_library(path: str = LIB_PATH):
     lib.wd_get_tile.argtypes = [vp]
     lib.wd_set_cg_mode.argtypes = [vp, ci]
     lib.wd_set_prefetch.argtypes = [vp, ci]
+    lib.wd_set_gauge_recon.argtypes = [vp, ci]
+    lib.wd_get_gauge_recon.argtypes = [vp]
     lib.wd_set_waves.argtypes = [vp, ci]
     lib.wd_set_zchunk.argtypes = [vp, ci]
     lib.wd_set_poll_interval.argtypes = [vp, ci]
@@ -352,6 +354,13 @@ class WilsonContext:
     def wd_set_cg_mode(self, mode):
         """0 automatic, 1 three kernels per iteration, 2 whole solve in one cooperative launch"""
         self._check(self.lib.wd_set_cg_mode(self._ctx, int(mode)))
+
+    def wd_set_gauge_recon(self, reals_per_link):
+        """18 (default) or 12 reals stored per link; call before wd_pack_gauge / empty_gauge"""
+        self._check(self.lib.wd_set_gauge_recon(self._ctx, int(reals_per_link)))
+
+    def wd_get_gauge_recon(self):
+        return int(self.lib.wd_get_gauge_recon(self._ctx))
 
     def wd_set_prefetch(self, tiles):
         self._check(self.lib.wd_set_prefetch(self._ctx, int(tiles)))

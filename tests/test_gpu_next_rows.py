@@ -207,3 +207,70 @@ def test_coo_spmv_any_entry_order_and_duplicates(wilson, oracle):
                                 torch.empty(0, dtype=torch.int32, device="cuda"),
                                 torch.empty(0, dtype=torch.int32, device="cuda"), gu.to_device(x.reshape(256, 4, 3)))
         assert not gu.to_host(empty).any()
+
+
+# ---------------------------------------------------------------- f3: 12-real link storage
+def _apply12(wilson, dims, U, psi, kappa, dagger, precision, bc_t=-1):
+    with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+        n18 = ctx.empty_gauge().numel()
+        ctx.wd_set_gauge_recon(12)
+        assert ctx.wd_get_gauge_recon() == 12 and ctx.empty_gauge().numel() * 3 == n18 * 2
+        return gu.apply_on_gpu(ctx, U, psi, kappa, dagger)
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("cfg_index", [0, 1, 2])
+def test_recon12_wd_apply_baseline_configs(wilson, oracle, cfg_index, precision):
+    """rows 0, 1 stored, row 2 = conj(row0 x row1) rebuilt in the kernel: same per-site tolerance as the 18-real path
+    (the fp32-rounded links are unitary to ~1e-7, far inside 1e-5)"""
+    cfg = inputs.CONFIGS[cfg_index]
+    U, eta = gu.config_fields(cfg.index, precision)
+    for dagger in (False, True):
+        got = _apply12(wilson, cfg.dims, U, eta, cfg.kappa, dagger, precision, cfg.bc_t)
+        want = oracle.wd_apply(cfg.dims, U.astype(np.complex128), eta.astype(np.complex128), cfg.kappa, dagger, cfg.bc_t)
+        assert lm.per_site_rel_err(got, want)[0] <= (1e-5 if precision == 32 else 1e-12)
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("dims", [(5, 7, 4, 6), (18, 4, 6, 4), (4, 4, 4, 34)])
+def test_recon12_ragged(wilson, oracle, dims, precision):
+    cdt = gu.np_complex(precision)
+    U = inputs.gauge_field(CFG_TEST + 20, dims, "haar", dtype=cdt)
+    psi = inputs.source_field(CFG_TEST + 20, dims, dtype=cdt, field=inputs.FIELD_AUX)
+    for bc_t in (-1, 1):
+        got = _apply12(wilson, dims, U, psi, 0.12, bc_t == 1, precision, bc_t)
+        want = oracle.wd_apply(dims, U.astype(np.complex128), psi.astype(np.complex128), 0.12, bc_t == 1, bc_t)
+        assert lm.per_site_rel_err(got, want)[0] <= (1e-5 if precision == 32 else 1e-12)
+
+
+def test_recon12_rebuilds_the_third_row(wilson, oracle):
+    """the stored third row is really ignored: corrupting it in the caller's U changes nothing, and the result equals
+    the oracle's on the UNcorrupted SU(3) field"""
+    dims = (4, 6, 4, 8)
+    U = inputs.gauge_field(CFG_TEST + 21, dims, "haar")
+    psi = inputs.source_field(CFG_TEST + 21, dims, field=inputs.FIELD_AUX)
+    bad = U.copy()
+    bad[:, :, 2, :] = 7.0
+    got = _apply12(wilson, dims, bad, psi, 0.12, False, 64)
+    want = oracle.wd_apply(dims, U, psi, 0.12, False, -1)
+    assert lm.per_site_rel_err(got, want)[0] <= 1e-12
+
+
+@pytest.mark.parametrize("precision,r_min", [(32, 1e-6), (64, 1e-10)])
+@pytest.mark.parametrize("cfg_index", [0, 1, 2])
+def test_recon12_cg_solve(wilson, oracle, cfg_index, precision, r_min):
+    cfg = inputs.CONFIGS[cfg_index]
+    U, eta = gu.config_fields(cfg.index, precision)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        ctx.wd_set_gauge_recon(12)
+        psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, r_min, cfg.max_iter)
+        assert info["cg_mode"] == 1   # the one-launch kernel is 18-real only
+        with pytest.raises(wilson.WilsonError):
+            bicgstab_on_gpu(ctx, U, eta, cfg.kappa, r_min, 10)
+    psi_o, info_o = oracle.cg_solve(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t)
+    assert info["status"] == 0
+    assert abs(info["iterations"] - info_o["iterations"]) <= math.floor(0.02 * info_o["iterations"] + 0.5)
+    res_gpu = oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
+    res_orc = oracle.true_residual(cfg.dims, U64, eta64, psi_o, cfg.kappa, cfg.bc_t)
+    assert res_gpu <= 2.0 * res_orc, (res_gpu, res_orc)
