@@ -2,6 +2,7 @@
 """bench.py — the measurement contract of this repo.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config I] [--precision 32|64] [--impl ours|reference]
+    python bench.py --report | --rows | --sweep        (measurement tables of BASELINE.md; not the bench line)
 
 One "step" = one pass of the whole hot path over one synthetic lattice: cg_solve (a1 init, the fused CG
 loop a2-a5 until |r|/|eta| < r_min, a6 final D-dagger) on BASELINE.json's config I (default 4: 48^3x96,
@@ -236,6 +237,127 @@ def run_report(args):
     return 0
 
 
+FLOP_BICG_ITER = 2 * 1368 + 960   # two D applications + 10 complex vector/dot operations
+BYTES_BICG = {32: (576, 288, 480, 672, 384), 64: (1152, 576, 960, 1344, 768)}   # the five kernels of one iteration
+FLOP_COO_NNZ = 8                   # one complex multiply-add per stored entry
+NNZ_PER_SITE = 588
+
+
+def run_rows(args):
+    """The SURVEY.md 8(f) rows, one JSON line each: BiCGSTAB (f4) and 12-real links (f3) at configs 3 and 4, the paper's
+    COO SpMV (f2) at 14^4 (config 2, the largest volume of the paper's range) beside the matrix-free stencil."""
+    import torch
+
+    from paper_2111_14958_b200 import build as wbuild
+    from paper_2111_14958_b200 import wilson
+
+    wbuild.build()
+    wilson.load_library()
+    peak, _ = measured_peak()
+    prec = args.precision
+    cdt = np.complex64 if prec == 32 else np.complex128
+    rb = 4 if prec == 32 else 8
+    for ci in (3, 4):
+        cfg = inputs.CONFIGS[ci]
+        r_min = cfg.r_min if prec == 32 else 1e-10
+        U, eta = inputs.config_inputs(cfg, dtype=cdt)
+        V = cfg.volume
+        for recon in (18, 12):
+            with wilson.WilsonContext(cfg.dims, prec, cfg.bc_t) as ctx:
+                ctx.wd_set_gauge_recon(recon)
+                Un = ctx.wd_pack_gauge(torch.from_numpy(U).cuda())
+                en = ctx.wd_pack_spinor(torch.from_numpy(eta).cuda())
+                out = ctx.empty_spinor()
+                d_ms = time_wd_apply(ctx, Un, en, out, cfg.kappa, False)
+                for _ in range(2):
+                    ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=out)
+                ctx.wd_set_profile(True)
+                ms = []
+                for _ in range(3):
+                    _, info = ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=out)
+                    ms.append(info["gpu_ms"])
+                p = ctx.wd_get_profile()
+                ctx.wd_set_profile(False)
+                n = max(p["iterations"], 1)
+                gb = (72 if recon == 18 else 48) * rb          # gauge bytes per site
+                sb = 24 * rb                                    # spinor bytes per site
+                b2, b3, b4 = 2 * sb + gb, 3 * sb + gb, 5 * sb
+                a2, a3, a4 = p["a2_ms"] / n, p["a3_ms"] / n, p["a4_ms"] / n
+                t = float(np.median(ms))
+                print(json.dumps({
+                    "row": "f3 link storage", "config": ci, "precision": prec, "reals_per_link": recon,
+                    "bytes_per_site": {"wd_apply": b2, "a2": b2, "a3": b3, "a4": b4, "cg_iteration": b2 + b3 + b4},
+                    "wd_apply_D_us": d_ms * 1e3, "wd_apply_D_gbs": b2 * V / (d_ms * 1e-3) / 1e9,
+                    "cg_iterations": info["iterations"], "cg_solve_ms": t,
+                    "cg_gflops": cg_flops(V, info["iterations"]) / (t * 1e-3) / 1e9,
+                    "a2_us": a2 * 1e3, "a3_us": a3 * 1e3, "a4_us": a4 * 1e3,
+                    "a2_gbs": b2 * V / (a2 * 1e-3) / 1e9, "a3_gbs": b3 * V / (a3 * 1e-3) / 1e9,
+                    "cg_iteration_gbs": (b2 + b3 + b4) * V / ((a2 + a3 + a4) * 1e-3) / 1e9,
+                    "cg_iteration_frac_of_measured": (b2 + b3 + b4) * V / ((a2 + a3 + a4) * 1e-3) / 1e9 / peak}), flush=True)
+                if recon == 18:
+                    for _ in range(2):
+                        ctx.bicgstab_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=out)
+                    ctx.wd_set_profile(True)
+                    ms = []
+                    for _ in range(5):
+                        _, ib = ctx.bicgstab_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=out)
+                        ms.append(ib["gpu_ms"])
+                    pb = ctx.wd_get_profile_bicgstab()
+                    ctx.wd_set_profile(False)
+                    kus = [m / max(pb["iterations"], 1) * 1e3 for m in pb["ms"]]
+                    bb = BYTES_BICG[prec]
+                    tb = float(np.median(ms))
+                    print(json.dumps({
+                        "row": "f4 bicgstab", "config": ci, "precision": prec, "iterations": ib["iterations"],
+                        "status": ib["status"], "rel_residual": ib["rel_residual"], "solve_ms": tb,
+                        "gflops": FLOP_BICG_ITER * V * ib["iterations"] / (tb * 1e-3) / 1e9,
+                        "kernel_us": dict(zip(("Dp_rv", "s", "Ds_ts", "xr", "p"), kus)),
+                        "kernel_gbs": dict(zip(("Dp_rv", "s", "Ds_ts", "xr", "p"),
+                                               [b * V / (u * 1e-6) / 1e9 if u > 0 else None for b, u in zip(bb, kus)])),
+                        "iteration_gbs": sum(bb) * V / (sum(kus) * 1e-6) / 1e9 if sum(kus) > 0 else None,
+                        "iteration_frac_of_measured": sum(bb) * V / (sum(kus) * 1e-6) / 1e9 / peak if sum(kus) > 0 else None,
+                        "cg_solve_ms_same_problem": t, "speedup_vs_cg": t / tb}), flush=True)
+    # f2: the paper's COO SpMV at its largest volume
+    cfg = inputs.CONFIGS[2]
+    U, eta = inputs.config_inputs(cfg, dtype=cdt)
+    V = cfg.volume
+    with wilson.WilsonContext(cfg.dims, prec, cfg.bc_t) as ctx:
+        Un = ctx.wd_pack_gauge(torch.from_numpy(U).cuda())
+        eta_d = torch.from_numpy(eta).cuda()
+        en = ctx.wd_pack_spinor(eta_d)
+        out_n = ctx.empty_spinor()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        val, row, col = ctx.wd_coo_assemble(Un, cfg.kappa, False)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(10):
+            ctx.lib.wd_coo_assemble(ctx._ctx, ctx._p(Un), cfg.kappa, 0, ctx._p(val), ctx._p(row), ctx._p(col))
+        e1.record()
+        torch.cuda.synchronize()
+        asm_ms = e0.elapsed_time(e1) / 10
+        out = torch.empty_like(eta_d)
+        for _ in range(5):
+            ctx.wd_coo_spmv(val, row, col, eta_d, out=out)
+        reps = 100
+        e0.record()
+        for _ in range(reps):
+            ctx.wd_coo_spmv(val, row, col, eta_d, out=out)
+        e1.record()
+        torch.cuda.synchronize()
+        sp_ms = e0.elapsed_time(e1) / reps
+        st_ms = time_wd_apply(ctx, Un, en, out_n, cfg.kappa, False)
+        nnz = NNZ_PER_SITE * V
+        coo_bytes = nnz * (2 * rb + 8) + 2 * 12 * V * 2 * rb   # Val + Row + Col once, in and out vectors once
+        print(json.dumps({
+            "row": "f2 coo spmv", "config": 2, "precision": prec, "nnz": nnz, "assemble_ms": asm_ms,
+            "spmv_us": sp_ms * 1e3, "spmv_gflops_8_per_nnz": FLOP_COO_NNZ * nnz / (sp_ms * 1e-3) / 1e9,
+            "spmv_gbs": coo_bytes / (sp_ms * 1e-3) / 1e9, "spmv_frac_of_measured": coo_bytes / (sp_ms * 1e-3) / 1e9 / peak,
+            "bytes_per_site": coo_bytes / V, "stencil_wd_apply_us": st_ms * 1e3,
+            "stencil_speedup": sp_ms / st_ms,
+            "paper": "about 65 GFLOP/s COO SpMV on an A100-PCIE-40GB (PAPER.md:96), other hardware: context only"}), flush=True)
+    return 0
+
+
 def run_sweep(args, cfg, ctx, wilson, Un, en, psi_n, r_min):
     """Per launch configuration: device time of a2 / a3 / a4 per CG iteration (CUDA events inside the solve) and
     of a standalone wd_apply, as achieved algorithmic GB/s."""
@@ -293,6 +415,9 @@ def main():
     ap.add_argument("--report", action="store_true",
                     help="one JSON line per BASELINE config (0..4, plus config 3 in fp64): wd_apply D / D-dagger over 100 "
                          "applications and the CG solve; the table of BASELINE.md section 3")
+    ap.add_argument("--rows", action="store_true",
+                    help="one JSON line per SURVEY.md 8(f) row: 12-real links and BiCGSTAB at configs 3 and 4, the paper's COO "
+                         "SpMV at 14^4 beside the stencil")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -311,6 +436,8 @@ def main():
     torch.cuda.set_device(local)
     if args.report:
         return run_report(args) if rank == 0 else 0
+    if args.rows:
+        return run_rows(args) if rank == 0 else 0
     dist = None
     if world > 1:
         import torch.distributed as dist

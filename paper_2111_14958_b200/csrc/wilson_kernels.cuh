@@ -363,6 +363,74 @@ __device__ __forceinline__ void reconstruct(const real g[12], real sg, real acc[
     }
 }
 
+// ---------------------------------------------------------------- forward links through shared memory (PIPE = 3)
+// The four forward links U_mu(x) of a site are read exactly once per pass, by the thread that owns x: a pure stream
+// that always misses the caches.  PIPE = 3 takes them out of the register-held software pipeline: every thread
+// copies the links of ITS site of the NEXT tile into its own shared-memory slots with cp.async (no register is held
+// while the copy is in flight, the copy is issued half a tile ahead of its use, and because a thread only ever
+// reads what it copied itself no barrier is needed, only cp.async.wait_all).  Slots are plane-major
+// ([chunk][thread]) so that the 128-bit shared loads of a warp are conflict-free.
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async8(void *smem, const void *gmem)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+template <int NT>
+__device__ __forceinline__ void stage_links(const float2 *__restrict__ U, int s, void *smem, int tid)
+{
+    float4 *sm4 = reinterpret_cast<float4 *>(smem);
+    float2 *sm2 = reinterpret_cast<float2 *>(sm4 + 16 * NT);
+    const float2 *blk = U + (size_t)(s >> SB_SHIFT) * (36 * SB);
+    const int lane = s & (SB - 1);
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        const float4 *p4 = reinterpret_cast<const float4 *>(blk + mu * 9 * SB) + lane;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) cp_async16(sm4 + (mu * 4 + q) * NT + tid, p4 + q * SB);
+        cp_async8(sm2 + mu * NT + tid, blk + mu * 9 * SB + 8 * SB + lane);
+    }
+}
+template <int NT>
+__device__ __forceinline__ void stage_links(const double2 *__restrict__ U, int s, void *smem, int tid)
+{
+    double2 *sm = reinterpret_cast<double2 *>(smem);
+    const double2 *p = U + gauge_index(s);
+#pragma unroll
+    for (int k = 0; k < 36; ++k) cp_async16(sm + k * NT + tid, p + k * SB);
+}
+template <int MU, int NT>
+__device__ __forceinline__ void load_link_sm(const float2 *, const void *smem, int tid, float u[18])
+{
+    const float4 *sm4 = reinterpret_cast<const float4 *>(smem);
+    const float2 *sm2 = reinterpret_cast<const float2 *>(sm4 + 16 * NT);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float4 t = sm4[(MU * 4 + q) * NT + tid];
+        u[4 * q] = t.x; u[4 * q + 1] = t.y; u[4 * q + 2] = t.z; u[4 * q + 3] = t.w;
+    }
+    const float2 t2 = sm2[MU * NT + tid];
+    u[16] = t2.x; u[17] = t2.y;
+}
+template <int MU, int NT>
+__device__ __forceinline__ void load_link_sm(const double2 *, const void *smem, int tid, double u[18])
+{
+    const double2 *sm = reinterpret_cast<const double2 *>(smem);
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        const double2 t = sm[(MU * 9 + k) * NT + tid];
+        u[2 * k] = t.x; u[2 * k + 1] = t.y;
+    }
+}
+// bytes of shared memory per thread of a PIPE = 3 kernel
+template <typename real> constexpr int staged_link_bytes() { return 72 * (int)sizeof(real); }
+
 // One hop, split into its loads and its arithmetic so that the loads of the next hop can be in flight
 // while this one is computed:  acc += sg (1 + S gamma_MU) (x) [U or U^dagger](link_site) in(spinor_site).
 // RO = true: `in` is not written while the kernel runs -> read-only (non-coherent) path; false: coherent loads
@@ -418,10 +486,10 @@ __device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, i
 // hop k+1 are issued before hop k is computed, so every thread keeps one hop (168 B fp32) in flight while
 // it computes (memory-level parallelism without more threads).
 // LOADR: also fetch r(s) into rv together with the centre spinor (MODE_RUPD), so that it too overlaps the last hop.
-template <int DAG, int PIPE, bool LOADR, bool RO, typename real, typename svec, typename gvec, int RECON = 18>
+template <int DAG, int PIPE, bool LOADR, bool RO, typename real, typename svec, typename gvec, int RECON = 18, int NT = 0>
 __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const svec *in,
                                             const svec *r, int x, int y, int z, int t, int s, real acc[24],
-                                            real c[24], real rv[24])
+                                            real c[24], real rv[24], void *smem = nullptr, int next_s = -1)
 {
     constexpr int SF = DAG ? +1 : -1;
     const Hops n = neighbours(g, x, y, z, t, s);
@@ -471,6 +539,28 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
         if (LOADR) load_spinor_rw(r, s, rv);
         hop_compute<3, SF, false, real>(va, ua, sgf, acc);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
+    } else if (PIPE == 3) {
+        // forward hops first, their links from this thread's shared-memory slots (staged one tile ahead); only the
+        // neighbour spinors (and, in the second half, the backward links) go through the register pipeline
+        const int tid = threadIdx.x;
+        real va[24], vb[24], ua[18], ub[18], us[18];
+        load_spinor_sel<RO>(in, n.f[0], va);
+        load_spinor_sel<RO>(in, n.f[1], vb);
+        load_link_sm<0, NT>(U, smem, tid, us);               hop_compute<0, SF, false, real>(va, us, one, acc);
+        load_spinor_sel<RO>(in, n.f[2], va);
+        load_link_sm<1, NT>(U, smem, tid, us);               hop_compute<1, SF, false, real>(vb, us, one, acc);
+        load_spinor_sel<RO>(in, n.f[3], vb);
+        load_link_sm<2, NT>(U, smem, tid, us);               hop_compute<2, SF, false, real>(va, us, one, acc);
+        hop_load<0, RO, RECON, real>(U, in, n.b[0], n.b[0], va, ua);
+        load_link_sm<3, NT>(U, smem, tid, us);               hop_compute<3, SF, false, real>(vb, us, sgf, acc);
+        // the slots are free: stage the forward links of this thread's site of the next tile
+        if (next_s >= 0) stage_links<NT>(U, next_s, smem, tid);
+        hop_load<1, RO, RECON, real>(U, in, n.b[1], n.b[1], vb, ub);  hop_compute<0, -SF, true, real>(va, ua, one, acc);
+        hop_load<2, RO, RECON, real>(U, in, n.b[2], n.b[2], va, ua);  hop_compute<1, -SF, true, real>(vb, ub, one, acc);
+        hop_load<3, RO, RECON, real>(U, in, n.b[3], n.b[3], vb, ub);  hop_compute<2, -SF, true, real>(va, ua, one, acc);
+        load_spinor_sel<RO>(in, s, c);
+        hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
+        if (LOADR) load_spinor_rw(r, s, rv);
     }
 }
 
@@ -653,6 +743,20 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     const int lx = tid % BX, ly = (tid / BX) % BY, lz = (tid / (BX * BY)) % BZ, lt = tid / (BX * BY * BZ);
     const real alpha = (MODE == MODE_RUPD) ? (real)sc->alpha : (real)0;
     double local = 0.0, local1 = 0.0, local2 = 0.0;
+    extern __shared__ __align__(16) unsigned char wd_dyn_smem[];   // PIPE = 3: staged forward links, 72 reals per thread
+    // site of this thread in tile b, or -1 (no such tile / thread outside the lattice)
+    auto site_in_tile = [&](int b) -> int {
+        if (b >= g.ntiles) return -1;
+        int tx, ty, tz, tt;
+        tile_of_block(g, b, tx, ty, tz, tt);
+        const int x = tx * BX + lx, y = ty * BY + ly, z = tz * BZ + lz, t = tt * BT + lt;
+        if (x >= g.L[0] || y >= g.L[1] || z >= g.L[2] || t >= g.L[3]) return -1;
+        return x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
+    };
+    if (PIPE == 3) {
+        const int s0 = site_in_tile(blockIdx.x);
+        if (s0 >= 0) stage_links<NT>(U, s0, wd_dyn_smem, tid);
+    }
     // Persistent CTAs: the grid is one resident wave; CTA i takes tiles i, i + gridDim.x, ... so that at any
     // moment the chip works on gridDim.x consecutive tiles of the rasterisation (L2 locality) and the
     // reduction epilogue (barriers, fence, ticket) is paid once per CTA, not once per tile.
@@ -673,11 +777,17 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
         tile_of_block(g, b, tx, ty, tz, tt);
         const int x = tx * BX + lx, y = ty * BY + ly, z = tz * BZ + lz, t = tt * BT + lt;
         const bool active = (x < g.L[0]) && (y < g.L[1]) && (z < g.L[2]) && (t < g.L[3]);
+        int next_s = -1;
+        if (PIPE == 3) {
+            next_s = site_in_tile(b + gridDim.x);
+            cp_async_wait_all();                       // this thread's own copies for tile b have landed
+            if (!active && next_s >= 0) stage_links<NT>(U, next_s, wd_dyn_smem, tid);
+        }
         if (!active) continue;
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24], rv[24];
-        hopping_sum<DAG, PIPE, MODE == MODE_RUPD || MODE == MODE_RV, true, real, svec, gvec, RECON>(g, U, in, r, x, y, z, t,
-                                                                                                   s, acc, c, rv);
+        hopping_sum<DAG, PIPE, MODE == MODE_RUPD || MODE == MODE_RV, true, real, svec, gvec, RECON, NT>(
+            g, U, in, r, x, y, z, t, s, acc, c, rv, wd_dyn_smem, next_s);
         if constexpr (MODE == MODE_TS) {
             // c holds s(x); t(x) = s(x) - kappa * hops replaces it component by component
             real tsr = 0, tsi = 0, tt = 0;

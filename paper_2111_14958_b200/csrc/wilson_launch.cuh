@@ -1,7 +1,8 @@
 // wilson_launch.cuh — the table of compiled stencil launch configurations and the per-precision launchers.
 // A "tile" (the name of the C ABI, wd_set_tile) is one row: CTA tile BX x BY x BZ x BT (threads per CTA =
 // product), MINB = minimum resident CTAs per SM asked of ptxas (bounds registers per thread), PIPE = 1 for
-// the software-pipelined hop loop (2 = three register buffers).  This is the CUDA analogue of the paper's workgroup-size knob
+// the software-pipelined hop loop (2 = three register buffers, 3 = forward links staged through shared memory with
+// cp.async one tile ahead, 18-real links only).  This is the CUDA analogue of the paper's workgroup-size knob
 // (PAPER.md:58,76).  F64 = 1 if the row is also compiled for double precision.
 #pragma once
 #include "wilson_kernels.cuh"
@@ -26,8 +27,9 @@
     X(13, 4, 4, 4, 2, 2, 1, 1) \
     X(14, 16, 2, 2, 2, 0, 0, 1) \
     X(15, 8, 4, 4, 2, 0, 0, 1) \
-    X(16, 16, 2, 2, 2, 3, 2, 0)
-#define WD_NUM_TILES 17
+    X(16, 16, 2, 2, 2, 3, 2, 0) \
+    X(17, 16, 2, 2, 2, 4, 3, 0)
+#define WD_NUM_TILES 18
 
 // Launch configurations of the one-launch CG kernel (small volumes): 64- and 128-thread tiles,
 // no register bound (ptxas then hoists the loads of all 8 hops: one memory round trip per site instead of 8,
@@ -113,11 +115,16 @@ static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
     switch (tile) {
 #define X(i, bx, by, bz, bt, m, p, f)                                                                          \
     case i:                                                                                                    \
-        if constexpr (sizeof(real) == 4 || f) {                                                                \
+        if constexpr ((sizeof(real) == 4 || f) && !(p == 3 && RECON != 18)) {                                  \
             static int occ = 0;                                                                                \
+            const size_t dyn = (p == 3) ? (size_t)(bx * by * bz * bt) * staged_link_bytes<real>() : 0;         \
             if (!occ) {                                                                                        \
-                cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(                                 \
-                    &occ, dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON>, bx * by * bz * bt, 0);         \
+                auto kern = dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON>;                       \
+                if (dyn > 48 * 1024) {                                                                         \
+                    cudaError_t e2 = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); \
+                    if (e2 != cudaSuccess) return e2;                                                          \
+                }                                                                                              \
+                cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, bx * by * bz * bt, dyn); \
                 if (e != cudaSuccess) return e;                                                                \
                 if (occ < 1) occ = 1;                                                                          \
             }                                                                                                  \
@@ -125,7 +132,7 @@ static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
             if (grid > a.g.ntiles) grid = a.g.ntiles;                                                          \
             Geom g = a.g;                                                                                      \
             g.pf = a.prefetch < 0 ? (int)grid : a.prefetch;                                                    \
-            dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON><<<(unsigned)grid, bx * by * bz * bt, 0, a.stream>>>(  \
+            dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON><<<(unsigned)grid, bx * by * bz * bt, dyn, a.stream>>>(  \
                 g, (const gvec *)a.U, (const svec *)a.in, (svec *)a.out, (real)a.kappa, (svec *)a.r, a.sc,   \
                 a.partials, a.counter, a.hist, a.it);                                                          \
             return cudaGetLastError();                                                                         \
