@@ -68,6 +68,10 @@ def _load():
         lib.oracle_coo_assemble.restype = ctypes.c_int
         lib.oracle_coo_spmv.argtypes = [ctypes.c_long, dp, ip, ip, dp, dp, ctypes.c_long]
         lib.oracle_coo_spmv.restype = ctypes.c_int
+        lib.oracle_cg_solve_eo.argtypes = lib.oracle_cg_solve.argtypes
+        lib.oracle_cg_solve_eo.restype = ctypes.c_int
+        lib.oracle_schur_apply.argtypes = lib.oracle_wd_apply.argtypes
+        lib.oracle_schur_apply.restype = ctypes.c_int
         lib.oracle_norm2.argtypes = [dp, ctypes.c_long]
         lib.oracle_norm2.restype = ctypes.c_double
         lib.oracle_num_threads.restype = ctypes.c_int
@@ -164,6 +168,45 @@ def bicgstab_solve(dims, U, eta, kappa, r_min, max_iter, bc_t=-1, history=False)
         ctypes.byref(info), _ptr(hist) if history else None)
     if rc < 0:
         raise RuntimeError(f"oracle_bicgstab_solve failed: {rc}")
+    out = {
+        "iterations": info.iterations,
+        "converged": bool(info.converged),
+        "rel_residual": info.rel_residual,
+        "eta_norm2": info.eta_norm2,
+        "seconds": info.seconds,
+        "status": rc,
+    }
+    if history:
+        out["rr_history"] = hist[: info.iterations + 1].copy()
+    return psi, out
+
+
+def schur_apply(dims, U, v, kappa, dagger=False, bc_t=-1):
+    """Mhat v_e = (1 - kappa^2 H_eo H_oe) v_e (or Mhat-dagger) on the even part of v; odd sites of the result are 0."""
+    d, vol = _dims(dims)
+    U = _c128(U, (vol, 4, 3, 3))
+    v = _c128(v, (vol, 4, 3))
+    out = np.empty_like(v)
+    rc = _load().oracle_schur_apply(d, int(bc_t), _ptr(U), _ptr(v), _ptr(out), float(kappa), int(bool(dagger)))
+    if rc != 0:
+        raise RuntimeError(f"oracle_schur_apply failed: {rc}")
+    return out
+
+
+def cg_solve_eo(dims, U, eta, kappa, r_min, max_iter, bc_t=-1, history=False):
+    """Even-odd preconditioned CG (reading E1): the paper's recurrence on Mhat Mhat-dagger, then
+    psi_e = Mhat-dagger y and psi_o = eta_o + kappa H_oe psi_e.  Returns (psi, info) like cg_solve."""
+    d, vol = _dims(dims)
+    U = _c128(U, (vol, 4, 3, 3))
+    eta = _c128(eta, (vol, 4, 3))
+    psi = np.empty_like(eta)
+    info = OracleCgInfo()
+    hist = np.zeros(max_iter + 1, dtype=np.float64) if history else None
+    rc = _load().oracle_cg_solve_eo(
+        d, int(bc_t), _ptr(U), _ptr(eta), _ptr(psi), float(kappa), float(r_min), int(max_iter),
+        ctypes.byref(info), _ptr(hist) if history else None)
+    if rc < 0:
+        raise RuntimeError(f"oracle_cg_solve_eo failed: {rc}")
     out = {
         "iterations": info.iterations,
         "converged": bool(info.converged),

@@ -518,3 +518,107 @@ def test_cp2_coo_spmv_equals_stencil(oracle):
     ref = np.zeros(psi.size, dtype=np.complex128)
     np.add.at(ref, row, val * psi.reshape(-1)[col])
     assert np.max(np.abs(ref - got.reshape(-1))) < 1e-13
+
+
+# ---------------------------------------------------------------- even-odd preconditioned CG (reading E1)
+def _parity(dims):
+    return lm.coords(dims).sum(axis=1) & 1
+
+
+def _dense_blocks(dims, U, kappa, bc_t):
+    """M_ee, M_eo, M_oe, M_oo of the Kronecker-built dense D, and the component index sets of the two parities"""
+    M = lm.dense_wilson(dims, U, kappa, bc_t)
+    par = np.repeat(_parity(dims), 12)
+    e, o = np.nonzero(par == 0)[0], np.nonzero(par == 1)[0]
+    return M, e, o
+
+
+@pytest.mark.parametrize("dims", [(2, 2, 2, 2), (4, 2, 2, 4)])
+@pytest.mark.parametrize("bc_t", [-1, +1])
+def test_ep1_schur_operator_is_the_dense_schur_complement(oracle, dims, bc_t):
+    kappa = 0.12
+    U = inputs.gauge_field(CFG_TEST + 40, dims, "haar")
+    v = rand_spinor(CFG_TEST + 40, dims)
+    M, e, o = _dense_blocks(dims, U, kappa, bc_t)
+    assert np.allclose(M[np.ix_(e, e)], np.eye(e.size)) and np.allclose(M[np.ix_(o, o)], np.eye(o.size))
+    S = M[np.ix_(e, e)] - M[np.ix_(e, o)] @ M[np.ix_(o, e)]      # D_ee - D_eo D_oo^-1 D_oe with D_oo = 1
+    for dagger, A in ((False, S), (True, S.conj().T)):
+        got = oracle.schur_apply(dims, U, v, kappa, dagger, bc_t).reshape(-1)
+        assert np.max(np.abs(got[e] - A @ v.reshape(-1)[e])) < 1e-13
+        assert not got[o].any()
+
+
+@pytest.mark.parametrize("bc_t", [-1, +1])
+def test_ep2_eo_cg_matches_dense_solve_and_plain_cg(oracle, bc_t):
+    dims = (4, 2, 2, 4)
+    kappa = 0.12
+    U = inputs.gauge_field(CFG_TEST + 41, dims, "haar")
+    eta = inputs.source_field(CFG_TEST + 41, dims)
+    M = lm.dense_wilson(dims, U, kappa, bc_t)
+    exact = np.linalg.solve(M, eta.reshape(-1)).reshape(eta.shape)
+    psi, info = oracle.cg_solve_eo(dims, U, eta, kappa, 1e-12, 500, bc_t, history=True)
+    assert info["converged"] and info["status"] == 0
+    assert np.linalg.norm(psi - exact) < 1e-10 * np.linalg.norm(exact)
+    # the recursed residual IS the true residual of the full system (its odd rows vanish identically)
+    assert abs(oracle.true_residual(dims, U, eta, psi, kappa, bc_t) - info["rel_residual"]) < 1e-12
+    r_full = (eta - oracle.wd_apply(dims, U, psi, kappa, False, bc_t)).reshape(-1, 12)
+    assert np.max(np.abs(r_full[_parity(dims) == 1])) < 1e-13
+    # first history entry: <etahat, etahat> with etahat = eta_e - M_eo eta_o from the dense blocks
+    _, e, o = _dense_blocks(dims, U, kappa, bc_t)
+    etahat = eta.reshape(-1)[e] - M[np.ix_(e, o)] @ eta.reshape(-1)[o]
+    assert info["rr_history"][0] == pytest.approx(np.vdot(etahat, etahat).real, rel=1e-13)
+    assert info["eta_norm2"] == pytest.approx(np.vdot(eta, eta).real, rel=1e-13)
+    # same solution as the unpreconditioned recurrence, in fewer iterations
+    psi_p, info_p = oracle.cg_solve(dims, U, eta, kappa, 1e-12, 500, bc_t)
+    assert np.linalg.norm(psi - psi_p) < 1e-10 * np.linalg.norm(psi_p)
+    assert info["iterations"] < info_p["iterations"]
+
+
+def test_ep3_eo_cg_first_step_and_finite_termination(oracle):
+    """one step retyped from the dense Schur complement (pins alpha, the order Mhat-dagger then Mhat, and the
+    reconstruction of psi_o); free field on 2^4: as many iterations as Mhat Mhat-dagger has distinct eigenvalues"""
+    dims = (2, 2, 2, 2)
+    kappa = 0.11
+    U = inputs.gauge_field(CFG_TEST + 42, dims, "haar")
+    eta = inputs.source_field(CFG_TEST + 42, dims)
+    M, e, o = _dense_blocks(dims, U, kappa, -1)
+    S = M[np.ix_(e, e)] - M[np.ix_(e, o)] @ M[np.ix_(o, e)]
+    b = eta.reshape(-1)
+    etahat = b[e] - M[np.ix_(e, o)] @ b[o]
+    q = S.conj().T @ etahat
+    alpha = np.vdot(etahat, etahat).real / np.vdot(q, q).real
+    psi_e = S.conj().T @ (alpha * etahat)
+    want = np.zeros_like(b)
+    want[e] = psi_e
+    want[o] = b[o] - M[np.ix_(o, e)] @ psi_e
+    psi, info = oracle.cg_solve_eo(dims, U, eta, kappa, 1e-30, 1, -1)
+    assert info["iterations"] == 1 and info["status"] == 1
+    assert np.linalg.norm(psi.reshape(-1) - want) < 1e-13 * np.linalg.norm(want)
+    Uf = unit_gauge(dims)
+    for bc_t in (-1, +1):
+        Mf, e, o = _dense_blocks(dims, Uf, 0.1, bc_t)
+        Sf = Mf[np.ix_(e, e)] - Mf[np.ix_(e, o)] @ Mf[np.ix_(o, e)]
+        n_ev = len(np.unique(np.round(np.linalg.eigvalsh(Sf @ Sf.conj().T), 10)))
+        psi, info = oracle.cg_solve_eo(dims, Uf, eta, 0.1, 1e-11, 50, bc_t)
+        assert info["iterations"] == n_ev and info["converged"]
+        exact = np.linalg.solve(Mf, eta.reshape(-1)).reshape(eta.shape)
+        assert np.linalg.norm(psi - exact) < 1e-10 * np.linalg.norm(exact)
+
+
+def test_ep4_eo_cg_baseline_configs_and_edge_cases(oracle):
+    for ci in (0, 1):
+        cfg = inputs.CONFIGS[ci]
+        U, eta = inputs.config_inputs(cfg)
+        pe, ie = oracle.cg_solve_eo(cfg.dims, U, eta, cfg.kappa, 1e-10, cfg.max_iter, cfg.bc_t)
+        pp, ip = oracle.cg_solve(cfg.dims, U, eta, cfg.kappa, 1e-10, cfg.max_iter, cfg.bc_t)
+        assert ie["converged"] and ie["iterations"] < 0.7 * ip["iterations"]
+        assert np.linalg.norm(pe - pp) < 1e-8 * np.linalg.norm(pp)
+        assert oracle.true_residual(cfg.dims, U, eta, pe, cfg.kappa, cfg.bc_t) < 1e-10
+    z, iz = oracle.cg_solve_eo(cfg.dims, U, np.zeros_like(eta), cfg.kappa, 1e-6, 10)
+    assert iz["iterations"] == 0 and iz["converged"] and not z.any()
+    # max_iter = 0: psi_e = 0 and psi_o = eta_o (the exact odd rows for psi_e = 0)
+    z, iz = oracle.cg_solve_eo(cfg.dims, U, eta, cfg.kappa, 1e-6, 0)
+    par = _parity(cfg.dims)
+    assert iz["iterations"] == 0 and iz["status"] == 1 and not z[par == 0].any() and np.array_equal(z[par == 1], eta[par == 1])
+    with pytest.raises(RuntimeError):
+        oracle.cg_solve_eo((4, 3, 4, 4), U[:192], eta[:192], 0.1, 1e-6, 10)   # odd extent
