@@ -81,7 +81,7 @@ typedef struct wd_cg_info {
     double gpu_ms;         /* device time of init + loop + final D-dagger (CUDA events on the ctx stream) */
     double total_ms;       /* *_host calls: device time including H2D copies, pack, solve, unpack, D2H; else = gpu_ms */
     int kernel_launches;   /* number of this library's kernels launched by the call */
-    int cg_mode;           /* 1 = three kernels per iteration, 2 = whole solve in one cooperative launch, 3 = BiCGSTAB */
+    int cg_mode;           /* 1 = three kernels per iteration, 2 = whole solve in one cooperative launch, 3 = BiCGSTAB, 4 = even-odd CG */
 } wd_cg_info;
 
 /*
@@ -180,6 +180,37 @@ int bicgstab_solve(wd_ctx *ctx, const void *U_native, const void *eta_native, vo
                    double kappa, double r_min, int max_iter, wd_cg_info *info);
 
 /*
+ * Even-odd (Schur) preconditioned CG ("the solver performance is often improved by preconditioning",
+ * PAPER.md:32).  Reading E1: sites are coloured by the parity of x+y+z+t (all four extents must be even);
+ * the hopping term H of D = 1 - kappa H connects opposite parities only, so D psi = eta is equivalent to
+ *     Mhat psi_e = etahat,   Mhat = 1 - kappa^2 H_eo H_oe,   etahat = eta_e + kappa H_eo eta_o,
+ *     psi_o = eta_o + kappa H_oe psi_e.
+ * cg_solve_eo runs the paper's CG recurrence (readings G1-G5) on Mhat Mhat-dagger over half-length
+ * vectors, then psi_e = Mhat-dagger y.  The loop test is sqrt(<r,r>) < r_min*sqrt(<eta,eta>) with the FULL source eta:
+ * <r,r> is the squared true residual of the full system, because the odd rows of eta - D psi vanish identically.
+ * Per iteration: two plain half-lattice hop passes, two with the fused CG epilogues of cg_solve (|q|^2; r update +
+ * |r|^2), one fused axpy-xpay.
+ *
+ * Checkerboard ("eo") native layouts: two halves, even parity first; inside a half the site index is (lexicographic
+ * index)/2 and the data is blocked exactly like the plain native layout.  18-real links only.
+ *   wd_eo_spinor_bytes / wd_eo_gauge_bytes   sizes of the device buffers the caller allocates.
+ *   wd_eo_pack_spinor / wd_eo_unpack_spinor / wd_eo_pack_gauge   permutations canonical <-> eo native (device pointers).
+ *   wd_eo_hop(ctx, U_eo, in_eo, out_eo, out_parity, dagger)   out(x) = sum over the 8 hops (H in)(x) (H-dagger for
+ *       dagger != 0) on the sites of parity out_parity, read from the other half of in_eo; the other half of out_eo is
+ *       not touched.  No kappa, no diagonal term.  Asynchronous.
+ *   cg_solve_eo   arguments as cg_solve with eo-native buffers; info->cg_mode = 4.  Synchronous.
+ * Errors: WD_ERR_DIMS for an odd extent, WD_ERR_ARG (NULL, aliasing, 12-real links selected), WD_ERR_CUDA, WD_ERR_ALLOC.
+ */
+size_t wd_eo_spinor_bytes(wd_ctx *ctx);
+size_t wd_eo_gauge_bytes(wd_ctx *ctx);
+int wd_eo_pack_spinor(wd_ctx *ctx, const void *psi_canonical_dev, void *psi_eo_dev);
+int wd_eo_unpack_spinor(wd_ctx *ctx, const void *psi_eo_dev, void *psi_canonical_dev);
+int wd_eo_pack_gauge(wd_ctx *ctx, const void *U_canonical_dev, void *U_eo_dev);
+int wd_eo_hop(wd_ctx *ctx, const void *U_eo, const void *in_eo, void *out_eo, int out_parity, int dagger);
+int cg_solve_eo(wd_ctx *ctx, const void *U_eo, const void *eta_eo, void *psi_eo_out,
+                double kappa, double r_min, int max_iter, wd_cg_info *info);
+
+/*
  * The paper's own route: "we store the sparse matrix D in the so-called coordinate format, i.e. D is
  * stored using three arrays: one array contains the value of the non-zero elements and the other two arrays the
  * corresponding row and column indices", and the SpMV loop
@@ -272,7 +303,9 @@ int wd_set_poll_interval(wd_ctx *ctx, int n);
 int wd_set_profile(wd_ctx *ctx, int on);
 int wd_get_profile(wd_ctx *ctx, double ms[3], long *iterations);
 /* The same for bicgstab_solve: ms[0..4] = accumulated milliseconds of its five kernels (D p + <rhat,v>; s update;
- * D s + dots; psi/r update + dots; p update) over *iters sampled iterations (the first of every poll chunk). */
+ * D s + dots; psi/r update + dots; p update) over *iters sampled iterations (the first of every poll chunk).
+ * After cg_solve_eo the same call returns its five kernels (H-dagger_oe p; Mhat-dagger tail + |q|^2; H_oe q; Mhat tail
+ * + r update + |r|^2; axpy-xpay). */
 int wd_get_profile_bicgstab(wd_ctx *ctx, double ms[5], long *iterations);
 
 /* Host-only self-test of the fast-division constants of the CTA tile decode: returns the number of n in

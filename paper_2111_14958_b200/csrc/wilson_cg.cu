@@ -18,25 +18,6 @@ using namespace wd;
 
 char g_create_err[512] = "";
 
-static long tile_blocks(const wd_ctx *c, int tile)
-{
-    long n = 1;
-    for (int d = 0; d < 4; ++d) n *= (c->dims[d] + kTiles[tile].b[d] - 1) / kTiles[tile].b[d];
-    return n;
-}
-static FastDiv make_fastdiv(unsigned int d)
-{
-    FastDiv f;
-    f.d = d;
-    if (d <= 1) { f.d = 1; f.M = 0; f.sh = -1; return f; }
-    int s = 0;
-    while ((1u << s) < d) ++s;                       // s = ceil(log2 d) >= 1
-    const unsigned long long p2 = 1ull << (31 + s);
-    f.M = (unsigned int)((p2 + d - 1) / d);          // in [2^31, 2^32)
-    f.sh = s - 1;                                    // (n*M) >> (31+s) = umulhi(n,M) >> (s-1)
-    return f;
-}
-
 /* Host self-test of the fast-division constants used by the tile decode: number of n in [0, n_max) for which
    (n * M) >> (32 + sh) differs from n / d (0 = correct).  No GPU needed. */
 extern "C" long wd_selftest_fastdiv(unsigned int d, unsigned int n_max)
@@ -51,64 +32,6 @@ extern "C" long wd_selftest_fastdiv(unsigned int d, unsigned int n_max)
     return bad;
 }
 
-static Geom make_geom_dims(const wd_ctx *c, const int tb[4], int zchunk_user);
-static Geom make_geom(const wd_ctx *c, int tile) { return make_geom_dims(c, kTiles[tile].b, c->zchunk_user); }
-static Geom make_geom_dims(const wd_ctx *c, const int tb[4], int zchunk_user)
-{
-    Geom g;
-    for (int d = 0; d < 4; ++d) {
-        g.L[d] = c->dims[d];
-        g.nt[d] = (c->dims[d] + tb[d] - 1) / tb[d];
-    }
-    g.V = c->V;
-    g.bc_t = c->bc_t;
-    // z chunk of the CTA rasterisation: the largest divisor of the z tile count whose t-reuse distance
-    // Lx*Ly*(zc*BZ)*BT sites * ~600 B (spinor in/out, gauge, halos) stays within the L2 budget.
-    const double layer = 600.0 * c->dims[0] * c->dims[1] * tb[3];   // bytes per z layer of one t-tile row
-    const double budget = c->l2_budget_mb * 1.0e6;
-    int zc = 1;
-    if (zchunk_user > 0) {
-        zc = (zchunk_user + tb[2] - 1) / tb[2];
-        if (zc > g.nt[2]) zc = g.nt[2];
-    } else {
-        for (int d = 1; d <= g.nt[2]; ++d)
-            if (g.nt[2] % d == 0 && layer * d * tb[2] <= budget) zc = d;
-    }
-    g.zc = zc;
-    g.ntiles = g.nt[0] * g.nt[1] * g.nt[2] * g.nt[3];
-    g.pf = 0;   // set per launch (needs the grid size)
-    g.d_chunk = make_fastdiv((unsigned)(g.nt[0] * g.nt[1] * g.zc * g.nt[3]));
-    g.d_nt0 = make_fastdiv((unsigned)g.nt[0]);
-    g.d_nt1 = make_fastdiv((unsigned)g.nt[1]);
-    g.d_zc = make_fastdiv((unsigned)g.zc);
-    const int zlast = g.nt[2] % g.zc ? g.nt[2] % g.zc : g.zc;
-    g.d_zlast = make_fastdiv((unsigned)zlast);
-    return g;
-}
-static int tile_threads(int tile)
-{
-    return kTiles[tile].b[0] * kTiles[tile].b[1] * kTiles[tile].b[2] * kTiles[tile].b[3];
-}
-static bool tile_ok(const wd_ctx *c, int tile)
-{
-    if (tile < 0 || tile >= WD_NUM_TILES) return false;
-    if (c->precision == 64 && !kTiles[tile].f64) return false;
-    return true;
-}
-// Automatic choice: the first row of the table (rows are in order of measured preference) among those compiled
-// for this precision that waste the fewest threads on tiles overhanging the lattice.
-static int auto_tile(const wd_ctx *c)
-{
-    int best = -1;
-    double best_waste = 1e300;
-    for (int t = 0; t < WD_NUM_TILES; ++t) {
-        if (!tile_ok(c, t)) continue;
-        const double waste = (double)tile_blocks(c, t) * tile_threads(t) / (double)c->V;
-        if (waste < best_waste - 1e-12) { best_waste = waste; best = t; }
-    }
-    return best;
-}
-
 // ---------------------------------------------------------------- launches
 template <int DAG, int MODE>
 static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void *out, double kappa, void *r, int it)
@@ -119,8 +42,9 @@ static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void 
     a.waves = c->waves > 0 ? c->waves : 1;
     a.prefetch = (c->dims[0] % SB == 0 && c->recon == 18) ? c->prefetch : 0;
     a.stream = c->stream;
-    a.U = U; a.in = in; a.out = out; a.kappa = kappa; a.r = r;
-    a.sc = c->sc; a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = it;
+    a.U = U; a.Ub = U; a.in = in; a.cen = in; a.out = out; a.kappa = kappa; a.r = r;
+    a.sc = MODE == MODE_PLAIN ? nullptr : c->sc;
+    a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = it;
     c->launches++;
     if (c->recon == 12)
         return c->precision == 32 ? launch_dslash12_f32(c->tile, DAG, MODE, a) : launch_dslash12_f64(c->tile, DAG, MODE, a);
@@ -134,7 +58,7 @@ static unsigned int vec_grid(const wd_ctx *c, size_t n)
     return (unsigned int)(need < cap ? (need ? need : 1) : cap);
 }
 
-static int ensure_workspace(wd_ctx *c, int max_iter)
+int wd_ensure_workspace(wd_ctx *c, int max_iter)
 {
     const size_t sb = spinor_bytes(c);
     if (!c->r) {
@@ -232,7 +156,7 @@ extern "C" int wd_destroy(wd_ctx *c)
 {
     if (!c) return WD_OK;
     cudaStreamSynchronize(c->stream);
-    void *dev[] = {c->r, c->p, c->q, c->y, c->w5, c->sc, c->partials, c->counter, c->hist, c->result_dev,
+    void *dev[] = {c->r, c->p, c->q, c->y, c->w5, c->w6, c->eo_n2, c->sc, c->partials, c->counter, c->hist, c->result_dev,
                    c->U_can, c->U_nat, c->s_can, c->s_nat_in, c->s_nat_out};
     for (void *ptr : dev)
         if (ptr) cudaFree(ptr);
@@ -477,7 +401,7 @@ static int cg_onelaunch(wd_ctx *c, const void *U, const void *eta, void *psi, do
 static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, double kappa, double r_min, int max_iter,
                      wd_cg_info *info, bool record_events)
 {
-    int rc = ensure_workspace(c, max_iter);
+    int rc = wd_ensure_workspace(c, max_iter);
     if (rc != WD_OK) return rc;
     if (use_onelaunch(c)) {
         c->last_cg_mode = 2;
@@ -619,7 +543,7 @@ static cudaError_t launch_dslash_bi(wd_ctx *c, const void *U, const void *in, vo
     a.waves = c->waves > 0 ? c->waves : 1;
     a.prefetch = 0;
     a.stream = c->stream;
-    a.U = U; a.in = in; a.out = out; a.kappa = kappa; a.r = rhat;
+    a.U = U; a.Ub = U; a.in = in; a.cen = in; a.out = out; a.kappa = kappa; a.r = rhat;
     a.sc = c->sc; a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = it;
     c->launches++;
     return c->precision == 32 ? launch_dslash_bi_f32(c->tile, MODE, a) : launch_dslash_bi_f64(c->tile, MODE, a);
@@ -687,7 +611,7 @@ extern "C" int bicgstab_solve(wd_ctx *c, const void *U, const void *eta, void *p
     int rc = check_cg_args(c, U, eta, psi, kappa, r_min, max_iter, "bicgstab_solve");
     if (rc != WD_OK) return rc;
     if (c->recon != 18) return fail(c, WD_ERR_ARG, "bicgstab_solve: compiled for 18-real links only (wd_set_gauge_recon)");
-    rc = ensure_workspace(c, max_iter);
+    rc = wd_ensure_workspace(c, max_iter);
     if (rc != WD_OK) return rc;
     if (!c->w5) {
         CUDA_TRY(c, cudaMalloc(&c->w5, spinor_bytes(c)));

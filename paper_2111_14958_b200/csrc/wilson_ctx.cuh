@@ -27,7 +27,9 @@ struct wd_ctx {
     int sm_count;
     // CG workspace (native layout), device
     void *r, *p, *q, *y;
-    void *w5;             // fifth work vector (BiCGSTAB: t)
+    void *w5;             // fifth work vector (BiCGSTAB: t; even-odd: the odd-parity intermediate)
+    void *w6;             // even-odd: etahat (half length)
+    double *eo_n2;        // even-odd: <eta_e,eta_e>, <eta_o,eta_o> (device)
     wd::CgScalars *sc;
     double *partials;
     size_t partials_cap;
@@ -85,3 +87,96 @@ static inline size_t spinor_can_bytes(const wd_ctx *c) { return (size_t)24 * c->
 static inline size_t gauge_can_bytes(const wd_ctx *c) { return (size_t)72 * c->V * real_bytes(c); }      // canonical
 static inline size_t spinor_vecs(const wd_ctx *c) { return (size_t)(c->precision == 32 ? 6 : 12) * vpad(c); }
 
+
+// CG workspace of the ctx (r, p, q, y at full length, zeroed once; history of max_iter + 1 doubles); wilson_cg.cu
+int wd_ensure_workspace(wd_ctx *c, int max_iter);
+
+// ---------------------------------------------------------------- geometry helpers shared by the ABI translation units
+static inline wd::FastDiv make_fastdiv(unsigned int d)
+{
+    wd::FastDiv f;
+    f.d = d;
+    if (d <= 1) { f.d = 1; f.M = 0; f.sh = -1; return f; }
+    int s = 0;
+    while ((1u << s) < d) ++s;                       // s = ceil(log2 d) >= 1
+    const unsigned long long p2 = 1ull << (31 + s);
+    f.M = (unsigned int)((p2 + d - 1) / d);          // in [2^31, 2^32)
+    f.sh = s - 1;                                    // (n*M) >> (31+s) = umulhi(n,M) >> (s-1)
+    return f;
+}
+
+// Launch geometry of a lattice of extents `dims` (the real lattice, or one parity of it with dims[0] = Lx/2) tiled
+// by tb.  z chunk of the CTA rasterisation: the largest divisor of the z tile count whose t-reuse distance
+// Lx*Ly*(zc*BZ)*BT sites * ~600 B (spinor in/out, gauge, halos) stays within the L2 budget.
+static inline wd::Geom make_geom_lattice(const int dims[4], int bc_t, const int tb[4], int zchunk_user, double l2_budget_mb)
+{
+    wd::Geom g;
+    long vol = 1;
+    for (int d = 0; d < 4; ++d) {
+        g.L[d] = dims[d];
+        g.nt[d] = (dims[d] + tb[d] - 1) / tb[d];
+        vol *= dims[d];
+    }
+    g.V = (int)vol;
+    g.bc_t = bc_t;
+    g.eo = 0;
+    g.par = 0;
+    const double layer = 600.0 * dims[0] * dims[1] * tb[3];   // bytes per z layer of one t-tile row
+    const double budget = l2_budget_mb * 1.0e6;
+    int zc = 1;
+    if (zchunk_user > 0) {
+        zc = (zchunk_user + tb[2] - 1) / tb[2];
+        if (zc > g.nt[2]) zc = g.nt[2];
+    } else {
+        for (int d = 1; d <= g.nt[2]; ++d)
+            if (g.nt[2] % d == 0 && layer * d * tb[2] <= budget) zc = d;
+    }
+    g.zc = zc;
+    g.ntiles = g.nt[0] * g.nt[1] * g.nt[2] * g.nt[3];
+    g.pf = 0;   // set per launch (needs the grid size)
+    g.d_chunk = make_fastdiv((unsigned)(g.nt[0] * g.nt[1] * g.zc * g.nt[3]));
+    g.d_nt0 = make_fastdiv((unsigned)g.nt[0]);
+    g.d_nt1 = make_fastdiv((unsigned)g.nt[1]);
+    g.d_zc = make_fastdiv((unsigned)g.zc);
+    const int zlast = g.nt[2] % g.zc ? g.nt[2] % g.zc : g.zc;
+    g.d_zlast = make_fastdiv((unsigned)zlast);
+    return g;
+}
+static inline wd::Geom make_geom_dims(const wd_ctx *c, const int tb[4], int zchunk_user)
+{
+    return make_geom_lattice(c->dims, c->bc_t, tb, zchunk_user, c->l2_budget_mb);
+}
+static inline wd::Geom make_geom(const wd_ctx *c, int tile) { return make_geom_dims(c, wd::kTiles[tile].b, c->zchunk_user); }
+
+static inline long tile_blocks_dims(const int dims[4], int tile)
+{
+    long n = 1;
+    for (int d = 0; d < 4; ++d) n *= (dims[d] + wd::kTiles[tile].b[d] - 1) / wd::kTiles[tile].b[d];
+    return n;
+}
+static inline long tile_blocks(const wd_ctx *c, int tile) { return tile_blocks_dims(c->dims, tile); }
+static inline int tile_threads(int tile)
+{
+    return wd::kTiles[tile].b[0] * wd::kTiles[tile].b[1] * wd::kTiles[tile].b[2] * wd::kTiles[tile].b[3];
+}
+static inline bool tile_ok(const wd_ctx *c, int tile)
+{
+    if (tile < 0 || tile >= WD_NUM_TILES) return false;
+    if (c->precision == 64 && !wd::kTiles[tile].f64) return false;
+    return true;
+}
+// Automatic choice: the first row of the table (rows are in order of measured preference) among those compiled
+// for this precision that waste the fewest threads on tiles overhanging the lattice `dims`.
+static inline int auto_tile_dims(const wd_ctx *c, const int dims[4])
+{
+    int best = -1;
+    double best_waste = 1e300, vol = 1.0;
+    for (int d = 0; d < 4; ++d) vol *= dims[d];
+    for (int t = 0; t < WD_NUM_TILES; ++t) {
+        if (!tile_ok(c, t)) continue;
+        const double waste = (double)tile_blocks_dims(dims, t) * tile_threads(t) / vol;
+        if (waste < best_waste - 1e-12) { best_waste = waste; best = t; }
+    }
+    return best;
+}
+static inline int auto_tile(const wd_ctx *c) { return auto_tile_dims(c, c->dims); }

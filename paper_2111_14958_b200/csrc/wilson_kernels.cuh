@@ -41,6 +41,9 @@ struct Geom {
     int zc;      // z tiles per chunk of the CTA rasterisation (see tile_of_block)
     int ntiles;  // nt[0]*nt[1]*nt[2]*nt[3]
     int pf;      // L2 prefetch distance in tiles (0 = off; needs Lx % 16 == 0 so that a 16-site run is one block)
+    int eo;      // 1: the lattice of this launch is ONE PARITY of the real lattice (even-odd preconditioning, SURVEY.md
+                 //    8(f3)): L[0] = Lx/2, site (xh,y,z,t) stands for x = 2 xh + ((y+z+t+par) & 1); 0: plain lattice
+    int par;     // eo = 1: parity (x+y+z+t) & 1 of the sites this launch WRITES; its neighbours have parity 1 - par
     FastDiv d_chunk, d_nt0, d_nt1, d_zc, d_zlast;   // per_chunk, nt[0], nt[1], zc, size of the last z chunk
 };
 
@@ -441,6 +444,15 @@ __device__ __forceinline__ void load_spinor_sel(const svec *in, int s, real v[24
     if (RO) load_spinor(in, s, v);
     else load_spinor_rw(in, s, v);
 }
+template <bool RO, typename svec, typename real>
+__device__ __forceinline__ void load_centre(const svec *cen, int s, real c[24])
+{
+    if (cen) load_spinor_sel<RO>(cen, s, c);
+    else {
+#pragma unroll
+        for (int i = 0; i < 24; ++i) c[i] = 0;
+    }
+}
 // RECON = 18: all nine complex entries are stored; 12: rows 0, 1 stored, row 2 rebuilt.  With RECON = 12 the rebuild
 // happens at load time, i.e. inside the software pipeline one hop ahead of its use.
 template <int MU, bool RO, int RECON, typename real, typename svec, typename gvec>
@@ -471,6 +483,13 @@ __device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, i
     Hops h;
     h.f[0] = s + (x == L0 - 1 ? 1 - L0 : 1);
     h.b[0] = s + (x == 0 ? L0 - 1 : -1);
+    if (g.eo) {
+        // checkerboard: the +-x neighbours live in the other parity's field; a site with odd real x (rp = 1) has its
+        // +x neighbour in the NEXT pair and its -x neighbour in its own pair, a site with even x the other way round
+        const int rp = (y + z + t + g.par) & 1;
+        if (rp) h.b[0] = s;
+        else h.f[0] = s;
+    }
     h.f[1] = s + (y == L1 - 1 ? (1 - L1) * s1 : s1);
     h.b[1] = s + (y == 0 ? (L1 - 1) * s1 : -s1);
     h.f[2] = s + (z == L2 - 1 ? (1 - L2) * s2 : s2);
@@ -486,10 +505,14 @@ __device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, i
 // hop k+1 are issued before hop k is computed, so every thread keeps one hop (168 B fp32) in flight while
 // it computes (memory-level parallelism without more threads).
 // LOADR: also fetch r(s) into rv together with the centre spinor (MODE_RUPD), so that it too overlaps the last hop.
+// U: links of the sites being written (forward hops); UB: links of the neighbours' field (backward hops; == U on a
+// plain lattice, the other parity's links with even-odd); cen: the field of the diagonal term (== in on a plain
+// lattice; nullptr = no diagonal term, c = 0).
 template <int DAG, int PIPE, bool LOADR, bool RO, typename real, typename svec, typename gvec, int RECON = 18, int NT = 0>
-__device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const svec *in,
-                                            const svec *r, int x, int y, int z, int t, int s, real acc[24],
-                                            real c[24], real rv[24], void *smem = nullptr, int next_s = -1)
+__device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const gvec *__restrict__ UB,
+                                            const svec *in, const svec *cen, const svec *r, int x, int y, int z, int t,
+                                            int s, real acc[24], real c[24], real rv[24], void *smem = nullptr,
+                                            int next_s = -1)
 {
     constexpr int SF = DAG ? +1 : -1;
     const Hops n = neighbours(g, x, y, z, t, s);
@@ -502,40 +525,40 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
     if (PIPE == 0) {
         real v[24], u[18];
         hop_load<0, RO, RECON, real>(U, in, s, n.f[0], v, u);       hop_compute<0, SF, false, real>(v, u, one, acc);
-        hop_load<0, RO, RECON, real>(U, in, n.b[0], n.b[0], v, u);  hop_compute<0, -SF, true, real>(v, u, one, acc);
+        hop_load<0, RO, RECON, real>(UB, in, n.b[0], n.b[0], v, u);  hop_compute<0, -SF, true, real>(v, u, one, acc);
         hop_load<1, RO, RECON, real>(U, in, s, n.f[1], v, u);       hop_compute<1, SF, false, real>(v, u, one, acc);
-        hop_load<1, RO, RECON, real>(U, in, n.b[1], n.b[1], v, u);  hop_compute<1, -SF, true, real>(v, u, one, acc);
+        hop_load<1, RO, RECON, real>(UB, in, n.b[1], n.b[1], v, u);  hop_compute<1, -SF, true, real>(v, u, one, acc);
         hop_load<2, RO, RECON, real>(U, in, s, n.f[2], v, u);       hop_compute<2, SF, false, real>(v, u, one, acc);
-        hop_load<2, RO, RECON, real>(U, in, n.b[2], n.b[2], v, u);  hop_compute<2, -SF, true, real>(v, u, one, acc);
+        hop_load<2, RO, RECON, real>(UB, in, n.b[2], n.b[2], v, u);  hop_compute<2, -SF, true, real>(v, u, one, acc);
         hop_load<3, RO, RECON, real>(U, in, s, n.f[3], v, u);       hop_compute<3, SF, false, real>(v, u, sgf, acc);
-        hop_load<3, RO, RECON, real>(U, in, n.b[3], n.b[3], v, u);  hop_compute<3, -SF, true, real>(v, u, sgb, acc);
-        load_spinor_sel<RO>(in, s, c);
+        hop_load<3, RO, RECON, real>(UB, in, n.b[3], n.b[3], v, u);  hop_compute<3, -SF, true, real>(v, u, sgb, acc);
+        load_centre<RO>(cen, s, c);
         if (LOADR) load_spinor_rw(r, s, rv);
     } else if (PIPE == 1) {
         real va[24], ua[18], vb[24], ub[18];
         hop_load<0, RO, RECON, real>(U, in, s, n.f[0], va, ua);
-        hop_load<0, RO, RECON, real>(U, in, n.b[0], n.b[0], vb, ub);  hop_compute<0, SF, false, real>(va, ua, one, acc);
+        hop_load<0, RO, RECON, real>(UB, in, n.b[0], n.b[0], vb, ub);  hop_compute<0, SF, false, real>(va, ua, one, acc);
         hop_load<1, RO, RECON, real>(U, in, s, n.f[1], va, ua);       hop_compute<0, -SF, true, real>(vb, ub, one, acc);
-        hop_load<1, RO, RECON, real>(U, in, n.b[1], n.b[1], vb, ub);  hop_compute<1, SF, false, real>(va, ua, one, acc);
+        hop_load<1, RO, RECON, real>(UB, in, n.b[1], n.b[1], vb, ub);  hop_compute<1, SF, false, real>(va, ua, one, acc);
         hop_load<2, RO, RECON, real>(U, in, s, n.f[2], va, ua);       hop_compute<1, -SF, true, real>(vb, ub, one, acc);
-        hop_load<2, RO, RECON, real>(U, in, n.b[2], n.b[2], vb, ub);  hop_compute<2, SF, false, real>(va, ua, one, acc);
+        hop_load<2, RO, RECON, real>(UB, in, n.b[2], n.b[2], vb, ub);  hop_compute<2, SF, false, real>(va, ua, one, acc);
         hop_load<3, RO, RECON, real>(U, in, s, n.f[3], va, ua);       hop_compute<2, -SF, true, real>(vb, ub, one, acc);
-        hop_load<3, RO, RECON, real>(U, in, n.b[3], n.b[3], vb, ub);  hop_compute<3, SF, false, real>(va, ua, sgf, acc);
-        load_spinor_sel<RO>(in, s, c);
+        hop_load<3, RO, RECON, real>(UB, in, n.b[3], n.b[3], vb, ub);  hop_compute<3, SF, false, real>(va, ua, sgf, acc);
+        load_centre<RO>(cen, s, c);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
         if (LOADR) load_spinor_rw(r, s, rv);   // after the last hop: an earlier fetch costs registers (spills at 128)
     } else if (PIPE == 2) {
         // three register buffers: two hops (336 B fp32 per thread) in flight while a third is computed
         real va[24], ua[18], vb[24], ub[18], vc[24], uc[18];
         hop_load<0, RO, RECON, real>(U, in, s, n.f[0], va, ua);
-        hop_load<0, RO, RECON, real>(U, in, n.b[0], n.b[0], vb, ub);
+        hop_load<0, RO, RECON, real>(UB, in, n.b[0], n.b[0], vb, ub);
         hop_load<1, RO, RECON, real>(U, in, s, n.f[1], vc, uc);          hop_compute<0, SF, false, real>(va, ua, one, acc);
-        hop_load<1, RO, RECON, real>(U, in, n.b[1], n.b[1], va, ua);     hop_compute<0, -SF, true, real>(vb, ub, one, acc);
+        hop_load<1, RO, RECON, real>(UB, in, n.b[1], n.b[1], va, ua);     hop_compute<0, -SF, true, real>(vb, ub, one, acc);
         hop_load<2, RO, RECON, real>(U, in, s, n.f[2], vb, ub);          hop_compute<1, SF, false, real>(vc, uc, one, acc);
-        hop_load<2, RO, RECON, real>(U, in, n.b[2], n.b[2], vc, uc);     hop_compute<1, -SF, true, real>(va, ua, one, acc);
+        hop_load<2, RO, RECON, real>(UB, in, n.b[2], n.b[2], vc, uc);     hop_compute<1, -SF, true, real>(va, ua, one, acc);
         hop_load<3, RO, RECON, real>(U, in, s, n.f[3], va, ua);          hop_compute<2, SF, false, real>(vb, ub, one, acc);
-        hop_load<3, RO, RECON, real>(U, in, n.b[3], n.b[3], vb, ub);     hop_compute<2, -SF, true, real>(vc, uc, one, acc);
-        load_spinor_sel<RO>(in, s, c);
+        hop_load<3, RO, RECON, real>(UB, in, n.b[3], n.b[3], vb, ub);     hop_compute<2, -SF, true, real>(vc, uc, one, acc);
+        load_centre<RO>(cen, s, c);
         if (LOADR) load_spinor_rw(r, s, rv);
         hop_compute<3, SF, false, real>(va, ua, sgf, acc);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
@@ -551,14 +574,14 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
         load_link_sm<1, NT>(U, smem, tid, us);               hop_compute<1, SF, false, real>(vb, us, one, acc);
         load_spinor_sel<RO>(in, n.f[3], vb);
         load_link_sm<2, NT>(U, smem, tid, us);               hop_compute<2, SF, false, real>(va, us, one, acc);
-        hop_load<0, RO, RECON, real>(U, in, n.b[0], n.b[0], va, ua);
+        hop_load<0, RO, RECON, real>(UB, in, n.b[0], n.b[0], va, ua);
         load_link_sm<3, NT>(U, smem, tid, us);               hop_compute<3, SF, false, real>(vb, us, sgf, acc);
         // the slots are free: stage the forward links of this thread's site of the next tile
         if (next_s >= 0) stage_links<NT>(U, next_s, smem, tid);
-        hop_load<1, RO, RECON, real>(U, in, n.b[1], n.b[1], vb, ub);  hop_compute<0, -SF, true, real>(va, ua, one, acc);
-        hop_load<2, RO, RECON, real>(U, in, n.b[2], n.b[2], va, ua);  hop_compute<1, -SF, true, real>(vb, ub, one, acc);
-        hop_load<3, RO, RECON, real>(U, in, n.b[3], n.b[3], vb, ub);  hop_compute<2, -SF, true, real>(va, ua, one, acc);
-        load_spinor_sel<RO>(in, s, c);
+        hop_load<1, RO, RECON, real>(UB, in, n.b[1], n.b[1], vb, ub);  hop_compute<0, -SF, true, real>(va, ua, one, acc);
+        hop_load<2, RO, RECON, real>(UB, in, n.b[2], n.b[2], va, ua);  hop_compute<1, -SF, true, real>(vb, ub, one, acc);
+        hop_load<3, RO, RECON, real>(UB, in, n.b[3], n.b[3], vb, ub);  hop_compute<2, -SF, true, real>(va, ua, one, acc);
+        load_centre<RO>(cen, s, c);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
         if (LOADR) load_spinor_rw(r, s, rv);
     }
@@ -729,7 +752,8 @@ enum { MODE_PLAIN = 0, MODE_QQ = 1, MODE_RUPD = 2, MODE_RV = 3, MODE_TS = 4 };
 template <typename real, int DAG, int MODE, int BX, int BY, int BZ, int BT, int MINB, int PIPE, int RECON = 18>
 __global__ void __launch_bounds__(BX *BY *BZ *BT, MINB)
 dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
-              const typename Field<real>::svec *__restrict__ in, typename Field<real>::svec *out, real kappa,
+              const typename Field<real>::gvec *__restrict__ UB, const typename Field<real>::svec *__restrict__ in,
+              const typename Field<real>::svec *__restrict__ cen, typename Field<real>::svec *out, real kappa,
               typename Field<real>::svec *r, CgScalars *sc, double *partials, unsigned int *counter,
               double *hist, int it)
 {
@@ -738,6 +762,8 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     constexpr int NT = BX * BY * BZ * BT;
     if (MODE != MODE_PLAIN) {
         if (it >= sc->k_stop) return;  // uniform over the grid: over-launched iterations are no-ops
+    } else if (sc) {
+        if (it >= sc->k_stop) return;  // a plain pass inside a solver loop (even-odd: the inner hop of Mhat)
     }
     const int tid = threadIdx.x;
     const int lx = tid % BX, ly = (tid / BX) % BY, lz = (tid / (BX * BY)) % BZ, lt = tid / (BX * BY * BZ);
@@ -787,7 +813,7 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24], rv[24];
         hopping_sum<DAG, PIPE, MODE == MODE_RUPD || MODE == MODE_RV, true, real, svec, gvec, RECON, NT>(
-            g, U, in, r, x, y, z, t, s, acc, c, rv, wd_dyn_smem, next_s);
+            g, U, UB, in, cen, r, x, y, z, t, s, acc, c, rv, wd_dyn_smem, next_s);
         if constexpr (MODE == MODE_TS) {
             // c holds s(x); t(x) = s(x) - kappa * hops replaces it component by component
             real tsr = 0, tsi = 0, tt = 0;
@@ -928,7 +954,7 @@ cg_onelaunch_kernel(const Geom g, const typename Field<real>::gvec *__restrict__
         local = 0.0;
         WD_FOR_EACH_SITE({
             real acc[24], c[24], dummy[24];
-            hopping_sum<1, PIPE, false, false, real, svec, gvec>(g, U, p, nullptr, x, y_, z, t, s, acc, c, dummy);
+            hopping_sum<1, PIPE, false, false, real, svec, gvec>(g, U, U, p, p, nullptr, x, y_, z, t, s, acc, c, dummy);
             real n2 = 0;
 #pragma unroll
             for (int i = 0; i < 24; ++i) { c[i] = fma(-kappa, acc[i], c[i]); n2 = fma(c[i], c[i], n2); }
@@ -947,7 +973,7 @@ cg_onelaunch_kernel(const Geom g, const typename Field<real>::gvec *__restrict__
         local = 0.0;
         WD_FOR_EACH_SITE({
             real acc[24], c[24], rv[24];
-            hopping_sum<0, PIPE, true, false, real, svec, gvec>(g, U, q, r, x, y_, z, t, s, acc, c, rv);
+            hopping_sum<0, PIPE, true, false, real, svec, gvec>(g, U, U, q, q, r, x, y_, z, t, s, acc, c, rv);
             real n2 = 0;
 #pragma unroll
             for (int i = 0; i < 24; ++i) {
@@ -983,7 +1009,7 @@ cg_onelaunch_kernel(const Geom g, const typename Field<real>::gvec *__restrict__
     // a6: psi = D-dagger y
     WD_FOR_EACH_SITE({
         real acc[24], c[24], dummy[24];
-        hopping_sum<1, PIPE, false, false, real, svec, gvec>(g, U, y, nullptr, x, y_, z, t, s, acc, c, dummy);
+        hopping_sum<1, PIPE, false, false, real, svec, gvec>(g, U, U, y, y, nullptr, x, y_, z, t, s, acc, c, dummy);
 #pragma unroll
         for (int i = 0; i < 24; ++i) c[i] = fma(-kappa, acc[i], c[i]);
         store_spinor(psi, s, c);

@@ -86,9 +86,11 @@ struct DslashArgs {
     int prefetch;   // L2 prefetch distance in tiles: -1 = one grid ahead, 0 = off
     cudaStream_t stream;
     const void *U;
+    const void *Ub;   // links read by the backward hops: U itself on a plain lattice, the other parity's with even-odd
     const void *in;
+    const void *cen;  // field of the diagonal term: `in` on a plain lattice; nullptr = none
     void *out;
-    double kappa;
+    double kappa;     // out = cen - kappa * (hopping sum)
     void *r;
     CgScalars *sc;
     double *partials;
@@ -133,7 +135,7 @@ static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
             Geom g = a.g;                                                                                      \
             g.pf = a.prefetch < 0 ? (int)grid : a.prefetch;                                                    \
             dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON><<<(unsigned)grid, bx * by * bz * bt, dyn, a.stream>>>(  \
-                g, (const gvec *)a.U, (const svec *)a.in, (svec *)a.out, (real)a.kappa, (svec *)a.r, a.sc,   \
+                g, (const gvec *)a.U, (const gvec *)a.Ub, (const svec *)a.in, (const svec *)a.cen, (svec *)a.out, (real)a.kappa, (svec *)a.r, a.sc,   \
                 a.partials, a.counter, a.hist, a.it);                                                          \
             return cudaGetLastError();                                                                         \
         }                                                                                                      \

@@ -80,6 +80,15 @@ def load_library(path: str = LIB_PATH):
     lib.cg_solve.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
     lib.bicgstab_solve.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
     lib.wd_get_profile_bicgstab.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_long)]
+    lib.wd_eo_spinor_bytes.argtypes = [vp]
+    lib.wd_eo_spinor_bytes.restype = ctypes.c_size_t
+    lib.wd_eo_gauge_bytes.argtypes = [vp]
+    lib.wd_eo_gauge_bytes.restype = ctypes.c_size_t
+    lib.wd_eo_pack_spinor.argtypes = [vp, vp, vp]
+    lib.wd_eo_unpack_spinor.argtypes = [vp, vp, vp]
+    lib.wd_eo_pack_gauge.argtypes = [vp, vp, vp]
+    lib.wd_eo_hop.argtypes = [vp, vp, vp, vp, ci, ci]
+    lib.cg_solve_eo.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
     lib.wd_coo_nnz.argtypes = [vp]
     lib.wd_coo_nnz.restype = ctypes.c_size_t
     lib.wd_coo_assemble.argtypes = [vp, vp, cd, ci, vp, vp, vp]
@@ -259,6 +268,51 @@ class WilsonContext:
         n = ctypes.c_long()
         self._check(self.lib.wd_get_profile_bicgstab(self._ctx, ms, ctypes.byref(n)))
         return {"ms": list(ms), "iterations": n.value}
+
+    # -- f3: even-odd preconditioned CG
+    def empty_eo_spinor(self):
+        torch = _torch()
+        n = self.lib.wd_eo_spinor_bytes(self._ctx) // (4 if self.precision == 32 else 8)
+        return torch.empty(n, dtype=self.real_dtype, device="cuda")
+
+    def empty_eo_gauge(self):
+        torch = _torch()
+        n = self.lib.wd_eo_gauge_bytes(self._ctx) // (4 if self.precision == 32 else 8)
+        return torch.empty(n, dtype=self.real_dtype, device="cuda")
+
+    def wd_eo_pack_spinor(self, psi_canonical, out=None):
+        psi_canonical = self._canon(psi_canonical, (self.volume, 4, 3))
+        out = self.empty_eo_spinor() if out is None else out
+        self._check(self.lib.wd_eo_pack_spinor(self._ctx, self._p(psi_canonical), self._p(out)))
+        return out
+
+    def wd_eo_unpack_spinor(self, psi_eo, out=None):
+        torch = _torch()
+        if out is None:
+            out = torch.empty((self.volume, 4, 3), dtype=self.complex_dtype, device="cuda")
+        self._check(self.lib.wd_eo_unpack_spinor(self._ctx, self._p(psi_eo), self._p(out)))
+        return out
+
+    def wd_eo_pack_gauge(self, U_canonical, out=None):
+        U_canonical = self._canon(U_canonical, (self.volume, 4, 3, 3))
+        out = self.empty_eo_gauge() if out is None else out
+        self._check(self.lib.wd_eo_pack_gauge(self._ctx, self._p(U_canonical), self._p(out)))
+        return out
+
+    def wd_eo_hop(self, U_eo, in_eo, out_eo, out_parity, dagger=False):
+        self._check(self.lib.wd_eo_hop(self._ctx, self._p(U_eo), self._p(in_eo), self._p(out_eo), int(out_parity),
+                                       int(bool(dagger))))
+        return out_eo
+
+    def cg_solve_eo(self, U_eo, eta_eo, kappa, r_min, max_iter, out=None):
+        out = self.empty_eo_spinor() if out is None else out
+        info = WdCgInfo()
+        rc = self.lib.cg_solve_eo(self._ctx, self._p(U_eo), self._p(eta_eo), self._p(out), float(kappa),
+                                  float(r_min), int(max_iter), ctypes.byref(info))
+        self._check(rc, allow_not_converged=True)
+        d = info.as_dict()
+        d["status"] = rc
+        return out, d
 
     # -- f2: the paper's coordinate-format route
     def wd_coo_nnz(self):

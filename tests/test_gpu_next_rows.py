@@ -274,3 +274,131 @@ def test_recon12_cg_solve(wilson, oracle, cfg_index, precision, r_min):
     res_gpu = oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
     res_orc = oracle.true_residual(cfg.dims, U64, eta64, psi_o, cfg.kappa, cfg.bc_t)
     assert res_gpu <= 2.0 * res_orc, (res_gpu, res_orc)
+
+
+# ---------------------------------------------------------------- f3: even-odd preconditioned CG
+def _parity(dims):
+    return lm.coords(dims).sum(axis=1) & 1
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (6, 4, 10, 8), (14, 14, 14, 14), (36, 4, 6, 4)])
+def test_eo_pack_unpack_roundtrip_and_layout(wilson, dims, precision):
+    """canonical -> checkerboard -> canonical is bit-exact, and the checkerboard buffer is [even half | odd half] with
+    site index lexicographic/2 inside a half (checked through wd_unpack of a half read as a plain half lattice)"""
+    cdt = gu.np_complex(precision)
+    psi = inputs.source_field(CFG_TEST + 30, dims, dtype=cdt, field=inputs.FIELD_AUX)
+    hd = (dims[0] // 2,) + tuple(dims[1:])
+    par = _parity(dims)
+    with wilson.WilsonContext(dims, precision) as ctx:
+        eo = ctx.wd_eo_pack_spinor(gu.to_device(psi))
+        assert gu.to_host(ctx.wd_eo_unpack_spinor(eo)).tobytes() == psi.tobytes()
+        n = eo.numel() // 2
+        if hd[0] < 4:      # a plain ctx needs extents >= 4
+            return
+        with wilson.WilsonContext(hd, precision) as half:
+            assert n == half.empty_spinor().numel()
+            for p in (0, 1):
+                got = gu.to_host(half.wd_unpack_spinor(eo[p * n:(p + 1) * n].contiguous()))
+                assert got.tobytes() == psi[par == p].tobytes()      # lexicographic order restricted to one parity
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("bc_t", [-1, 1])
+@pytest.mark.parametrize("dims,links", [((4, 4, 4, 4), "haar"), ((6, 4, 10, 8), "haar"), ((14, 14, 14, 14), "near_identity"),
+                                        ((36, 4, 6, 4), "haar")])
+def test_eo_hop_matches_oracle(wilson, oracle, dims, links, bc_t, precision):
+    """H_{p,1-p} on each parity == the oracle's hopping sum (psi - D psi)/kappa restricted to that parity"""
+    cdt = gu.np_complex(precision)
+    U = inputs.gauge_field(CFG_TEST + 31, dims, links, dtype=cdt)
+    psi = inputs.source_field(CFG_TEST + 31, dims, dtype=cdt, field=inputs.FIELD_AUX)
+    U64, p64 = U.astype(np.complex128), psi.astype(np.complex128)
+    par = _parity(dims)
+    with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+        Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
+        pe = ctx.wd_eo_pack_spinor(gu.to_device(psi))
+        for dagger in (False, True):
+            out = ctx.empty_eo_spinor().zero_()
+            ctx.wd_eo_hop(Ue, pe, out, 0, dagger)
+            ctx.wd_eo_hop(Ue, pe, out, 1, dagger)
+            got = gu.to_host(ctx.wd_eo_unpack_spinor(out))
+            want = p64 - oracle.wd_apply(dims, U64, p64, 1.0, dagger, bc_t)     # D = 1 - kappa H at kappa = 1
+            assert lm.per_site_rel_err(got, want)[0] <= (1e-5 if precision == 32 else 1e-12)
+            # one parity only: the other half of out is untouched
+            out.zero_()
+            ctx.wd_eo_hop(Ue, pe, out, 1, dagger)
+            assert not gu.to_host(ctx.wd_eo_unpack_spinor(out))[par == 0].any()
+
+
+@pytest.mark.parametrize("precision,r_min", [(32, 1e-6), (64, 1e-10)])
+@pytest.mark.parametrize("cfg_index", [0, 1, 2])
+def test_eo_cg_baseline_configs(wilson, oracle, cfg_index, precision, r_min):
+    cfg = inputs.CONFIGS[cfg_index]
+    U, eta = gu.config_fields(cfg.index, precision)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
+        ee = ctx.wd_eo_pack_spinor(gu.to_device(eta))
+        pe, info = ctx.cg_solve_eo(Ue, ee, cfg.kappa, r_min, cfg.max_iter)
+        psi = gu.to_host(ctx.wd_eo_unpack_spinor(pe))
+        hist = ctx.wd_cg_history()
+    psi_o, info_o = oracle.cg_solve_eo(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t, history=True)
+    assert info["status"] == 0 and info["cg_mode"] == 4 and info_o["converged"]
+    assert abs(info["iterations"] - info_o["iterations"]) <= math.floor(0.02 * info_o["iterations"] + 0.5)
+    assert abs(info["eta_norm2"] - info_o["eta_norm2"]) < (1e-6 if precision == 32 else 1e-13) * info_o["eta_norm2"]
+    res_gpu = oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
+    res_orc = oracle.true_residual(cfg.dims, U64, eta64, psi_o, cfg.kappa, cfg.bc_t)
+    assert res_gpu <= 2.0 * res_orc and res_gpu < 2.0 * r_min, (res_gpu, res_orc)
+    n = min(len(hist), len(info_o["rr_history"]))
+    assert len(hist) == info["iterations"] + 1
+    rel = np.abs(hist[:n] - info_o["rr_history"][:n]) / info_o["rr_history"][:n]
+    assert rel[0] < (1e-6 if precision == 32 else 1e-13) and np.max(rel[: max(2, n // 2)]) < (2e-2 if precision == 32 else 1e-6)
+    diff = np.linalg.norm(psi - psi_o) / np.linalg.norm(psi_o)
+    assert diff < 4.0 * r_min / (1.0 - 8.0 * cfg.kappa) * (1 + 8 * cfg.kappa)
+    # fewer iterations than the unpreconditioned recurrence on the same problem
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        _, plain = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, r_min, cfg.max_iter)
+    assert info["iterations"] < 0.7 * plain["iterations"]
+
+
+def test_eo_cg_edge_cases(wilson, oracle):
+    cfg = inputs.CONFIGS[0]
+    U, eta = gu.config_fields(0, 32)
+    par = _parity(cfg.dims)
+    with wilson.WilsonContext(cfg.dims, 32) as ctx:
+        Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
+        ee = ctx.wd_eo_pack_spinor(gu.to_device(eta))
+        pe, info = ctx.cg_solve_eo(Ue, ctx.wd_eo_pack_spinor(gu.to_device(np.zeros_like(eta))), cfg.kappa, 1e-6, 10)
+        assert info["status"] == 0 and info["iterations"] == 0 and not gu.to_host(ctx.wd_eo_unpack_spinor(pe)).any()
+        pe, info = ctx.cg_solve_eo(Ue, ee, cfg.kappa, 1e-6, 0)
+        z = gu.to_host(ctx.wd_eo_unpack_spinor(pe))
+        assert info["status"] == 1 and info["iterations"] == 0
+        assert not z[par == 0].any() and np.array_equal(z[par == 1], eta[par == 1])   # psi_o = eta_o for psi_e = 0
+        a, ia = ctx.cg_solve_eo(Ue, ee, cfg.kappa, 1e-6, 100)
+        ctx.wd_set_poll_interval(1)
+        b, ib = ctx.cg_solve_eo(Ue, ee, cfg.kappa, 1e-6, 100)
+        assert gu.to_host(a).tobytes() == gu.to_host(b).tobytes() and ia["iterations"] == ib["iterations"]
+    with wilson.WilsonContext((5, 4, 4, 6), 32) as ctx:
+        with pytest.raises(wilson.WilsonError) as ei:
+            ctx.empty_eo_spinor(); ctx.wd_eo_pack_spinor(gu.to_device(np.zeros((480, 4, 3), np.complex64)))
+        assert ei.value.code == -2
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_eo_cg_32_4_closed_form(wilson, precision):
+    """BASELINE volume 32^4, exact solution known: pure-gauge links, Gaussian source (pin P8 through free_solve)"""
+    dims, kappa = (32, 32, 32, 32), 0.12
+    g = inputs.gauge_transform_field(CFG_TEST + 3, dims)
+    U = lm.pure_gauge_links(dims, g)
+    eta = inputs.source_field(CFG_TEST + 3, dims)
+    want = np.einsum("xab,xib->xia", g, lm.free_solve(dims, kappa, np.einsum("xba,xib->xia", np.conj(g), eta), -1))
+    cdt = gu.np_complex(precision)
+    tol = 1e-6 if precision == 32 else 1e-11
+    with wilson.WilsonContext(dims, precision) as ctx:
+        Ue = ctx.wd_eo_pack_gauge(gu.to_device(U.astype(cdt)))
+        ee = ctx.wd_eo_pack_spinor(gu.to_device(eta.astype(cdt)))
+        pe, info = ctx.cg_solve_eo(Ue, ee, kappa, tol, 2000)
+        psi = gu.to_host(ctx.wd_eo_unpack_spinor(pe))
+    assert info["status"] == 0
+    err = np.linalg.norm(psi - want) / np.linalg.norm(want)
+    assert err < (2e-5 if precision == 32 else 1e-9), err
