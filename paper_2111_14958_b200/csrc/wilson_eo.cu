@@ -130,7 +130,7 @@ cudaError_t eo_launch(wd_ctx *c, const void *U_eo, const EoPass &p)
     a.sc = (p.mode != MODE_PLAIN || p.in_loop) ? c->sc : nullptr;
     a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = p.it;
     c->launches++;
-    return c->precision == 32 ? launch_dslash_f32(tile, p.dagger, p.mode, a) : launch_dslash_f64(tile, p.dagger, p.mode, a);
+    return c->precision == 32 ? launch_dslash_eo_f32(tile, p.dagger, p.mode, a) : launch_dslash_eo_f64(tile, p.dagger, p.mode, a);
 }
 
 }  // namespace

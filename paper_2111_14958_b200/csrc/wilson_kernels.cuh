@@ -476,6 +476,7 @@ __device__ __forceinline__ void hop_compute(const real v[24], const real u[18], 
 struct Hops {
     int f[4], b[4];
 };
+template <int EO = 0>
 __device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, int t, int s)
 {
     const int L0 = g.L[0], L1 = g.L[1], L2 = g.L[2], L3 = g.L[3];
@@ -483,7 +484,7 @@ __device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, i
     Hops h;
     h.f[0] = s + (x == L0 - 1 ? 1 - L0 : 1);
     h.b[0] = s + (x == 0 ? L0 - 1 : -1);
-    if (g.eo) {
+    if (EO) {
         // checkerboard: the +-x neighbours live in the other parity's field; a site with odd real x (rp = 1) has its
         // +x neighbour in the NEXT pair and its -x neighbour in its own pair, a site with even x the other way round
         const int rp = (y + z + t + g.par) & 1;
@@ -508,14 +509,15 @@ __device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, i
 // U: links of the sites being written (forward hops); UB: links of the neighbours' field (backward hops; == U on a
 // plain lattice, the other parity's links with even-odd); cen: the field of the diagonal term (== in on a plain
 // lattice; nullptr = no diagonal term, c = 0).
-template <int DAG, int PIPE, bool LOADR, bool RO, typename real, typename svec, typename gvec, int RECON = 18, int NT = 0>
+template <int DAG, int PIPE, bool LOADR, bool RO, typename real, typename svec, typename gvec, int RECON = 18, int NT = 0,
+          int EO = 0>
 __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const gvec *__restrict__ UB,
                                             const svec *in, const svec *cen, const svec *r, int x, int y, int z, int t,
                                             int s, real acc[24], real c[24], real rv[24], void *smem = nullptr,
                                             int next_s = -1)
 {
     constexpr int SF = DAG ? +1 : -1;
-    const Hops n = neighbours(g, x, y, z, t, s);
+    const Hops n = neighbours<EO>(g, x, y, z, t, s);
     // boundary sign sigma+- of reading C-1: only the hop that wraps the t boundary carries bc_t
     const real sgf = (t == g.L[3] - 1) ? (real)g.bc_t : (real)1;
     const real sgb = (t == 0) ? (real)g.bc_t : (real)1;
@@ -749,7 +751,9 @@ enum { MODE_PLAIN = 0, MODE_QQ = 1, MODE_RUPD = 2, MODE_RV = 3, MODE_TS = 4 };
 // MODE_RUPD  : s = D q (not stored), r <- r - alpha s, rr' = |r|^2, beta, loop condition   (a3)
 // MODE_RV    : out = v = D p, <rhat, v> (rhat passed as `r`, read only), alpha = rho/<rhat,v>   (BiCGSTAB)
 // MODE_TS    : out = t = D s, <t,s> and <t,t>, omega = <t,s>/<t,t>                              (BiCGSTAB)
-template <typename real, int DAG, int MODE, int BX, int BY, int BZ, int BT, int MINB, int PIPE, int RECON = 18>
+// EO = 0: plain lattice (UB and cen are ignored: the backward links come from U, the diagonal term from `in`);
+// EO = 1: the launch covers one parity of the lattice (even-odd preconditioning, Geom.eo / Geom.par).
+template <typename real, int DAG, int MODE, int BX, int BY, int BZ, int BT, int MINB, int PIPE, int RECON = 18, int EO = 0>
 __global__ void __launch_bounds__(BX *BY *BZ *BT, MINB)
 dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
               const typename Field<real>::gvec *__restrict__ UB, const typename Field<real>::svec *__restrict__ in,
@@ -812,8 +816,8 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
         if (!active) continue;
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24], rv[24];
-        hopping_sum<DAG, PIPE, MODE == MODE_RUPD || MODE == MODE_RV, true, real, svec, gvec, RECON, NT>(
-            g, U, UB, in, cen, r, x, y, z, t, s, acc, c, rv, wd_dyn_smem, next_s);
+        hopping_sum<DAG, PIPE, MODE == MODE_RUPD || MODE == MODE_RV, true, real, svec, gvec, RECON, NT, EO>(
+            g, U, EO ? UB : U, in, EO ? cen : in, r, x, y, z, t, s, acc, c, rv, wd_dyn_smem, next_s);
         if constexpr (MODE == MODE_TS) {
             // c holds s(x); t(x) = s(x) - kappa * hops replaces it component by component
             real tsr = 0, tsi = 0, tt = 0;

@@ -105,11 +105,14 @@ cudaError_t launch_dslash_f64(int tile, int dagger, int mode, const DslashArgs &
 // the same with 12-real link storage (wd_set_gauge_recon(ctx, 12))
 cudaError_t launch_dslash12_f32(int tile, int dagger, int mode, const DslashArgs &a);
 cudaError_t launch_dslash12_f64(int tile, int dagger, int mode, const DslashArgs &a);
+// one parity of the lattice (even-odd preconditioning; a.g.eo = 1)
+cudaError_t launch_dslash_eo_f32(int tile, int dagger, int mode, const DslashArgs &a);
+cudaError_t launch_dslash_eo_f64(int tile, int dagger, int mode, const DslashArgs &a);
 // BiCGSTAB passes (D only): mode in {MODE_RV, MODE_TS}
 cudaError_t launch_dslash_bi_f32(int tile, int mode, const DslashArgs &a);
 cudaError_t launch_dslash_bi_f64(int tile, int mode, const DslashArgs &a);
 
-template <typename real, int DAG, int MODE, int RECON = 18>
+template <typename real, int DAG, int MODE, int RECON = 18, int EO = 0>
 static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
 {
     using svec = typename Field<real>::svec;
@@ -121,7 +124,7 @@ static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
             static int occ = 0;                                                                                \
             const size_t dyn = (p == 3) ? (size_t)(bx * by * bz * bt) * staged_link_bytes<real>() : 0;         \
             if (!occ) {                                                                                        \
-                auto kern = dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON>;                       \
+                auto kern = dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON, EO>;                       \
                 if (dyn > 48 * 1024) {                                                                         \
                     cudaError_t e2 = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); \
                     if (e2 != cudaSuccess) return e2;                                                          \
@@ -134,7 +137,7 @@ static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
             if (grid > a.g.ntiles) grid = a.g.ntiles;                                                          \
             Geom g = a.g;                                                                                      \
             g.pf = a.prefetch < 0 ? (int)grid : a.prefetch;                                                    \
-            dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON><<<(unsigned)grid, bx * by * bz * bt, dyn, a.stream>>>(  \
+            dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON, EO><<<(unsigned)grid, bx * by * bz * bt, dyn, a.stream>>>(  \
                 g, (const gvec *)a.U, (const gvec *)a.Ub, (const svec *)a.in, (const svec *)a.cen, (svec *)a.out, (real)a.kappa, (svec *)a.r, a.sc,   \
                 a.partials, a.counter, a.hist, a.it);                                                          \
             return cudaGetLastError();                                                                         \
@@ -183,14 +186,14 @@ static cudaError_t launch_cg_onelaunch_any(int small_tile, const CgOneLaunchArgs
     }
 }
 
-template <typename real, int RECON = 18>
+template <typename real, int RECON = 18, int EO = 0>
 static cudaError_t launch_dslash_any(int tile, int dagger, int mode, const DslashArgs &a)
 {
     if (mode == MODE_PLAIN)
-        return dagger ? launch_dslash_tile<real, 1, MODE_PLAIN, RECON>(tile, a)
-                      : launch_dslash_tile<real, 0, MODE_PLAIN, RECON>(tile, a);
-    if (mode == MODE_QQ && dagger) return launch_dslash_tile<real, 1, MODE_QQ, RECON>(tile, a);
-    if (mode == MODE_RUPD && !dagger) return launch_dslash_tile<real, 0, MODE_RUPD, RECON>(tile, a);
+        return dagger ? launch_dslash_tile<real, 1, MODE_PLAIN, RECON, EO>(tile, a)
+                      : launch_dslash_tile<real, 0, MODE_PLAIN, RECON, EO>(tile, a);
+    if (mode == MODE_QQ && dagger) return launch_dslash_tile<real, 1, MODE_QQ, RECON, EO>(tile, a);
+    if (mode == MODE_RUPD && !dagger) return launch_dslash_tile<real, 0, MODE_RUPD, RECON, EO>(tile, a);
     return cudaErrorInvalidValue;
 }
 
