@@ -444,10 +444,12 @@ __device__ __forceinline__ void load_spinor_sel(const svec *in, int s, real v[24
     if (RO) load_spinor(in, s, v);
     else load_spinor_rw(in, s, v);
 }
-template <bool RO, typename svec, typename real>
+// MAYBE_NULL = false (plain lattice): cen is the input field itself, no test (a run-time test here costs the plain
+// kernels a spill and ~4 % because the centre loads can no longer be scheduled freely around the last hop)
+template <bool RO, bool MAYBE_NULL, typename svec, typename real>
 __device__ __forceinline__ void load_centre(const svec *cen, int s, real c[24])
 {
-    if (cen) load_spinor_sel<RO>(cen, s, c);
+    if (!MAYBE_NULL || cen) load_spinor_sel<RO>(cen, s, c);
     else {
 #pragma unroll
         for (int i = 0; i < 24; ++i) c[i] = 0;
@@ -534,7 +536,7 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
         hop_load<2, RO, RECON, real>(UB, in, n.b[2], n.b[2], v, u);  hop_compute<2, -SF, true, real>(v, u, one, acc);
         hop_load<3, RO, RECON, real>(U, in, s, n.f[3], v, u);       hop_compute<3, SF, false, real>(v, u, sgf, acc);
         hop_load<3, RO, RECON, real>(UB, in, n.b[3], n.b[3], v, u);  hop_compute<3, -SF, true, real>(v, u, sgb, acc);
-        load_centre<RO>(cen, s, c);
+        load_centre<RO, EO != 0>(cen, s, c);
         if (LOADR) load_spinor_rw(r, s, rv);
     } else if (PIPE == 1) {
         real va[24], ua[18], vb[24], ub[18];
@@ -546,7 +548,7 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
         hop_load<2, RO, RECON, real>(UB, in, n.b[2], n.b[2], vb, ub);  hop_compute<2, SF, false, real>(va, ua, one, acc);
         hop_load<3, RO, RECON, real>(U, in, s, n.f[3], va, ua);       hop_compute<2, -SF, true, real>(vb, ub, one, acc);
         hop_load<3, RO, RECON, real>(UB, in, n.b[3], n.b[3], vb, ub);  hop_compute<3, SF, false, real>(va, ua, sgf, acc);
-        load_centre<RO>(cen, s, c);
+        load_centre<RO, EO != 0>(cen, s, c);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
         if (LOADR) load_spinor_rw(r, s, rv);   // after the last hop: an earlier fetch costs registers (spills at 128)
     } else if (PIPE == 2) {
@@ -560,7 +562,7 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
         hop_load<2, RO, RECON, real>(UB, in, n.b[2], n.b[2], vc, uc);     hop_compute<1, -SF, true, real>(va, ua, one, acc);
         hop_load<3, RO, RECON, real>(U, in, s, n.f[3], va, ua);          hop_compute<2, SF, false, real>(vb, ub, one, acc);
         hop_load<3, RO, RECON, real>(UB, in, n.b[3], n.b[3], vb, ub);     hop_compute<2, -SF, true, real>(vc, uc, one, acc);
-        load_centre<RO>(cen, s, c);
+        load_centre<RO, EO != 0>(cen, s, c);
         if (LOADR) load_spinor_rw(r, s, rv);
         hop_compute<3, SF, false, real>(va, ua, sgf, acc);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
@@ -583,7 +585,7 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
         hop_load<1, RO, RECON, real>(UB, in, n.b[1], n.b[1], vb, ub);  hop_compute<0, -SF, true, real>(va, ua, one, acc);
         hop_load<2, RO, RECON, real>(UB, in, n.b[2], n.b[2], va, ua);  hop_compute<1, -SF, true, real>(vb, ub, one, acc);
         hop_load<3, RO, RECON, real>(UB, in, n.b[3], n.b[3], vb, ub);  hop_compute<2, -SF, true, real>(va, ua, one, acc);
-        load_centre<RO>(cen, s, c);
+        load_centre<RO, EO != 0>(cen, s, c);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
         if (LOADR) load_spinor_rw(r, s, rv);
     }

@@ -402,3 +402,35 @@ def test_eo_cg_32_4_closed_form(wilson, precision):
     assert info["status"] == 0
     err = np.linalg.norm(psi - want) / np.linalg.norm(want)
     assert err < (2e-5 if precision == 32 else 1e-9), err
+
+
+# ---------------------------------------------------------------- full BASELINE sizes (configs 3 and 4)
+@pytest.mark.parametrize("cfg_index", [3, 4])
+def test_next_rows_at_full_size(wilson, oracle, cfg_index):
+    """32^4 and 48^3x96 in the launch configuration bench.py --rows times: BiCGSTAB, even-odd CG and the 12-real CG
+    each reach the tolerance, with the TRUE residual |eta - D psi|/|eta| evaluated by the oracle's fp64 D on the full
+    lattice, and agree with the plain CG solution (whose parity with the stored oracle solve is tested in
+    test_gpu_parity.py) to what the tolerance allows."""
+    cfg = inputs.CONFIGS[cfg_index]
+    U, eta = gu.config_fields(cfg_index, 32)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    bound = 4.0 * cfg.r_min / (1.0 - 8.0 * cfg.kappa) * (1 + 8 * cfg.kappa)
+    sols = {}
+    with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+        sols["cg"], info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
+        it_cg = info["iterations"]
+        sols["bicgstab"], ib = bicgstab_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
+        assert ib["status"] == 0 and ib["iterations"] < 0.5 * it_cg
+        Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
+        pe, ie = ctx.cg_solve_eo(Ue, ctx.wd_eo_pack_spinor(gu.to_device(eta)), cfg.kappa, cfg.r_min, cfg.max_iter)
+        sols["eo"] = gu.to_host(ctx.wd_eo_unpack_spinor(pe))
+        del Ue, pe
+        assert ie["status"] == 0 and ie["iterations"] < 0.5 * it_cg
+        ctx.wd_set_gauge_recon(12)
+        sols["recon12"], i12 = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
+        assert i12["status"] == 0 and abs(i12["iterations"] - it_cg) <= math.floor(0.02 * it_cg + 0.5)
+    for name in ("bicgstab", "eo", "recon12"):
+        res = oracle.true_residual(cfg.dims, U64, eta64, sols[name].astype(np.complex128), cfg.kappa, cfg.bc_t)
+        assert res < 2.0 * cfg.r_min, (name, res)
+        diff = np.linalg.norm(sols[name] - sols["cg"]) / np.linalg.norm(sols["cg"])
+        assert diff < bound, (name, diff)
