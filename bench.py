@@ -257,7 +257,7 @@ def run_rows(args):
     prec = args.precision
     cdt = np.complex64 if prec == 32 else np.complex128
     rb = 4 if prec == 32 else 8
-    for ci in (3, 4):
+    for ci in [int(x) for x in args.rows_configs.split(",") if x]:
         cfg = inputs.CONFIGS[ci]
         r_min = cfg.r_min if prec == 32 else 1e-10
         U, eta = inputs.config_inputs(cfg, dtype=cdt)
@@ -447,6 +447,7 @@ def main():
     ap.add_argument("--rows", action="store_true",
                     help="one JSON line per SURVEY.md 8(f) row: 12-real links and BiCGSTAB at configs 3 and 4, the paper's COO "
                          "SpMV at 14^4 beside the stencil")
+    ap.add_argument("--rows-configs", default="3,4", help="configs the solver rows of --rows run on (comma separated)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()

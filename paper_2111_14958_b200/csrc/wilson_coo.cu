@@ -94,32 +94,40 @@ __global__ void __launch_bounds__(COO_NT)
 coo_spmv_kernel(long nnz, const cvec *__restrict__ val, const int *__restrict__ row, const int *__restrict__ col,
                 const cvec *__restrict__ in, cvec *out)
 {
+    constexpr int UNROLL = 4;   // independent 32-entry groups per trip: the Col -> in[Col] dependent loads overlap
     const int lane = threadIdx.x & 31;
     const long warp = ((long)blockIdx.x * COO_NT + threadIdx.x) >> 5;
     const long nwarps = ((long)gridDim.x * COO_NT) >> 5;
-    for (long base = warp * 32; base < nnz; base += nwarps * 32) {
-        const long k = base + lane;
-        int r = -1;
-        cvec p;
-        p.x = 0; p.y = 0;
-        if (k < nnz) {
-            r = __ldg(row + k);
-            const cvec v = __ldg(val + k), x = __ldg(in + __ldg(col + k));
-            p.x = v.x * x.x - v.y * x.y;
-            p.y = v.x * x.y + v.y * x.x;
-        }
-        // runs of equal Row among ADJACENT lanes: head flags -> lane of my run's head -> segmented inclusive scan
-        const int rprev = __shfl_up_sync(0xffffffffu, r, 1);
-        const unsigned int heads = __ballot_sync(0xffffffffu, lane == 0 || rprev != r);
-        const int head = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
+    for (long base = warp * (32 * UNROLL); base < nnz; base += nwarps * (32 * UNROLL)) {
+        int r[UNROLL];
+        cvec p[UNROLL];
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const auto px = __shfl_up_sync(0xffffffffu, p.x, o);
-            const auto py = __shfl_up_sync(0xffffffffu, p.y, o);
-            if (lane - o >= head) { p.x += px; p.y += py; }
+        for (int u = 0; u < UNROLL; ++u) {
+            const long k = base + u * 32 + lane;
+            r[u] = -1;
+            p[u].x = 0; p[u].y = 0;
+            if (k < nnz) {
+                r[u] = __ldg(row + k);
+                const cvec v = __ldg(val + k), x = __ldg(in + __ldg(col + k));
+                p[u].x = v.x * x.x - v.y * x.y;
+                p[u].y = v.x * x.y + v.y * x.x;
+            }
         }
-        const int rnext = __shfl_down_sync(0xffffffffu, r, 1);
-        if (r >= 0 && (lane == 31 || rnext != r)) atomic_add_c(out + r, p);
+#pragma unroll
+        for (int u = 0; u < UNROLL; ++u) {
+            // runs of equal Row among ADJACENT lanes: head flags -> lane of my run's head -> segmented inclusive scan
+            const int rprev = __shfl_up_sync(0xffffffffu, r[u], 1);
+            const unsigned int heads = __ballot_sync(0xffffffffu, lane == 0 || rprev != r[u]);
+            const int head = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const auto px = __shfl_up_sync(0xffffffffu, p[u].x, o);
+                const auto py = __shfl_up_sync(0xffffffffu, p[u].y, o);
+                if (lane - o >= head) { p[u].x += px; p[u].y += py; }
+            }
+            const int rnext = __shfl_down_sync(0xffffffffu, r[u], 1);
+            if (r[u] >= 0 && (lane == 31 || rnext != r[u])) atomic_add_c(out + r[u], p[u]);
+        }
     }
 }
 
@@ -160,7 +168,7 @@ extern "C" int wd_coo_spmv(wd_ctx *c, size_t nnz, const void *val, const int *ro
     const size_t out_bytes = (size_t)c->V * 12 * 2 * (c->precision == 32 ? 4 : 8);
     CUDA_TRY(c, cudaMemsetAsync(out, 0, out_bytes, c->stream));
     if (nnz == 0) return WD_OK;
-    size_t need = (nnz + COO_NT - 1) / COO_NT;
+    size_t need = (nnz + 4 * COO_NT - 1) / (4 * COO_NT);   // 4 groups of 32 entries per warp and trip
     const size_t cap = (size_t)c->sm_count * 8 * 4;   // 8 CTAs per SM resident, 4 waves: warps stride over the entries
     const unsigned int grid = (unsigned int)(need < cap ? need : cap);
     if (c->precision == 32)

@@ -55,5 +55,51 @@ def main(max_cfg=4):
               f"{res:.3e} / {res_o:.3e} | {info['rel_residual']:.3e} |", flush=True)
 
 
+def rows(max_cfg=4):
+    """The SURVEY.md 8(f) rows: BiCGSTAB, even-odd CG, 12-real CG (iterations and true residual, GPU / oracle) and the
+    COO route.  The oracle solves run live for configs 0-2; at configs 3 and 4 only the true residual of the GPU
+    solution is evaluated (one oracle D application)."""
+    print("\n| config | solver | iterations GPU / oracle | true residual GPU / oracle |")
+    print("|---|---|---|---|")
+    for ci in range(0, max_cfg + 1):
+        cfg = inputs.CONFIGS[ci]
+        U, eta = inputs.config_inputs(cfg, dtype=np.complex64)
+        U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+        live = ci <= 2
+        with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+            Ud, ed = torch.from_numpy(U).cuda(), torch.from_numpy(eta).cuda()
+            Un, en = ctx.wd_pack_gauge(Ud), ctx.wd_pack_spinor(ed)
+            out = {}
+            pn, ib = ctx.bicgstab_solve(Un, en, cfg.kappa, cfg.r_min, cfg.max_iter)
+            out["BiCGSTAB on D"] = (ctx.wd_unpack_spinor(pn).cpu().numpy(), ib, wilson_oracle.bicgstab_solve)
+            Ue, ee = ctx.wd_eo_pack_gauge(Ud), ctx.wd_eo_pack_spinor(ed)
+            pe, ie = ctx.cg_solve_eo(Ue, ee, cfg.kappa, cfg.r_min, cfg.max_iter)
+            out["even-odd CG"] = (ctx.wd_eo_unpack_spinor(pe).cpu().numpy(), ie, wilson_oracle.cg_solve_eo)
+            del Ue, ee, pe
+            ctx.wd_set_gauge_recon(12)
+            p12, i12 = ctx.cg_solve(ctx.wd_pack_gauge(Ud), en, cfg.kappa, cfg.r_min, cfg.max_iter)
+            out["CG, 12-real links"] = (ctx.wd_unpack_spinor(p12).cpu().numpy(), i12, wilson_oracle.cg_solve)
+        for name, (psi, info, ofun) in out.items():
+            res = wilson_oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
+            if live:
+                po, io = ofun(cfg.dims, U64, eta64, cfg.kappa, cfg.r_min, cfg.max_iter, cfg.bc_t)
+                ro = wilson_oracle.true_residual(cfg.dims, U64, eta64, po, cfg.kappa, cfg.bc_t)
+                print(f"| {ci}: {cfg.name} | {name} | {info['iterations']} / {io['iterations']} | {res:.3e} / {ro:.3e} |", flush=True)
+            else:
+                print(f"| {ci}: {cfg.name} | {name} | {info['iterations']} / (not run) | {res:.3e} / — |", flush=True)
+    # COO at 14^4
+    cfg = inputs.CONFIGS[2]
+    U, eta = inputs.config_inputs(cfg, dtype=np.complex64)
+    with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+        Un = ctx.wd_pack_gauge(torch.from_numpy(U).cuda())
+        val, row, col = ctx.wd_coo_assemble(Un, cfg.kappa, False)
+        got = ctx.wd_coo_spmv(val, row, col, torch.from_numpy(eta).cuda()).cpu().numpy()
+    want = wilson_oracle.wd_apply(cfg.dims, U.astype(np.complex128), eta.astype(np.complex128), cfg.kappa, False, cfg.bc_t)
+    print(f"\nCOO SpMV at 14^4 (N_NZ = {val.numel()}): per-site relative error against the oracle's D "
+          f"{lm.per_site_rel_err(got, want)[0]:.2e}", flush=True)
+
+
 if __name__ == "__main__":
-    main(int(sys.argv[1]) if len(sys.argv) > 1 else 4)
+    mc = int(sys.argv[1]) if len(sys.argv) > 1 else 4
+    main(mc)
+    rows(mc)
