@@ -318,6 +318,36 @@ def run_rows(args):
                         "iteration_frac_of_measured": sum(bb) * V / (sum(kus) * 1e-6) / 1e9 / peak if sum(kus) > 0 else None,
                         "cg_solve_ms_same_problem": t, "speedup_vs_cg": t / tb}), flush=True)
                 if recon == 18:
+                    for nrhs in (2, 4):
+                        em = torch.stack([en * (1.0 + 0.25 * j) for j in range(nrhs)]).contiguous()
+                        om = ctx.empty_multi_spinor(nrhs)
+                        for _ in range(3):
+                            ctx.wd_apply_multi(Un, em, cfg.kappa, False, out=om)
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        torch.cuda.synchronize()
+                        e0.record()
+                        for _ in range(20):
+                            ctx.wd_apply_multi(Un, em, cfg.kappa, False, out=om)
+                        e1.record()
+                        torch.cuda.synchronize()
+                        ap_ms = e0.elapsed_time(e1) / 20
+                        ctx.cg_solve_multi(Un, em, cfg.kappa, r_min, cfg.max_iter, out=om)
+                        ctx.wd_set_profile(True)
+                        _, infos = ctx.cg_solve_multi(Un, em, cfg.kappa, r_min, cfg.max_iter, out=om)
+                        pm = ctx.wd_get_profile_bicgstab()
+                        ctx.wd_set_profile(False)
+                        km = [m / max(pm["iterations"], 1) * 1e3 / nrhs for m in pm["ms"][:3]]
+                        bm = (2 * sb + gb / nrhs, 3 * sb + gb / nrhs, 5 * sb)     # per source: the links are shared
+                        print(json.dumps({
+                            "row": "f3 multi-rhs", "config": ci, "precision": prec, "nrhs": nrhs,
+                            "iterations": [i["iterations"] for i in infos],
+                            "wd_apply_us_per_source": ap_ms * 1e3 / nrhs, "wd_apply_us_single": d_ms * 1e3,
+                            "solve_ms_per_source": infos[0]["gpu_ms"] / nrhs, "solve_ms_single": t,
+                            "kernel_us_per_source": dict(zip(("a2", "a3", "a4"), km)),
+                            "bytes_per_site_per_source": dict(zip(("a2", "a3", "a4"), bm)),
+                            "iteration_gbs": sum(bm) * V / (sum(km) * 1e-6) / 1e9 if sum(km) > 0 else None,
+                            "speedup_per_source_vs_single": t / (infos[0]["gpu_ms"] / nrhs)}), flush=True)
+                        del em, om
                     Ue = ctx.wd_eo_pack_gauge(torch.from_numpy(U).cuda())
                     ee = ctx.wd_eo_pack_spinor(torch.from_numpy(eta).cuda())
                     pe = ctx.empty_eo_spinor()

@@ -81,7 +81,7 @@ typedef struct wd_cg_info {
     double gpu_ms;         /* device time of init + loop + final D-dagger (CUDA events on the ctx stream) */
     double total_ms;       /* *_host calls: device time including H2D copies, pack, solve, unpack, D2H; else = gpu_ms */
     int kernel_launches;   /* number of this library's kernels launched by the call */
-    int cg_mode;           /* 1 = three kernels per iteration, 2 = whole solve in one cooperative launch, 3 = BiCGSTAB, 4 = even-odd CG */
+    int cg_mode;           /* 1 = three kernels per iteration, 2 = whole solve in one cooperative launch, 3 = BiCGSTAB, 4 = even-odd CG, 5 = multi-source CG */
 } wd_cg_info;
 
 /*
@@ -209,6 +209,24 @@ int wd_eo_pack_gauge(wd_ctx *ctx, const void *U_canonical_dev, void *U_eo_dev);
 int wd_eo_hop(wd_ctx *ctx, const void *U_eo, const void *in_eo, void *out_eo, int out_parity, int dagger);
 int cg_solve_eo(wd_ctx *ctx, const void *U_eo, const void *eta_eo, void *psi_eo_out,
                 double kappa, double r_min, int max_iter, wd_cg_info *info);
+
+/*
+ * Several right-hand sides at once (the gauge field is 60 % of the bytes of a stencil pass and is the
+ * same for every source).  The nrhs sources are INDEPENDENT problems D psi_j = eta_j on one gauge field: each has its own
+ * alpha, beta, residual, loop test and iteration count, exactly as nrhs calls of cg_solve would (the oracle of these calls
+ * is nrhs oracle solves).  Fields: nrhs native spinors one after the other (source j at byte offset
+ * j * wd_spinor_native_bytes(ctx)).  Sources are processed in groups of 4 (then 2; a last single one through the plain
+ * path); inside a group one CTA handles a tile of sites for all sources of the group, so every link is fetched from
+ * DRAM / L2 once per group instead of once per source.  18-real links only.
+ *   wd_apply_multi   out_j = D in_j (or D-dagger in_j), j < nrhs.  Asynchronous on the ctx stream.
+ *   cg_solve_multi   psi_j = solution of D psi_j = eta_j by the CG of cg_solve; infos: host array of nrhs records
+ *                    (may be NULL; gpu_ms is the device time of the source's whole group, cg_mode = 5).  Returns WD_OK,
+ *                    WD_NOT_CONVERGED if any source hit max_iter, or an error.  Synchronous.
+ */
+int wd_apply_multi(wd_ctx *ctx, const void *U_native, const void *in_multi, void *out_multi, int nrhs,
+                   double kappa, int dagger);
+int cg_solve_multi(wd_ctx *ctx, const void *U_native, const void *eta_multi, void *psi_multi_out, int nrhs,
+                   double kappa, double r_min, int max_iter, wd_cg_info *infos);
 
 /*
  * The paper's own route: "we store the sparse matrix D in the so-called coordinate format, i.e. D is

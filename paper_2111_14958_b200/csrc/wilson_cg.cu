@@ -156,11 +156,13 @@ extern "C" int wd_destroy(wd_ctx *c)
 {
     if (!c) return WD_OK;
     cudaStreamSynchronize(c->stream);
-    void *dev[] = {c->r, c->p, c->q, c->y, c->w5, c->w6, c->eo_n2, c->sc, c->partials, c->counter, c->hist, c->result_dev,
+    void *dev[] = {c->r, c->p, c->q, c->y, c->w5, c->w6, c->eo_n2, c->m_ws[0], c->m_ws[1], c->m_ws[2], c->m_ws[3], c->m_sc,
+                   c->m_counter, c->m_hist, c->sc, c->partials, c->counter, c->hist, c->result_dev,
                    c->U_can, c->U_nat, c->s_can, c->s_nat_in, c->s_nat_out};
     for (void *ptr : dev)
         if (ptr) cudaFree(ptr);
     if (c->sc_host) cudaFreeHost(c->sc_host);
+    if (c->m_sc_host) cudaFreeHost(c->m_sc_host);
     if (c->result_host) cudaFreeHost(c->result_host);
     for (int i = 0; i < 4; ++i)
         if (c->ev[i]) cudaEventDestroy(c->ev[i]);

@@ -30,6 +30,13 @@ struct wd_ctx {
     void *w5;             // fifth work vector (BiCGSTAB: t; even-odd: the odd-parity intermediate)
     void *w6;             // even-odd: etahat (half length)
     double *eo_n2;        // even-odd: <eta_e,eta_e>, <eta_o,eta_o> (device)
+    // multi-right-hand-side CG: r, p, q, y for a group of up to 4 sources, per-source scalars, counters, histories
+    void *m_ws[4];
+    size_t m_bytes;
+    wd::CgScalars *m_sc, *m_sc_host;
+    unsigned int *m_counter;
+    double *m_hist;
+    int m_hist_cap;
     wd::CgScalars *sc;
     double *partials;
     size_t partials_cap;

@@ -89,6 +89,8 @@ def load_library(path: str = LIB_PATH):
     lib.wd_eo_pack_gauge.argtypes = [vp, vp, vp]
     lib.wd_eo_hop.argtypes = [vp, vp, vp, vp, ci, ci]
     lib.cg_solve_eo.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
+    lib.wd_apply_multi.argtypes = [vp, vp, vp, vp, ci, cd, ci]
+    lib.cg_solve_multi.argtypes = [vp, vp, vp, vp, ci, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
     lib.wd_coo_nnz.argtypes = [vp]
     lib.wd_coo_nnz.restype = ctypes.c_size_t
     lib.wd_coo_assemble.argtypes = [vp, vp, cd, ci, vp, vp, vp]
@@ -313,6 +315,28 @@ class WilsonContext:
         d = info.as_dict()
         d["status"] = rc
         return out, d
+
+    # -- f3: several right-hand sides at once (fields: (nrhs, n) real tensors, row j = native spinor of source j)
+    def empty_multi_spinor(self, nrhs):
+        torch = _torch()
+        n = self.lib.wd_spinor_native_bytes(self._ctx) // (4 if self.precision == 32 else 8)
+        return torch.empty((int(nrhs), n), dtype=self.real_dtype, device="cuda")
+
+    def wd_apply_multi(self, U_native, in_multi, kappa, dagger=False, out=None):
+        nrhs = in_multi.shape[0]
+        out = self.empty_multi_spinor(nrhs) if out is None else out
+        self._check(self.lib.wd_apply_multi(self._ctx, self._p(U_native), self._p(in_multi), self._p(out), int(nrhs),
+                                            float(kappa), int(bool(dagger))))
+        return out
+
+    def cg_solve_multi(self, U_native, eta_multi, kappa, r_min, max_iter, out=None):
+        nrhs = eta_multi.shape[0]
+        out = self.empty_multi_spinor(nrhs) if out is None else out
+        infos = (WdCgInfo * nrhs)()
+        rc = self.lib.cg_solve_multi(self._ctx, self._p(U_native), self._p(eta_multi), self._p(out), int(nrhs),
+                                     float(kappa), float(r_min), int(max_iter), infos)
+        self._check(rc, allow_not_converged=True)
+        return out, [dict(i.as_dict(), status=0 if i.converged else 1) for i in infos]
 
     # -- f2: the paper's coordinate-format route
     def wd_coo_nnz(self):

@@ -434,3 +434,96 @@ def test_next_rows_at_full_size(wilson, oracle, cfg_index):
         assert res < 2.0 * cfg.r_min, (name, res)
         diff = np.linalg.norm(sols[name] - sols["cg"]) / np.linalg.norm(sols["cg"])
         assert diff < bound, (name, diff)
+
+
+# ---------------------------------------------------------------- f3: several right-hand sides at once
+def _sources(cfg_seed, dims, nrhs, cdt):
+    """nrhs different sources: Gaussian fields, a point source (other iteration count) and, last, the zero field
+    (0 iterations: its warps are idle from the first pass on)"""
+    V = int(np.prod(dims))
+    out = []
+    for j in range(nrhs):
+        if j == 1:
+            e = np.zeros((V, 4, 3), dtype=np.complex128)
+            e[V // 3] = inputs.complex_gaussian(inputs.slice_rng(cfg_seed, inputs.FIELD_AUX, 99), (4, 3))
+        elif j == nrhs - 1 and nrhs > 2:
+            e = np.zeros((V, 4, 3), dtype=np.complex128)
+        else:
+            e = inputs.source_field(cfg_seed + 50 + j, dims)
+        out.append(e.astype(cdt))
+    return out
+
+
+def _pack_multi(ctx, fields):
+    import torch
+
+    return torch.stack([ctx.wd_pack_spinor(gu.to_device(f)) for f in fields]).contiguous()
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("nrhs", [2, 3, 4, 7])
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (5, 7, 4, 6), (14, 14, 14, 14)])
+def test_apply_multi_equals_single_applications(wilson, oracle, dims, nrhs, precision):
+    """out_j = D in_j for every source: bit-identical to nrhs calls of wd_apply (same per-site arithmetic), and within
+    the wd_apply tolerance of the oracle"""
+    cdt = gu.np_complex(precision)
+    U = inputs.gauge_field(CFG_TEST + 60, dims, "haar", dtype=cdt)
+    srcs = _sources(CFG_TEST + 60, dims, nrhs, cdt)
+    with wilson.WilsonContext(dims, precision) as ctx:
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        multi = _pack_multi(ctx, srcs)
+        for dagger in (False, True):
+            out = ctx.wd_apply_multi(Un, multi, 0.12, dagger)
+            for j in range(nrhs):
+                single = ctx.wd_apply(Un, multi[j], 0.12, dagger)
+                # (compared after unpacking: the pad lanes of a ragged volume are never written)
+                assert gu.to_host(ctx.wd_unpack_spinor(out[j])).tobytes() == gu.to_host(ctx.wd_unpack_spinor(single)).tobytes()
+            got = gu.to_host(ctx.wd_unpack_spinor(out[0]))
+            want = oracle.wd_apply(dims, U.astype(np.complex128), srcs[0].astype(np.complex128), 0.12, dagger, -1)
+            assert lm.per_site_rel_err(got, want)[0] <= (1e-5 if precision == 32 else 1e-12)
+
+
+@pytest.mark.parametrize("precision,r_min", [(32, 1e-6), (64, 1e-10)])
+@pytest.mark.parametrize("cfg_index,nrhs", [(0, 4), (1, 4), (1, 3), (2, 2), (2, 5)])
+def test_cg_solve_multi_matches_oracle_per_source(wilson, oracle, cfg_index, nrhs, precision, r_min):
+    cfg = inputs.CONFIGS[cfg_index]
+    cdt = gu.np_complex(precision)
+    U, _ = gu.config_fields(cfg.index, precision)
+    U64 = U.astype(np.complex128)
+    srcs = _sources(cfg.index, cfg.dims, nrhs, cdt)
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        ctx.wd_set_cg_mode(1)
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        psi_m, infos = ctx.cg_solve_multi(Un, _pack_multi(ctx, srcs), cfg.kappa, r_min, cfg.max_iter)
+        psis = [gu.to_host(ctx.wd_unpack_spinor(psi_m[j])) for j in range(nrhs)]
+    its = []
+    for j in range(nrhs):
+        e64 = srcs[j].astype(np.complex128)
+        po, io = oracle.cg_solve(cfg.dims, U64, e64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t)
+        its.append(io["iterations"])
+        assert infos[j]["converged"] == 1
+        assert abs(infos[j]["iterations"] - io["iterations"]) <= math.floor(0.02 * io["iterations"] + 0.5), (j, infos[j], io)
+        if not e64.any():
+            assert infos[j]["iterations"] == 0 and not psis[j].any()
+            continue
+        res = oracle.true_residual(cfg.dims, U64, e64, psis[j].astype(np.complex128), cfg.kappa, cfg.bc_t)
+        res_o = oracle.true_residual(cfg.dims, U64, e64, po, cfg.kappa, cfg.bc_t)
+        assert res <= 2.0 * res_o and res < 2.0 * r_min, (j, res, res_o)
+        assert abs(infos[j]["eta_norm2"] - io["eta_norm2"]) < (1e-6 if precision == 32 else 1e-13) * io["eta_norm2"]
+    if nrhs > 2:
+        assert len(set(its)) > 1      # the sources really stop at different iterations (the zero source at 0)
+
+
+def test_cg_solve_multi_max_iter_and_determinism(wilson):
+    cfg = inputs.CONFIGS[1]
+    U, _ = gu.config_fields(1, 32)
+    srcs = _sources(cfg.index, cfg.dims, 4, np.complex64)
+    with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        em = _pack_multi(ctx, srcs)
+        a, ia = ctx.cg_solve_multi(Un, em, cfg.kappa, 1e-6, 1000)
+        ctx.wd_set_poll_interval(1)
+        b, ib = ctx.cg_solve_multi(Un, em, cfg.kappa, 1e-6, 1000)
+        assert gu.to_host(a).tobytes() == gu.to_host(b).tobytes() and [i["iterations"] for i in ia] == [i["iterations"] for i in ib]
+        _, ic = ctx.cg_solve_multi(Un, em, cfg.kappa, 1e-6, 5)
+        assert [i["iterations"] for i in ic] == [5, 5, 5, 0] and [i["converged"] for i in ic] == [0, 0, 0, 1]
