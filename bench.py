@@ -424,7 +424,10 @@ def run_sweep(args, cfg, ctx, wilson, Un, en, psi_n, r_min):
 
     V = cfg.volume
     b2, b3, b4 = (480, 576, 480) if args.precision == 32 else (960, 1152, 960)
+    only = [int(t) for t in args.sweep_tiles.split(",")] if args.sweep_tiles else None
     for tile, inf in enumerate(wilson.tile_infos()):
+        if only is not None and tile not in only:
+            continue
         try:
             ctx.wd_set_tile(tile)
         except wilson.WilsonError:
@@ -471,6 +474,7 @@ def main():
     ap.add_argument("--sweep", action="store_true",
                     help="time every compiled launch configuration (the paper's workgroup-size tuning, PAPER.md:76) "
                          "on this config and print one JSON line per configuration instead of the bench line")
+    ap.add_argument("--sweep-tiles", default="", help="launch configurations --sweep visits (comma separated; default all)")
     ap.add_argument("--report", action="store_true",
                     help="one JSON line per BASELINE config (0..4, plus config 3 in fp64): wd_apply D / D-dagger over 100 "
                          "applications and the CG solve; the table of BASELINE.md section 3")

@@ -511,21 +511,30 @@ __device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, i
 // U: links of the sites being written (forward hops); UB: links of the neighbours' field (backward hops; == U on a
 // plain lattice, the other parity's links with even-odd); cen: the field of the diagonal term (== in on a plain
 // lattice; nullptr = no diagonal term, c = 0).
+// CFIRST (PIPE = 1 only): the diagonal term goes FIRST.  acc starts as in(s), fetched together with the +-x hops (the
+// same cache lines), and every hop is accumulated with the factor -kappa folded into its boundary sign, so that on
+// return acc = in(s) - kappa * hops = (D in)(s) and c is not touched: no centre fetch at the end of the tile's life
+// (when its lines have left the L1), one dependent load step and 24 live registers fewer in the epilogue.
 template <int DAG, int PIPE, bool LOADR, bool RO, typename real, typename svec, typename gvec, int RECON = 18, int NT = 0,
-          int EO = 0>
+          int EO = 0, bool CFIRST = false>
 __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const gvec *__restrict__ UB,
                                             const svec *in, const svec *cen, const svec *r, int x, int y, int z, int t,
                                             int s, real acc[24], real c[24], real rv[24], void *smem = nullptr,
-                                            int next_s = -1)
+                                            int next_s = -1, real kappa = 0)
 {
+    static_assert(!CFIRST || PIPE == 1, "centre-first is implemented for the two-buffer pipeline");
     constexpr int SF = DAG ? +1 : -1;
     const Hops n = neighbours<EO>(g, x, y, z, t, s);
     // boundary sign sigma+- of reading C-1: only the hop that wraps the t boundary carries bc_t
-    const real sgf = (t == g.L[3] - 1) ? (real)g.bc_t : (real)1;
-    const real sgb = (t == 0) ? (real)g.bc_t : (real)1;
-    const real one = (real)1;
+    const real one = CFIRST ? -kappa : (real)1;
+    const real sgf = (t == g.L[3] - 1) ? (real)g.bc_t * one : one;
+    const real sgb = (t == 0) ? (real)g.bc_t * one : one;
+    if (CFIRST) {
+        load_centre<RO, EO != 0>(cen, s, acc);
+    } else {
 #pragma unroll
-    for (int i = 0; i < 24; ++i) acc[i] = 0;
+        for (int i = 0; i < 24; ++i) acc[i] = 0;
+    }
     if (PIPE == 0) {
         real v[24], u[18];
         hop_load<0, RO, RECON, real>(U, in, s, n.f[0], v, u);       hop_compute<0, SF, false, real>(v, u, one, acc);
@@ -548,7 +557,7 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
         hop_load<2, RO, RECON, real>(UB, in, n.b[2], n.b[2], vb, ub);  hop_compute<2, SF, false, real>(va, ua, one, acc);
         hop_load<3, RO, RECON, real>(U, in, s, n.f[3], va, ua);       hop_compute<2, -SF, true, real>(vb, ub, one, acc);
         hop_load<3, RO, RECON, real>(UB, in, n.b[3], n.b[3], vb, ub);  hop_compute<3, SF, false, real>(va, ua, sgf, acc);
-        load_centre<RO, EO != 0>(cen, s, c);
+        if (!CFIRST) load_centre<RO, EO != 0>(cen, s, c);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
         if (LOADR) load_spinor_rw(r, s, rv);   // after the last hop: an earlier fetch costs registers (spills at 128)
     } else if (PIPE == 2) {
@@ -766,6 +775,13 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     using svec = typename Field<real>::svec;
     using gvec = typename Field<real>::gvec;
     constexpr int NT = BX * BY * BZ * BT;
+    // PIPE = 1: the two-buffer pipeline with the diagonal term FIRST (hopping_sum CFIRST) wherever the pass has no
+    // second per-site stream: measured at 48^3x96 fp32, a2 999 -> 920-934 us, wd_apply 990 -> 940 us.  MODE_RUPD keeps
+    // the centre and r last: centre-first made a3 slower (1017 -> 1086 us), and so did folding r into the
+    // accumulator as well (acc = r - alpha in, hops scaled by alpha kappa: 1056 us).  MODE_TS needs s(x) beside t(x).
+    // PIPE = 4: the same pipeline with the centre last in every mode (the comparison row of the table).
+    constexpr bool CF = (PIPE == 1) && MODE != MODE_TS && MODE != MODE_RUPD;
+    constexpr int HP = (PIPE == 4) ? 1 : PIPE;
     if (MODE != MODE_PLAIN) {
         if (it >= sc->k_stop) return;  // uniform over the grid: over-launched iterations are no-ops
     } else if (sc) {
@@ -818,8 +834,8 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
         if (!active) continue;
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24], rv[24];
-        hopping_sum<DAG, PIPE, MODE == MODE_RUPD || MODE == MODE_RV, true, real, svec, gvec, RECON, NT, EO>(
-            g, U, EO ? UB : U, in, EO ? cen : in, r, x, y, z, t, s, acc, c, rv, wd_dyn_smem, next_s);
+        hopping_sum<DAG, HP, MODE == MODE_RUPD || MODE == MODE_RV, true, real, svec, gvec, RECON, NT, EO, CF>(
+            g, U, EO ? UB : U, in, EO ? cen : in, r, x, y, z, t, s, acc, c, rv, wd_dyn_smem, next_s, kappa);
         if constexpr (MODE == MODE_TS) {
             // c holds s(x); t(x) = s(x) - kappa * hops replaces it component by component
             real tsr = 0, tsi = 0, tt = 0;
@@ -836,7 +852,7 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
             local += (double)tsr; local1 += (double)tsi; local2 += (double)tt;
         } else {
 #pragma unroll
-        for (int i = 0; i < 24; ++i) c[i] = fma(-kappa, acc[i], c[i]);  // (D in)(x) = in(x) - kappa * hops
+        for (int i = 0; i < 24; ++i) c[i] = CF ? acc[i] : fma(-kappa, acc[i], c[i]);  // (D in)(x) = in(x) - kappa * hops
         if (MODE == MODE_RV) {
             real dr = 0, di = 0;
 #pragma unroll

@@ -1,7 +1,8 @@
 // wilson_launch.cuh — the table of compiled stencil launch configurations and the per-precision launchers.
 // A "tile" (the name of the C ABI, wd_set_tile) is one row: CTA tile BX x BY x BZ x BT (threads per CTA =
 // product), MINB = minimum resident CTAs per SM asked of ptxas (bounds registers per thread), PIPE = 1 for
-// the software-pipelined hop loop (2 = three register buffers, 3 = forward links staged through shared memory with
+// the software-pipelined hop loop with the diagonal term first (4 = the same with the diagonal term last, the
+// comparison rows 18 and 19; 2 = three register buffers, 3 = forward links staged through shared memory with
 // cp.async one tile ahead, 18-real links only).  This is the CUDA analogue of the paper's workgroup-size knob
 // (PAPER.md:58,76).  F64 = 1 if the row is also compiled for double precision.
 #pragma once
@@ -28,8 +29,10 @@
     X(14, 16, 2, 2, 2, 0, 0, 1) \
     X(15, 8, 4, 4, 2, 0, 0, 1) \
     X(16, 16, 2, 2, 2, 3, 2, 0) \
-    X(17, 16, 2, 2, 2, 4, 3, 0)
-#define WD_NUM_TILES 18
+    X(17, 16, 2, 2, 2, 4, 3, 0) \
+    X(18, 16, 2, 2, 2, 4, 4, 0) \
+    X(19, 32, 2, 2, 1, 2, 4, 1)
+#define WD_NUM_TILES 20
 
 // Launch configurations of the one-launch CG kernel (small volumes): 64- and 128-thread tiles,
 // no register bound (ptxas then hoists the loads of all 8 hops: one memory round trip per site instead of 8,

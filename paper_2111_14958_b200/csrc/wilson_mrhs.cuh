@@ -51,9 +51,11 @@ dslash_mrhs_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ 
         if (!live || x >= g.L[0] || y >= g.L[1] || z >= g.L[2] || t >= g.L[3]) continue;
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24], rv[24];
-        hopping_sum<DAG, 1, MODE == MODE_RUPD, true, real, svec, gvec>(g, U, U, in, in, r, x, y, z, t, s, acc, c, rv);
+        constexpr bool CF = MODE != MODE_RUPD;   // diagonal term first, as in dslash_kernel PIPE = 1
+        hopping_sum<DAG, 1, MODE == MODE_RUPD, true, real, svec, gvec, 18, 0, 0, CF>(g, U, U, in, in, r, x, y, z, t, s,
+                                                                                  acc, c, rv, nullptr, -1, kappa);
 #pragma unroll
-        for (int i = 0; i < 24; ++i) c[i] = fma(-kappa, acc[i], c[i]);
+        for (int i = 0; i < 24; ++i) c[i] = CF ? acc[i] : fma(-kappa, acc[i], c[i]);
         if (MODE == MODE_RUPD) {
             real n2 = 0;
 #pragma unroll
