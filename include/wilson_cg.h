@@ -298,6 +298,11 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *                             stride over the tiles; w = 0 or 1: exactly one resident wave (default).
  *   wd_set_zchunk(ctx, layers)    z extent (in sites) of one chunk of the CTA rasterisation x,y,z-in-chunk,t,z-chunk that
  *                             keeps the +-t neighbours of a tile in L2; 0 = automatic (fits a 40 MB reuse distance).
+ *   wd_set_sweep(ctx, a)          a = 1: consecutive passes over the lattice (the three kernels of a cg_solve iteration,
+ *                             back-to-back wd_apply calls) walk it in alternating directions, so that each pass starts on
+ *                             the data the previous one left in the 126 MB L2; a = 0 (default: the alternation measured no
+ *                             gain on B200): every pass walks forward.  The per-site arithmetic is identical; only the
+ *                             grouping of the reduction partials changes.
  *   wd_set_poll_interval(ctx, n)  CG iterations enqueued between two host polls of the device stop flag (n >= 1; 0 = automatic).
  */
 int wd_num_tiles(void);
@@ -309,6 +314,7 @@ int wd_set_cg_mode(wd_ctx *ctx, int mode);
 int wd_set_prefetch(wd_ctx *ctx, int tiles);
 int wd_set_waves(wd_ctx *ctx, int waves);
 int wd_set_zchunk(wd_ctx *ctx, int layers);
+int wd_set_sweep(wd_ctx *ctx, int alternate);
 int wd_set_poll_interval(wd_ctx *ctx, int n);
 
 /*

@@ -34,10 +34,12 @@ extern "C" long wd_selftest_fastdiv(unsigned int d, unsigned int n_max)
 
 // ---------------------------------------------------------------- launches
 template <int DAG, int MODE>
-static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void *out, double kappa, void *r, int it)
+static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void *out, double kappa, void *r, int it,
+                                 int rev = 0)
 {
     DslashArgs a;
     a.g = make_geom(c, c->tile);
+    a.g.rev = rev;
     a.sm_count = c->sm_count;
     a.waves = c->waves > 0 ? c->waves : 1;
     a.prefetch = (c->dims[0] % SB == 0 && c->recon == 18) ? c->prefetch : 0;
@@ -132,6 +134,7 @@ extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_
     c->tile_user = -1;
     c->tile = auto_tile(c);
     c->l2_budget_mb = 40.0;
+    c->sweep = 0;      // measured on B200: alternating the walk direction gains nothing
     c->prefetch = 0;   // measured on B200: bulk L2 prefetch of the next tile slows the stencil by 15-30 %
     bool ok = true;
     ok = ok && cudaMalloc(&c->sc, sizeof(CgScalars)) == cudaSuccess;
@@ -245,6 +248,12 @@ extern "C" int wd_set_zchunk(wd_ctx *c, int layers)
     c->zchunk_user = layers;
     return WD_OK;
 }
+extern "C" int wd_set_sweep(wd_ctx *c, int alternate)
+{
+    if (!c || alternate < 0 || alternate > 1) return WD_ERR_ARG;
+    c->sweep = alternate;
+    return WD_OK;
+}
 extern "C" int wd_set_poll_interval(wd_ctx *c, int n)
 {
     if (!c || n < 0) return WD_ERR_ARG;
@@ -323,8 +332,9 @@ extern "C" int wd_apply(wd_ctx *c, const void *U, const void *psi, void *out, do
     if (!c) return WD_ERR_ARG;
     if (!U || !psi || !out || psi == out) return fail(c, WD_ERR_ARG, "wd_apply: NULL argument or out aliases psi");
     if (!std::isfinite(kappa)) return fail(c, WD_ERR_ARG, "wd_apply: kappa is not finite");
-    cudaError_t e = dagger ? launch_dslash<1, MODE_PLAIN>(c, U, psi, out, kappa, nullptr, 0)
-                           : launch_dslash<0, MODE_PLAIN>(c, U, psi, out, kappa, nullptr, 0);
+    const int rev = c->sweep ? (int)(c->apply_calls++ & 1u) : 0;   // back-to-back applications alternate (Geom.rev)
+    cudaError_t e = dagger ? launch_dslash<1, MODE_PLAIN>(c, U, psi, out, kappa, nullptr, 0, rev)
+                           : launch_dslash<0, MODE_PLAIN>(c, U, psi, out, kappa, nullptr, 0, rev);
     CUDA_TRY(c, e);
     return WD_OK;
 }
@@ -457,20 +467,24 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
         const int chunk = (max_iter - launched) < poll ? (max_iter - launched) : poll;
         for (int i = 0; i < chunk; ++i) {
             const int it = launched + i;
+            // direction of the three passes of iteration `it`: the init kernel ran forward, every pass after it walks
+            // against the one before (pass number 3 it + j + 1), so each starts on what the last one left in L2
+            const int rev2 = c->sweep ? (3 * it + 1) & 1 : 0, rev3 = c->sweep ? (3 * it + 2) & 1 : 0,
+                      rev4 = c->sweep ? (3 * it + 3) & 1 : 0;
             if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 0], c->stream));
             // a2: q = D-dagger p, qq, alpha
-            CUDA_TRY(c, (launch_dslash<1, MODE_QQ>(c, U, c->p, c->q, kappa, nullptr, it)));
+            CUDA_TRY(c, (launch_dslash<1, MODE_QQ>(c, U, c->p, c->q, kappa, nullptr, it, rev2)));
             if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 1], c->stream));
             // a3: r -= alpha D q, rr', beta, loop condition
-            CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it)));
+            CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it, rev3)));
             if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 2], c->stream));
             // a4: y += alpha p ; p = r + beta p
             if (c->precision == 32)
                 cg_update_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((float4 *)c->y, (float4 *)c->p,
-                                                                          (const float4 *)c->r, n, c->sc, it);
+                                                                          (const float4 *)c->r, n, c->sc, it, rev4);
             else
                 cg_update_kernel<double><<<vgrid, VEC_NT, 0, c->stream>>>((double2 *)c->y, (double2 *)c->p,
-                                                                           (const double2 *)c->r, n, c->sc, it);
+                                                                           (const double2 *)c->r, n, c->sc, it, rev4);
             c->launches++;
             CUDA_TRY(c, cudaGetLastError());
             if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 3], c->stream));
@@ -492,7 +506,9 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
         if (c->sc_host->k_stop <= launched) break;  // the device loop condition failed (or eta = 0)
     }
     // a6: psi = D-dagger y ("then we multiply the solution by D-dagger")
-    CUDA_TRY(c, (launch_dslash<1, MODE_PLAIN>(c, U, c->y, psi, kappa, nullptr, 0)));
+    // (against the last a4 that really ran: pass number 3 k, so this is pass 3 k + 1)
+    CUDA_TRY(c, (launch_dslash<1, MODE_PLAIN>(c, U, c->y, psi, kappa, nullptr, 0,
+                                              c->sweep ? (3 * c->sc_host->k + 1) & 1 : 0)));
     if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));

@@ -23,6 +23,8 @@ struct wd_ctx {
     int last_cg_mode;     // what the last cg_solve used
     int prefetch;         // L2 prefetch distance: -1 = automatic (one grid ahead), 0 = off, n > 0 = n tiles
     int zchunk_user;      // z layers per rasterisation chunk, 0 = automatic
+    int sweep;            // 1: consecutive passes walk the lattice in alternating directions (Geom.rev); 0 (default): all forward
+    unsigned apply_calls; // wd_apply calls so far (their direction alternates too)
     double l2_budget_mb;  // reuse-distance budget of the automatic choice
     int sm_count;
     // CG workspace (native layout), device
@@ -128,6 +130,7 @@ static inline wd::Geom make_geom_lattice(const int dims[4], int bc_t, const int 
     g.bc_t = bc_t;
     g.eo = 0;
     g.par = 0;
+    g.rev = 0;
     const double layer = 600.0 * dims[0] * dims[1] * tb[3];   // bytes per z layer of one t-tile row
     const double budget = l2_budget_mb * 1.0e6;
     int zc = 1;

@@ -258,7 +258,7 @@ static int eo_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, void *psi_eo
             CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_RUPD, 0, t, q, nullptr, r, k2, it, true}));
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[4], c->stream));
             // y += alpha p ; p = r + beta p
-            cg_update_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((svec *)y, (svec *)p, (const svec *)r, n, c->sc, it);
+            cg_update_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((svec *)y, (svec *)p, (const svec *)r, n, c->sc, it, 0);
             c->launches++;
             CUDA_TRY(c, cudaGetLastError());
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[5], c->stream));

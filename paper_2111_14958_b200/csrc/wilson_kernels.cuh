@@ -44,6 +44,9 @@ struct Geom {
     int eo;      // 1: the lattice of this launch is ONE PARITY of the real lattice (even-odd preconditioning, SURVEY.md
                  //    8(f3)): L[0] = Lx/2, site (xh,y,z,t) stands for x = 2 xh + ((y+z+t+par) & 1); 0: plain lattice
     int par;     // eo = 1: parity (x+y+z+t) & 1 of the sites this launch WRITES; its neighbours have parity 1 - par
+    int rev;     // 1: the persistent CTAs walk the rasterisation from its LAST tile to its first.  Consecutive passes of a
+                 //    solver alternate the direction, so that a pass starts on the ~100 MB the previous one left in L2
+                 //    (its output and the links it read last) instead of on the lines that were evicted first
     FastDiv d_chunk, d_nt0, d_nt1, d_zc, d_zlast;   // per_chunk, nt[0], nt[1], zc, size of the last z chunk
 };
 
@@ -793,10 +796,10 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     double local = 0.0, local1 = 0.0, local2 = 0.0;
     extern __shared__ __align__(16) unsigned char wd_dyn_smem[];   // PIPE = 3: staged forward links, 72 reals per thread
     // site of this thread in tile b, or -1 (no such tile / thread outside the lattice)
-    auto site_in_tile = [&](int b) -> int {
-        if (b >= g.ntiles) return -1;
+    auto site_in_tile = [&](int v) -> int {   // v: position in the walk
+        if (v >= g.ntiles) return -1;
         int tx, ty, tz, tt;
-        tile_of_block(g, b, tx, ty, tz, tt);
+        tile_of_block(g, g.rev ? g.ntiles - 1 - v : v, tx, ty, tz, tt);
         const int x = tx * BX + lx, y = ty * BY + ly, z = tz * BZ + lz, t = tt * BT + lt;
         if (x >= g.L[0] || y >= g.L[1] || z >= g.L[2] || t >= g.L[3]) return -1;
         return x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
@@ -808,11 +811,12 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     // Persistent CTAs: the grid is one resident wave; CTA i takes tiles i, i + gridDim.x, ... so that at any
     // moment the chip works on gridDim.x consecutive tiles of the rasterisation (L2 locality) and the
     // reduction epilogue (barriers, fence, ticket) is paid once per CTA, not once per tile.
-    for (int b = blockIdx.x; b < g.ntiles; b += gridDim.x) {
+    for (int v = blockIdx.x; v < g.ntiles; v += gridDim.x) {
+        const int b = g.rev ? g.ntiles - 1 - v : v;   // position v of the walk -> tile of the rasterisation
         int tx, ty, tz, tt;
-        if (BX % SB == 0 && g.pf > 0 && (lx % SB) == 0 && b + g.pf < g.ntiles) {
+        if (BX % SB == 0 && g.pf > 0 && (lx % SB) == 0 && v + g.pf < g.ntiles) {
             // one thread per 16-site run of the tile `pf` tiles ahead: its spinor block, its gauge block (and r)
-            tile_of_block(g, b + g.pf, tx, ty, tz, tt);
+            tile_of_block(g, g.rev ? b - g.pf : b + g.pf, tx, ty, tz, tt);
             const int px = tx * BX + lx, py = ty * BY + ly, pz = tz * BZ + lz, pt = tt * BT + lt;
             if (px < g.L[0] && py < g.L[1] && pz < g.L[2] && pt < g.L[3]) {
                 const int ps = px + g.L[0] * (py + g.L[1] * (pz + g.L[2] * pt));
@@ -827,7 +831,7 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
         const bool active = (x < g.L[0]) && (y < g.L[1]) && (z < g.L[2]) && (t < g.L[3]);
         int next_s = -1;
         if (PIPE == 3) {
-            next_s = site_in_tile(b + gridDim.x);
+            next_s = site_in_tile(v + gridDim.x);
             cp_async_wait_all();                       // this thread's own copies for tile b have landed
             if (!active && next_s >= 0) stage_links<NT>(U, next_s, wd_dyn_smem, tid);
         }
@@ -1107,12 +1111,13 @@ cg_init_kernel(const typename Field<real>::svec *__restrict__ eta, typename Fiel
 template <typename real>
 __global__ void __launch_bounds__(VEC_NT)
 cg_update_kernel(typename Field<real>::svec *y, typename Field<real>::svec *p,
-                 const typename Field<real>::svec *__restrict__ r, size_t n, const CgScalars *sc, int it)
+                 const typename Field<real>::svec *__restrict__ r, size_t n, const CgScalars *sc, int it, int rev)
 {
     using svec = typename Field<real>::svec;
     if (it >= sc->k_stop) return;
     const real alpha = (real)sc->alpha, beta = (real)sc->beta;
-    for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT) {
+    for (size_t j = (size_t)blockIdx.x * VEC_NT + threadIdx.x; j < n; j += (size_t)gridDim.x * VEC_NT) {
+        const size_t i = rev ? n - 1 - j : j;   // rev: from the end of the buffers to their start (Geom.rev)
         const svec pv = p[i];
         const svec rv = __ldg(r + i);
         y[i] = vaxpy(alpha, pv, y[i]);

@@ -110,6 +110,7 @@ def load_library(path: str = LIB_PATH):
     lib.wd_get_gauge_recon.argtypes = [vp]
     lib.wd_set_waves.argtypes = [vp, ci]
     lib.wd_set_zchunk.argtypes = [vp, ci]
+    lib.wd_set_sweep.argtypes = [vp, ci]
     lib.wd_set_poll_interval.argtypes = [vp, ci]
     lib.wd_set_profile.argtypes = [vp, ci]
     lib.wd_get_profile.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_long)]
@@ -448,6 +449,10 @@ class WilsonContext:
 
     def wd_set_zchunk(self, layers):
         self._check(self.lib.wd_set_zchunk(self._ctx, int(layers)))
+
+    def wd_set_sweep(self, alternate):
+        """1: consecutive passes walk the lattice in alternating directions (L2 reuse); 0 (default): all forward"""
+        self._check(self.lib.wd_set_sweep(self._ctx, int(alternate)))
 
     def wd_set_poll_interval(self, n):
         self._check(self.lib.wd_set_poll_interval(self._ctx, int(n)))

@@ -274,6 +274,30 @@ def test_cg_result_independent_of_poll_interval_and_repeatable(wilson):
     assert all(o == outs[0] for o in outs)
 
 
+@pytest.mark.parametrize("cfg_index,precision", [(1, 32), (2, 64)])
+def test_alternating_sweep_direction(wilson, cfg_index, precision):
+    """wd_set_sweep(1): passes walk the tiles backwards and forwards in turn.  Per-site arithmetic is unchanged, so
+    wd_apply is bit-identical; in cg_solve only the grouping of the fp64 reduction partials differs."""
+    cfg = inputs.CONFIGS[cfg_index]
+    U, eta = gu.config_fields(cfg_index, precision)
+    res = {}
+    for sweep in (0, 1):
+        with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+            ctx.wd_set_sweep(sweep)
+            ctx.wd_set_cg_mode(1)
+            Un = ctx.wd_pack_gauge(gu.to_device(U))
+            en = ctx.wd_pack_spinor(gu.to_device(eta))
+            applied = [gu.to_host(ctx.wd_unpack_spinor(ctx.wd_apply(Un, en, cfg.kappa, dag))) for dag in (0, 1, 0, 1)]
+            psi_n, info = ctx.cg_solve(Un, en, cfg.kappa, cfg.r_min, cfg.max_iter)
+            res[sweep] = (applied, gu.to_host(ctx.wd_unpack_spinor(psi_n)), info)
+    for a, b in zip(res[0][0], res[1][0]):
+        assert a.tobytes() == b.tobytes()
+    assert np.array_equal(res[1][0][0], res[1][0][2]) and np.array_equal(res[1][0][1], res[1][0][3])
+    assert res[0][2]["iterations"] == res[1][2]["iterations"]
+    tol = 1e-5 if precision == 32 else 1e-12
+    assert np.linalg.norm(res[0][1] - res[1][1]) <= tol * np.linalg.norm(res[0][1])
+
+
 @pytest.mark.parametrize("mode", [1, 2])
 def test_cg_edge_cases(wilson, oracle, mode):
     cfg = inputs.CONFIGS[0]
