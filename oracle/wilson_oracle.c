@@ -26,7 +26,8 @@
  * from Kronecker blocks (P1), gamma5-hermiticity (P2), free-field plane-wave eigenvalue (P3),
  * gauge covariance (P4), per-direction unitarity (P5), CG vs dense LU solve + monotone error
  * (P6), finite termination in the free field (P7), closed-form inverse incl. point source by
- * FFT (P8), residual identity (P10), COO route with N_NZ = 588 V (P11).
+ * FFT (P8), residual identity (P10), COO route with N_NZ = 588 V (P11); BiCGSTAB (B-P1..4), even-odd CG (E-P1..4),
+ * even-odd BiCGSTAB (EB-P1..3): dense solves and dense-matrix retyping of the first iterates on 2^4.
  * Iteration counts of the five BASELINE configs: parity unpinned by the paper (it prints none).
  *
  * Canonical layouts (x fastest): site s = x + Lx (y + Ly (z + Lz t));
@@ -493,6 +494,109 @@ int oracle_cg_solve_eo(const int L[4], int bc_t, const double *U_, const double 
     }
     free(eo); free(y); free(r); free(p); free(q); free(w); free(tmp);
     return converged ? 0 : 1;
+}
+
+/*
+ * Even-odd preconditioned BiCGSTAB: the two SURVEY.md 8(f) rows composed (reading EB1 of DESIGN.md).  The Schur system
+ * Mhat psi_e = etahat of reading E1 (above) is solved with the BiCGSTAB listing of reading B1 (oracle_bicgstab_solve)
+ * applied to Mhat itself, shadow residual rhat = r0 = etahat, psi_e0 = 0; then psi_o = eta_o + kappa H_oe psi_e.
+ * Stopping test as in oracle_cg_solve_eo: sqrt(<r,r>) < r_min sqrt(<eta,eta>) with the FULL source, r = etahat - Mhat psi_e
+ * (the even rows of eta - D psi; the odd rows vanish identically), tested at the top of the loop.
+ * Full-lattice arrays, even-supported fields, as in oracle_cg_solve_eo.
+ * Pins (tests/test_oracle_pins.py): dense LU solve of the full system (EB-P1), first iterates retyped with the dense
+ * Schur complement (EB-P2), kappa = 0 and agreement with the three other oracle solvers on the BASELINE configs (EB-P3).
+ * Returns 0 converged, 1 max_iter reached, 2 breakdown, <0 bad argument / out of memory.
+ */
+int oracle_bicgstab_solve_eo(const int L[4], int bc_t, const double *U_, const double *eta_, double *psi_out,
+                             double kappa, double r_min, int max_iter, oracle_cg_info *info, double *rr_history)
+{
+    if (!L || !U_ || !eta_ || !psi_out || max_iter < 0 || !(r_min > 0.0)) return -1;
+    for (int d = 0; d < 4; ++d)
+        if (L[d] < 2 || (L[d] & 1)) return -2;
+    const long V = volume_of(L), n = V * 12;
+    const cplx *U = (const cplx *)U_, *eta = (const cplx *)eta_;
+    cplx *psi = (cplx *)psi_out;
+    cplx *eo = calloc((size_t)n, sizeof(cplx));   /* eta_o, odd-supported */
+    cplx *x = calloc((size_t)n, sizeof(cplx));    /* psi_e */
+    cplx *rhat = calloc((size_t)n, sizeof(cplx)); /* etahat */
+    cplx *r = malloc((size_t)n * sizeof(cplx));
+    cplx *p = malloc((size_t)n * sizeof(cplx));
+    cplx *v = malloc((size_t)n * sizeof(cplx));
+    cplx *s = malloc((size_t)n * sizeof(cplx));
+    cplx *t = malloc((size_t)n * sizeof(cplx));
+    cplx *tmp = malloc((size_t)n * sizeof(cplx));
+    if (!eo || !x || !rhat || !r || !p || !v || !s || !t || !tmp) {
+        free(eo); free(x); free(rhat); free(r); free(p); free(v); free(s); free(t); free(tmp);
+        return -4;
+    }
+#ifdef _OPENMP
+    double t0 = omp_get_wtime();
+#endif
+    const double eta2 = norm2(eta, n);
+    /* etahat = eta_e + kappa H_eo eta_o */
+    for (long i = 0; i < V; ++i)
+        if (parity_of(L, i) == 1) memcpy(eo + i * 12, eta + i * 12, 12 * sizeof(cplx));
+    hop_apply(L, bc_t, U, eo, tmp, 0);
+    for (long i = 0; i < V; ++i)
+        if (parity_of(L, i) == 0)
+            for (int j = 0; j < 12; ++j) rhat[i * 12 + j] = eta[i * 12 + j] + kappa * tmp[i * 12 + j];
+    memcpy(r, rhat, (size_t)n * sizeof(cplx));
+    memcpy(p, rhat, (size_t)n * sizeof(cplx));
+    double rr = norm2(r, n);
+    cplx rho = rr;
+    int k = 0, breakdown = 0;
+    if (rr_history) rr_history[0] = rr;
+    if (eta2 > 0.0) {
+        while (sqrt(rr) >= r_min * sqrt(eta2) && k < max_iter) {
+            schur_apply(L, bc_t, U, p, v, tmp, kappa, 0); /* v = Mhat p */
+            const cplx rv = cdot(rhat, v, n);
+            if (rv == 0.0 || rho == 0.0) { breakdown = 1; break; }
+            const cplx alpha = rho / rv;
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; ++i) s[i] = r[i] - alpha * v[i];
+            schur_apply(L, bc_t, U, s, t, tmp, kappa, 0); /* t = Mhat s */
+            const double tt = norm2(t, n);
+            if (tt == 0.0) { /* s = 0: psi_e + alpha p is exact */
+#pragma omp parallel for schedule(static)
+                for (long i = 0; i < n; ++i) x[i] += alpha * p[i];
+                rr = 0.0;
+                ++k;
+                if (rr_history) rr_history[k] = rr;
+                break;
+            }
+            const cplx omega = cdot(t, s, n) / tt;
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; ++i) x[i] += alpha * p[i] + omega * s[i];
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; ++i) r[i] = s[i] - omega * t[i];
+            const cplx rho_new = cdot(rhat, r, n);
+            rr = norm2(r, n);
+            ++k;
+            if (rr_history) rr_history[k] = rr;
+            if (omega == 0.0 || !isfinite(creal(omega)) || !isfinite(cimag(omega))) { breakdown = 1; break; }
+            const cplx beta = (rho_new / rho) * (alpha / omega);
+#pragma omp parallel for schedule(static)
+            for (long i = 0; i < n; ++i) p[i] = r[i] + beta * (p[i] - omega * v[i]);
+            rho = rho_new;
+        }
+    }
+    hop_apply(L, bc_t, U, x, tmp, 0); /* H_oe psi_e, odd-supported */
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < n; ++i) psi[i] = x[i] + eo[i] + kappa * tmp[i];
+    const int converged = (eta2 == 0.0) || (sqrt(rr) < r_min * sqrt(eta2));
+    if (info) {
+        info->iterations = k;
+        info->converged = converged;
+        info->rel_residual = eta2 > 0.0 ? sqrt(rr / eta2) : 0.0;
+        info->eta_norm2 = eta2;
+#ifdef _OPENMP
+        info->seconds = omp_get_wtime() - t0;
+#else
+        info->seconds = 0.0;
+#endif
+    }
+    free(eo); free(x); free(rhat); free(r); free(p); free(v); free(s); free(t); free(tmp);
+    return converged ? 0 : (breakdown ? 2 : 1);
 }
 
 /*

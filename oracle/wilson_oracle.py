@@ -70,6 +70,8 @@ def _load():
         lib.oracle_coo_spmv.restype = ctypes.c_int
         lib.oracle_cg_solve_eo.argtypes = lib.oracle_cg_solve.argtypes
         lib.oracle_cg_solve_eo.restype = ctypes.c_int
+        lib.oracle_bicgstab_solve_eo.argtypes = lib.oracle_cg_solve.argtypes
+        lib.oracle_bicgstab_solve_eo.restype = ctypes.c_int
         lib.oracle_schur_apply.argtypes = lib.oracle_wd_apply.argtypes
         lib.oracle_schur_apply.restype = ctypes.c_int
         lib.oracle_norm2.argtypes = [dp, ctypes.c_long]
@@ -207,6 +209,33 @@ def cg_solve_eo(dims, U, eta, kappa, r_min, max_iter, bc_t=-1, history=False):
         ctypes.byref(info), _ptr(hist) if history else None)
     if rc < 0:
         raise RuntimeError(f"oracle_cg_solve_eo failed: {rc}")
+    out = {
+        "iterations": info.iterations,
+        "converged": bool(info.converged),
+        "rel_residual": info.rel_residual,
+        "eta_norm2": info.eta_norm2,
+        "seconds": info.seconds,
+        "status": rc,
+    }
+    if history:
+        out["rr_history"] = hist[: info.iterations + 1].copy()
+    return psi, out
+
+
+def bicgstab_solve_eo(dims, U, eta, kappa, r_min, max_iter, bc_t=-1, history=False):
+    """Even-odd preconditioned BiCGSTAB (readings E1 + B1 composed = EB1): the BiCGSTAB listing on Mhat, then
+    psi_o = eta_o + kappa H_oe psi_e.  Returns (psi, info) like cg_solve; status 2 = breakdown."""
+    d, vol = _dims(dims)
+    U = _c128(U, (vol, 4, 3, 3))
+    eta = _c128(eta, (vol, 4, 3))
+    psi = np.empty_like(eta)
+    info = OracleCgInfo()
+    hist = np.zeros(max_iter + 1, dtype=np.float64) if history else None
+    rc = _load().oracle_bicgstab_solve_eo(
+        d, int(bc_t), _ptr(U), _ptr(eta), _ptr(psi), float(kappa), float(r_min), int(max_iter),
+        ctypes.byref(info), _ptr(hist) if history else None)
+    if rc < 0:
+        raise RuntimeError(f"oracle_bicgstab_solve_eo failed: {rc}")
     out = {
         "iterations": info.iterations,
         "converged": bool(info.converged),

@@ -622,3 +622,97 @@ def test_ep4_eo_cg_baseline_configs_and_edge_cases(oracle):
     assert iz["iterations"] == 0 and iz["status"] == 1 and not z[par == 0].any() and np.array_equal(z[par == 1], eta[par == 1])
     with pytest.raises(RuntimeError):
         oracle.cg_solve_eo((4, 3, 4, 4), U[:192], eta[:192], 0.1, 1e-6, 10)   # odd extent
+
+
+# ---------------------------------------------------------------- even-odd preconditioned BiCGSTAB (readings E1 + B1 = EB1)
+@pytest.mark.parametrize("bc_t", [-1, +1])
+def test_ebp1_eo_bicgstab_matches_dense_solve(oracle, bc_t):
+    dims = (4, 2, 2, 4)
+    kappa = 0.12
+    U = inputs.gauge_field(CFG_TEST + 50, dims, "haar")
+    eta = inputs.source_field(CFG_TEST + 50, dims)
+    M, e, o = _dense_blocks(dims, U, kappa, bc_t)
+    exact = np.linalg.solve(M, eta.reshape(-1)).reshape(eta.shape)
+    psi, info = oracle.bicgstab_solve_eo(dims, U, eta, kappa, 1e-12, 500, bc_t, history=True)
+    assert info["converged"] and info["status"] == 0
+    assert np.linalg.norm(psi - exact) < 1e-10 * np.linalg.norm(exact)
+    # the recursed residual is the true residual of the FULL system, whose odd rows vanish identically
+    assert abs(oracle.true_residual(dims, U, eta, psi, kappa, bc_t) - info["rel_residual"]) < 1e-12
+    r_full = (eta - oracle.wd_apply(dims, U, psi, kappa, False, bc_t)).reshape(-1, 12)
+    assert np.max(np.abs(r_full[_parity(dims) == 1])) < 1e-13
+    etahat = eta.reshape(-1)[e] - M[np.ix_(e, o)] @ eta.reshape(-1)[o]
+    assert info["rr_history"][0] == pytest.approx(np.vdot(etahat, etahat).real, rel=1e-13)
+    assert info["eta_norm2"] == pytest.approx(np.vdot(eta, eta).real, rel=1e-13)
+
+
+def test_ebp2_eo_bicgstab_first_iterates_from_dense_schur_complement(oracle):
+    """The listing of reading B1 retyped on the dense Schur complement of the Kronecker-built matrix, followed by the
+    odd-site reconstruction from the dense off-diagonal block: pins that the iteration runs on Mhat (not Mhat-dagger,
+    not D), the shadow residual etahat, the complex scalars and psi_o."""
+    dims = (2, 2, 2, 2)
+    kappa = 0.11
+    U = inputs.gauge_field(CFG_TEST + 51, dims, "haar")
+    eta = inputs.source_field(CFG_TEST + 51, dims)
+    M, e, o = _dense_blocks(dims, U, kappa, -1)
+    S = M[np.ix_(e, e)] - M[np.ix_(e, o)] @ M[np.ix_(o, e)]
+    b = eta.reshape(-1)
+    etahat = b[e] - M[np.ix_(e, o)] @ b[o]
+    x = np.zeros_like(etahat)
+    r = etahat.copy()
+    rhat = etahat.copy()
+    p = r.copy()
+    rho = np.vdot(rhat, r)
+    for k in range(1, 4):
+        v = S @ p
+        alpha = rho / np.vdot(rhat, v)
+        s = r - alpha * v
+        t = S @ s
+        omega = np.vdot(t, s) / np.vdot(t, t)
+        x = x + alpha * p + omega * s
+        r = s - omega * t
+        rho_new = np.vdot(rhat, r)
+        beta = (rho_new / rho) * (alpha / omega)
+        p = r + beta * (p - omega * v)
+        rho = rho_new
+        want = np.zeros_like(b)
+        want[e] = x
+        want[o] = b[o] - M[np.ix_(o, e)] @ x
+        psi, info = oracle.bicgstab_solve_eo(dims, U, eta, kappa, 1e-30, k, -1, history=True)
+        assert info["iterations"] == k and info["status"] == 1
+        assert np.linalg.norm(psi.reshape(-1) - want) < 1e-12 * np.linalg.norm(want)
+        assert info["rr_history"][k] == pytest.approx(np.vdot(r, r).real, rel=1e-9)
+    assert abs(alpha.imag) > 1e-6 * abs(alpha) or abs(omega.imag) > 1e-6 * abs(omega)
+    # Mhat is not normal here, so a solver on Mhat-dagger would give different iterates
+    assert np.linalg.norm(S @ S.conj().T - S.conj().T @ S) > 1e-6
+
+
+def test_ebp3_eo_bicgstab_special_cases_and_other_solvers(oracle):
+    # kappa = 0: Mhat = 1, one iteration, psi = eta
+    dims = (4, 6, 4, 8)
+    Uh = inputs.gauge_field(CFG_TEST + 52, dims, "haar")
+    src = inputs.source_field(CFG_TEST + 52, dims)
+    psi, info = oracle.bicgstab_solve_eo(dims, Uh, src, 0.0, 1e-12, 10)
+    assert info["iterations"] == 1 and info["converged"] and np.max(np.abs(psi - src)) < 1e-14
+    # free field, Gaussian source: exact solution mode by mode with the closed-form D(p)^-1 (pin P8)
+    kappa = 0.12
+    exact = lm.free_solve(dims, kappa, src, -1)
+    psi, info = oracle.bicgstab_solve_eo(dims, unit_gauge(dims), src, kappa, 1e-12, 2000, -1)
+    assert info["converged"] and np.linalg.norm(psi - exact) < 1e-9 * np.linalg.norm(exact)
+    # BASELINE configs 0, 1: same solution as the plain CG, fewer iterations than the plain BiCGSTAB and the even-odd CG
+    for ci in (0, 1):
+        cfg = inputs.CONFIGS[ci]
+        U, eta = inputs.config_inputs(cfg)
+        pe, ie = oracle.bicgstab_solve_eo(cfg.dims, U, eta, cfg.kappa, 1e-10, cfg.max_iter, cfg.bc_t)
+        pb, ib = oracle.bicgstab_solve(cfg.dims, U, eta, cfg.kappa, 1e-10, cfg.max_iter, cfg.bc_t)
+        pc, ic = oracle.cg_solve_eo(cfg.dims, U, eta, cfg.kappa, 1e-10, cfg.max_iter, cfg.bc_t)
+        pp, ip = oracle.cg_solve(cfg.dims, U, eta, cfg.kappa, 1e-10, cfg.max_iter, cfg.bc_t)
+        assert ie["converged"] and ie["iterations"] < ib["iterations"] and ie["iterations"] < ic["iterations"]
+        assert np.linalg.norm(pe - pp) < 1e-8 * np.linalg.norm(pp)
+        assert oracle.true_residual(cfg.dims, U, eta, pe, cfg.kappa, cfg.bc_t) < 1e-10
+    z, iz = oracle.bicgstab_solve_eo(cfg.dims, U, np.zeros_like(eta), cfg.kappa, 1e-6, 10)
+    assert iz["iterations"] == 0 and iz["converged"] and not z.any()
+    z, iz = oracle.bicgstab_solve_eo(cfg.dims, U, eta, cfg.kappa, 1e-6, 0)
+    par = _parity(cfg.dims)
+    assert iz["iterations"] == 0 and iz["status"] == 1 and not z[par == 0].any() and np.array_equal(z[par == 1], eta[par == 1])
+    with pytest.raises(RuntimeError):
+        oracle.bicgstab_solve_eo((4, 3, 4, 4), U[:192], eta[:192], 0.1, 1e-6, 10)   # odd extent
