@@ -375,6 +375,32 @@ def run_rows(args):
                         "iteration_gbs": sum(hb) * V / (sum(kus) * 1e-6) / 1e9 if sum(kus) > 0 else None,
                         "iteration_frac_of_measured": sum(hb) * V / (sum(kus) * 1e-6) / 1e9 / peak if sum(kus) > 0 else None,
                         "cg_solve_ms_same_problem": t, "speedup_vs_cg": t / te}), flush=True)
+                    # f3 x f4: BiCGSTAB on the Schur operator (even-odd preconditioned BiCGSTAB)
+                    for _ in range(2):
+                        ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, r_min, cfg.max_iter, out=pe)
+                    ctx.wd_set_poll_interval(1)     # one sampled iteration per poll chunk: sample them all
+                    ctx.wd_set_profile(True)
+                    for _ in range(3):
+                        ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, r_min, cfg.max_iter, out=pe)
+                    pb = ctx.wd_get_profile_eo_bicgstab()
+                    ctx.wd_set_profile(False)
+                    ctx.wd_set_poll_interval(0)
+                    ms = []
+                    for _ in range(5):
+                        _, ieb = ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, r_min, cfg.max_iter, out=pe)
+                        ms.append(ieb["gpu_ms"])
+                    kus = [m / max(pb["iterations"], 1) * 1e3 for m in pb["ms"]]
+                    hb = (sb + gb, 2 * sb + gb, 3 * sb // 2, sb + gb, 3 * sb // 2 + gb, 7 * sb // 2, 2 * sb)
+                    teb = float(np.median(ms))
+                    names = ("H_oe_p", "M_rv", "s", "H_oe_s", "M_ts", "xr", "p")
+                    print(json.dumps({
+                        "row": "f3xf4 even-odd bicgstab", "config": ci, "precision": prec, "iterations": ieb["iterations"],
+                        "status": ieb["status"], "rel_residual": ieb["rel_residual"], "solve_ms": teb,
+                        "kernel_us": dict(zip(names, kus)), "bytes_per_full_site": dict(zip(names, hb)),
+                        "kernel_gbs": dict(zip(names, [b * V / (u * 1e-6) / 1e9 if u > 0 else None for b, u in zip(hb, kus)])),
+                        "iteration_gbs": sum(hb) * V / (sum(kus) * 1e-6) / 1e9 if sum(kus) > 0 else None,
+                        "iteration_frac_of_measured": sum(hb) * V / (sum(kus) * 1e-6) / 1e9 / peak if sum(kus) > 0 else None,
+                        "cg_solve_ms_same_problem": t, "speedup_vs_cg": t / teb}), flush=True)
                     del Ue, ee, pe
     # f2: the paper's COO SpMV at its largest volume
     cfg = inputs.CONFIGS[2]

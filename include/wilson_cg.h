@@ -199,6 +199,12 @@ int bicgstab_solve(wd_ctx *ctx, const void *U_native, const void *eta_native, vo
  *       dagger != 0) on the sites of parity out_parity, read from the other half of in_eo; the other half of out_eo is
  *       not touched.  No kappa, no diagonal term.  Asynchronous.
  *   cg_solve_eo   arguments as cg_solve with eo-native buffers; info->cg_mode = 4.  Synchronous.
+ *   bicgstab_solve_eo   the BiCGSTAB recurrence of bicgstab_solve (reading B1) applied to Mhat itself (readings E1 + B1
+ *       composed; the two SURVEY.md 8(f) rows together): shadow residual rhat = etahat, psi_e0 = 0, the same loop test as
+ *       cg_solve_eo, then psi_o = eta_o + kappa H_oe psi_e.  Per iteration: two plain half-lattice hops to the odd sites,
+ *       the two hops back fused with the diagonal term and the dot products of the BiCGSTAB passes (<rhat,v>; <t,s>,
+ *       <t,t>), three half-length vector kernels.  Arguments as cg_solve_eo; returns WD_OK, WD_NOT_CONVERGED,
+ *       WD_BREAKDOWN or an error; info->cg_mode = 5.  Synchronous.
  * Errors: WD_ERR_DIMS for an odd extent, WD_ERR_ARG (NULL, aliasing, 12-real links selected), WD_ERR_CUDA, WD_ERR_ALLOC.
  */
 size_t wd_eo_spinor_bytes(wd_ctx *ctx);
@@ -209,6 +215,8 @@ int wd_eo_pack_gauge(wd_ctx *ctx, const void *U_canonical_dev, void *U_eo_dev);
 int wd_eo_hop(wd_ctx *ctx, const void *U_eo, const void *in_eo, void *out_eo, int out_parity, int dagger);
 int cg_solve_eo(wd_ctx *ctx, const void *U_eo, const void *eta_eo, void *psi_eo_out,
                 double kappa, double r_min, int max_iter, wd_cg_info *info);
+int bicgstab_solve_eo(wd_ctx *ctx, const void *U_eo, const void *eta_eo, void *psi_eo_out,
+                      double kappa, double r_min, int max_iter, wd_cg_info *info);
 
 /*
  * Several right-hand sides at once (the gauge field is 60 % of the bytes of a stencil pass and is the
@@ -331,6 +339,9 @@ int wd_get_profile(wd_ctx *ctx, double ms[3], long *iterations);
  * After cg_solve_eo the same call returns its five kernels (H-dagger_oe p; Mhat-dagger tail + |q|^2; H_oe q; Mhat tail
  * + r update + |r|^2; axpy-xpay). */
 int wd_get_profile_bicgstab(wd_ctx *ctx, double ms[5], long *iterations);
+/* After bicgstab_solve_eo: ms[0..6] = its seven kernels (H_oe p; Mhat tail + <rhat,v>; s update; H_oe s; Mhat tail +
+ * <t,s>, <t,t>; psi/r update + dots; p update) over *iters sampled iterations. */
+int wd_get_profile_eo_bicgstab(wd_ctx *ctx, double ms[7], long *iterations);
 
 /* Host-only self-test of the fast-division constants of the CTA tile decode: returns the number of n in
  * [0, n_max) with a wrong quotient n / d (0 = correct), or -1 for d = 0.  Needs no GPU. */

@@ -159,7 +159,7 @@ extern "C" int wd_destroy(wd_ctx *c)
 {
     if (!c) return WD_OK;
     cudaStreamSynchronize(c->stream);
-    void *dev[] = {c->r, c->p, c->q, c->y, c->w5, c->w6, c->eo_n2, c->m_ws[0], c->m_ws[1], c->m_ws[2], c->m_ws[3], c->m_sc,
+    void *dev[] = {c->r, c->p, c->q, c->y, c->w5, c->w6, c->w7, c->eo_n2, c->m_ws[0], c->m_ws[1], c->m_ws[2], c->m_ws[3], c->m_sc,
                    c->m_counter, c->m_hist, c->sc, c->partials, c->counter, c->hist, c->result_dev,
                    c->U_can, c->U_nat, c->s_can, c->s_nat_in, c->s_nat_out};
     for (void *ptr : dev)
@@ -170,7 +170,7 @@ extern "C" int wd_destroy(wd_ctx *c)
     for (int i = 0; i < 4; ++i)
         if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     for (int i = 0; i < 4 * c->pev_cap; ++i) cudaEventDestroy(c->pev[i]);
-    for (int i = 0; i < 6; ++i)
+    for (int i = 0; i < 8; ++i)
         if (c->bev[i]) cudaEventDestroy(c->bev[i]);
     free(c->pev);
     free(c);
@@ -267,7 +267,7 @@ extern "C" int wd_set_profile(wd_ctx *c, int on)
     c->profile = on ? 1 : 0;
     c->prof_ms[0] = c->prof_ms[1] = c->prof_ms[2] = 0.0;
     c->prof_n = 0;
-    for (int j = 0; j < 5; ++j) c->bprof_ms[j] = 0.0;
+    for (int j = 0; j < 7; ++j) c->bprof_ms[j] = 0.0;
     c->bprof_n = 0;
     return WD_OK;
 }
@@ -636,7 +636,7 @@ extern "C" int bicgstab_solve(wd_ctx *c, const void *U, const void *eta, void *p
         CUDA_TRY(c, cudaMemsetAsync(c->w5, 0, spinor_bytes(c), c->stream));
     }
     if (c->profile && !c->bev[0])
-        for (int j = 0; j < 6; ++j) CUDA_TRY(c, cudaEventCreate(&c->bev[j]));
+        for (int j = 0; j < 8; ++j) CUDA_TRY(c, cudaEventCreate(&c->bev[j]));
     c->launches = 0;
     CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
     rc = c->precision == 32 ? bicgstab_loop<float>(c, U, eta, psi, kappa, r_min, max_iter)
@@ -666,6 +666,14 @@ extern "C" int wd_get_profile_bicgstab(wd_ctx *c, double ms[5], long *iterations
 {
     if (!c || !ms || !iterations) return WD_ERR_ARG;
     for (int j = 0; j < 5; ++j) ms[j] = c->bprof_ms[j];
+    *iterations = c->bprof_n;
+    return WD_OK;
+}
+
+extern "C" int wd_get_profile_eo_bicgstab(wd_ctx *c, double ms[7], long *iterations)
+{
+    if (!c || !ms || !iterations) return WD_ERR_ARG;
+    for (int j = 0; j < 7; ++j) ms[j] = c->bprof_ms[j];
     *iterations = c->bprof_n;
     return WD_OK;
 }

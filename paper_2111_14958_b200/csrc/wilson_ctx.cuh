@@ -31,6 +31,7 @@ struct wd_ctx {
     void *r, *p, *q, *y;
     void *w5;             // fifth work vector (BiCGSTAB: t; even-odd: the odd-parity intermediate)
     void *w6;             // even-odd: etahat (half length)
+    void *w7;             // even-odd BiCGSTAB: t = Mhat s (half length)
     double *eo_n2;        // even-odd: <eta_e,eta_e>, <eta_o,eta_o> (device)
     // multi-right-hand-side CG: r, p, q, y for a group of up to 4 sources, per-source scalars, counters, histories
     void *m_ws[4];
@@ -59,8 +60,9 @@ struct wd_ctx {
     int pev_cap;            // iterations the pool covers
     double prof_ms[3];      // accumulated device time of a2, a3, a4
     long prof_n;            // iterations accumulated
-    cudaEvent_t bev[6];     // BiCGSTAB: events around the five kernels of the first iteration of every poll chunk
-    double bprof_ms[5];
+    cudaEvent_t bev[8];     // BiCGSTAB / even-odd solvers: events around the 5 (7: even-odd BiCGSTAB) kernels of the first
+                            // iteration of every poll chunk
+    double bprof_ms[7];
     long bprof_n;
     int last_iters;
     int launches;

@@ -130,6 +130,8 @@ cudaError_t eo_launch(wd_ctx *c, const void *U_eo, const EoPass &p)
     a.sc = (p.mode != MODE_PLAIN || p.in_loop) ? c->sc : nullptr;
     a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = p.it;
     c->launches++;
+    if (p.mode == MODE_RV || p.mode == MODE_TS)
+        return c->precision == 32 ? launch_dslash_eo_bi_f32(tile, p.mode, a) : launch_dslash_eo_bi_f64(tile, p.mode, a);
     return c->precision == 32 ? launch_dslash_eo_f32(tile, p.dagger, p.mode, a) : launch_dslash_eo_f64(tile, p.dagger, p.mode, a);
 }
 
@@ -299,10 +301,13 @@ extern "C" int cg_solve_eo(wd_ctx *c, const void *U_eo, const void *eta_eo, void
         CUDA_TRY(c, cudaMalloc(&c->w5, spinor_bytes(c)));
         CUDA_TRY(c, cudaMemsetAsync(c->w5, 0, spinor_bytes(c), c->stream));
     }
-    if (!c->w6) CUDA_TRY(c, cudaMalloc(&c->w6, half_spinor_bytes(c)));
+    if (!c->w6) {
+        CUDA_TRY(c, cudaMalloc(&c->w6, half_spinor_bytes(c)));
+        CUDA_TRY(c, cudaMemsetAsync(c->w6, 0, half_spinor_bytes(c), c->stream));   // pad lanes stay zero
+    }
     if (!c->eo_n2) CUDA_TRY(c, cudaMalloc(&c->eo_n2, 2 * sizeof(double)));
     if (c->profile && !c->bev[0])
-        for (int j = 0; j < 6; ++j) CUDA_TRY(c, cudaEventCreate(&c->bev[j]));
+        for (int j = 0; j < 8; ++j) CUDA_TRY(c, cudaEventCreate(&c->bev[j]));
     c->launches = 0;
     CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
     rc = c->precision == 32 ? eo_loop<float>(c, U_eo, eta_eo, psi_eo, kappa, r_min, max_iter)
@@ -326,4 +331,140 @@ extern "C" int cg_solve_eo(wd_ctx *c, const void *U_eo, const void *eta_eo, void
         info->cg_mode = 4;
     }
     return s.converged ? WD_OK : WD_NOT_CONVERGED;
+}
+
+// ---------------------------------------------------------------- even-odd preconditioned BiCGSTAB (readings E1 + B1)
+// The BiCGSTAB recurrence of bicgstab_solve (wilson_cg.cu) on the Schur operator Mhat = 1 - kappa^2 H_eo H_oe over
+// half-length vectors.  Every Mhat application is two launches of the one-parity stencil: a plain hop to the odd sites
+// and the hop back fused with the diagonal term and the dot products of the BiCGSTAB pass (MODE_RV / MODE_TS, EO = 1).
+template <typename real>
+static int eo_bicgstab_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, void *psi_eo, double kappa, double r_min,
+                            int max_iter)
+{
+    using svec = typename Field<real>::svec;
+    const EoDims e = eo_dims(c);
+    const size_t hs = half_spinor_bytes(c), n = half_spinor_vecs(c);
+    const int pad = e.Vh_pad != (size_t)e.Vh;
+    const char *eta_e = (const char *)eta_eo, *eta_o = eta_e + hs;
+    char *psi_e = (char *)psi_eo, *psi_o = psi_e + hs;
+    svec *r = (svec *)c->r, *p = (svec *)c->p, *v = (svec *)c->q, *s = (svec *)c->y;
+    void *to = c->w5;                                 // odd-parity intermediate H_oe (.)
+    svec *t = (svec *)c->w7;                          // t = Mhat s
+    const svec *etah = (const svec *)c->w6;           // etahat = shadow residual rhat
+    const double k2 = kappa * kappa;
+    const size_t need = (n + VEC_NT - 1) / VEC_NT, cap = (size_t)c->sm_count * 16;
+    const unsigned int vgrid = (unsigned int)(need < cap ? (need ? need : 1) : cap);
+
+    norm2_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((const svec *)eta_e, n, e.Vh, pad, c->partials, c->counter, c->eo_n2);
+    norm2_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((const svec *)eta_o, n, e.Vh, pad, c->partials, c->counter, c->eo_n2 + 1);
+    c->launches += 2;
+    CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_PLAIN, 0, eta_o, eta_e, c->w6, nullptr, -kappa, 0, false}));
+    // psi_e <- 0, r <- etahat, p <- etahat, rho = rr = <etahat,etahat>; then the loop test against the FULL source norm
+    bi_init_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(etah, (svec *)psi_e, r, p, n, e.Vh, pad, c->sc, c->partials,
+                                                         c->counter, c->hist, r_min, max_iter);
+    eo_set_eta2_kernel<<<1, 1, 0, c->stream>>>(c->sc, c->eo_n2, r_min, max_iter);
+    c->launches += 2;
+    CUDA_TRY(c, cudaGetLastError());
+
+    const int poll = c->poll > 0 ? c->poll : 4;
+    int launched = 0;
+    while (launched < max_iter) {
+        const int chunk = (max_iter - launched) < poll ? (max_iter - launched) : poll;
+        for (int i = 0; i < chunk; ++i) {
+            const int it = launched + i;
+            const bool ev = c->profile && i == 0;
+            if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[0], c->stream));
+            // to = H_oe p
+            CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_PLAIN, 1, p, nullptr, to, nullptr, -1.0, it, true}));
+            if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[1], c->stream));
+            // v = p - kappa^2 H_eo to = Mhat p ; <rhat,v> ; alpha
+            CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_RV, 0, to, p, v, (void *)etah, k2, it, true}));
+            if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[2], c->stream));
+            // s = r - alpha v
+            bi_s_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(s, r, v, n, c->sc, it);
+            if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[3], c->stream));
+            // to = H_oe s
+            CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_PLAIN, 1, s, nullptr, to, nullptr, -1.0, it, true}));
+            if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[4], c->stream));
+            // t = s - kappa^2 H_eo to = Mhat s ; <t,s>, <t,t> ; omega
+            CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_TS, 0, to, s, t, nullptr, k2, it, true}));
+            if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[5], c->stream));
+            // psi_e += alpha p + omega s ; r = s - omega t ; rho', rr, beta, loop test
+            bi_xr_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((svec *)psi_e, r, p, s, t, etah, n, c->sc, c->partials,
+                                                               c->counter, c->hist, it);
+            if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[6], c->stream));
+            // p = r + beta (p - omega v)
+            bi_p_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(p, r, v, n, c->sc, it);
+            if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[7], c->stream));
+            c->launches += 3;
+            CUDA_TRY(c, cudaGetLastError());
+        }
+        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (c->profile && launched < c->sc_host->k_stop) {
+            for (int j = 0; j < 7; ++j) {
+                float ms = 0.f;
+                CUDA_TRY(c, cudaEventElapsedTime(&ms, c->bev[j], c->bev[j + 1]));
+                c->bprof_ms[j] += ms;
+            }
+            c->bprof_n++;
+        }
+        launched += chunk;
+        if (c->sc_host->k_stop <= launched) break;
+    }
+    // psi_o = eta_o + kappa H_oe psi_e
+    CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_PLAIN, 1, psi_e, eta_o, psi_o, nullptr, -kappa, 0, false}));
+    return WD_OK;
+}
+
+extern "C" int bicgstab_solve_eo(wd_ctx *c, const void *U_eo, const void *eta_eo, void *psi_eo, double kappa, double r_min,
+                                 int max_iter, wd_cg_info *info)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!U_eo || !eta_eo || !psi_eo || eta_eo == psi_eo) return fail(c, WD_ERR_ARG, "bicgstab_solve_eo: NULL argument or output aliases eta");
+    if (!std::isfinite(kappa)) return fail(c, WD_ERR_ARG, "bicgstab_solve_eo: kappa is not finite");
+    if (!(r_min > 0.0) || !std::isfinite(r_min)) return fail(c, WD_ERR_ARG, "bicgstab_solve_eo: r_min must be > 0");
+    if (max_iter < 0) return fail(c, WD_ERR_ARG, "bicgstab_solve_eo: max_iter < 0");
+    int rc = eo_check(c, "bicgstab_solve_eo");
+    if (rc != WD_OK) return rc;
+    rc = wd_ensure_workspace(c, max_iter);
+    if (rc != WD_OK) return rc;
+    if (!c->w5) {
+        CUDA_TRY(c, cudaMalloc(&c->w5, spinor_bytes(c)));
+        CUDA_TRY(c, cudaMemsetAsync(c->w5, 0, spinor_bytes(c), c->stream));
+    }
+    if (!c->w6) {
+        CUDA_TRY(c, cudaMalloc(&c->w6, half_spinor_bytes(c)));
+        CUDA_TRY(c, cudaMemsetAsync(c->w6, 0, half_spinor_bytes(c), c->stream));   // pad lanes stay zero
+    }
+    if (!c->w7) {
+        CUDA_TRY(c, cudaMalloc(&c->w7, half_spinor_bytes(c)));
+        CUDA_TRY(c, cudaMemsetAsync(c->w7, 0, half_spinor_bytes(c), c->stream));   // pad lanes stay zero
+    }
+    if (!c->eo_n2) CUDA_TRY(c, cudaMalloc(&c->eo_n2, 2 * sizeof(double)));
+    if (c->profile && !c->bev[0])
+        for (int j = 0; j < 8; ++j) CUDA_TRY(c, cudaEventCreate(&c->bev[j]));
+    c->launches = 0;
+    CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
+    rc = c->precision == 32 ? eo_bicgstab_loop<float>(c, U_eo, eta_eo, psi_eo, kappa, r_min, max_iter)
+                            : eo_bicgstab_loop<double>(c, U_eo, eta_eo, psi_eo, kappa, r_min, max_iter);
+    if (rc != WD_OK) return rc;
+    CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    const CgScalars &s = *c->sc_host;
+    c->last_iters = s.k;
+    if (info) {
+        info->iterations = s.k;
+        info->converged = s.converged;
+        info->rel_residual = s.eta2 > 0.0 ? std::sqrt(s.rr / s.eta2) : 0.0;
+        info->eta_norm2 = s.eta2;
+        float ms = 0.f;
+        CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]));
+        info->gpu_ms = ms;
+        info->total_ms = ms;
+        info->kernel_launches = c->launches;
+        info->cg_mode = 5;
+    }
+    return s.converged ? WD_OK : (s.breakdown ? WD_BREAKDOWN : WD_NOT_CONVERGED);
 }

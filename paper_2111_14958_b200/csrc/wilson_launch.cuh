@@ -114,6 +114,9 @@ cudaError_t launch_dslash_eo_f64(int tile, int dagger, int mode, const DslashArg
 // BiCGSTAB passes (D only): mode in {MODE_RV, MODE_TS}
 cudaError_t launch_dslash_bi_f32(int tile, int mode, const DslashArgs &a);
 cudaError_t launch_dslash_bi_f64(int tile, int mode, const DslashArgs &a);
+// the same on one parity of the lattice (even-odd preconditioned BiCGSTAB)
+cudaError_t launch_dslash_eo_bi_f32(int tile, int mode, const DslashArgs &a);
+cudaError_t launch_dslash_eo_bi_f64(int tile, int mode, const DslashArgs &a);
 
 template <typename real, int DAG, int MODE, int RECON = 18, int EO = 0>
 static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)

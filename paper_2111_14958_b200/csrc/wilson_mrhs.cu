@@ -187,7 +187,7 @@ extern "C" int cg_solve_multi(wd_ctx *c, const void *U, const void *eta, void *p
     if (max_iter < 0) return fail(c, WD_ERR_ARG, "cg_solve_multi: max_iter < 0");
     if (c->recon != 18) return fail(c, WD_ERR_ARG, "cg_solve_multi: 18-real links only (wd_set_gauge_recon)");
     if (c->profile && !c->bev[0])
-        for (int j = 0; j < 6; ++j) CUDA_TRY(c, cudaEventCreate(&c->bev[j]));
+        for (int j = 0; j < 8; ++j) CUDA_TRY(c, cudaEventCreate(&c->bev[j]));
     const size_t sb = spinor_bytes(c);
     int status = WD_OK, done = 0;
     c->launches = 0;

@@ -89,6 +89,8 @@ def load_library(path: str = LIB_PATH):
     lib.wd_eo_pack_gauge.argtypes = [vp, vp, vp]
     lib.wd_eo_hop.argtypes = [vp, vp, vp, vp, ci, ci]
     lib.cg_solve_eo.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
+    lib.bicgstab_solve_eo.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
+    lib.wd_get_profile_eo_bicgstab.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_long)]
     lib.wd_apply_multi.argtypes = [vp, vp, vp, vp, ci, cd, ci]
     lib.cg_solve_multi.argtypes = [vp, vp, vp, vp, ci, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
     lib.wd_coo_nnz.argtypes = [vp]
@@ -316,6 +318,23 @@ class WilsonContext:
         d = info.as_dict()
         d["status"] = rc
         return out, d
+
+    def bicgstab_solve_eo(self, U_eo, eta_eo, kappa, r_min, max_iter, out=None):
+        """even-odd preconditioned BiCGSTAB (BiCGSTAB on the Schur operator Mhat); status 2 = breakdown"""
+        out = self.empty_eo_spinor() if out is None else out
+        info = WdCgInfo()
+        rc = self.lib.bicgstab_solve_eo(self._ctx, self._p(U_eo), self._p(eta_eo), self._p(out), float(kappa),
+                                        float(r_min), int(max_iter), ctypes.byref(info))
+        self._check(rc, allow_not_converged=True)
+        d = info.as_dict()
+        d["status"] = rc
+        return out, d
+
+    def wd_get_profile_eo_bicgstab(self):
+        ms = (ctypes.c_double * 7)()
+        n = ctypes.c_long()
+        self._check(self.lib.wd_get_profile_eo_bicgstab(self._ctx, ms, ctypes.byref(n)))
+        return {"ms": list(ms), "iterations": n.value}
 
     # -- f3: several right-hand sides at once (fields: (nrhs, n) real tensors, row j = native spinor of source j)
     def empty_multi_spinor(self, nrhs):

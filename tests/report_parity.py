@@ -75,6 +75,8 @@ def rows(max_cfg=4):
             Ue, ee = ctx.wd_eo_pack_gauge(Ud), ctx.wd_eo_pack_spinor(ed)
             pe, ie = ctx.cg_solve_eo(Ue, ee, cfg.kappa, cfg.r_min, cfg.max_iter)
             out["even-odd CG"] = (ctx.wd_eo_unpack_spinor(pe).cpu().numpy(), ie, wilson_oracle.cg_solve_eo)
+            pe, ieb = ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, cfg.r_min, cfg.max_iter)
+            out["even-odd BiCGSTAB"] = (ctx.wd_eo_unpack_spinor(pe).cpu().numpy(), ieb, wilson_oracle.bicgstab_solve_eo)
             del Ue, ee, pe
             ctx.wd_set_gauge_recon(12)
             p12, i12 = ctx.cg_solve(ctx.wd_pack_gauge(Ud), en, cfg.kappa, cfg.r_min, cfg.max_iter)

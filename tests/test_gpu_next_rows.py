@@ -404,6 +404,122 @@ def test_eo_cg_32_4_closed_form(wilson, precision):
     assert err < (2e-5 if precision == 32 else 1e-9), err
 
 
+# ---------------------------------------------------------------- f3 x f4: even-odd preconditioned BiCGSTAB (readings E1 + B1)
+def eo_bicgstab_on_gpu(ctx, U, eta, kappa, r_min, max_iter):
+    Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
+    ee = ctx.wd_eo_pack_spinor(gu.to_device(eta))
+    pe, info = ctx.bicgstab_solve_eo(Ue, ee, kappa, r_min, max_iter)
+    return gu.to_host(ctx.wd_eo_unpack_spinor(pe)), info
+
+
+@pytest.mark.parametrize("precision,r_min", [(32, 1e-6), (64, 1e-10)])
+@pytest.mark.parametrize("cfg_index", [0, 1, 2])
+def test_eo_bicgstab_baseline_configs(wilson, oracle, cfg_index, precision, r_min):
+    cfg = inputs.CONFIGS[cfg_index]
+    U, eta = gu.config_fields(cfg.index, precision)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        psi, info = eo_bicgstab_on_gpu(ctx, U, eta, cfg.kappa, r_min, cfg.max_iter)
+        hist = ctx.wd_cg_history()
+        _, plain = bicgstab_on_gpu(ctx, U, eta, cfg.kappa, r_min, cfg.max_iter)
+    psi_o, info_o = oracle.bicgstab_solve_eo(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t, history=True)
+    assert info["status"] == 0 and info["converged"] == 1 and info["cg_mode"] == 5 and info_o["converged"]
+    assert info["kernel_launches"] >= 7 * info["iterations"] + 1
+    slack = 0 if precision == 64 else max(1, int(0.05 * info_o["iterations"] + 0.5))
+    assert abs(info["iterations"] - info_o["iterations"]) <= slack, (info["iterations"], info_o["iterations"])
+    assert abs(info["eta_norm2"] - info_o["eta_norm2"]) < (1e-6 if precision == 32 else 1e-13) * info_o["eta_norm2"]
+    res_gpu = oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
+    res_orc = oracle.true_residual(cfg.dims, U64, eta64, psi_o, cfg.kappa, cfg.bc_t)
+    assert res_gpu < 2.0 * r_min
+    if info["iterations"] == info_o["iterations"]:
+        assert res_gpu <= 2.0 * res_orc, (res_gpu, res_orc)
+    assert len(hist) == info["iterations"] + 1
+    n = min(len(hist), len(info_o["rr_history"]))
+    rel = np.abs(hist[:n] - info_o["rr_history"][:n]) / info_o["rr_history"][:n]
+    assert rel[0] < (1e-6 if precision == 32 else 1e-13)
+    assert np.max(rel[: max(2, n // 2)]) < (5e-2 if precision == 32 else 1e-6), rel
+    diff = np.linalg.norm(psi - psi_o) / np.linalg.norm(psi_o)
+    assert diff < 4.0 * r_min / (1.0 - 8.0 * cfg.kappa) * (1 + 8 * cfg.kappa)
+    # the odd rows of eta - D psi vanish up to rounding: psi_o = eta_o + kappa H_oe psi_e is exact for the psi_e found
+    r_full = (eta64 - oracle.wd_apply(cfg.dims, U64, psi.astype(np.complex128), cfg.kappa, False, cfg.bc_t)).reshape(-1, 12)
+    odd = np.linalg.norm(r_full[_parity(cfg.dims) == 1]) / np.linalg.norm(eta64)
+    assert odd < (2e-7 if precision == 32 else 1e-15), odd
+    # fewer iterations than the unpreconditioned BiCGSTAB on the same problem
+    assert info["iterations"] < plain["iterations"]
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_eo_bicgstab_ragged_lattices(wilson, oracle, precision):
+    """even extents that are not multiples of the tile, a half volume that is not a multiple of the 16-site block
+    (6^4: 648 sites per parity), both boundary conditions"""
+    r_min = 1e-6 if precision == 32 else 1e-10
+    cdt = gu.np_complex(precision)
+    for dims, links, bc_t in (((6, 6, 6, 6), "haar", -1), ((10, 4, 6, 8), "near_identity", 1), ((36, 4, 6, 4), "haar", -1)):
+        kappa = 0.121
+        U = inputs.gauge_field(CFG_TEST + 60, dims, links).astype(cdt)
+        eta = inputs.source_field(CFG_TEST + 60, dims).astype(cdt)
+        U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+        with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+            psi, info = eo_bicgstab_on_gpu(ctx, U, eta, kappa, r_min, 500)
+        psi_o, info_o = oracle.bicgstab_solve_eo(dims, U64, eta64, kappa, r_min, 500, bc_t)
+        assert info["status"] == 0 and abs(info["iterations"] - info_o["iterations"]) <= (0 if precision == 64 else 1)
+        res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), kappa, bc_t)
+        assert res < 2.0 * r_min, (dims, res)
+        assert np.linalg.norm(psi - psi_o) < 4.0 * r_min * (1 + 8 * kappa) / (1 - 8 * kappa) * np.linalg.norm(psi_o)
+
+
+def test_eo_bicgstab_edge_cases(wilson, oracle):
+    cfg = inputs.CONFIGS[0]
+    U, eta = gu.config_fields(0, 32)
+    par = _parity(cfg.dims)
+    with wilson.WilsonContext(cfg.dims, 32) as ctx:
+        Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
+        ee = ctx.wd_eo_pack_spinor(gu.to_device(eta))
+        pe, info = ctx.bicgstab_solve_eo(Ue, ctx.wd_eo_pack_spinor(gu.to_device(np.zeros_like(eta))), cfg.kappa, 1e-6, 10)
+        assert info["status"] == 0 and info["iterations"] == 0 and not gu.to_host(ctx.wd_eo_unpack_spinor(pe)).any()
+        pe, info = ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, 1e-6, 0)
+        z = gu.to_host(ctx.wd_eo_unpack_spinor(pe))
+        assert info["status"] == 1 and info["iterations"] == 0
+        assert not z[par == 0].any() and np.array_equal(z[par == 1], eta[par == 1])   # psi_o = eta_o for psi_e = 0
+        # kappa = 0: Mhat = 1, one iteration, psi = eta up to the rounding of alpha and omega
+        pe, info = ctx.bicgstab_solve_eo(Ue, ee, 0.0, 1e-6, 10)
+        assert info["status"] == 0 and info["iterations"] == 1
+        assert np.linalg.norm(gu.to_host(ctx.wd_eo_unpack_spinor(pe)) - eta) < 1e-6 * np.linalg.norm(eta)
+        # repeatable, independent of the poll interval, and the other even-odd solver still works on the same ctx
+        a, ia = ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, 1e-6, 100)
+        ctx.wd_set_poll_interval(1)
+        b, ib = ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, 1e-6, 100)
+        assert gu.to_host(a).tobytes() == gu.to_host(b).tobytes() and ia["iterations"] == ib["iterations"]
+        c, ic = ctx.cg_solve_eo(Ue, ee, cfg.kappa, 1e-6, 100)
+        assert ic["status"] == 0
+        assert np.linalg.norm(gu.to_host(a) - gu.to_host(c)) < 1e-4 * np.linalg.norm(gu.to_host(c))
+        with pytest.raises(wilson.WilsonError):
+            ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, 0.0, 10)
+        with pytest.raises(wilson.WilsonError):
+            ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, 1e-6, 10, out=ee)
+    with wilson.WilsonContext(cfg.dims, 32) as ctx:
+        ctx.wd_set_gauge_recon(12)
+        with pytest.raises(wilson.WilsonError):
+            ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, 1e-6, 10)
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_eo_bicgstab_32_4_closed_form(wilson, precision):
+    """BASELINE volume 32^4, exact solution known: pure-gauge links, Gaussian source (pin P8 through free_solve)"""
+    dims, kappa = (32, 32, 32, 32), 0.12
+    g = inputs.gauge_transform_field(CFG_TEST + 3, dims)
+    U = lm.pure_gauge_links(dims, g)
+    eta = inputs.source_field(CFG_TEST + 3, dims)
+    want = np.einsum("xab,xib->xia", g, lm.free_solve(dims, kappa, np.einsum("xba,xib->xia", np.conj(g), eta), -1))
+    cdt = gu.np_complex(precision)
+    tol = 1e-6 if precision == 32 else 1e-11
+    with wilson.WilsonContext(dims, precision) as ctx:
+        psi, info = eo_bicgstab_on_gpu(ctx, U.astype(cdt), eta.astype(cdt), kappa, tol, 2000)
+    assert info["status"] == 0
+    err = np.linalg.norm(psi - want) / np.linalg.norm(want)
+    assert err < (2e-5 if precision == 32 else 1e-9), err
+
+
 # ---------------------------------------------------------------- full BASELINE sizes (configs 3 and 4)
 @pytest.mark.parametrize("cfg_index", [3, 4])
 def test_next_rows_at_full_size(wilson, oracle, cfg_index):
@@ -424,12 +540,15 @@ def test_next_rows_at_full_size(wilson, oracle, cfg_index):
         Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
         pe, ie = ctx.cg_solve_eo(Ue, ctx.wd_eo_pack_spinor(gu.to_device(eta)), cfg.kappa, cfg.r_min, cfg.max_iter)
         sols["eo"] = gu.to_host(ctx.wd_eo_unpack_spinor(pe))
-        del Ue, pe
         assert ie["status"] == 0 and ie["iterations"] < 0.5 * it_cg
+        pe, ieb = ctx.bicgstab_solve_eo(Ue, ctx.wd_eo_pack_spinor(gu.to_device(eta)), cfg.kappa, cfg.r_min, cfg.max_iter)
+        sols["eo_bicgstab"] = gu.to_host(ctx.wd_eo_unpack_spinor(pe))
+        del Ue, pe
+        assert ieb["status"] == 0 and ieb["iterations"] < ib["iterations"] and ieb["iterations"] < ie["iterations"]
         ctx.wd_set_gauge_recon(12)
         sols["recon12"], i12 = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
         assert i12["status"] == 0 and abs(i12["iterations"] - it_cg) <= math.floor(0.02 * it_cg + 0.5)
-    for name in ("bicgstab", "eo", "recon12"):
+    for name in ("bicgstab", "eo", "eo_bicgstab", "recon12"):
         res = oracle.true_residual(cfg.dims, U64, eta64, sols[name].astype(np.complex128), cfg.kappa, cfg.bc_t)
         assert res < 2.0 * cfg.r_min, (name, res)
         diff = np.linalg.norm(sols[name] - sols["cg"]) / np.linalg.norm(sols["cg"])
