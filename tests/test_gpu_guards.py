@@ -1,0 +1,158 @@
+"""Out-of-bounds checks of our own (-m gpu).  compute-sanitizer is closed on the GPU pool, so every caller-visible
+device buffer of a call is carved out of a larger allocation whose guard bands (4 KiB on either side) hold a NaN
+pattern with a payload: a kernel that WRITES outside its buffer changes the pattern, one that READS outside it pulls NaNs
+into its result.  Lattices are ragged on purpose: volume (and half volume) not a multiple of the 16-site block, extents
+not multiples of the tile.  The volume-dependent pad lanes INSIDE the buffers are poisoned too where the call's contract
+says they are ignored (inputs of wd_apply / cg_solve / the even-odd calls come from the pack kernels, which zero them)."""
+import numpy as np
+import pytest
+
+from paper_2111_14958_b200 import inputs
+import gpu_util as gu
+
+pytestmark = pytest.mark.gpu
+
+GUARD = 1024          # elements on either side
+PATTERN32 = 0x7FC0BEEF
+PATTERN64 = 0x7FF80000DEADBEEF
+CFG_TEST = 870
+
+
+@pytest.fixture(scope="module")
+def wilson():
+    from paper_2111_14958_b200 import build as wbuild
+    from paper_2111_14958_b200 import wilson as w
+
+    wbuild.build()
+    w.load_library()
+    return w
+
+
+class Guarded:
+    """n elements of `dtype` between two guard bands"""
+
+    def __init__(self, like):
+        import torch
+
+        self.n = like.numel()
+        self.itype = torch.int32 if like.element_size() == 4 else torch.int64
+        self.pattern = PATTERN32 if like.element_size() == 4 else PATTERN64
+        self.raw = torch.full((self.n + 2 * GUARD,), self.pattern, dtype=self.itype, device="cuda")
+        self.t = self.raw[GUARD:GUARD + self.n].view(like.dtype)
+
+    def intact(self):
+        lo, hi = self.raw[:GUARD], self.raw[GUARD + self.n:]
+        return bool((lo == self.pattern).all()) and bool((hi == self.pattern).all())
+
+
+def guarded_copy(src):
+    g = Guarded(src)
+    g.t.copy_(src)
+    return g
+
+
+def all_intact(*gs):
+    return all(g.intact() for g in gs)
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("dims", [(5, 7, 4, 6), (4, 4, 4, 4), (18, 4, 6, 4)])
+def test_plain_calls_stay_inside_their_buffers(wilson, dims, precision):
+    import torch
+
+    cdt = gu.np_complex(precision)
+    r_min = 1e-6 if precision == 32 else 1e-10
+    kappa = 0.12
+    U = inputs.gauge_field(CFG_TEST, dims, "haar", dtype=cdt)
+    eta = inputs.source_field(CFG_TEST, dims, dtype=cdt)
+    with wilson.WilsonContext(dims, precision, -1) as ctx:
+        Uc, ec = guarded_copy(torch.view_as_real(gu.to_device(U)).reshape(-1)), guarded_copy(torch.view_as_real(gu.to_device(eta)).reshape(-1))
+        Un, en, out = Guarded(ctx.empty_gauge()), Guarded(ctx.empty_spinor()), Guarded(ctx.empty_spinor())
+        ctx._check(ctx.lib.wd_pack_gauge(ctx._ctx, ctx._p(Uc.t), ctx._p(Un.t)))
+        ctx._check(ctx.lib.wd_pack_spinor(ctx._ctx, ctx._p(ec.t), ctx._p(en.t)))
+        assert torch.isfinite(Un.t).all() and torch.isfinite(en.t).all()     # pad lanes were written (zeros)
+        for tile in range(wilson.load_library().wd_num_tiles()):
+            try:
+                ctx.wd_set_tile(tile)
+            except wilson.WilsonError:
+                continue                                                     # not compiled for this precision
+            for dag in (0, 1):
+                ctx.wd_apply(Un.t, en.t, kappa, dag, out=out.t)
+                got = ctx.wd_unpack_spinor(out.t)
+                assert torch.isfinite(torch.view_as_real(got)).all(), (tile, dag)
+        ctx.wd_set_tile(-1)
+        for mode in (1, 2):
+            ctx.wd_set_cg_mode(mode)
+            _, info = ctx.cg_solve(Un.t, en.t, kappa, r_min, 500, out=out.t)
+            assert info["status"] == 0 and torch.isfinite(torch.view_as_real(ctx.wd_unpack_spinor(out.t))).all()
+        ctx.wd_set_cg_mode(0)
+        _, info = ctx.bicgstab_solve(Un.t, en.t, kappa, r_min, 500, out=out.t)
+        assert info["status"] == 0 and torch.isfinite(torch.view_as_real(ctx.wd_unpack_spinor(out.t))).all()
+        assert np.isfinite(ctx.wd_norm2(en.t))
+        can = Guarded(torch.view_as_real(gu.to_device(eta)).reshape(-1))
+        ctx._check(ctx.lib.wd_unpack_spinor(ctx._ctx, ctx._p(out.t), ctx._p(can.t)))
+        assert torch.isfinite(can.t).all()
+        # the paper's COO arrays
+        nnz = ctx.wd_coo_nnz()
+        val = Guarded(torch.empty(2 * nnz, dtype=ctx.real_dtype, device="cuda"))
+        row = Guarded(torch.empty(nnz, dtype=torch.int32, device="cuda"))
+        col = Guarded(torch.empty(nnz, dtype=torch.int32, device="cuda"))
+        ctx._check(ctx.lib.wd_coo_assemble(ctx._ctx, ctx._p(Un.t), kappa, 0, ctx._p(val.t), ctx._p(row.t), ctx._p(col.t)))
+        assert int(row.t.min()) == 0 and int(row.t.max()) == 12 * ctx.volume - 1
+        assert int(col.t.min()) >= 0 and int(col.t.max()) < 12 * ctx.volume
+        ctx._check(ctx.lib.wd_coo_spmv(ctx._ctx, nnz, ctx._p(val.t), ctx._p(row.t), ctx._p(col.t), ctx._p(ec.t), ctx._p(can.t)))
+        assert torch.isfinite(can.t).all()
+        # several right-hand sides: 3 sources in one guarded buffer
+        n = en.t.numel()
+        em, om = Guarded(torch.empty(3 * n, dtype=ctx.real_dtype, device="cuda")), Guarded(torch.empty(3 * n, dtype=ctx.real_dtype, device="cuda"))
+        for j in range(3):
+            em.t[j * n:(j + 1) * n] = en.t * (1.0 + j)
+        ctx.wd_apply_multi(Un.t, em.t.view(3, n), kappa, False, out=om.t.view(3, n))
+        _, infos = ctx.cg_solve_multi(Un.t, em.t.view(3, n), kappa, r_min, 500, out=om.t.view(3, n))
+        assert all(i["status"] == 0 for i in infos)
+        for j in range(3):
+            assert torch.isfinite(torch.view_as_real(ctx.wd_unpack_spinor(om.t[j * n:(j + 1) * n]))).all()
+        # 12-real links
+        ctx.wd_set_gauge_recon(12)
+        U12 = Guarded(ctx.empty_gauge())
+        ctx._check(ctx.lib.wd_pack_gauge(ctx._ctx, ctx._p(Uc.t), ctx._p(U12.t)))
+        ctx.wd_set_cg_mode(1)
+        _, info = ctx.cg_solve(U12.t, en.t, kappa, r_min, 500, out=out.t)
+        assert info["status"] == 0 and torch.isfinite(torch.view_as_real(ctx.wd_unpack_spinor(out.t))).all()
+        torch.cuda.synchronize()
+        assert all_intact(Uc, ec, Un, en, out, can, val, row, col, em, om, U12)
+        # inputs were not modified
+        assert torch.equal(ec.t, torch.view_as_real(gu.to_device(eta)).reshape(-1))
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("dims", [(6, 6, 6, 6), (4, 4, 4, 4), (10, 4, 6, 8)])
+def test_even_odd_calls_stay_inside_their_buffers(wilson, dims, precision):
+    import torch
+
+    cdt = gu.np_complex(precision)
+    r_min = 1e-6 if precision == 32 else 1e-10
+    kappa = 0.12
+    U = inputs.gauge_field(CFG_TEST + 1, dims, "near_identity", dtype=cdt)
+    eta = inputs.source_field(CFG_TEST + 1, dims, dtype=cdt)
+    with wilson.WilsonContext(dims, precision, -1) as ctx:
+        Uc, ec = guarded_copy(torch.view_as_real(gu.to_device(U)).reshape(-1)), guarded_copy(torch.view_as_real(gu.to_device(eta)).reshape(-1))
+        Ue, ee, pe, tmp = (Guarded(ctx.empty_eo_gauge()), Guarded(ctx.empty_eo_spinor()), Guarded(ctx.empty_eo_spinor()),
+                           Guarded(ctx.empty_eo_spinor()))
+        ctx._check(ctx.lib.wd_eo_pack_gauge(ctx._ctx, ctx._p(Uc.t), ctx._p(Ue.t)))
+        ctx._check(ctx.lib.wd_eo_pack_spinor(ctx._ctx, ctx._p(ec.t), ctx._p(ee.t)))
+        assert torch.isfinite(Ue.t).all() and torch.isfinite(ee.t).all()
+        tmp.t.zero_()
+        for par in (0, 1):
+            for dag in (0, 1):
+                ctx.wd_eo_hop(Ue.t, ee.t, tmp.t, par, dag)
+        assert torch.isfinite(tmp.t).all()
+        _, info = ctx.cg_solve_eo(Ue.t, ee.t, kappa, r_min, 500, out=pe.t)
+        assert info["status"] == 0 and torch.isfinite(torch.view_as_real(ctx.wd_eo_unpack_spinor(pe.t))).all()
+        _, info = ctx.bicgstab_solve_eo(Ue.t, ee.t, kappa, r_min, 500, out=pe.t)
+        assert info["status"] == 0 and torch.isfinite(torch.view_as_real(ctx.wd_eo_unpack_spinor(pe.t))).all()
+        can = Guarded(torch.view_as_real(gu.to_device(eta)).reshape(-1))
+        ctx._check(ctx.lib.wd_eo_unpack_spinor(ctx._ctx, ctx._p(pe.t), ctx._p(can.t)))
+        torch.cuda.synchronize()
+        assert all_intact(Uc, ec, Ue, ee, pe, tmp, can)
+        assert torch.equal(ec.t, torch.view_as_real(gu.to_device(eta)).reshape(-1))
