@@ -174,19 +174,9 @@ def run_reference(args, cfg):
 
 
 def time_wd_apply(ctx, Un, en, out, kappa, dagger, reps=100):
-    """device time per application over `reps` back-to-back applications (CUDA events on the ctx stream)"""
-    import torch
-
-    for _ in range(5):
-        ctx.wd_apply(Un, en, kappa, dagger, out=out)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    e0.record()
-    for _ in range(reps):
-        ctx.wd_apply(Un, en, kappa, dagger, out=out)
-    e1.record()
-    torch.cuda.synchronize()
-    return e0.elapsed_time(e1) / reps
+    """device time per application over `reps` back-to-back applications (enqueued from C by wd_apply_repeat, CUDA
+    events on the ctx stream; median of three rounds)"""
+    return sorted(ctx.wd_apply_repeat(Un, en, kappa, dagger, reps, out=out) for _ in range(3))[1]
 
 
 def run_report(args):

@@ -143,6 +143,15 @@ int wd_apply(wd_ctx *ctx, const void *U_native, const void *psi_native, void *ou
              double kappa, int dagger);
 
 /*
+ * wd_apply_repeat — measurement aid for "standalone wd_apply timing over 100 applications" (BASELINE.json configs[2]):
+ * one warm-up application, then `reps` applications of the same input enqueued back to back from C (at 4^4..14^4 an
+ * application is shorter than the call overhead of a scripting-language binding), bracketed by CUDA events on the ctx
+ * stream.  *ms_per_application (host pointer) = device time / reps.  Arguments as wd_apply; reps >= 1.  Synchronous.
+ */
+int wd_apply_repeat(wd_ctx *ctx, const void *U_native, const void *psi_native, void *out_native, double kappa,
+                    int dagger, int reps, double *ms_per_application);
+
+/*
  * cg_solve — solve D psi = eta (Eq. 1) by the paper's CG on D D-dagger followed
  * by one multiplication with D-dagger (readings G1-G5):
  *     y <- 0; r <- eta; p <- r; rr <- <r,r>

@@ -339,6 +339,28 @@ extern "C" int wd_apply(wd_ctx *c, const void *U, const void *psi, void *out, do
     return WD_OK;
 }
 
+/* `reps` back-to-back applications enqueued from C (no binding overhead between the launches), timed with CUDA events
+   on the ctx stream: *ms_per_application = device time / reps.  Synchronous. */
+extern "C" int wd_apply_repeat(wd_ctx *c, const void *U, const void *psi, void *out, double kappa, int dagger, int reps,
+                               double *ms_per_application)
+{
+    if (!c) return WD_ERR_ARG;
+    if (reps < 1 || !ms_per_application) return fail(c, WD_ERR_ARG, "wd_apply_repeat: reps < 1 or NULL result");
+    int rc = wd_apply(c, U, psi, out, kappa, dagger);   // argument checks + warm-up
+    if (rc != WD_OK) return rc;
+    CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
+    for (int i = 0; i < reps; ++i) {
+        rc = wd_apply(c, U, psi, out, kappa, dagger);
+        if (rc != WD_OK) return rc;
+    }
+    CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
+    CUDA_TRY(c, cudaEventSynchronize(c->ev[1]));
+    float ms = 0.f;
+    CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]));
+    *ms_per_application = (double)ms / reps;
+    return WD_OK;
+}
+
 extern "C" int wd_norm2(wd_ctx *c, const void *a, double *result)
 {
     if (!c) return WD_ERR_ARG;

@@ -98,6 +98,7 @@ def load_library(path: str = LIB_PATH):
     lib.wd_coo_assemble.argtypes = [vp, vp, cd, ci, vp, vp, vp]
     lib.wd_coo_spmv.argtypes = [vp, ctypes.c_size_t, vp, vp, vp, vp, vp]
     lib.wd_apply_host.argtypes = [vp, vp, vp, vp, cd, ci]
+    lib.wd_apply_repeat.argtypes = [vp, vp, vp, vp, cd, ci, ci, dp]
     lib.cg_solve_host.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
     lib.wd_cg_history.argtypes = [vp, dp, ci]
     lib.wd_norm2.argtypes = [vp, vp, dp]
@@ -245,6 +246,14 @@ class WilsonContext:
         self._check(self.lib.wd_apply(self._ctx, self._p(U_native), self._p(psi_native), self._p(out),
                                       float(kappa), int(bool(dagger))))
         return out
+
+    def wd_apply_repeat(self, U_native, psi_native, kappa, dagger=False, reps=100, out=None):
+        """device milliseconds per application over `reps` back-to-back applications enqueued from C"""
+        out = self.empty_spinor() if out is None else out
+        ms = ctypes.c_double()
+        self._check(self.lib.wd_apply_repeat(self._ctx, self._p(U_native), self._p(psi_native), self._p(out),
+                                             float(kappa), int(bool(dagger)), int(reps), ctypes.byref(ms)))
+        return ms.value
 
     # -- a1..a6
     def cg_solve(self, U_native, eta_native, kappa, r_min, max_iter, out=None):
