@@ -142,6 +142,8 @@ extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_
     ok = ok && cudaMalloc(&c->result_dev, sizeof(double)) == cudaSuccess;
     ok = ok && cudaMallocHost(&c->sc_host, sizeof(CgScalars)) == cudaSuccess;
     ok = ok && cudaMallocHost(&c->result_host, sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMallocHost(&c->sc_poll, 2 * sizeof(CgScalars)) == cudaSuccess;
+    for (int i = 0; i < 2 && ok; ++i) ok = cudaEventCreateWithFlags(&c->poll_ev[i], cudaEventDisableTiming) == cudaSuccess;
     ok = ok && cudaMemsetAsync(c->counter, 0, sizeof(unsigned int), c->stream) == cudaSuccess;
     ok = ok && cudaMemsetAsync(c->sc, 0, sizeof(CgScalars), c->stream) == cudaSuccess;
     for (int i = 0; i < 4 && ok; ++i) ok = cudaEventCreate(&c->ev[i]) == cudaSuccess;
@@ -167,6 +169,9 @@ extern "C" int wd_destroy(wd_ctx *c)
     if (c->sc_host) cudaFreeHost(c->sc_host);
     if (c->m_sc_host) cudaFreeHost(c->m_sc_host);
     if (c->result_host) cudaFreeHost(c->result_host);
+    if (c->sc_poll) cudaFreeHost(c->sc_poll);
+    for (int i = 0; i < 2; ++i)
+        if (c->poll_ev[i]) cudaEventDestroy(c->poll_ev[i]);
     for (int i = 0; i < 4; ++i)
         if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     for (int i = 0; i < 4 * c->pev_cap; ++i) cudaEventDestroy(c->pev[i]);
@@ -477,29 +482,30 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
     CUDA_TRY(c, cudaGetLastError());
 
     const int poll = c->poll > 0 ? c->poll : auto_poll(c);
-    if (c->profile && c->pev_cap < poll) {
-        cudaEvent_t *pe = (cudaEvent_t *)realloc(c->pev, sizeof(cudaEvent_t) * 4 * (size_t)poll);
+    if (c->profile && c->pev_cap < 2 * poll) {   // two chunks of `poll` iterations are in flight at a time
+        cudaEvent_t *pe = (cudaEvent_t *)realloc(c->pev, sizeof(cudaEvent_t) * 4 * (size_t)(2 * poll));
         if (!pe) return fail(c, WD_ERR_ALLOC, "cg_solve: out of host memory");
         c->pev = pe;
-        for (; c->pev_cap < poll; ++c->pev_cap)
+        for (; c->pev_cap < 2 * poll; ++c->pev_cap)
             for (int j = 0; j < 4; ++j) CUDA_TRY(c, cudaEventCreate(&c->pev[4 * c->pev_cap + j]));
     }
-    int launched = 0;
-    while (launched < max_iter) {
-        const int chunk = (max_iter - launched) < poll ? (max_iter - launched) : poll;
+    // One chunk of `poll` iterations is always enqueued AHEAD of the one whose stop flag the host waits for
+    // (wd_poll_loop).  The per-kernel profiling events come from a pool of two chunks, indexed like the poll mirrors.
+    auto enqueue_chunk = [&](int first, int chunk, int pslot) -> int {
+        cudaEvent_t *pev = c->profile ? c->pev + 4 * (size_t)pslot * poll : nullptr;
         for (int i = 0; i < chunk; ++i) {
-            const int it = launched + i;
+            const int it = first + i;
             // direction of the three passes of iteration `it`: the init kernel ran forward, every pass after it walks
             // against the one before (pass number 3 it + j + 1), so each starts on what the last one left in L2
             const int rev2 = c->sweep ? (3 * it + 1) & 1 : 0, rev3 = c->sweep ? (3 * it + 2) & 1 : 0,
                       rev4 = c->sweep ? (3 * it + 3) & 1 : 0;
-            if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 0], c->stream));
+            if (c->profile) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 0], c->stream));
             // a2: q = D-dagger p, qq, alpha
             CUDA_TRY(c, (launch_dslash<1, MODE_QQ>(c, U, c->p, c->q, kappa, nullptr, it, rev2)));
-            if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 1], c->stream));
+            if (c->profile) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 1], c->stream));
             // a3: r -= alpha D q, rr', beta, loop condition
             CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it, rev3)));
-            if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 2], c->stream));
+            if (c->profile) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 2], c->stream));
             // a4: y += alpha p ; p = r + beta p
             if (c->precision == 32)
                 cg_update_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((float4 *)c->y, (float4 *)c->p,
@@ -509,24 +515,29 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
                                                                            (const double2 *)c->r, n, c->sc, it, rev4);
             c->launches++;
             CUDA_TRY(c, cudaGetLastError());
-            if (c->profile) CUDA_TRY(c, cudaEventRecord(c->pev[4 * i + 3], c->stream));
+            if (c->profile) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 3], c->stream));
         }
-        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
-        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-        if (c->profile) {
-            // only iterations that really ran (it < k_stop) count; over-launched ones are no-ops
-            for (int i = 0; i < chunk && launched + i < c->sc_host->k_stop; ++i) {
-                for (int j = 0; j < 3; ++j) {
-                    float ms = 0.f;
-                    CUDA_TRY(c, cudaEventElapsedTime(&ms, c->pev[4 * i + j], c->pev[4 * i + j + 1]));
-                    c->prof_ms[j] += ms;
-                }
-                c->prof_n++;
+        return WD_OK;
+    };
+    auto polled = [&](int first, int chunk, int pslot) -> int {
+        if (!c->profile) return WD_OK;
+        // only iterations that really ran (it < k_stop) count; over-launched ones are no-ops
+        const cudaEvent_t *pev = c->pev + 4 * (size_t)pslot * poll;
+        for (int i = 0; i < chunk && first + i < c->sc_host->k_stop; ++i) {
+            for (int j = 0; j < 3; ++j) {
+                float ms = 0.f;
+                CUDA_TRY(c, cudaEventElapsedTime(&ms, pev[4 * i + j], pev[4 * i + j + 1]));
+                c->prof_ms[j] += ms;
             }
+            c->prof_n++;
         }
-        launched += chunk;
-        if (c->sc_host->k_stop <= launched) break;  // the device loop condition failed (or eta = 0)
-    }
+        return WD_OK;
+    };
+    // look ahead only where a chunk of real iterations is long against the chunk of no-op launches it can cost at the end
+    // of the solve (3 x poll launches of ~2.5 us): measured at 32^4 40.6 -> 39.8 ms per solve, at 4^4..14^4 a loss
+    const bool ahead = (c->precision == 32 ? 1536.0 : 3072.0) * c->V / 6.0e12 >= 150.0e-6;
+    rc = wd_poll_loop(c, max_iter, poll, ahead, enqueue_chunk, polled);
+    if (rc != WD_OK) return rc;
     // a6: psi = D-dagger y ("then we multiply the solution by D-dagger")
     // (against the last a4 that really ran: pass number 3 k, so this is pass 3 k + 1)
     CUDA_TRY(c, (launch_dslash<1, MODE_PLAIN>(c, U, c->y, psi, kappa, nullptr, 0,
@@ -602,11 +613,9 @@ static int bicgstab_loop(wd_ctx *c, const void *U, const void *eta_, void *psi_,
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
     const int poll = c->poll > 0 ? c->poll : auto_poll(c);
-    int launched = 0;
-    while (launched < max_iter) {
-        const int chunk = (max_iter - launched) < poll ? (max_iter - launched) : poll;
+    auto enqueue = [&](int first, int chunk, int) -> int {
         for (int i = 0; i < chunk; ++i) {
-            const int it = launched + i;
+            const int it = first + i;
             if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[0], c->stream));
             // v = D p, <rhat,v>, alpha
             CUDA_TRY(c, (launch_dslash_bi<MODE_RV>(c, U, p, v, kappa, (void *)eta, it)));
@@ -627,9 +636,10 @@ static int bicgstab_loop(wd_ctx *c, const void *U, const void *eta_, void *psi_,
             c->launches += 3;
             CUDA_TRY(c, cudaGetLastError());
         }
-        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
-        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-        if (c->profile && launched < c->sc_host->k_stop) {   // the first iteration of the chunk really ran
+        return WD_OK;
+    };
+    auto polled = [&](int first, int, int) -> int {
+        if (c->profile && first < c->sc_host->k_stop) {   // the first iteration of the chunk really ran
             for (int j = 0; j < 5; ++j) {
                 float ms = 0.f;
                 CUDA_TRY(c, cudaEventElapsedTime(&ms, c->bev[j], c->bev[j + 1]));
@@ -637,9 +647,12 @@ static int bicgstab_loop(wd_ctx *c, const void *U, const void *eta_, void *psi_,
             }
             c->bprof_n++;
         }
-        launched += chunk;
-        if (c->sc_host->k_stop <= launched) break;
-    }
+        return WD_OK;
+    };
+    // one chunk at a time: looking ahead measured no gain here (five launches per iteration make the over-launched
+    // chunk at the end as expensive as the poll gaps it removes)
+    int rc = wd_poll_loop(c, max_iter, poll, false, enqueue, polled);
+    if (rc != WD_OK) return rc;
     return WD_OK;
 }
 

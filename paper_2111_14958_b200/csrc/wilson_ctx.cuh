@@ -50,6 +50,8 @@ struct wd_ctx {
     // pinned host mirrors
     wd::CgScalars *sc_host;
     double *result_host;
+    wd::CgScalars *sc_poll;   // two pinned mirrors of sc: the poll of chunk k is read while chunk k+1 is already enqueued
+    cudaEvent_t poll_ev[2];
     // staging of the *_host calls
     void *U_can, *U_nat, *s_can, *s_nat_in, *s_nat_out;
     int have_gauge;
@@ -98,6 +100,48 @@ static inline size_t spinor_can_bytes(const wd_ctx *c) { return (size_t)24 * c->
 static inline size_t gauge_can_bytes(const wd_ctx *c) { return (size_t)72 * c->V * real_bytes(c); }      // canonical
 static inline size_t spinor_vecs(const wd_ctx *c) { return (size_t)(c->precision == 32 ? 6 : 12) * vpad(c); }
 
+
+// Host side of the device-resident solver loops (reading R1).  Iterations are enqueued in chunks of
+// `poll`; after each chunk the device scalars are copied to a pinned mirror and the host waits for that copy to learn
+// whether the loop condition has failed (k_stop).  With `ahead`, the NEXT chunk is enqueued before the host waits, so the
+// stream never drains at a poll; kernels of iterations >= k_stop return at once, which makes the over-launch harmless.
+//   enqueue(first_iteration, n_iterations, slot) -> WD_OK / error      slot in {0,1}: which of two event pools to use
+//   polled(first_iteration, n_iterations, slot)  -> WD_OK / error      called after the chunk's scalars are in c->sc_host
+template <typename Enqueue, typename Polled>
+static inline int wd_poll_loop(wd_ctx *c, int max_iter, int poll, bool ahead, Enqueue enqueue, Polled polled)
+{
+    int launched = 0;      // iterations whose stop flag has been read back
+    int enqueued = 0;      // iterations enqueued
+    int slot = 0;          // pinned mirror / event the next chunk reports into
+    auto report = [&](int sl) -> int {
+        CUDA_TRY(c, cudaMemcpyAsync(&c->sc_poll[sl], c->sc, sizeof(wd::CgScalars), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaEventRecord(c->poll_ev[sl], c->stream));
+        return WD_OK;
+    };
+    while (launched < max_iter) {
+        const int chunk = (max_iter - launched) < poll ? (max_iter - launched) : poll;
+        int rc;
+        if (enqueued == launched) {   // nothing in flight for this chunk yet
+            if ((rc = enqueue(launched, chunk, slot)) != WD_OK) return rc;
+            enqueued = launched + chunk;
+            if ((rc = report(slot)) != WD_OK) return rc;
+        }
+        const int wait_slot = slot;
+        slot ^= 1;
+        if (ahead && enqueued < max_iter) {   // the next chunk, before this one's flag is known
+            const int next = (max_iter - enqueued) < poll ? (max_iter - enqueued) : poll;
+            if ((rc = enqueue(enqueued, next, slot)) != WD_OK) return rc;
+            enqueued += next;
+            if ((rc = report(slot)) != WD_OK) return rc;
+        }
+        CUDA_TRY(c, cudaEventSynchronize(c->poll_ev[wait_slot]));
+        *c->sc_host = c->sc_poll[wait_slot];
+        if ((rc = polled(launched, chunk, wait_slot)) != WD_OK) return rc;
+        launched += chunk;
+        if (c->sc_host->k_stop <= launched) break;  // the device loop condition failed (or eta = 0)
+    }
+    return WD_OK;
+}
 
 // CG workspace of the ctx (r, p, q, y at full length, zeroed once; history of max_iter + 1 doubles); wilson_cg.cu
 int wd_ensure_workspace(wd_ctx *c, int max_iter);

@@ -240,11 +240,9 @@ static int eo_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, void *psi_eo
     CUDA_TRY(c, cudaGetLastError());
 
     const int poll = c->poll > 0 ? c->poll : 8;
-    int launched = 0;
-    while (launched < max_iter) {
-        const int chunk = (max_iter - launched) < poll ? (max_iter - launched) : poll;
+    auto enqueue = [&](int first, int chunk, int) -> int {
         for (int i = 0; i < chunk; ++i) {
-            const int it = launched + i;
+            const int it = first + i;
             const bool ev = c->profile && i == 0;
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[0], c->stream));
             // t_o = H-dagger_oe p_e
@@ -265,9 +263,10 @@ static int eo_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, void *psi_eo
             CUDA_TRY(c, cudaGetLastError());
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[5], c->stream));
         }
-        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
-        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-        if (c->profile && launched < c->sc_host->k_stop) {
+        return WD_OK;
+    };
+    auto polled = [&](int first, int, int) -> int {
+        if (c->profile && first < c->sc_host->k_stop) {
             for (int j = 0; j < 5; ++j) {
                 float ms = 0.f;
                 CUDA_TRY(c, cudaEventElapsedTime(&ms, c->bev[j], c->bev[j + 1]));
@@ -275,9 +274,10 @@ static int eo_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, void *psi_eo
             }
             c->bprof_n++;
         }
-        launched += chunk;
-        if (c->sc_host->k_stop <= launched) break;
-    }
+        return WD_OK;
+    };
+    int rc = wd_poll_loop(c, max_iter, poll, false, enqueue, polled);   // no look-ahead: measured no gain (wilson_cg.cu)
+    if (rc != WD_OK) return rc;
     // psi_e = Mhat-dagger y ; psi_o = eta_o + kappa H_oe psi_e
     CUDA_TRY(c, eo_launch(c, U_eo, EoPass{1, MODE_PLAIN, 1, y, nullptr, t, nullptr, -1.0, 0, false}));
     CUDA_TRY(c, eo_launch(c, U_eo, EoPass{1, MODE_PLAIN, 0, t, y, psi_e, nullptr, k2, 0, false}));
@@ -367,11 +367,9 @@ static int eo_bicgstab_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, voi
     CUDA_TRY(c, cudaGetLastError());
 
     const int poll = c->poll > 0 ? c->poll : 4;
-    int launched = 0;
-    while (launched < max_iter) {
-        const int chunk = (max_iter - launched) < poll ? (max_iter - launched) : poll;
+    auto enqueue = [&](int first, int chunk, int) -> int {
         for (int i = 0; i < chunk; ++i) {
-            const int it = launched + i;
+            const int it = first + i;
             const bool ev = c->profile && i == 0;
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[0], c->stream));
             // to = H_oe p
@@ -399,9 +397,10 @@ static int eo_bicgstab_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, voi
             c->launches += 3;
             CUDA_TRY(c, cudaGetLastError());
         }
-        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
-        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
-        if (c->profile && launched < c->sc_host->k_stop) {
+        return WD_OK;
+    };
+    auto polled = [&](int first, int, int) -> int {
+        if (c->profile && first < c->sc_host->k_stop) {
             for (int j = 0; j < 7; ++j) {
                 float ms = 0.f;
                 CUDA_TRY(c, cudaEventElapsedTime(&ms, c->bev[j], c->bev[j + 1]));
@@ -409,9 +408,10 @@ static int eo_bicgstab_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, voi
             }
             c->bprof_n++;
         }
-        launched += chunk;
-        if (c->sc_host->k_stop <= launched) break;
-    }
+        return WD_OK;
+    };
+    int rc = wd_poll_loop(c, max_iter, poll, false, enqueue, polled);   // no look-ahead: measured no gain (wilson_cg.cu)
+    if (rc != WD_OK) return rc;
     // psi_o = eta_o + kappa H_oe psi_e
     CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_PLAIN, 1, psi_e, eta_o, psi_o, nullptr, -kappa, 0, false}));
     return WD_OK;
