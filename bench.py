@@ -217,6 +217,8 @@ def run_report(args):
                 "wd_apply_D_us": d_ms * 1e3, "wd_apply_Ddag_us": dd_ms * 1e3, "applications": 100,
                 "wd_apply_D_gflops": FLOP_APPLY * V / (d_ms * 1e-3) / 1e9,
                 "wd_apply_Ddag_gflops": FLOP_APPLY * V / (dd_ms * 1e-3) / 1e9,
+                "wd_apply_D_gflops_hopping_only_1320": 1320 * V / (d_ms * 1e-3) / 1e9,
+                "wd_apply_Ddag_gflops_hopping_only_1320": 1320 * V / (dd_ms * 1e-3) / 1e9,
                 "wd_apply_D_gbs": (480 if prec == 32 else 960) * V / (d_ms * 1e-3) / 1e9,
                 "cg_iterations": it, "cg_rel_residual": info["rel_residual"], "cg_mode": info["cg_mode"],
                 "cg_solve_ms": t, "cg_gflops": cg_flops(V, it) / (t * 1e-3) / 1e9,
@@ -224,6 +226,53 @@ def run_report(args):
                 "cg_iteration_gbs_live": bpi * V / (iter_ms * 1e-3) / 1e9 if iter_ms else None,
                 "cg_iteration_gbs_whole_solve": bpi * V * it / (t * 1e-3) / 1e9,
                 "tile": list(wilson.tile_shapes()[ctx.wd_get_tile()])}), flush=True)
+    return 0
+
+
+def run_oracle_report(args):
+    """SURVEY.md 8(d) "Oracle timing": the fp64 CPU oracle as it stands on this box's host cores, at all cores and at
+    one thread.  Full CG at configs 0-2 (both thread counts) and at config 3 (all cores; one thread: 2 iterations);
+    config 4: 10 iterations + final D-dagger at all cores, one wd_apply at both thread counts.  One JSON line each.
+    Needs no GPU.  Reported baseline, not a target."""
+    from oracle import wilson_oracle
+
+    cpu = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            cpu = next(l.split(":", 1)[1].strip() for l in f if l.startswith("model name"))
+    except Exception:
+        pass
+    all_threads = wilson_oracle.num_threads()
+    for ci in [int(x) for x in args.rows_configs.split(",") if x] if args.rows_configs != "3,4" else range(5):
+        cfg = inputs.CONFIGS[ci]
+        U, eta = inputs.config_inputs(cfg, dtype=np.complex64)
+        U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+        del U, eta
+        V = cfg.volume
+        for nt in (all_threads, 1):
+            wilson_oracle.set_num_threads(nt)
+            reps = max(1, min(100, int(2.0e6 * nt / V)))
+            if V <= 1 << 20:
+                wilson_oracle.wd_apply(cfg.dims, U64, eta64, cfg.kappa, False, cfg.bc_t)   # warm-up (thread pool start)
+            t0 = time.perf_counter()
+            for _ in range(reps):
+                wilson_oracle.wd_apply(cfg.dims, U64, eta64, cfg.kappa, False, cfg.bc_t)
+            apply_s = (time.perf_counter() - t0) / reps
+            line = {"oracle_report": f"config{ci}", "name": cfg.name, "volume": V, "threads": nt, "host_cores": os.cpu_count(),
+                    "cpu": cpu, "wd_apply_ms": apply_s * 1e3, "wd_apply_gflops": FLOP_APPLY * V / apply_s / 1e9,
+                    "wd_apply_applications": reps}
+            full = ci <= 2 or (ci == 3 and nt == all_threads)
+            iters = cfg.max_iter if full else (10 if (ci == 4 and nt == all_threads) else (2 if ci == 3 else 0))
+            if iters:
+                t0 = time.perf_counter()
+                _, info = wilson_oracle.cg_solve(cfg.dims, U64, eta64, cfg.kappa, cfg.r_min if full else 1e-30, iters, cfg.bc_t)
+                dt = time.perf_counter() - t0
+                line.update({"cg": "full solve" if full else f"{iters} iterations + final D-dagger",
+                             "cg_iterations": info["iterations"], "cg_seconds": dt,
+                             "cg_seconds_per_iteration": dt / max(info["iterations"], 1),
+                             "cg_gflops": cg_flops(V, info["iterations"]) / dt / 1e9})
+            print(json.dumps(line), flush=True)
+        wilson_oracle.set_num_threads(all_threads)
     return 0
 
 
@@ -498,6 +547,9 @@ def main():
                     help="one JSON line per SURVEY.md 8(f) row: 12-real links and BiCGSTAB at configs 3 and 4, the paper's COO "
                          "SpMV at 14^4 beside the stencil")
     ap.add_argument("--rows-configs", default="3,4", help="configs the solver rows of --rows run on (comma separated)")
+    ap.add_argument("--oracle-report", action="store_true",
+                    help="time the fp64 CPU oracle on this box's host cores at all cores and at one thread (SURVEY.md 8(d)); "
+                         "needs no GPU; --rows-configs selects the configs (default all five)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -505,6 +557,8 @@ def main():
     r_min = cfg.r_min if args.precision == 32 else 1e-10
     if args.impl == "reference":
         return run_reference(args, cfg)
+    if args.oracle_report:
+        return run_oracle_report(args) if int(os.environ.get("RANK", "0")) == 0 else 0
 
     import torch
 

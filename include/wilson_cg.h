@@ -81,7 +81,9 @@ typedef struct wd_cg_info {
     double gpu_ms;         /* device time of init + loop + final D-dagger (CUDA events on the ctx stream) */
     double total_ms;       /* *_host calls: device time including H2D copies, pack, solve, unpack, D2H; else = gpu_ms */
     int kernel_launches;   /* number of this library's kernels launched by the call */
-    int cg_mode;           /* 1 = three kernels per iteration, 2 = whole solve in one cooperative launch, 3 = BiCGSTAB, 4 = even-odd CG, 5 = multi-source CG */
+    int cg_mode;           /* 1 = three kernels per iteration, 2 = whole solve in one cooperative launch (one thread per site),
+                              3 = BiCGSTAB, 4 = even-odd CG, 5 = multi-source CG, 6 = one cooperative launch with the hopping sum of
+                              a site split over four warps, 7 = even-odd BiCGSTAB */
 } wd_cg_info;
 
 /*
@@ -213,7 +215,7 @@ int bicgstab_solve(wd_ctx *ctx, const void *U_native, const void *eta_native, vo
  *       cg_solve_eo, then psi_o = eta_o + kappa H_oe psi_e.  Per iteration: two plain half-lattice hops to the odd sites,
  *       the two hops back fused with the diagonal term and the dot products of the BiCGSTAB passes (<rhat,v>; <t,s>,
  *       <t,t>), three half-length vector kernels.  Arguments as cg_solve_eo; returns WD_OK, WD_NOT_CONVERGED,
- *       WD_BREAKDOWN or an error; info->cg_mode = 5.  Synchronous.
+ *       WD_BREAKDOWN or an error; info->cg_mode = 7.  Synchronous.
  * Errors: WD_ERR_DIMS for an odd extent, WD_ERR_ARG (NULL, aliasing, 12-real links selected), WD_ERR_CUDA, WD_ERR_ALLOC.
  */
 size_t wd_eo_spinor_bytes(wd_ctx *ctx);
@@ -306,9 +308,12 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *                             software-pipelined, 1 if also compiled for precision 64}.
  *   wd_set_tile(ctx, i)       select tile i for the stencil kernels of this ctx; i = -1 restores the automatic choice.
  *   wd_get_tile(ctx)          index in use.
- *   wd_set_cg_mode(ctx, m)        0 = automatic (one cooperative launch for the whole solve when V <= 65536 sites in fp32 /
- *                             32768 in fp64 — the paper's own 4^4..14^4 range — else three kernels per iteration), 1 = always three kernels,
- *                             2 = always one launch (grid barriers between the phases; same recurrence and precision).
+ *   wd_set_cg_mode(ctx, m)        0 = automatic (one cooperative launch for the whole solve when V <= 200000 sites in fp32 /
+ *                             32768 in fp64 — this covers the paper's own 4^4..14^4 range — else three kernels per iteration),
+ *                             1 = always three kernels, 2 = always one launch, one thread per site (grid barriers between the
+ *                             phases; same recurrence and precision), 6 = always one launch with a CTA of 32 sites x 4
+ *                             directions: warp mu computes the two hops of direction mu, the partial sums meet in shared
+ *                             memory (the automatic choice in fp64 up to 8192 sites).
  *   wd_set_prefetch(ctx, n)       L2 bulk-prefetch distance of the stencil kernels in tiles: 0 = off (default: it measured
  *                             slower on B200), -1 = each CTA prefetches the tile it will process next, n > 0 = n tiles ahead.
  *   wd_set_waves(ctx, w)          the stencil kernels run a persistent grid of w * (SMs * resident CTAs per SM) CTAs that

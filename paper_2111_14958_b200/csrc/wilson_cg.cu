@@ -2,6 +2,7 @@
 // Every arithmetic step runs in the kernels of wilson_kernels.cuh; this file only sizes grids,
 // enqueues launches on the caller's stream and polls the device stop flag.
 #include "wilson_ctx.cuh"
+#include "wilson_split.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -11,9 +12,18 @@
 
 using namespace wd;
 
-// Largest volume solved by the one-launch CG kernel in automatic mode (sites).  Measured on B200 (profiles/).
-#ifndef WD_ONELAUNCH_MAX_SITES
-#define WD_ONELAUNCH_MAX_SITES 65536
+// Largest volumes solved by the one-launch CG kernels in automatic mode (sites).  Measured on B200 (near-identity links,
+// ms per solve, three kernels / one launch): fp32 16^4 3.48 / 3.00, 20^4 7.50 / 6.49, 24^4 13.27 / 14.06; fp64 12^4
+// 5.50 / 4.14, 16^4 9.08 / 10.36.  The split kernel (hopping sum over four warps) wins in fp64 at 4^4 and 8^4 (0.65 / 2.58
+// -> 0.49 / 1.76 ms) and loses from 12^4 on.
+#ifndef WD_ONELAUNCH_MAX_SITES_F32
+#define WD_ONELAUNCH_MAX_SITES_F32 200000
+#endif
+#ifndef WD_ONELAUNCH_MAX_SITES_F64
+#define WD_ONELAUNCH_MAX_SITES_F64 32768
+#endif
+#ifndef WD_SPLIT_MAX_SITES_F64
+#define WD_SPLIT_MAX_SITES_F64 8192
 #endif
 
 char g_create_err[512] = "";
@@ -216,9 +226,9 @@ extern "C" int wd_set_tile(wd_ctx *c, int index)
 extern "C" int wd_get_tile(wd_ctx *c) { return c ? c->tile : WD_ERR_ARG; }
 extern "C" int wd_set_cg_mode(wd_ctx *c, int mode)
 {
-    if (!c || mode < 0 || mode > 2) return WD_ERR_ARG;
-    if (mode == 2 && !c->coop_ok) return fail(c, WD_ERR_CUDA, "wd_set_cg_mode: the device does not support cooperative launches");
-    if (mode == 2 && c->recon != 18) return fail(c, WD_ERR_ARG, "wd_set_cg_mode: the one-launch kernel needs 18-real links");
+    if (!c || mode < 0 || (mode > 2 && mode != 6)) return WD_ERR_ARG;
+    if (mode >= 2 && !c->coop_ok) return fail(c, WD_ERR_CUDA, "wd_set_cg_mode: the device does not support cooperative launches");
+    if (mode >= 2 && c->recon != 18) return fail(c, WD_ERR_ARG, "wd_set_cg_mode: the one-launch kernels need 18-real links");
     c->cg_mode = mode;
     return WD_OK;
 }
@@ -412,28 +422,47 @@ static int small_tile_for(const wd_ctx *c)
     return best;
 }
 
+static int split_tile_for(const wd_ctx *c)
+{
+    int best = 0;
+    double best_waste = 1e300;
+    for (int t = 0; t < WD_NUM_SPLIT_TILES; ++t) {
+        double blocks = 1.0;
+        for (int d = 0; d < 4; ++d) blocks *= (c->dims[d] + kSplitTiles[t][d] - 1) / kSplitTiles[t][d];
+        const double waste = blocks * 32.0 / (double)c->V;
+        if (waste < best_waste - 1e-12) { best_waste = waste; best = t; }
+    }
+    return best;
+}
+
 static bool use_onelaunch(const wd_ctx *c)
 {
-    if (!c->coop_ok || c->recon != 18) return false;   // the one-launch kernel is compiled for 18-real links only
+    if (!c->coop_ok || c->recon != 18) return false;   // the one-launch kernels are compiled for 18-real links only
     if (c->cg_mode == 1) return false;
-    if (c->cg_mode == 2) return true;
-    // automatic: volumes whose CG iteration is shorter than three launches (measured crossover on B200: between
-    // 16^4 and 24^4 in fp32, between 14^4 and 16^4 in fp64)
-    return (long)c->V * (c->precision == 64 ? 2 : 1) <= WD_ONELAUNCH_MAX_SITES;
+    if (c->cg_mode >= 2) return true;
+    // automatic: volumes whose CG iteration is shorter than three launches (measured crossovers above)
+    return c->V <= (c->precision == 64 ? WD_ONELAUNCH_MAX_SITES_F64 : WD_ONELAUNCH_MAX_SITES_F32);
+}
+
+static bool use_split(const wd_ctx *c)
+{
+    return c->cg_mode == 6 || (c->cg_mode == 0 && c->precision == 64 && c->V <= WD_SPLIT_MAX_SITES_F64);
 }
 
 static int cg_onelaunch(wd_ctx *c, const void *U, const void *eta, void *psi, double kappa, double r_min, int max_iter)
 {
-    const int st = small_tile_for(c);
+    const bool split = use_split(c);
+    const int st = split ? split_tile_for(c) : small_tile_for(c);
     CgOneLaunchArgs a;
-    a.g = make_geom_dims(c, kSmallTiles[st], 0);
+    a.g = make_geom_dims(c, split ? kSplitTiles[st] : kSmallTiles[st], 0);
     a.sm_count = c->sm_count;
     a.stream = c->stream;
     a.U = U; a.eta = eta; a.y = c->y; a.r = c->r; a.p = c->p; a.q = c->q; a.psi = psi;
     a.kappa = kappa; a.sc = c->sc; a.partials = c->partials; a.partials_cap = c->partials_cap; a.hist = c->hist;
     a.r_min = r_min; a.max_iter = max_iter;
     c->launches++;
-    CUDA_TRY(c, c->precision == 32 ? launch_cg_onelaunch_f32(st, a) : launch_cg_onelaunch_f64(st, a));
+    if (split) CUDA_TRY(c, c->precision == 32 ? launch_cg_split_f32(st, a) : launch_cg_split_f64(st, a));
+    else CUDA_TRY(c, c->precision == 32 ? launch_cg_onelaunch_f32(st, a) : launch_cg_onelaunch_f64(st, a));
     return WD_OK;
 }
 
@@ -443,7 +472,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
     int rc = wd_ensure_workspace(c, max_iter);
     if (rc != WD_OK) return rc;
     if (use_onelaunch(c)) {
-        c->last_cg_mode = 2;
+        c->last_cg_mode = use_split(c) ? 6 : 2;
         if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
         rc = cg_onelaunch(c, U, eta, psi, kappa, r_min, max_iter);
         if (rc != WD_OK) return rc;
@@ -462,7 +491,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
             info->gpu_ms = ms;
             info->total_ms = ms;
             info->kernel_launches = c->launches;
-            info->cg_mode = 2;
+            info->cg_mode = c->last_cg_mode;
         }
         return s1.converged ? WD_OK : WD_NOT_CONVERGED;
     }

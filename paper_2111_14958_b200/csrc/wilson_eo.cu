@@ -464,7 +464,7 @@ extern "C" int bicgstab_solve_eo(wd_ctx *c, const void *U_eo, const void *eta_eo
         info->gpu_ms = ms;
         info->total_ms = ms;
         info->kernel_launches = c->launches;
-        info->cg_mode = 5;
+        info->cg_mode = 7;
     }
     return s.converged ? WD_OK : (s.breakdown ? WD_BREAKDOWN : WD_NOT_CONVERGED);
 }

@@ -1,0 +1,5 @@
+// fp64 instantiations of the split one-launch CG kernel; own translation unit for parallel builds.
+#include "wilson_split.cuh"
+namespace wd {
+cudaError_t launch_cg_split_f64(int split_tile, const CgOneLaunchArgs &a) { return launch_cg_split_any<double>(split_tile, a); }
+}  // namespace wd

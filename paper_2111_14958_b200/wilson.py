@@ -459,7 +459,8 @@ class WilsonContext:
         return {"a2_ms": ms[0], "a3_ms": ms[1], "a4_ms": ms[2], "iterations": n.value}
 
     def wd_set_cg_mode(self, mode):
-        """0 automatic, 1 three kernels per iteration, 2 whole solve in one cooperative launch"""
+        """0 automatic, 1 three kernels per iteration, 2 whole solve in one cooperative launch (thread per site), 6 one launch with
+        the hopping sum split over four warps"""
         self._check(self.lib.wd_set_cg_mode(self._ctx, int(mode)))
 
     def wd_set_gauge_recon(self, reals_per_link):

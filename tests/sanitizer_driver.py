@@ -37,7 +37,7 @@ def plain(dims, links, precision, kappa=0.12):
             out = ctx.wd_apply(Un, en, kappa, dag)
             assert torch.isfinite(out).all()
         assert ctx.wd_norm2(en) > 0
-        for mode in (1, 2):
+        for mode in (1, 2, 6):
             ctx.wd_set_cg_mode(mode)
             _, info = ctx.cg_solve(Un, en, kappa, r_min, 500)
             assert info["status"] == 0, info

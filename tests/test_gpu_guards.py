@@ -81,7 +81,7 @@ def test_plain_calls_stay_inside_their_buffers(wilson, dims, precision):
                 got = ctx.wd_unpack_spinor(out.t)
                 assert torch.isfinite(torch.view_as_real(got)).all(), (tile, dag)
         ctx.wd_set_tile(-1)
-        for mode in (1, 2):
+        for mode in (1, 2, 6):
             ctx.wd_set_cg_mode(mode)
             _, info = ctx.cg_solve(Un.t, en.t, kappa, r_min, 500, out=out.t)
             assert info["status"] == 0 and torch.isfinite(torch.view_as_real(ctx.wd_unpack_spinor(out.t))).all()

@@ -423,7 +423,7 @@ def test_eo_bicgstab_baseline_configs(wilson, oracle, cfg_index, precision, r_mi
         hist = ctx.wd_cg_history()
         _, plain = bicgstab_on_gpu(ctx, U, eta, cfg.kappa, r_min, cfg.max_iter)
     psi_o, info_o = oracle.bicgstab_solve_eo(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t, history=True)
-    assert info["status"] == 0 and info["converged"] == 1 and info["cg_mode"] == 5 and info_o["converged"]
+    assert info["status"] == 0 and info["converged"] == 1 and info["cg_mode"] == 7 and info_o["converged"]
     assert info["kernel_launches"] >= 7 * info["iterations"] + 1
     slack = 0 if precision == 64 else max(1, int(0.05 * info_o["iterations"] + 0.5))
     assert abs(info["iterations"] - info_o["iterations"]) <= slack, (info["iterations"], info_o["iterations"])

@@ -179,7 +179,8 @@ def test_norm2_matches_oracle_and_is_deterministic(wilson, oracle, precision):
 
 # ---------------------------------------------------------------- a1-a6: cg_solve
 def _cg_case(wilson, oracle, cfg, precision, r_min, poll=None, mode=0):
-    """mode: 0 automatic, 1 three kernels per iteration, 2 whole solve in one cooperative launch"""
+    """mode: 0 automatic, 1 three kernels per iteration, 2 whole solve in one cooperative launch (thread per site), 6 one
+    cooperative launch with the hopping sum of a site split over four warps"""
     U, eta = gu.config_fields(cfg.index, precision)
     U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
     with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
@@ -190,7 +191,7 @@ def _cg_case(wilson, oracle, cfg, precision, r_min, poll=None, mode=0):
         hist = ctx.wd_cg_history()
     if mode:
         assert info["cg_mode"] == mode
-        assert info["kernel_launches"] == 1 if mode == 2 else info["kernel_launches"] >= 3 * info["iterations"] + 2
+        assert info["kernel_launches"] == 1 if mode in (2, 6) else info["kernel_launches"] >= 3 * info["iterations"] + 2
     psi_o, info_o = oracle.cg_solve(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t, history=True)
     res_gpu = oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
     res_orc = oracle.true_residual(cfg.dims, U64, eta64, psi_o, cfg.kappa, cfg.bc_t)
@@ -210,15 +211,15 @@ def _cg_case(wilson, oracle, cfg, precision, r_min, poll=None, mode=0):
     return info, info_o, res_gpu, res_orc
 
 
-@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("mode", [1, 2, 6])
 @pytest.mark.parametrize("cfg_index", [0, 1, 2])
 def test_cg_solve_fp32_baseline_configs(wilson, oracle, cfg_index, mode):
-    """both CG drivers: three kernels per iteration (mode 1) and the one-launch cooperative kernel (mode 2)"""
+    """the CG drivers: three kernels per iteration (mode 1) and the two one-launch cooperative kernels (modes 2, 6)"""
     cfg = inputs.CONFIGS[cfg_index]
     _cg_case(wilson, oracle, cfg, 32, cfg.r_min, mode=mode)
 
 
-@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("mode", [1, 2, 6])
 @pytest.mark.parametrize("cfg_index", [0, 1, 2])
 def test_cg_solve_fp64_tight(wilson, oracle, cfg_index, mode):
     cfg = inputs.CONFIGS[cfg_index]
@@ -227,30 +228,31 @@ def test_cg_solve_fp64_tight(wilson, oracle, cfg_index, mode):
 
 def test_cg_automatic_mode_by_volume(wilson):
     """4^4 .. 14^4 (the paper's range) take the one-launch kernel, 32^4 the three-kernel loop"""
-    for ci, want in ((0, 2), (2, 2)):
+    for ci, precision, want in ((0, 32, 2), (2, 32, 2), (0, 64, 6), (1, 64, 6)):
         cfg = inputs.CONFIGS[ci]
-        U, eta = gu.config_fields(ci, 32)
-        with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+        U, eta = gu.config_fields(ci, precision)
+        with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
             _, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
         assert info["cg_mode"] == want and info["kernel_launches"] == 1
 
 
 @pytest.mark.parametrize("precision", [32, 64])
 def test_cg_onelaunch_ragged_lattice(wilson, oracle, precision):
-    """one-launch kernel on extents that no tile divides, periodic t as well"""
-    for dims, bc_t in (((6, 4, 10, 8), -1), ((5, 7, 4, 6), 1)):
+    """both one-launch kernels on extents that no tile divides, periodic t as well"""
+    for dims, bc_t in (((6, 4, 10, 8), -1), ((5, 7, 4, 6), 1), ((18, 4, 6, 4), -1)):
         cdt = gu.np_complex(precision)
         U = inputs.gauge_field(CFG_TEST + 6, dims, "near_identity", dtype=cdt)
         eta = inputs.source_field(CFG_TEST + 6, dims, dtype=cdt)
         tol = 1e-6 if precision == 32 else 1e-11
-        with wilson.WilsonContext(dims, precision, bc_t) as ctx:
-            ctx.wd_set_cg_mode(2)
-            psi, info = gu.solve_on_gpu(ctx, U, eta, 0.12, tol, 500)
         U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
         psi_o, info_o = oracle.cg_solve(dims, U64, eta64, 0.12, tol, 500, bc_t)
-        assert info["status"] == 0 and iters_close(info["iterations"], info_o["iterations"])
-        res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), 0.12, bc_t)
-        assert res <= 2.0 * oracle.true_residual(dims, U64, eta64, psi_o, 0.12, bc_t)
+        for mode in (2, 6):
+            with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+                ctx.wd_set_cg_mode(mode)
+                psi, info = gu.solve_on_gpu(ctx, U, eta, 0.12, tol, 500)
+            assert info["status"] == 0 and info["cg_mode"] == mode and iters_close(info["iterations"], info_o["iterations"])
+            res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), 0.12, bc_t)
+            assert res <= 2.0 * oracle.true_residual(dims, U64, eta64, psi_o, 0.12, bc_t)
 
 
 def test_cg_result_independent_of_poll_interval_and_repeatable(wilson):
@@ -269,6 +271,13 @@ def test_cg_result_independent_of_poll_interval_and_repeatable(wilson):
     for _ in range(3):
         with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
             ctx.wd_set_cg_mode(2)
+            psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
+            outs.append((psi.tobytes(), info["iterations"], info["rel_residual"]))
+    assert all(o == outs[0] for o in outs)
+    outs = []
+    for _ in range(3):
+        with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+            ctx.wd_set_cg_mode(6)
             psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
             outs.append((psi.tobytes(), info["iterations"], info["rel_residual"]))
     assert all(o == outs[0] for o in outs)
@@ -298,7 +307,7 @@ def test_alternating_sweep_direction(wilson, cfg_index, precision):
     assert np.linalg.norm(res[0][1] - res[1][1]) <= tol * np.linalg.norm(res[0][1])
 
 
-@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("mode", [1, 2, 6])
 def test_cg_edge_cases(wilson, oracle, mode):
     cfg = inputs.CONFIGS[0]
     U, eta = gu.config_fields(0, 64)
