@@ -283,6 +283,25 @@ def test_cg_result_independent_of_poll_interval_and_repeatable(wilson):
     assert all(o == outs[0] for o in outs)
 
 
+def test_wd_apply_repeat_is_wd_apply(wilson):
+    """the measurement aid enqueues the same launches as wd_apply: same output, a positive device time, argument checks"""
+    cfg = inputs.CONFIGS[2]
+    U, eta = gu.config_fields(2, 32)
+    with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        en = ctx.wd_pack_spinor(gu.to_device(eta))
+        for dag in (False, True):
+            want = gu.to_host(ctx.wd_unpack_spinor(ctx.wd_apply(Un, en, cfg.kappa, dag)))
+            out = ctx.empty_spinor()
+            ms = ctx.wd_apply_repeat(Un, en, cfg.kappa, dag, reps=20, out=out)
+            assert 0.0 < ms < 1.0
+            assert np.array_equal(gu.to_host(ctx.wd_unpack_spinor(out)), want)
+        with pytest.raises(wilson.WilsonError):
+            ctx.wd_apply_repeat(Un, en, cfg.kappa, False, reps=0)
+        with pytest.raises(wilson.WilsonError):
+            ctx.wd_apply_repeat(Un, en, cfg.kappa, False, reps=3, out=en)
+
+
 @pytest.mark.parametrize("cfg_index,precision", [(1, 32), (2, 64)])
 def test_alternating_sweep_direction(wilson, cfg_index, precision):
     """wd_set_sweep(1): passes walk the tiles backwards and forwards in turn.  Per-site arithmetic is unchanged, so
