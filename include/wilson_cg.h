@@ -203,7 +203,8 @@ int bicgstab_solve(wd_ctx *ctx, const void *U_native, const void *eta_native, vo
  * |r|^2), one fused axpy-xpay.
  *
  * Checkerboard ("eo") native layouts: two halves, even parity first; inside a half the site index is (lexicographic
- * index)/2 and the data is blocked exactly like the plain native layout.  18-real links only.
+ * index)/2 and the data is blocked exactly like the plain native layout.  With wd_set_gauge_recon(ctx, 12) selected
+ * BEFORE wd_eo_gauge_bytes / wd_eo_pack_gauge the links are stored as 12 reals and every even-odd call below uses them.
  *   wd_eo_spinor_bytes / wd_eo_gauge_bytes   sizes of the device buffers the caller allocates.
  *   wd_eo_pack_spinor / wd_eo_unpack_spinor / wd_eo_pack_gauge   permutations canonical <-> eo native (device pointers).
  *   wd_eo_hop(ctx, U_eo, in_eo, out_eo, out_parity, dagger)   out(x) = sum over the 8 hops (H in)(x) (H-dagger for
@@ -216,7 +217,7 @@ int bicgstab_solve(wd_ctx *ctx, const void *U_native, const void *eta_native, vo
  *       the two hops back fused with the diagonal term and the dot products of the BiCGSTAB passes (<rhat,v>; <t,s>,
  *       <t,t>), three half-length vector kernels.  Arguments as cg_solve_eo; returns WD_OK, WD_NOT_CONVERGED,
  *       WD_BREAKDOWN or an error; info->cg_mode = 7.  Synchronous.
- * Errors: WD_ERR_DIMS for an odd extent, WD_ERR_ARG (NULL, aliasing, 12-real links selected), WD_ERR_CUDA, WD_ERR_ALLOC.
+ * Errors: WD_ERR_DIMS for an odd extent, WD_ERR_ARG (NULL, aliasing), WD_ERR_CUDA, WD_ERR_ALLOC.
  */
 size_t wd_eo_spinor_bytes(wd_ctx *ctx);
 size_t wd_eo_gauge_bytes(wd_ctx *ctx);

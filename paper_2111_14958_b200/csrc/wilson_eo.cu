@@ -29,14 +29,13 @@ EoDims eo_dims(const wd_ctx *c)
     return e;
 }
 size_t half_spinor_bytes(const wd_ctx *c) { return 24 * eo_dims(c).Vh_pad * real_bytes(c); }
-size_t half_gauge_bytes(const wd_ctx *c) { return 72 * eo_dims(c).Vh_pad * real_bytes(c); }
+size_t half_gauge_bytes(const wd_ctx *c) { return (size_t)(c->recon == 12 ? 48 : 72) * eo_dims(c).Vh_pad * real_bytes(c); }
 size_t half_spinor_vecs(const wd_ctx *c) { return (size_t)(c->precision == 32 ? 6 : 12) * eo_dims(c).Vh_pad; }
 
 int eo_check(wd_ctx *c, const char *who)
 {
     for (int d = 0; d < 4; ++d)
         if (c->dims[d] & 1) return fail(c, WD_ERR_DIMS, "%s: extent %d of direction %d is odd (even-odd needs even extents)", who, c->dims[d], d);
-    if (c->recon != 18) return fail(c, WD_ERR_ARG, "%s: the even-odd path stores 18-real links (wd_set_gauge_recon)", who);
     return WD_OK;
 }
 
@@ -74,7 +73,7 @@ eo_unpack_spinor_kernel(const typename Field<real>::svec *__restrict__ nat, type
 #pragma unroll
     for (int j = 0; j < NSP; ++j) can[(size_t)s * NSP + j] = __ldg(p + j * SB);
 }
-template <typename real>
+template <typename real, int RECON>
 __global__ void __launch_bounds__(VEC_NT)
 eo_pack_gauge_kernel(const typename Field<real>::gvec *__restrict__ can, typename Field<real>::gvec *nat, int V, int L0,
                      int L1, int L2, size_t half_cplx)
@@ -87,7 +86,8 @@ eo_pack_gauge_kernel(const typename Field<real>::gvec *__restrict__ can, typenam
         gvec k9[9];
 #pragma unroll
         for (int k = 0; k < 9; ++k) k9[k] = __ldg(can + (size_t)s * 36 + mu * 9 + k);
-        store_link(half, s >> 1, mu, k9);
+        if (RECON == 12) store_link12(half, s >> 1, mu, k9);
+        else store_link(half, s >> 1, mu, k9);
     }
 }
 
@@ -130,6 +130,8 @@ cudaError_t eo_launch(wd_ctx *c, const void *U_eo, const EoPass &p)
     a.sc = (p.mode != MODE_PLAIN || p.in_loop) ? c->sc : nullptr;
     a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = p.it;
     c->launches++;
+    if (c->recon == 12)
+        return c->precision == 32 ? launch_dslash12_eo_f32(tile, p.dagger, p.mode, a) : launch_dslash12_eo_f64(tile, p.dagger, p.mode, a);
     if (p.mode == MODE_RV || p.mode == MODE_TS)
         return c->precision == 32 ? launch_dslash_eo_bi_f32(tile, p.mode, a) : launch_dslash_eo_bi_f64(tile, p.mode, a);
     return c->precision == 32 ? launch_dslash_eo_f32(tile, p.dagger, p.mode, a) : launch_dslash_eo_f64(tile, p.dagger, p.mode, a);
@@ -187,13 +189,16 @@ extern "C" int wd_eo_pack_gauge(wd_ctx *c, const void *can, void *nat)
     const EoDims e = eo_dims(c);
     if (e.Vh_pad != (size_t)e.Vh) CUDA_TRY(c, cudaMemsetAsync(nat, 0, 2 * half_gauge_bytes(c), c->stream));
     const unsigned int grid = (c->V + VEC_NT - 1) / VEC_NT;
-    const size_t half_cplx = 36 * e.Vh_pad;
-    if (c->precision == 32)
-        eo_pack_gauge_kernel<float><<<grid, VEC_NT, 0, c->stream>>>((const float2 *)can, (float2 *)nat, c->V, c->dims[0],
-                                                                   c->dims[1], c->dims[2], half_cplx);
+    const size_t half_cplx = (size_t)(c->recon == 12 ? 24 : 36) * e.Vh_pad;   // complex slots per parity
+    const int d0 = c->dims[0], d1 = c->dims[1], d2 = c->dims[2];
+    if (c->precision == 32 && c->recon == 18)
+        eo_pack_gauge_kernel<float, 18><<<grid, VEC_NT, 0, c->stream>>>((const float2 *)can, (float2 *)nat, c->V, d0, d1, d2, half_cplx);
+    else if (c->precision == 32)
+        eo_pack_gauge_kernel<float, 12><<<grid, VEC_NT, 0, c->stream>>>((const float2 *)can, (float2 *)nat, c->V, d0, d1, d2, half_cplx);
+    else if (c->recon == 18)
+        eo_pack_gauge_kernel<double, 18><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V, d0, d1, d2, half_cplx);
     else
-        eo_pack_gauge_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V, c->dims[0],
-                                                                    c->dims[1], c->dims[2], half_cplx);
+        eo_pack_gauge_kernel<double, 12><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)can, (double2 *)nat, c->V, d0, d1, d2, half_cplx);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
     return WD_OK;

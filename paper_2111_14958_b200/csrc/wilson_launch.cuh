@@ -111,6 +111,9 @@ cudaError_t launch_dslash12_f64(int tile, int dagger, int mode, const DslashArgs
 // one parity of the lattice (even-odd preconditioning; a.g.eo = 1)
 cudaError_t launch_dslash_eo_f32(int tile, int dagger, int mode, const DslashArgs &a);
 cudaError_t launch_dslash_eo_f64(int tile, int dagger, int mode, const DslashArgs &a);
+// one parity with 12-real links; mode in {MODE_PLAIN, MODE_QQ, MODE_RUPD, MODE_RV, MODE_TS}
+cudaError_t launch_dslash12_eo_f32(int tile, int dagger, int mode, const DslashArgs &a);
+cudaError_t launch_dslash12_eo_f64(int tile, int dagger, int mode, const DslashArgs &a);
 // BiCGSTAB passes (D only): mode in {MODE_RV, MODE_TS}
 cudaError_t launch_dslash_bi_f32(int tile, int mode, const DslashArgs &a);
 cudaError_t launch_dslash_bi_f64(int tile, int mode, const DslashArgs &a);

@@ -153,6 +153,15 @@ def test_even_odd_calls_stay_inside_their_buffers(wilson, dims, precision):
         assert info["status"] == 0 and torch.isfinite(torch.view_as_real(ctx.wd_eo_unpack_spinor(pe.t))).all()
         can = Guarded(torch.view_as_real(gu.to_device(eta)).reshape(-1))
         ctx._check(ctx.lib.wd_eo_unpack_spinor(ctx._ctx, ctx._p(pe.t), ctx._p(can.t)))
+        # the same on 12-real links
+        ctx.wd_set_gauge_recon(12)
+        U12 = Guarded(ctx.empty_eo_gauge())
+        ctx._check(ctx.lib.wd_eo_pack_gauge(ctx._ctx, ctx._p(Uc.t), ctx._p(U12.t)))
+        assert torch.isfinite(U12.t).all()
+        _, info = ctx.cg_solve_eo(U12.t, ee.t, kappa, r_min, 500, out=pe.t)
+        assert info["status"] == 0 and torch.isfinite(torch.view_as_real(ctx.wd_eo_unpack_spinor(pe.t))).all()
+        _, info = ctx.bicgstab_solve_eo(U12.t, ee.t, kappa, r_min, 500, out=pe.t)
+        assert info["status"] == 0 and torch.isfinite(torch.view_as_real(ctx.wd_eo_unpack_spinor(pe.t))).all()
         torch.cuda.synchronize()
-        assert all_intact(Uc, ec, Ue, ee, pe, tmp, can)
+        assert all_intact(Uc, ec, Ue, ee, pe, tmp, can, U12)
         assert torch.equal(ec.t, torch.view_as_real(gu.to_device(eta)).reshape(-1))

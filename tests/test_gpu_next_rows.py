@@ -497,10 +497,6 @@ def test_eo_bicgstab_edge_cases(wilson, oracle):
             ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, 0.0, 10)
         with pytest.raises(wilson.WilsonError):
             ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, 1e-6, 10, out=ee)
-    with wilson.WilsonContext(cfg.dims, 32) as ctx:
-        ctx.wd_set_gauge_recon(12)
-        with pytest.raises(wilson.WilsonError):
-            ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, 1e-6, 10)
 
 
 @pytest.mark.parametrize("precision", [32, 64])
@@ -518,6 +514,43 @@ def test_eo_bicgstab_32_4_closed_form(wilson, precision):
     assert info["status"] == 0
     err = np.linalg.norm(psi - want) / np.linalg.norm(want)
     assert err < (2e-5 if precision == 32 else 1e-9), err
+
+
+# ---------------------------------------------------------------- f3 composed: even-odd solvers on 12-real links
+@pytest.mark.parametrize("precision,r_min", [(32, 1e-6), (64, 1e-10)])
+@pytest.mark.parametrize("cfg_index", [0, 1, 2])
+def test_eo_solvers_with_12_real_links(wilson, oracle, cfg_index, precision, r_min):
+    """wd_set_gauge_recon(12) before wd_eo_pack_gauge: hop, even-odd CG and even-odd BiCGSTAB against the oracle"""
+    cfg = inputs.CONFIGS[cfg_index]
+    U, eta = gu.config_fields(cfg.index, precision)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    par = _parity(cfg.dims)
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        n18 = ctx.empty_eo_gauge().numel()
+        ctx.wd_set_gauge_recon(12)
+        Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
+        assert Ue.numel() * 3 == n18 * 2
+        ee = ctx.wd_eo_pack_spinor(gu.to_device(eta))
+        out = ctx.wd_eo_pack_spinor(gu.to_device(np.zeros_like(eta)))
+        for p in (0, 1):
+            ctx.wd_eo_hop(Ue, ee, out, p, False)
+        hop = gu.to_host(ctx.wd_eo_unpack_spinor(out))
+        pc, ic = ctx.cg_solve_eo(Ue, ee, cfg.kappa, r_min, cfg.max_iter)
+        psi_c = gu.to_host(ctx.wd_eo_unpack_spinor(pc))
+        pb, ib = ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, r_min, cfg.max_iter)
+        psi_b = gu.to_host(ctx.wd_eo_unpack_spinor(pb))
+    # H eta = (eta - D eta) / kappa at every site (both parities were written)
+    want = (eta64 - oracle.wd_apply(cfg.dims, U64, eta64, cfg.kappa, False, cfg.bc_t)) / cfg.kappa
+    err, _ = lm.per_site_rel_err(hop, want)
+    assert err <= (1e-5 if precision == 32 else 1e-12), err
+    _, ioc = oracle.cg_solve_eo(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t)
+    _, iob = oracle.bicgstab_solve_eo(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t)
+    assert ic["status"] == 0 and abs(ic["iterations"] - ioc["iterations"]) <= math.floor(0.02 * ioc["iterations"] + 0.5)
+    slack = 0 if precision == 64 else max(1, int(0.05 * iob["iterations"] + 0.5))
+    assert ib["status"] == 0 and abs(ib["iterations"] - iob["iterations"]) <= slack
+    for psi in (psi_c, psi_b):
+        assert oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t) < 2.0 * r_min
+    assert par.size == psi_c.shape[0]
 
 
 # ---------------------------------------------------------------- full BASELINE sizes (configs 3 and 4)
