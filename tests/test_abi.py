@@ -46,6 +46,11 @@ def test_argument_errors_without_touching_a_gpu(lib):
     bad = (ctypes.c_int * 4)(4, 4, 2, 4)
     assert lib.wd_create(ctypes.byref(ctx), bad, 32, -1, None) == -2  # WD_ERR_DIMS
     assert b"extent" in lib.wd_last_error(None)
+    # 36 V must stay below 2^31 (32-bit plane indexing): 96^2 x 64 x 96 is the largest lattice of that shape family
+    # (tests/test_gpu_parity.py::test_largest_supported_volume runs it), one more z-slab of 32 is refused
+    big = (ctypes.c_int * 4)(96, 96, 96, 96)
+    assert lib.wd_create(ctypes.byref(ctx), big, 32, -1, None) == -2
+    assert b"too large" in lib.wd_last_error(None)
     ok = (ctypes.c_int * 4)(4, 4, 4, 4)
     assert lib.wd_create(ctypes.byref(ctx), ok, 16, -1, None) == -5   # WD_ERR_PRECISION
     assert lib.wd_create(ctypes.byref(ctx), ok, 32, 0, None) == -1    # WD_ERR_ARG

@@ -163,6 +163,37 @@ def test_wd_apply_32_4_sampled_sites(wilson, oracle, precision):
             assert lm.per_site_rel_err(got, want)[0] <= TOL_APPLY[precision]
 
 
+def test_largest_supported_volume(wilson, oracle):
+    """96^2 x 64 x 96 = 56.6 M sites: 36 V = 2.04e9 is just below the 2^31 limit of the 32-bit plane indexing that
+    wd_create enforces (16 GB of links, 5.4 GB per spinor in fp32).  wd_apply D and D-dagger at sampled sites, among them
+    the last sites of the lattice (largest indices) and its corners, one by one against the oracle; then the whole
+    cg_solve, its true residual evaluated by the oracle's fp64 D on the full lattice."""
+    dims, kappa, r_min = (96, 96, 64, 96), 0.124, 1e-6
+    V = int(np.prod(dims))
+    assert 0.94 * 2 ** 31 < 36 * V < 2 ** 31
+    U = inputs.gauge_field(CFG_TEST + 9, dims, "near_identity", dtype=np.complex64)
+    eta = inputs.source_field(CFG_TEST + 9, dims, dtype=np.complex64)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    rng = np.random.Generator(np.random.PCG64(7))
+    lx, ly, lz, lt = dims
+    edge = [0, lx - 1, lx, V - 1, V - 2, V - lx, lx * ly * lz * (lt - 1), lx * ly * lz - 1, lx * ly - 1, V // 2, V - 17]
+    sites = np.unique(np.concatenate([edge, rng.choice(V, 3000, replace=False)])).astype(np.int64)
+    with wilson.WilsonContext(dims, 32, -1) as ctx:
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        en = ctx.wd_pack_spinor(gu.to_device(eta))
+        for dagger in (False, True):
+            got = gu.to_host(ctx.wd_unpack_spinor(ctx.wd_apply(Un, en, kappa, dagger))[gu.to_device(sites)])
+            want = oracle.wd_apply_sites(dims, U64, eta64, kappa, sites, dagger, -1)
+            assert lm.per_site_rel_err(got, want)[0] <= TOL_APPLY[32]
+        psi_n, info = ctx.cg_solve(Un, en, kappa, r_min, 5000)
+        psi = gu.to_host(ctx.wd_unpack_spinor(psi_n))
+        del Un, en, psi_n
+    assert info["status"] == 0 and info["cg_mode"] == 1 and 50 < info["iterations"] < 400
+    res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), kappa, -1)
+    assert res < 2.0 * r_min, res
+    assert abs(info["eta_norm2"] / (24.0 * V) - 1.0) < 1e-3        # pin P9 at this size
+
+
 # ---------------------------------------------------------------- reductions
 @pytest.mark.parametrize("precision", [32, 64])
 def test_norm2_matches_oracle_and_is_deterministic(wilson, oracle, precision):
