@@ -10,9 +10,10 @@
 //     fused into the stencil passes: MODE_QQ produces |D-dagger p|^2 and alpha, MODE_RUPD applies
 //     r <- r - alpha D q and produces |r|^2, beta and the loop condition, all in device memory.
 //
-// Data layout (include/wilson_cg.h "Native layouts"): site-blocked SoA.  Blocks of 32 lexicographic sites;
+// Data layout (include/wilson_cg.h "Native layouts"): site-blocked SoA.  Blocks of 16 lexicographic sites;
 // inside a block a spinor is NSP planes of 128-bit vectors (float4 = two complex components, double2 = one)
-// and the 4 links are 36 planes of one complex each.  One thread owns one site; a CTA owns a
+// and each of the 4 links occupies 9 complex slots per site (fp32: four float4 planes and one float2 plane; 12-real
+// storage: 6 slots).  One thread owns one site; a CTA owns a
 // BX x BY x BZ x BT tile so that the 8 neighbours of most sites are fetched by the same CTA (L1 reuse) and
 // all loads of a warp are contiguous runs of BX sites.
 #pragma once
