@@ -310,7 +310,7 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *   wd_set_tile(ctx, i)       select tile i for the stencil kernels of this ctx; i = -1 restores the automatic choice.
  *   wd_get_tile(ctx)          index in use.
  *   wd_set_cg_mode(ctx, m)        0 = automatic (one cooperative launch for the whole solve when V <= 200000 sites in fp32 /
- *                             32768 in fp64 — this covers the paper's own 4^4..14^4 range — else three kernels per iteration),
+ *                             65536 in fp64 — this covers the paper's own 4^4..14^4 range — else three kernels per iteration),
  *                             1 = always three kernels, 2 = always one launch, one thread per site (grid barriers between the
  *                             phases; same recurrence and precision), 6 = always one launch with a CTA of 32 sites x 4
  *                             directions: warp mu computes the two hops of direction mu, the partial sums meet in shared
@@ -321,6 +321,8 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *                             stride over the tiles; w = 0 or 1: exactly one resident wave (default).
  *   wd_set_zchunk(ctx, layers)    z extent (in sites) of one chunk of the CTA rasterisation x,y,z-in-chunk,t,z-chunk that
  *                             keeps the +-t neighbours of a tile in L2; 0 = automatic (fits a 40 MB reuse distance).
+ *   wd_set_small_tile(ctx, i)     launch configuration (CTA tile, register bound) of the one-launch CG kernel of mode 2:
+ *                             -1 = automatic (default), 0 <= i < number of compiled configurations.
  *   wd_set_sweep(ctx, a)          a = 1: consecutive passes over the lattice (the three kernels of a cg_solve iteration,
  *                             back-to-back wd_apply calls) walk it in alternating directions, so that each pass starts on
  *                             the data the previous one left in the 126 MB L2; a = 0 (default: the alternation measured no
@@ -338,6 +340,7 @@ int wd_set_prefetch(wd_ctx *ctx, int tiles);
 int wd_set_waves(wd_ctx *ctx, int waves);
 int wd_set_zchunk(wd_ctx *ctx, int layers);
 int wd_set_sweep(wd_ctx *ctx, int alternate);
+int wd_set_small_tile(wd_ctx *ctx, int index);
 int wd_set_poll_interval(wd_ctx *ctx, int n);
 
 /*

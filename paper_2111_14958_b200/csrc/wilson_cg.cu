@@ -13,14 +13,14 @@
 using namespace wd;
 
 // Largest volumes solved by the one-launch CG kernels in automatic mode (sites).  Measured on B200 (near-identity links,
-// ms per solve, three kernels / one launch): fp32 16^4 3.48 / 3.00, 20^4 7.50 / 6.49, 24^4 13.27 / 14.06; fp64 12^4
-// 5.50 / 4.14, 16^4 9.08 / 10.36.  The split kernel (hopping sum over four warps) wins in fp64 at 4^4 and 8^4 (0.65 / 2.58
+// ms per solve, three kernels / one launch with the launch configuration small_tile_for picks): fp32 16^4 3.48 / 2.23,
+// 20^4 7.50 / 6.4, 24^4 13.27 / 14.06; fp64 12^4 5.50 / 3.77, 16^4 9.08 / 8.4, 20^4 24.3 / 26.7.  The split kernel (hopping sum over four warps) wins in fp64 at 4^4 and 8^4 (0.65 / 2.58
 // -> 0.49 / 1.76 ms) and loses from 12^4 on.
 #ifndef WD_ONELAUNCH_MAX_SITES_F32
 #define WD_ONELAUNCH_MAX_SITES_F32 200000
 #endif
 #ifndef WD_ONELAUNCH_MAX_SITES_F64
-#define WD_ONELAUNCH_MAX_SITES_F64 32768
+#define WD_ONELAUNCH_MAX_SITES_F64 65536
 #endif
 #ifndef WD_SPLIT_MAX_SITES_F64
 #define WD_SPLIT_MAX_SITES_F64 8192
@@ -144,6 +144,7 @@ extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_
     c->tile_user = -1;
     c->tile = auto_tile(c);
     c->l2_budget_mb = 40.0;
+    c->small_tile_user = -1;
     c->sweep = 0;      // measured on B200: alternating the walk direction gains nothing
     c->prefetch = 0;   // measured on B200: bulk L2 prefetch of the next tile slows the stencil by 15-30 %
     bool ok = true;
@@ -261,6 +262,12 @@ extern "C" int wd_set_zchunk(wd_ctx *c, int layers)
 {
     if (!c || layers < 0) return WD_ERR_ARG;
     c->zchunk_user = layers;
+    return WD_OK;
+}
+extern "C" int wd_set_small_tile(wd_ctx *c, int index)
+{
+    if (!c || index < -1 || index >= WD_NUM_SMALL_TILES) return WD_ERR_ARG;
+    c->small_tile_user = index;
     return WD_OK;
 }
 extern "C" int wd_set_sweep(wd_ctx *c, int alternate)
@@ -408,16 +415,25 @@ static int auto_poll(const wd_ctx *c)
 // Small-volume path: the whole solve in one cooperative launch.
 static int small_tile_for(const wd_ctx *c)
 {
+    if (c->small_tile_user >= 0) return c->small_tile_user;
+    // modelled time of a phase = rounds of tiles x cost of the row per round (x a mild penalty for threads hanging
+    // over the lattice); rounds = ceil(tiles / co-resident CTAs), co-resident CTAs per SM = the row's register bound, or
+    // what 255 registers allow (4 CTAs of 64 threads, 2 of 128).  E.g. 14^4: 16x2x2x2 needs 343 CTAs, 296 fit at 255
+    // registers (two rounds), 444 at 168 registers (one round): the bounded row wins, 0.61 -> 0.51 ms per solve.
     int best = 0;
-    double best_waste = 1e300;
+    double best_cost = 1e300;
     for (int t = 0; t < WD_NUM_SMALL_TILES; ++t) {
         double blocks = 1.0, threads = 1.0;
         for (int d = 0; d < 4; ++d) {
             blocks *= (c->dims[d] + kSmallTiles[t][d] - 1) / kSmallTiles[t][d];
             threads *= kSmallTiles[t][d];
         }
+        const int occ = kSmallMinb[t] > 1 ? kSmallMinb[t] : (threads <= 64 ? 4 : 2);
+        const double resident = (double)occ * c->sm_count;
+        const double rounds = std::ceil(blocks / resident);
         const double waste = blocks * threads / (double)c->V;
-        if (waste < best_waste - 1e-12) { best_waste = waste; best = t; }
+        const double cost = rounds * kSmallCost[t] * (1.0 + 0.1 * (waste - 1.0));
+        if (cost < best_cost - 1e-12) { best_cost = cost; best = t; }
     }
     return best;
 }

@@ -23,6 +23,7 @@ struct wd_ctx {
     int last_cg_mode;     // what the last cg_solve used
     int prefetch;         // L2 prefetch distance: -1 = automatic (one grid ahead), 0 = off, n > 0 = n tiles
     int zchunk_user;      // z layers per rasterisation chunk, 0 = automatic
+    int small_tile_user;  // launch configuration of the one-launch CG kernel: -1 = automatic
     int sweep;            // 1: consecutive passes walk the lattice in alternating directions (Geom.rev); 0 (default): all forward
     unsigned apply_calls; // wd_apply calls so far (their direction alternates too)
     double l2_budget_mb;  // reuse-distance budget of the automatic choice

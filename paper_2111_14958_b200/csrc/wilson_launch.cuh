@@ -43,8 +43,14 @@
     Y(1, 8, 4, 2, 1, 1, 0) \
     Y(2, 16, 2, 2, 1, 1, 0) \
     Y(3, 16, 2, 2, 2, 1, 0) \
-    Y(4, 8, 4, 2, 2, 1, 0)
-#define WD_NUM_SMALL_TILES 5
+    Y(4, 8, 4, 2, 2, 1, 0) \
+    Y(5, 16, 2, 2, 1, 5, 0) \
+    Y(6, 16, 2, 2, 2, 3, 0) \
+    Y(7, 8, 4, 2, 1, 5, 0) \
+    Y(8, 4, 4, 2, 2, 5, 0) \
+    Y(9, 16, 2, 2, 1, 6, 1) \
+    Y(10, 16, 2, 2, 2, 4, 1)
+#define WD_NUM_SMALL_TILES 11
 
 namespace wd {
 
@@ -63,6 +69,15 @@ static const int kSmallTiles[WD_NUM_SMALL_TILES][4] = {
     WD_SMALL_TABLE(Y)
 #undef Y
 };
+// register bound (MINB) of each row, and its measured relative cost per round of tiles (B200, 4^4 ... 20^4, both
+// precisions): 128-thread CTAs with x runs of 16 sites are the cheapest, 4-site x runs and the
+// register-bounded / pipelined rows the dearest
+static const int kSmallMinb[WD_NUM_SMALL_TILES] = {
+#define Y(i, a, b, c, d, m, p) m,
+    WD_SMALL_TABLE(Y)
+#undef Y
+};
+static const double kSmallCost[WD_NUM_SMALL_TILES] = {1.10, 1.00, 1.00, 0.93, 1.02, 1.25, 1.19, 1.25, 1.40, 1.90, 1.93};
 
 struct CgOneLaunchArgs {
     Geom g;            // nt / ntiles / fast-division constants for the chosen small tile

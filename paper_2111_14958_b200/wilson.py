@@ -114,6 +114,7 @@ def load_library(path: str = LIB_PATH):
     lib.wd_set_waves.argtypes = [vp, ci]
     lib.wd_set_zchunk.argtypes = [vp, ci]
     lib.wd_set_sweep.argtypes = [vp, ci]
+    lib.wd_set_small_tile.argtypes = [vp, ci]
     lib.wd_set_poll_interval.argtypes = [vp, ci]
     lib.wd_set_profile.argtypes = [vp, ci]
     lib.wd_get_profile.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_long)]
@@ -478,6 +479,9 @@ class WilsonContext:
 
     def wd_set_zchunk(self, layers):
         self._check(self.lib.wd_set_zchunk(self._ctx, int(layers)))
+
+    def wd_set_small_tile(self, index):
+        self._check(self.lib.wd_set_small_tile(self._ctx, int(index)))
 
     def wd_set_sweep(self, alternate):
         """1: consecutive passes walk the lattice in alternating directions (L2 reuse); 0 (default): all forward"""
