@@ -534,14 +534,7 @@ def run_sweep(args, cfg, ctx, wilson, Un, en, psi_n, r_min):
         ctx.wd_set_profile(False)
         n = max(p["iterations"], 1)
         a2, a3, a4 = p["a2_ms"] / n, p["a3_ms"] / n, p["a4_ms"] / n
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        reps = 100
-        e0.record()
-        for _ in range(reps):
-            ctx.wd_apply(Un, en, cfg.kappa, False, out=psi_n)
-        e1.record()
-        torch.cuda.synchronize()
-        ap_ms = e0.elapsed_time(e1) / reps
+        ap_ms = time_wd_apply(ctx, Un, en, psi_n, cfg.kappa, False)
         gbs = lambda b, ms: b * V / (ms * 1e-3) / 1e9 if ms > 0 else None
         print(json.dumps({
             "sweep": f"config{cfg.index}", "precision": args.precision, "tile_index": tile, "tile": list(inf[:4]),
