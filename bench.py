@@ -16,7 +16,7 @@ unspecified gauge fields.
 `e2e`     : the same solve through the C-ABI host-buffer call cg_solve_host (pinned HOST canonical
             buffers; H2D copies of U and eta, pack, solve, unpack and the D2H copy of psi inside the timed region).
 `roofline`: the dominant kernel (a3: D pass + fused r update + |r|^2, 576 B/site fp32) timed live with CUDA
-            events around each of its launches inside the timed steps (wd_set_profile).
+            events around its launches (every 4th iteration) inside the timed steps (wd_set_profile).
 `cpu_baseline`: the fp64 CPU oracle, as it stands, on a bounded sample (max_iter = 2) of the same workload.
 
 N > 1 (torchrun): the path does not shard (north_star: one GPU, no collectives) -> N independent replicas
@@ -636,7 +636,9 @@ def main():
     # ---------------- device-resident arm
     for _ in range(args.warmup):
         ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=psi_n)
-    ctx.wd_set_profile(True)
+    # CUDA events around the three kernels of every 4th iteration of the timed solves (31 of 124 iterations per solve at
+    # config 4): every launch costs about 1.5 us of stream time per event, which is 2 % of an iteration at 32^4
+    ctx.wd_set_profile(4)
     sampler = ClockSampler(local)
     barrier()
     sampler.start()

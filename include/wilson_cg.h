@@ -347,8 +347,9 @@ int wd_set_poll_interval(wd_ctx *ctx, int n);
  * Per-kernel timing of the CG loop (measurement aid).  With profiling on, cg_solve records
  * CUDA events on the ctx stream around the three kernels of every iteration (a2: D-dagger pass + |q|^2,
  * a3: D pass + r update + |r|^2, a4: axpy-xpay) and accumulates their device times.
- *   wd_set_profile(ctx, on)            switch on/off and clear the accumulators.
- *   wd_get_profile(ctx, ms, iters)     ms[0..2] = accumulated milliseconds of a2, a3, a4 over *iters iterations.
+ *   wd_set_profile(ctx, n)             n = 0 off, 1 every iteration, n > 1 every n-th iteration (the events cost about
+ *                                      1.5 us each on the stream, which shows at 32^4); clears the accumulators.
+ *   wd_get_profile(ctx, ms, iters)     ms[0..2] = accumulated milliseconds of a2, a3, a4 over the *iters timed iterations.
  */
 int wd_set_profile(wd_ctx *ctx, int on);
 int wd_get_profile(wd_ctx *ctx, double ms[3], long *iterations);

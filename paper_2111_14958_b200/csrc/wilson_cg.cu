@@ -286,7 +286,7 @@ extern "C" int wd_set_poll_interval(wd_ctx *c, int n)
 extern "C" int wd_set_profile(wd_ctx *c, int on)
 {
     if (!c) return WD_ERR_ARG;
-    c->profile = on ? 1 : 0;
+    c->profile = on > 0 ? on : 0;   // n > 1: cg_solve times the kernels of every n-th iteration only
     c->prof_ms[0] = c->prof_ms[1] = c->prof_ms[2] = 0.0;
     c->prof_n = 0;
     for (int j = 0; j < 7; ++j) c->bprof_ms[j] = 0.0;
@@ -544,13 +544,14 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
             // against the one before (pass number 3 it + j + 1), so each starts on what the last one left in L2
             const int rev2 = c->sweep ? (3 * it + 1) & 1 : 0, rev3 = c->sweep ? (3 * it + 2) & 1 : 0,
                       rev4 = c->sweep ? (3 * it + 3) & 1 : 0;
-            if (c->profile) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 0], c->stream));
+            const bool sample = c->profile && (it % c->profile == 0);
+            if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 0], c->stream));
             // a2: q = D-dagger p, qq, alpha
             CUDA_TRY(c, (launch_dslash<1, MODE_QQ>(c, U, c->p, c->q, kappa, nullptr, it, rev2)));
-            if (c->profile) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 1], c->stream));
+            if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 1], c->stream));
             // a3: r -= alpha D q, rr', beta, loop condition
             CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it, rev3)));
-            if (c->profile) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 2], c->stream));
+            if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 2], c->stream));
             // a4: y += alpha p ; p = r + beta p
             if (c->precision == 32)
                 cg_update_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((float4 *)c->y, (float4 *)c->p,
@@ -560,7 +561,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
                                                                            (const double2 *)c->r, n, c->sc, it, rev4);
             c->launches++;
             CUDA_TRY(c, cudaGetLastError());
-            if (c->profile) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 3], c->stream));
+            if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 3], c->stream));
         }
         return WD_OK;
     };
@@ -569,6 +570,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
         // only iterations that really ran (it < k_stop) count; over-launched ones are no-ops
         const cudaEvent_t *pev = c->pev + 4 * (size_t)pslot * poll;
         for (int i = 0; i < chunk && first + i < c->sc_host->k_stop; ++i) {
+            if ((first + i) % c->profile != 0) continue;   // not sampled
             for (int j = 0; j < 3; ++j) {
                 float ms = 0.f;
                 CUDA_TRY(c, cudaEventElapsedTime(&ms, pev[4 * i + j], pev[4 * i + j + 1]));

@@ -450,7 +450,8 @@ class WilsonContext:
         return int(self.lib.wd_get_tile(self._ctx))
 
     def wd_set_profile(self, on):
-        self._check(self.lib.wd_set_profile(self._ctx, int(bool(on))))
+        """False/0 off, True/1 time the kernels of every iteration, n > 1 of every n-th iteration (cg_solve only)"""
+        self._check(self.lib.wd_set_profile(self._ctx, int(on)))
 
     def wd_get_profile(self):
         """{'a2_ms', 'a3_ms', 'a4_ms', 'iterations'}: accumulated device time per kernel class of the CG loop."""
