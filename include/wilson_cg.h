@@ -83,7 +83,8 @@ typedef struct wd_cg_info {
     int kernel_launches;   /* number of this library's kernels launched by the call */
     int cg_mode;           /* 1 = three kernels per iteration, 2 = whole solve in one cooperative launch (one thread per site),
                               3 = BiCGSTAB, 4 = even-odd CG, 5 = multi-source CG, 6 = one cooperative launch with the hopping sum of
-                              a site split over four warps, 7 = even-odd BiCGSTAB */
+                              a site split over four warps, 7 = even-odd BiCGSTAB (seven kernels per iteration), 8 = even-odd BiCGSTAB in one
+                              cooperative launch */
 } wd_cg_info;
 
 /*
@@ -216,7 +217,10 @@ int bicgstab_solve(wd_ctx *ctx, const void *U_native, const void *eta_native, vo
  *       cg_solve_eo, then psi_o = eta_o + kappa H_oe psi_e.  Per iteration: two plain half-lattice hops to the odd sites,
  *       the two hops back fused with the diagonal term and the dot products of the BiCGSTAB passes (<rhat,v>; <t,s>,
  *       <t,t>), three half-length vector kernels.  Arguments as cg_solve_eo; returns WD_OK, WD_NOT_CONVERGED,
- *       WD_BREAKDOWN or an error; info->cg_mode = 7.  Synchronous.
+ *       WD_BREAKDOWN or an error; info->cg_mode = 7.  Synchronous.  Up to 65536 sites (the paper's 4^4..14^4 range and
+ *       16^4) the whole solve runs in ONE cooperative launch instead (grid barriers where the launch boundaries were, the
+ *       same recurrence, precision and breakdown rules; info->cg_mode = 8); wd_set_cg_mode(ctx, 1) forces the seven-kernel
+ *       loop, 2 the one-launch kernel (18-real links only).
  * Errors: WD_ERR_DIMS for an odd extent, WD_ERR_ARG (NULL, aliasing), WD_ERR_CUDA, WD_ERR_ALLOC.
  */
 size_t wd_eo_spinor_bytes(wd_ctx *ctx);

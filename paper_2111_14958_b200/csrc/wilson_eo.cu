@@ -8,6 +8,7 @@
 // half lattice (Geom.eo = 1): same tiles, same fused epilogues; only the +-x neighbour rule and the fields the
 // links / the diagonal term come from differ.  This file holds the checkerboard pack kernels and the host loop.
 #include "wilson_ctx.cuh"
+#include "wilson_eo_onelaunch.cuh"
 
 #include <cmath>
 
@@ -422,6 +423,53 @@ static int eo_bicgstab_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, voi
     return WD_OK;
 }
 
+// Largest volume (sites of the FULL lattice) that bicgstab_solve_eo solves in one cooperative launch in automatic mode.
+// Measured on B200, ms per solve, seven kernels per iteration / one launch: fp32 4^4 0.40 / 0.17, 14^4 0.40 / 0.29, 16^4
+// 1.15 / 0.89, 20^4 1.78 / 2.47; fp64 4^4 0.54 / 0.32, 14^4 0.77 / 0.62, 16^4 2.66 / 2.29, 20^4 5.63 / 8.60.
+#ifndef WD_EO_ONELAUNCH_MAX_SITES
+#define WD_EO_ONELAUNCH_MAX_SITES 65536
+#endif
+
+static bool eo_use_onelaunch(const wd_ctx *c)
+{
+    if (!c->coop_ok || c->recon != 18) return false;
+    if (c->cg_mode == 1) return false;
+    if (c->cg_mode == 2) return true;
+    return c->V <= WD_EO_ONELAUNCH_MAX_SITES;
+}
+
+static int eo_bicgstab_onelaunch(wd_ctx *c, const void *U_eo, const void *eta_eo, void *psi_eo, double kappa, double r_min,
+                                 int max_iter)
+{
+    const EoDims e = eo_dims(c);
+    int best = 0;
+    double best_waste = 1e300;
+    for (int t = 0; t < WD_NUM_EO1_TILES; ++t) {
+        double blocks = 1.0, threads = 1.0;
+        for (int d = 0; d < 4; ++d) {
+            blocks *= (e.hd[d] + kEo1Tiles[t][d] - 1) / kEo1Tiles[t][d];
+            threads *= kEo1Tiles[t][d];
+        }
+        const double waste = blocks * threads / (double)e.Vh;
+        if (waste < best_waste - 1e-12) { best_waste = waste; best = t; }
+    }
+    const size_t hs = half_spinor_bytes(c), hg = half_gauge_bytes(c);
+    EoOneLaunchArgs a;
+    a.g = make_geom_lattice(e.hd, c->bc_t, kEo1Tiles[best], 0, c->l2_budget_mb);
+    a.g.eo = 1;
+    a.sm_count = c->sm_count;
+    a.stream = c->stream;
+    a.Ue = U_eo; a.Uo = (const char *)U_eo + hg;
+    a.eta_e = eta_eo; a.eta_o = (const char *)eta_eo + hs;
+    a.psi_e = psi_eo; a.psi_o = (char *)psi_eo + hs;
+    a.r = c->r; a.p = c->p; a.v = c->q; a.s = c->y; a.t = c->w7; a.to = c->w5; a.etah = c->w6;
+    a.kappa = kappa; a.sc = c->sc; a.partials = c->partials; a.partials_cap = c->partials_cap; a.hist = c->hist;
+    a.r_min = r_min; a.max_iter = max_iter;
+    c->launches++;
+    CUDA_TRY(c, c->precision == 32 ? launch_eo_bicgstab_onelaunch_f32(best, a) : launch_eo_bicgstab_onelaunch_f64(best, a));
+    return WD_OK;
+}
+
 extern "C" int bicgstab_solve_eo(wd_ctx *c, const void *U_eo, const void *eta_eo, void *psi_eo, double kappa, double r_min,
                                  int max_iter, wd_cg_info *info)
 {
@@ -451,8 +499,10 @@ extern "C" int bicgstab_solve_eo(wd_ctx *c, const void *U_eo, const void *eta_eo
         for (int j = 0; j < 8; ++j) CUDA_TRY(c, cudaEventCreate(&c->bev[j]));
     c->launches = 0;
     CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
-    rc = c->precision == 32 ? eo_bicgstab_loop<float>(c, U_eo, eta_eo, psi_eo, kappa, r_min, max_iter)
-                            : eo_bicgstab_loop<double>(c, U_eo, eta_eo, psi_eo, kappa, r_min, max_iter);
+    const bool one = eo_use_onelaunch(c);
+    if (one) rc = eo_bicgstab_onelaunch(c, U_eo, eta_eo, psi_eo, kappa, r_min, max_iter);
+    else rc = c->precision == 32 ? eo_bicgstab_loop<float>(c, U_eo, eta_eo, psi_eo, kappa, r_min, max_iter)
+                                 : eo_bicgstab_loop<double>(c, U_eo, eta_eo, psi_eo, kappa, r_min, max_iter);
     if (rc != WD_OK) return rc;
     CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
@@ -469,7 +519,7 @@ extern "C" int bicgstab_solve_eo(wd_ctx *c, const void *U_eo, const void *eta_eo
         info->gpu_ms = ms;
         info->total_ms = ms;
         info->kernel_launches = c->launches;
-        info->cg_mode = 7;
+        info->cg_mode = one ? 8 : 7;
     }
     return s.converged ? WD_OK : (s.breakdown ? WD_BREAKDOWN : WD_NOT_CONVERGED);
 }

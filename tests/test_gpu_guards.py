@@ -149,8 +149,12 @@ def test_even_odd_calls_stay_inside_their_buffers(wilson, dims, precision):
         assert torch.isfinite(tmp.t).all()
         _, info = ctx.cg_solve_eo(Ue.t, ee.t, kappa, r_min, 500, out=pe.t)
         assert info["status"] == 0 and torch.isfinite(torch.view_as_real(ctx.wd_eo_unpack_spinor(pe.t))).all()
-        _, info = ctx.bicgstab_solve_eo(Ue.t, ee.t, kappa, r_min, 500, out=pe.t)
-        assert info["status"] == 0 and torch.isfinite(torch.view_as_real(ctx.wd_eo_unpack_spinor(pe.t))).all()
+        for mode in (1, 2):     # seven kernels per iteration, one cooperative launch
+            ctx.wd_set_cg_mode(mode)
+            _, info = ctx.bicgstab_solve_eo(Ue.t, ee.t, kappa, r_min, 500, out=pe.t)
+            assert info["status"] == 0 and info["cg_mode"] == 6 + mode
+            assert torch.isfinite(torch.view_as_real(ctx.wd_eo_unpack_spinor(pe.t))).all()
+        ctx.wd_set_cg_mode(0)
         can = Guarded(torch.view_as_real(gu.to_device(eta)).reshape(-1))
         ctx._check(ctx.lib.wd_eo_unpack_spinor(ctx._ctx, ctx._p(pe.t), ctx._p(can.t)))
         # the same on 12-real links

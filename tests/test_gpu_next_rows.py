@@ -405,26 +405,31 @@ def test_eo_cg_32_4_closed_form(wilson, precision):
 
 
 # ---------------------------------------------------------------- f3 x f4: even-odd preconditioned BiCGSTAB (readings E1 + B1)
-def eo_bicgstab_on_gpu(ctx, U, eta, kappa, r_min, max_iter):
+def eo_bicgstab_on_gpu(ctx, U, eta, kappa, r_min, max_iter, mode=None):
+    """mode: None = automatic, 1 = seven kernels per iteration (info cg_mode 7), 2 = one cooperative launch (8)"""
+    if mode is not None:
+        ctx.wd_set_cg_mode(mode)
     Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
     ee = ctx.wd_eo_pack_spinor(gu.to_device(eta))
     pe, info = ctx.bicgstab_solve_eo(Ue, ee, kappa, r_min, max_iter)
     return gu.to_host(ctx.wd_eo_unpack_spinor(pe)), info
 
 
+@pytest.mark.parametrize("mode", [1, 2])
 @pytest.mark.parametrize("precision,r_min", [(32, 1e-6), (64, 1e-10)])
 @pytest.mark.parametrize("cfg_index", [0, 1, 2])
-def test_eo_bicgstab_baseline_configs(wilson, oracle, cfg_index, precision, r_min):
+def test_eo_bicgstab_baseline_configs(wilson, oracle, cfg_index, precision, r_min, mode):
+    """both drivers: seven kernels per iteration (mode 1) and the whole solve in one cooperative launch (mode 2)"""
     cfg = inputs.CONFIGS[cfg_index]
     U, eta = gu.config_fields(cfg.index, precision)
     U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
     with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
-        psi, info = eo_bicgstab_on_gpu(ctx, U, eta, cfg.kappa, r_min, cfg.max_iter)
+        psi, info = eo_bicgstab_on_gpu(ctx, U, eta, cfg.kappa, r_min, cfg.max_iter, mode)
         hist = ctx.wd_cg_history()
         _, plain = bicgstab_on_gpu(ctx, U, eta, cfg.kappa, r_min, cfg.max_iter)
     psi_o, info_o = oracle.bicgstab_solve_eo(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t, history=True)
-    assert info["status"] == 0 and info["converged"] == 1 and info["cg_mode"] == 7 and info_o["converged"]
-    assert info["kernel_launches"] >= 7 * info["iterations"] + 1
+    assert info["status"] == 0 and info["converged"] == 1 and info["cg_mode"] == (7 if mode == 1 else 8) and info_o["converged"]
+    assert info["kernel_launches"] >= 7 * info["iterations"] + 1 if mode == 1 else info["kernel_launches"] == 1
     slack = 0 if precision == 64 else max(1, int(0.05 * info_o["iterations"] + 0.5))
     assert abs(info["iterations"] - info_o["iterations"]) <= slack, (info["iterations"], info_o["iterations"])
     assert abs(info["eta_norm2"] - info_o["eta_norm2"]) < (1e-6 if precision == 32 else 1e-13) * info_o["eta_norm2"]
@@ -459,20 +464,24 @@ def test_eo_bicgstab_ragged_lattices(wilson, oracle, precision):
         U = inputs.gauge_field(CFG_TEST + 60, dims, links).astype(cdt)
         eta = inputs.source_field(CFG_TEST + 60, dims).astype(cdt)
         U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
-        with wilson.WilsonContext(dims, precision, bc_t) as ctx:
-            psi, info = eo_bicgstab_on_gpu(ctx, U, eta, kappa, r_min, 500)
         psi_o, info_o = oracle.bicgstab_solve_eo(dims, U64, eta64, kappa, r_min, 500, bc_t)
-        assert info["status"] == 0 and abs(info["iterations"] - info_o["iterations"]) <= (0 if precision == 64 else 1)
-        res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), kappa, bc_t)
-        assert res < 2.0 * r_min, (dims, res)
-        assert np.linalg.norm(psi - psi_o) < 4.0 * r_min * (1 + 8 * kappa) / (1 - 8 * kappa) * np.linalg.norm(psi_o)
+        for mode in (1, 2):
+            with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+                psi, info = eo_bicgstab_on_gpu(ctx, U, eta, kappa, r_min, 500, mode)
+            assert info["status"] == 0 and abs(info["iterations"] - info_o["iterations"]) <= (0 if precision == 64 else 1)
+            assert info["cg_mode"] == (7 if mode == 1 else 8)
+            res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), kappa, bc_t)
+            assert res < 2.0 * r_min, (dims, mode, res)
+            assert np.linalg.norm(psi - psi_o) < 4.0 * r_min * (1 + 8 * kappa) / (1 - 8 * kappa) * np.linalg.norm(psi_o)
 
 
-def test_eo_bicgstab_edge_cases(wilson, oracle):
+@pytest.mark.parametrize("mode", [1, 2])
+def test_eo_bicgstab_edge_cases(wilson, oracle, mode):
     cfg = inputs.CONFIGS[0]
     U, eta = gu.config_fields(0, 32)
     par = _parity(cfg.dims)
     with wilson.WilsonContext(cfg.dims, 32) as ctx:
+        ctx.wd_set_cg_mode(mode)
         Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
         ee = ctx.wd_eo_pack_spinor(gu.to_device(eta))
         pe, info = ctx.bicgstab_solve_eo(Ue, ctx.wd_eo_pack_spinor(gu.to_device(np.zeros_like(eta))), cfg.kappa, 1e-6, 10)
