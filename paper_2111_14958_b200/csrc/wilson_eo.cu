@@ -424,8 +424,8 @@ static int eo_bicgstab_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, voi
 }
 
 // Largest volume (sites of the FULL lattice) that bicgstab_solve_eo solves in one cooperative launch in automatic mode.
-// Measured on B200, ms per solve, seven kernels per iteration / one launch: fp32 4^4 0.40 / 0.17, 14^4 0.40 / 0.29, 16^4
-// 1.15 / 0.89, 20^4 1.78 / 2.47; fp64 4^4 0.54 / 0.32, 14^4 0.77 / 0.62, 16^4 2.66 / 2.29, 20^4 5.63 / 8.60.
+// Measured on B200, ms per solve, seven kernels per iteration / one launch: fp32 4^4 0.39 / 0.16, 14^4 0.40 / 0.26, 16^4
+// 1.14 / 0.78, 20^4 1.79 / 2.14; fp64 4^4 0.54 / 0.33, 14^4 0.77 / 0.64, 16^4 2.67 / 2.38, 20^4 5.63 / 8.99.
 #ifndef WD_EO_ONELAUNCH_MAX_SITES
 #define WD_EO_ONELAUNCH_MAX_SITES 65536
 #endif

@@ -78,7 +78,7 @@ __device__ __forceinline__ real site_norm2(const real a[24])
 }
 
 template <typename real, int BX, int BY, int BZ, int BT>
-__global__ void __launch_bounds__(BX *BY *BZ *BT)
+__global__ void __launch_bounds__(BX *BY *BZ *BT, 1)
 eo_bicgstab_onelaunch_kernel(const Geom g0, const typename Field<real>::gvec *__restrict__ Ue,
                              const typename Field<real>::gvec *__restrict__ Uo,
                              const typename Field<real>::svec *__restrict__ eta_e,
