@@ -58,7 +58,7 @@ __device__ __forceinline__ void dir_hops(const gvec *__restrict__ U, const svec 
 }
 
 template <typename real, int BX, int BY, int BZ, int BT>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 1)
 cg_split_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
                 const typename Field<real>::svec *__restrict__ eta, typename Field<real>::svec *y,
                 typename Field<real>::svec *r, typename Field<real>::svec *p, typename Field<real>::svec *q,
