@@ -332,6 +332,10 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *                             the data the previous one left in the 126 MB L2; a = 0 (default: the alternation measured no
  *                             gain on B200): every pass walks forward.  The per-site arithmetic is identical; only the
  *                             grouping of the reduction partials changes.
+ *   wd_set_fuse_y(ctx, on)        on = 1: in the three-kernel cg_solve the update y <- y + alpha p (half of a4, PAPER.md:47
+ *                             "psi <- psi + alpha p") is done inside the a3 stencil pass, which already holds alpha, and a4
+ *                             shrinks to p <- r + beta p (1536 B/site per iteration either way; every element sees the same
+ *                             operations, so the iterates are bit-identical).  18-real links only (ignored otherwise).
  *   wd_set_poll_interval(ctx, n)  CG iterations enqueued between two host polls of the device stop flag (n >= 1; 0 = automatic).
  */
 int wd_num_tiles(void);
@@ -345,6 +349,7 @@ int wd_set_waves(wd_ctx *ctx, int waves);
 int wd_set_zchunk(wd_ctx *ctx, int layers);
 int wd_set_sweep(wd_ctx *ctx, int alternate);
 int wd_set_small_tile(wd_ctx *ctx, int index);
+int wd_set_fuse_y(wd_ctx *ctx, int on);
 int wd_set_poll_interval(wd_ctx *ctx, int n);
 
 /*

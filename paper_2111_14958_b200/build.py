@@ -20,7 +20,8 @@ UNITS = ["wilson_cg.cu", "wilson_dslash_f32.cu", "wilson_dslash_f64.cu", "wilson
          "wilson_coo.cu", "wilson_eo.cu", "wilson_mrhs.cu", "wilson_mrhs_f32.cu", "wilson_mrhs_f64.cu", "wilson_dslash_eo_f32.cu", "wilson_dslash_eo_f64.cu", "wilson_dslash12_f32.cu", "wilson_dslash12_f64.cu",
          "wilson_bicg_eo_f32.cu", "wilson_bicg_eo_f64.cu", "wilson_split_f32.cu", "wilson_split_f64.cu",
          "wilson_dslash12_eo_f32.cu", "wilson_dslash12_eo_f64.cu",
-         "wilson_eo_onelaunch_f32.cu", "wilson_eo_onelaunch_f64.cu"]
+         "wilson_eo_onelaunch_f32.cu", "wilson_eo_onelaunch_f64.cu",
+         "wilson_dslash_y_f32.cu", "wilson_dslash_y_f64.cu"]
 HEADERS = [os.path.join(CSRC, "wilson_kernels.cuh"), os.path.join(CSRC, "wilson_launch.cuh"),
            os.path.join(CSRC, "wilson_ctx.cuh"), os.path.join(CSRC, "wilson_mrhs.cuh"), os.path.join(CSRC, "wilson_split.cuh"), os.path.join(CSRC, "wilson_eo_onelaunch.cuh"),
            os.path.join(ROOT, "include", "wilson_cg.h")]

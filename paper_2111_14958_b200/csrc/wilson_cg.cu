@@ -63,6 +63,23 @@ static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void 
     return c->precision == 32 ? launch_dslash_f32(c->tile, DAG, MODE, a) : launch_dslash_f64(c->tile, DAG, MODE, a);
 }
 
+// a3 with the y half of a4 fused in: r -= alpha D q, rr', beta, loop test, y += alpha p  (MODE_RUPDY)
+static cudaError_t launch_dslash_y(wd_ctx *c, const void *U, double kappa, int it, int rev)
+{
+    DslashArgs a;
+    a.g = make_geom(c, c->tile);
+    a.g.rev = rev;
+    a.sm_count = c->sm_count;
+    a.waves = c->waves > 0 ? c->waves : 1;
+    a.prefetch = (c->dims[0] % SB == 0) ? c->prefetch : 0;
+    a.stream = c->stream;
+    a.U = U; a.Ub = U; a.in = c->q; a.cen = c->p; a.out = c->y; a.kappa = kappa; a.r = c->r;
+    a.sc = c->sc;
+    a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = it;
+    c->launches++;
+    return c->precision == 32 ? launch_dslash_y_f32(c->tile, a) : launch_dslash_y_f64(c->tile, a);
+}
+
 static unsigned int vec_grid(const wd_ctx *c, size_t n)
 {
     const size_t need = (n + VEC_NT - 1) / VEC_NT;
@@ -145,6 +162,7 @@ extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_
     c->tile = auto_tile(c);
     c->l2_budget_mb = 40.0;
     c->small_tile_user = -1;
+    c->fuse_y = 0;
     c->sweep = 0;      // measured on B200: alternating the walk direction gains nothing
     c->prefetch = 0;   // measured on B200: bulk L2 prefetch of the next tile slows the stencil by 15-30 %
     bool ok = true;
@@ -274,6 +292,12 @@ extern "C" int wd_set_sweep(wd_ctx *c, int alternate)
 {
     if (!c || alternate < 0 || alternate > 1) return WD_ERR_ARG;
     c->sweep = alternate;
+    return WD_OK;
+}
+extern "C" int wd_set_fuse_y(wd_ctx *c, int on)
+{
+    if (!c || on < 0 || on > 1) return WD_ERR_ARG;
+    c->fuse_y = on;
     return WD_OK;
 }
 extern "C" int wd_set_poll_interval(wd_ctx *c, int n)
@@ -550,10 +574,17 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
             CUDA_TRY(c, (launch_dslash<1, MODE_QQ>(c, U, c->p, c->q, kappa, nullptr, it, rev2)));
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 1], c->stream));
             // a3: r -= alpha D q, rr', beta, loop condition
-            CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it, rev3)));
+            // (fuse_y: y += alpha p in the same pass, then a4 is p = r + beta p alone; same arithmetic per element)
+            const bool fy = c->fuse_y && c->recon == 18;
+            if (fy) CUDA_TRY(c, launch_dslash_y(c, U, kappa, it, rev3));
+            else CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it, rev3)));
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 2], c->stream));
             // a4: y += alpha p ; p = r + beta p
-            if (c->precision == 32)
+            if (fy && c->precision == 32)
+                cg_pupdate_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((float4 *)c->p, (const float4 *)c->r, n, c->sc, it, rev4);
+            else if (fy)
+                cg_pupdate_kernel<double><<<vgrid, VEC_NT, 0, c->stream>>>((double2 *)c->p, (const double2 *)c->r, n, c->sc, it, rev4);
+            else if (c->precision == 32)
                 cg_update_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((float4 *)c->y, (float4 *)c->p,
                                                                           (const float4 *)c->r, n, c->sc, it, rev4);
             else

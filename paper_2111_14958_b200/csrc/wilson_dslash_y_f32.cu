@@ -1,0 +1,8 @@
+// 32-bit instantiations of the a3 pass with the y update fused in (MODE_RUPDY); own translation unit for parallel builds.
+#include "wilson_launch.cuh"
+namespace wd {
+cudaError_t launch_dslash_y_f32(int tile, const DslashArgs &a)
+{
+    return launch_dslash_tile<float, 0, MODE_RUPDY>(tile, a);
+}
+}  // namespace wd

@@ -759,11 +759,13 @@ __device__ __forceinline__ void finish_bi(CgScalars *sc, const double rho_new[2]
 }
 
 // ---------------------------------------------------------------- the stencil kernel
-enum { MODE_PLAIN = 0, MODE_QQ = 1, MODE_RUPD = 2, MODE_RV = 3, MODE_TS = 4 };
+enum { MODE_PLAIN = 0, MODE_QQ = 1, MODE_RUPD = 2, MODE_RV = 3, MODE_TS = 4, MODE_RUPDY = 5 };
 
 // MODE_PLAIN : out = D in / D-dagger in                                  (wd_apply, a6, a7)
 // MODE_QQ    : out = q = D-dagger p, qq = |q|^2, alpha = rr/qq           (a2)
 // MODE_RUPD  : s = D q (not stored), r <- r - alpha s, rr' = |r|^2, beta, loop condition   (a3)
+// MODE_RUPDY : MODE_RUPD and, in the same pass, y <- y + alpha p (y passed as `out`, p as `cen`, plain lattice only):
+//              the y half of a4 rides on the latency-bound stencil pass, a4 shrinks to p <- r + beta p   (a3 + a4y)
 // MODE_RV    : out = v = D p, <rhat, v> (rhat passed as `r`, read only), alpha = rho/<rhat,v>   (BiCGSTAB)
 // MODE_TS    : out = t = D s, <t,s> and <t,t>, omega = <t,s>/<t,t>                              (BiCGSTAB)
 // EO = 0: plain lattice (UB and cen are ignored: the backward links come from U, the diagonal term from `in`);
@@ -784,7 +786,9 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     // the centre and r last: centre-first made a3 slower (1017 -> 1086 us), and so did folding r into the
     // accumulator as well (acc = r - alpha in, hops scaled by alpha kappa: 1056 us).  MODE_TS needs s(x) beside t(x).
     // PIPE = 4: the same pipeline with the centre last in every mode (the comparison row of the table).
-    constexpr bool CF = (PIPE == 1) && MODE != MODE_TS && MODE != MODE_RUPD;
+    constexpr bool RU = MODE == MODE_RUPD || MODE == MODE_RUPDY;
+    static_assert(MODE != MODE_RUPDY || EO == 0, "MODE_RUPDY: plain lattice only (cen carries p)");
+    constexpr bool CF = (PIPE == 1) && MODE != MODE_TS && !RU;
     constexpr int HP = (PIPE == 4) ? 1 : PIPE;
     if (MODE != MODE_PLAIN) {
         if (it >= sc->k_stop) return;  // uniform over the grid: over-launched iterations are no-ops
@@ -793,7 +797,7 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     }
     const int tid = threadIdx.x;
     const int lx = tid % BX, ly = (tid / BX) % BY, lz = (tid / (BX * BY)) % BZ, lt = tid / (BX * BY * BZ);
-    const real alpha = (MODE == MODE_RUPD) ? (real)sc->alpha : (real)0;
+    const real alpha = RU ? (real)sc->alpha : (real)0;
     double local = 0.0, local1 = 0.0, local2 = 0.0;
     extern __shared__ __align__(16) unsigned char wd_dyn_smem[];   // PIPE = 3: staged forward links, 72 reals per thread
     // site of this thread in tile b, or -1 (no such tile / thread outside the lattice)
@@ -823,7 +827,7 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
                 const int ps = px + g.L[0] * (py + g.L[1] * (pz + g.L[2] * pt));
                 prefetch_l2(in + spinor_index<svec, Field<real>::NSP>(ps), Field<real>::NSP * SB * sizeof(svec));
                 prefetch_l2(U + gauge_index(ps), 36 * SB * sizeof(gvec));
-                if (MODE == MODE_RUPD)
+                if (RU)
                     prefetch_l2(r + spinor_index<svec, Field<real>::NSP>(ps), Field<real>::NSP * SB * sizeof(svec));
             }
         }
@@ -839,7 +843,8 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
         if (!active) continue;
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24], rv[24];
-        hopping_sum<DAG, HP, MODE == MODE_RUPD || MODE == MODE_RV, true, real, svec, gvec, RECON, NT, EO, CF>(
+        [[maybe_unused]] real yv[24];
+        hopping_sum<DAG, HP, RU || MODE == MODE_RV, true, real, svec, gvec, RECON, NT, EO, CF>(
             g, U, EO ? UB : U, in, EO ? cen : in, r, x, y, z, t, s, acc, c, rv, wd_dyn_smem, next_s, kappa);
         if constexpr (MODE == MODE_TS) {
             // c holds s(x); t(x) = s(x) - kappa * hops replaces it component by component
@@ -867,7 +872,11 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
             }
             store_spinor(out, s, c);
             local += (double)dr; local1 += (double)di;
-        } else if (MODE == MODE_RUPD) {
+        } else if (RU) {
+            if (MODE == MODE_RUPDY) {                                  // issue the two per-site loads before the r algebra
+                load_spinor(cen, s, acc);                              // p(s)
+                load_spinor_rw(out, s, yv);                            // y(s)
+            }
             real n2 = 0;
 #pragma unroll
             for (int i = 0; i < 24; ++i) {
@@ -876,6 +885,11 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
             }
             store_spinor(r, s, rv);
             local += (double)n2;
+            if (MODE == MODE_RUPDY) {
+#pragma unroll
+                for (int i = 0; i < 24; ++i) yv[i] = fma(alpha, acc[i], yv[i]);   // y <- y + alpha p (as cg_update_kernel)
+                store_spinor(out, s, yv);
+            }
         } else {
             store_spinor(out, s, c);
             if (MODE == MODE_QQ) {
@@ -887,7 +901,7 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
         }
         }  // MODE != MODE_TS
     }
-    if (MODE == MODE_QQ || MODE == MODE_RUPD) {
+    if (MODE == MODE_QQ || RU) {
         double total;
         if (grid_sum<NT>(local, partials, counter, &total)) {
             if (MODE == MODE_QQ) finish_qq(sc, total);
@@ -1123,6 +1137,21 @@ cg_update_kernel(typename Field<real>::svec *y, typename Field<real>::svec *p,
         const svec rv = __ldg(r + i);
         y[i] = vaxpy(alpha, pv, y[i]);
         p[i] = vaxpy(beta, pv, rv);
+    }
+}
+
+// a4 without its y half (the y update rode on the a3 pass, MODE_RUPDY): p <- r + beta p
+template <typename real>
+__global__ void __launch_bounds__(VEC_NT)
+cg_pupdate_kernel(typename Field<real>::svec *p, const typename Field<real>::svec *__restrict__ r, size_t n,
+                  const CgScalars *sc, int it, int rev)
+{
+    using svec = typename Field<real>::svec;
+    if (it >= sc->k_stop) return;
+    const real beta = (real)sc->beta;
+    for (size_t j = (size_t)blockIdx.x * VEC_NT + threadIdx.x; j < n; j += (size_t)gridDim.x * VEC_NT) {
+        const size_t i = rev ? n - 1 - j : j;
+        p[i] = vaxpy(beta, p[i], __ldg(r + i));
     }
 }
 

@@ -120,6 +120,9 @@ struct DslashArgs {
 // dagger in {0,1}; mode in {MODE_PLAIN, MODE_QQ (dagger = 1 only), MODE_RUPD (dagger = 0 only)}
 cudaError_t launch_dslash_f32(int tile, int dagger, int mode, const DslashArgs &a);
 cudaError_t launch_dslash_f64(int tile, int dagger, int mode, const DslashArgs &a);
+// a3 with the y half of a4 fused in (MODE_RUPDY: a.out = y, a.cen = p); 18-real links, plain lattice
+cudaError_t launch_dslash_y_f32(int tile, const DslashArgs &a);
+cudaError_t launch_dslash_y_f64(int tile, const DslashArgs &a);
 // the same with 12-real link storage (wd_set_gauge_recon(ctx, 12))
 cudaError_t launch_dslash12_f32(int tile, int dagger, int mode, const DslashArgs &a);
 cudaError_t launch_dslash12_f64(int tile, int dagger, int mode, const DslashArgs &a);

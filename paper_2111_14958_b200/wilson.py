@@ -114,6 +114,7 @@ def load_library(path: str = LIB_PATH):
     lib.wd_set_waves.argtypes = [vp, ci]
     lib.wd_set_zchunk.argtypes = [vp, ci]
     lib.wd_set_sweep.argtypes = [vp, ci]
+    lib.wd_set_fuse_y.argtypes = [vp, ci]
     lib.wd_set_small_tile.argtypes = [vp, ci]
     lib.wd_set_poll_interval.argtypes = [vp, ci]
     lib.wd_set_profile.argtypes = [vp, ci]
@@ -487,6 +488,10 @@ class WilsonContext:
     def wd_set_sweep(self, alternate):
         """1: consecutive passes walk the lattice in alternating directions (L2 reuse); 0 (default): all forward"""
         self._check(self.lib.wd_set_sweep(self._ctx, int(alternate)))
+
+    def wd_set_fuse_y(self, on):
+        """1: y += alpha p rides on the a3 stencil pass, a4 is p = r + beta p alone (bit-identical iterates)"""
+        self._check(self.lib.wd_set_fuse_y(self._ctx, int(on)))
 
     def wd_set_poll_interval(self, n):
         self._check(self.lib.wd_set_poll_interval(self._ctx, int(n)))

@@ -357,6 +357,52 @@ def test_alternating_sweep_direction(wilson, cfg_index, precision):
     assert np.linalg.norm(res[0][1] - res[1][1]) <= tol * np.linalg.norm(res[0][1])
 
 
+@pytest.mark.parametrize("precision", [32, 64])
+def test_cg_y_update_inside_the_a3_pass(wilson, oracle, precision):
+    """wd_set_fuse_y(1): y <- y + alpha p runs inside the a3 stencil pass (MODE_RUPDY), a4 is p <- r + beta p
+    alone.  Every element sees the same operations, so solution, iteration count and residual history are bit-identical
+    to the three-kernel driver with the whole a4; the solution is checked against the oracle as well.  Config 1 and a
+    ragged lattice (V not a multiple of the 16-site block, no tile divides the extents)."""
+    cfg = inputs.CONFIGS[1]
+    cdt = gu.np_complex(precision)
+    tol = 1e-6 if precision == 32 else 1e-11
+    cases = [(cfg.dims, cfg.bc_t, cfg.kappa) + gu.config_fields(1, precision),
+             ((5, 7, 4, 6), 1, 0.12, inputs.gauge_field(CFG_TEST + 6, (5, 7, 4, 6), "near_identity", dtype=cdt),
+              inputs.source_field(CFG_TEST + 6, (5, 7, 4, 6), dtype=cdt))]
+    # every compiled launch configuration on the ragged lattice, the automatic one on config 1
+    runs = [cases[0] + (-1,)] + [cases[1] + (t,) for t in range(len(wilson.tile_shapes()))]
+    ran = 0
+    for dims, bc_t, kappa, U, eta, tile in runs:
+        got = {}
+        for fy in (0, 1):
+            with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+                ctx.wd_set_cg_mode(1)
+                ctx.wd_set_fuse_y(fy)
+                if tile >= 0:
+                    try:
+                        ctx.wd_set_tile(tile)
+                    except wilson.WilsonError as e:
+                        assert precision == 64 and e.code == -1  # large tiles are fp32-only
+                        break
+                psi, info = gu.solve_on_gpu(ctx, U, eta, kappa, tol, 500)
+                got[fy] = (psi, info, ctx.wd_cg_history())
+                with pytest.raises(wilson.WilsonError):
+                    ctx.wd_set_fuse_y(2)
+        if not got:
+            continue
+        ran += 1
+        assert got[0][1]["status"] == got[1][1]["status"] == 0
+        assert got[0][1]["iterations"] == got[1][1]["iterations"]
+        assert got[0][0].tobytes() == got[1][0].tobytes()
+        assert np.array_equal(got[0][2], got[1][2])
+        U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+        psi_o, info_o = oracle.cg_solve(dims, U64, eta64, kappa, tol, 500, bc_t)
+        assert iters_close(got[1][1]["iterations"], info_o["iterations"])
+        res = oracle.true_residual(dims, U64, eta64, got[1][0].astype(np.complex128), kappa, bc_t)
+        assert res <= 2.0 * oracle.true_residual(dims, U64, eta64, psi_o, kappa, bc_t)
+    assert ran >= 9
+
+
 @pytest.mark.parametrize("mode", [1, 2, 6])
 def test_cg_edge_cases(wilson, oracle, mode):
     cfg = inputs.CONFIGS[0]
