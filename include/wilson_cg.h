@@ -336,6 +336,9 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *                             "psi <- psi + alpha p") is done inside the a3 stencil pass, which already holds alpha, and a4
  *                             shrinks to p <- r + beta p (1536 B/site per iteration either way; every element sees the same
  *                             operations, so the iterates are bit-identical).  18-real links only (ignored otherwise).
+ *   wd_set_pdl(ctx, on)           on = 1: the kernels of the three-kernel cg_solve loop are launched with programmatic stream
+ *                             serialization (each starts with griddepcontrol.wait, so it touches memory only after its
+ *                             predecessor has completed): launch latency overlaps the drain of the previous kernel.  Same results.
  *   wd_set_poll_interval(ctx, n)  CG iterations enqueued between two host polls of the device stop flag (n >= 1; 0 = automatic).
  */
 int wd_num_tiles(void);
@@ -350,6 +353,7 @@ int wd_set_zchunk(wd_ctx *ctx, int layers);
 int wd_set_sweep(wd_ctx *ctx, int alternate);
 int wd_set_small_tile(wd_ctx *ctx, int index);
 int wd_set_fuse_y(wd_ctx *ctx, int on);
+int wd_set_pdl(wd_ctx *ctx, int on);
 int wd_set_poll_interval(wd_ctx *ctx, int n);
 
 /*

@@ -45,9 +45,10 @@ extern "C" long wd_selftest_fastdiv(unsigned int d, unsigned int n_max)
 // ---------------------------------------------------------------- launches
 template <int DAG, int MODE>
 static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void *out, double kappa, void *r, int it,
-                                 int rev = 0)
+                                 int rev = 0, int pdl = 0)
 {
     DslashArgs a;
+    a.pdl = pdl;
     a.g = make_geom(c, c->tile);
     a.g.rev = rev;
     a.sm_count = c->sm_count;
@@ -64,9 +65,10 @@ static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void 
 }
 
 // a3 with the y half of a4 fused in: r -= alpha D q, rr', beta, loop test, y += alpha p  (MODE_RUPDY)
-static cudaError_t launch_dslash_y(wd_ctx *c, const void *U, double kappa, int it, int rev)
+static cudaError_t launch_dslash_y(wd_ctx *c, const void *U, double kappa, int it, int rev, int pdl)
 {
     DslashArgs a;
+    a.pdl = pdl;
     a.g = make_geom(c, c->tile);
     a.g.rev = rev;
     a.sm_count = c->sm_count;
@@ -163,6 +165,7 @@ extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_
     c->l2_budget_mb = 40.0;
     c->small_tile_user = -1;
     c->fuse_y = 0;
+    c->pdl = 0;
     c->sweep = 0;      // measured on B200: alternating the walk direction gains nothing
     c->prefetch = 0;   // measured on B200: bulk L2 prefetch of the next tile slows the stencil by 15-30 %
     bool ok = true;
@@ -298,6 +301,12 @@ extern "C" int wd_set_fuse_y(wd_ctx *c, int on)
 {
     if (!c || on < 0 || on > 1) return WD_ERR_ARG;
     c->fuse_y = on;
+    return WD_OK;
+}
+extern "C" int wd_set_pdl(wd_ctx *c, int on)
+{
+    if (!c || on < 0 || on > 1) return WD_ERR_ARG;
+    c->pdl = on;
     return WD_OK;
 }
 extern "C" int wd_set_poll_interval(wd_ctx *c, int n)
@@ -571,25 +580,32 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
             const bool sample = c->profile && (it % c->profile == 0);
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 0], c->stream));
             // a2: q = D-dagger p, qq, alpha
-            CUDA_TRY(c, (launch_dslash<1, MODE_QQ>(c, U, c->p, c->q, kappa, nullptr, it, rev2)));
+            CUDA_TRY(c, (launch_dslash<1, MODE_QQ>(c, U, c->p, c->q, kappa, nullptr, it, rev2, c->pdl)));
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 1], c->stream));
             // a3: r -= alpha D q, rr', beta, loop condition
             // (fuse_y: y += alpha p in the same pass, then a4 is p = r + beta p alone; same arithmetic per element)
             const bool fy = c->fuse_y && c->recon == 18;
-            if (fy) CUDA_TRY(c, launch_dslash_y(c, U, kappa, it, rev3));
-            else CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it, rev3)));
+            if (fy) CUDA_TRY(c, launch_dslash_y(c, U, kappa, it, rev3, c->pdl));
+            else CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it, rev3, c->pdl)));
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 2], c->stream));
             // a4: y += alpha p ; p = r + beta p
-            if (fy && c->precision == 32)
-                cg_pupdate_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((float4 *)c->p, (const float4 *)c->r, n, c->sc, it, rev4);
-            else if (fy)
-                cg_pupdate_kernel<double><<<vgrid, VEC_NT, 0, c->stream>>>((double2 *)c->p, (const double2 *)c->r, n, c->sc, it, rev4);
-            else if (c->precision == 32)
-                cg_update_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((float4 *)c->y, (float4 *)c->p,
-                                                                          (const float4 *)c->r, n, c->sc, it, rev4);
-            else
-                cg_update_kernel<double><<<vgrid, VEC_NT, 0, c->stream>>>((double2 *)c->y, (double2 *)c->p,
-                                                                           (const double2 *)c->r, n, c->sc, it, rev4);
+            {
+                cudaLaunchConfig_t lc = {};
+                lc.gridDim = dim3(vgrid); lc.blockDim = dim3(VEC_NT); lc.stream = c->stream;
+                cudaLaunchAttribute at[1];
+                at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+                at[0].val.programmaticStreamSerializationAllowed = 1;
+                lc.attrs = at; lc.numAttrs = c->pdl ? 1 : 0;
+                const CgScalars *scc = c->sc;
+                if (fy && c->precision == 32)
+                    CUDA_TRY(c, cudaLaunchKernelEx(&lc, cg_pupdate_kernel<float>, (float4 *)c->p, (const float4 *)c->r, n, scc, it, rev4));
+                else if (fy)
+                    CUDA_TRY(c, cudaLaunchKernelEx(&lc, cg_pupdate_kernel<double>, (double2 *)c->p, (const double2 *)c->r, n, scc, it, rev4));
+                else if (c->precision == 32)
+                    CUDA_TRY(c, cudaLaunchKernelEx(&lc, cg_update_kernel<float>, (float4 *)c->y, (float4 *)c->p, (const float4 *)c->r, n, scc, it, rev4));
+                else
+                    CUDA_TRY(c, cudaLaunchKernelEx(&lc, cg_update_kernel<double>, (double2 *)c->y, (double2 *)c->p, (const double2 *)c->r, n, scc, it, rev4));
+            }
             c->launches++;
             CUDA_TRY(c, cudaGetLastError());
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 3], c->stream));

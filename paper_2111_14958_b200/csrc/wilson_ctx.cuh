@@ -25,6 +25,7 @@ struct wd_ctx {
     int zchunk_user;      // z layers per rasterisation chunk, 0 = automatic
     int small_tile_user;  // launch configuration of the one-launch CG kernel: -1 = automatic
     int sweep;            // 1: consecutive passes walk the lattice in alternating directions (Geom.rev); 0 (default): all forward
+    int pdl;              // 1: the kernels of the three-kernel CG loop are launched with programmatic stream serialization
     int fuse_y;           // 1: the y update of a4 rides on the a3 pass (MODE_RUPDY), a4 = p <- r + beta p; 0: a4 does both
     unsigned apply_calls; // wd_apply calls so far (their direction alternates too)
     double l2_budget_mb;  // reuse-distance budget of the automatic choice

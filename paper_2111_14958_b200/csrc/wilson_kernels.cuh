@@ -60,6 +60,13 @@ __device__ __forceinline__ void prefetch_l2(const void *p, unsigned int bytes)
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
+// Programmatic dependent launch (wd_set_pdl): a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may be
+// scheduled while its predecessor in the stream still drains; pdl_wait() blocks until that predecessor has completed and
+// its writes are visible, so nothing before it may touch global memory.  pdl_trigger() lets the NEXT kernel of the stream
+// be scheduled as soon as every CTA of this one has issued it.  Both are no-ops in a launch without the attribute.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // CTA rasterisation.  Tiles are visited x, y, z-within-chunk fastest, then t, then z-chunk: the sites a CTA
 // shares with its +-t neighbours (2 spinor layers and one layer of U_t per tile) are then touched again
 // after Lx*Ly*(zc*BZ)*BT sites instead of after a whole t-slice, which keeps them in L2 on lattices whose
@@ -790,6 +797,8 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     static_assert(MODE != MODE_RUPDY || EO == 0, "MODE_RUPDY: plain lattice only (cen carries p)");
     constexpr bool CF = (PIPE == 1) && MODE != MODE_TS && !RU;
     constexpr int HP = (PIPE == 4) ? 1 : PIPE;
+    pdl_trigger();
+    pdl_wait();
     if (MODE != MODE_PLAIN) {
         if (it >= sc->k_stop) return;  // uniform over the grid: over-launched iterations are no-ops
     } else if (sc) {
@@ -1129,6 +1138,8 @@ cg_update_kernel(typename Field<real>::svec *y, typename Field<real>::svec *p,
                  const typename Field<real>::svec *__restrict__ r, size_t n, const CgScalars *sc, int it, int rev)
 {
     using svec = typename Field<real>::svec;
+    pdl_trigger();
+    pdl_wait();
     if (it >= sc->k_stop) return;
     const real alpha = (real)sc->alpha, beta = (real)sc->beta;
     for (size_t j = (size_t)blockIdx.x * VEC_NT + threadIdx.x; j < n; j += (size_t)gridDim.x * VEC_NT) {
@@ -1147,6 +1158,8 @@ cg_pupdate_kernel(typename Field<real>::svec *p, const typename Field<real>::sve
                   const CgScalars *sc, int it, int rev)
 {
     using svec = typename Field<real>::svec;
+    pdl_trigger();
+    pdl_wait();
     if (it >= sc->k_stop) return;
     const real beta = (real)sc->beta;
     for (size_t j = (size_t)blockIdx.x * VEC_NT + threadIdx.x; j < n; j += (size_t)gridDim.x * VEC_NT) {

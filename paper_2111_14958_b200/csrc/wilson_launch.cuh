@@ -115,6 +115,7 @@ struct DslashArgs {
     unsigned int *counter;
     double *hist;
     int it;
+    int pdl = 0;      // 1: launch with programmatic stream serialization (wd_set_pdl; the kernel starts with pdl_wait())
 };
 
 // dagger in {0,1}; mode in {MODE_PLAIN, MODE_QQ (dagger = 1 only), MODE_RUPD (dagger = 0 only)}
@@ -164,6 +165,18 @@ static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
             if (grid > a.g.ntiles) grid = a.g.ntiles;                                                          \
             Geom g = a.g;                                                                                      \
             g.pf = a.prefetch < 0 ? (int)grid : a.prefetch;                                                    \
+            if (a.pdl) {                                                                                       \
+                cudaLaunchConfig_t lc = {};                                                                    \
+                lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3(bx * by * bz * bt);                      \
+                lc.dynamicSmemBytes = dyn; lc.stream = a.stream;                                               \
+                cudaLaunchAttribute at[1];                                                                     \
+                at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                                 \
+                at[0].val.programmaticStreamSerializationAllowed = 1;                                          \
+                lc.attrs = at; lc.numAttrs = 1;                                                                \
+                return cudaLaunchKernelEx(&lc, dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON, EO>, g, \
+                    (const gvec *)a.U, (const gvec *)a.Ub, (const svec *)a.in, (const svec *)a.cen, (svec *)a.out, (real)a.kappa, \
+                    (svec *)a.r, a.sc, a.partials, a.counter, a.hist, a.it);                                   \
+            }                                                                                                  \
             dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON, EO><<<(unsigned)grid, bx * by * bz * bt, dyn, a.stream>>>(  \
                 g, (const gvec *)a.U, (const gvec *)a.Ub, (const svec *)a.in, (const svec *)a.cen, (svec *)a.out, (real)a.kappa, (svec *)a.r, a.sc,   \
                 a.partials, a.counter, a.hist, a.it);                                                          \

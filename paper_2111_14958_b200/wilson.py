@@ -115,6 +115,7 @@ def load_library(path: str = LIB_PATH):
     lib.wd_set_zchunk.argtypes = [vp, ci]
     lib.wd_set_sweep.argtypes = [vp, ci]
     lib.wd_set_fuse_y.argtypes = [vp, ci]
+    lib.wd_set_pdl.argtypes = [vp, ci]
     lib.wd_set_small_tile.argtypes = [vp, ci]
     lib.wd_set_poll_interval.argtypes = [vp, ci]
     lib.wd_set_profile.argtypes = [vp, ci]
@@ -492,6 +493,10 @@ class WilsonContext:
     def wd_set_fuse_y(self, on):
         """1: y += alpha p rides on the a3 stencil pass, a4 is p = r + beta p alone (bit-identical iterates)"""
         self._check(self.lib.wd_set_fuse_y(self._ctx, int(on)))
+
+    def wd_set_pdl(self, on):
+        """1: programmatic dependent launch of the kernels of the three-kernel CG loop (same results)"""
+        self._check(self.lib.wd_set_pdl(self._ctx, int(on)))
 
     def wd_set_poll_interval(self, n):
         self._check(self.lib.wd_set_poll_interval(self._ctx, int(n)))

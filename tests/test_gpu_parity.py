@@ -403,6 +403,45 @@ def test_cg_y_update_inside_the_a3_pass(wilson, oracle, precision):
     assert ran >= 9
 
 
+@pytest.mark.parametrize("precision", [32, 64])
+def test_cg_programmatic_dependent_launch(wilson, oracle, precision):
+    """wd_set_pdl(1): the kernels of the three-kernel loop are launched with programmatic stream serialization and start
+    with griddepcontrol.wait.  Same kernels, same order of memory operations: solution, iteration count and residual
+    history are bit-identical to the plain launches, with and without wd_set_fuse_y, also when the loop over-launches
+    no-op iterations past convergence (poll interval 7) and on a ragged lattice; checked against the oracle as well."""
+    cdt = gu.np_complex(precision)
+    tol = 1e-6 if precision == 32 else 1e-11
+    cfg = inputs.CONFIGS[1]
+    cases = [(cfg.dims, cfg.bc_t, cfg.kappa) + gu.config_fields(1, precision),
+             ((6, 4, 10, 8), -1, 0.12, inputs.gauge_field(CFG_TEST + 6, (6, 4, 10, 8), "near_identity", dtype=cdt),
+              inputs.source_field(CFG_TEST + 6, (6, 4, 10, 8), dtype=cdt))]
+    for dims, bc_t, kappa, U, eta in cases:
+        got = {}
+        for pdl, fy in ((0, 0), (1, 0), (1, 1)):
+            with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+                ctx.wd_set_cg_mode(1)
+                ctx.wd_set_poll_interval(7)
+                ctx.wd_set_pdl(pdl)
+                ctx.wd_set_fuse_y(fy)
+                psi, info = gu.solve_on_gpu(ctx, U, eta, kappa, tol, 500)
+                psi2, info2 = gu.solve_on_gpu(ctx, U, eta, kappa, tol, 500)   # a second solve on the same ctx
+                assert psi.tobytes() == psi2.tobytes() and info["iterations"] == info2["iterations"]
+                got[(pdl, fy)] = (psi, info, ctx.wd_cg_history())
+                with pytest.raises(wilson.WilsonError):
+                    ctx.wd_set_pdl(-1)
+        ref = got[(0, 0)]
+        assert ref[1]["status"] == 0
+        for key in ((1, 0), (1, 1)):
+            assert got[key][1]["status"] == 0 and got[key][1]["iterations"] == ref[1]["iterations"]
+            assert got[key][0].tobytes() == ref[0].tobytes()
+            assert np.array_equal(got[key][2], ref[2])
+        U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+        psi_o, info_o = oracle.cg_solve(dims, U64, eta64, kappa, tol, 500, bc_t)
+        assert iters_close(ref[1]["iterations"], info_o["iterations"])
+        res = oracle.true_residual(dims, U64, eta64, got[(1, 0)][0].astype(np.complex128), kappa, bc_t)
+        assert res <= 2.0 * oracle.true_residual(dims, U64, eta64, psi_o, kappa, bc_t)
+
+
 @pytest.mark.parametrize("mode", [1, 2, 6])
 def test_cg_edge_cases(wilson, oracle, mode):
     cfg = inputs.CONFIGS[0]
