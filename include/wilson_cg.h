@@ -63,7 +63,9 @@ extern "C" {
 
 #define WD_OK 0
 #define WD_NOT_CONVERGED 1
-#define WD_BREAKDOWN 2       /* bicgstab_solve only: a denominator of the recurrence vanished; psi holds the last iterate */
+#define WD_BREAKDOWN 2       /* the loop stopped without converging and without reaching max_iter: a denominator of the
+                                BiCGSTAB recurrence vanished, or (every solver) the residual norm is not a number because U,
+                                eta or a step length is not finite; info->converged = 0, psi holds the last iterate */
 #define WD_ERR_ARG (-1)     /* NULL pointer, aliasing out == in, non-finite kappa, r_min <= 0, max_iter < 0 */
 #define WD_ERR_DIMS (-2)    /* an extent < 4 (forward and backward neighbours must be distinct sites) or volume too large */
 #define WD_ERR_CUDA (-3)    /* a CUDA runtime call or kernel launch failed; wd_last_error() has the CUDA string */
@@ -165,9 +167,11 @@ int wd_apply_repeat(wd_ctx *ctx, const void *U_native, const void *psi_native, v
  *     psi <- D-dagger y
  * alpha, beta, rr, k and the loop condition live in device memory; the host only polls.
  *   U_native, eta_native: device inputs (native layout); psi_native_out: device output, must not alias eta.
- *   r_min: relative tolerance (> 0); max_iter >= 0.  eta == 0 gives psi = 0, 0 iterations, WD_OK.
- *   info: host pointer, may be NULL.
- * Returns WD_OK, WD_NOT_CONVERGED or an error.  Synchronous (returns after info is filled).
+ *   r_min: relative tolerance (> 0); max_iter >= 0 (INT_MAX = no limit; the residual history then keeps its first
+ *   2^20 entries).  eta == 0 gives psi = 0, 0 iterations, WD_OK.
+ *   info: host pointer, may be NULL.  info->converged = 1 iff sqrt(rr) < r_min*sqrt(<eta,eta>) held (a true comparison:
+ *   a NaN or infinite residual stops the loop but is reported as WD_BREAKDOWN, never as converged).
+ * Returns WD_OK, WD_NOT_CONVERGED, WD_BREAKDOWN or an error.  Synchronous (returns after info is filled).
  */
 int cg_solve(wd_ctx *ctx, const void *U_native, const void *eta_native, void *psi_native_out,
              double kappa, double r_min, int max_iter, wd_cg_info *info);
@@ -309,8 +313,8 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  * Tuning knobs (the paper's workgroup-size tuning):
  *   wd_num_tiles()            number of compiled stencil launch configurations ("tiles").
  *   wd_tile_shape(i, shape)   writes {BX,BY,BZ,BT} of tile i (threads per CTA = product); returns 0 or WD_ERR_ARG.
- *   wd_tile_info(i, info)     writes {min resident CTAs per SM asked of the compiler, 1 if the hop loop is
- *                             software-pipelined, 1 if also compiled for precision 64}.
+ *   wd_tile_info(i, info)     writes {min resident CTAs per SM asked of the compiler, 1 if compiled for precision 32,
+ *                             1 if compiled for precision 64}.
  *   wd_set_tile(ctx, i)       select tile i for the stencil kernels of this ctx; i = -1 restores the automatic choice.
  *   wd_get_tile(ctx)          index in use.
  *   wd_set_cg_mode(ctx, m)        0 = automatic (one cooperative launch for the whole solve when V <= 200000 sites in fp32 /
@@ -319,26 +323,10 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *                             phases; same recurrence and precision), 6 = always one launch with a CTA of 32 sites x 4
  *                             directions: warp mu computes the two hops of direction mu, the partial sums meet in shared
  *                             memory (the automatic choice in fp64 up to 8192 sites).
- *   wd_set_prefetch(ctx, n)       L2 bulk-prefetch distance of the stencil kernels in tiles: 0 = off (default: it measured
- *                             slower on B200), -1 = each CTA prefetches the tile it will process next, n > 0 = n tiles ahead.
- *   wd_set_waves(ctx, w)          the stencil kernels run a persistent grid of w * (SMs * resident CTAs per SM) CTAs that
- *                             stride over the tiles; w = 0 or 1: exactly one resident wave (default).
  *   wd_set_zchunk(ctx, layers)    z extent (in sites) of one chunk of the CTA rasterisation x,y,z-in-chunk,t,z-chunk that
  *                             keeps the +-t neighbours of a tile in L2; 0 = automatic (fits a 40 MB reuse distance).
  *   wd_set_small_tile(ctx, i)     launch configuration (CTA tile, register bound) of the one-launch CG kernel of mode 2:
  *                             -1 = automatic (default), 0 <= i < number of compiled configurations.
- *   wd_set_sweep(ctx, a)          a = 1: consecutive passes over the lattice (the three kernels of a cg_solve iteration,
- *                             back-to-back wd_apply calls) walk it in alternating directions, so that each pass starts on
- *                             the data the previous one left in the 126 MB L2; a = 0 (default: the alternation measured no
- *                             gain on B200): every pass walks forward.  The per-site arithmetic is identical; only the
- *                             grouping of the reduction partials changes.
- *   wd_set_fuse_y(ctx, on)        on = 1: in the three-kernel cg_solve the update y <- y + alpha p (half of a4, PAPER.md:47
- *                             "psi <- psi + alpha p") is done inside the a3 stencil pass, which already holds alpha, and a4
- *                             shrinks to p <- r + beta p (1536 B/site per iteration either way; every element sees the same
- *                             operations, so the iterates are bit-identical).  18-real links only (ignored otherwise).
- *   wd_set_pdl(ctx, on)           on = 1: the kernels of the three-kernel cg_solve loop are launched with programmatic stream
- *                             serialization (each starts with griddepcontrol.wait, so it touches memory only after its
- *                             predecessor has completed): launch latency overlaps the drain of the previous kernel.  Same results.
  *   wd_set_poll_interval(ctx, n)  CG iterations enqueued between two host polls of the device stop flag (n >= 1; 0 = automatic).
  */
 int wd_num_tiles(void);
@@ -347,13 +335,8 @@ int wd_tile_info(int index, int info[3]);
 int wd_set_tile(wd_ctx *ctx, int index);
 int wd_get_tile(wd_ctx *ctx);
 int wd_set_cg_mode(wd_ctx *ctx, int mode);
-int wd_set_prefetch(wd_ctx *ctx, int tiles);
-int wd_set_waves(wd_ctx *ctx, int waves);
 int wd_set_zchunk(wd_ctx *ctx, int layers);
-int wd_set_sweep(wd_ctx *ctx, int alternate);
 int wd_set_small_tile(wd_ctx *ctx, int index);
-int wd_set_fuse_y(wd_ctx *ctx, int on);
-int wd_set_pdl(wd_ctx *ctx, int on);
 int wd_set_poll_interval(wd_ctx *ctx, int n);
 
 /*

@@ -44,42 +44,19 @@ extern "C" long wd_selftest_fastdiv(unsigned int d, unsigned int n_max)
 
 // ---------------------------------------------------------------- launches
 template <int DAG, int MODE>
-static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void *out, double kappa, void *r, int it,
-                                 int rev = 0, int pdl = 0)
+static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void *out, double kappa, void *r, int it)
 {
     DslashArgs a;
-    a.pdl = pdl;
     a.g = make_geom(c, c->tile);
-    a.g.rev = rev;
     a.sm_count = c->sm_count;
-    a.waves = c->waves > 0 ? c->waves : 1;
-    a.prefetch = (c->dims[0] % SB == 0 && c->recon == 18) ? c->prefetch : 0;
     a.stream = c->stream;
     a.U = U; a.Ub = U; a.in = in; a.cen = in; a.out = out; a.kappa = kappa; a.r = r;
     a.sc = MODE == MODE_PLAIN ? nullptr : c->sc;
-    a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = it;
+    a.partials = c->partials; a.counter = c->counter; a.hist = hist_at(c, it); a.it = it;
     c->launches++;
     if (c->recon == 12)
         return c->precision == 32 ? launch_dslash12_f32(c->tile, DAG, MODE, a) : launch_dslash12_f64(c->tile, DAG, MODE, a);
     return c->precision == 32 ? launch_dslash_f32(c->tile, DAG, MODE, a) : launch_dslash_f64(c->tile, DAG, MODE, a);
-}
-
-// a3 with the y half of a4 fused in: r -= alpha D q, rr', beta, loop test, y += alpha p  (MODE_RUPDY)
-static cudaError_t launch_dslash_y(wd_ctx *c, const void *U, double kappa, int it, int rev, int pdl)
-{
-    DslashArgs a;
-    a.pdl = pdl;
-    a.g = make_geom(c, c->tile);
-    a.g.rev = rev;
-    a.sm_count = c->sm_count;
-    a.waves = c->waves > 0 ? c->waves : 1;
-    a.prefetch = (c->dims[0] % SB == 0) ? c->prefetch : 0;
-    a.stream = c->stream;
-    a.U = U; a.Ub = U; a.in = c->q; a.cen = c->p; a.out = c->y; a.kappa = kappa; a.r = c->r;
-    a.sc = c->sc;
-    a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = it;
-    c->launches++;
-    return c->precision == 32 ? launch_dslash_y_f32(c->tile, a) : launch_dslash_y_f64(c->tile, a);
 }
 
 static unsigned int vec_grid(const wd_ctx *c, size_t n)
@@ -101,12 +78,12 @@ int wd_ensure_workspace(wd_ctx *c, int max_iter)
         // vector kernels can stream whole buffers
         for (void *b : {c->r, c->p, c->q, c->y}) CUDA_TRY(c, cudaMemsetAsync(b, 0, sb, c->stream));
     }
-    if (max_iter + 1 > c->hist_cap) {
+    if (hist_len(max_iter) > c->hist_cap) {
         if (c->hist) cudaFree(c->hist);
         c->hist = nullptr;
         c->hist_cap = 0;
-        CUDA_TRY(c, cudaMalloc(&c->hist, sizeof(double) * (size_t)(max_iter + 1)));
-        c->hist_cap = max_iter + 1;
+        CUDA_TRY(c, cudaMalloc(&c->hist, sizeof(double) * (size_t)hist_len(max_iter)));
+        c->hist_cap = hist_len(max_iter);
     }
     return WD_OK;
 }
@@ -164,10 +141,6 @@ extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_
     c->tile = auto_tile(c);
     c->l2_budget_mb = 40.0;
     c->small_tile_user = -1;
-    c->fuse_y = 0;
-    c->pdl = 0;
-    c->sweep = 0;      // measured on B200: alternating the walk direction gains nothing
-    c->prefetch = 0;   // measured on B200: bulk L2 prefetch of the next tile slows the stencil by 15-30 %
     bool ok = true;
     ok = ok && cudaMalloc(&c->sc, sizeof(CgScalars)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->counter, sizeof(unsigned int)) == cudaSuccess;
@@ -229,7 +202,7 @@ extern "C" int wd_tile_shape(int index, int shape[4])
 extern "C" int wd_tile_info(int index, int info[3])
 {
     if (index < 0 || index >= WD_NUM_TILES || !info) return WD_ERR_ARG;
-    info[0] = kTiles[index].minb; info[1] = kTiles[index].pipe; info[2] = kTiles[index].f64;
+    info[0] = kTiles[index].minb; info[1] = kTiles[index].f32; info[2] = kTiles[index].f64;
     return WD_OK;
 }
 extern "C" int wd_set_tile(wd_ctx *c, int index)
@@ -267,18 +240,6 @@ extern "C" int wd_set_gauge_recon(wd_ctx *c, int reals)
     return WD_OK;
 }
 extern "C" int wd_get_gauge_recon(wd_ctx *c) { return c ? c->recon : WD_ERR_ARG; }
-extern "C" int wd_set_prefetch(wd_ctx *c, int tiles)
-{
-    if (!c || tiles < -1) return WD_ERR_ARG;
-    c->prefetch = tiles;
-    return WD_OK;
-}
-extern "C" int wd_set_waves(wd_ctx *c, int waves)
-{
-    if (!c || waves < 0) return WD_ERR_ARG;
-    c->waves = waves;
-    return WD_OK;
-}
 extern "C" int wd_set_zchunk(wd_ctx *c, int layers)
 {
     if (!c || layers < 0) return WD_ERR_ARG;
@@ -289,24 +250,6 @@ extern "C" int wd_set_small_tile(wd_ctx *c, int index)
 {
     if (!c || index < -1 || index >= WD_NUM_SMALL_TILES) return WD_ERR_ARG;
     c->small_tile_user = index;
-    return WD_OK;
-}
-extern "C" int wd_set_sweep(wd_ctx *c, int alternate)
-{
-    if (!c || alternate < 0 || alternate > 1) return WD_ERR_ARG;
-    c->sweep = alternate;
-    return WD_OK;
-}
-extern "C" int wd_set_fuse_y(wd_ctx *c, int on)
-{
-    if (!c || on < 0 || on > 1) return WD_ERR_ARG;
-    c->fuse_y = on;
-    return WD_OK;
-}
-extern "C" int wd_set_pdl(wd_ctx *c, int on)
-{
-    if (!c || on < 0 || on > 1) return WD_ERR_ARG;
-    c->pdl = on;
     return WD_OK;
 }
 extern "C" int wd_set_poll_interval(wd_ctx *c, int n)
@@ -387,9 +330,8 @@ extern "C" int wd_apply(wd_ctx *c, const void *U, const void *psi, void *out, do
     if (!c) return WD_ERR_ARG;
     if (!U || !psi || !out || psi == out) return fail(c, WD_ERR_ARG, "wd_apply: NULL argument or out aliases psi");
     if (!std::isfinite(kappa)) return fail(c, WD_ERR_ARG, "wd_apply: kappa is not finite");
-    const int rev = c->sweep ? (int)(c->apply_calls++ & 1u) : 0;   // back-to-back applications alternate (Geom.rev)
-    cudaError_t e = dagger ? launch_dslash<1, MODE_PLAIN>(c, U, psi, out, kappa, nullptr, 0, rev)
-                           : launch_dslash<0, MODE_PLAIN>(c, U, psi, out, kappa, nullptr, 0, rev);
+    cudaError_t e = dagger ? launch_dslash<1, MODE_PLAIN>(c, U, psi, out, kappa, nullptr, 0)
+                           : launch_dslash<0, MODE_PLAIN>(c, U, psi, out, kappa, nullptr, 0);
     CUDA_TRY(c, e);
     return WD_OK;
 }
@@ -507,7 +449,7 @@ static int cg_onelaunch(wd_ctx *c, const void *U, const void *eta, void *psi, do
     a.sm_count = c->sm_count;
     a.stream = c->stream;
     a.U = U; a.eta = eta; a.y = c->y; a.r = c->r; a.p = c->p; a.q = c->q; a.psi = psi;
-    a.kappa = kappa; a.sc = c->sc; a.partials = c->partials; a.partials_cap = c->partials_cap; a.hist = c->hist;
+    a.kappa = kappa; a.sc = c->sc; a.partials = c->partials; a.partials_cap = c->partials_cap; a.hist = hist_whole(c, max_iter);
     a.r_min = r_min; a.max_iter = max_iter;
     c->launches++;
     if (split) CUDA_TRY(c, c->precision == 32 ? launch_cg_split_f32(st, a) : launch_cg_split_f64(st, a));
@@ -542,7 +484,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
             info->kernel_launches = c->launches;
             info->cg_mode = c->last_cg_mode;
         }
-        return s1.converged ? WD_OK : WD_NOT_CONVERGED;
+        return s1.converged ? WD_OK : (s1.breakdown ? WD_BREAKDOWN : WD_NOT_CONVERGED);
     }
     c->last_cg_mode = 1;
     const size_t n = spinor_vecs(c);
@@ -573,39 +515,19 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
         cudaEvent_t *pev = c->profile ? c->pev + 4 * (size_t)pslot * poll : nullptr;
         for (int i = 0; i < chunk; ++i) {
             const int it = first + i;
-            // direction of the three passes of iteration `it`: the init kernel ran forward, every pass after it walks
-            // against the one before (pass number 3 it + j + 1), so each starts on what the last one left in L2
-            const int rev2 = c->sweep ? (3 * it + 1) & 1 : 0, rev3 = c->sweep ? (3 * it + 2) & 1 : 0,
-                      rev4 = c->sweep ? (3 * it + 3) & 1 : 0;
             const bool sample = c->profile && (it % c->profile == 0);
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 0], c->stream));
             // a2: q = D-dagger p, qq, alpha
-            CUDA_TRY(c, (launch_dslash<1, MODE_QQ>(c, U, c->p, c->q, kappa, nullptr, it, rev2, c->pdl)));
+            CUDA_TRY(c, (launch_dslash<1, MODE_QQ>(c, U, c->p, c->q, kappa, nullptr, it)));
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 1], c->stream));
             // a3: r -= alpha D q, rr', beta, loop condition
-            // (fuse_y: y += alpha p in the same pass, then a4 is p = r + beta p alone; same arithmetic per element)
-            const bool fy = c->fuse_y && c->recon == 18;
-            if (fy) CUDA_TRY(c, launch_dslash_y(c, U, kappa, it, rev3, c->pdl));
-            else CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it, rev3, c->pdl)));
+            CUDA_TRY(c, (launch_dslash<0, MODE_RUPD>(c, U, c->q, nullptr, kappa, c->r, it)));
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 2], c->stream));
             // a4: y += alpha p ; p = r + beta p
-            {
-                cudaLaunchConfig_t lc = {};
-                lc.gridDim = dim3(vgrid); lc.blockDim = dim3(VEC_NT); lc.stream = c->stream;
-                cudaLaunchAttribute at[1];
-                at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-                at[0].val.programmaticStreamSerializationAllowed = 1;
-                lc.attrs = at; lc.numAttrs = c->pdl ? 1 : 0;
-                const CgScalars *scc = c->sc;
-                if (fy && c->precision == 32)
-                    CUDA_TRY(c, cudaLaunchKernelEx(&lc, cg_pupdate_kernel<float>, (float4 *)c->p, (const float4 *)c->r, n, scc, it, rev4));
-                else if (fy)
-                    CUDA_TRY(c, cudaLaunchKernelEx(&lc, cg_pupdate_kernel<double>, (double2 *)c->p, (const double2 *)c->r, n, scc, it, rev4));
-                else if (c->precision == 32)
-                    CUDA_TRY(c, cudaLaunchKernelEx(&lc, cg_update_kernel<float>, (float4 *)c->y, (float4 *)c->p, (const float4 *)c->r, n, scc, it, rev4));
-                else
-                    CUDA_TRY(c, cudaLaunchKernelEx(&lc, cg_update_kernel<double>, (double2 *)c->y, (double2 *)c->p, (const double2 *)c->r, n, scc, it, rev4));
-            }
+            if (c->precision == 32)
+                cg_update_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((float4 *)c->y, (float4 *)c->p, (const float4 *)c->r, n, c->sc, it);
+            else
+                cg_update_kernel<double><<<vgrid, VEC_NT, 0, c->stream>>>((double2 *)c->y, (double2 *)c->p, (const double2 *)c->r, n, c->sc, it);
             c->launches++;
             CUDA_TRY(c, cudaGetLastError());
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 3], c->stream));
@@ -633,9 +555,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
     rc = wd_poll_loop(c, max_iter, poll, ahead, enqueue_chunk, polled);
     if (rc != WD_OK) return rc;
     // a6: psi = D-dagger y ("then we multiply the solution by D-dagger")
-    // (against the last a4 that really ran: pass number 3 k, so this is pass 3 k + 1)
-    CUDA_TRY(c, (launch_dslash<1, MODE_PLAIN>(c, U, c->y, psi, kappa, nullptr, 0,
-                                              c->sweep ? (3 * c->sc_host->k + 1) & 1 : 0)));
+    CUDA_TRY(c, (launch_dslash<1, MODE_PLAIN>(c, U, c->y, psi, kappa, nullptr, 0)));
     if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
@@ -653,7 +573,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
         info->kernel_launches = c->launches;
         info->cg_mode = 1;
     }
-    return s.converged ? WD_OK : WD_NOT_CONVERGED;
+    return s.converged ? WD_OK : (s.breakdown ? WD_BREAKDOWN : WD_NOT_CONVERGED);
 }
 
 static int check_cg_args(wd_ctx *c, const void *a, const void *b, const void *out, double kappa, double r_min,
@@ -685,11 +605,9 @@ static cudaError_t launch_dslash_bi(wd_ctx *c, const void *U, const void *in, vo
     DslashArgs a;
     a.g = make_geom(c, c->tile);
     a.sm_count = c->sm_count;
-    a.waves = c->waves > 0 ? c->waves : 1;
-    a.prefetch = 0;
     a.stream = c->stream;
     a.U = U; a.Ub = U; a.in = in; a.cen = in; a.out = out; a.kappa = kappa; a.r = rhat;
-    a.sc = c->sc; a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = it;
+    a.sc = c->sc; a.partials = c->partials; a.counter = c->counter; a.hist = hist_at(c, it); a.it = it;
     c->launches++;
     return c->precision == 32 ? launch_dslash_bi_f32(c->tile, MODE, a) : launch_dslash_bi_f64(c->tile, MODE, a);
 }
@@ -715,17 +633,17 @@ static int bicgstab_loop(wd_ctx *c, const void *U, const void *eta_, void *psi_,
             CUDA_TRY(c, (launch_dslash_bi<MODE_RV>(c, U, p, v, kappa, (void *)eta, it)));
             if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[1], c->stream));
             // s = r - alpha v
-            bi_s_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(s, r, v, n, c->sc, it);
+            bi_s_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(s, r, v, n, c->V, padded(c), c->sc, it);
             if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[2], c->stream));
             // t = D s, <t,s>, <t,t>, omega
             CUDA_TRY(c, (launch_dslash_bi<MODE_TS>(c, U, s, t, kappa, nullptr, it)));
             if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[3], c->stream));
             // psi += alpha p + omega s ; r = s - omega t ; rho', rr, beta, loop test
-            bi_xr_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(psi, r, p, s, t, eta, n, c->sc, c->partials, c->counter,
-                                                               c->hist, it);
+            bi_xr_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(psi, r, p, s, t, eta, n, c->V, padded(c), c->sc, c->partials, c->counter,
+                                                               hist_at(c, it), it);
             if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[4], c->stream));
             // p = r + beta (p - omega v)
-            bi_p_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(p, r, v, n, c->sc, it);
+            bi_p_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(p, r, v, n, c->V, padded(c), c->sc, it);
             if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[5], c->stream));
             c->launches += 3;
             CUDA_TRY(c, cudaGetLastError());

@@ -17,17 +17,11 @@ struct wd_ctx {
     int tile;       // tile index in use
     int tile_user;  // -1 = automatic
     int poll;       // 0 = automatic
-    int waves;            // resident waves of the persistent stencil grid (0 -> 1)
     int cg_mode;          // 0 = automatic, 1 = three kernels per iteration, 2 = one cooperative launch
     int coop_ok;          // device supports cooperative launches
     int last_cg_mode;     // what the last cg_solve used
-    int prefetch;         // L2 prefetch distance: -1 = automatic (one grid ahead), 0 = off, n > 0 = n tiles
     int zchunk_user;      // z layers per rasterisation chunk, 0 = automatic
     int small_tile_user;  // launch configuration of the one-launch CG kernel: -1 = automatic
-    int sweep;            // 1: consecutive passes walk the lattice in alternating directions (Geom.rev); 0 (default): all forward
-    int pdl;              // 1: the kernels of the three-kernel CG loop are launched with programmatic stream serialization
-    int fuse_y;           // 1: the y update of a4 rides on the a3 pass (MODE_RUPDY), a4 = p <- r + beta p; 0: a4 does both
-    unsigned apply_calls; // wd_apply calls so far (their direction alternates too)
     double l2_budget_mb;  // reuse-distance budget of the automatic choice
     int sm_count;
     // CG workspace (native layout), device
@@ -146,8 +140,17 @@ static inline int wd_poll_loop(wd_ctx *c, int max_iter, int poll, bool ahead, En
     return WD_OK;
 }
 
-// CG workspace of the ctx (r, p, q, y at full length, zeroed once; history of max_iter + 1 doubles); wilson_cg.cu
+// CG workspace of the ctx (r, p, q, y at full length, zeroed once; history of min(max_iter, WD_HIST_MAX) + 1 doubles);
+// wilson_cg.cu
 int wd_ensure_workspace(wd_ctx *c, int max_iter);
+
+// The residual history is a measurement aid, not part of the method: its length is capped so that max_iter = INT_MAX
+// ("no limit") neither overflows max_iter + 1 nor asks for gigabytes.  Iterations beyond the cap are not recorded: the
+// host passes a NULL history to their launches (hist_at) and to a one-launch solve that could outrun it (hist_whole).
+constexpr int WD_HIST_MAX = 1 << 20;
+static inline int hist_len(int max_iter) { return (max_iter < WD_HIST_MAX ? max_iter : WD_HIST_MAX) + 1; }
+static inline double *hist_at(const wd_ctx *c, int it) { return (long)it + 1 < (long)c->hist_cap ? c->hist : nullptr; }
+static inline double *hist_whole(const wd_ctx *c, int max_iter) { return (long)max_iter + 1 <= (long)c->hist_cap ? c->hist : nullptr; }
 
 // ---------------------------------------------------------------- geometry helpers shared by the ABI translation units
 static inline wd::FastDiv make_fastdiv(unsigned int d)
@@ -179,7 +182,6 @@ static inline wd::Geom make_geom_lattice(const int dims[4], int bc_t, const int 
     g.bc_t = bc_t;
     g.eo = 0;
     g.par = 0;
-    g.rev = 0;
     const double layer = 600.0 * dims[0] * dims[1] * tb[3];   // bytes per z layer of one t-tile row
     const double budget = l2_budget_mb * 1.0e6;
     int zc = 1;
@@ -192,7 +194,6 @@ static inline wd::Geom make_geom_lattice(const int dims[4], int bc_t, const int 
     }
     g.zc = zc;
     g.ntiles = g.nt[0] * g.nt[1] * g.nt[2] * g.nt[3];
-    g.pf = 0;   // set per launch (needs the grid size)
     g.d_chunk = make_fastdiv((unsigned)(g.nt[0] * g.nt[1] * g.zc * g.nt[3]));
     g.d_nt0 = make_fastdiv((unsigned)g.nt[0]);
     g.d_nt1 = make_fastdiv((unsigned)g.nt[1]);
@@ -221,8 +222,7 @@ static inline int tile_threads(int tile)
 static inline bool tile_ok(const wd_ctx *c, int tile)
 {
     if (tile < 0 || tile >= WD_NUM_TILES) return false;
-    if (c->precision == 64 && !wd::kTiles[tile].f64) return false;
-    return true;
+    return c->precision == 64 ? wd::kTiles[tile].f64 != 0 : wd::kTiles[tile].f32 != 0;
 }
 // Automatic choice: the first row of the table (rows are in order of measured preference) among those compiled
 // for this precision that waste the fewest threads on tiles overhanging the lattice `dims`.

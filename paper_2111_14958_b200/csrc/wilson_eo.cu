@@ -97,9 +97,7 @@ __global__ void eo_set_eta2_kernel(CgScalars *sc, const double *n2, double r_min
 {
     const double eta2 = n2[0] + n2[1];
     sc->eta2 = eta2;
-    const bool go = eta2 > 0.0 && (sqrt(sc->rr) >= r_min * sqrt(eta2));
-    sc->k_stop = go ? max_iter : 0;
-    sc->converged = go ? 0 : 1;
+    loop_begin(sc, sc->rr, eta2, r_min, max_iter);
 }
 
 // one stencil pass on the sites of parity `par`:  out = cen - coef * (hopping sum over the other parity's `in`)
@@ -121,15 +119,13 @@ cudaError_t eo_launch(wd_ctx *c, const void *U_eo, const EoPass &p)
     a.g.eo = 1;
     a.g.par = p.par;
     a.sm_count = c->sm_count;
-    a.waves = c->waves > 0 ? c->waves : 1;
-    a.prefetch = 0;
     a.stream = c->stream;
     const size_t hg = half_gauge_bytes(c);
     a.U = (const char *)U_eo + (size_t)p.par * hg;
     a.Ub = (const char *)U_eo + (size_t)(1 - p.par) * hg;
     a.in = p.in; a.cen = p.cen; a.out = p.out; a.kappa = p.coef; a.r = p.r;
     a.sc = (p.mode != MODE_PLAIN || p.in_loop) ? c->sc : nullptr;
-    a.partials = c->partials; a.counter = c->counter; a.hist = c->hist; a.it = p.it;
+    a.partials = c->partials; a.counter = c->counter; a.hist = hist_at(c, p.it); a.it = p.it;
     c->launches++;
     if (c->recon == 12)
         return c->precision == 32 ? launch_dslash12_eo_f32(tile, p.dagger, p.mode, a) : launch_dslash12_eo_f64(tile, p.dagger, p.mode, a);
@@ -264,7 +260,7 @@ static int eo_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, void *psi_eo
             CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_RUPD, 0, t, q, nullptr, r, k2, it, true}));
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[4], c->stream));
             // y += alpha p ; p = r + beta p
-            cg_update_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((svec *)y, (svec *)p, (const svec *)r, n, c->sc, it, 0);
+            cg_update_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((svec *)y, (svec *)p, (const svec *)r, n, c->sc, it);
             c->launches++;
             CUDA_TRY(c, cudaGetLastError());
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[5], c->stream));
@@ -336,7 +332,7 @@ extern "C" int cg_solve_eo(wd_ctx *c, const void *U_eo, const void *eta_eo, void
         info->kernel_launches = c->launches;
         info->cg_mode = 4;
     }
-    return s.converged ? WD_OK : WD_NOT_CONVERGED;
+    return s.converged ? WD_OK : (s.breakdown ? WD_BREAKDOWN : WD_NOT_CONVERGED);
 }
 
 // ---------------------------------------------------------------- even-odd preconditioned BiCGSTAB (readings E1 + B1)
@@ -385,7 +381,7 @@ static int eo_bicgstab_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, voi
             CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_RV, 0, to, p, v, (void *)etah, k2, it, true}));
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[2], c->stream));
             // s = r - alpha v
-            bi_s_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(s, r, v, n, c->sc, it);
+            bi_s_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(s, r, v, n, e.Vh, pad, c->sc, it);
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[3], c->stream));
             // to = H_oe s
             CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_PLAIN, 1, s, nullptr, to, nullptr, -1.0, it, true}));
@@ -394,11 +390,11 @@ static int eo_bicgstab_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, voi
             CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_TS, 0, to, s, t, nullptr, k2, it, true}));
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[5], c->stream));
             // psi_e += alpha p + omega s ; r = s - omega t ; rho', rr, beta, loop test
-            bi_xr_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((svec *)psi_e, r, p, s, t, etah, n, c->sc, c->partials,
-                                                               c->counter, c->hist, it);
+            bi_xr_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((svec *)psi_e, r, p, s, t, etah, n, e.Vh, pad, c->sc, c->partials,
+                                                               c->counter, hist_at(c, it), it);
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[6], c->stream));
             // p = r + beta (p - omega v)
-            bi_p_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(p, r, v, n, c->sc, it);
+            bi_p_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(p, r, v, n, e.Vh, pad, c->sc, it);
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[7], c->stream));
             c->launches += 3;
             CUDA_TRY(c, cudaGetLastError());
@@ -463,7 +459,7 @@ static int eo_bicgstab_onelaunch(wd_ctx *c, const void *U_eo, const void *eta_eo
     a.eta_e = eta_eo; a.eta_o = (const char *)eta_eo + hs;
     a.psi_e = psi_eo; a.psi_o = (char *)psi_eo + hs;
     a.r = c->r; a.p = c->p; a.v = c->q; a.s = c->y; a.t = c->w7; a.to = c->w5; a.etah = c->w6;
-    a.kappa = kappa; a.sc = c->sc; a.partials = c->partials; a.partials_cap = c->partials_cap; a.hist = c->hist;
+    a.kappa = kappa; a.sc = c->sc; a.partials = c->partials; a.partials_cap = c->partials_cap; a.hist = hist_whole(c, max_iter);
     a.r_min = r_min; a.max_iter = max_iter;
     c->launches++;
     CUDA_TRY(c, c->precision == 32 ? launch_eo_bicgstab_onelaunch_f32(best, a) : launch_eo_bicgstab_onelaunch_f64(best, a));

@@ -124,7 +124,7 @@ eo_bicgstab_onelaunch_kernel(const Geom g0, const typename Field<real>::gvec *__
     real acc[24];                                                                                              \
     {                                                                                                          \
         real c_[24], rv_[24];                                                                                  \
-        hopping_sum<0, 0, false, false, real, svec, gvec, 18, 0, 1, false>(                                    \
+        hopping_sum<0, 0, false, false, real, svec, gvec, 18, 1, false>(                                       \
             (PAR) ? gO : gE, (PAR) ? Uo : Ue, (PAR) ? Ue : Uo, in, (const svec *)nullptr, (const svec *)nullptr, x, y, z, t, s, \
             acc, c_, rv_);                                                                                     \
     }
@@ -148,7 +148,7 @@ eo_bicgstab_onelaunch_kernel(const Geom g0, const typename Field<real>::gvec *__
     const double eta2 = get(1);
     double rho[2] = {rr, 0.0}, alpha[2] = {0.0, 0.0}, omega[2] = {0.0, 0.0}, beta[2] = {0.0, 0.0};
     int k = 0, breakdown = 0;
-    bool go = eta2 > 0.0 && (sqrt(rr) >= r_min * sqrt(eta2));
+    bool go = isfinite(eta2) && isfinite(rr) && eta2 > 0.0 && loop_test(rr, eta2, r_min).go;
     if (blockIdx.x == 0 && tid == 0 && hist) hist[0] = rr;
 
     while (go && k < max_iter) {
@@ -285,8 +285,8 @@ eo_bicgstab_onelaunch_kernel(const Geom g0, const typename Field<real>::gvec *__
         sc->rho[0] = rho[0]; sc->rho[1] = rho[1]; sc->calpha[0] = alpha[0]; sc->calpha[1] = alpha[1];
         sc->omega[0] = omega[0]; sc->omega[1] = omega[1]; sc->cbeta[0] = beta[0]; sc->cbeta[1] = beta[1];
         sc->k = k; sc->k_stop = k; sc->max_iter = max_iter;
-        sc->converged = (eta2 == 0.0 || !(sqrt(rr) >= r_min * sqrt(eta2))) ? 1 : 0;
-        sc->breakdown = breakdown;
+        sc->converged = (eta2 == 0.0 || loop_test(rr, eta2, r_min).converged) ? 1 : 0;
+        sc->breakdown = (breakdown || (!go && !sc->converged)) ? 1 : 0;   // a stop that is not a convergence: NaN or vanishing denominator
     }
 }
 
@@ -299,11 +299,11 @@ static cudaError_t launch_eo_bicgstab_onelaunch_any(int tile, const EoOneLaunchA
 #define Z(i, bx, by, bz, bt)                                                                                   \
     case i: {                                                                                                  \
         auto kern = eo_bicgstab_onelaunch_kernel<real, bx, by, bz, bt>;                                        \
-        static int occ = 0;                                                                                    \
-        if (!occ) {                                                                                            \
-            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, bx * by * bz * bt, 0);   \
+        static int occ_tab[WD_MAXDEV];                                                                         \
+        int occ = 0;                                                                                           \
+        {                                                                                                      \
+            cudaError_t e = cached_occupancy(occ_tab, kern, bx * by * bz * bt, 0, &occ);                       \
             if (e != cudaSuccess) return e;                                                                    \
-            if (occ < 1) return cudaErrorLaunchOutOfResources;                                                 \
         }                                                                                                      \
         long grid = (long)occ * a.sm_count;            /* all CTAs must be co-resident (grid barrier) */       \
         if (grid > a.g.ntiles) grid = a.g.ntiles;                                                              \

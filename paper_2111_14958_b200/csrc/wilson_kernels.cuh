@@ -41,31 +41,11 @@ struct Geom {
     int bc_t;    // -1 antiperiodic, +1 periodic
     int zc;      // z tiles per chunk of the CTA rasterisation (see tile_of_block)
     int ntiles;  // nt[0]*nt[1]*nt[2]*nt[3]
-    int pf;      // L2 prefetch distance in tiles (0 = off; needs Lx % 16 == 0 so that a 16-site run is one block)
     int eo;      // 1: the lattice of this launch is ONE PARITY of the real lattice (even-odd preconditioning, SURVEY.md
                  //    8(f3)): L[0] = Lx/2, site (xh,y,z,t) stands for x = 2 xh + ((y+z+t+par) & 1); 0: plain lattice
     int par;     // eo = 1: parity (x+y+z+t) & 1 of the sites this launch WRITES; its neighbours have parity 1 - par
-    int rev;     // 1: the persistent CTAs walk the rasterisation from its LAST tile to its first.  Consecutive passes of a
-                 //    solver alternate the direction, so that a pass starts on the ~100 MB the previous one left in L2
-                 //    (its output and the links it read last) instead of on the lines that were evicted first
     FastDiv d_chunk, d_nt0, d_nt1, d_zc, d_zlast;   // per_chunk, nt[0], nt[1], zc, size of the last z chunk
 };
-
-// Bulk prefetch of `bytes` (multiple of 16) contiguous bytes into L2 (sm_90+: cp.async.bulk.prefetch.L2).
-// It holds no register and no shared memory while in flight: the DRAM latency of the NEXT tile is paid by L2,
-// and the loads of that tile later hit L2 (~1/3 of the DRAM latency), which is what the register-held
-// software pipeline of the hop loop can cover.
-__device__ __forceinline__ void prefetch_l2(const void *p, unsigned int bytes)
-{
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
-}
-
-// Programmatic dependent launch (wd_set_pdl): a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may be
-// scheduled while its predecessor in the stream still drains; pdl_wait() blocks until that predecessor has completed and
-// its writes are visible, so nothing before it may touch global memory.  pdl_trigger() lets the NEXT kernel of the stream
-// be scheduled as soon as every CTA of this one has issued it.  Both are no-ops in a launch without the attribute.
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // CTA rasterisation.  Tiles are visited x, y, z-within-chunk fastest, then t, then z-chunk: the sites a CTA
 // shares with its +-t neighbours (2 spinor layers and one layer of U_t per tile) are then touched again
@@ -377,74 +357,6 @@ __device__ __forceinline__ void reconstruct(const real g[12], real sg, real acc[
     }
 }
 
-// ---------------------------------------------------------------- forward links through shared memory (PIPE = 3)
-// The four forward links U_mu(x) of a site are read exactly once per pass, by the thread that owns x: a pure stream
-// that always misses the caches.  PIPE = 3 takes them out of the register-held software pipeline: every thread
-// copies the links of ITS site of the NEXT tile into its own shared-memory slots with cp.async (no register is held
-// while the copy is in flight, the copy is issued half a tile ahead of its use, and because a thread only ever
-// reads what it copied itself no barrier is needed, only cp.async.wait_all).  Slots are plane-major
-// ([chunk][thread]) so that the 128-bit shared loads of a warp are conflict-free.
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem)
-                 : "memory");
-}
-__device__ __forceinline__ void cp_async8(void *smem, const void *gmem)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem)
-                 : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
-template <int NT>
-__device__ __forceinline__ void stage_links(const float2 *__restrict__ U, int s, void *smem, int tid)
-{
-    float4 *sm4 = reinterpret_cast<float4 *>(smem);
-    float2 *sm2 = reinterpret_cast<float2 *>(sm4 + 16 * NT);
-    const float2 *blk = U + (size_t)(s >> SB_SHIFT) * (36 * SB);
-    const int lane = s & (SB - 1);
-#pragma unroll
-    for (int mu = 0; mu < 4; ++mu) {
-        const float4 *p4 = reinterpret_cast<const float4 *>(blk + mu * 9 * SB) + lane;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) cp_async16(sm4 + (mu * 4 + q) * NT + tid, p4 + q * SB);
-        cp_async8(sm2 + mu * NT + tid, blk + mu * 9 * SB + 8 * SB + lane);
-    }
-}
-template <int NT>
-__device__ __forceinline__ void stage_links(const double2 *__restrict__ U, int s, void *smem, int tid)
-{
-    double2 *sm = reinterpret_cast<double2 *>(smem);
-    const double2 *p = U + gauge_index(s);
-#pragma unroll
-    for (int k = 0; k < 36; ++k) cp_async16(sm + k * NT + tid, p + k * SB);
-}
-template <int MU, int NT>
-__device__ __forceinline__ void load_link_sm(const float2 *, const void *smem, int tid, float u[18])
-{
-    const float4 *sm4 = reinterpret_cast<const float4 *>(smem);
-    const float2 *sm2 = reinterpret_cast<const float2 *>(sm4 + 16 * NT);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const float4 t = sm4[(MU * 4 + q) * NT + tid];
-        u[4 * q] = t.x; u[4 * q + 1] = t.y; u[4 * q + 2] = t.z; u[4 * q + 3] = t.w;
-    }
-    const float2 t2 = sm2[MU * NT + tid];
-    u[16] = t2.x; u[17] = t2.y;
-}
-template <int MU, int NT>
-__device__ __forceinline__ void load_link_sm(const double2 *, const void *smem, int tid, double u[18])
-{
-    const double2 *sm = reinterpret_cast<const double2 *>(smem);
-#pragma unroll
-    for (int k = 0; k < 9; ++k) {
-        const double2 t = sm[(MU * 9 + k) * NT + tid];
-        u[2 * k] = t.x; u[2 * k + 1] = t.y;
-    }
-}
-// bytes of shared memory per thread of a PIPE = 3 kernel
-template <typename real> constexpr int staged_link_bytes() { return 72 * (int)sizeof(real); }
-
 // One hop, split into its loads and its arithmetic so that the loads of the next hop can be in flight
 // while this one is computed:  acc += sg (1 + S gamma_MU) (x) [U or U^dagger](link_site) in(spinor_site).
 // RO = true: `in` is not written while the kernel runs -> read-only (non-coherent) path; false: coherent loads
@@ -526,12 +438,11 @@ __device__ __forceinline__ Hops neighbours(const Geom &g, int x, int y, int z, i
 // same cache lines), and every hop is accumulated with the factor -kappa folded into its boundary sign, so that on
 // return acc = in(s) - kappa * hops = (D in)(s) and c is not touched: no centre fetch at the end of the tile's life
 // (when its lines have left the L1), one dependent load step and 24 live registers fewer in the epilogue.
-template <int DAG, int PIPE, bool LOADR, bool RO, typename real, typename svec, typename gvec, int RECON = 18, int NT = 0,
+template <int DAG, int PIPE, bool LOADR, bool RO, typename real, typename svec, typename gvec, int RECON = 18,
           int EO = 0, bool CFIRST = false>
 __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restrict__ U, const gvec *__restrict__ UB,
                                             const svec *in, const svec *cen, const svec *r, int x, int y, int z, int t,
-                                            int s, real acc[24], real c[24], real rv[24], void *smem = nullptr,
-                                            int next_s = -1, real kappa = 0)
+                                            int s, real acc[24], real c[24], real rv[24], real kappa = 0)
 {
     static_assert(!CFIRST || PIPE == 1, "centre-first is implemented for the two-buffer pipeline");
     constexpr int SF = DAG ? +1 : -1;
@@ -571,43 +482,6 @@ __device__ __forceinline__ void hopping_sum(const Geom &g, const gvec *__restric
         if (!CFIRST) load_centre<RO, EO != 0>(cen, s, c);
         hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
         if (LOADR) load_spinor_rw(r, s, rv);   // after the last hop: an earlier fetch costs registers (spills at 128)
-    } else if (PIPE == 2) {
-        // three register buffers: two hops (336 B fp32 per thread) in flight while a third is computed
-        real va[24], ua[18], vb[24], ub[18], vc[24], uc[18];
-        hop_load<0, RO, RECON, real>(U, in, s, n.f[0], va, ua);
-        hop_load<0, RO, RECON, real>(UB, in, n.b[0], n.b[0], vb, ub);
-        hop_load<1, RO, RECON, real>(U, in, s, n.f[1], vc, uc);          hop_compute<0, SF, false, real>(va, ua, one, acc);
-        hop_load<1, RO, RECON, real>(UB, in, n.b[1], n.b[1], va, ua);     hop_compute<0, -SF, true, real>(vb, ub, one, acc);
-        hop_load<2, RO, RECON, real>(U, in, s, n.f[2], vb, ub);          hop_compute<1, SF, false, real>(vc, uc, one, acc);
-        hop_load<2, RO, RECON, real>(UB, in, n.b[2], n.b[2], vc, uc);     hop_compute<1, -SF, true, real>(va, ua, one, acc);
-        hop_load<3, RO, RECON, real>(U, in, s, n.f[3], va, ua);          hop_compute<2, SF, false, real>(vb, ub, one, acc);
-        hop_load<3, RO, RECON, real>(UB, in, n.b[3], n.b[3], vb, ub);     hop_compute<2, -SF, true, real>(vc, uc, one, acc);
-        load_centre<RO, EO != 0>(cen, s, c);
-        if (LOADR) load_spinor_rw(r, s, rv);
-        hop_compute<3, SF, false, real>(va, ua, sgf, acc);
-        hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
-    } else if (PIPE == 3) {
-        // forward hops first, their links from this thread's shared-memory slots (staged one tile ahead); only the
-        // neighbour spinors (and, in the second half, the backward links) go through the register pipeline
-        const int tid = threadIdx.x;
-        real va[24], vb[24], ua[18], ub[18], us[18];
-        load_spinor_sel<RO>(in, n.f[0], va);
-        load_spinor_sel<RO>(in, n.f[1], vb);
-        load_link_sm<0, NT>(U, smem, tid, us);               hop_compute<0, SF, false, real>(va, us, one, acc);
-        load_spinor_sel<RO>(in, n.f[2], va);
-        load_link_sm<1, NT>(U, smem, tid, us);               hop_compute<1, SF, false, real>(vb, us, one, acc);
-        load_spinor_sel<RO>(in, n.f[3], vb);
-        load_link_sm<2, NT>(U, smem, tid, us);               hop_compute<2, SF, false, real>(va, us, one, acc);
-        hop_load<0, RO, RECON, real>(UB, in, n.b[0], n.b[0], va, ua);
-        load_link_sm<3, NT>(U, smem, tid, us);               hop_compute<3, SF, false, real>(vb, us, sgf, acc);
-        // the slots are free: stage the forward links of this thread's site of the next tile
-        if (next_s >= 0) stage_links<NT>(U, next_s, smem, tid);
-        hop_load<1, RO, RECON, real>(UB, in, n.b[1], n.b[1], vb, ub);  hop_compute<0, -SF, true, real>(va, ua, one, acc);
-        hop_load<2, RO, RECON, real>(UB, in, n.b[2], n.b[2], va, ua);  hop_compute<1, -SF, true, real>(vb, ub, one, acc);
-        hop_load<3, RO, RECON, real>(UB, in, n.b[3], n.b[3], vb, ub);  hop_compute<2, -SF, true, real>(va, ua, one, acc);
-        load_centre<RO, EO != 0>(cen, s, c);
-        hop_compute<3, -SF, true, real>(vb, ub, sgb, acc);
-        if (LOADR) load_spinor_rw(r, s, rv);
     }
 }
 
@@ -697,6 +571,33 @@ __device__ __forceinline__ bool grid_sum_n(const double v[N], double *partials, 
     return false;
 }
 
+// The while-test of PAPER.md:47 read as relative 2-norm (G4): the loop goes on while sqrt(rr) >= r_min sqrt(eta2).  It
+// STOPS as soon as that comparison fails -- also when rr is NaN or infinite (a non-finite link or source, qq = 0) --
+// but `converged` is set only by the true comparison sqrt(rr) < r_min sqrt(eta2); a stop that is not a convergence
+// raises `breakdown` and the solver returns WD_BREAKDOWN, never WD_OK with a NaN field.
+struct LoopTest {
+    bool go, converged;
+};
+__device__ __forceinline__ LoopTest loop_test(double rr, double eta2, double r_min)
+{
+    LoopTest t;
+    const double rn = sqrt(rr), thr = r_min * sqrt(eta2);
+    t.go = rn >= thr;
+    t.converged = rn < thr;
+    return t;
+}
+// state before the first iteration, rr = <r0,r0> (r0 = eta: rr = eta2, or the Schur source with eta2 the full norm):
+// eta2 = 0 means psi = 0 is the solution (converged, no iteration); a non-finite norm is a breakdown
+__device__ __forceinline__ void loop_begin(CgScalars *sc, double rr, double eta2, double r_min, int max_iter)
+{
+    const LoopTest t = loop_test(rr, eta2, r_min);
+    const bool finite = isfinite(rr) && isfinite(eta2);
+    const bool go = finite && eta2 > 0.0 && t.go;
+    sc->k_stop = go ? max_iter : 0;
+    sc->converged = (finite && !go) ? 1 : 0;
+    sc->breakdown = finite ? 0 : 1;
+}
+
 // Scalar epilogues, run by one thread of the last CTA.
 __device__ __forceinline__ void finish_qq(CgScalars *sc, double qq)
 {
@@ -710,9 +611,11 @@ __device__ __forceinline__ void finish_rr(CgScalars *sc, double rr_new, int it, 
     sc->k = it + 1;
     if (hist) hist[it + 1] = rr_new;
     // while |r| >= r_min read as relative 2-norm (G4): stop as soon as it fails
-    if (!(sqrt(rr_new) >= sc->r_min * sqrt(sc->eta2))) {
+    const LoopTest t = loop_test(rr_new, sc->eta2, sc->r_min);
+    if (!t.go) {
         sc->k_stop = it + 1;
-        sc->converged = 1;
+        if (t.converged) sc->converged = 1;
+        else sc->breakdown = 1;              // rr is not a number: alpha or the fields are not finite
     }
 }
 
@@ -747,9 +650,11 @@ __device__ __forceinline__ void finish_bi(CgScalars *sc, const double rho_new[2]
     sc->rr = rr_new;
     sc->k = it + 1;
     if (hist) hist[it + 1] = rr_new;
-    if (!(sqrt(rr_new) >= sc->r_min * sqrt(sc->eta2))) {
+    const LoopTest lt = loop_test(rr_new, sc->eta2, sc->r_min);
+    if (!lt.go) {
         sc->k_stop = it + 1;
-        sc->converged = 1;
+        if (lt.converged) sc->converged = 1;
+        else sc->breakdown = 1;
         return;
     }
     double a[2], b[2];
@@ -766,18 +671,16 @@ __device__ __forceinline__ void finish_bi(CgScalars *sc, const double rho_new[2]
 }
 
 // ---------------------------------------------------------------- the stencil kernel
-enum { MODE_PLAIN = 0, MODE_QQ = 1, MODE_RUPD = 2, MODE_RV = 3, MODE_TS = 4, MODE_RUPDY = 5 };
+enum { MODE_PLAIN = 0, MODE_QQ = 1, MODE_RUPD = 2, MODE_RV = 3, MODE_TS = 4 };
 
 // MODE_PLAIN : out = D in / D-dagger in                                  (wd_apply, a6, a7)
 // MODE_QQ    : out = q = D-dagger p, qq = |q|^2, alpha = rr/qq           (a2)
 // MODE_RUPD  : s = D q (not stored), r <- r - alpha s, rr' = |r|^2, beta, loop condition   (a3)
-// MODE_RUPDY : MODE_RUPD and, in the same pass, y <- y + alpha p (y passed as `out`, p as `cen`, plain lattice only):
-//              the y half of a4 rides on the latency-bound stencil pass, a4 shrinks to p <- r + beta p   (a3 + a4y)
 // MODE_RV    : out = v = D p, <rhat, v> (rhat passed as `r`, read only), alpha = rho/<rhat,v>   (BiCGSTAB)
 // MODE_TS    : out = t = D s, <t,s> and <t,t>, omega = <t,s>/<t,t>                              (BiCGSTAB)
 // EO = 0: plain lattice (UB and cen are ignored: the backward links come from U, the diagonal term from `in`);
 // EO = 1: the launch covers one parity of the lattice (even-odd preconditioning, Geom.eo / Geom.par).
-template <typename real, int DAG, int MODE, int BX, int BY, int BZ, int BT, int MINB, int PIPE, int RECON = 18, int EO = 0>
+template <typename real, int DAG, int MODE, int BX, int BY, int BZ, int BT, int MINB, int RECON = 18, int EO = 0>
 __global__ void __launch_bounds__(BX *BY *BZ *BT, MINB)
 dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
               const typename Field<real>::gvec *__restrict__ UB, const typename Field<real>::svec *__restrict__ in,
@@ -788,17 +691,12 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     using svec = typename Field<real>::svec;
     using gvec = typename Field<real>::gvec;
     constexpr int NT = BX * BY * BZ * BT;
-    // PIPE = 1: the two-buffer pipeline with the diagonal term FIRST (hopping_sum CFIRST) wherever the pass has no
-    // second per-site stream: measured at 48^3x96 fp32, a2 999 -> 920-934 us, wd_apply 990 -> 940 us.  MODE_RUPD keeps
+    // The two-buffer pipeline with the diagonal term FIRST (hopping_sum CFIRST) wherever the pass has no second
+    // per-site stream: measured at 48^3x96 fp32, a2 999 -> 920-934 us, wd_apply 990 -> 940 us.  MODE_RUPD keeps
     // the centre and r last: centre-first made a3 slower (1017 -> 1086 us), and so did folding r into the
     // accumulator as well (acc = r - alpha in, hops scaled by alpha kappa: 1056 us).  MODE_TS needs s(x) beside t(x).
-    // PIPE = 4: the same pipeline with the centre last in every mode (the comparison row of the table).
-    constexpr bool RU = MODE == MODE_RUPD || MODE == MODE_RUPDY;
-    static_assert(MODE != MODE_RUPDY || EO == 0, "MODE_RUPDY: plain lattice only (cen carries p)");
-    constexpr bool CF = (PIPE == 1) && MODE != MODE_TS && !RU;
-    constexpr int HP = (PIPE == 4) ? 1 : PIPE;
-    pdl_trigger();
-    pdl_wait();
+    constexpr bool RU = MODE == MODE_RUPD;
+    constexpr bool CF = MODE != MODE_TS && !RU;
     if (MODE != MODE_PLAIN) {
         if (it >= sc->k_stop) return;  // uniform over the grid: over-launched iterations are no-ops
     } else if (sc) {
@@ -808,53 +706,19 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     const int lx = tid % BX, ly = (tid / BX) % BY, lz = (tid / (BX * BY)) % BZ, lt = tid / (BX * BY * BZ);
     const real alpha = RU ? (real)sc->alpha : (real)0;
     double local = 0.0, local1 = 0.0, local2 = 0.0;
-    extern __shared__ __align__(16) unsigned char wd_dyn_smem[];   // PIPE = 3: staged forward links, 72 reals per thread
-    // site of this thread in tile b, or -1 (no such tile / thread outside the lattice)
-    auto site_in_tile = [&](int v) -> int {   // v: position in the walk
-        if (v >= g.ntiles) return -1;
-        int tx, ty, tz, tt;
-        tile_of_block(g, g.rev ? g.ntiles - 1 - v : v, tx, ty, tz, tt);
-        const int x = tx * BX + lx, y = ty * BY + ly, z = tz * BZ + lz, t = tt * BT + lt;
-        if (x >= g.L[0] || y >= g.L[1] || z >= g.L[2] || t >= g.L[3]) return -1;
-        return x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
-    };
-    if (PIPE == 3) {
-        const int s0 = site_in_tile(blockIdx.x);
-        if (s0 >= 0) stage_links<NT>(U, s0, wd_dyn_smem, tid);
-    }
     // Persistent CTAs: the grid is one resident wave; CTA i takes tiles i, i + gridDim.x, ... so that at any
     // moment the chip works on gridDim.x consecutive tiles of the rasterisation (L2 locality) and the
     // reduction epilogue (barriers, fence, ticket) is paid once per CTA, not once per tile.
-    for (int v = blockIdx.x; v < g.ntiles; v += gridDim.x) {
-        const int b = g.rev ? g.ntiles - 1 - v : v;   // position v of the walk -> tile of the rasterisation
+    for (int b = blockIdx.x; b < g.ntiles; b += gridDim.x) {
         int tx, ty, tz, tt;
-        if (BX % SB == 0 && g.pf > 0 && (lx % SB) == 0 && v + g.pf < g.ntiles) {
-            // one thread per 16-site run of the tile `pf` tiles ahead: its spinor block, its gauge block (and r)
-            tile_of_block(g, g.rev ? b - g.pf : b + g.pf, tx, ty, tz, tt);
-            const int px = tx * BX + lx, py = ty * BY + ly, pz = tz * BZ + lz, pt = tt * BT + lt;
-            if (px < g.L[0] && py < g.L[1] && pz < g.L[2] && pt < g.L[3]) {
-                const int ps = px + g.L[0] * (py + g.L[1] * (pz + g.L[2] * pt));
-                prefetch_l2(in + spinor_index<svec, Field<real>::NSP>(ps), Field<real>::NSP * SB * sizeof(svec));
-                prefetch_l2(U + gauge_index(ps), 36 * SB * sizeof(gvec));
-                if (RU)
-                    prefetch_l2(r + spinor_index<svec, Field<real>::NSP>(ps), Field<real>::NSP * SB * sizeof(svec));
-            }
-        }
         tile_of_block(g, b, tx, ty, tz, tt);
         const int x = tx * BX + lx, y = ty * BY + ly, z = tz * BZ + lz, t = tt * BT + lt;
         const bool active = (x < g.L[0]) && (y < g.L[1]) && (z < g.L[2]) && (t < g.L[3]);
-        int next_s = -1;
-        if (PIPE == 3) {
-            next_s = site_in_tile(v + gridDim.x);
-            cp_async_wait_all();                       // this thread's own copies for tile b have landed
-            if (!active && next_s >= 0) stage_links<NT>(U, next_s, wd_dyn_smem, tid);
-        }
         if (!active) continue;
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24], rv[24];
-        [[maybe_unused]] real yv[24];
-        hopping_sum<DAG, HP, RU || MODE == MODE_RV, true, real, svec, gvec, RECON, NT, EO, CF>(
-            g, U, EO ? UB : U, in, EO ? cen : in, r, x, y, z, t, s, acc, c, rv, wd_dyn_smem, next_s, kappa);
+        hopping_sum<DAG, 1, RU || MODE == MODE_RV, true, real, svec, gvec, RECON, EO, CF>(
+            g, U, EO ? UB : U, in, EO ? cen : in, r, x, y, z, t, s, acc, c, rv, kappa);
         if constexpr (MODE == MODE_TS) {
             // c holds s(x); t(x) = s(x) - kappa * hops replaces it component by component
             real tsr = 0, tsi = 0, tt = 0;
@@ -882,10 +746,6 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
             store_spinor(out, s, c);
             local += (double)dr; local1 += (double)di;
         } else if (RU) {
-            if (MODE == MODE_RUPDY) {                                  // issue the two per-site loads before the r algebra
-                load_spinor(cen, s, acc);                              // p(s)
-                load_spinor_rw(out, s, yv);                            // y(s)
-            }
             real n2 = 0;
 #pragma unroll
             for (int i = 0; i < 24; ++i) {
@@ -894,11 +754,6 @@ dslash_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
             }
             store_spinor(r, s, rv);
             local += (double)n2;
-            if (MODE == MODE_RUPDY) {
-#pragma unroll
-                for (int i = 0; i < 24; ++i) yv[i] = fma(alpha, acc[i], yv[i]);   // y <- y + alpha p (as cg_update_kernel)
-                store_spinor(out, s, yv);
-            }
         } else {
             store_spinor(out, s, c);
             if (MODE == MODE_QQ) {
@@ -996,7 +851,7 @@ cg_onelaunch_kernel(const Geom g, const typename Field<real>::gvec *__restrict__
     const double eta2 = all_cta_sum<NT>(part0, G, sm);
     double rr = eta2, alpha = 0.0, beta = 0.0;
     int k = 0;
-    bool go = eta2 > 0.0 && (sqrt(rr) >= r_min * sqrt(eta2));
+    bool go = isfinite(eta2) && eta2 > 0.0 && loop_test(rr, eta2, r_min).go;
     if (blockIdx.x == 0 && tid == 0 && hist) hist[0] = eta2;
 
     while (go && k < max_iter) {
@@ -1053,7 +908,7 @@ cg_onelaunch_kernel(const Geom g, const typename Field<real>::gvec *__restrict__
         rr = rr_new;
         ++k;
         if (blockIdx.x == 0 && tid == 0 && hist) hist[k] = rr;
-        go = sqrt(rr) >= r_min * sqrt(eta2);                 // while |r| >= r_min (G4)
+        go = loop_test(rr, eta2, r_min).go;                  // while |r| >= r_min (G4)
         grid.sync();                                         // p complete before its neighbours are read
     }
     // a6: psi = D-dagger y
@@ -1068,7 +923,9 @@ cg_onelaunch_kernel(const Geom g, const typename Field<real>::gvec *__restrict__
     if (blockIdx.x == 0 && tid == 0) {
         sc->rr = rr; sc->eta2 = eta2; sc->alpha = alpha; sc->beta = beta; sc->qq = 0.0; sc->r_min = r_min;
         sc->k = k; sc->k_stop = k; sc->max_iter = max_iter;
-        sc->converged = go ? 0 : 1;
+        // converged: psi = 0 for eta = 0, or the true comparison; a loop that stopped otherwise met a NaN (loop_test)
+        sc->converged = (eta2 == 0.0 || loop_test(rr, eta2, r_min).converged) ? 1 : 0;
+        sc->breakdown = (!go && !sc->converged) ? 1 : 0;
     }
 }
 
@@ -1124,9 +981,7 @@ cg_init_kernel(const typename Field<real>::svec *__restrict__ eta, typename Fiel
     if (grid_sum<VEC_NT>(local, partials, counter, &total)) {
         sc->rr = total; sc->eta2 = total; sc->qq = 0.0; sc->alpha = 0.0; sc->beta = 0.0;
         sc->r_min = r_min; sc->k = 0; sc->max_iter = max_iter;
-        const bool go = total > 0.0 && (sqrt(total) >= r_min * sqrt(total));
-        sc->k_stop = go ? max_iter : 0;
-        sc->converged = go ? 0 : 1;
+        loop_begin(sc, total, total, r_min, max_iter);
         if (hist) hist[0] = total;
     }
 }
@@ -1135,36 +990,16 @@ cg_init_kernel(const typename Field<real>::svec *__restrict__ eta, typename Fiel
 template <typename real>
 __global__ void __launch_bounds__(VEC_NT)
 cg_update_kernel(typename Field<real>::svec *y, typename Field<real>::svec *p,
-                 const typename Field<real>::svec *__restrict__ r, size_t n, const CgScalars *sc, int it, int rev)
+                 const typename Field<real>::svec *__restrict__ r, size_t n, const CgScalars *sc, int it)
 {
     using svec = typename Field<real>::svec;
-    pdl_trigger();
-    pdl_wait();
     if (it >= sc->k_stop) return;
     const real alpha = (real)sc->alpha, beta = (real)sc->beta;
-    for (size_t j = (size_t)blockIdx.x * VEC_NT + threadIdx.x; j < n; j += (size_t)gridDim.x * VEC_NT) {
-        const size_t i = rev ? n - 1 - j : j;   // rev: from the end of the buffers to their start (Geom.rev)
+    for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT) {
         const svec pv = p[i];
         const svec rv = __ldg(r + i);
         y[i] = vaxpy(alpha, pv, y[i]);
         p[i] = vaxpy(beta, pv, rv);
-    }
-}
-
-// a4 without its y half (the y update rode on the a3 pass, MODE_RUPDY): p <- r + beta p
-template <typename real>
-__global__ void __launch_bounds__(VEC_NT)
-cg_pupdate_kernel(typename Field<real>::svec *p, const typename Field<real>::svec *__restrict__ r, size_t n,
-                  const CgScalars *sc, int it, int rev)
-{
-    using svec = typename Field<real>::svec;
-    pdl_trigger();
-    pdl_wait();
-    if (it >= sc->k_stop) return;
-    const real beta = (real)sc->beta;
-    for (size_t j = (size_t)blockIdx.x * VEC_NT + threadIdx.x; j < n; j += (size_t)gridDim.x * VEC_NT) {
-        const size_t i = rev ? n - 1 - j : j;
-        p[i] = vaxpy(beta, p[i], __ldg(r + i));
     }
 }
 
@@ -1212,24 +1047,27 @@ bi_init_kernel(const typename Field<real>::svec *__restrict__ eta, typename Fiel
         sc->rr = total; sc->eta2 = total; sc->qq = 0.0; sc->alpha = 0.0; sc->beta = 0.0;
         sc->rho[0] = total; sc->rho[1] = 0.0;
         sc->calpha[0] = sc->calpha[1] = sc->omega[0] = sc->omega[1] = sc->cbeta[0] = sc->cbeta[1] = 0.0;
-        sc->r_min = r_min; sc->k = 0; sc->max_iter = max_iter; sc->breakdown = 0;
-        const bool go = total > 0.0 && (sqrt(total) >= r_min * sqrt(total));
-        sc->k_stop = go ? max_iter : 0;
-        sc->converged = go ? 0 : 1;
+        sc->r_min = r_min; sc->k = 0; sc->max_iter = max_iter;
+        loop_begin(sc, total, total, r_min, max_iter);
         if (hist) hist[0] = total;
     }
 }
 
+// The BiCGSTAB vector kernels never trust the pad lanes of their inputs (volume not a multiple of the 16-site block):
+// v and t are written by the stencil, which skips pad lanes, and the even-odd solvers run on half-length views of
+// work vectors that earlier full-lattice solves have filled; rhat = eta belongs to the caller.  Pad lanes of every
+// output are written as zero and contribute nothing to the dot products.
 // s <- r - alpha v
 template <typename real>
 __global__ void __launch_bounds__(VEC_NT)
 bi_s_kernel(typename Field<real>::svec *s, const typename Field<real>::svec *__restrict__ r,
-            const typename Field<real>::svec *__restrict__ v, size_t n, const CgScalars *sc, int it)
+            const typename Field<real>::svec *__restrict__ v, size_t n, int V, int padded, const CgScalars *sc, int it)
 {
+    using svec = typename Field<real>::svec;
     if (it >= sc->k_stop) return;
     const real ar = (real)(-sc->calpha[0]), ai = (real)(-sc->calpha[1]);
     for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT)
-        s[i] = vcaxpy(ar, ai, __ldg(v + i), __ldg(r + i));
+        s[i] = real_site<Field<real>::NSP>(i, V, padded) ? vcaxpy(ar, ai, __ldg(v + i), __ldg(r + i)) : vzero(svec());
 }
 
 // psi <- psi + alpha p + omega s ; r <- s - omega t ; rho' = <rhat,r> ; rr = <r,r> ; beta ; k ; loop test
@@ -1238,7 +1076,7 @@ __global__ void __launch_bounds__(VEC_NT)
 bi_xr_kernel(typename Field<real>::svec *psi, typename Field<real>::svec *r,
              const typename Field<real>::svec *__restrict__ p, const typename Field<real>::svec *__restrict__ s,
              const typename Field<real>::svec *__restrict__ t, const typename Field<real>::svec *__restrict__ rhat,
-             size_t n, CgScalars *sc, double *partials, unsigned int *counter, double *hist, int it)
+             size_t n, int V, int padded, CgScalars *sc, double *partials, unsigned int *counter, double *hist, int it)
 {
     using svec = typename Field<real>::svec;
     if (it >= sc->k_stop) return;
@@ -1246,6 +1084,11 @@ bi_xr_kernel(typename Field<real>::svec *psi, typename Field<real>::svec *r,
     const real wr = (real)sc->omega[0], wi = (real)sc->omega[1];
     double v3[3] = {0.0, 0.0, 0.0};
     for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT) {
+        if (!real_site<Field<real>::NSP>(i, V, padded)) {
+            psi[i] = vzero(svec());
+            r[i] = vzero(svec());
+            continue;
+        }
         const svec sv = __ldg(s + i);
         psi[i] = vcaxpy(wr, wi, sv, vcaxpy(ar, ai, __ldg(p + i), psi[i]));
         const svec rn = vcaxpy(-wr, -wi, __ldg(t + i), sv);
@@ -1261,13 +1104,15 @@ bi_xr_kernel(typename Field<real>::svec *psi, typename Field<real>::svec *r,
 template <typename real>
 __global__ void __launch_bounds__(VEC_NT)
 bi_p_kernel(typename Field<real>::svec *p, const typename Field<real>::svec *__restrict__ r,
-            const typename Field<real>::svec *__restrict__ v, size_t n, const CgScalars *sc, int it)
+            const typename Field<real>::svec *__restrict__ v, size_t n, int V, int padded, const CgScalars *sc, int it)
 {
+    using svec = typename Field<real>::svec;
     if (it >= sc->k_stop) return;
     const real br = (real)sc->cbeta[0], bi = (real)sc->cbeta[1];
     const real wr = (real)(-sc->omega[0]), wi = (real)(-sc->omega[1]);
     for (size_t i = (size_t)blockIdx.x * VEC_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * VEC_NT)
-        p[i] = vcaxpy(br, bi, vcaxpy(wr, wi, __ldg(v + i), p[i]), __ldg(r + i));
+        p[i] = real_site<Field<real>::NSP>(i, V, padded)
+                   ? vcaxpy(br, bi, vcaxpy(wr, wi, __ldg(v + i), p[i]), __ldg(r + i)) : vzero(svec());
 }
 
 // the paper's dot-product kernel on its own: <a,a>
@@ -1325,6 +1170,29 @@ unpack_spinor_kernel(const typename Field<real>::svec *__restrict__ nat, typenam
     const svec *p = nat + spinor_index<svec, NSP>(s);
 #pragma unroll
     for (int j = 0; j < NSP; ++j) can[(size_t)s * NSP + j] = __ldg(p + j * SB);
+}
+
+// ---------------------------------------------------------------- host helper shared by all launchers
+// Resident CTAs per SM of a kernel on the CURRENT device, cached per device in `table` (WD_MAXDEV ints, zero-initialised,
+// one table per kernel instantiation: declare it `static` next to the launch).  A process may drive several GPUs (one ctx
+// per device) and the persistent / cooperative grids are sized from this number, so one process-wide value is not enough.
+constexpr int WD_MAXDEV = 64;
+template <typename Kern>
+static cudaError_t cached_occupancy(int *table, Kern kern, int threads, size_t dyn_smem, int *out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= WD_MAXDEV) dev = WD_MAXDEV - 1;
+    int v = __atomic_load_n(&table[dev], __ATOMIC_RELAXED);
+    if (!v) {
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, kern, threads, dyn_smem);
+        if (e != cudaSuccess) return e;
+        if (v < 1) return cudaErrorLaunchOutOfResources;
+        __atomic_store_n(&table[dev], v, __ATOMIC_RELAXED);
+    }
+    *out = v;
+    return cudaSuccess;
 }
 
 }  // namespace wd

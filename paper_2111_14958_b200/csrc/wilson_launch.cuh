@@ -1,38 +1,27 @@
 // wilson_launch.cuh — the table of compiled stencil launch configurations and the per-precision launchers.
 // A "tile" (the name of the C ABI, wd_set_tile) is one row: CTA tile BX x BY x BZ x BT (threads per CTA =
-// product), MINB = minimum resident CTAs per SM asked of ptxas (bounds registers per thread), PIPE = 1 for
-// the software-pipelined hop loop with the diagonal term first (4 = the same with the diagonal term last, the
-// comparison rows 18 and 19; 2 = three register buffers, 3 = forward links staged through shared memory with
-// cp.async one tile ahead, 18-real links only).  This is the CUDA analogue of the paper's workgroup-size knob
-// (PAPER.md:58,76).  F64 = 1 if the row is also compiled for double precision.
+// product) and MINB = minimum resident CTAs per SM asked of ptxas (bounds registers per thread).  Every row runs the
+// software-pipelined hop loop (two register buffers, diagonal term first where the pass allows it).  This is the CUDA
+// analogue of the paper's workgroup-size knob.  F32 / F64 = 1 if the row is compiled for that precision.
+// Rows measured and retired in round 1 (unpipelined, three buffers, cp.async-staged forward links, 64-thread and 4-site-run
+// tiles that never won: DESIGN.md section 6) are no longer compiled.
 #pragma once
 #include "wilson_kernels.cuh"
 
 // Rows are in order of preference (measured on B200, profiles/): the automatic choice takes the first row
 // with the fewest padded threads for the lattice and precision at hand.
-//   X(index, BX, BY, BZ, BT, MINB, PIPE, F64)
+//   X(index, BX, BY, BZ, BT, MINB, F32, F64)
 #define WD_TILE_TABLE(X) \
     X(0, 16, 2, 2, 2, 4, 1, 0) \
     X(1, 16, 4, 4, 2, 1, 1, 0) \
     X(2, 32, 2, 2, 1, 4, 1, 0) \
-    X(3, 16, 2, 4, 2, 2, 1, 0) \
-    X(4, 16, 4, 2, 2, 2, 1, 0) \
-    X(5, 32, 2, 4, 2, 1, 1, 0) \
-    X(6, 8, 4, 2, 2, 4, 1, 0) \
-    X(7, 32, 2, 2, 1, 2, 1, 1) \
-    X(8, 16, 2, 2, 1, 3, 1, 1) \
-    X(9, 16, 2, 2, 2, 2, 1, 1) \
-    X(10, 8, 4, 2, 1, 4, 1, 1) \
-    X(11, 8, 2, 2, 2, 4, 1, 1) \
-    X(12, 4, 4, 2, 2, 4, 1, 1) \
-    X(13, 4, 4, 4, 2, 2, 1, 1) \
-    X(14, 16, 2, 2, 2, 0, 0, 1) \
-    X(15, 8, 4, 4, 2, 0, 0, 1) \
-    X(16, 16, 2, 2, 2, 3, 2, 0) \
-    X(17, 16, 2, 2, 2, 4, 3, 0) \
-    X(18, 16, 2, 2, 2, 4, 4, 0) \
-    X(19, 32, 2, 2, 1, 2, 4, 1)
-#define WD_NUM_TILES 20
+    X(3, 8, 4, 2, 2, 4, 1, 0) \
+    X(4, 32, 2, 2, 1, 2, 0, 1) \
+    X(5, 16, 2, 2, 1, 3, 0, 1) \
+    X(6, 16, 2, 2, 2, 2, 0, 1) \
+    X(7, 8, 4, 2, 1, 4, 0, 1) \
+    X(8, 4, 4, 2, 2, 4, 1, 1)
+#define WD_NUM_TILES 9
 
 // Launch configurations of the one-launch CG kernel (small volumes): 64- and 128-thread tiles,
 // no register bound (ptxas then hoists the loads of all 8 hops: one memory round trip per site instead of 8,
@@ -56,10 +45,10 @@ namespace wd {
 
 struct TileInfo {
     int b[4];
-    int minb, pipe, f64;
+    int minb, f32, f64;
 };
 static const TileInfo kTiles[WD_NUM_TILES] = {
-#define X(i, a, b, c, d, m, p, f) {{a, b, c, d}, m, p, f},
+#define X(i, a, b, c, d, m, f32, f64) {{a, b, c, d}, m, f32, f64},
     WD_TILE_TABLE(X)
 #undef X
 };
@@ -100,8 +89,6 @@ cudaError_t launch_cg_onelaunch_f64(int small_tile, const CgOneLaunchArgs &a);
 struct DslashArgs {
     Geom g;
     int sm_count;
-    int waves;      // resident waves of CTAs to launch (persistent grid = waves * SMs * CTAs per SM), >= 1
-    int prefetch;   // L2 prefetch distance in tiles: -1 = one grid ahead, 0 = off
     cudaStream_t stream;
     const void *U;
     const void *Ub;   // links read by the backward hops: U itself on a plain lattice, the other parity's with even-odd
@@ -115,15 +102,11 @@ struct DslashArgs {
     unsigned int *counter;
     double *hist;
     int it;
-    int pdl = 0;      // 1: launch with programmatic stream serialization (wd_set_pdl; the kernel starts with pdl_wait())
 };
 
 // dagger in {0,1}; mode in {MODE_PLAIN, MODE_QQ (dagger = 1 only), MODE_RUPD (dagger = 0 only)}
 cudaError_t launch_dslash_f32(int tile, int dagger, int mode, const DslashArgs &a);
 cudaError_t launch_dslash_f64(int tile, int dagger, int mode, const DslashArgs &a);
-// a3 with the y half of a4 fused in (MODE_RUPDY: a.out = y, a.cen = p); 18-real links, plain lattice
-cudaError_t launch_dslash_y_f32(int tile, const DslashArgs &a);
-cudaError_t launch_dslash_y_f64(int tile, const DslashArgs &a);
 // the same with 12-real link storage (wd_set_gauge_recon(ctx, 12))
 cudaError_t launch_dslash12_f32(int tile, int dagger, int mode, const DslashArgs &a);
 cudaError_t launch_dslash12_f64(int tile, int dagger, int mode, const DslashArgs &a);
@@ -146,40 +129,19 @@ static cudaError_t launch_dslash_tile(int tile, const DslashArgs &a)
     using svec = typename Field<real>::svec;
     using gvec = typename Field<real>::gvec;
     switch (tile) {
-#define X(i, bx, by, bz, bt, m, p, f)                                                                          \
+#define X(i, bx, by, bz, bt, m, f32, f64)                                                                      \
     case i:                                                                                                    \
-        if constexpr ((sizeof(real) == 4 || f) && !(p == 3 && RECON != 18)) {                                  \
-            static int occ = 0;                                                                                \
-            const size_t dyn = (p == 3) ? (size_t)(bx * by * bz * bt) * staged_link_bytes<real>() : 0;         \
-            if (!occ) {                                                                                        \
-                auto kern = dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON, EO>;                       \
-                if (dyn > 48 * 1024) {                                                                         \
-                    cudaError_t e2 = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); \
-                    if (e2 != cudaSuccess) return e2;                                                          \
-                }                                                                                              \
-                cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, bx * by * bz * bt, dyn); \
-                if (e != cudaSuccess) return e;                                                                \
-                if (occ < 1) occ = 1;                                                                          \
-            }                                                                                                  \
-            long grid = (long)occ * a.sm_count * a.waves;                                                      \
+        if constexpr (sizeof(real) == 4 ? f32 : f64) {                                                         \
+            auto kern = dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, RECON, EO>;                          \
+            static int occ_tab[WD_MAXDEV];                                                                     \
+            int occ = 0;                                                                                       \
+            cudaError_t e = cached_occupancy(occ_tab, kern, bx * by * bz * bt, 0, &occ);                       \
+            if (e != cudaSuccess) return e;                                                                    \
+            long grid = (long)occ * a.sm_count;                                                                \
             if (grid > a.g.ntiles) grid = a.g.ntiles;                                                          \
-            Geom g = a.g;                                                                                      \
-            g.pf = a.prefetch < 0 ? (int)grid : a.prefetch;                                                    \
-            if (a.pdl) {                                                                                       \
-                cudaLaunchConfig_t lc = {};                                                                    \
-                lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3(bx * by * bz * bt);                      \
-                lc.dynamicSmemBytes = dyn; lc.stream = a.stream;                                               \
-                cudaLaunchAttribute at[1];                                                                     \
-                at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                                 \
-                at[0].val.programmaticStreamSerializationAllowed = 1;                                          \
-                lc.attrs = at; lc.numAttrs = 1;                                                                \
-                return cudaLaunchKernelEx(&lc, dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON, EO>, g, \
-                    (const gvec *)a.U, (const gvec *)a.Ub, (const svec *)a.in, (const svec *)a.cen, (svec *)a.out, (real)a.kappa, \
-                    (svec *)a.r, a.sc, a.partials, a.counter, a.hist, a.it);                                   \
-            }                                                                                                  \
-            dslash_kernel<real, DAG, MODE, bx, by, bz, bt, m, p, RECON, EO><<<(unsigned)grid, bx * by * bz * bt, dyn, a.stream>>>(  \
-                g, (const gvec *)a.U, (const gvec *)a.Ub, (const svec *)a.in, (const svec *)a.cen, (svec *)a.out, (real)a.kappa, (svec *)a.r, a.sc,   \
-                a.partials, a.counter, a.hist, a.it);                                                          \
+            kern<<<(unsigned)grid, bx * by * bz * bt, 0, a.stream>>>(                                          \
+                a.g, (const gvec *)a.U, (const gvec *)a.Ub, (const svec *)a.in, (const svec *)a.cen, (svec *)a.out, \
+                (real)a.kappa, (svec *)a.r, a.sc, a.partials, a.counter, a.hist, a.it);                        \
             return cudaGetLastError();                                                                         \
         }                                                                                                      \
         return cudaErrorInvalidValue;
@@ -198,11 +160,11 @@ static cudaError_t launch_cg_onelaunch_any(int small_tile, const CgOneLaunchArgs
 #define Y(i, bx, by, bz, bt, mb_, pi_)                                                                           \
     case i: {                                                                                                  \
         auto kern = cg_onelaunch_kernel<real, bx, by, bz, bt, mb_, pi_>;                                      \
-        static int occ = 0;                                                                                    \
-        if (!occ) {                                                                                            \
-            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, bx * by * bz * bt, 0);   \
+        static int occ_tab[WD_MAXDEV];                                                                         \
+        int occ = 0;                                                                                           \
+        {                                                                                                      \
+            cudaError_t e = cached_occupancy(occ_tab, kern, bx * by * bz * bt, 0, &occ);                       \
             if (e != cudaSuccess) return e;                                                                    \
-            if (occ < 1) return cudaErrorLaunchOutOfResources;                                                 \
         }                                                                                                      \
         long grid = (long)occ * a.sm_count;            /* all CTAs must be co-resident (grid barrier) */       \
         if (grid > a.g.ntiles) grid = a.g.ntiles;                                                              \

@@ -67,12 +67,12 @@ int ensure_multi(wd_ctx *c, int max_iter)
         CUDA_TRY(c, cudaMalloc(&c->m_counter, 4 * sizeof(unsigned int)));
         CUDA_TRY(c, cudaMemsetAsync(c->m_counter, 0, 4 * sizeof(unsigned int), c->stream));
     }
-    if (c->m_hist_cap < max_iter + 1) {
+    if (c->m_hist_cap < hist_len(max_iter)) {
         if (c->m_hist) cudaFree(c->m_hist);
         c->m_hist = nullptr;
         c->m_hist_cap = 0;
-        CUDA_TRY(c, cudaMalloc(&c->m_hist, 4 * sizeof(double) * (size_t)(max_iter + 1)));
-        c->m_hist_cap = max_iter + 1;
+        CUDA_TRY(c, cudaMalloc(&c->m_hist, 4 * sizeof(double) * (size_t)hist_len(max_iter)));
+        c->m_hist_cap = hist_len(max_iter);
     }
     return WD_OK;
 }
@@ -103,7 +103,7 @@ int cg_group(wd_ctx *c, int g, const void *U, const void *eta, void *psi, double
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[0], c->stream));
             CUDA_TRY(c, mrhs_launch(c, g, 1, MODE_QQ, U, p, q, nullptr, kappa, c->m_sc, c->m_hist, hs, it));
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[1], c->stream));
-            CUDA_TRY(c, mrhs_launch(c, g, 0, MODE_RUPD, U, q, nullptr, r, kappa, c->m_sc, c->m_hist, hs, it));
+            CUDA_TRY(c, mrhs_launch(c, g, 0, MODE_RUPD, U, q, nullptr, r, kappa, c->m_sc, (long)it + 1 < (long)hs ? c->m_hist : nullptr, hs, it));
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[2], c->stream));
             cg_update_mrhs_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(y, p, r, n, stride, c->m_sc, it);
             c->launches++;
@@ -135,7 +135,7 @@ int cg_group(wd_ctx *c, int g, const void *U, const void *eta, void *psi, double
     int status = WD_OK;
     for (int j = 0; j < g; ++j) {
         const CgScalars &s = c->m_sc_host[j];
-        if (!s.converged) status = WD_NOT_CONVERGED;
+        if (!s.converged && status != WD_BREAKDOWN) status = s.breakdown ? WD_BREAKDOWN : WD_NOT_CONVERGED;
         if (infos) {
             infos[j].iterations = s.k;
             infos[j].converged = s.converged;

@@ -51,9 +51,9 @@ dslash_mrhs_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ 
         if (!live || x >= g.L[0] || y >= g.L[1] || z >= g.L[2] || t >= g.L[3]) continue;
         const int s = x + g.L[0] * (y + g.L[1] * (z + g.L[2] * t));
         real acc[24], c[24], rv[24];
-        constexpr bool CF = MODE != MODE_RUPD;   // diagonal term first, as in dslash_kernel PIPE = 1
-        hopping_sum<DAG, 1, MODE == MODE_RUPD, true, real, svec, gvec, 18, 0, 0, CF>(g, U, U, in, in, r, x, y, z, t, s,
-                                                                                  acc, c, rv, nullptr, -1, kappa);
+        constexpr bool CF = MODE != MODE_RUPD;   // diagonal term first, as in dslash_kernel
+        hopping_sum<DAG, 1, MODE == MODE_RUPD, true, real, svec, gvec, 18, 0, CF>(g, U, U, in, in, r, x, y, z, t, s,
+                                                                               acc, c, rv, kappa);
 #pragma unroll
         for (int i = 0; i < 24; ++i) c[i] = CF ? acc[i] : fma(-kappa, acc[i], c[i]);
         if (MODE == MODE_RUPD) {
@@ -114,10 +114,8 @@ cg_init_mrhs_kernel(const typename Field<real>::svec *__restrict__ eta, typename
     double total;
     if (grid_sum<VEC_NT>(local, partials + (size_t)blockIdx.y * gridDim.x, counter + blockIdx.y, &total)) {
         sc->rr = total; sc->eta2 = total; sc->qq = 0.0; sc->alpha = 0.0; sc->beta = 0.0;
-        sc->r_min = r_min; sc->k = 0; sc->max_iter = max_iter; sc->breakdown = 0;
-        const bool go = total > 0.0 && (sqrt(total) >= r_min * sqrt(total));
-        sc->k_stop = go ? max_iter : 0;
-        sc->converged = go ? 0 : 1;
+        sc->r_min = r_min; sc->k = 0; sc->max_iter = max_iter;
+        loop_begin(sc, total, total, r_min, max_iter);
         if (hist) hist[(size_t)blockIdx.y * hist_stride] = total;
     }
 }
@@ -187,12 +185,12 @@ static cudaError_t launch_mrhs_tile(int tile, const MrhsArgs &a)
         constexpr int minb = per_sm / nt > 0 ? per_sm / nt : 1;                                                    \
         if constexpr (nt <= per_sm) {                                                                              \
             auto kern = dslash_mrhs_kernel<real, DAG, MODE, bx, by, bz, bt, NRHS, minb>;                           \
-            static int occ = 0;                                                                                    \
-            if (!occ) {                                                                                            \
-                cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, nt, 0);                  \
-                if (e != cudaSuccess) return e;                                                                    \
-                if (occ < 1) occ = 1;                                                                              \
-            }                                                                                                      \
+            static int occ_tab[WD_MAXDEV];                                                                     \
+            int occ = 0;                                                                                       \
+            {                                                                                                  \
+                cudaError_t e = cached_occupancy(occ_tab, kern, nt, 0, &occ);                                  \
+                if (e != cudaSuccess) return e;                                                                \
+            }                                                                                                  \
             long grid = (long)occ * a.sm_count;                                                                    \
             if (grid > a.g.ntiles) grid = a.g.ntiles;                                                              \
             kern<<<(unsigned)grid, nt, 0, a.stream>>>(a.g, (const gvec *)a.U, (const svec *)a.in, (svec *)a.out,   \

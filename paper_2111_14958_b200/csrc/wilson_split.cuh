@@ -146,7 +146,7 @@ cg_split_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     const double eta2 = all_cta_sum<NT>(part0, G, sm);
     double rr = eta2, alpha = 0.0, beta = 0.0;
     int k = 0;
-    bool go = eta2 > 0.0 && (sqrt(rr) >= r_min * sqrt(eta2));
+    bool go = isfinite(eta2) && eta2 > 0.0 && loop_test(rr, eta2, r_min).go;
     if (blockIdx.x == 0 && tid == 0 && hist) hist[0] = eta2;
 
     while (go && k < max_iter) {
@@ -246,7 +246,8 @@ cg_split_kernel(const Geom g, const typename Field<real>::gvec *__restrict__ U,
     if (blockIdx.x == 0 && tid == 0) {
         sc->rr = rr; sc->eta2 = eta2; sc->alpha = alpha; sc->beta = beta; sc->qq = 0.0; sc->r_min = r_min;
         sc->k = k; sc->k_stop = k; sc->max_iter = max_iter;
-        sc->converged = go ? 0 : 1;
+        sc->converged = (eta2 == 0.0 || loop_test(rr, eta2, r_min).converged) ? 1 : 0;
+        sc->breakdown = (!go && !sc->converged) ? 1 : 0;
     }
 }
 
@@ -259,11 +260,11 @@ static cudaError_t launch_cg_split_any(int split_tile, const CgOneLaunchArgs &a)
 #define Z(i, bx, by, bz, bt)                                                                                   \
     case i: {                                                                                                  \
         auto kern = cg_split_kernel<real, bx, by, bz, bt>;                                                     \
-        static int occ = 0;                                                                                    \
-        if (!occ) {                                                                                            \
-            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, 128, 0);                 \
+        static int occ_tab[WD_MAXDEV];                                                                         \
+        int occ = 0;                                                                                           \
+        {                                                                                                      \
+            cudaError_t e = cached_occupancy(occ_tab, kern, 128, 0, &occ);                                     \
             if (e != cudaSuccess) return e;                                                                    \
-            if (occ < 1) return cudaErrorLaunchOutOfResources;                                                 \
         }                                                                                                      \
         long grid = (long)occ * a.sm_count;            /* all CTAs must be co-resident (grid barrier) */       \
         if (grid > a.g.ntiles) grid = a.g.ntiles;                                                              \

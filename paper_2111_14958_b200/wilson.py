@@ -108,14 +108,9 @@ def load_library(path: str = LIB_PATH):
     lib.wd_set_tile.argtypes = [vp, ci]
     lib.wd_get_tile.argtypes = [vp]
     lib.wd_set_cg_mode.argtypes = [vp, ci]
-    lib.wd_set_prefetch.argtypes = [vp, ci]
     lib.wd_set_gauge_recon.argtypes = [vp, ci]
     lib.wd_get_gauge_recon.argtypes = [vp]
-    lib.wd_set_waves.argtypes = [vp, ci]
     lib.wd_set_zchunk.argtypes = [vp, ci]
-    lib.wd_set_sweep.argtypes = [vp, ci]
-    lib.wd_set_fuse_y.argtypes = [vp, ci]
-    lib.wd_set_pdl.argtypes = [vp, ci]
     lib.wd_set_small_tile.argtypes = [vp, ci]
     lib.wd_set_poll_interval.argtypes = [vp, ci]
     lib.wd_set_profile.argtypes = [vp, ci]
@@ -139,7 +134,7 @@ def tile_shapes():
 
 
 def tile_infos():
-    """[(BX,BY,BZ,BT, min_blocks_per_sm, pipelined, has_fp64), ...] for every compiled launch configuration."""
+    """[(BX,BY,BZ,BT, min_blocks_per_sm, has_fp32, has_fp64), ...] for every compiled launch configuration."""
     lib = load_library()
     out = []
     for i, shp in enumerate(tile_shapes()):
@@ -474,29 +469,11 @@ class WilsonContext:
     def wd_get_gauge_recon(self):
         return int(self.lib.wd_get_gauge_recon(self._ctx))
 
-    def wd_set_prefetch(self, tiles):
-        self._check(self.lib.wd_set_prefetch(self._ctx, int(tiles)))
-
-    def wd_set_waves(self, waves):
-        self._check(self.lib.wd_set_waves(self._ctx, int(waves)))
-
     def wd_set_zchunk(self, layers):
         self._check(self.lib.wd_set_zchunk(self._ctx, int(layers)))
 
     def wd_set_small_tile(self, index):
         self._check(self.lib.wd_set_small_tile(self._ctx, int(index)))
-
-    def wd_set_sweep(self, alternate):
-        """1: consecutive passes walk the lattice in alternating directions (L2 reuse); 0 (default): all forward"""
-        self._check(self.lib.wd_set_sweep(self._ctx, int(alternate)))
-
-    def wd_set_fuse_y(self, on):
-        """1: y += alpha p rides on the a3 stencil pass, a4 is p = r + beta p alone (bit-identical iterates)"""
-        self._check(self.lib.wd_set_fuse_y(self._ctx, int(on)))
-
-    def wd_set_pdl(self, on):
-        """1: programmatic dependent launch of the kernels of the three-kernel CG loop (same results)"""
-        self._check(self.lib.wd_set_pdl(self._ctx, int(on)))
 
     def wd_set_poll_interval(self, n):
         self._check(self.lib.wd_set_poll_interval(self._ctx, int(n)))

@@ -4,6 +4,8 @@ pattern with a payload: a kernel that WRITES outside its buffer changes the patt
 into its result.  Lattices are ragged on purpose: volume (and half volume) not a multiple of the 16-site block, extents
 not multiples of the tile.  The volume-dependent pad lanes INSIDE the buffers are poisoned too where the call's contract
 says they are ignored (inputs of wd_apply / cg_solve / the even-odd calls come from the pack kernels, which zero them)."""
+import math
+
 import numpy as np
 import pytest
 
@@ -169,3 +171,130 @@ def test_even_odd_calls_stay_inside_their_buffers(wilson, dims, precision):
         torch.cuda.synchronize()
         assert all_intact(Uc, ec, Ue, ee, pe, tmp, can, U12)
         assert torch.equal(ec.t, torch.view_as_real(gu.to_device(eta)).reshape(-1))
+
+
+# ---------------------------------------------------------------- non-finite inputs, stale pad lanes, max_iter = INT_MAX
+@pytest.mark.parametrize("precision", [32, 64])
+def test_non_finite_inputs_are_a_breakdown_not_a_convergence(wilson, precision):
+    """A NaN link or a NaN / infinite source makes the residual norm NaN; `!(x >= thr)` then ends the loop, and the
+    solvers must report WD_BREAKDOWN (status 2, converged 0), never WD_OK with a NaN field (include/wilson_cg.h)."""
+    cfg = inputs.CONFIGS[0]
+    U, eta = gu.config_fields(0, precision)
+    U_bad = U.copy()
+    U_bad[17, 2, 1, 1] = np.nan
+    eta_nan = eta.copy()
+    eta_nan[5, 1, 2] = np.nan
+    eta_inf = eta.copy()
+    eta_inf[9, 0, 0] = np.inf
+    r_min = 1e-6 if precision == 32 else 1e-10
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
+        for mode in (1, 2, 6):
+            ctx.wd_set_cg_mode(mode)
+            for Ux, ex in ((U_bad, eta), (U, eta_nan), (U, eta_inf)):
+                _, info = gu.solve_on_gpu(ctx, Ux, ex, cfg.kappa, r_min, 200)
+                assert info["status"] == 2 and info["converged"] == 0 and info["iterations"] <= 2, (mode, info)
+            # and the ctx is not poisoned: the clean problem still converges
+            _, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, r_min, 200)
+            assert info["status"] == 0 and info["converged"] == 1
+        ctx.wd_set_cg_mode(1)
+        Un, Ub = ctx.wd_pack_gauge(gu.to_device(U)), ctx.wd_pack_gauge(gu.to_device(U_bad))
+        en, eb = ctx.wd_pack_spinor(gu.to_device(eta)), ctx.wd_pack_spinor(gu.to_device(eta_nan))
+        for Ux, ex in ((Ub, en), (Un, eb)):
+            _, info = ctx.bicgstab_solve(Ux, ex, cfg.kappa, r_min, 200)
+            assert info["status"] == 2 and info["converged"] == 0, info
+        for mode in (1, 2):     # seven / five kernels per iteration, and the one-launch even-odd BiCGSTAB
+            ctx.wd_set_cg_mode(mode)
+            for Ux, ex in ((U_bad, eta), (U, eta_nan)):
+                Ue = ctx.wd_eo_pack_gauge(gu.to_device(Ux))
+                ee = ctx.wd_eo_pack_spinor(gu.to_device(ex))
+                _, info = ctx.bicgstab_solve_eo(Ue, ee, cfg.kappa, r_min, 200)
+                assert info["status"] == 2 and info["converged"] == 0, (mode, info)
+                if mode == 1:
+                    _, info = ctx.cg_solve_eo(Ue, ee, cfg.kappa, r_min, 200)
+                    assert info["status"] == 2 and info["converged"] == 0, info
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("dims", [(14, 14, 14, 14), (6, 6, 6, 10)])
+def test_even_odd_solvers_ignore_stale_pad_lanes(wilson, oracle, dims, precision):
+    """V/2 is not a multiple of the 16-site block here.  The even-odd solvers run on half-length views of the ctx work
+    vectors; a full-lattice solve that stopped after one iteration leaves O(1) data where those views have their pad
+    lanes.  It must not leak into the recurrence: iteration counts and residuals equal the oracle's as on a fresh ctx."""
+    assert (int(np.prod(dims)) // 2) % 16 != 0
+    cdt = gu.np_complex(precision)
+    kappa, r_min = 0.12, (1e-6 if precision == 32 else 1e-10)
+    U = inputs.gauge_field(777, dims, "haar", dtype=cdt)
+    eta = inputs.source_field(777, dims, dtype=cdt)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    _, ioc = oracle.cg_solve_eo(dims, U64, eta64, kappa, r_min, 500, -1)
+    _, iob = oracle.bicgstab_solve_eo(dims, U64, eta64, kappa, r_min, 500, -1)
+    with wilson.WilsonContext(dims, precision, -1) as ctx:
+        ctx.wd_set_cg_mode(1)                       # kernel-per-phase drivers (the one-launch kernels own their vectors)
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        en = ctx.wd_pack_spinor(gu.to_device(eta))
+        # poison: every work vector holds O(1) data at all lanes the stencil and the vector kernels ever wrote
+        ctx.cg_solve(Un, en, kappa, r_min, 1)
+        ctx.bicgstab_solve(Un, en, kappa, r_min, 1)
+        Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
+        ee = ctx.wd_eo_pack_spinor(gu.to_device(eta))
+        pb, ib = ctx.bicgstab_solve_eo(Ue, ee, kappa, r_min, 500)
+        psi_b = gu.to_host(ctx.wd_eo_unpack_spinor(pb))
+        pc, ic = ctx.cg_solve_eo(Ue, ee, kappa, r_min, 500)
+        psi_c = gu.to_host(ctx.wd_eo_unpack_spinor(pc))
+    slack = 0 if precision == 64 else max(1, int(0.05 * iob["iterations"] + 0.5))
+    assert ib["status"] == 0 and abs(ib["iterations"] - iob["iterations"]) <= slack, (ib, iob)
+    assert ic["status"] == 0 and abs(ic["iterations"] - ioc["iterations"]) <= math.floor(0.02 * ioc["iterations"] + 0.5)
+    for name, psi in (("bicgstab_eo", psi_b), ("cg_eo", psi_c)):
+        res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), kappa, -1)
+        assert res < 2.0 * r_min, (name, res)
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_bicgstab_ignores_the_pad_lanes_of_its_source(wilson, oracle, precision):
+    """5 x 7 x 4 x 6 = 840 sites = 52.5 blocks.  The source is the output of wd_apply into a buffer full of NaN: its
+    real sites hold D eta, its 8 pad lanes stay NaN (the stencil never writes them).  rhat = that source enters two dot
+    products per iteration: they must skip the pad lanes."""
+    import torch
+
+    dims, kappa = (5, 7, 4, 6), 0.12
+    cdt = gu.np_complex(precision)
+    r_min = 1e-6 if precision == 32 else 1e-10
+    U = inputs.gauge_field(778, dims, "haar", dtype=cdt)
+    eta = inputs.source_field(778, dims, dtype=cdt)
+    with wilson.WilsonContext(dims, precision, 1) as ctx:
+        ctx.wd_set_cg_mode(1)
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        en = ctx.wd_pack_spinor(gu.to_device(eta))
+        src = torch.full_like(en, float("nan"))
+        ctx.wd_apply(Un, en, kappa, False, out=src)
+        assert bool(torch.isnan(src).any())                      # the pad lanes
+        src_can = gu.to_host(ctx.wd_unpack_spinor(src))
+        assert np.isfinite(src_can).all()
+        for solve in (ctx.bicgstab_solve, ctx.cg_solve):
+            psi_n, info = solve(Un, src, kappa, r_min, 500)
+            psi = gu.to_host(ctx.wd_unpack_spinor(psi_n))
+            assert info["status"] == 0 and np.isfinite(psi).all(), info
+            # D psi = D eta  =>  psi = eta
+            assert np.linalg.norm(psi - eta) / np.linalg.norm(eta) < 4.0 * r_min * (1 + 8 * kappa) / (1 - 8 * kappa)
+    U64, s64 = U.astype(np.complex128), src_can.astype(np.complex128)
+    _, io = oracle.bicgstab_solve(dims, U64, s64, kappa, r_min, 500, 1)
+    assert abs(info["iterations"] - oracle.cg_solve(dims, U64, s64, kappa, r_min, 500, 1)[1]["iterations"]) <= 1
+    assert io["converged"]
+
+
+def test_max_iter_int_max_means_no_limit(wilson):
+    """max_iter = INT_MAX: max_iter + 1 must not overflow, the history stays bounded, the solve converges as usual"""
+    cfg = inputs.CONFIGS[0]
+    U, eta = gu.config_fields(0, 32)
+    with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+        ref = None
+        for mode in (1, 2, 6):
+            ctx.wd_set_cg_mode(mode)
+            psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, 2 ** 31 - 1)
+            assert info["status"] == 0 and info["converged"] == 1 and 20 < info["iterations"] < 40
+            ref = ref or info["iterations"]
+            assert info["iterations"] == ref
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        en = ctx.wd_pack_spinor(gu.to_device(eta))
+        _, ib = ctx.bicgstab_solve(Un, en, cfg.kappa, cfg.r_min, 2 ** 31 - 1)
+        assert ib["status"] == 0
