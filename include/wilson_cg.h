@@ -327,6 +327,16 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *                             keeps the +-t neighbours of a tile in L2; 0 = automatic (fits a 40 MB reuse distance).
  *   wd_set_small_tile(ctx, i)     launch configuration (CTA tile, register bound) of the one-launch CG kernel of mode 2:
  *                             -1 = automatic (default), 0 <= i < number of compiled configurations.
+ *   wd_set_link_staging(ctx, row) the stencil passes of wd_apply and of the three-kernel cg_solve fetch the gauge field through the
+ *                             shared-memory link pipeline of csrc/wilson_tma.cuh (bulk copies global -> shared of the contiguous
+ *                             16-site link blocks, mbarrier ring, both uses of every link served from shared memory; BASELINE.json
+ *                             north_star (2)); row selects a compiled configuration {16,BY,BZ,BT, stages, copies ahead, min CTAs/SM},
+ *                             -1 = off: links through L1 with the register pipeline, -2 = automatic (default): the row that measured
+ *                             faster, which today means the D-dagger / plain passes in fp64 (a2 9 % faster at 32^4) and nothing in
+ *                             fp32 (profiles/r2_ncu_link_staging.md).  Results are bit-identical either way.  A row covers
+ *                             a lattice only if Lx % 16 == 0 and Ly, Lz, Lt are multiples of BY, BZ, BT, 18 reals per link; otherwise
+ *                             WD_ERR_ARG.  wd_get_link_staging(ctx) = row the D-dagger passes run on (-1 = none).  wd_num_staging_rows() / wd_staging_row_info(row, info[9]) list the rows
+ *                             (info = {16, BY, BZ, BT, stages, ahead, min CTAs per SM, compiled for fp32, for fp64}).
  *   wd_set_poll_interval(ctx, n)  CG iterations enqueued between two host polls of the device stop flag (n >= 1; 0 = automatic).
  */
 int wd_num_tiles(void);
@@ -337,6 +347,10 @@ int wd_get_tile(wd_ctx *ctx);
 int wd_set_cg_mode(wd_ctx *ctx, int mode);
 int wd_set_zchunk(wd_ctx *ctx, int layers);
 int wd_set_small_tile(wd_ctx *ctx, int index);
+int wd_num_staging_rows(void);
+int wd_staging_row_info(int row, int info[9]);
+int wd_set_link_staging(wd_ctx *ctx, int row);
+int wd_get_link_staging(wd_ctx *ctx);
 int wd_set_poll_interval(wd_ctx *ctx, int n);
 
 /*

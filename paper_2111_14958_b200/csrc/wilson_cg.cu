@@ -46,6 +46,18 @@ extern "C" long wd_selftest_fastdiv(unsigned int d, unsigned int n_max)
 template <int DAG, int MODE>
 static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void *out, double kappa, void *r, int it)
 {
+    const int srow = stage_row_for(c, MODE);
+    if (srow >= 0) {   // links through the shared-memory pipeline (wilson_tma.cuh)
+        TmaArgs t;
+        t.g = make_geom_dims(c, kTmaRows[srow].b, c->zchunk_user);
+        t.sm_count = c->sm_count;
+        t.stream = c->stream;
+        t.U = U; t.in = in; t.out = out; t.r = r; t.kappa = kappa;
+        t.sc = MODE == MODE_PLAIN ? nullptr : c->sc;
+        t.partials = c->partials; t.counter = c->counter; t.hist = hist_at(c, it); t.it = it;
+        c->launches++;
+        return c->precision == 32 ? launch_dslash_tma_f32(srow, DAG, MODE, t) : launch_dslash_tma_f64(srow, DAG, MODE, t);
+    }
     DslashArgs a;
     a.g = make_geom(c, c->tile);
     a.sm_count = c->sm_count;
@@ -141,6 +153,7 @@ extern "C" int wd_create(wd_ctx **out, const int dims[4], int precision, int bc_
     c->tile = auto_tile(c);
     c->l2_budget_mb = 40.0;
     c->small_tile_user = -1;
+    c->stage_row = -2;
     bool ok = true;
     ok = ok && cudaMalloc(&c->sc, sizeof(CgScalars)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->counter, sizeof(unsigned int)) == cudaSuccess;
@@ -252,6 +265,25 @@ extern "C" int wd_set_small_tile(wd_ctx *c, int index)
     c->small_tile_user = index;
     return WD_OK;
 }
+extern "C" int wd_num_staging_rows(void) { return WD_NUM_TMA_ROWS; }
+extern "C" int wd_staging_row_info(int row, int info[9])
+{
+    if (row < 0 || row >= WD_NUM_TMA_ROWS || !info) return WD_ERR_ARG;
+    const TmaRowInfo &t = kTmaRows[row];
+    for (int d = 0; d < 4; ++d) info[d] = t.b[d];
+    info[4] = t.nstage; info[5] = t.ahead; info[6] = t.minb; info[7] = t.f32; info[8] = t.f64;
+    return WD_OK;
+}
+extern "C" int wd_set_link_staging(wd_ctx *c, int row)
+{
+    if (!c) return WD_ERR_ARG;
+    if (row == -1 || row == -2) { c->stage_row = row; return WD_OK; }
+    if (!stage_row_ok(c, row))
+        return fail(c, WD_ERR_ARG, "wd_set_link_staging: row %d does not cover this lattice / precision / link storage", row);
+    c->stage_row = row;
+    return WD_OK;
+}
+extern "C" int wd_get_link_staging(wd_ctx *c) { return c ? stage_row_for(c, MODE_QQ) : WD_ERR_ARG; }
 extern "C" int wd_set_poll_interval(wd_ctx *c, int n)
 {
     if (!c || n < 0) return WD_ERR_ARG;

@@ -3,6 +3,7 @@
 #pragma once
 #include "../../include/wilson_cg.h"
 #include "wilson_launch.cuh"
+#include "wilson_tma.cuh"
 
 #include <cstdarg>
 #include <cstdio>
@@ -22,6 +23,8 @@ struct wd_ctx {
     int last_cg_mode;     // what the last cg_solve used
     int zchunk_user;      // z layers per rasterisation chunk, 0 = automatic
     int small_tile_user;  // launch configuration of the one-launch CG kernel: -1 = automatic
+    int stage_row;        // row of the shared-memory link pipeline (wilson_tma.cuh) used by wd_apply / cg_solve: -1 = off,
+                          // -2 = automatic (fp64: the D-dagger / plain passes, where it measured 9 % faster; fp32: off)
     double l2_budget_mb;  // reuse-distance budget of the automatic choice
     int sm_count;
     // CG workspace (native layout), device
@@ -239,3 +242,23 @@ static inline int auto_tile_dims(const wd_ctx *c, const int dims[4])
     return best;
 }
 static inline int auto_tile(const wd_ctx *c) { return auto_tile_dims(c, c->dims); }
+
+// The staged stencil (wilson_tma.cuh) covers: plain lattice, 18 reals per link, the row compiled for the precision, Lx a
+// multiple of the 16-site block and every other extent a multiple of the row's tile edge (whole tiles only).
+static inline bool stage_row_ok(const wd_ctx *c, int row)
+{
+    if (row < 0 || row >= WD_NUM_TMA_ROWS || c->recon != 18) return false;
+    const wd::TmaRowInfo &t = wd::kTmaRows[row];
+    if (!(c->precision == 64 ? t.f64 : t.f32)) return false;
+    for (int d = 0; d < 4; ++d)
+        if (c->dims[d] % t.b[d] != 0) return false;
+    return true;
+}
+// row the pass of the given mode runs on, or -1 = links through L1
+static inline int stage_row_for(const wd_ctx *c, int mode)
+{
+    if (c->stage_row >= 0) return stage_row_ok(c, c->stage_row) ? c->stage_row : -1;
+    if (c->stage_row == -2 && c->precision == 64 && mode != wd::MODE_RUPD && stage_row_ok(c, WD_TMA_AUTO_ROW_F64))
+        return WD_TMA_AUTO_ROW_F64;
+    return -1;
+}

@@ -6,6 +6,11 @@
                                                                 even-odd solvers at configs 3 and 4, the COO SpMV)
     python -m paper_2111_14958_b200.measure --sweep --config I  every compiled launch configuration (the paper's
                                                                 workgroup-size tuning) on config I
+    python -m paper_2111_14958_b200.measure --staging --config I [--precision 64] [--reps N]
+                                                                the stencil with the shared-memory link pipeline
+                                                                (wd_set_link_staging, csrc/wilson_tma.cuh): every compiled
+                                                                row that covers config I beside the kernel that reads the
+                                                                links through L1, a2 / a3 / a4 inside the CG loop and wd_apply
 
 All of it runs through the C-ABI binding (wilson.py) on seeded synthetic lattices (inputs.py); nothing here touches the
 CPU oracle.  Needs a CUDA device.
@@ -367,6 +372,62 @@ def run_sweep(args, cfg, ctx, wilson, Un, en, psi_n, r_min):
     return 0
 
 
+def run_staging(args):
+    """Per row of the staged stencil (and -1 = links through L1, first and last): a2 / a3 / a4 per CG iteration from CUDA
+    events inside `--steps` solves, the solve time, wd_apply over `--reps` applications, and whether wd_apply is
+    bit-identical to the unstaged kernel."""
+    import torch
+
+    from . import build as wbuild
+    from . import wilson
+
+    wbuild.build()
+    wilson.load_library()
+    prec = args.precision
+    cfg = inputs.CONFIGS[args.config]
+    r_min = cfg.r_min if prec == 32 else 1e-10
+    U, eta = inputs.config_inputs(cfg, dtype=np.complex64 if prec == 32 else np.complex128)
+    V = cfg.volume
+    b2, b3, b4 = (480, 576, 480) if prec == 32 else (960, 1152, 960)
+    with wilson.WilsonContext(cfg.dims, prec, cfg.bc_t) as ctx:
+        ctx.wd_set_cg_mode(1)
+        Un = ctx.wd_pack_gauge(torch.from_numpy(U).cuda())
+        en = ctx.wd_pack_spinor(torch.from_numpy(eta).cuda())
+        out = ctx.empty_spinor()
+        infos = wilson.staging_rows()
+        rows = [i for i, inf in enumerate(infos) if inf[7 if prec == 32 else 8] and all(cfg.dims[d] % inf[d] == 0 for d in range(4))]
+        if args.staging_rows:
+            rows = [r for r in rows if r in [int(v) for v in args.staging_rows.split(",")]]
+        ref = None
+        for row in [-1] + rows + [-1]:
+            ctx.wd_set_link_staging(row)
+            if args.steps > 0:
+                ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=out)
+                ctx.wd_set_profile(1)
+                ms = []
+                for _ in range(args.steps):
+                    _, info = ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=out)
+                    ms.append(info["gpu_ms"])
+                p = ctx.wd_get_profile()
+                ctx.wd_set_profile(0)
+            else:
+                p, ms, info = {"a2_ms": 0.0, "a3_ms": 0.0, "a4_ms": 0.0, "iterations": 0}, [0.0], {"iterations": 0}
+            n = max(p["iterations"], 1)
+            ap = sorted(ctx.wd_apply_repeat(Un, en, cfg.kappa, True, args.reps, out=out) for _ in range(3))[1]
+            got = out.clone()
+            ref = got if ref is None else ref
+            a2, a3, a4 = p["a2_ms"] / n, p["a3_ms"] / n, p["a4_ms"] / n
+            gbs = lambda b, t: b * V / (t * 1e-3) / 1e9 if t > 0 else None
+            print(json.dumps({
+                "staging": f"config{cfg.index}", "precision": prec, "row": row,
+                "tile_stages_buffers_minb": list(infos[row][:7]) if row >= 0 else None,
+                "a2_us": a2 * 1e3, "a3_us": a3 * 1e3, "a4_us": a4 * 1e3, "a2_gbs": gbs(b2, a2), "a3_gbs": gbs(b3, a3),
+                "cg_iteration_gbs": gbs(b2 + b3 + b4, a2 + a3 + a4), "solve_ms": float(np.median(ms)),
+                "iterations": info["iterations"], "wd_apply_dagger_us": ap * 1e3, "wd_apply_gbs": gbs(b2, ap),
+                "bit_identical_to_unstaged": bool(torch.equal(got, ref))}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--report", action="store_true")
@@ -377,6 +438,9 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--precision", type=int, default=32, choices=[32, 64])
     ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--staging", action="store_true")
+    ap.add_argument("--staging-rows", default="", help="rows --staging visits (comma separated; default: all that cover the lattice)")
+    ap.add_argument("--reps", type=int, default=50, help="wd_apply applications per timing of --staging")
     args = ap.parse_args()
     import torch
 
@@ -386,6 +450,8 @@ def main():
         return run_report(args)
     if args.rows:
         return run_rows(args)
+    if args.staging:
+        return run_staging(args)
     if args.sweep:
         from . import build as wbuild
         from . import wilson

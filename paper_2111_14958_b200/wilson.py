@@ -113,6 +113,10 @@ def load_library(path: str = LIB_PATH):
     lib.wd_set_zchunk.argtypes = [vp, ci]
     lib.wd_set_small_tile.argtypes = [vp, ci]
     lib.wd_set_poll_interval.argtypes = [vp, ci]
+    lib.wd_num_staging_rows.argtypes = []
+    lib.wd_staging_row_info.argtypes = [ci, ip]
+    lib.wd_set_link_staging.argtypes = [vp, ci]
+    lib.wd_get_link_staging.argtypes = [vp]
     lib.wd_set_profile.argtypes = [vp, ci]
     lib.wd_get_profile.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_long)]
     lib.wd_selftest_fastdiv.argtypes = [ctypes.c_uint, ctypes.c_uint]
@@ -141,6 +145,18 @@ def tile_infos():
         info = (ctypes.c_int * 3)()
         lib.wd_tile_info(i, info)
         out.append(tuple(shp) + tuple(info))
+    return out
+
+
+def staging_rows():
+    """[(16, BY, BZ, BT, stages, copies_ahead, min_blocks_per_sm, has_fp32, has_fp64), ...]: the compiled configurations of
+    the stencil kernel with the shared-memory link pipeline (wd_set_link_staging)."""
+    lib = load_library()
+    out = []
+    for i in range(lib.wd_num_staging_rows()):
+        info = (ctypes.c_int * 9)()
+        lib.wd_staging_row_info(i, info)
+        out.append(tuple(info))
     return out
 
 
@@ -474,6 +490,13 @@ class WilsonContext:
 
     def wd_set_small_tile(self, index):
         self._check(self.lib.wd_set_small_tile(self._ctx, int(index)))
+
+    def wd_set_link_staging(self, row):
+        """row of staging_rows() for the stencil passes of wd_apply / cg_solve (three-kernel driver); -1 = off"""
+        self._check(self.lib.wd_set_link_staging(self._ctx, int(row)))
+
+    def wd_get_link_staging(self):
+        return int(self.lib.wd_get_link_staging(self._ctx))
 
     def wd_set_poll_interval(self, n):
         self._check(self.lib.wd_set_poll_interval(self._ctx, int(n)))

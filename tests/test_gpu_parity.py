@@ -228,6 +228,89 @@ def test_largest_supported_volume(wilson, oracle):
     assert abs(info["eta_norm2"] / (24.0 * V) - 1.0) < 1e-3        # pin P9 at this size
 
 
+# ---------------------------------------------------------------- the shared-memory link pipeline (wilson_tma.cuh)
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("dims,bc_t", [((16, 4, 4, 4), -1), ((32, 8, 4, 8), 1), ((48, 4, 8, 6), -1), ((16, 12, 8, 10), -1)])
+def test_link_staging_is_bit_identical_and_matches_oracle(wilson, oracle, dims, bc_t, precision):
+    """wd_set_link_staging(row): the gauge field reaches the stencil through bulk copies into a shared-memory ring, both
+    uses of every link served from there.  Same arithmetic in the same order: wd_apply D and D-dagger are bit-identical to
+    the kernel that reads the links through L1 for every compiled row that covers the lattice (several tiles per CTA, so the
+    ring wraps across tile boundaries; both boundary conditions; x extent of one, two and three 16-site blocks), and
+    within the wd_apply tolerance of the oracle.  A row that does not cover the lattice is refused."""
+    cdt = gu.np_complex(precision)
+    U = inputs.gauge_field(CFG_TEST + 11, dims, "haar", dtype=cdt)
+    psi = inputs.source_field(CFG_TEST + 11, dims, dtype=cdt, field=inputs.FIELD_AUX)
+    U64, psi64 = U.astype(np.complex128), psi.astype(np.complex128)
+    ran = 0
+    with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        pn = ctx.wd_pack_spinor(gu.to_device(psi))
+        ctx.wd_set_link_staging(-1)      # the reference: links through L1
+        ref = {dag: gu.to_host(ctx.wd_unpack_spinor(ctx.wd_apply(Un, pn, 0.12, dag))) for dag in (False, True)}
+        for dag in (False, True):
+            want = oracle.wd_apply(dims, U64, psi64, 0.12, dag, bc_t)
+            assert lm.per_site_rel_err(ref[dag], want)[0] <= TOL_APPLY[precision]
+        for row, info in enumerate(wilson.staging_rows()):
+            covers = info[7 if precision == 32 else 8] and all(dims[d] % info[d] == 0 for d in range(4))
+            if not covers:
+                with pytest.raises(wilson.WilsonError):
+                    ctx.wd_set_link_staging(row)
+                continue
+            ctx.wd_set_link_staging(row)
+            assert ctx.wd_get_link_staging() == row
+            for dag in (False, True):
+                for _ in range(2):      # twice: the barriers are re-initialised by every launch
+                    got = gu.to_host(ctx.wd_unpack_spinor(ctx.wd_apply(Un, pn, 0.12, dag)))
+                    assert got.tobytes() == ref[dag].tobytes(), (row, info, dag)
+            ran += 1
+            ctx.wd_set_link_staging(-1)
+            assert ctx.wd_get_link_staging() == -1
+    assert ran >= 1
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_cg_solve_with_link_staging(wilson, oracle, precision):
+    """the three-kernel CG with every stencil pass (a2, a3, a6) on the staged kernel: iteration count, residual history and
+    true residual against the oracle (config 1, 8^4 is too narrow: a 16 x 8 x 8 x 8 lattice with config 1's recipe), and
+    against the unstaged solve (per-site arithmetic identical, only the grouping of the reduction partials differs)."""
+    dims, kappa, bc_t = (16, 8, 8, 8), 0.124, -1
+    r_min = 1e-6 if precision == 32 else 1e-10
+    cdt = gu.np_complex(precision)
+    U = inputs.gauge_field(CFG_TEST + 12, dims, "near_identity", dtype=cdt)
+    eta = inputs.source_field(CFG_TEST + 12, dims, dtype=cdt)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    psi_o, info_o = oracle.cg_solve(dims, U64, eta64, kappa, r_min, 1000, bc_t, history=True)
+    res_o = oracle.true_residual(dims, U64, eta64, psi_o, kappa, bc_t)
+    ran = 0
+    with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+        ctx.wd_set_cg_mode(1)
+        ctx.wd_set_link_staging(-1)
+        psi0, info0 = gu.solve_on_gpu(ctx, U, eta, kappa, r_min, 1000)
+        for row, info in list(enumerate(wilson.staging_rows())) + [(-2, None)]:
+            if row == -2:          # the automatic choice (the default of a fresh ctx)
+                ctx.wd_set_link_staging(-2)
+                assert ctx.wd_get_link_staging() == (-1 if precision == 32 else 2)
+                psi, inf = gu.solve_on_gpu(ctx, U, eta, kappa, r_min, 1000)
+                assert inf["status"] == 0 and inf["iterations"] == info0["iterations"]
+                assert np.linalg.norm(psi - psi0) <= (1e-5 if precision == 32 else 1e-12) * np.linalg.norm(psi0)
+                continue
+            if not (info[7 if precision == 32 else 8] and all(dims[d] % info[d] == 0 for d in range(4))):
+                continue
+            ctx.wd_set_link_staging(row)
+            psi, inf = gu.solve_on_gpu(ctx, U, eta, kappa, r_min, 1000)
+            hist = ctx.wd_cg_history()
+            assert inf["status"] == 0 and inf["cg_mode"] == 1
+            assert iters_close(inf["iterations"], info_o["iterations"]) and inf["iterations"] == info0["iterations"]
+            res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), kappa, bc_t)
+            assert res <= 2.0 * res_o, (row, res, res_o)
+            n = min(len(hist), len(info_o["rr_history"])) // 2
+            rel = np.abs(hist[:n] - info_o["rr_history"][:n]) / info_o["rr_history"][:n]
+            assert np.max(rel) < (2e-2 if precision == 32 else 1e-6)
+            assert np.linalg.norm(psi - psi0) <= (1e-5 if precision == 32 else 1e-12) * np.linalg.norm(psi0)
+            ran += 1
+    assert ran >= 1
+
+
 # ---------------------------------------------------------------- reductions
 @pytest.mark.parametrize("precision", [32, 64])
 def test_norm2_matches_oracle_and_is_deterministic(wilson, oracle, precision):
