@@ -272,10 +272,14 @@ int cg_solve_multi(wd_ctx *ctx, const void *U_native, const void *eta_multi, voi
  *                    forward : Val = -kappa s+ (1 - gamma_mu)[alpha][beta] U_mu(x)[a][b],            Col = (x+mu, beta, b)
  *                    backward: Val = -kappa s- (1 + gamma_mu)[alpha][beta] conj(U_mu(x-mu)[b][a]),   Col = (x-mu, beta, b)
  *                  (gamma_mu -> -gamma_mu for D-dagger; s+- = bc_t on the hop that wraps in t).  Needs 12 V < 2^31.
- * wd_coo_spmv      out = 0, then the loop above for ANY coordinate-format matrix with 12 V rows (entries in any order,
- *                  duplicates are summed): parallel over k, equal rows of adjacent entries are combined inside a warp
- *                  before one atomic add per run (the sum order of a row is therefore not fixed: results agree to
- *                  rounding, not bitwise).  in_dev, out_dev: canonical vectors on the device, must not alias.
+ * wd_coo_spmv      the loop above for ANY coordinate-format matrix with 12 V rows (entries in any order, duplicates are
+ *                  summed).  General path: out = 0, then parallel over k, equal rows of adjacent entries combined inside a
+ *                  warp before one atomic add per run (the sum order of a row is not fixed: results agree to rounding, not
+ *                  bitwise).  Fast path, taken in fp32 when val/row/col are the arrays the last wd_coo_assemble of this ctx wrote
+ *                  (N_NZ = 588 V): one warp per site, 12 row accumulators, plain stores, fixed summation order; Row is still
+ *                  read and checked entry by entry, and if it is not the assembled structure any more (the caller edited the
+ *                  arrays) the general path recomputes the product inside the same call.  wd_set_coo_fast(ctx, 0) forces
+ *                  the general path.  in_dev, out_dev: canonical vectors on the device, must not alias.
  * All three are asynchronous on the ctx stream.  Errors: WD_ERR_ARG, WD_ERR_DIMS, WD_ERR_CUDA.
  */
 size_t wd_coo_nnz(wd_ctx *ctx);
@@ -283,6 +287,7 @@ int wd_coo_assemble(wd_ctx *ctx, const void *U_native, double kappa, int dagger,
                     int *col_dev);
 int wd_coo_spmv(wd_ctx *ctx, size_t nnz, const void *val_dev, const int *row_dev, const int *col_dev,
                 const void *in_dev, void *out_dev);
+int wd_set_coo_fast(wd_ctx *ctx, int on);
 
 /*
  * Host-buffer forms: the same operations with HOST pointers in the CANONICAL layout.  Each call

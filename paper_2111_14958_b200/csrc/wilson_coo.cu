@@ -4,6 +4,7 @@
 // the product path is the matrix-free stencil (the paper itself calls the format "not optimal").
 #include "wilson_ctx.cuh"
 
+#include <algorithm>
 #include <cmath>
 
 using namespace wd;
@@ -89,11 +90,13 @@ __device__ __forceinline__ void atomic_add_c(double2 *p, double2 v)
 // The paper's loop, parallel over k.  A warp takes 32 consecutive entries per step, multiplies, then adds up runs
 // of equal Row inside the warp with shuffles (a segmented scan: rows sorted as wd_coo_assemble writes them give at
 // most two runs per step) and only the last lane of each run issues the atomic add.  Any entry order is correct.
+// only_if != nullptr: run only if *only_if == epoch (the fall-back behind the sorted-row fast path below)
 template <typename cvec>
 __global__ void __launch_bounds__(COO_NT)
 coo_spmv_kernel(long nnz, const cvec *__restrict__ val, const int *__restrict__ row, const int *__restrict__ col,
-                const cvec *__restrict__ in, cvec *out)
+                const cvec *__restrict__ in, cvec *out, const unsigned int *only_if, unsigned int epoch)
 {
+    if (only_if && *only_if != epoch) return;
     constexpr int UNROLL = 4;   // independent 32-entry groups per trip: the Col -> in[Col] dependent loads overlap
     const int lane = threadIdx.x & 31;
     const long warp = ((long)blockIdx.x * COO_NT + threadIdx.x) >> 5;
@@ -131,6 +134,96 @@ coo_spmv_kernel(long nnz, const cvec *__restrict__ val, const int *__restrict__ 
     }
 }
 
+template <typename cvec>
+__global__ void __launch_bounds__(COO_NT)
+coo_zero_if_kernel(cvec *out, size_t n, const unsigned int *only_if, unsigned int epoch)
+{
+    if (*only_if != epoch) return;
+    for (size_t i = (size_t)blockIdx.x * COO_NT + threadIdx.x; i < n; i += (size_t)gridDim.x * COO_NT) { out[i].x = 0; out[i].y = 0; }
+}
+
+// Sorted-row fast path: the matrix as wd_coo_assemble writes it has its entries grouped by row, 49 per row, i.e. 588
+// consecutive entries per site.  One warp takes one site at a time: 19 coalesced groups of 32 entries (Val, Row, Col read
+// exactly once, as in the paper's loop), the product of every entry added to one of 12 per-lane row accumulators -- which
+// row a lane's entry of group i belongs to is a compile-time function of (i, lane), because the rows are 49 long -- then
+// one butterfly reduction per row and 12 plain stores: no atomics, no zero-fill pass, and a fixed summation order (the
+// result is bitwise reproducible).  The Row array is still READ and CHECKED entry by entry: the first entry that is not
+// where the structure says raises *bad = epoch, and the caller's fall-back (zero-fill + the any-order kernel above, both
+// conditional on that flag) recomputes the product, so the call is correct for any coordinate-format input.
+template <typename cvec>
+__global__ void __launch_bounds__(COO_NT)
+coo_spmv_rows49_kernel(int nsites, const cvec *__restrict__ val, const int *__restrict__ row, const int *__restrict__ col,
+                       const cvec *__restrict__ in, cvec *out, unsigned int *bad, unsigned int epoch)
+{
+    constexpr int SITE_NNZ = 12 * ROW_NNZ;            // 588
+    constexpr int NG = (SITE_NNZ + 31) / 32;           // 19 groups of 32 entries
+    const int lane = threadIdx.x & 31;
+    const int warp = (int)(((long)blockIdx.x * COO_NT + threadIdx.x) >> 5);
+    const int nwarps = (int)(((long)gridDim.x * COO_NT) >> 5);
+    bool viol = false;
+    for (int site = warp; site < nsites; site += nwarps) {
+        const long base = (long)site * SITE_NNZ;
+        cvec acc[12];
+#pragma unroll
+        for (int r = 0; r < 12; ++r) { acc[r].x = 0; acc[r].y = 0; }
+        // groups in batches of GB: all Val / Row / Col loads of a batch are issued before the first dependent in[Col] gather.
+        // (Measured and not kept: prefetching the next batch's three streams before the gathers of this one, on a grid of
+        // exactly one resident wave -- 32^4 fp32 1710 -> 1900 us: the extra registers cost more warps than the overlap gains.)
+        constexpr int GB = 5;
+#pragma unroll
+        for (int i0 = 0; i0 < NG; i0 += GB) {
+            cvec v[GB];
+            int rw[GB], cl[GB];
+#pragma unroll
+            for (int u = 0; u < GB; ++u) {
+                const int e = 32 * (i0 + u) + lane;
+                v[u].x = 0; v[u].y = 0; rw[u] = -1; cl[u] = 0;
+                if (i0 + u < NG && e < SITE_NNZ) {
+                    v[u] = __ldg(val + base + e);
+                    rw[u] = __ldg(row + base + e);
+                    cl[u] = __ldg(col + base + e);
+                }
+            }
+            cvec x[GB];
+#pragma unroll
+            for (int u = 0; u < GB; ++u) {
+                x[u].x = 0; x[u].y = 0;
+                if (rw[u] >= 0) x[u] = __ldg(in + cl[u]);
+            }
+#pragma unroll
+            for (int u = 0; u < GB; ++u) {
+                const int i = i0 + u;
+                if (i < NG) {
+                    const int r0 = (32 * i) / ROW_NNZ;                       // compile-time after unrolling
+                    const int bnd = ROW_NNZ * (r0 + 1) - 32 * i;             // lanes >= bnd belong to row r0 + 1
+                    const int r1 = r0 + 1 < 12 ? r0 + 1 : 11;                // (group 18: lanes >= bnd are past the site)
+                    const bool in_a = lane < bnd;
+                    const bool valid = 32 * i + lane < SITE_NNZ;
+                    viol = viol || (valid && rw[u] != site * 12 + (in_a ? r0 : r0 + 1));
+                    cvec p;
+                    p.x = v[u].x * x[u].x - v[u].y * x[u].y;
+                    p.y = v[u].x * x[u].y + v[u].y * x[u].x;
+                    if (in_a) { acc[r0].x += p.x; acc[r0].y += p.y; }
+                    else { acc[r1].x += p.x; acc[r1].y += p.y; }
+                }
+            }
+        }
+        cvec mine;
+        mine.x = 0; mine.y = 0;
+#pragma unroll
+        for (int r = 0; r < 12; ++r) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                acc[r].x += __shfl_xor_sync(0xffffffffu, acc[r].x, o);
+                acc[r].y += __shfl_xor_sync(0xffffffffu, acc[r].y, o);
+            }
+            if (lane == r) mine = acc[r];
+        }
+        if (lane < 12) out[(size_t)site * 12 + lane] = mine;
+    }
+    if (__any_sync(0xffffffffu, viol) && lane == 0) atomicExch(bad, epoch);
+}
+
 }  // namespace
 
 extern "C" size_t wd_coo_nnz(wd_ctx *c) { return c ? (size_t)c->V * 588 : 0; }
@@ -156,6 +249,8 @@ extern "C" int wd_coo_assemble(wd_ctx *c, const void *U_native, double kappa, in
                                                                             (double2 *)val, row, col, nnz);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
+    // wd_coo_spmv takes its sorted-row fast path for exactly these arrays (and checks the structure as it reads them)
+    c->coo_val = val; c->coo_row = row; c->coo_col = col;
     return WD_OK;
 }
 
@@ -166,18 +261,53 @@ extern "C" int wd_coo_spmv(wd_ctx *c, size_t nnz, const void *val, const int *ro
     if (!in || !out || in == out || (nnz > 0 && (!val || !row || !col)))
         return fail(c, WD_ERR_ARG, "wd_coo_spmv: NULL or aliased argument");
     const size_t out_bytes = (size_t)c->V * 12 * 2 * (c->precision == 32 ? 4 : 8);
-    CUDA_TRY(c, cudaMemsetAsync(out, 0, out_bytes, c->stream));
-    if (nnz == 0) return WD_OK;
     size_t need = (nnz + 4 * COO_NT - 1) / (4 * COO_NT);   // 4 groups of 32 entries per warp and trip
     const size_t cap = (size_t)c->sm_count * 8 * 4;   // 8 CTAs per SM resident, 4 waves: warps stride over the entries
-    const unsigned int grid = (unsigned int)(need < cap ? need : cap);
+    const unsigned int grid = (unsigned int)(need < cap ? (need ? need : 1) : cap);
+    // fp32 only: in fp64 the 12 complex accumulators per lane cost too many warps (measured 14^4 / 32^4: 174 / 4009 us
+    // against 133 / 3656 us for the any-order kernel), so fp64 keeps the atomic path
+    const bool assembled = c->coo_fast && c->precision == 32 && nnz == (size_t)c->V * 588 && val == c->coo_val &&
+                           row == c->coo_row && col == c->coo_col;
+    if (assembled) {
+        // the arrays wd_coo_assemble wrote: sorted-row kernel (plain stores, structure checked on the fly), and behind it the
+        // any-order path as a fall-back that runs only if the check failed (the caller changed the arrays since)
+        if (!c->coo_bad) {
+            CUDA_TRY(c, cudaMalloc(&c->coo_bad, sizeof(unsigned int)));
+            CUDA_TRY(c, cudaMemsetAsync(c->coo_bad, 0, sizeof(unsigned int), c->stream));
+        }
+        const unsigned int epoch = ++c->coo_epoch ? c->coo_epoch : ++c->coo_epoch;   // never 0
+        const size_t wneed = ((size_t)c->V * 32 + COO_NT - 1) / COO_NT;             // one warp per site at a time ...
+        const size_t wcap = (size_t)c->sm_count * 8;                                // ... 8 CTAs per SM, warps stride over the sites
+        const unsigned int fgrid = (unsigned int)(wneed < wcap ? wneed : wcap);
+        const size_t nout = (size_t)c->V * 12;
+        const unsigned int zgrid = (unsigned int)std::min<size_t>((nout + COO_NT - 1) / COO_NT, (size_t)c->sm_count * 8);
+        coo_spmv_rows49_kernel<float2><<<fgrid, COO_NT, 0, c->stream>>>(c->V, (const float2 *)val, row, col, (const float2 *)in,
+                                                                      (float2 *)out, c->coo_bad, epoch);
+        coo_zero_if_kernel<float2><<<zgrid, COO_NT, 0, c->stream>>>((float2 *)out, nout, c->coo_bad, epoch);
+        coo_spmv_kernel<float2><<<grid, COO_NT, 0, c->stream>>>((long)nnz, (const float2 *)val, row, col, (const float2 *)in,
+                                                               (float2 *)out, c->coo_bad, epoch);
+        c->launches += 3;
+        CUDA_TRY(c, cudaGetLastError());
+        return WD_OK;
+    }
+    CUDA_TRY(c, cudaMemsetAsync(out, 0, out_bytes, c->stream));
+    if (nnz == 0) return WD_OK;
     if (c->precision == 32)
         coo_spmv_kernel<float2><<<grid, COO_NT, 0, c->stream>>>((long)nnz, (const float2 *)val, row, col,
-                                                               (const float2 *)in, (float2 *)out);
+                                                               (const float2 *)in, (float2 *)out, nullptr, 0u);
     else
         coo_spmv_kernel<double2><<<grid, COO_NT, 0, c->stream>>>((long)nnz, (const double2 *)val, row, col,
-                                                                (const double2 *)in, (double2 *)out);
+                                                                (const double2 *)in, (double2 *)out, nullptr, 0u);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
+    return WD_OK;
+}
+
+/* 1 (default): wd_coo_spmv takes the sorted-row kernel for the arrays the last wd_coo_assemble of this ctx wrote; 0: always
+   the any-order atomic kernel (the comparison row of the measurement tables). */
+extern "C" int wd_set_coo_fast(wd_ctx *c, int on)
+{
+    if (!c || on < 0 || on > 1) return WD_ERR_ARG;
+    c->coo_fast = on;
     return WD_OK;
 }

@@ -8,6 +8,10 @@
 #include <cstdarg>
 #include <cstdio>
 
+#ifndef WD_HOST_SLABS
+#define WD_HOST_SLABS 8   // slabs the host-buffer calls move their fields in (wilson_cg.cu, stage_inputs)
+#endif
+
 struct wd_ctx {
     int dims[4];
     int V;
@@ -55,6 +59,8 @@ struct wd_ctx {
     // staging of the *_host calls
     void *U_can, *U_nat, *s_can, *s_nat_in, *s_nat_out;
     int have_gauge;
+    cudaStream_t copy_stream;   // the *_host calls: transfers run here, slab by slab, beside the pack / unpack kernels
+    cudaEvent_t slab_ev[WD_HOST_SLABS + 1];
     cudaEvent_t ev[4];
     // per-kernel-class timing (wd_set_profile): 4 events per iteration of one poll chunk
     int profile;
@@ -66,6 +72,11 @@ struct wd_ctx {
                             // iteration of every poll chunk
     double bprof_ms[7];
     long bprof_n;
+    // the arrays of the last wd_coo_assemble (wd_coo_spmv's sorted-row fast path), its violation flag and call counter
+    const void *coo_val, *coo_row, *coo_col;
+    unsigned int *coo_bad;
+    unsigned int coo_epoch;
+    int coo_fast;
     int last_iters;
     int launches;
     char err[512];

@@ -1134,10 +1134,12 @@ norm2_kernel(const typename Field<real>::svec *__restrict__ a, size_t n, int V, 
 // the site's block; canonical spinor psi[s][alpha][a] (NSP vectors, contiguous) -> plane j.  Pad lanes get zeros.
 template <typename real, int RECON = 18>
 __global__ void __launch_bounds__(VEC_NT)
-pack_gauge_kernel(const typename Field<real>::gvec *__restrict__ can, typename Field<real>::gvec *nat, int V, int Vpad)
+pack_gauge_kernel(const typename Field<real>::gvec *__restrict__ can, typename Field<real>::gvec *nat, int V, int Vpad,
+                  int s0 = 0)
 {
+    // sites s0 .. Vpad - 1 (the host-buffer calls pack slab by slab as the copies land; the grid bounds the slab)
     using gvec = typename Field<real>::gvec;
-    const int s = blockIdx.x * VEC_NT + threadIdx.x;
+    const int s = s0 + blockIdx.x * VEC_NT + threadIdx.x;
     if (s >= Vpad) return;
     for (int mu = 0; mu < 4; ++mu) {
         gvec k9[9];
@@ -1149,11 +1151,12 @@ pack_gauge_kernel(const typename Field<real>::gvec *__restrict__ can, typename F
 }
 template <typename real>
 __global__ void __launch_bounds__(VEC_NT)
-pack_spinor_kernel(const typename Field<real>::svec *__restrict__ can, typename Field<real>::svec *nat, int V, int Vpad)
+pack_spinor_kernel(const typename Field<real>::svec *__restrict__ can, typename Field<real>::svec *nat, int V, int Vpad,
+                   int s0 = 0)
 {
     using svec = typename Field<real>::svec;
     constexpr int NSP = Field<real>::NSP;
-    const int s = blockIdx.x * VEC_NT + threadIdx.x;
+    const int s = s0 + blockIdx.x * VEC_NT + threadIdx.x;
     if (s >= Vpad) return;
     svec *p = nat + spinor_index<svec, NSP>(s);
 #pragma unroll
@@ -1161,11 +1164,11 @@ pack_spinor_kernel(const typename Field<real>::svec *__restrict__ can, typename 
 }
 template <typename real>
 __global__ void __launch_bounds__(VEC_NT)
-unpack_spinor_kernel(const typename Field<real>::svec *__restrict__ nat, typename Field<real>::svec *can, int V)
+unpack_spinor_kernel(const typename Field<real>::svec *__restrict__ nat, typename Field<real>::svec *can, int V, int s0 = 0)
 {
     using svec = typename Field<real>::svec;
     constexpr int NSP = Field<real>::NSP;
-    const int s = blockIdx.x * VEC_NT + threadIdx.x;
+    const int s = s0 + blockIdx.x * VEC_NT + threadIdx.x;
     if (s >= V) return;
     const svec *p = nat + spinor_index<svec, NSP>(s);
 #pragma unroll

@@ -294,9 +294,18 @@ def run_rows(args):
                         "cg_solve_ms_same_problem": t, "speedup_vs_cg": t / t12}), flush=True)
                     ctx.wd_set_gauge_recon(18)
                     del Ue, U12, ee, pe
-    # f2: the paper's COO SpMV at its largest volume
-    cfg = inputs.CONFIGS[2]
-    U, eta = inputs.config_inputs(cfg, dtype=cdt)
+    # f2: the paper's COO SpMV at its largest volume (14^4) and at 32^4 (9.9 GB of Val / Row / Col in fp32)
+    for ci in (2, 3):
+        run_coo_row(torch, wilson, ci, prec, peak)
+    return 0
+
+
+def run_coo_row(torch, wilson, ci, prec, peak):
+    """wd_coo_spmv on the arrays wd_coo_assemble wrote: the sorted-row fast path and, beside it, the any-order atomic
+    kernel (wd_set_coo_fast(0)), as GB/s of the algorithmic 9600 B/site (fp32) and as GFLOP/s at 8 flop per entry."""
+    cfg = inputs.CONFIGS[ci]
+    rb = 4 if prec == 32 else 8
+    U, eta = inputs.config_inputs(cfg, dtype=np.complex64 if prec == 32 else np.complex128)
     V = cfg.volume
     with wilson.WilsonContext(cfg.dims, prec, cfg.bc_t) as ctx:
         Un = ctx.wd_pack_gauge(torch.from_numpy(U).cuda())
@@ -313,26 +322,32 @@ def run_rows(args):
         torch.cuda.synchronize()
         asm_ms = e0.elapsed_time(e1) / 10
         out = torch.empty_like(eta_d)
-        for _ in range(5):
-            ctx.wd_coo_spmv(val, row, col, eta_d, out=out)
-        reps = 100
-        e0.record()
-        for _ in range(reps):
-            ctx.wd_coo_spmv(val, row, col, eta_d, out=out)
-        e1.record()
-        torch.cuda.synchronize()
-        sp_ms = e0.elapsed_time(e1) / reps
+        reps = 100 if ci == 2 else 20
+        times = {}
+        for fast in (1, 0):
+            ctx.wd_set_coo_fast(fast)
+            for _ in range(5):
+                ctx.wd_coo_spmv(val, row, col, eta_d, out=out)
+            e0.record()
+            for _ in range(reps):
+                ctx.wd_coo_spmv(val, row, col, eta_d, out=out)
+            e1.record()
+            torch.cuda.synchronize()
+            times[fast] = e0.elapsed_time(e1) / reps
+        ctx.wd_set_coo_fast(1)
         st_ms = time_wd_apply(ctx, Un, en, out_n, cfg.kappa, False)
         nnz = NNZ_PER_SITE * V
         coo_bytes = nnz * (2 * rb + 8) + 2 * 12 * V * 2 * rb   # Val + Row + Col once, in and out vectors once
+        gbs = lambda ms: coo_bytes / (ms * 1e-3) / 1e9
         print(json.dumps({
-            "row": "f2 coo spmv", "config": 2, "precision": prec, "nnz": nnz, "assemble_ms": asm_ms,
-            "spmv_us": sp_ms * 1e3, "spmv_gflops_8_per_nnz": FLOP_COO_NNZ * nnz / (sp_ms * 1e-3) / 1e9,
-            "spmv_gbs": coo_bytes / (sp_ms * 1e-3) / 1e9, "spmv_frac_of_measured": coo_bytes / (sp_ms * 1e-3) / 1e9 / peak,
-            "bytes_per_site": coo_bytes / V, "stencil_wd_apply_us": st_ms * 1e3,
-            "stencil_speedup": sp_ms / st_ms,
+            "row": "f2 coo spmv", "config": ci, "name": cfg.name, "precision": prec, "nnz": nnz, "assemble_ms": asm_ms,
+            "spmv_us": times[1] * 1e3, "spmv_gflops_8_per_nnz": FLOP_COO_NNZ * nnz / (times[1] * 1e-3) / 1e9,
+            "spmv_gbs": gbs(times[1]), "spmv_frac_of_measured": gbs(times[1]) / peak,
+            "any_order_kernel_us": times[0] * 1e3, "any_order_kernel_gbs": gbs(times[0]),
+            "any_order_kernel_frac_of_measured": gbs(times[0]) / peak,
+            "bytes_per_site": coo_bytes / V, "coo_bytes_total": coo_bytes, "stencil_wd_apply_us": st_ms * 1e3,
+            "stencil_speedup": times[1] / st_ms,
             "paper": "about 65 GFLOP/s COO SpMV on an A100-PCIE-40GB (PAPER.md:96), other hardware: context only"}), flush=True)
-    return 0
 
 
 def run_sweep(args, cfg, ctx, wilson, Un, en, psi_n, r_min):
@@ -438,6 +453,7 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--precision", type=int, default=32, choices=[32, 64])
     ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--coo", action="store_true", help="only the COO SpMV rows of --rows (14^4 and 32^4)")
     ap.add_argument("--staging", action="store_true")
     ap.add_argument("--staging-rows", default="", help="rows --staging visits (comma separated; default: all that cover the lattice)")
     ap.add_argument("--reps", type=int, default=50, help="wd_apply applications per timing of --staging")
@@ -450,6 +466,15 @@ def main():
         return run_report(args)
     if args.rows:
         return run_rows(args)
+    if args.coo:
+        from . import build as wbuild
+        from . import wilson
+
+        wbuild.build()
+        wilson.load_library()
+        for ci in (2, 3):
+            run_coo_row(torch, wilson, ci, args.precision, measured_peak()[0])
+        return 0
     if args.staging:
         return run_staging(args)
     if args.sweep:

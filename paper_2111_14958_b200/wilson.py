@@ -113,6 +113,7 @@ def load_library(path: str = LIB_PATH):
     lib.wd_set_zchunk.argtypes = [vp, ci]
     lib.wd_set_small_tile.argtypes = [vp, ci]
     lib.wd_set_poll_interval.argtypes = [vp, ci]
+    lib.wd_set_coo_fast.argtypes = [vp, ci]
     lib.wd_num_staging_rows.argtypes = []
     lib.wd_staging_row_info.argtypes = [ci, ip]
     lib.wd_set_link_staging.argtypes = [vp, ci]
@@ -490,6 +491,10 @@ class WilsonContext:
 
     def wd_set_small_tile(self, index):
         self._check(self.lib.wd_set_small_tile(self._ctx, int(index)))
+
+    def wd_set_coo_fast(self, on):
+        """1 (default): wd_coo_spmv uses the sorted-row kernel for the arrays wd_coo_assemble wrote; 0: always the any-order kernel"""
+        self._check(self.lib.wd_set_coo_fast(self._ctx, int(on)))
 
     def wd_set_link_staging(self, row):
         """row of staging_rows() for the stencil passes of wd_apply / cg_solve (three-kernel driver); -1 = off"""

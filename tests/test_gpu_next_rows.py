@@ -181,6 +181,54 @@ def test_coo_spmv_baseline_configs(wilson, oracle, cfg_index, precision):
             assert lm.per_site_rel_err(got, oracle.coo_spmv(vo, ro, co, eta64))[0] <= tol
 
 
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (5, 7, 4, 6), (14, 14, 14, 14)])
+def test_coo_spmv_sorted_row_fast_path(wilson, oracle, dims, precision):
+    """The arrays wd_coo_assemble wrote take the sorted-row kernel (one warp per site, plain stores): same product as the
+    any-order atomic kernel and as the oracle, bitwise reproducible.  It CHECKS the structure it relies on while reading
+    Row: if the caller has edited the arrays in place (entries permuted across rows, a row index changed, an out array
+    full of NaN because the fast path does not zero it) the general path recomputes inside the same call."""
+    import torch
+
+    cdt = gu.np_complex(precision)
+    tol = 1e-5 if precision == 32 else 1e-12
+    kappa = 0.12
+    U = inputs.gauge_field(CFG_TEST + 21, dims, "haar", dtype=cdt)
+    x = inputs.source_field(CFG_TEST + 21, dims, dtype=cdt)
+    want = oracle.wd_apply(dims, U.astype(np.complex128), x.astype(np.complex128), kappa, False, -1)
+    with wilson.WilsonContext(dims, precision, -1) as ctx:
+        Un = ctx.wd_pack_gauge(gu.to_device(U))
+        xd = gu.to_device(x)
+        val, row, col = ctx.wd_coo_assemble(Un, kappa, False)
+        fast = [gu.to_host(ctx.wd_coo_spmv(val, row, col, xd, out=torch.full_like(xd, float("nan")))) for _ in range(3)]
+        if precision == 32:     # (fp64 keeps the atomic kernel: the sorted-row kernel measured slower there)
+            assert fast[0].tobytes() == fast[1].tobytes() == fast[2].tobytes()      # fixed summation order
+        assert lm.per_site_rel_err(fast[0], want)[0] <= tol
+        ctx.wd_set_coo_fast(0)
+        slow = gu.to_host(ctx.wd_coo_spmv(val, row, col, xd))
+        ctx.wd_set_coo_fast(1)
+        assert lm.per_site_rel_err(fast[0], slow)[0] <= 2 * tol
+        # the caller permutes the entries in place (still the same matrix): structure check fails, fall-back recomputes
+        perm = torch.randperm(val.numel(), device="cuda", generator=torch.Generator(device="cuda").manual_seed(5))
+        val.copy_(val[perm]); row.copy_(row[perm]); col.copy_(col[perm])
+        got = gu.to_host(ctx.wd_coo_spmv(val, row, col, xd, out=torch.full_like(xd, float("nan"))))
+        assert lm.per_site_rel_err(got, want)[0] <= tol
+        # a single row index moved to another row of the same site: a different matrix, and the product follows it
+        val, row, col = ctx.wd_coo_assemble(Un, kappa, False)
+        k = 49 * 7 + 3
+        old = int(row[k].item())
+        row[k] = old + 1
+        got = gu.to_host(ctx.wd_coo_spmv(val, row, col, xd)).reshape(-1)
+        v, r, c = gu.to_host(val), gu.to_host(row), gu.to_host(col)
+        ref = np.zeros(12 * int(np.prod(dims)), dtype=np.complex128)
+        np.add.at(ref, r, v.astype(np.complex128) * x.reshape(-1).astype(np.complex128)[c])
+        assert np.max(np.abs(got - ref)) <= tol * np.max(np.abs(ref))
+        # and a fresh assembly is fast and exact again
+        val, row, col = ctx.wd_coo_assemble(Un, kappa, False)
+        again = gu.to_host(ctx.wd_coo_spmv(val, row, col, xd))
+        assert lm.per_site_rel_err(again, want)[0] <= tol and (precision == 64 or again.tobytes() == fast[0].tobytes())
+
+
 def test_coo_spmv_any_entry_order_and_duplicates(wilson, oracle):
     """the loop is defined for any coordinate-format matrix: shuffled entries, repeated (row, col) pairs, empty rows"""
     import torch
