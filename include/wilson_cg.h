@@ -322,12 +322,18 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *                             1 if compiled for precision 64}.
  *   wd_set_tile(ctx, i)       select tile i for the stencil kernels of this ctx; i = -1 restores the automatic choice.
  *   wd_get_tile(ctx)          index in use.
- *   wd_set_cg_mode(ctx, m)        0 = automatic (one cooperative launch for the whole solve when V <= 200000 sites in fp32 /
+ *   wd_set_cg_mode(ctx, m)        0 = automatic (mode 9 where the lattice fits one or two CTAs of it, else one cooperative launch for the whole solve when V <= 200000 sites in fp32 /
  *                             65536 in fp64 — this covers the paper's own 4^4..14^4 range — else three kernels per iteration),
  *                             1 = always three kernels, 2 = always one launch, one thread per site (grid barriers between the
  *                             phases; same recurrence and precision), 6 = always one launch with a CTA of 32 sites x 4
  *                             directions: warp mu computes the two hops of direction mu, the partial sums meet in shared
- *                             memory (the automatic choice in fp64 up to 8192 sites).
+ *                             memory (the automatic choice in fp64 up to 8192 sites),
+ *                             9 = one launch with the whole lattice RESIDENT IN SHARED MEMORY (csrc/wilson_resident.cuh): a
+ *                             thread-block cluster of nc <= 16 CTAs, V / nc sites each (a power of two, <= 256 in fp32, <= 128
+ *                             in fp64), neighbours in other CTAs read through distributed shared memory, barrier.cluster
+ *                             between the phases; covers 4^4 (one CTA in fp32) and 8^4 in fp32 (16 CTAs); WD_ERR_ARG if the
+ *                             lattice does not fit.  Automatic where nc <= 2 (larger clusters are bound by the distributed-shared-
+ *                             memory bandwidth and measured slower than mode 2).
  *   wd_set_zchunk(ctx, layers)    z extent (in sites) of one chunk of the CTA rasterisation x,y,z-in-chunk,t,z-chunk that
  *                             keeps the +-t neighbours of a tile in L2; 0 = automatic (fits a 40 MB reuse distance).
  *   wd_set_small_tile(ctx, i)     launch configuration (CTA tile, register bound) of the one-launch CG kernel of mode 2:

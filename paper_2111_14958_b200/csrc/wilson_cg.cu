@@ -3,6 +3,7 @@
 // enqueues launches on the caller's stream and polls the device stop flag.
 #include "wilson_ctx.cuh"
 #include "wilson_split.cuh"
+#include "wilson_resident.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -236,9 +237,16 @@ extern "C" int wd_set_tile(wd_ctx *c, int index)
     return WD_OK;
 }
 extern "C" int wd_get_tile(wd_ctx *c) { return c ? c->tile : WD_ERR_ARG; }
+static bool resident_plan(const wd_ctx *c, int *nc_out, int *spc_out);
 extern "C" int wd_set_cg_mode(wd_ctx *c, int mode)
 {
-    if (!c || mode < 0 || (mode > 2 && mode != 6)) return WD_ERR_ARG;
+    if (!c || mode < 0 || (mode > 2 && mode != 6 && mode != 9)) return WD_ERR_ARG;
+    if (mode == 9) {
+        int nc, spc;
+        if (!resident_plan(c, &nc, &spc))
+            return fail(c, WD_ERR_ARG, "wd_set_cg_mode(9): the lattice does not fit a cluster's shared memory (V / nc a power of two <= %d, nc <= 16, 18-real links)",
+                        c->precision == 32 ? 256 : 128);
+    }
     if (mode >= 2 && !c->coop_ok) return fail(c, WD_ERR_CUDA, "wd_set_cg_mode: the device does not support cooperative launches");
     if (mode >= 2 && c->recon != 18) return fail(c, WD_ERR_ARG, "wd_set_cg_mode: the one-launch kernels need 18-real links");
     c->cg_mode = mode;
@@ -466,9 +474,38 @@ static bool use_onelaunch(const wd_ctx *c)
 {
     if (!c->coop_ok || c->recon != 18) return false;   // the one-launch kernels are compiled for 18-real links only
     if (c->cg_mode == 1) return false;
-    if (c->cg_mode >= 2) return true;
+    if (c->cg_mode >= 2 && c->cg_mode != 9) return true;
     // automatic: volumes whose CG iteration is shorter than three launches (measured crossovers above)
     return c->V <= (c->precision == 64 ? WD_ONELAUNCH_MAX_SITES_F64 : WD_ONELAUNCH_MAX_SITES_F32);
+}
+
+// Shared-memory-resident CG (wilson_resident.cuh): the lattice is cut into nc slabs of spc consecutive sites, one CTA of a
+// thread-block cluster each.  spc must be a power of two (owner and local index of a neighbour are a shift and a mask), a
+// multiple of 32, at most 256 sites in fp32 / 128 in fp64 (672 / 1344 B of shared memory per site), nc <= 16.
+static bool resident_plan(const wd_ctx *c, int *nc_out, int *spc_out)
+{
+    if (c->recon != 18) return false;
+    const int max_spc = c->precision == 32 ? 256 : 128;
+    for (int nc = 1; nc <= 16; nc *= 2) {
+        if (c->V % nc) continue;
+        const int spc = c->V / nc;
+        if (spc > max_spc || spc % 32 || (spc & (spc - 1))) continue;
+        *nc_out = nc; *spc_out = spc;
+        return true;
+    }
+    return false;
+}
+
+// Automatic only for clusters of one or two CTAs (4^4: 0.143 ms per solve in fp32 against 0.22-0.24 for the one-launch
+// kernels, 0.35 against 0.41 in fp64).  Larger clusters are bound by distributed shared memory: at 8^4 (16 CTAs) every CTA
+// pulls 84 KB of remote spinors and links per stencil pass at the ~17 B/clk a CTA gets from its peers, 10.9 us per iteration
+// against 9.8 for the L2-resident one-launch kernel (measured); wd_set_cg_mode(ctx, 9) still selects them.
+static bool use_resident(const wd_ctx *c)
+{
+    int nc, spc;
+    if (c->cg_mode != 0 && c->cg_mode != 9) return false;
+    if (!resident_plan(c, &nc, &spc)) return false;
+    return c->cg_mode == 9 || nc <= 2;
 }
 
 static bool use_split(const wd_ctx *c)
@@ -498,6 +535,38 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
 {
     int rc = wd_ensure_workspace(c, max_iter);
     if (rc != WD_OK) return rc;
+    if (use_resident(c)) {
+        // the paper's smallest volumes: the whole solve in one launch with every field resident in shared memory
+        ResidentArgs a;
+        for (int d = 0; d < 4; ++d) a.L[d] = c->dims[d];
+        a.bc_t = c->bc_t;
+        resident_plan(c, &a.nc, &a.spc);
+        a.stream = c->stream;
+        a.U = U; a.eta = eta; a.psi = psi; a.kappa = kappa; a.sc = c->sc; a.hist = hist_whole(c, max_iter);
+        a.r_min = r_min; a.max_iter = max_iter;
+        c->last_cg_mode = 9;
+        if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
+        c->launches++;
+        CUDA_TRY(c, c->precision == 32 ? launch_cg_resident_f32(a) : launch_cg_resident_f64(a));
+        if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
+        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        const CgScalars &s1 = *c->sc_host;
+        c->last_iters = s1.k;
+        if (info) {
+            info->iterations = s1.k;
+            info->converged = s1.converged;
+            info->rel_residual = s1.eta2 > 0.0 ? std::sqrt(s1.rr / s1.eta2) : 0.0;
+            info->eta_norm2 = s1.eta2;
+            float ms = 0.f;
+            if (record_events) CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]));
+            info->gpu_ms = ms;
+            info->total_ms = ms;
+            info->kernel_launches = c->launches;
+            info->cg_mode = 9;
+        }
+        return s1.converged ? WD_OK : (s1.breakdown ? WD_BREAKDOWN : WD_NOT_CONVERGED);
+    }
     if (use_onelaunch(c)) {
         c->last_cg_mode = use_split(c) ? 6 : 2;
         if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));

@@ -476,7 +476,7 @@ class WilsonContext:
 
     def wd_set_cg_mode(self, mode):
         """0 automatic, 1 three kernels per iteration, 2 whole solve in one cooperative launch (thread per site), 6 one launch with
-        the hopping sum split over four warps"""
+        the hopping sum split over four warps, 9 one launch with the lattice resident in the shared memory of a cluster"""
         self._check(self.lib.wd_set_cg_mode(self._ctx, int(mode)))
 
     def wd_set_gauge_recon(self, reals_per_link):

@@ -339,7 +339,7 @@ def _cg_case(wilson, oracle, cfg, precision, r_min, poll=None, mode=0):
         hist = ctx.wd_cg_history()
     if mode:
         assert info["cg_mode"] == mode
-        assert info["kernel_launches"] == 1 if mode in (2, 6) else info["kernel_launches"] >= 3 * info["iterations"] + 2
+        assert info["kernel_launches"] == 1 if mode in (2, 6, 9) else info["kernel_launches"] >= 3 * info["iterations"] + 2
     psi_o, info_o = oracle.cg_solve(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t, history=True)
     res_gpu = oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
     res_orc = oracle.true_residual(cfg.dims, U64, eta64, psi_o, cfg.kappa, cfg.bc_t)
@@ -359,24 +359,69 @@ def _cg_case(wilson, oracle, cfg, precision, r_min, poll=None, mode=0):
     return info, info_o, res_gpu, res_orc
 
 
-@pytest.mark.parametrize("mode", [1, 2, 6])
+def _resident_covers(cfg, precision):
+    """mode 9 (lattice resident in the shared memory of a cluster): V / nc a power of two <= 256 (fp32) / 128 (fp64), nc <= 16"""
+    return cfg.index == 0 or (cfg.index == 1 and precision == 32)
+
+
+@pytest.mark.parametrize("mode", [1, 2, 6, 9])
 @pytest.mark.parametrize("cfg_index", [0, 1, 2])
 def test_cg_solve_fp32_baseline_configs(wilson, oracle, cfg_index, mode):
-    """the CG drivers: three kernels per iteration (mode 1) and the two one-launch cooperative kernels (modes 2, 6)"""
+    """the CG drivers: three kernels per iteration (mode 1), the two one-launch cooperative kernels (modes 2, 6) and the
+    shared-memory-resident cluster kernel (mode 9: 4^4 on one CTA, 8^4 on a 16-CTA cluster)"""
     cfg = inputs.CONFIGS[cfg_index]
+    if mode == 9 and not _resident_covers(cfg, 32):
+        with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx, pytest.raises(wilson.WilsonError):
+            ctx.wd_set_cg_mode(9)
+        return
     _cg_case(wilson, oracle, cfg, 32, cfg.r_min, mode=mode)
 
 
-@pytest.mark.parametrize("mode", [1, 2, 6])
+@pytest.mark.parametrize("mode", [1, 2, 6, 9])
 @pytest.mark.parametrize("cfg_index", [0, 1, 2])
 def test_cg_solve_fp64_tight(wilson, oracle, cfg_index, mode):
     cfg = inputs.CONFIGS[cfg_index]
+    if mode == 9 and not _resident_covers(cfg, 64):
+        with wilson.WilsonContext(cfg.dims, 64, cfg.bc_t) as ctx, pytest.raises(wilson.WilsonError):
+            ctx.wd_set_cg_mode(9)
+        return
     _cg_case(wilson, oracle, cfg, 64, 1e-10, mode=mode)
 
 
+@pytest.mark.parametrize("precision", [32, 64])
+@pytest.mark.parametrize("dims,bc_t", [((4, 4, 4, 8), 1), ((8, 4, 4, 4), -1), ((4, 8, 4, 8), -1), ((8, 8, 4, 4), 1), ((4, 4, 8, 16), -1)])
+def test_cg_resident_cluster_sizes(wilson, oracle, dims, bc_t, precision):
+    """mode 9 on anisotropic lattices: clusters of 2, 4, 8 and 16 CTAs (fp32: 512 ... 2048 sites at 256 per CTA; fp64: 128 per
+    CTA), slabs that cut the z and t directions at different places, both boundary conditions; against the oracle and
+    repeatable bit for bit"""
+    V = int(np.prod(dims))
+    if V // (256 if precision == 32 else 128) > 16:
+        with wilson.WilsonContext(dims, precision, bc_t) as ctx, pytest.raises(wilson.WilsonError):
+            ctx.wd_set_cg_mode(9)
+        return
+    cdt = gu.np_complex(precision)
+    tol = 1e-6 if precision == 32 else 1e-10
+    U = inputs.gauge_field(CFG_TEST + 31, dims, "haar", dtype=cdt)
+    eta = inputs.source_field(CFG_TEST + 31, dims, dtype=cdt)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    psi_o, info_o = oracle.cg_solve(dims, U64, eta64, 0.12, tol, 500, bc_t)
+    outs = []
+    with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+        ctx.wd_set_cg_mode(9)
+        for _ in range(2):
+            psi, info = gu.solve_on_gpu(ctx, U, eta, 0.12, tol, 500)
+            outs.append(psi.tobytes())
+        assert info["status"] == 0 and info["cg_mode"] == 9 and info["kernel_launches"] == 1
+    assert outs[0] == outs[1]
+    assert iters_close(info["iterations"], info_o["iterations"])
+    res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), 0.12, bc_t)
+    assert res <= 2.0 * oracle.true_residual(dims, U64, eta64, psi_o, 0.12, bc_t)
+
+
 def test_cg_automatic_mode_by_volume(wilson):
-    """4^4 .. 14^4 (the paper's range) take the one-launch kernel, 32^4 the three-kernel loop"""
-    for ci, precision, want in ((0, 32, 2), (2, 32, 2), (0, 64, 6), (1, 64, 6)):
+    """4^4 takes the shared-memory-resident kernel (one CTA in fp32, a cluster of two in fp64), the rest of the paper's range
+     a one-launch cooperative kernel, 32^4 the three-kernel loop"""
+    for ci, precision, want in ((0, 32, 9), (1, 32, 2), (2, 32, 2), (0, 64, 9), (1, 64, 6)):
         cfg = inputs.CONFIGS[ci]
         U, eta = gu.config_fields(ci, precision)
         with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
@@ -422,6 +467,14 @@ def test_cg_result_independent_of_poll_interval_and_repeatable(wilson):
             psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
             outs.append((psi.tobytes(), info["iterations"], info["rel_residual"]))
     assert all(o == outs[0] for o in outs)
+    for mode9 in (9,):
+        outs = []
+        for _ in range(3):
+            with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
+                ctx.wd_set_cg_mode(mode9)     # 8^4: a 16-CTA cluster, partial sums through distributed shared memory
+                psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
+                outs.append((psi.tobytes(), info["iterations"], info["rel_residual"]))
+        assert all(o == outs[0] for o in outs)
     outs = []
     for _ in range(3):
         with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
@@ -450,7 +503,7 @@ def test_wd_apply_repeat_is_wd_apply(wilson):
             ctx.wd_apply_repeat(Un, en, cfg.kappa, False, reps=3, out=en)
 
 
-@pytest.mark.parametrize("mode", [1, 2, 6])
+@pytest.mark.parametrize("mode", [1, 2, 6, 9])
 def test_cg_edge_cases(wilson, oracle, mode):
     cfg = inputs.CONFIGS[0]
     U, eta = gu.config_fields(0, 64)
