@@ -384,7 +384,9 @@ def main():
                    if ws_bytes > 2 * 126e6 else "working set fits L2 (latency-bound regime, no roofline claim)",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "clocks": m["clocks"], "e2e": e2e, "gpu_launches": m["launches"], "roofline": roofline, "cpu_baseline": cpu,
-        "also": also, "build": wbuild.last_report() if rank == 0 else None,
+        "also": also,
+        "build": ({k: (len(v) if isinstance(v, list) else v) for k, v in wbuild.last_report().items() if k != "flags"}
+                  if rank == 0 else None),
     }
     if rank == 0:
         print(json.dumps(line), flush=True)
