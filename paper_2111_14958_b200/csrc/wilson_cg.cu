@@ -74,9 +74,7 @@ static cudaError_t launch_dslash(wd_ctx *c, const void *U, const void *in, void 
 
 static unsigned int vec_grid(const wd_ctx *c, size_t n)
 {
-    const size_t need = (n + VEC_NT - 1) / VEC_NT;
-    const size_t cap = (size_t)c->sm_count * 16;  // 16 CTAs of 256 threads per SM, grid-stride beyond
-    return (unsigned int)(need < cap ? (need ? need : 1) : cap);
+    return wd_vec_grid(c, n, WD_VEC_PER_SM);
 }
 
 int wd_ensure_workspace(wd_ctx *c, int max_iter)
@@ -606,6 +604,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
 
+    const unsigned int ugrid = wd_vec_grid(c, n, WD_UPD_PER_SM);
     const int poll = c->poll > 0 ? c->poll : auto_poll(c);
     if (c->profile && c->pev_cap < 2 * poll) {   // two chunks of `poll` iterations are in flight at a time
         cudaEvent_t *pe = (cudaEvent_t *)realloc(c->pev, sizeof(cudaEvent_t) * 4 * (size_t)(2 * poll));
@@ -630,9 +629,9 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 2], c->stream));
             // a4: y += alpha p ; p = r + beta p
             if (c->precision == 32)
-                cg_update_kernel<float><<<vgrid, VEC_NT, 0, c->stream>>>((float4 *)c->y, (float4 *)c->p, (const float4 *)c->r, n, c->sc, it);
+                cg_update_kernel<float><<<ugrid, VEC_NT, 0, c->stream>>>((float4 *)c->y, (float4 *)c->p, (const float4 *)c->r, n, c->sc, it);
             else
-                cg_update_kernel<double><<<vgrid, VEC_NT, 0, c->stream>>>((double2 *)c->y, (double2 *)c->p, (const double2 *)c->r, n, c->sc, it);
+                cg_update_kernel<double><<<ugrid, VEC_NT, 0, c->stream>>>((double2 *)c->y, (double2 *)c->p, (const double2 *)c->r, n, c->sc, it);
             c->launches++;
             CUDA_TRY(c, cudaGetLastError());
             if (sample) CUDA_TRY(c, cudaEventRecord(pev[4 * i + 3], c->stream));
@@ -744,7 +743,7 @@ static int bicgstab_loop(wd_ctx *c, const void *U, const void *eta_, void *psi_,
             CUDA_TRY(c, (launch_dslash_bi<MODE_TS>(c, U, s, t, kappa, nullptr, it)));
             if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[3], c->stream));
             // psi += alpha p + omega s ; r = s - omega t ; rho', rr, beta, loop test
-            bi_xr_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(psi, r, p, s, t, eta, n, c->V, padded(c), c->sc, c->partials, c->counter,
+            bi_xr_kernel<real><<<wd_vec_grid(c, n, WD_UPD_PER_SM), VEC_NT, 0, c->stream>>>(psi, r, p, s, t, eta, n, c->V, padded(c), c->sc, c->partials, c->counter,
                                                                hist_at(c, it), it);
             if (c->profile && i == 0) CUDA_TRY(c, cudaEventRecord(c->bev[4], c->stream));
             // p = r + beta (p - omega v)

@@ -7,6 +7,7 @@
 
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 
 #ifndef WD_HOST_SLABS
 #define WD_HOST_SLABS 8   // slabs the host-buffer calls move their fields in (wilson_cg.cu, stage_inputs)
@@ -152,6 +153,23 @@ static inline int wd_poll_loop(wd_ctx *c, int max_iter, int poll, bool ahead, En
         if (c->sc_host->k_stop <= launched) break;  // the device loop condition failed (or eta = 0)
     }
     return WD_OK;
+}
+
+// Grid of a streaming vector kernel over n 128-bit vectors: enough CTAs of VEC_NT threads to cover n, at most `per_sm` per SM
+// (the kernels grid-stride beyond), divided over `parts` grid rows.  How many CTAs per SM stream fastest depends on the number of
+// streams of the kernel (measured on B200 at 48^3x96, round 2): the kernels with five or more streams do best with 1024
+// threads per SM -- cg_update (3 reads, 2 writes) 861 -> 783 us = 6.5 TB/s at 4 instead of 16 CTAs per SM (982 us at 2, 839 at 3,
+// 842 at 5), fp64 163.5 -> 153.3 us at 32^4, the even-odd axpy 428 -> 389 us, bi_xr (5 reads, 2 writes) 1136 -> 1087 us --
+// while the two- and three-stream kernels (bi_s, bi_p, the init kernels, norm2) are already at 6.3-6.7 TB/s with 16 and lose 2-6 %
+// with fewer.  Fewer concurrent streams per SM keep more of each DRAM page's accesses together.
+constexpr int WD_VEC_PER_SM = 16;    // two- and three-stream kernels
+constexpr int WD_UPD_PER_SM = 4;     // cg_update, bi_xr
+static inline unsigned int wd_vec_grid(const wd_ctx *c, size_t n, int per_sm, int parts = 1)
+{
+    const size_t need = (n + wd::VEC_NT - 1) / wd::VEC_NT;
+    size_t cap = (size_t)c->sm_count * per_sm / parts;
+    if (cap < 1) cap = 1;
+    return (unsigned int)(need < cap ? (need ? need : 1) : cap);
 }
 
 // CG workspace of the ctx (r, p, q, y at full length, zeroed once; history of min(max_iter, WD_HIST_MAX) + 1 doubles);

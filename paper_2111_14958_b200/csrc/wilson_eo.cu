@@ -226,8 +226,7 @@ static int eo_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, void *psi_eo
     char *psi_e = (char *)psi_eo, *psi_o = psi_e + hs;
     void *r = c->r, *p = c->p, *q = c->q, *y = c->y, *t = c->w5, *etah = c->w6;
     const double k2 = kappa * kappa;
-    const size_t need = (n + VEC_NT - 1) / VEC_NT, cap = (size_t)c->sm_count * 16;
-    const unsigned int vgrid = (unsigned int)(need < cap ? (need ? need : 1) : cap);
+    const unsigned int vgrid = wd_vec_grid(c, n, WD_VEC_PER_SM), ugrid = wd_vec_grid(c, n, WD_UPD_PER_SM);
 
     // <eta,eta> of the full source (two halves), etahat = eta_e + kappa H_eo eta_o
     norm2_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((const svec *)eta_e, n, e.Vh, pad, c->partials, c->counter, c->eo_n2);
@@ -260,7 +259,7 @@ static int eo_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, void *psi_eo
             CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_RUPD, 0, t, q, nullptr, r, k2, it, true}));
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[4], c->stream));
             // y += alpha p ; p = r + beta p
-            cg_update_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((svec *)y, (svec *)p, (const svec *)r, n, c->sc, it);
+            cg_update_kernel<real><<<ugrid, VEC_NT, 0, c->stream>>>((svec *)y, (svec *)p, (const svec *)r, n, c->sc, it);
             c->launches++;
             CUDA_TRY(c, cudaGetLastError());
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[5], c->stream));
@@ -354,8 +353,7 @@ static int eo_bicgstab_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, voi
     svec *t = (svec *)c->w7;                          // t = Mhat s
     const svec *etah = (const svec *)c->w6;           // etahat = shadow residual rhat
     const double k2 = kappa * kappa;
-    const size_t need = (n + VEC_NT - 1) / VEC_NT, cap = (size_t)c->sm_count * 16;
-    const unsigned int vgrid = (unsigned int)(need < cap ? (need ? need : 1) : cap);
+    const unsigned int vgrid = wd_vec_grid(c, n, WD_VEC_PER_SM), ugrid = wd_vec_grid(c, n, WD_UPD_PER_SM);
 
     norm2_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((const svec *)eta_e, n, e.Vh, pad, c->partials, c->counter, c->eo_n2);
     norm2_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((const svec *)eta_o, n, e.Vh, pad, c->partials, c->counter, c->eo_n2 + 1);
@@ -390,7 +388,7 @@ static int eo_bicgstab_loop(wd_ctx *c, const void *U_eo, const void *eta_eo, voi
             CUDA_TRY(c, eo_launch(c, U_eo, EoPass{0, MODE_TS, 0, to, s, t, nullptr, k2, it, true}));
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[5], c->stream));
             // psi_e += alpha p + omega s ; r = s - omega t ; rho', rr, beta, loop test
-            bi_xr_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((svec *)psi_e, r, p, s, t, etah, n, e.Vh, pad, c->sc, c->partials,
+            bi_xr_kernel<real><<<ugrid, VEC_NT, 0, c->stream>>>((svec *)psi_e, r, p, s, t, etah, n, e.Vh, pad, c->sc, c->partials,
                                                                c->counter, hist_at(c, it), it);
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[6], c->stream));
             // p = r + beta (p - omega v)

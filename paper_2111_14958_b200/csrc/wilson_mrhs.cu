@@ -85,8 +85,7 @@ int cg_group(wd_ctx *c, int g, const void *U, const void *eta, void *psi, double
     using svec = typename Field<real>::svec;
     const size_t n = spinor_vecs(c), stride = n;
     svec *r = (svec *)c->m_ws[0], *p = (svec *)c->m_ws[1], *q = (svec *)c->m_ws[2], *y = (svec *)c->m_ws[3];
-    const size_t need = (n + VEC_NT - 1) / VEC_NT, cap = (size_t)c->sm_count * 16 / g;
-    const dim3 vgrid((unsigned int)(need < cap ? (need ? need : 1) : cap), g);
+    const dim3 vgrid(wd_vec_grid(c, n, WD_VEC_PER_SM, g), g), ugrid(wd_vec_grid(c, n, WD_UPD_PER_SM, g), g);
     const int hs = c->m_hist_cap;
     CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
     cg_init_mrhs_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>((const svec *)eta, y, r, p, n, stride, c->V, padded(c), c->m_sc,
@@ -105,7 +104,7 @@ int cg_group(wd_ctx *c, int g, const void *U, const void *eta, void *psi, double
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[1], c->stream));
             CUDA_TRY(c, mrhs_launch(c, g, 0, MODE_RUPD, U, q, nullptr, r, kappa, c->m_sc, (long)it + 1 < (long)hs ? c->m_hist : nullptr, hs, it));
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[2], c->stream));
-            cg_update_mrhs_kernel<real><<<vgrid, VEC_NT, 0, c->stream>>>(y, p, r, n, stride, c->m_sc, it);
+            cg_update_mrhs_kernel<real><<<ugrid, VEC_NT, 0, c->stream>>>(y, p, r, n, stride, c->m_sc, it);
             c->launches++;
             CUDA_TRY(c, cudaGetLastError());
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[3], c->stream));
