@@ -332,7 +332,12 @@ int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
  *                             thread-block cluster of nc <= 16 CTAs, V / nc sites each (a power of two, <= 256 in fp32, <= 128
  *                             in fp64), neighbours in other CTAs read through distributed shared memory, barrier.cluster
  *                             between the phases; covers 4^4 (one CTA in fp32) and 8^4 in fp32 (16 CTAs); WD_ERR_ARG if the
- *                             lattice does not fit.  Automatic where nc <= 2 (larger clusters are bound by the distributed-shared-
+ *                             lattice does not fit;
+ *                             10 = one cooperative launch with the GAUGE FIELD resident in shared memory (csrc/wilson_ures.cuh): every
+ *                             CTA owns one tile for the whole solve and keeps its links (and the backward links of its faces) in
+ *                             shared memory, the spinors stay in L2 with three hops in flight; needs no more tiles than co-resident
+ *                             CTAs (up to ~57 000 sites in fp32, ~37 000 in fp64), automatic there; per-site arithmetic and hop order of mode 2.
+ *                             Mode 9 is automatic where nc <= 2 (larger clusters are bound by the distributed-shared-
  *                             memory bandwidth and measured slower than mode 2).
  *   wd_set_zchunk(ctx, layers)    z extent (in sites) of one chunk of the CTA rasterisation x,y,z-in-chunk,t,z-chunk that
  *                             keeps the +-t neighbours of a tile in L2; 0 = automatic (fits a 40 MB reuse distance).

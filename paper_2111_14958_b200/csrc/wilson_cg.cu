@@ -4,6 +4,7 @@
 #include "wilson_ctx.cuh"
 #include "wilson_split.cuh"
 #include "wilson_resident.cuh"
+#include "wilson_ures.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -236,9 +237,17 @@ extern "C" int wd_set_tile(wd_ctx *c, int index)
 }
 extern "C" int wd_get_tile(wd_ctx *c) { return c ? c->tile : WD_ERR_ARG; }
 static bool resident_plan(const wd_ctx *c, int *nc_out, int *spc_out);
+static int ures_row_for(const wd_ctx *c);
 extern "C" int wd_set_cg_mode(wd_ctx *c, int mode)
 {
-    if (!c || mode < 0 || (mode > 2 && mode != 6 && mode != 9)) return WD_ERR_ARG;
+    if (!c || mode < 0 || (mode > 2 && mode != 6 && mode != 9 && mode != 10)) return WD_ERR_ARG;
+    if (mode == 10) {
+        const int keep = c->cg_mode;
+        c->cg_mode = 10;
+        const bool ok = c->recon == 18 && ures_row_for(c) >= 0;
+        c->cg_mode = keep;
+        if (!ok) return fail(c, WD_ERR_ARG, "wd_set_cg_mode(10): the lattice has more tiles than CTAs can be co-resident (or 12-real links)");
+    }
     if (mode == 9) {
         int nc, spc;
         if (!resident_plan(c, &nc, &spc))
@@ -472,7 +481,7 @@ static bool use_onelaunch(const wd_ctx *c)
 {
     if (!c->coop_ok || c->recon != 18) return false;   // the one-launch kernels are compiled for 18-real links only
     if (c->cg_mode == 1) return false;
-    if (c->cg_mode >= 2 && c->cg_mode != 9) return true;
+    if (c->cg_mode >= 2 && c->cg_mode != 9 && c->cg_mode != 10) return true;
     // automatic: volumes whose CG iteration is shorter than three launches (measured crossovers above)
     return c->V <= (c->precision == 64 ? WD_ONELAUNCH_MAX_SITES_F64 : WD_ONELAUNCH_MAX_SITES_F32);
 }
@@ -511,8 +520,55 @@ static bool use_split(const wd_ctx *c)
     return c->cg_mode == 6 || (c->cg_mode == 0 && c->precision == 64 && c->V <= WD_SPLIT_MAX_SITES_F64);
 }
 
+// One-launch CG with the gauge field resident in shared memory (wilson_ures.cuh): the row with the fewest padded threads among
+// those compiled for the precision whose tiles all fit one co-resident wave (one tile per CTA for the whole solve); -1 = none.
+static int ures_row_for(const wd_ctx *c)
+{
+    if (!c->coop_ok || c->recon != 18) return -1;
+    int best = -1;
+    double best_waste = 1e300;
+    for (int r = 0; r < WD_NUM_URES_ROWS; ++r) {
+        if (!(c->precision == 64 ? kUresRows[r].f64 : kUresRows[r].f32)) continue;
+        double blocks = 1.0, threads = 1.0;
+        for (int d = 0; d < 4; ++d) {
+            blocks *= (c->dims[d] + kUresRows[r].b[d] - 1) / kUresRows[r].b[d];
+            threads *= kUresRows[r].b[d];
+        }
+        const int occ = c->precision == 64 ? ures_occupancy_f64(r) : ures_occupancy_f32(r);
+        if (occ < 1 || blocks > (double)occ * c->sm_count) continue;
+        const double waste = blocks * threads / (double)c->V;
+        if (waste < best_waste - 1e-12) { best_waste = waste; best = r; }
+    }
+    return best;
+}
+
+static bool use_ures(const wd_ctx *c)
+{
+    if (c->cg_mode != 0 && c->cg_mode != 10) return false;
+    if (ures_row_for(c) < 0) return false;
+    if (c->cg_mode == 10) return true;
+    // automatic: wherever it fits, it beat the L2-resident one-launch kernel (8^4 ... 16^3 x 12, ms per solve, fp32: 0.812 / 0.823,
+    // 10^4 0.934 / 0.987, 12^4 1.141 / 1.231, 14^4 1.653 / 1.836, 16^3x12 1.638 / 1.851; fp64: 10^4 2.485 / 2.833, 12^4 3.226 / 3.745,
+    // 16^2x12^2 4.024 / 4.366) -- except in fp64 up to 4096 sites, where the four-warp split kernel is faster (8^4: 1.591 / 1.894)
+    if (c->precision == 64 && c->V <= 4096) return false;
+    return c->V <= (c->precision == 64 ? WD_ONELAUNCH_MAX_SITES_F64 : WD_ONELAUNCH_MAX_SITES_F32);
+}
+
 static int cg_onelaunch(wd_ctx *c, const void *U, const void *eta, void *psi, double kappa, double r_min, int max_iter)
 {
+    if (use_ures(c)) {
+        const int row = ures_row_for(c);
+        CgOneLaunchArgs a;
+        a.g = make_geom_dims(c, kUresRows[row].b, 0);
+        a.sm_count = c->sm_count;
+        a.stream = c->stream;
+        a.U = U; a.eta = eta; a.y = c->y; a.r = c->r; a.p = c->p; a.q = c->q; a.psi = psi;
+        a.kappa = kappa; a.sc = c->sc; a.partials = c->partials; a.partials_cap = c->partials_cap; a.hist = hist_whole(c, max_iter);
+        a.r_min = r_min; a.max_iter = max_iter;
+        c->launches++;
+        CUDA_TRY(c, c->precision == 32 ? launch_cg_ures_f32(row, a) : launch_cg_ures_f64(row, a));
+        return WD_OK;
+    }
     const bool split = use_split(c);
     const int st = split ? split_tile_for(c) : small_tile_for(c);
     CgOneLaunchArgs a;
@@ -565,8 +621,8 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
         }
         return s1.converged ? WD_OK : (s1.breakdown ? WD_BREAKDOWN : WD_NOT_CONVERGED);
     }
-    if (use_onelaunch(c)) {
-        c->last_cg_mode = use_split(c) ? 6 : 2;
+    if (use_ures(c) || use_onelaunch(c)) {
+        c->last_cg_mode = use_ures(c) ? 10 : (use_split(c) ? 6 : 2);
         if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[0], c->stream));
         rc = cg_onelaunch(c, U, eta, psi, kappa, r_min, max_iter);
         if (rc != WD_OK) return rc;

@@ -476,7 +476,8 @@ class WilsonContext:
 
     def wd_set_cg_mode(self, mode):
         """0 automatic, 1 three kernels per iteration, 2 whole solve in one cooperative launch (thread per site), 6 one launch with
-        the hopping sum split over four warps, 9 one launch with the lattice resident in the shared memory of a cluster"""
+        the hopping sum split over four warps, 9 one launch with the lattice resident in the shared memory of a cluster, 10 one launch with the gauge field resident in
+        shared memory"""
         self._check(self.lib.wd_set_cg_mode(self._ctx, int(mode)))
 
     def wd_set_gauge_recon(self, reals_per_link):

@@ -188,7 +188,7 @@ def test_non_finite_inputs_are_a_breakdown_not_a_convergence(wilson, precision):
     eta_inf[9, 0, 0] = np.inf
     r_min = 1e-6 if precision == 32 else 1e-10
     with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
-        for mode in (1, 2, 6, 9):
+        for mode in (1, 2, 6, 9, 10):
             ctx.wd_set_cg_mode(mode)
             for Ux, ex in ((U_bad, eta), (U, eta_nan), (U, eta_inf)):
                 _, info = gu.solve_on_gpu(ctx, Ux, ex, cfg.kappa, r_min, 200)
@@ -288,7 +288,7 @@ def test_max_iter_int_max_means_no_limit(wilson):
     U, eta = gu.config_fields(0, 32)
     with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
         ref = None
-        for mode in (1, 2, 6, 9):
+        for mode in (1, 2, 6, 9, 10):
             ctx.wd_set_cg_mode(mode)
             psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, 2 ** 31 - 1)
             assert info["status"] == 0 and info["converged"] == 1 and 20 < info["iterations"] < 40

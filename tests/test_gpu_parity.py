@@ -339,7 +339,7 @@ def _cg_case(wilson, oracle, cfg, precision, r_min, poll=None, mode=0):
         hist = ctx.wd_cg_history()
     if mode:
         assert info["cg_mode"] == mode
-        assert info["kernel_launches"] == 1 if mode in (2, 6, 9) else info["kernel_launches"] >= 3 * info["iterations"] + 2
+        assert info["kernel_launches"] == 1 if mode in (2, 6, 9, 10) else info["kernel_launches"] >= 3 * info["iterations"] + 2
     psi_o, info_o = oracle.cg_solve(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t, history=True)
     res_gpu = oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
     res_orc = oracle.true_residual(cfg.dims, U64, eta64, psi_o, cfg.kappa, cfg.bc_t)
@@ -364,7 +364,7 @@ def _resident_covers(cfg, precision):
     return cfg.index == 0 or (cfg.index == 1 and precision == 32)
 
 
-@pytest.mark.parametrize("mode", [1, 2, 6, 9])
+@pytest.mark.parametrize("mode", [1, 2, 6, 9, 10])
 @pytest.mark.parametrize("cfg_index", [0, 1, 2])
 def test_cg_solve_fp32_baseline_configs(wilson, oracle, cfg_index, mode):
     """the CG drivers: three kernels per iteration (mode 1), the two one-launch cooperative kernels (modes 2, 6) and the
@@ -377,13 +377,14 @@ def test_cg_solve_fp32_baseline_configs(wilson, oracle, cfg_index, mode):
     _cg_case(wilson, oracle, cfg, 32, cfg.r_min, mode=mode)
 
 
-@pytest.mark.parametrize("mode", [1, 2, 6, 9])
+@pytest.mark.parametrize("mode", [1, 2, 6, 9, 10])
 @pytest.mark.parametrize("cfg_index", [0, 1, 2])
 def test_cg_solve_fp64_tight(wilson, oracle, cfg_index, mode):
     cfg = inputs.CONFIGS[cfg_index]
-    if mode == 9 and not _resident_covers(cfg, 64):
+    if (mode == 9 and not _resident_covers(cfg, 64)) or (mode == 10 and cfg_index == 2):
+        # (mode 10 in fp64: 14^4 has 686 tiles of 16x2x2x1, more than the 592 CTAs that can be co-resident)
         with wilson.WilsonContext(cfg.dims, 64, cfg.bc_t) as ctx, pytest.raises(wilson.WilsonError):
-            ctx.wd_set_cg_mode(9)
+            ctx.wd_set_cg_mode(mode)
         return
     _cg_case(wilson, oracle, cfg, 64, 1e-10, mode=mode)
 
@@ -420,8 +421,9 @@ def test_cg_resident_cluster_sizes(wilson, oracle, dims, bc_t, precision):
 
 def test_cg_automatic_mode_by_volume(wilson):
     """4^4 takes the shared-memory-resident kernel (one CTA in fp32, a cluster of two in fp64), the rest of the paper's range
-     a one-launch cooperative kernel, 32^4 the three-kernel loop"""
-    for ci, precision, want in ((0, 32, 9), (1, 32, 2), (2, 32, 2), (0, 64, 9), (1, 64, 6)):
+     a one-launch cooperative kernel (gauge field in shared memory: mode 10; fp64 8^4: the split kernel), 32^4
+    the three-kernel loop"""
+    for ci, precision, want in ((0, 32, 9), (1, 32, 10), (2, 32, 10), (0, 64, 9), (1, 64, 6)):
         cfg = inputs.CONFIGS[ci]
         U, eta = gu.config_fields(ci, precision)
         with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
@@ -439,7 +441,7 @@ def test_cg_onelaunch_ragged_lattice(wilson, oracle, precision):
         tol = 1e-6 if precision == 32 else 1e-11
         U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
         psi_o, info_o = oracle.cg_solve(dims, U64, eta64, 0.12, tol, 500, bc_t)
-        for mode in (2, 6):
+        for mode in (2, 6, 10):
             with wilson.WilsonContext(dims, precision, bc_t) as ctx:
                 ctx.wd_set_cg_mode(mode)
                 psi, info = gu.solve_on_gpu(ctx, U, eta, 0.12, tol, 500)
@@ -467,7 +469,7 @@ def test_cg_result_independent_of_poll_interval_and_repeatable(wilson):
             psi, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
             outs.append((psi.tobytes(), info["iterations"], info["rel_residual"]))
     assert all(o == outs[0] for o in outs)
-    for mode9 in (9,):
+    for mode9 in (9, 10):
         outs = []
         for _ in range(3):
             with wilson.WilsonContext(cfg.dims, 32, cfg.bc_t) as ctx:
@@ -503,7 +505,7 @@ def test_wd_apply_repeat_is_wd_apply(wilson):
             ctx.wd_apply_repeat(Un, en, cfg.kappa, False, reps=3, out=en)
 
 
-@pytest.mark.parametrize("mode", [1, 2, 6, 9])
+@pytest.mark.parametrize("mode", [1, 2, 6, 9, 10])
 def test_cg_edge_cases(wilson, oracle, mode):
     cfg = inputs.CONFIGS[0]
     U, eta = gu.config_fields(0, 64)
