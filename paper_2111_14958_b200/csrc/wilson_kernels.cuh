@@ -357,6 +357,118 @@ __device__ __forceinline__ void reconstruct(const real g[12], real sg, real acc[
     }
 }
 
+// ---------------------------------------------------------------- the fp32 hop on packed arithmetic (FFMA2 / FADD2)
+// sm_100 executes fma.rn.f32x2 / add.rn.f32x2: two IEEE fp32 operations on a 64-bit register pair per instruction,
+// with a scalar-broadcast, a swapped-halves and per-half sign form of the operands.  A complex number (re, im) of the
+// spinor layout already IS such a pair (two adjacent 32-bit registers of a 128-bit load), so the complex arithmetic of a
+// hop maps onto it without any data movement:
+//     u h           = u_re (h_re, h_im) + u_im (-h_im, h_re)         u_re, u_im broadcast, the second pair is i h
+//     conj(u) h     = u_re (h_re, h_im) - u_im (i h)
+//     h = p + S i q = (p_re, p_im) + S (-q_im, q_re)                  one FADD2 with a swapped, half-negated operand
+// Per hop: projection 12 FADD2 (h and i h), SU(3) multiply 36 FFMA2, reconstruction 12 FFMA2 -- 60 instructions for the
+// 108 scalar ones, every lane performing exactly the scalar code's operations in the scalar code's order (bit-identical).
+// MEASURED SLOWER and therefore compiled out (WD_F32X2 = 0; -DWD_F32X2=1 builds it, the whole -m gpu suite passed with
+// it): ptxas folds every pack, swap and sign into operand modifiers (FP instructions of the fp32 stencil unit 48 452 ->
+// 28 328, MOVs unchanged), yet at 48^3x96 a2 goes 1.027 -> 1.190 ms and a3 1.084 -> 1.178 ms on the same box, same
+// session, although the SM clock under the power cap rises 1440 -> 1533 MHz.  DESIGN.md section 6.
+#ifndef WD_F32X2
+#define WD_F32X2 0
+#endif
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk2(f32x2 p, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(p)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+// h[sp*3+c] = (re, im) of the half-spinor, ih = i h (the operand of the u_im products)
+template <int MU, int S>
+__device__ __forceinline__ void project_x2(const float v[24], f32x2 h[6], f32x2 ih[6])
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float p0r = v[(0 + c) * 2], p0i = v[(0 + c) * 2 + 1];
+        const float p1r = v[(3 + c) * 2], p1i = v[(3 + c) * 2 + 1];
+        const float p2r = v[(6 + c) * 2], p2i = v[(6 + c) * 2 + 1];
+        const float p3r = v[(9 + c) * 2], p3i = v[(9 + c) * 2 + 1];
+        const f32x2 P0 = pk2(p0r, p0i), P1 = pk2(p1r, p1i), iP0 = pk2(-p0i, p0r), iP1 = pk2(-p1i, p1r);
+        if (MU == 0) {        // h0 = p0 + S i p3 ; h1 = p1 + S i p2
+            h[c] = add2(P0, pk2(-S * p3i, S * p3r));      ih[c] = add2(iP0, pk2(-S * p3r, -S * p3i));
+            h[3 + c] = add2(P1, pk2(-S * p2i, S * p2r));  ih[3 + c] = add2(iP1, pk2(-S * p2r, -S * p2i));
+        } else if (MU == 1) { // h0 = p0 - S p3 ; h1 = p1 + S p2
+            h[c] = add2(P0, pk2(-S * p3r, -S * p3i));     ih[c] = add2(iP0, pk2(S * p3i, -S * p3r));
+            h[3 + c] = add2(P1, pk2(S * p2r, S * p2i));   ih[3 + c] = add2(iP1, pk2(-S * p2i, S * p2r));
+        } else if (MU == 2) { // h0 = p0 + S i p2 ; h1 = p1 - S i p3
+            h[c] = add2(P0, pk2(-S * p2i, S * p2r));      ih[c] = add2(iP0, pk2(-S * p2r, -S * p2i));
+            h[3 + c] = add2(P1, pk2(S * p3i, -S * p3r));  ih[3 + c] = add2(iP1, pk2(S * p3r, S * p3i));
+        } else {              // h0 = p0 + S p2 ; h1 = p1 + S p3
+            h[c] = add2(P0, pk2(S * p2r, S * p2i));       ih[c] = add2(iP0, pk2(-S * p2i, S * p2r));
+            h[3 + c] = add2(P1, pk2(S * p3r, S * p3i));   ih[3 + c] = add2(iP1, pk2(-S * p3i, S * p3r));
+        }
+    }
+}
+template <bool ADJ>
+__device__ __forceinline__ void mul_su3_x2(const float u[18], const f32x2 h[6], const f32x2 ih[6], f32x2 g[6])
+{
+#pragma unroll
+    for (int sp = 0; sp < 2; ++sp)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            f32x2 acc = pk2(0.f, 0.f);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const float ur = ADJ ? u[(c * 3 + a) * 2] : u[(a * 3 + c) * 2];
+                const float ui = ADJ ? -u[(c * 3 + a) * 2 + 1] : u[(a * 3 + c) * 2 + 1];
+                acc = fma2(pk2(ur, ur), h[sp * 3 + c], acc);
+                acc = fma2(pk2(ui, ui), ih[sp * 3 + c], acc);
+            }
+            g[sp * 3 + a] = acc;
+        }
+}
+template <int MU, int S>
+__device__ __forceinline__ void reconstruct_x2(const f32x2 g[6], float sg, float acc[24])
+{
+    const float c = sg * S;
+    const f32x2 sg2 = pk2(sg, sg), cpp = pk2(c, c), cpn = pk2(c, -c), cnp = pk2(-c, c), cnn = pk2(-c, -c);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        float g0r, g0i, g1r, g1i;
+        upk2(g[a], g0r, g0i);
+        upk2(g[3 + a], g1r, g1i);
+        const f32x2 G0 = g[a], G1 = g[3 + a], G0s = pk2(g0i, g0r), G1s = pk2(g1i, g1r);
+        f32x2 A0 = pk2(acc[(0 + a) * 2], acc[(0 + a) * 2 + 1]), A1 = pk2(acc[(3 + a) * 2], acc[(3 + a) * 2 + 1]);
+        f32x2 A2 = pk2(acc[(6 + a) * 2], acc[(6 + a) * 2 + 1]), A3 = pk2(acc[(9 + a) * 2], acc[(9 + a) * 2 + 1]);
+        A0 = fma2(sg2, G0, A0);
+        A1 = fma2(sg2, G1, A1);
+        if (MU == 0) {        // row2 += -S i g1 ; row3 += -S i g0
+            A2 = fma2(cpn, G1s, A2);  A3 = fma2(cpn, G0s, A3);
+        } else if (MU == 1) { // row2 += S g1 ; row3 += -S g0
+            A2 = fma2(cpp, G1, A2);   A3 = fma2(cnn, G0, A3);
+        } else if (MU == 2) { // row2 += -S i g0 ; row3 += S i g1
+            A2 = fma2(cpn, G0s, A2);  A3 = fma2(cnp, G1s, A3);
+        } else {              // row2 += S g0 ; row3 += S g1
+            A2 = fma2(cpp, G0, A2);   A3 = fma2(cpp, G1, A3);
+        }
+        upk2(A0, acc[(0 + a) * 2], acc[(0 + a) * 2 + 1]);
+        upk2(A1, acc[(3 + a) * 2], acc[(3 + a) * 2 + 1]);
+        upk2(A2, acc[(6 + a) * 2], acc[(6 + a) * 2 + 1]);
+        upk2(A3, acc[(9 + a) * 2], acc[(9 + a) * 2 + 1]);
+    }
+}
+
 // One hop, split into its loads and its arithmetic so that the loads of the next hop can be in flight
 // while this one is computed:  acc += sg (1 + S gamma_MU) (x) [U or U^dagger](link_site) in(spinor_site).
 // RO = true: `in` is not written while the kernel runs -> read-only (non-coherent) path; false: coherent loads
@@ -391,10 +503,17 @@ __device__ __forceinline__ void hop_load(const gvec *__restrict__ U, const svec 
 template <int MU, int S, bool ADJ, typename real>
 __device__ __forceinline__ void hop_compute(const real v[24], const real u[18], real sg, real acc[24])
 {
-    real h[12], g[12];
-    project<MU, S, real>(v, h);
-    mul_su3<ADJ, real>(u, h, g);
-    reconstruct<MU, S, real>(g, sg, acc);
+    if constexpr (WD_F32X2 && sizeof(real) == 4) {
+        f32x2 h[6], ih[6], g[6];
+        project_x2<MU, S>(v, h, ih);
+        mul_su3_x2<ADJ>(u, h, ih, g);
+        reconstruct_x2<MU, S>(g, sg, acc);
+    } else {
+        real h[12], g[12];
+        project<MU, S, real>(v, h);
+        mul_su3<ADJ, real>(u, h, g);
+        reconstruct<MU, S, real>(g, sg, acc);
+    }
 }
 
 // Neighbour sites and boundary signs of site s = (x,y,z,t).

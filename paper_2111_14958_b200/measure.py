@@ -147,6 +147,7 @@ def run_rows(args):
                 b2, b3, b4 = 2 * sb + gb, 3 * sb + gb, 5 * sb
                 a2, a3, a4 = p["a2_ms"] / n, p["a3_ms"] / n, p["a4_ms"] / n
                 t = float(np.median(ms))
+                gbs = lambda b, msec: b * V / (msec * 1e-3) / 1e9 if msec > 0 else None
                 print(json.dumps({
                     "row": "f3 link storage", "config": ci, "precision": prec, "reals_per_link": recon,
                     "bytes_per_site": {"wd_apply": b2, "a2": b2, "a3": b3, "a4": b4, "cg_iteration": b2 + b3 + b4},
@@ -154,9 +155,10 @@ def run_rows(args):
                     "cg_iterations": info["iterations"], "cg_solve_ms": t,
                     "cg_gflops": cg_flops(V, info["iterations"]) / (t * 1e-3) / 1e9,
                     "a2_us": a2 * 1e3, "a3_us": a3 * 1e3, "a4_us": a4 * 1e3,
-                    "a2_gbs": b2 * V / (a2 * 1e-3) / 1e9, "a3_gbs": b3 * V / (a3 * 1e-3) / 1e9,
-                    "cg_iteration_gbs": (b2 + b3 + b4) * V / ((a2 + a3 + a4) * 1e-3) / 1e9,
-                    "cg_iteration_frac_of_measured": (b2 + b3 + b4) * V / ((a2 + a3 + a4) * 1e-3) / 1e9 / peak}), flush=True)
+                    # one-launch solves (small volumes) have no per-kernel times: the rates are then null
+                    "a2_gbs": gbs(b2, a2), "a3_gbs": gbs(b3, a3),
+                    "cg_iteration_gbs": gbs(b2 + b3 + b4, a2 + a3 + a4),
+                    "cg_iteration_frac_of_measured": (gbs(b2 + b3 + b4, a2 + a3 + a4) or 0.0) / peak or None}), flush=True)
                 if recon == 18:
                     for _ in range(2):
                         ctx.bicgstab_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=out)
