@@ -315,6 +315,35 @@ int wd_cg_history(wd_ctx *ctx, double *out, int n);
 int wd_norm2(wd_ctx *ctx, const void *a_native, double *result);
 
 /*
+ * wd_norm2_noalloc — the same <a,a> for callers that cannot call cudaMalloc: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid allocation.  Needs NO context and allocates nothing, on the host
+ * or on the device: the scratch of the grid reduction (one fp64 partial per 4096 128-bit vectors of the field, and the
+ * ticket counter) lives in a file-scope __device__ array of 128.25 KB that every GPU loading the library holds until
+ * the process exits.  The call enqueues a 256-byte memset (the ticket counter must start at zero) and one kernel on
+ * `cuda_stream` and returns; it does not synchronise.
+ *   precision     32 or 64.
+ *   n_sites       V, the number of lattice sites of the field (native layout: Vpad = V rounded up to 16).
+ *   a_native      DEVICE pointer, native spinor layout, 24 * Vpad reals; read only.
+ *   result_dev    DEVICE pointer to one double, owned by the caller; written by the kernel in stream order.
+ *   cuda_stream   a cudaStream_t (as void*) of the CURRENT device, or NULL for the legacy default stream.  The current
+ *                 device must be the one that owns the stream and the buffers.
+ * Limit: n_sites <= wd_noalloc_max_sites(precision) = 11 184 800 (fp32) / 5 592 400 (fp64) — 16384 partials; 48^3x96
+ * in fp32 and 32^4 in both precisions fit.  Larger fields are rejected with WD_ERR_DIMS (use wd_norm2).
+ * Result: fp64 accumulation in an order fixed by n_sites alone (bit-identical from call to call and from GPU to GPU);
+ * it differs from wd_norm2's, whose grouping follows the SM count, by fp64 rounding only.
+ * SHARED STATE: every call on a device uses the one static array.  Calls that overlap on the GPU (two streams, or two
+ * host threads without ordering between their streams) race on it and give wrong sums: serialise them per device.
+ * Errors: WD_ERR_PRECISION, WD_ERR_ARG (NULL pointer), WD_ERR_DIMS (n_sites 0 or beyond the limit), WD_ERR_CUDA;
+ * wd_noalloc_last_error() returns the message of the calling thread's last failed call ("" after a success).
+ * wd_noalloc_prepare() does the one-time set-up for the current device (cudaGetSymbolAddress of the static array) so
+ * that a caller can have it done before a stream capture begins; wd_norm2_noalloc does it itself if it was not.
+ */
+int wd_norm2_noalloc(int precision, size_t n_sites, const void *a_native, double *result_dev, void *cuda_stream);
+size_t wd_noalloc_max_sites(int precision);   /* 0 for a precision other than 32 / 64; needs no GPU */
+int wd_noalloc_prepare(void);
+const char *wd_noalloc_last_error(void);
+
+/*
  * Tuning knobs (the paper's workgroup-size tuning):
  *   wd_num_tiles()            number of compiled stencil launch configurations ("tiles").
  *   wd_tile_shape(i, shape)   writes {BX,BY,BZ,BT} of tile i (threads per CTA = product); returns 0 or WD_ERR_ARG.

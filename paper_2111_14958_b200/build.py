@@ -32,7 +32,8 @@ UNITS = ["wilson_cg.cu", "wilson_dslash_f32.cu", "wilson_dslash_f64.cu", "wilson
          "wilson_bicg_eo_f32.cu", "wilson_bicg_eo_f64.cu", "wilson_split_f32.cu", "wilson_split_f64.cu",
          "wilson_dslash12_eo_f32.cu", "wilson_dslash12_eo_f64.cu",
          "wilson_eo_onelaunch_f32.cu", "wilson_eo_onelaunch_f64.cu", "wilson_tma_f32.cu", "wilson_tma_f64.cu",
-         "wilson_resident_f32.cu", "wilson_resident_f64.cu", "wilson_ures_f32.cu", "wilson_ures_f64.cu"]
+         "wilson_resident_f32.cu", "wilson_resident_f64.cu", "wilson_ures_f32.cu", "wilson_ures_f64.cu",
+         "wilson_noalloc.cu"]
 
 ARCH_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a"]
 # --compress-mode=size: the SASS of the ~500 template instantiations compresses about tenfold (the library went from

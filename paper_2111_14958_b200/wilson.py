@@ -102,6 +102,12 @@ def load_library(path: str = LIB_PATH):
     lib.cg_solve_host.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
     lib.wd_cg_history.argtypes = [vp, dp, ci]
     lib.wd_norm2.argtypes = [vp, vp, dp]
+    lib.wd_norm2_noalloc.argtypes = [ci, ctypes.c_size_t, vp, vp, vp]
+    lib.wd_noalloc_max_sites.argtypes = [ci]
+    lib.wd_noalloc_max_sites.restype = ctypes.c_size_t
+    lib.wd_noalloc_prepare.argtypes = []
+    lib.wd_noalloc_last_error.argtypes = []
+    lib.wd_noalloc_last_error.restype = ctypes.c_char_p
     lib.wd_num_tiles.argtypes = []
     lib.wd_tile_shape.argtypes = [ci, ip]
     lib.wd_tile_info.argtypes = [ci, ip]
@@ -165,6 +171,35 @@ def _torch():
     import torch
 
     return torch
+
+
+def wd_noalloc_max_sites(precision: int) -> int:
+    """Largest number of sites wd_norm2_noalloc accepts (its scratch is a static device array); needs no GPU."""
+    return int(load_library().wd_noalloc_max_sites(int(precision)))
+
+
+def wd_noalloc_prepare() -> None:
+    """One-time set-up of wd_norm2_noalloc for the current device (e.g. before a stream capture begins)."""
+    lib = load_library()
+    rc = lib.wd_noalloc_prepare()
+    if rc != 0:
+        raise WilsonError(rc, lib.wd_noalloc_last_error().decode())
+
+
+def wd_norm2_noalloc(a_native, n_sites: int, precision: int, out, stream=None) -> None:
+    """<a,a> of a native spinor field without a context and without any allocation inside the library: enqueues the work on
+    `stream` (a torch.cuda.Stream; None = the legacy default stream) and returns.  `out` is a CUDA float64 tensor of one
+    element owned by the caller; read it after synchronising the stream.  Calls that overlap on the GPU race on the
+    library's static scratch (include/wilson_cg.h)."""
+    torch = _torch()
+    lib = load_library()
+    if not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64 and out.numel() >= 1):
+        raise ValueError("out must be a CUDA float64 tensor with one element")
+    sp = ctypes.c_void_p(stream.cuda_stream) if stream is not None else None
+    rc = lib.wd_norm2_noalloc(int(precision), int(n_sites), ctypes.c_void_p(a_native.data_ptr()),
+                              ctypes.c_void_p(out.data_ptr()), sp)
+    if rc != 0:
+        raise WilsonError(rc, lib.wd_noalloc_last_error().decode())
 
 
 class WilsonContext:
