@@ -298,3 +298,57 @@ def test_max_iter_int_max_means_no_limit(wilson):
         en = ctx.wd_pack_spinor(gu.to_device(eta))
         _, ib = ctx.bicgstab_solve(Un, en, cfg.kappa, cfg.r_min, 2 ** 31 - 1)
         assert ib["status"] == 0
+
+
+def test_contexts_on_their_own_streams_run_concurrently(wilson):
+    """include/wilson_cg.h: "use one ctx per host thread / stream".  Two host threads, each with its own context on its own
+    stream, solve at the same time (ctypes releases the GIL during a call): every driver of cg_solve and BiCGSTAB, each
+    with the per-context scratch of its reductions and the process-wide occupancy tables.  Every result must be
+    bit-identical to the same solve run alone (the reductions are deterministic)."""
+    import threading
+
+    import torch
+
+    jobs = [(0, 32, 1), (1, 32, 2), (0, 64, 6), (0, 32, 9), (2, 32, 10), (1, 32, 1), (2, 32, 0), (1, 64, 0)]
+    prepared = []
+    for ci, precision, mode in jobs:
+        cfg = inputs.CONFIGS[ci]
+        U, eta = gu.config_fields(ci, precision)
+        r_min = cfg.r_min if precision == 32 else 1e-10
+        stream = torch.cuda.Stream()
+        with torch.cuda.stream(stream):
+            ctx = wilson.WilsonContext(cfg.dims, precision, cfg.bc_t, stream=stream)
+            ctx.wd_set_cg_mode(mode)
+            Un = ctx.wd_pack_gauge(gu.to_device(U))
+            en = ctx.wd_pack_spinor(gu.to_device(eta))
+            out, outb = ctx.empty_spinor(), ctx.empty_spinor()
+            _, info = ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=out)
+            _, infob = ctx.bicgstab_solve(Un, en, cfg.kappa, r_min, cfg.max_iter, out=outb)
+            stream.synchronize()
+            prepared.append((ctx, stream, cfg, r_min, Un, en, out.clone(), info, outb.clone(), infob))
+    torch.cuda.synchronize()
+    errors = []
+
+    def worker(items, rounds):
+        try:
+            for _ in range(rounds):
+                for ctx, stream, cfg, r_min, Un, en, want, info, wantb, infob in items:
+                    with torch.cuda.stream(stream):
+                        got, gi = ctx.cg_solve(Un, en, cfg.kappa, r_min, cfg.max_iter)
+                        gotb, gib = ctx.bicgstab_solve(Un, en, cfg.kappa, r_min, cfg.max_iter)
+                        stream.synchronize()
+                        if gi["iterations"] != info["iterations"] or gi["cg_mode"] != info["cg_mode"] or not torch.equal(got, want):
+                            errors.append(("cg", cfg.index, ctx.precision, gi, info))
+                        if gib["iterations"] != infob["iterations"] or not torch.equal(gotb, wantb):
+                            errors.append(("bicgstab", cfg.index, ctx.precision, gib, infob))
+        except Exception as e:  # noqa: BLE001 - reported by the main thread
+            errors.append(("exception", repr(e)))
+
+    threads = [threading.Thread(target=worker, args=(prepared[k::2], 6)) for k in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    for p in prepared:
+        p[0].close()
+    assert not errors, errors[:3]
