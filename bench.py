@@ -13,8 +13,10 @@ kernel.  Inputs are seeded and synthetic (paper_2111_14958_b200/inputs.py); they
 unspecified gauge fields.
 
 `value`   : device-resident inputs (native layout already in HBM), CUDA events around K steps.
-`e2e`     : the same solve through the C-ABI host-buffer call cg_solve_host (pinned HOST canonical
-            buffers; H2D copies of U and eta, pack, solve, unpack and the D2H copy of psi inside the timed region).
+`e2e`     : the same solves through the C-ABI host-buffer calls (pinned HOST canonical buffers; per step the H2D copies
+            of U and eta, pack, solve, unpack and the D2H copy of psi, all inside the timed region).  `value` = the K
+            steps as a queue pipelined over two contexts (cg_solve_host_begin / _run / _wait: the transfers of one step
+            overlap the iterations of its neighbours); `one_call_at_a_time` = the same K steps as K cg_solve_host calls.
 `roofline`: the dominant kernel (a3: D pass + fused r update + |r|^2, 576 B/site fp32) timed live with CUDA
             events around its launches (every 4th iteration) inside the timed steps (wd_set_profile);
             `roofline.kernels` lists a2, a3, a4 the same way and `roofline.cg_iteration` the fused iteration
@@ -350,7 +352,48 @@ def main():
                "device_solve_ms_inside": info_h["gpu_ms"], "transfer_ms": dt * 1e3 - info_h["gpu_ms"],
                "effective_pcie_gbs": (h2d + d2h) / max(dt - info_h["gpu_ms"] * 1e-3, 1e-9) / 1e9,
                "plain_pinned_copy_ms_same_bytes": plain_copy_ms, "plain_pinned_copy_gbs": (h2d + d2h) / plain_copy_ms / 1e6}
-        del U_pin, eta_pin, psi_pin
+        # The same K solves as a QUEUE: two contexts on two streams, split-phase calls (cg_solve_host_begin / _run / _wait).
+        # Every step still uploads its own U and eta from pinned memory and downloads its own psi inside the timed region;
+        # the uploads of step i+1 and the download of step i-1 run while the GPU iterates on step i.  Pipeline fill (the
+        # first upload) and drain (the last download) are inside the timed region too.
+        psi_pin2 = torch.empty_like(psi_pin).pin_memory()
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        pctx = [wilson.WilsonContext(cfg.dims, args.precision, cfg.bc_t, stream=st) for st in streams]
+        for pc in pctx:
+            if args.tile is not None:
+                pc.wd_set_tile(args.tile)
+        outs = [psi_pin, psi_pin2]
+
+        def pipelined(nsteps):
+            pctx[0].cg_solve_host_begin(U_pin, eta_pin)
+            inf = None
+            for i in range(nsteps):
+                if i + 1 < nsteps:
+                    pctx[(i + 1) % 2].cg_solve_host_begin(U_pin, eta_pin)
+                inf = pctx[i % 2].cg_solve_host_run(cfg.kappa, r_min, cfg.max_iter, outs[i % 2])
+                if i > 0:
+                    pctx[(i - 1) % 2].cg_solve_host_wait()
+            pctx[(nsteps - 1) % 2].cg_solve_host_wait()
+            return inf
+
+        pipelined(2)                                    # warm-up: staging buffers of both contexts
+        barrier()
+        t0 = time.perf_counter()
+        info_p = pipelined(args.steps)
+        barrier()
+        dtp = max_over_ranks((time.perf_counter() - t0) / args.steps, dist, "cuda")
+        same = bool(torch.equal(psi_pin, psi_pin2)) if args.steps > 1 else None
+        for pc in pctx:
+            pc.close()
+        serial = {k: e2e[k] for k in ("value", "ms_per_step", "device_solve_ms_inside", "transfer_ms", "effective_pcie_gbs")}
+        e2e.update({"value": whole_job_value(world, V, info_p["iterations"], dtp), "ms_per_step": dtp * 1e3,
+                    "mode": "queue of K solves pipelined over 2 contexts / streams (cg_solve_host_begin, _run, _wait): every "
+                            "step copies its own inputs H2D and its result D2H inside the timed region, overlapped with the "
+                            "neighbouring steps' iterations; fill and drain included",
+                    "device_solve_ms_inside": info_p["gpu_ms"], "outputs_identical": same,
+                    "one_call_at_a_time": serial})
+        del e2e["transfer_ms"], e2e["effective_pcie_gbs"]
+        del U_pin, eta_pin, psi_pin, psi_pin2
     ctx.close()
     torch.cuda.empty_cache()
 

@@ -301,6 +301,34 @@ int cg_solve_host(wd_ctx *ctx, const void *U_host, const void *eta_host, void *p
                   double kappa, double r_min, int max_iter, wd_cg_info *info);
 
 /*
+ * Split-phase form of cg_solve_host, for callers with a queue of systems to solve (PAPER.md:44-48 is one solve; a
+ * production run is thousands of them).  A solve needs all of U and eta before its first iteration, so inside ONE solve
+ * the PCIe transfers cannot hide; with TWO contexts (two streams) the uploads of solve i+1 and the download of solve i-1
+ * run while the GPU iterates on solve i:
+ *
+ *     cg_solve_host_begin(ctx[0], U_0, eta_0);
+ *     for i = 0 .. n-1:   if (i+1 < n) cg_solve_host_begin(ctx[(i+1)%2], U_{i+1}, eta_{i+1});   // enqueues, returns
+ *                         cg_solve_host_run(ctx[i%2], psi_i, kappa, r_min, max_iter, &info);   // the solve (host polls)
+ *                         if (i > 0) cg_solve_host_wait(ctx[(i-1)%2]);                          // psi_{i-1} is complete
+ *     cg_solve_host_wait(ctx[(n-1)%2]);
+ *
+ *   cg_solve_host_begin   enqueues the copies of U_host (NULL = the gauge field of the previous *_host call on this ctx) and
+ *                         eta_host to the device and the pack kernels, slab by slab, and returns without waiting.  The host
+ *                         buffers must be pinned for the copies to overlap anything, and must stay untouched until
+ *                         cg_solve_host_run on the same ctx has returned.  Device-ordered behind a download of this ctx that is
+ *                         still in flight.  WD_ERR_ARG if inputs are already staged.
+ *   cg_solve_host_run     cg_solve on the staged fields (same recurrence, same result as cg_solve_host, bit for bit), then
+ *                         enqueues the unpack kernels and the copy to psi_host_out and returns WITHOUT waiting for that copy.
+ *                         Return value and *info as cg_solve (info->total_ms = info->gpu_ms: there is no per-call total when
+ *                         transfers overlap other solves; kernel_launches counts begin + run).  WD_ERR_ARG if nothing is staged.
+ *   cg_solve_host_wait    returns when psi_host_out of the last run on this ctx is complete (no-op if nothing is pending).
+ * cg_solve_host(ctx, ...) is begin + run + wait on one ctx.  A ctx is still single-threaded: one host thread drives both.
+ */
+int cg_solve_host_begin(wd_ctx *ctx, const void *U_host, const void *eta_host);
+int cg_solve_host_run(wd_ctx *ctx, void *psi_host_out, double kappa, double r_min, int max_iter, wd_cg_info *info);
+int cg_solve_host_wait(wd_ctx *ctx);
+
+/*
  * wd_cg_history — rr = <r,r> after 0, 1, ..., k iterations of the last cg_solve / cg_solve_host on this
  * ctx (the device-side record of the recursed residual; used to compare convergence with the oracle).
  *   out: host pointer to n doubles.  Returns the number of values written (<= k+1), or < 0 on error.

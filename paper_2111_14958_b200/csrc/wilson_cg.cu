@@ -981,7 +981,7 @@ static int stage_inputs(wd_ctx *c, const void *U_host, const void *s_host)
 }
 
 template <typename real>
-static int return_output_t(wd_ctx *c, void *out_host)
+static int return_output_t(wd_ctx *c, void *out_host, bool sync)
 {
     using svec = typename Field<real>::svec;
     const size_t site_bytes = 24 * sizeof(real);
@@ -1004,13 +1004,13 @@ static int return_output_t(wd_ctx *c, void *out_host)
     CUDA_TRY(c, cudaEventRecord(c->slab_ev[WD_HOST_SLABS], c->copy_stream));
     CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->slab_ev[WD_HOST_SLABS], 0));
     CUDA_TRY(c, cudaEventRecord(c->ev[3], c->stream));
-    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    if (sync) CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return WD_OK;
 }
 
-static int return_output(wd_ctx *c, void *out_host)
+static int return_output(wd_ctx *c, void *out_host, bool sync = true)
 {
-    return c->precision == 32 ? return_output_t<float>(c, out_host) : return_output_t<double>(c, out_host);
+    return c->precision == 32 ? return_output_t<float>(c, out_host, sync) : return_output_t<double>(c, out_host, sync);
 }
 
 extern "C" int wd_apply_host(wd_ctx *c, const void *U_host, const void *psi_host, void *out_host, double kappa, int dagger)
@@ -1048,4 +1048,51 @@ extern "C" int cg_solve_host(wd_ctx *c, const void *U_host, const void *eta_host
         info->kernel_launches = c->launches;
     }
     return status;
+}
+
+// Split-phase form of cg_solve_host (include/wilson_cg.h): begin = enqueue the uploads, run = the solve and the enqueue of the
+// download, wait = the download has landed.  With two contexts a caller overlaps the transfers of one solve with the
+// iterations of another; every piece is the code of cg_solve_host.
+extern "C" int cg_solve_host_begin(wd_ctx *c, const void *U_host, const void *eta_host)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!U_host && !c->have_gauge) return fail(c, WD_ERR_ARG, "cg_solve_host_begin: NULL gauge field and none cached");
+    if (!eta_host) return fail(c, WD_ERR_ARG, "cg_solve_host_begin: NULL source");
+    if (c->host_staged) return fail(c, WD_ERR_ARG, "cg_solve_host_begin: inputs are already staged (call cg_solve_host_run)");
+    c->launches = 0;
+    // device-ordered behind a download that may still be in flight (same streams): no host wait here
+    const int rc = stage_inputs(c, U_host, eta_host);
+    if (rc != WD_OK) return rc;
+    c->host_staged = 1;
+    return WD_OK;
+}
+
+extern "C" int cg_solve_host_run(wd_ctx *c, void *psi_host, double kappa, double r_min, int max_iter, wd_cg_info *info)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!c->host_staged) return fail(c, WD_ERR_ARG, "cg_solve_host_run: no inputs staged (call cg_solve_host_begin)");
+    if (!psi_host) return fail(c, WD_ERR_ARG, "cg_solve_host_run: NULL output");
+    if (!std::isfinite(kappa)) return fail(c, WD_ERR_ARG, "cg_solve_host_run: kappa is not finite");
+    if (!(r_min > 0.0) || !std::isfinite(r_min)) return fail(c, WD_ERR_ARG, "cg_solve_host_run: r_min must be > 0");
+    if (max_iter < 0) return fail(c, WD_ERR_ARG, "cg_solve_host_run: max_iter < 0");
+    const int status = cg_device(c, c->U_nat, c->s_nat_in, c->s_nat_out, kappa, r_min, max_iter, info, true);
+    c->host_staged = 0;   // consumed, also by a failed solve: the caller starts again from begin
+    if (status < 0) return status;
+    const int rc = return_output(c, psi_host, false);
+    if (rc != WD_OK) return rc;
+    c->host_out_pending = 1;
+    if (info) {
+        info->total_ms = info->gpu_ms;   // the transfers of a split-phase solve overlap other work: no per-call total
+        info->kernel_launches = c->launches;   // pack kernels of begin + the solve + the unpack kernels
+    }
+    return status;
+}
+
+extern "C" int cg_solve_host_wait(wd_ctx *c)
+{
+    if (!c) return WD_ERR_ARG;
+    if (!c->host_out_pending) return WD_OK;
+    c->host_out_pending = 0;
+    CUDA_TRY(c, cudaEventSynchronize(c->ev[3]));
+    return WD_OK;
 }

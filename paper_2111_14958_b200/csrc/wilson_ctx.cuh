@@ -60,6 +60,8 @@ struct wd_ctx {
     // staging of the *_host calls
     void *U_can, *U_nat, *s_can, *s_nat_in, *s_nat_out;
     int have_gauge;
+    int host_staged;        // cg_solve_host_begin has staged inputs that no run has consumed yet
+    int host_out_pending;   // cg_solve_host_run has enqueued the copy of psi to the host; cg_solve_host_wait has not been called
     cudaStream_t copy_stream;   // the *_host calls: transfers run here, slab by slab, beside the pack / unpack kernels
     cudaEvent_t slab_ev[WD_HOST_SLABS + 1];
     cudaEvent_t ev[4];

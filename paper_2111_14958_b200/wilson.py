@@ -100,6 +100,9 @@ def load_library(path: str = LIB_PATH):
     lib.wd_apply_host.argtypes = [vp, vp, vp, vp, cd, ci]
     lib.wd_apply_repeat.argtypes = [vp, vp, vp, vp, cd, ci, ci, dp]
     lib.cg_solve_host.argtypes = [vp, vp, vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
+    lib.cg_solve_host_begin.argtypes = [vp, vp, vp]
+    lib.cg_solve_host_run.argtypes = [vp, vp, cd, cd, ci, ctypes.POINTER(WdCgInfo)]
+    lib.cg_solve_host_wait.argtypes = [vp]
     lib.wd_cg_history.argtypes = [vp, dp, ci]
     lib.wd_norm2.argtypes = [vp, vp, dp]
     lib.wd_norm2_noalloc.argtypes = [ci, ctypes.c_size_t, vp, vp, vp]
@@ -490,6 +493,27 @@ class WilsonContext:
         d = info.as_dict()
         d["status"] = rc
         return out, d
+
+    # -- split-phase form: with two contexts the transfers of one solve overlap the iterations of another
+    def cg_solve_host_begin(self, U_host, eta_host):
+        """enqueue the uploads of U_host (None = the gauge field already on this ctx) and eta_host; returns at once.  The
+        buffers (pinned, canonical layout) must stay untouched until cg_solve_host_run on this ctx has returned."""
+        V = self.volume
+        up = self._host_ptr(U_host, (V, 4, 3, 3)) if U_host is not None else None
+        self._check(self.lib.cg_solve_host_begin(self._ctx, up, self._host_ptr(eta_host, (V, 4, 3))))
+
+    def cg_solve_host_run(self, kappa, r_min, max_iter, out):
+        """the solve on the staged fields; enqueues the download into `out` (complete after cg_solve_host_wait)"""
+        info = WdCgInfo()
+        rc = self.lib.cg_solve_host_run(self._ctx, self._host_ptr(out, (self.volume, 4, 3), True), float(kappa),
+                                        float(r_min), int(max_iter), ctypes.byref(info))
+        self._check(rc, allow_not_converged=True)
+        d = info.as_dict()
+        d["status"] = rc
+        return d
+
+    def cg_solve_host_wait(self):
+        self._check(self.lib.cg_solve_host_wait(self._ctx))
 
     # -- tuning knobs
     def wd_set_tile(self, index):

@@ -33,6 +33,9 @@ def test_bench_line_small_workload():
     e = d["e2e"]
     assert e["value"] > 0 and e["value"] < 1.5 * d["value"] and e["steps"] == d["steps"]
     assert e["h2d_bytes_per_step"] == 4096 * (72 + 24) * 4 and e["d2h_bytes_per_step"] == 4096 * 24 * 4
+    # value = the K steps pipelined over two contexts; the same steps as K cg_solve_host calls beside it
+    assert "pipelined" in e["mode"] and e["outputs_identical"] is True
+    assert e["one_call_at_a_time"]["value"] > 0 and e["one_call_at_a_time"]["ms_per_step"] > 0
     r = d["roofline"]
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["peak"] > 1000
     assert len(r["kernels"]) == 3 and [k["name"][:2] for k in r["kernels"]] == ["a2", "a3", "a4"]

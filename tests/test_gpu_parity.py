@@ -624,6 +624,65 @@ def test_host_forms_equal_device_forms(wilson, precision):
         assert out_h.tobytes() == out_d.tobytes()
 
 
+@pytest.mark.parametrize("precision,ci", [(32, 1), (32, 2), (64, 1)])
+def test_split_phase_host_solves_pipelined_over_two_contexts(wilson, oracle, precision, ci):
+    """cg_solve_host_begin / _run / _wait (include/wilson_cg.h): a queue of DIFFERENT systems (own gauge field and source
+    each) pipelined over two contexts on two streams, one host thread.  Every solution must be bit-identical to
+    cg_solve_host on the same inputs, and the first one is checked against the oracle like every other solve."""
+    import torch
+
+    cfg = inputs.CONFIGS[ci]
+    n = 5
+    cdt = gu.np_complex(precision)
+    r_min = cfg.r_min if precision == 32 else 1e-10
+    systems = []
+    for k in range(n):
+        U = inputs.gauge_field(CFG_TEST + 40 + k, cfg.dims, cfg.links, cfg.eps, dtype=cdt)
+        eta = inputs.source_field(CFG_TEST + 50 + k, cfg.dims, dtype=cdt)
+        systems.append((torch.from_numpy(U).pin_memory(), torch.from_numpy(eta).pin_memory()))
+    V = int(np.prod(cfg.dims))
+    outs = [torch.zeros((V, 4, 3), dtype=torch.complex64 if precision == 32 else torch.complex128).pin_memory() for _ in range(n)]
+    with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ref_ctx:
+        want = [ref_ctx.cg_solve_host(U, eta, cfg.kappa, r_min, cfg.max_iter) for U, eta in systems]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ctxs = [wilson.WilsonContext(cfg.dims, precision, cfg.bc_t, stream=s) for s in streams]
+    try:
+        infos = []
+        ctxs[0].cg_solve_host_begin(*systems[0])
+        with pytest.raises(wilson.WilsonError):
+            ctxs[0].cg_solve_host_begin(*systems[0])              # already staged
+        with pytest.raises(wilson.WilsonError):
+            ctxs[1].cg_solve_host_run(cfg.kappa, r_min, cfg.max_iter, outs[1])   # nothing staged on this ctx
+        ctxs[1].cg_solve_host_wait()                               # nothing pending: a no-op
+        for i in range(n):
+            if i + 1 < n:
+                ctxs[(i + 1) % 2].cg_solve_host_begin(*systems[i + 1])
+            infos.append(ctxs[i % 2].cg_solve_host_run(cfg.kappa, r_min, cfg.max_iter, outs[i]))
+            if i > 0:
+                ctxs[(i - 1) % 2].cg_solve_host_wait()
+        ctxs[(n - 1) % 2].cg_solve_host_wait()
+        for i in range(n):
+            psi_w, info_w = want[i]
+            assert infos[i]["status"] == 0 and infos[i]["iterations"] == info_w["iterations"]
+            assert outs[i].numpy().tobytes() == np.asarray(psi_w).tobytes(), i
+        # the gauge field of the previous call on a ctx is reused when U_host is None
+        ctxs[0].cg_solve_host_begin(None, systems[n - 1][1])       # ctx 0 last held U of system n-1 (n odd)
+        info = ctxs[0].cg_solve_host_run(cfg.kappa, r_min, cfg.max_iter, outs[0])
+        ctxs[0].cg_solve_host_wait()
+        assert info["iterations"] == want[n - 1][1]["iterations"]
+        assert outs[0].numpy().tobytes() == np.asarray(want[n - 1][0]).tobytes()
+    finally:
+        for c in ctxs:
+            c.close()
+    U0, eta0 = systems[0][0].numpy(), systems[0][1].numpy()
+    U64, eta64 = U0.astype(np.complex128), eta0.astype(np.complex128)
+    psi_o, info_o = oracle.cg_solve(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t)
+    assert iters_close(want[0][1]["iterations"], info_o["iterations"])
+    res = oracle.true_residual(cfg.dims, U64, eta64, np.asarray(want[0][0]).astype(np.complex128), cfg.kappa, cfg.bc_t)
+    res_o = oracle.true_residual(cfg.dims, U64, eta64, psi_o, cfg.kappa, cfg.bc_t)
+    assert res <= 2.0 * res_o
+
+
 def test_error_codes(wilson):
     cfg = inputs.CONFIGS[0]
     U, eta = gu.config_fields(0, 32)
