@@ -357,7 +357,9 @@ def main():
         # the uploads of step i+1 and the download of step i-1 run while the GPU iterates on step i.  Pipeline fill (the
         # first upload) and drain (the last download) are inside the timed region too.
         psi_pin2 = torch.empty_like(psi_pin).pin_memory()
-        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        # streams above the lowest priority: the library's pack kernels run on a lowest-priority stream of their own and
+        # take only the room the other context's solve leaves
+        streams = [torch.cuda.Stream(priority=-1), torch.cuda.Stream(priority=-1)]
         pctx = [wilson.WilsonContext(cfg.dims, args.precision, cfg.bc_t, stream=st) for st in streams]
         for pc in pctx:
             if args.tile is not None:

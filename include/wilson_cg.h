@@ -82,7 +82,8 @@ typedef struct wd_cg_info {
     double eta_norm2;      /* <eta,eta> */
     double gpu_ms;         /* device time of init + loop + final D-dagger (CUDA events on the ctx stream) */
     double total_ms;       /* *_host calls: device time including H2D copies, pack, solve, unpack, D2H; else = gpu_ms */
-    int kernel_launches;   /* number of this library's kernels launched by the call */
+    int kernel_launches;   /* number of this library's kernels launched by the call (including the one-warp kernels that write
+                              the device scalars to the pinned host mirror at every poll) */
     int cg_mode;           /* 1 = three kernels per iteration, 2 = whole solve in one cooperative launch (one thread per site),
                               3 = BiCGSTAB, 4 = even-odd CG, 5 = multi-source CG, 6 = one cooperative launch with the hopping sum of
                               a site split over four warps, 7 = even-odd BiCGSTAB (seven kernels per iteration), 8 = even-odd BiCGSTAB in one
@@ -323,6 +324,8 @@ int cg_solve_host(wd_ctx *ctx, const void *U_host, const void *eta_host, void *p
  *                         transfers overlap other solves; kernel_launches counts begin + run).  WD_ERR_ARG if nothing is staged.
  *   cg_solve_host_wait    returns when psi_host_out of the last run on this ctx is complete (no-op if nothing is pending).
  * cg_solve_host(ctx, ...) is begin + run + wait on one ctx.  A ctx is still single-threaded: one host thread drives both.
+ * The pack kernels of the uploads run on a library stream of the LOWEST priority; give the contexts streams of a higher
+ * priority (cudaStreamCreateWithPriority) and those kernels take only the room the other context's solve leaves.
  */
 int cg_solve_host_begin(wd_ctx *ctx, const void *U_host, const void *eta_host);
 int cg_solve_host_run(wd_ctx *ctx, void *psi_host_out, double kappa, double r_min, int max_iter, wd_cg_info *info);

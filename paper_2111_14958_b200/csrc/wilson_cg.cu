@@ -199,6 +199,7 @@ extern "C" int wd_destroy(wd_ctx *c)
     for (int i = 0; i < WD_HOST_SLABS + 1; ++i)
         if (c->slab_ev[i]) cudaEventDestroy(c->slab_ev[i]);
     if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
+    if (c->pack_stream) { cudaStreamSynchronize(c->pack_stream); cudaStreamDestroy(c->pack_stream); cudaEventDestroy(c->pack_ev); }
     free(c->pev);
     free(c);
     return WD_OK;
@@ -603,7 +604,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
         c->launches++;
         CUDA_TRY(c, c->precision == 32 ? launch_cg_resident_f32(a) : launch_cg_resident_f64(a));
         if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
-        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, wd_fetch(c, c->sc_host, c->sc, sizeof(CgScalars)));
         CUDA_TRY(c, cudaStreamSynchronize(c->stream));
         const CgScalars &s1 = *c->sc_host;
         c->last_iters = s1.k;
@@ -627,7 +628,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
         rc = cg_onelaunch(c, U, eta, psi, kappa, r_min, max_iter);
         if (rc != WD_OK) return rc;
         if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
-        CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, wd_fetch(c, c->sc_host, c->sc, sizeof(CgScalars)));
         CUDA_TRY(c, cudaStreamSynchronize(c->stream));
         const CgScalars &s1 = *c->sc_host;
         c->last_iters = s1.k;
@@ -717,7 +718,7 @@ static int cg_device(wd_ctx *c, const void *U, const void *eta, void *psi, doubl
     // a6: psi = D-dagger y ("then we multiply the solution by D-dagger")
     CUDA_TRY(c, (launch_dslash<1, MODE_PLAIN>(c, U, c->y, psi, kappa, nullptr, 0)));
     if (record_events) CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
-    CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, wd_fetch(c, c->sc_host, c->sc, sizeof(CgScalars)));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     const CgScalars &s = *c->sc_host;
     c->last_iters = s.k;
@@ -850,7 +851,7 @@ extern "C" int bicgstab_solve(wd_ctx *c, const void *U, const void *eta, void *p
                             : bicgstab_loop<double>(c, U, eta, psi, kappa, r_min, max_iter);
     if (rc != WD_OK) return rc;
     CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
-    CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, wd_fetch(c, c->sc_host, c->sc, sizeof(CgScalars)));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     const CgScalars &s = *c->sc_host;
     c->last_iters = s.k;
@@ -910,13 +911,19 @@ static int ensure_staging(wd_ctx *c)
 }
 
 // The host-buffer calls move their fields in WD_HOST_SLABS slabs of whole 16-site blocks on a second stream (copy_stream)
-// while the ctx stream packs / unpacks the slab that has just landed: the permutation kernels (about 2 ms for the 4 GB of
+// while a third stream (pack_stream) packs the slab that has just landed (the ctx stream unpacks on the way back): the permutation kernels (about 2 ms for the 4 GB of
 // config 4) hide behind the PCIe transfer instead of following it.  The solve itself needs all of U and eta, so the
 // transfers as such cannot overlap it: the host-buffer form stays PCIe-bound (bench.py reports the measured rate beside it).
 static int ensure_copy_stream(wd_ctx *c)
 {
     if (!c->copy_stream) {
         CUDA_TRY(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        // The pack kernels get a stream of the LOWEST priority: when a second ctx iterates on a stream of higher priority
+        // (split-phase calls, bench.py e2e), their CTAs are placed only where that solve leaves room
+        int least = 0, greatest = 0;
+        CUDA_TRY(c, cudaDeviceGetStreamPriorityRange(&least, &greatest));
+        CUDA_TRY(c, cudaStreamCreateWithPriority(&c->pack_stream, cudaStreamNonBlocking, least));
+        CUDA_TRY(c, cudaEventCreateWithFlags(&c->pack_ev, cudaEventDisableTiming));
         for (int i = 0; i < WD_HOST_SLABS + 1; ++i) CUDA_TRY(c, cudaEventCreateWithFlags(&c->slab_ev[i], cudaEventDisableTiming));
     }
     return WD_OK;
@@ -940,6 +947,7 @@ static int stage_inputs_t(wd_ctx *c, const void *U_host, const void *s_host)
     // the copy stream starts after everything already enqueued on the ctx stream (the staging buffers may be in use)
     CUDA_TRY(c, cudaEventRecord(c->slab_ev[WD_HOST_SLABS], c->stream));
     CUDA_TRY(c, cudaStreamWaitEvent(c->copy_stream, c->slab_ev[WD_HOST_SLABS], 0));
+    CUDA_TRY(c, cudaStreamWaitEvent(c->pack_stream, c->slab_ev[WD_HOST_SLABS], 0));
     for (int pass = 0; pass < 2; ++pass) {
         if (pass == 0 && !U_host) continue;
         const size_t site_bytes = (pass == 0 ? 72 : 24) * sizeof(real);
@@ -952,23 +960,26 @@ static int stage_inputs_t(wd_ctx *c, const void *U_host, const void *s_host)
                 CUDA_TRY(c, cudaMemcpyAsync(dst + (size_t)s0 * site_bytes, src + (size_t)s0 * site_bytes,
                                             (size_t)(s1 - s0) * site_bytes, cudaMemcpyHostToDevice, c->copy_stream));
             CUDA_TRY(c, cudaEventRecord(c->slab_ev[i], c->copy_stream));
-            CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->slab_ev[i], 0));
+            CUDA_TRY(c, cudaStreamWaitEvent(c->pack_stream, c->slab_ev[i], 0));
             if (s1p <= s0) continue;
             const unsigned int grid = (unsigned int)((s1p - s0 + VEC_NT - 1) / VEC_NT);
             // sites s0 .. s1p - 1: the kernels take the end of the slab as their padded-volume bound
             if (pass == 0) {
                 if (c->recon == 18)
-                    pack_gauge_kernel<real, 18><<<grid, VEC_NT, 0, c->stream>>>((const gvec *)c->U_can, (gvec *)c->U_nat, c->V, s1p, s0);
+                    pack_gauge_kernel<real, 18><<<grid, VEC_NT, 0, c->pack_stream>>>((const gvec *)c->U_can, (gvec *)c->U_nat, c->V, s1p, s0);
                 else
-                    pack_gauge_kernel<real, 12><<<grid, VEC_NT, 0, c->stream>>>((const gvec *)c->U_can, (gvec *)c->U_nat, c->V, s1p, s0);
+                    pack_gauge_kernel<real, 12><<<grid, VEC_NT, 0, c->pack_stream>>>((const gvec *)c->U_can, (gvec *)c->U_nat, c->V, s1p, s0);
             } else {
-                pack_spinor_kernel<real><<<grid, VEC_NT, 0, c->stream>>>((const svec *)c->s_can, (svec *)c->s_nat_in, c->V, s1p, s0);
+                pack_spinor_kernel<real><<<grid, VEC_NT, 0, c->pack_stream>>>((const svec *)c->s_can, (svec *)c->s_nat_in, c->V, s1p, s0);
             }
             c->launches++;
         }
         if (pass == 0) c->have_gauge = 1;
     }
     CUDA_TRY(c, cudaGetLastError());
+    // the ctx stream goes on when the last slab has been packed
+    CUDA_TRY(c, cudaEventRecord(c->pack_ev, c->pack_stream));
+    CUDA_TRY(c, cudaStreamWaitEvent(c->stream, c->pack_ev, 0));
     return WD_OK;
 }
 

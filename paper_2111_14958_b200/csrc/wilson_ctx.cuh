@@ -63,6 +63,8 @@ struct wd_ctx {
     int host_staged;        // cg_solve_host_begin has staged inputs that no run has consumed yet
     int host_out_pending;   // cg_solve_host_run has enqueued the copy of psi to the host; cg_solve_host_wait has not been called
     cudaStream_t copy_stream;   // the *_host calls: transfers run here, slab by slab, beside the pack / unpack kernels
+    cudaStream_t pack_stream;   // the pack kernels of the uploads: lowest priority, so that they fill gaps of another ctx's solve
+    cudaEvent_t pack_ev;
     cudaEvent_t slab_ev[WD_HOST_SLABS + 1];
     cudaEvent_t ev[4];
     // per-kernel-class timing (wd_set_profile): 4 events per iteration of one poll chunk
@@ -115,6 +117,23 @@ static inline size_t gauge_can_bytes(const wd_ctx *c) { return (size_t)72 * c->V
 static inline size_t spinor_vecs(const wd_ctx *c) { return (size_t)(c->precision == 32 ? 6 : 12) * vpad(c); }
 
 
+// Device scalars -> pinned host mirror WITHOUT the copy engine.  A D2H memcpy of a few bytes queues behind every large
+// download that any stream has in flight on the same engine: beside a continuous 4 GB download a 48^3x96 solve took 1860 ms
+// instead of 364 (each poll waited for a whole copy), and in the pipelined host-buffer solves (cg_solve_host_begin / _run /
+// _wait) the first polls of a solve waited for the previous solve's psi.  A one-warp kernel writes the mirror instead
+// (pinned host memory is device-accessible under UVA; the writes are visible to the host once an event recorded behind
+// the kernel has completed).
+static __global__ void wd_scalars_to_host_kernel(const unsigned int *__restrict__ src, unsigned int *dst, int nwords)
+{
+    for (int i = threadIdx.x; i < nwords; i += blockDim.x) dst[i] = src[i];
+}
+static inline cudaError_t wd_fetch(wd_ctx *c, void *host_dst, const void *dev_src, size_t bytes)
+{
+    wd_scalars_to_host_kernel<<<1, 64, 0, c->stream>>>((const unsigned int *)dev_src, (unsigned int *)host_dst, (int)(bytes / 4));
+    c->launches++;
+    return cudaGetLastError();
+}
+
 // Host side of the device-resident solver loops (reading R1).  Iterations are enqueued in chunks of
 // `poll`; after each chunk the device scalars are copied to a pinned mirror and the host waits for that copy to learn
 // whether the loop condition has failed (k_stop).  With `ahead`, the NEXT chunk is enqueued before the host waits, so the
@@ -128,7 +147,7 @@ static inline int wd_poll_loop(wd_ctx *c, int max_iter, int poll, bool ahead, En
     int enqueued = 0;      // iterations enqueued
     int slot = 0;          // pinned mirror / event the next chunk reports into
     auto report = [&](int sl) -> int {
-        CUDA_TRY(c, cudaMemcpyAsync(&c->sc_poll[sl], c->sc, sizeof(wd::CgScalars), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, wd_fetch(c, &c->sc_poll[sl], c->sc, sizeof(wd::CgScalars)));
         CUDA_TRY(c, cudaEventRecord(c->poll_ev[sl], c->stream));
         return WD_OK;
     };

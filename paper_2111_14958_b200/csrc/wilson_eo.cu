@@ -315,7 +315,7 @@ extern "C" int cg_solve_eo(wd_ctx *c, const void *U_eo, const void *eta_eo, void
                             : eo_loop<double>(c, U_eo, eta_eo, psi_eo, kappa, r_min, max_iter);
     if (rc != WD_OK) return rc;
     CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
-    CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, wd_fetch(c, c->sc_host, c->sc, sizeof(CgScalars)));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     const CgScalars &s = *c->sc_host;
     c->last_iters = s.k;
@@ -499,7 +499,7 @@ extern "C" int bicgstab_solve_eo(wd_ctx *c, const void *U_eo, const void *eta_eo
                                  : eo_bicgstab_loop<double>(c, U_eo, eta_eo, psi_eo, kappa, r_min, max_iter);
     if (rc != WD_OK) return rc;
     CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
-    CUDA_TRY(c, cudaMemcpyAsync(c->sc_host, c->sc, sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, wd_fetch(c, c->sc_host, c->sc, sizeof(CgScalars)));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     const CgScalars &s = *c->sc_host;
     c->last_iters = s.k;

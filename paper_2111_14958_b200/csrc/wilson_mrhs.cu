@@ -109,7 +109,7 @@ int cg_group(wd_ctx *c, int g, const void *U, const void *eta, void *psi, double
             CUDA_TRY(c, cudaGetLastError());
             if (ev) CUDA_TRY(c, cudaEventRecord(c->bev[3], c->stream));
         }
-        CUDA_TRY(c, cudaMemcpyAsync(c->m_sc_host, c->m_sc, g * sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, wd_fetch(c, c->m_sc_host, c->m_sc, g * sizeof(CgScalars)));
         CUDA_TRY(c, cudaStreamSynchronize(c->stream));
         int k_stop_max = 0;
         for (int j = 0; j < g; ++j)
@@ -127,7 +127,7 @@ int cg_group(wd_ctx *c, int g, const void *U, const void *eta, void *psi, double
     }
     CUDA_TRY(c, mrhs_launch(c, g, 1, MODE_PLAIN, U, y, psi, nullptr, kappa, c->m_sc, nullptr, 0, 0));
     CUDA_TRY(c, cudaEventRecord(c->ev[1], c->stream));
-    CUDA_TRY(c, cudaMemcpyAsync(c->m_sc_host, c->m_sc, g * sizeof(CgScalars), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, wd_fetch(c, c->m_sc_host, c->m_sc, g * sizeof(CgScalars)));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     float ms = 0.f;
     CUDA_TRY(c, cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]));

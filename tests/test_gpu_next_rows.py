@@ -477,7 +477,7 @@ def test_eo_bicgstab_baseline_configs(wilson, oracle, cfg_index, precision, r_mi
         _, plain = bicgstab_on_gpu(ctx, U, eta, cfg.kappa, r_min, cfg.max_iter)
     psi_o, info_o = oracle.bicgstab_solve_eo(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t, history=True)
     assert info["status"] == 0 and info["converged"] == 1 and info["cg_mode"] == (7 if mode == 1 else 8) and info_o["converged"]
-    assert info["kernel_launches"] >= 7 * info["iterations"] + 1 if mode == 1 else info["kernel_launches"] == 1
+    assert info["kernel_launches"] >= 7 * info["iterations"] + 1 if mode == 1 else info["kernel_launches"] == 2
     slack = 0 if precision == 64 else max(1, int(0.05 * info_o["iterations"] + 0.5))
     assert abs(info["iterations"] - info_o["iterations"]) <= slack, (info["iterations"], info_o["iterations"])
     assert abs(info["eta_norm2"] - info_o["eta_norm2"]) < (1e-6 if precision == 32 else 1e-13) * info_o["eta_norm2"]

@@ -339,7 +339,8 @@ def _cg_case(wilson, oracle, cfg, precision, r_min, poll=None, mode=0):
         hist = ctx.wd_cg_history()
     if mode:
         assert info["cg_mode"] == mode
-        assert info["kernel_launches"] == 1 if mode in (2, 6, 9, 10) else info["kernel_launches"] >= 3 * info["iterations"] + 2
+        # one-launch drivers: the solve kernel + the one-warp kernel that writes the scalars to the pinned host mirror
+        assert info["kernel_launches"] == 2 if mode in (2, 6, 9, 10) else info["kernel_launches"] >= 3 * info["iterations"] + 2
     psi_o, info_o = oracle.cg_solve(cfg.dims, U64, eta64, cfg.kappa, r_min, cfg.max_iter, cfg.bc_t, history=True)
     res_gpu = oracle.true_residual(cfg.dims, U64, eta64, psi.astype(np.complex128), cfg.kappa, cfg.bc_t)
     res_orc = oracle.true_residual(cfg.dims, U64, eta64, psi_o, cfg.kappa, cfg.bc_t)
@@ -412,7 +413,7 @@ def test_cg_resident_cluster_sizes(wilson, oracle, dims, bc_t, precision):
         for _ in range(2):
             psi, info = gu.solve_on_gpu(ctx, U, eta, 0.12, tol, 500)
             outs.append(psi.tobytes())
-        assert info["status"] == 0 and info["cg_mode"] == 9 and info["kernel_launches"] == 1
+        assert info["status"] == 0 and info["cg_mode"] == 9 and info["kernel_launches"] == 2
     assert outs[0] == outs[1]
     assert iters_close(info["iterations"], info_o["iterations"])
     res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), 0.12, bc_t)
@@ -428,7 +429,7 @@ def test_cg_automatic_mode_by_volume(wilson):
         U, eta = gu.config_fields(ci, precision)
         with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
             _, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
-        assert info["cg_mode"] == want and info["kernel_launches"] == 1
+        assert info["cg_mode"] == want and info["kernel_launches"] == 2
 
 
 @pytest.mark.parametrize("precision", [32, 64])
