@@ -422,7 +422,7 @@ extern "C" int wd_norm2(wd_ctx *c, const void *a, double *result)
         norm2_kernel<double><<<grid, VEC_NT, 0, c->stream>>>((const double2 *)a, n, c->V, padded(c), c->partials, c->counter, c->result_dev);
     c->launches++;
     CUDA_TRY(c, cudaGetLastError());
-    CUDA_TRY(c, cudaMemcpyAsync(c->result_host, c->result_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, wd_fetch(c, c->result_host, c->result_dev, sizeof(double)));   // not the copy engine: see wd_fetch
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     *result = *c->result_host;
     return WD_OK;
