@@ -451,6 +451,55 @@ def test_cg_onelaunch_ragged_lattice(wilson, oracle, precision):
             assert res <= 2.0 * oracle.true_residual(dims, U64, eta64, psi_o, 0.12, bc_t)
 
 
+def _random_lattices(n, seed):
+    """n seeded lattices with extents in [4, 19], skewed towards small ones (the oracle has to finish in seconds)"""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    out = []
+    while len(out) < n:
+        dims = tuple(int(d) for d in rng.choice([4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 16, 17, 19], size=4))
+        if 256 <= int(np.prod(dims)) <= 20000:
+            out.append((dims, int(rng.choice([-1, 1]))))
+    return out
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_random_lattices_operator_and_every_cg_driver(wilson, oracle, precision):
+    """16 seeded lattices with unrelated, mostly odd extents, either boundary condition: D and D-dagger per site against the
+    oracle, then cg_solve with the automatic choice and with every driver that accepts the lattice (a driver may refuse a
+    lattice it has no launch configuration for, with WD_ERR_ARG; it must not accept it and be wrong)."""
+    tol = 1e-6 if precision == 32 else 1e-11
+    drivers_run = {m: 0 for m in (0, 1, 2, 6, 9, 10)}
+    for k, (dims, bc_t) in enumerate(_random_lattices(16, 20211114)):
+        cdt = gu.np_complex(precision)
+        links = "haar" if k % 2 else "near_identity"
+        U = inputs.gauge_field(CFG_TEST + 20, dims, links, dtype=cdt)
+        eta = inputs.source_field(CFG_TEST + 20, dims, dtype=cdt)
+        U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+        kappa = 0.11 if links == "haar" else 0.122
+        with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+            for dagger in (False, True):
+                got = gu.apply_on_gpu(ctx, U, eta, kappa, dagger)
+                want = oracle.wd_apply(dims, U64, eta64, kappa, dagger, bc_t)
+                assert lm.per_site_rel_err(got, want)[0] <= TOL_APPLY[precision], (dims, bc_t, dagger)
+        psi_o, info_o = oracle.cg_solve(dims, U64, eta64, kappa, tol, 400, bc_t)
+        res_o = oracle.true_residual(dims, U64, eta64, psi_o, kappa, bc_t)
+        assert info_o["converged"]
+        for mode in drivers_run:
+            with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+                try:
+                    ctx.wd_set_cg_mode(mode)
+                    psi, info = gu.solve_on_gpu(ctx, U, eta, kappa, tol, 400)
+                except wilson.WilsonError as e:
+                    assert e.code == -1 and mode in (9, 10), (dims, mode, str(e))
+                    continue
+            drivers_run[mode] += 1
+            assert info["status"] == 0 and info["converged"] == 1, (dims, mode, info)
+            assert iters_close(info["iterations"], info_o["iterations"]), (dims, mode, info["iterations"], info_o["iterations"])
+            res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), kappa, bc_t)
+            assert res <= 2.0 * res_o, (dims, mode, res, res_o)
+    assert all(drivers_run[m] == 16 for m in (0, 1, 2, 6)) and drivers_run[10] >= 8, drivers_run
+
+
 def test_cg_result_independent_of_poll_interval_and_repeatable(wilson):
     cfg = inputs.CONFIGS[1]
     U, eta = gu.config_fields(1, 32)
