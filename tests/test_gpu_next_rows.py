@@ -611,6 +611,62 @@ def test_eo_solvers_with_12_real_links(wilson, oracle, cfg_index, precision, r_m
 
 
 # ---------------------------------------------------------------- full BASELINE sizes (configs 3 and 4)
+@pytest.mark.parametrize("precision", [32, 64])
+def test_random_lattices_next_rows(wilson, oracle, precision):
+    """12 seeded lattices with unrelated extents (odd ones for BiCGSTAB, 12-real links and the multi-source pass; even ones
+    for the even-odd solvers, with half volumes that are not multiples of the 16-site block): every next-row solver against
+    its oracle counterpart."""
+    r_min = 1e-6 if precision == 32 else 1e-10
+    cdt = gu.np_complex(precision)
+    rng = np.random.Generator(np.random.PCG64(2111149580))
+    cases = []
+    while len(cases) < 12:
+        even = len(cases) % 2 == 0
+        pool = [4, 6, 8, 10, 12, 14, 18] if even else [4, 5, 6, 7, 9, 11, 13, 15, 17]
+        dims = tuple(int(d) for d in rng.choice(pool, size=4))
+        if 256 <= int(np.prod(dims)) <= 16000:
+            cases.append((dims, int(rng.choice([-1, 1])), even))
+    for k, (dims, bc_t, even) in enumerate(cases):
+        links = "haar" if k % 3 == 0 else "near_identity"
+        kappa = 0.11 if links == "haar" else 0.121
+        U = inputs.gauge_field(CFG_TEST + 80, dims, links).astype(cdt)
+        eta = inputs.source_field(CFG_TEST + 80, dims).astype(cdt)
+        U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+        bound = 4.0 * r_min * (1 + 8 * kappa) / (1 - 8 * kappa)
+        # f4: BiCGSTAB on D
+        psi_o, info_o = oracle.bicgstab_solve(dims, U64, eta64, kappa, r_min, 500, bc_t)
+        with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+            psi, info = bicgstab_on_gpu(ctx, U, eta, kappa, r_min, 500)
+        slack = 0 if precision == 64 else max(1, int(0.05 * info_o["iterations"] + 0.5))
+        assert info["status"] == 0 and abs(info["iterations"] - info_o["iterations"]) <= slack, (dims, info, info_o["iterations"])
+        assert oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), kappa, bc_t) < 2.0 * r_min
+        assert np.linalg.norm(psi - psi_o) < bound * np.linalg.norm(psi_o)
+        # f3: 12-real links (operator, both daggers)
+        for dagger in (False, True):
+            got = _apply12(wilson, dims, U, eta, kappa, dagger, precision, bc_t)
+            want = oracle.wd_apply(dims, U64, eta64, kappa, dagger, bc_t)
+            assert lm.per_site_rel_err(got, want)[0] <= (1e-5 if precision == 32 else 1e-12), (dims, dagger)
+        if not even:
+            continue
+        # f3: even-odd CG and even-odd BiCGSTAB (both drivers)
+        psi_o, info_o = oracle.cg_solve_eo(dims, U64, eta64, kappa, r_min, 500, bc_t)
+        with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+            Ue = ctx.wd_eo_pack_gauge(gu.to_device(U))
+            ee = ctx.wd_eo_pack_spinor(gu.to_device(eta))
+            pe, info = ctx.cg_solve_eo(Ue, ee, kappa, r_min, 500)
+            psi = gu.to_host(ctx.wd_eo_unpack_spinor(pe))
+        assert info["status"] == 0 and abs(info["iterations"] - info_o["iterations"]) <= max(1, math.floor(0.02 * info_o["iterations"] + 0.5))
+        assert oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), kappa, bc_t) < 2.0 * r_min
+        assert np.linalg.norm(psi - psi_o) < bound * np.linalg.norm(psi_o)
+        psi_o, info_o = oracle.bicgstab_solve_eo(dims, U64, eta64, kappa, r_min, 500, bc_t)
+        for mode in (1, 2):
+            with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+                psi, info = eo_bicgstab_on_gpu(ctx, U, eta, kappa, r_min, 500, mode)
+            assert info["status"] == 0 and abs(info["iterations"] - info_o["iterations"]) <= (0 if precision == 64 else 1), (dims, mode)
+            assert oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), kappa, bc_t) < 2.0 * r_min
+            assert np.linalg.norm(psi - psi_o) < bound * np.linalg.norm(psi_o)
+
+
 def _rows_golden(cfg_index, precision):
     import json
     import os
