@@ -367,16 +367,8 @@ def main():
         outs = [psi_pin, psi_pin2]
 
         def pipelined(nsteps):
-            pctx[0].cg_solve_host_begin(U_pin, eta_pin)
-            inf = None
-            for i in range(nsteps):
-                if i + 1 < nsteps:
-                    pctx[(i + 1) % 2].cg_solve_host_begin(U_pin, eta_pin)
-                inf = pctx[i % 2].cg_solve_host_run(cfg.kappa, r_min, cfg.max_iter, outs[i % 2])
-                if i > 0:
-                    pctx[(i - 1) % 2].cg_solve_host_wait()
-            pctx[(nsteps - 1) % 2].cg_solve_host_wait()
-            return inf
+            return wilson.cg_solve_host_queue(pctx, [(U_pin, eta_pin)] * nsteps, cfg.kappa, r_min, cfg.max_iter,
+                                              [outs[i % 2] for i in range(nsteps)])[-1]
 
         pipelined(2)                                    # warm-up: staging buffers of both contexts
         barrier()

@@ -176,6 +176,29 @@ def _torch():
     return torch
 
 
+def cg_solve_host_queue(ctxs, systems, kappa, r_min, max_iter, outs):
+    """A queue of host-buffer solves pipelined over two contexts (include/wilson_cg.h, cg_solve_host_begin / _run / _wait): the
+    uploads of solve i+1 and the download of solve i-1 run while the GPU iterates on solve i.  `ctxs`: two WilsonContexts of
+    the same lattice on two different streams; `systems`: a sequence of (U_host or None, eta_host); `outs[i]`: the pinned
+    host buffer solve i writes (a buffer may be reused two solves later).  Returns the info dicts in order; every output is
+    complete on return.  Argument marshalling only: the choreography of the header's example, nothing else."""
+    if len(ctxs) != 2 or ctxs[0] is ctxs[1]:
+        raise ValueError("two distinct contexts are needed")
+    n = len(systems)
+    infos = []
+    if n == 0:
+        return infos
+    ctxs[0].cg_solve_host_begin(*systems[0])
+    for i in range(n):
+        if i + 1 < n:
+            ctxs[(i + 1) % 2].cg_solve_host_begin(*systems[i + 1])
+        infos.append(ctxs[i % 2].cg_solve_host_run(kappa, r_min, max_iter, outs[i]))
+        if i > 0:
+            ctxs[(i - 1) % 2].cg_solve_host_wait()
+    ctxs[(n - 1) % 2].cg_solve_host_wait()
+    return infos
+
+
 def wd_noalloc_max_sites(precision: int) -> int:
     """Largest number of sites wd_norm2_noalloc accepts (its scratch is a static device array); needs no GPU."""
     return int(load_library().wd_noalloc_max_sites(int(precision)))

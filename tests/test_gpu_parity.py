@@ -711,6 +711,11 @@ def test_split_phase_host_solves_pipelined_over_two_contexts(wilson, oracle, pre
             if i > 0:
                 ctxs[(i - 1) % 2].cg_solve_host_wait()
         ctxs[(n - 1) % 2].cg_solve_host_wait()
+        # the binding's helper does the same choreography
+        outs2 = [torch.zeros_like(o).pin_memory() for o in outs]
+        infos2 = wilson.cg_solve_host_queue(ctxs, systems, cfg.kappa, r_min, cfg.max_iter, outs2)
+        assert [d["iterations"] for d in infos2] == [d["iterations"] for d in infos]
+        assert all(torch.equal(a, b) for a, b in zip(outs, outs2))
         for i in range(n):
             psi_w, info_w = want[i]
             assert infos[i]["status"] == 0 and infos[i]["iterations"] == info_w["iterations"]
