@@ -135,7 +135,7 @@ static inline cudaError_t wd_fetch(wd_ctx *c, void *host_dst, const void *dev_sr
 }
 
 // Host side of the device-resident solver loops (reading R1).  Iterations are enqueued in chunks of
-// `poll`; after each chunk the device scalars are copied to a pinned mirror and the host waits for that copy to learn
+// `poll`; after each chunk the device scalars are written to a pinned mirror (wd_fetch) and the host waits for that write to learn
 // whether the loop condition has failed (k_stop).  With `ahead`, the NEXT chunk is enqueued before the host waits, so the
 // stream never drains at a poll; kernels of iterations >= k_stop return at once, which makes the over-launch harmless.
 //   enqueue(first_iteration, n_iterations, slot) -> WD_OK / error      slot in {0,1}: which of two event pools to use
