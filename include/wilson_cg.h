@@ -382,7 +382,7 @@ const char *wd_noalloc_last_error(void);
  *                             1 if compiled for precision 64}.
  *   wd_set_tile(ctx, i)       select tile i for the stencil kernels of this ctx; i = -1 restores the automatic choice.
  *   wd_get_tile(ctx)          index in use.
- *   wd_set_cg_mode(ctx, m)        0 = automatic (mode 9 where the lattice fits one or two CTAs of it, else one cooperative launch for the whole solve when V <= 200000 sites in fp32 /
+ *   wd_set_cg_mode(ctx, m)        0 = automatic (mode 9 where the lattice fits a cluster of at most four (fp32) or eight (fp64) CTAs of it, i.e. up to 1024 sites, else one cooperative launch for the whole solve when V <= 200000 sites in fp32 /
  *                             65536 in fp64 — this covers the paper's own 4^4..14^4 range — else three kernels per iteration),
  *                             1 = always three kernels, 2 = always one launch, one thread per site (grid barriers between the
  *                             phases; same recurrence and precision), 6 = always one launch with a CTA of 32 sites x 4

@@ -504,16 +504,18 @@ static bool resident_plan(const wd_ctx *c, int *nc_out, int *spc_out)
     return false;
 }
 
-// Automatic only for clusters of one or two CTAs (4^4: 0.143 ms per solve in fp32 against 0.22-0.24 for the one-launch
-// kernels, 0.35 against 0.41 in fp64).  Larger clusters are bound by distributed shared memory: at 8^4 (16 CTAs) every CTA
-// pulls 84 KB of remote spinors and links per stencil pass at the ~17 B/clk a CTA gets from its peers, 10.9 us per iteration
-// against 9.8 for the L2-resident one-launch kernel (measured); wd_set_cg_mode(ctx, 9) still selects them.
+// Automatic for clusters of up to four CTAs in fp32 and eight in fp64 (measured, us per iteration, resident / best of the other
+// one-launch kernels: fp32 4^4 5.1 / 8.6, 4^3x8 6.6 / 9.5, 8x4x4x8 and 4x4x8x8 (4 CTAs) 7.5 / 9.4-9.8, 8 CTAs 9.8-10.2 / 9.6-9.9;
+// fp64 4^4 (2 CTAs) 7.6 / 10.5, 4^3x8 (4) 7.7 / 10.5, 1024 sites (8) 9.6 / 10.4-11.2, 2048 sites (16) 11.5 / 10.5).  Larger clusters
+// are bound by distributed shared memory: at 8^4 (16 CTAs) every CTA pulls 84 KB of remote spinors and links per stencil pass at
+// the ~17 B/clk a CTA gets from its peers, 10.9 us per iteration against 9.8 for the L2-resident one-launch kernel;
+// wd_set_cg_mode(ctx, 9) still selects them.
 static bool use_resident(const wd_ctx *c)
 {
     int nc, spc;
     if (c->cg_mode != 0 && c->cg_mode != 9) return false;
     if (!resident_plan(c, &nc, &spc)) return false;
-    return c->cg_mode == 9 || nc <= 2;
+    return c->cg_mode == 9 || nc <= (c->precision == 64 ? 8 : 4);
 }
 
 static bool use_split(const wd_ctx *c)

@@ -430,6 +430,14 @@ def test_cg_automatic_mode_by_volume(wilson):
         with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
             _, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
         assert info["cg_mode"] == want and info["kernel_launches"] == 2
+    # between 4^4 and 8^4: the resident kernel up to a cluster of four CTAs in fp32 (1024 sites) and eight in fp64 (1024 sites)
+    for dims, precision, want in (((8, 4, 4, 8), 32, 9), ((4, 8, 8, 8), 32, 10), ((4, 4, 8, 8), 64, 9), ((4, 8, 8, 8), 64, 6)):
+        cdt = gu.np_complex(precision)
+        U = inputs.gauge_field(CFG_TEST + 7, dims, "haar", dtype=cdt)
+        eta = inputs.source_field(CFG_TEST + 7, dims, dtype=cdt)
+        with wilson.WilsonContext(dims, precision) as ctx:
+            _, info = gu.solve_on_gpu(ctx, U, eta, 0.12, 1e-6, 500)
+        assert info["status"] == 0 and info["cg_mode"] == want, (dims, precision, info["cg_mode"])
 
 
 @pytest.mark.parametrize("precision", [32, 64])
