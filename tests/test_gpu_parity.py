@@ -728,12 +728,20 @@ def test_split_phase_host_solves_pipelined_over_two_contexts(wilson, oracle, pre
             psi_w, info_w = want[i]
             assert infos[i]["status"] == 0 and infos[i]["iterations"] == info_w["iterations"]
             assert outs[i].numpy().tobytes() == np.asarray(psi_w).tobytes(), i
+        # queues of length 0 and 1, and an output buffer reused two solves later
+        assert wilson.cg_solve_host_queue(ctxs, [], cfg.kappa, r_min, cfg.max_iter, []) == []
+        one = wilson.cg_solve_host_queue(ctxs, systems[:1], cfg.kappa, r_min, cfg.max_iter, [outs2[0]])
+        assert one[0]["iterations"] == want[0][1]["iterations"] and torch.equal(outs2[0], outs[0])
+        ring = [outs2[0], outs2[1]]
+        infos3 = wilson.cg_solve_host_queue(ctxs, systems[:4], cfg.kappa, r_min, cfg.max_iter, [ring[i % 2] for i in range(4)])
+        assert [d["iterations"] for d in infos3] == [d["iterations"] for d in infos[:4]]
+        assert torch.equal(ring[0], outs[2]) and torch.equal(ring[1], outs[3])      # the last writers of the two buffers
         # the gauge field of the previous call on a ctx is reused when U_host is None
-        ctxs[0].cg_solve_host_begin(None, systems[n - 1][1])       # ctx 0 last held U of system n-1 (n odd)
-        info = ctxs[0].cg_solve_host_run(cfg.kappa, r_min, cfg.max_iter, outs[0])
-        ctxs[0].cg_solve_host_wait()
-        assert info["iterations"] == want[n - 1][1]["iterations"]
-        assert outs[0].numpy().tobytes() == np.asarray(want[n - 1][0]).tobytes()
+        ctxs[1].cg_solve_host_begin(None, systems[3][1])           # ctx 1 last held U of system 3 (the ring run above)
+        info = ctxs[1].cg_solve_host_run(cfg.kappa, r_min, cfg.max_iter, outs2[4])
+        ctxs[1].cg_solve_host_wait()
+        assert info["iterations"] == want[3][1]["iterations"]
+        assert outs2[4].numpy().tobytes() == np.asarray(want[3][0]).tobytes()
     finally:
         for c in ctxs:
             c.close()
