@@ -123,3 +123,37 @@ def test_noalloc_norm2_rejects_what_it_cannot_do(wilson):
     a.fill_(1.0)
     assert _noalloc(wilson, a, 256, 32) == 24.0 * 256
     assert lib.wd_noalloc_last_error() == b""
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_noalloc_norm2_reads_only_its_field(wilson, precision):
+    """the field sits between two bands of NaNs and its own pad lanes (V = 840 is not a multiple of the 16-site block) hold
+    NaNs too: a read outside the field, or of a pad lane, would make the result NaN; the result slot sits between guard
+    words that must stay untouched"""
+    import torch
+
+    dims = (5, 7, 4, 6)
+    V = int(np.prod(dims))
+    a = inputs.source_field(CFG_TEST + 9, dims, dtype=gu.np_complex(precision))
+    rdt = torch.float32 if precision == 32 else torch.float64
+    with wilson.WilsonContext(dims, precision) as ctx:
+        an = ctx.wd_pack_spinor(gu.to_device(a))
+        want = ctx.wd_norm2(an)
+    n = an.numel()
+    guard = 4096
+    buf = torch.full((n + 2 * guard,), float("nan"), dtype=rdt, device="cuda")
+    field = buf[guard:guard + n]
+    field.copy_(an)
+    # poison the pad lanes of the last 16-site block: plane-major blocks of NSP planes x 16 sites x (128 bit)
+    per_vec = 4 if precision == 32 else 2
+    nsp = 6 if precision == 32 else 12
+    blocks = field.view(-1, nsp, 16, per_vec)
+    assert blocks.shape[0] * 16 >= V
+    blocks[-1, :, V % 16:, :] = float("nan")
+    res = torch.full((3,), -7.0, dtype=torch.float64, device="cuda")
+    wilson.wd_norm2_noalloc(field, V, precision, res[1:2])
+    torch.cuda.synchronize()
+    got = res.cpu().numpy()
+    assert got[0] == -7.0 and got[2] == -7.0
+    assert np.isfinite(got[1]) and abs(got[1] - want) <= TOL[precision] * want
+    assert torch.isnan(buf[:guard]).all() and torch.isnan(buf[guard + n:]).all()
