@@ -352,3 +352,44 @@ def test_contexts_on_their_own_streams_run_concurrently(wilson):
     for p in prepared:
         p[0].close()
     assert not errors, errors[:3]
+
+
+@pytest.mark.parametrize("precision", [32, 64])
+def test_host_buffer_calls_stay_inside_their_host_buffers(wilson, oracle, precision):
+    """cg_solve_host, wd_apply_host and the split-phase calls move their fields in slabs of whole 16-site blocks; on a lattice
+    whose volume is not a multiple of 16 (and smaller than 8 slabs of blocks would like) the last slab must stop at V: the host
+    buffers sit between guard bands that must not change (output) and whose NaNs must not be read (inputs)."""
+    dims, kappa, bc_t = (5, 7, 4, 6), 0.12, -1
+    V = int(np.prod(dims))
+    cdt = gu.np_complex(precision)
+    r_min = 1e-6 if precision == 32 else 1e-10
+    U = inputs.gauge_field(CFG_TEST + 30, dims, "haar", dtype=cdt)
+    eta = inputs.source_field(CFG_TEST + 30, dims, dtype=cdt)
+    g = 64
+
+    def guarded(a):
+        big = np.full((a.shape[0] + 2 * g,) + a.shape[1:], np.nan + 1j * np.nan, dtype=a.dtype)
+        big[g:g + a.shape[0]] = a
+        return big, big[g:g + a.shape[0]]
+
+    Ub, Uv = guarded(U)
+    eb, ev = guarded(eta)
+    ob, ov = guarded(np.zeros_like(eta))
+    ob[:g] = 7.0
+    ob[g + V:] = 7.0
+    with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+        psi_d, info_d = gu.solve_on_gpu(ctx, U, eta, kappa, r_min, 500)
+        _, info_h = ctx.cg_solve_host(Uv, ev, kappa, r_min, 500, out=ov)
+        assert info_h["iterations"] == info_d["iterations"] and ov.tobytes() == psi_d.tobytes()
+        assert (ob[:g] == 7.0).all() and (ob[g + V:] == 7.0).all()
+        ov[:] = 0
+        out_d = gu.apply_on_gpu(ctx, U, eta, kappa, True)
+        ctx.wd_apply_host(Uv, ev, kappa, True, out=ov)
+        assert ov.tobytes() == out_d.tobytes() and (ob[:g] == 7.0).all() and (ob[g + V:] == 7.0).all()
+        ov[:] = 0
+        ctx.cg_solve_host_begin(Uv, ev)
+        info_s = ctx.cg_solve_host_run(kappa, r_min, 500, ov)
+        ctx.cg_solve_host_wait()
+        assert info_s["iterations"] == info_d["iterations"] and ov.tobytes() == psi_d.tobytes()
+        assert (ob[:g] == 7.0).all() and (ob[g + V:] == 7.0).all()
+    assert np.isnan(Ub[:g]).all() and np.isnan(eb[g + V:]).all()        # the inputs were not written either
