@@ -507,8 +507,9 @@ static bool resident_plan(const wd_ctx *c, int *nc_out, int *spc_out)
 // Automatic for clusters of up to four CTAs in fp32 and eight in fp64 (measured, us per iteration, resident / best of the other
 // one-launch kernels: fp32 4^4 5.1 / 8.6, 4^3x8 6.6 / 9.5, 8x4x4x8 and 4x4x8x8 (4 CTAs) 7.5 / 9.4-9.8, 8 CTAs 9.8-10.2 / 9.6-9.9;
 // fp64 4^4 (2 CTAs) 7.6 / 10.5, 4^3x8 (4) 7.7 / 10.5, 1024 sites (8) 9.6 / 10.4-11.2, 2048 sites (16) 11.5 / 10.5).  Larger clusters
-// are bound by distributed shared memory: at 8^4 (16 CTAs) every CTA pulls 84 KB of remote spinors and links per stencil pass at
-// the ~17 B/clk a CTA gets from its peers, 10.9 us per iteration against 9.8 for the L2-resident one-launch kernel;
+// lose to the cost of the cluster barrier, which grows with the cluster (about 0.5 / 0.8 / 1.6 / 2 us per barrier at 2 / 4 / 8 / 16
+// CTAs, three per iteration); neither the volume nor the latency of the remote reads is what holds them (a variant
+// that pulls owner-projected half-spinors, -64 % distributed-shared-memory bytes, measured the same 11.0 us at 8^4);
 // wd_set_cg_mode(ctx, 9) still selects them.
 static bool use_resident(const wd_ctx *c)
 {
