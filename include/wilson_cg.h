@@ -382,7 +382,7 @@ const char *wd_noalloc_last_error(void);
  *                             1 if compiled for precision 64}.
  *   wd_set_tile(ctx, i)       select tile i for the stencil kernels of this ctx; i = -1 restores the automatic choice.
  *   wd_get_tile(ctx)          index in use.
- *   wd_set_cg_mode(ctx, m)        0 = automatic (mode 9 where the lattice fits a cluster of at most four (fp32) or eight (fp64) CTAs of it, i.e. up to 1024 sites, else one cooperative launch for the whole solve when V <= 200000 sites in fp32 /
+ *   wd_set_cg_mode(ctx, m)        0 = automatic (mode 9 wherever the lattice fits a cluster of it: V / nc a power of two <= 256 (fp32) / 128 (fp64) for some nc <= 16, i.e. up to 4096 / 2048 sites, else one cooperative launch for the whole solve when V <= 200000 sites in fp32 /
  *                             65536 in fp64 — this covers the paper's own 4^4..14^4 range — else three kernels per iteration),
  *                             1 = always three kernels, 2 = always one launch, one thread per site (grid barriers between the
  *                             phases; same recurrence and precision), 6 = always one launch with a CTA of 32 sites x 4
@@ -390,7 +390,8 @@ const char *wd_noalloc_last_error(void);
  *                             memory (the automatic choice in fp64 up to 8192 sites),
  *                             9 = one launch with the whole lattice RESIDENT IN SHARED MEMORY (csrc/wilson_resident.cuh): a
  *                             thread-block cluster of nc <= 16 CTAs, V / nc sites each (a power of two, <= 256 in fp32, <= 128
- *                             in fp64), neighbours in other CTAs read through distributed shared memory, barrier.cluster
+ *                             in fp64), neighbours in other CTAs read through distributed shared memory (from eight CTAs on as
+ *                             half-spinors that their owner has already projected: csrc/wilson_resident_ex.cuh), barrier.cluster
  *                             between the phases; covers 4^4 (one CTA in fp32) and 8^4 in fp32 (16 CTAs); WD_ERR_ARG if the
  *                             lattice does not fit;
  *                             10 = one cooperative launch with the GAUGE FIELD resident in shared memory (csrc/wilson_ures.cuh): every

@@ -504,19 +504,19 @@ static bool resident_plan(const wd_ctx *c, int *nc_out, int *spc_out)
     return false;
 }
 
-// Automatic for clusters of up to four CTAs in fp32 and eight in fp64 (measured, us per iteration, resident / best of the other
-// one-launch kernels: fp32 4^4 5.1 / 8.6, 4^3x8 6.6 / 9.5, 8x4x4x8 and 4x4x8x8 (4 CTAs) 7.5 / 9.4-9.8, 8 CTAs 9.8-10.2 / 9.6-9.9;
-// fp64 4^4 (2 CTAs) 7.6 / 10.5, 4^3x8 (4) 7.7 / 10.5, 1024 sites (8) 9.6 / 10.4-11.2, 2048 sites (16) 11.5 / 10.5).  Larger clusters
-// lose to the cost of the cluster barrier, which grows with the cluster (about 0.5 / 0.8 / 1.6 / 2 us per barrier at 2 / 4 / 8 / 16
-// CTAs, three per iteration); neither the volume nor the latency of the remote reads is what holds them (a variant
-// that pulls owner-projected half-spinors, -64 % distributed-shared-memory bytes, measured the same 11.0 us at 8^4);
-// wd_set_cg_mode(ctx, 9) still selects them.
+// Automatic wherever the lattice fits a cluster (measured, us per iteration, resident / best of the other one-launch kernels:
+// fp32 4^4 5.1 / 8.6, 512 sites (2 CTAs) 6.6 / 9.5, 1024 sites (4) 7.5 / 9.4-9.8, 2048 sites (8, exports) 8.1-8.3 / 9.6-9.9, 8^4 and
+// other 4096-site lattices (16, exports) 8.9-9.0 / 9.7-10.3; fp64 4^4 (2 CTAs) 7.6 / 10.5, 512 sites (4) 7.7 / 10.5, 1024 sites (8)
+// 9.6-9.8 / 10.4-11.2, 2048 sites (16, exports) 10.1-10.2 / 10.5).  From eight CTAs on the remote neighbours are read as
+// half-spinors exported by their owners (wilson_resident_ex.cuh): pulling whole spinors and links through distributed shared
+// memory made the stencil phases of the 16-CTA cluster 4.1 us against 1.9 us without remote neighbours.
 static bool use_resident(const wd_ctx *c)
 {
     int nc, spc;
     if (c->cg_mode != 0 && c->cg_mode != 9) return false;
     if (!resident_plan(c, &nc, &spc)) return false;
-    return c->cg_mode == 9 || nc <= (c->precision == 64 ? 8 : 4);
+    (void)spc;
+    return true;
 }
 
 static bool use_split(const wd_ctx *c)

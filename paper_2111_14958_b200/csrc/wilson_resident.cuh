@@ -334,6 +334,38 @@ cg_resident_kernel(int L0, int L1, int L2, int L3, int bc_t, int spc_shift, cons
     rs_sync<CL>();                                           // no CTA leaves while its shared memory may still be read
 }
 
+}  // namespace wd
+#include "wilson_resident_ex.cuh"
+namespace wd {
+
+// Largest number of half-spinors a CTA has to export: over the sites of a slab, the hops that leave the slab (host, once per
+// geometry: the slabs are ranges of consecutive sites).
+static int resident_export_slots(const int L[4], int spc, int nc)
+{
+    thread_local int key[6] = {0, 0, 0, 0, 0, 0}, val = 0;
+    if (key[0] == L[0] && key[1] == L[1] && key[2] == L[2] && key[3] == L[3] && key[4] == spc && key[5] == nc) return val;
+    int worst = 0;
+    const int stride[4] = {1, L[0], L[0] * L[1], L[0] * L[1] * L[2]};
+    for (int r = 0; r < nc; ++r) {
+        int count = 0;
+        for (int l = 0; l < spc; ++l) {
+            const int s = r * spc + l;
+            int c[4], rem = s;
+            for (int d = 0; d < 4; ++d) { c[d] = rem % L[d]; rem /= L[d]; }
+            for (int d = 0; d < 4; ++d) {
+                const int f = s + (c[d] == L[d] - 1 ? -(L[d] - 1) : 1) * stride[d];
+                const int b = s + (c[d] == 0 ? (L[d] - 1) : -1) * stride[d];
+                count += (f / spc != r) + (b / spc != r);
+            }
+        }
+        if (count > worst) worst = count;
+    }
+    for (int d = 0; d < 4; ++d) key[d] = L[d];
+    key[4] = spc; key[5] = nc; val = worst;
+    return val;
+}
+constexpr size_t WD_RESIDENT_SMEM_MAX = 232448;   // 227 KB opt-in limit per CTA on sm_100
+
 template <typename real>
 static cudaError_t launch_cg_resident_any(const ResidentArgs &a)
 {
@@ -357,6 +389,28 @@ static cudaError_t launch_cg_resident_any(const ResidentArgs &a)
     svec *psi = (svec *)a.psi;
     const real kappa = (real)a.kappa;
     cudaError_t e;
+    // Clusters of eight and sixteen CTAs: remote neighbours as half-spinors exported by their owners (wilson_resident_ex.cuh).
+    // Measured, us per iteration, pulling whole spinors and links / exports: fp32 2048 sites (8 CTAs) 9.6-10.3 / 8.1-8.3, 4096
+    // sites (16) 10.5-11.0 / 8.9-9.0; fp64 1024 sites (8) 9.9 / 9.8, 2048 sites (16) 11.5-12.4 / 10.1-10.2; smaller clusters have
+    // too few remote hops to pay for the exports (4 CTAs 7.2 / 7.3, 2 CTAs 6.8 / 7.4; fp64 2 and 4 CTAs 7.6 / 8.8).
+    {
+        constexpr int min_nc = 8;
+        const int nslots = a.nc >= min_nc ? resident_export_slots(a.L, a.spc, a.nc) : 0;
+        const size_t ex_smem = resident_ex_smem<real>(a.spc, nslots);
+        if (a.nc >= min_nc && nslots < 65536 && ex_smem <= WD_RESIDENT_SMEM_MAX) {
+            auto kern = cg_resident_ex_kernel<real>;
+            e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ex_smem);
+            if (e != cudaSuccess) return e;
+            if (a.nc > 8) {
+                e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+                if (e != cudaSuccess) return e;
+            }
+            lc.dynamicSmemBytes = ex_smem;
+            lc.numAttrs = 1;
+            return cudaLaunchKernelEx(&lc, kern, a.L[0], a.L[1], a.L[2], a.L[3], a.bc_t, shift, nslots, U, eta, psi, kappa, a.sc,
+                                      a.hist, a.r_min, a.max_iter);
+        }
+    }
     if (a.nc > 1) {
         auto kern = cg_resident_kernel<real, true>;
         e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

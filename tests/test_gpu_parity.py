@@ -421,17 +421,18 @@ def test_cg_resident_cluster_sizes(wilson, oracle, dims, bc_t, precision):
 
 
 def test_cg_automatic_mode_by_volume(wilson):
-    """4^4 takes the shared-memory-resident kernel (one CTA in fp32, a cluster of two in fp64), the rest of the paper's range
-     a one-launch cooperative kernel (gauge field in shared memory: mode 10; fp64 8^4: the split kernel), 32^4
-    the three-kernel loop"""
-    for ci, precision, want in ((0, 32, 9), (1, 32, 10), (2, 32, 10), (0, 64, 9), (1, 64, 6)):
+    """4^4 and 8^4 (fp32) take the shared-memory-resident kernel (one CTA, a cluster of sixteen with exported half-spinors; 4^4
+    fp64: a cluster of two), the rest of the paper's range a one-launch cooperative kernel (gauge field in shared
+    memory: mode 10; fp64 8^4, which fits no cluster: the split kernel), 32^4 the three-kernel loop"""
+    for ci, precision, want in ((0, 32, 9), (1, 32, 9), (2, 32, 10), (0, 64, 9), (1, 64, 6)):
         cfg = inputs.CONFIGS[ci]
         U, eta = gu.config_fields(ci, precision)
         with wilson.WilsonContext(cfg.dims, precision, cfg.bc_t) as ctx:
             _, info = gu.solve_on_gpu(ctx, U, eta, cfg.kappa, cfg.r_min, cfg.max_iter)
         assert info["cg_mode"] == want and info["kernel_launches"] == 2
-    # between 4^4 and 8^4: the resident kernel up to a cluster of four CTAs in fp32 (1024 sites) and eight in fp64 (1024 sites)
-    for dims, precision, want in (((8, 4, 4, 8), 32, 9), ((4, 8, 8, 8), 32, 10), ((4, 4, 8, 8), 64, 9), ((4, 8, 8, 8), 64, 6)):
+    # in between: the resident kernel wherever V / nc is a power of two that fits a CTA (fp32 <= 4096 sites, fp64 <= 2048)
+    for dims, precision, want in (((8, 4, 4, 8), 32, 9), ((4, 8, 8, 8), 32, 9), ((4, 4, 8, 8), 64, 9), ((4, 8, 8, 8), 64, 9),
+                                  ((6, 6, 6, 6), 32, 10), ((8, 8, 8, 16), 32, 10)):
         cdt = gu.np_complex(precision)
         U = inputs.gauge_field(CFG_TEST + 7, dims, "haar", dtype=cdt)
         eta = inputs.source_field(CFG_TEST + 7, dims, dtype=cdt)
