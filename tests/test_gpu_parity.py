@@ -590,6 +590,43 @@ def test_cg_edge_cases(wilson, oracle, mode):
         assert info["status"] == 0 and info["iterations"] == 0
 
 
+@pytest.mark.parametrize("dims,precision", [((8, 8, 8, 8), 32), ((4, 8, 8, 8), 64), ((4, 8, 8, 8), 32)])
+def test_cg_edge_cases_on_clusters_with_exported_half_spinors(wilson, oracle, dims, precision):
+    """the degenerate cases on the resident kernel of 8 / 16 CTAs (cg_resident_ex_kernel; automatic for these lattices): the
+    paths that leave the loop at once still have to export y for the final D-dagger and keep every CTA in the barriers"""
+    cdt = gu.np_complex(precision)
+    tol = 1e-6 if precision == 32 else 1e-12
+    U = inputs.gauge_field(CFG_TEST + 11, dims, "haar", dtype=cdt)
+    eta = inputs.source_field(CFG_TEST + 11, dims, dtype=cdt)
+    U64, eta64 = U.astype(np.complex128), eta.astype(np.complex128)
+    for bc_t in (-1, 1):
+        with wilson.WilsonContext(dims, precision, bc_t) as ctx:
+            psi, info = gu.solve_on_gpu(ctx, U, np.zeros_like(eta), 0.12, 1e-8, 100)
+            assert info["cg_mode"] == 9 and info["status"] == 0 and info["iterations"] == 0 and not psi.any()
+            psi, info = gu.solve_on_gpu(ctx, U, eta, 0.12, 1e-8, 0)
+            assert info["status"] == 1 and info["iterations"] == 0 and not psi.any()
+            psi, info = gu.solve_on_gpu(ctx, U, eta, 0.12, 1e-12, 5)
+            psi_o, info_o = oracle.cg_solve(dims, U64, eta64, 0.12, 1e-12, 5, bc_t)
+            assert info["status"] == 1 and info["converged"] == 0 and info["iterations"] == 5 == info_o["iterations"]
+            assert np.linalg.norm(psi - psi_o) / np.linalg.norm(psi_o) < (2e-6 if precision == 32 else 1e-12)
+            psi, info = gu.solve_on_gpu(ctx, U, eta, 0.0, tol, 10)
+            assert info["iterations"] == 1 and np.max(np.abs(psi - eta)) < (1e-6 if precision == 32 else 1e-14)
+            psi, info = gu.solve_on_gpu(ctx, U, eta, 0.12, 1.5, 10)
+            assert info["status"] == 0 and info["iterations"] == 0
+            # a NaN in the source is a breakdown, not a convergence
+            bad = eta.copy()
+            bad[17, 2, 1] = np.nan
+            _, info = gu.solve_on_gpu(ctx, U, bad, 0.12, 1e-6, 50)
+            assert info["status"] == 2 and info["converged"] == 0
+            # the whole solve against the oracle, and repeatable bit for bit
+            psi, info = gu.solve_on_gpu(ctx, U, eta, 0.12, tol if precision == 32 else 1e-10, 500)
+            psi2, info2 = gu.solve_on_gpu(ctx, U, eta, 0.12, tol if precision == 32 else 1e-10, 500)
+            psi_o, info_o = oracle.cg_solve(dims, U64, eta64, 0.12, tol if precision == 32 else 1e-10, 500, bc_t)
+            assert info["status"] == 0 and iters_close(info["iterations"], info_o["iterations"]) and psi.tobytes() == psi2.tobytes()
+            res = oracle.true_residual(dims, U64, eta64, psi.astype(np.complex128), 0.12, bc_t)
+            assert res <= 2.0 * oracle.true_residual(dims, U64, eta64, psi_o, 0.12, bc_t)
+
+
 def test_cg_free_field_finite_termination(wilson):
     """pin P8: K plane waves with distinct |D(p)|^2 terminate after exactly K iterations, exact solution known"""
     dims, kappa = (8, 8, 8, 8), 0.12
