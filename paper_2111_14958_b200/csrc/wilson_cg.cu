@@ -515,8 +515,12 @@ static bool use_resident(const wd_ctx *c)
     int nc, spc;
     if (c->cg_mode != 0 && c->cg_mode != 9) return false;
     if (!resident_plan(c, &nc, &spc)) return false;
-    (void)spc;
-    return true;
+    if (c->cg_mode == 9 || nc <= 4) return true;
+    // eight and sixteen CTAs: only where the exported half-spinors fit the shared memory beside the slabs (otherwise the launcher
+    // falls back to pulling whole spinors and links, which loses to the cooperative kernels: 10.5-11 against 9.7-10.3 us)
+    const int nslots = resident_export_slots(c->dims, spc, nc);
+    const size_t need = c->precision == 64 ? resident_ex_smem<double>(spc, nslots) : resident_ex_smem<float>(spc, nslots);
+    return nslots < 65536 && need <= WD_RESIDENT_SMEM_MAX;
 }
 
 static bool use_split(const wd_ctx *c)

@@ -432,7 +432,8 @@ def test_cg_automatic_mode_by_volume(wilson):
         assert info["cg_mode"] == want and info["kernel_launches"] == 2
     # in between: the resident kernel wherever V / nc is a power of two that fits a CTA (fp32 <= 4096 sites, fp64 <= 2048)
     for dims, precision, want in (((8, 4, 4, 8), 32, 9), ((4, 8, 8, 8), 32, 9), ((4, 4, 8, 8), 64, 9), ((4, 8, 8, 8), 64, 9),
-                                  ((6, 6, 6, 6), 32, 10), ((8, 8, 8, 16), 32, 10)):
+                                  ((6, 6, 6, 6), 32, 10), ((8, 8, 8, 16), 32, 10),
+                                  ((16, 16, 4, 4), 32, 10)):   # 16 CTAs, but 1024 exports per CTA do not fit beside the slabs
         cdt = gu.np_complex(precision)
         U = inputs.gauge_field(CFG_TEST + 7, dims, "haar", dtype=cdt)
         eta = inputs.source_field(CFG_TEST + 7, dims, dtype=cdt)
